@@ -1,0 +1,143 @@
+"""CPU oracle of the 2DGS surfel renderer (fp64, written from PAPER.md).  TEST INFRASTRUCTURE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this package.  It never imports the CUDA path (paper_2506_00970_b200) and shares no code
+with it.  The arithmetic lives in oracle/sgs_oracle.c (plain C, OpenMP over pixel rows); this file
+only marshals numpy arrays through ctypes.
+
+Parity unpinned: absolute image values on the paper's datasets (the paper prints none; the
+datasets are not available).  Everything else is pinned by tests/test_oracle_pins.py (P1-P10).
+"""
+import ctypes
+import os
+import subprocess
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sgs_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+C_F32 = ctypes.POINTER(ctypes.c_float)
+C_F64 = ctypes.POINTER(ctypes.c_double)
+C_U8 = ctypes.POINTER(ctypes.c_uint8)
+C_U32 = ctypes.POINTER(ctypes.c_uint32)
+C_I32 = ctypes.POINTER(ctypes.c_int32)
+C_U64 = ctypes.POINTER(ctypes.c_uint64)
+C_I64 = ctypes.POINTER(ctypes.c_int64)
+
+
+def build(force=False):
+    """gcc -O2 -fopenmp -ffp-contract=off (no FMA contraction: the binning stage is a bit-exact
+    contract).  Building the checker is not using it."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        _lib.orc_preprocess.restype = ctypes.c_int64
+        _lib.orc_num_threads.restype = ctypes.c_int
+    return _lib
+
+
+def _p(a, t):
+    return None if a is None else a.ctypes.data_as(t)
+
+
+def make_cfg(tile=16, cutoff=3.0, alpha_min=1.0 / 255.0, alpha_max=0.99, t_min=1e-4, z_near=0.2):
+    """Truncation constants (readings R3-R7).  Values pass through float32 first because the C-ABI
+    config struct holds floats: both sides then use the identical real numbers."""
+    f = lambda v: float(np.float32(v))
+    return np.array([tile, f(cutoff), f(alpha_min), f(alpha_max), f(t_min), f(z_near)], dtype=np.float64)
+
+
+def smooth_cfg(tile=16):
+    """Plain Eq. 8: no cutoff, no alpha bounds, no stop, no near plane (used for finite differences)."""
+    return np.array([tile, np.inf, 0.0, 1.0, 0.0, 0.0], dtype=np.float64)
+
+
+def make_cam(cam, T_cw=None, widen_from_f32=True):
+    """Camera vector [W,H,fx,fy,cx,cy,T_cw(12)].  By default intrinsics and pose are rounded to
+    float32 first (what the C-ABI carries); pass widen_from_f32=False for fp64 finite differences."""
+    T = np.asarray(cam.T_cw if T_cw is None else T_cw, dtype=np.float64)[:3].reshape(12)
+    k = np.array([cam.fx, cam.fy, cam.cx, cam.cy], dtype=np.float64)
+    if widen_from_f32:
+        T = T.astype(np.float32).astype(np.float64)
+        k = k.astype(np.float32).astype(np.float64)
+    return np.concatenate([[cam.width, cam.height], k, T]).astype(np.float64)
+
+
+def _scene_arrays(sc):
+    f = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    act = None if sc.active is None else np.ascontiguousarray(sc.active, dtype=np.uint8)
+    return f(sc.mean), f(sc.scale), f(sc.quat), f(sc.opacity), f(sc.rgb), act
+
+
+def preprocess(sc, camv, cfgv):
+    mean, scale, quat, _, _, act = _scene_arrays(sc)
+    n = mean.shape[0]
+    out = dict(culled=np.zeros(n, np.uint8), depth_bits=np.zeros(n, np.uint32), rect=np.zeros((n, 4), np.int32),
+               count=np.zeros(n, np.uint32), M=np.zeros((n, 9)), aabb=np.zeros((n, 4)))
+    E = lib().orc_preprocess(ctypes.c_int64(n), _p(mean, C_F32), _p(scale, C_F32), _p(quat, C_F32), _p(act, C_U8),
+                             _p(camv, C_F64), _p(cfgv, C_F64), _p(out["culled"], C_U8), _p(out["depth_bits"], C_U32),
+                             _p(out["rect"], C_I32), _p(out["count"], C_U32), _p(out["M"], C_F64), _p(out["aabb"], C_F64))
+    out["E"] = int(E)
+    return out
+
+
+def binning(sc, camv, cfgv):
+    """Stage O2: culled flags, sorted (key, idx) list and per-tile ranges -- the bit-exact contract."""
+    pre = preprocess(sc, camv, cfgv)
+    W, H, tile = int(camv[0]), int(camv[1]), int(cfgv[0])
+    tx, ty = (W + tile - 1) // tile, (H + tile - 1) // tile
+    E = pre["E"]
+    keys = np.zeros(max(E, 1), np.uint64)
+    idx = np.zeros(max(E, 1), np.uint32)
+    ranges = np.zeros((tx * ty, 2), np.uint32)
+    lib().orc_bin(ctypes.c_int64(sc.n), _p(pre["culled"], C_U8), _p(pre["depth_bits"], C_U32), _p(pre["rect"], C_I32),
+                  ctypes.c_int(tx), ctypes.c_int(ty), ctypes.c_int64(E), _p(keys, C_U64), _p(idx, C_U32), _p(ranges, C_U32))
+    pre.update(keys=keys[:E], idx=idx[:E], ranges=ranges, tiles_x=tx, tiles_y=ty)
+    return pre
+
+
+def render(sc, camv, cfgv, brute=False, counters=True):
+    """Forward (O3-O4).  Returns dict: img (8,H,W) f64 [rgb, depth, normal, alpha], T_final, n_comp,
+    fragile (bit0: image-affecting decision within 1e-4; bit1: alpha_max clamp within 1e-4), counters."""
+    mean, scale, quat, opac, rgb, act = _scene_arrays(sc)
+    W, H = int(camv[0]), int(camv[1])
+    img = np.zeros((8, H, W)); T = np.zeros((H, W)); nc = np.zeros((H, W), np.int32)
+    frag = np.zeros((H, W), np.uint8); cnt = np.zeros(5, np.int64)
+    lib().orc_render(ctypes.c_int64(sc.n), _p(mean, C_F32), _p(scale, C_F32), _p(quat, C_F32), _p(opac, C_F32),
+                     _p(rgb, C_F32), _p(act, C_U8), _p(camv, C_F64), _p(cfgv, C_F64), ctypes.c_int(int(brute)),
+                     _p(img, C_F64), _p(T, C_F64), _p(nc, C_I32), _p(frag, C_U8), _p(cnt if counters else None, C_I64))
+    return dict(img=img, T_final=T, n_comp=nc, fragile=frag,
+                counters=dict(Q_t=int(cnt[0]), Q_c=int(cnt[1]), cover=int(cnt[2]), n_vis=int(cnt[3]), n_fragile=int(cnt[4])))
+
+
+def backward(sc, camv, cfgv, upstream, brute=False, debug=False):
+    """Analytic backward (O5-O7).  upstream: (8,H,W).  Returns fp64 grads for mean, scale, quat,
+    opacity, rgb, and pose (6,) = (rho, theta) under T <- Exp(tau) o T_cw (Eq. 11-13)."""
+    mean, scale, quat, opac, rgb, act = _scene_arrays(sc)
+    n = sc.n
+    up = np.ascontiguousarray(upstream, dtype=np.float64)
+    g = dict(mean=np.zeros((n, 3)), scale=np.zeros((n, 2)), quat=np.zeros((n, 4)), opacity=np.zeros(n),
+             rgb=np.zeros((n, 3)), pose=np.zeros(6), surfel_fragile=np.zeros(n, np.uint8))
+    dM = np.zeros((n, 9)) if debug else None
+    dnc = np.zeros((n, 3)) if debug else None
+    lib().orc_backward(ctypes.c_int64(n), _p(mean, C_F32), _p(scale, C_F32), _p(quat, C_F32), _p(opac, C_F32),
+                       _p(rgb, C_F32), _p(act, C_U8), _p(camv, C_F64), _p(cfgv, C_F64), ctypes.c_int(int(brute)),
+                       _p(up, C_F64), _p(g["mean"], C_F64), _p(g["scale"], C_F64), _p(g["quat"], C_F64),
+                       _p(g["opacity"], C_F64), _p(g["rgb"], C_F64), _p(g["pose"], C_F64), _p(dM, C_F64), _p(dnc, C_F64),
+                       _p(g["surfel_fragile"], C_U8))
+    if debug:
+        g["dM"] = dM; g["dnc"] = dnc
+    return g
+
+
+def num_threads():
+    return int(lib().orc_num_threads())

@@ -1,0 +1,578 @@
+/*
+ * sgs_oracle.c -- CPU ORACLE for the 2D-Gaussian (surfel) splatting renderer of 2DGS-SLAM
+ * (arxiv 2506.00970).  TEST INFRASTRUCTURE ONLY: nothing but tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may build, load or call this file.
+ * It shares no code with the CUDA path under paper_2506_00970_b200/.
+ *
+ * Plain, slow, fp64, one pixel at a time over all surfels in depth order, in the paper's
+ * notation (citations are PAPER.md line numbers; "R<n>" are the readings listed in DESIGN.md §3):
+ *   Eq. 1-2  (L83-93)   surfel frame  P(u,v) = mu + s_u t_u u + s_v t_v v
+ *   Eq. 3-7  (L95-110)  homography    M = K [s_u t_uc, s_v t_vc, mu_c]   (3x3 reduction of  W T_cw H, R14)
+ *   L112                ray-splat intersection (u,v,1) ~ (M0 - x M2) x (M1 - y M2)           (R1)
+ *   Eq. 8    (L114-120) depth-ordered alpha blending of colour, depth, normal, opacity
+ *   Eq. 9-13 (L130-152) gradient to H_c, R_c and the SE(3) pose (left perturbation)
+ *
+ * Pins (tests/test_oracle_pins.py): P1 closed-form footprint, P2 ray-plane depth, P3 hand-computed
+ * stacks, P4 invariants, P5 channel consistency, P6 truncation limit, P7 binning conservativeness,
+ * P8 central finite differences of every gradient incl. pose, P9 rigid-motion identity, P10
+ * symmetries.  Parity UNPINNED: absolute image values on the paper's datasets (not available).
+ *
+ * Build: gcc -O2 -fopenmp -ffp-contract=off -fPIC -shared (see oracle/build.py).
+ * -ffp-contract=off matters: the binning stage (orc_preprocess) is the bit-exact contract with
+ * the GPU and must evaluate the documented IEEE-754 binary64 operation sequence without FMA.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct {
+    int W, H;
+    double fx, fy, cx, cy;
+    double R[9], t[3]; /* T_cw = [R | t], row-major */
+} Cam;
+
+typedef struct {
+    int tile;
+    double cutoff, alpha_min, alpha_max, t_min, z_near;
+} Cfg;
+
+/* Per-surfel derived quantities (all fp64). */
+typedef struct {
+    int culled;          /* 1 = inactive, behind / across the camera plane, off-screen or non-finite */
+    uint32_t depth_bits; /* bit pattern of (float)mu_c.z */
+    int rect[4];         /* tile rect tx0, ty0, tx1, ty1 (inclusive) */
+    double aabb[4];      /* xmin, xmax, ymin, ymax of the cutoff ellipse on screen (pixels) */
+    double qn;           /* |q| */
+    double qh[4];        /* q / |q| */
+    double Rw[9];        /* R(qh), columns t_u, t_v, t_n (world) */
+    double tuc[3], tvc[3], tnc[3], muc[3];
+    double M[9];         /* rows M0, M1, M2 of K [s_u t_uc, s_v t_vc, mu_c] */
+} Prep;
+
+static void load_cam(const double* c, Cam* cam) {
+    cam->W = (int)c[0]; cam->H = (int)c[1];
+    cam->fx = c[2]; cam->fy = c[3]; cam->cx = c[4]; cam->cy = c[5];
+    for (int i = 0; i < 3; ++i) {
+        for (int j = 0; j < 3; ++j) cam->R[3 * i + j] = c[6 + 4 * i + j];
+        cam->t[i] = c[6 + 4 * i + 3];
+    }
+}
+static void load_cfg(const double* c, Cfg* cfg) {
+    cfg->tile = (int)c[0]; cfg->cutoff = c[1]; cfg->alpha_min = c[2];
+    cfg->alpha_max = c[3]; cfg->t_min = c[4]; cfg->z_near = c[5];
+}
+
+static uint32_t f32_bits(float f) { uint32_t u; memcpy(&u, &f, 4); return u; }
+
+/*
+ * O2: the binning reference.  STRICT operation order -- the GPU preprocess kernel
+ * evaluates exactly this binary64 sequence (no FMA, IEEE sqrt and division, no transcendental).
+ *   q_hat = q / sqrt(((w*w + x*x) + y*y) + z*z)
+ *   R(q_hat) by the unit-quaternion formula, (w,x,y,z) order
+ *   t_uc = R_cw t_u, t_vc = R_cw t_v, t_nc = R_cw t_n, mu_c = R_cw mu + t_cw      (Eq. 5-6)
+ *   M = K [s_u t_uc, s_v t_vc, mu_c]                                               (Eq. 7)
+ *   cull iff inactive, mu_c.z <= z_near, den = c^2 (M20^2 + M21^2) - M22^2 >= 0,
+ *            non-finite, or the AABB misses [0,W] x [0,H]
+ *   AABB of u^2+v^2 = c^2 under the homography (closed form from Eq. 4):
+ *     ctr_x = (c^2 (M00 M20 + M01 M21) - M02 M22) / den
+ *     half_x = sqrt(ctr_x^2 - (c^2 (M00^2 + M01^2) - M02^2) / den),  same for y with M1
+ *   tile rect = floor(min/tile) .. floor(max/tile), clamped to the tile grid
+ */
+static inline double dot3r(const double* r, const double* v) { return (r[0] * v[0] + r[1] * v[1]) + r[2] * v[2]; }
+
+static void prep_surfel(const float* mean, const float* scale, const float* quat, int is_active,
+                        const Cam* cam, const Cfg* cfg, Prep* p) {
+    memset(p, 0, sizeof(*p));
+    p->culled = 1;
+    if (!is_active) return;
+    const double w = quat[0], x = quat[1], y = quat[2], z = quat[3];
+    const double qn = sqrt(((w * w + x * x) + y * y) + z * z);
+    p->qn = qn;
+    if (!(qn > 0.0) || !isfinite(qn)) return;
+    const double qw = w / qn, qx = x / qn, qy = y / qn, qz = z / qn;
+    p->qh[0] = qw; p->qh[1] = qx; p->qh[2] = qy; p->qh[3] = qz;
+    double* R = p->Rw;
+    R[0] = 1.0 - 2.0 * (qy * qy + qz * qz); R[1] = 2.0 * (qx * qy - qw * qz); R[2] = 2.0 * (qx * qz + qw * qy);
+    R[3] = 2.0 * (qx * qy + qw * qz); R[4] = 1.0 - 2.0 * (qx * qx + qz * qz); R[5] = 2.0 * (qy * qz - qw * qx);
+    R[6] = 2.0 * (qx * qz - qw * qy); R[7] = 2.0 * (qy * qz + qw * qx); R[8] = 1.0 - 2.0 * (qx * qx + qy * qy);
+    const double tu[3] = {R[0], R[3], R[6]}, tv[3] = {R[1], R[4], R[7]}, tn[3] = {R[2], R[5], R[8]};
+    const double mu[3] = {mean[0], mean[1], mean[2]};
+    for (int i = 0; i < 3; ++i) {
+        p->tuc[i] = dot3r(cam->R + 3 * i, tu);
+        p->tvc[i] = dot3r(cam->R + 3 * i, tv);
+        p->tnc[i] = dot3r(cam->R + 3 * i, tn);
+        p->muc[i] = dot3r(cam->R + 3 * i, mu) + cam->t[i];
+    }
+    const double su = scale[0], sv = scale[1];
+    const double A0[3] = {su * p->tuc[0], sv * p->tvc[0], p->muc[0]};
+    const double A1[3] = {su * p->tuc[1], sv * p->tvc[1], p->muc[1]};
+    const double A2[3] = {su * p->tuc[2], sv * p->tvc[2], p->muc[2]};
+    double* M = p->M;
+    for (int j = 0; j < 3; ++j) {
+        M[j] = cam->fx * A0[j] + cam->cx * A2[j];
+        M[3 + j] = cam->fy * A1[j] + cam->cy * A2[j];
+        M[6 + j] = A2[j];
+    }
+    p->depth_bits = f32_bits((float)p->muc[2]);
+    if (!(p->muc[2] > cfg->z_near)) return;
+    const int tiles_x = (cam->W + cfg->tile - 1) / cfg->tile, tiles_y = (cam->H + cfg->tile - 1) / cfg->tile;
+    if (isinf(cfg->cutoff)) { /* oracle-only smooth mode (plain Eq. 8, used for finite differences): no footprint */
+        p->aabb[0] = p->aabb[2] = -INFINITY; p->aabb[1] = p->aabb[3] = INFINITY;
+        p->rect[0] = 0; p->rect[1] = 0; p->rect[2] = tiles_x - 1; p->rect[3] = tiles_y - 1;
+        p->culled = 0;
+        return;
+    }
+    const double c2 = cfg->cutoff * cfg->cutoff;
+    const double den = c2 * (M[6] * M[6] + M[7] * M[7]) - M[8] * M[8];
+    if (!(den < 0.0)) return;
+    const double ctrx = (c2 * (M[0] * M[6] + M[1] * M[7]) - M[2] * M[8]) / den;
+    const double ctry = (c2 * (M[3] * M[6] + M[4] * M[7]) - M[5] * M[8]) / den;
+    const double hx = sqrt(ctrx * ctrx - (c2 * (M[0] * M[0] + M[1] * M[1]) - M[2] * M[2]) / den);
+    const double hy = sqrt(ctry * ctry - (c2 * (M[3] * M[3] + M[4] * M[4]) - M[5] * M[5]) / den);
+    const double xmin = ctrx - hx, xmax = ctrx + hx, ymin = ctry - hy, ymax = ctry + hy;
+    p->aabb[0] = xmin; p->aabb[1] = xmax; p->aabb[2] = ymin; p->aabb[3] = ymax;
+    if (!(isfinite(xmin) && isfinite(xmax) && isfinite(ymin) && isfinite(ymax))) return;
+    if (!(xmax > 0.0 && xmin < (double)cam->W && ymax > 0.0 && ymin < (double)cam->H)) return;
+    const double ts = (double)cfg->tile;
+    /* floor and clamp in double (exact: tile is a power of two or small integer), then cast */
+    double fx0 = floor(xmin / ts), fx1 = floor(xmax / ts), fy0 = floor(ymin / ts), fy1 = floor(ymax / ts);
+    if (fx0 < 0.0) fx0 = 0.0;
+    if (fy0 < 0.0) fy0 = 0.0;
+    if (fx1 > (double)(tiles_x - 1)) fx1 = (double)(tiles_x - 1);
+    if (fy1 > (double)(tiles_y - 1)) fy1 = (double)(tiles_y - 1);
+    const int tx0 = (int)fx0, tx1 = (int)fx1, ty0 = (int)fy0, ty1 = (int)fy1;
+    p->rect[0] = tx0; p->rect[1] = ty0; p->rect[2] = tx1; p->rect[3] = ty1;
+    p->culled = 0;
+}
+
+static Prep* prep_all(int64_t n, const float* mean, const float* scale, const float* quat,
+                      const uint8_t* active, const Cam* cam, const Cfg* cfg) {
+    Prep* P = (Prep*)malloc(sizeof(Prep) * (size_t)(n > 0 ? n : 1));
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i)
+        prep_surfel(mean + 3 * i, scale + 2 * i, quat + 4 * i, active ? active[i] != 0 : 1, cam, cfg, P + i);
+    return P;
+}
+
+/* ---- public: stage O2, per-surfel part.  Returns E = sum of tile counts. ---- */
+int64_t orc_preprocess(int64_t n, const float* mean, const float* scale, const float* quat,
+                       const uint8_t* active, const double* camv, const double* cfgv,
+                       uint8_t* culled, uint32_t* depth_bits, int32_t* rect, uint32_t* count,
+                       double* M_out, double* aabb_out) {
+    Cam cam; Cfg cfg; load_cam(camv, &cam); load_cfg(cfgv, &cfg);
+    Prep* P = prep_all(n, mean, scale, quat, active, &cam, &cfg);
+    int64_t E = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        const Prep* p = P + i;
+        culled[i] = (uint8_t)p->culled;
+        depth_bits[i] = p->culled ? 0u : p->depth_bits;
+        uint32_t c = 0;
+        for (int j = 0; j < 4; ++j) rect[4 * i + j] = p->culled ? 0 : p->rect[j];
+        if (!p->culled) c = (uint32_t)((p->rect[2] - p->rect[0] + 1) * (p->rect[3] - p->rect[1] + 1));
+        count[i] = c;
+        E += c;
+        if (M_out) memcpy(M_out + 9 * i, p->M, sizeof(double) * 9);
+        if (aabb_out) memcpy(aabb_out + 4 * i, p->aabb, sizeof(double) * 4);
+    }
+    free(P);
+    return E;
+}
+
+typedef struct { uint64_t key; uint32_t idx; } Entry;
+static int cmp_entry(const void* a, const void* b) {
+    const Entry* x = (const Entry*)a; const Entry* y = (const Entry*)b;
+    if (x->key != y->key) return x->key < y->key ? -1 : 1;
+    if (x->idx != y->idx) return x->idx < y->idx ? -1 : 1; /* stable sort of a surfel-major emission */
+    return 0;
+}
+
+/* ---- public: stage O2, list part.  key = tile_id << 32 | depth bits (R2); entries emitted
+ * surfel-major, tiles row-major; stable sort => ties ordered by surfel index; ranges[t] = [start,end). */
+void orc_bin(int64_t n, const uint8_t* culled, const uint32_t* depth_bits, const int32_t* rect,
+             int tiles_x, int tiles_y, int64_t E, uint64_t* keys, uint32_t* idx, uint32_t* ranges) {
+    Entry* e = (Entry*)malloc(sizeof(Entry) * (size_t)(E > 0 ? E : 1));
+    int64_t m = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        if (culled[i]) continue;
+        for (int ty = rect[4 * i + 1]; ty <= rect[4 * i + 3]; ++ty)
+            for (int tx = rect[4 * i + 0]; tx <= rect[4 * i + 2]; ++tx) {
+                e[m].key = ((uint64_t)(uint32_t)(ty * tiles_x + tx) << 32) | depth_bits[i];
+                e[m].idx = (uint32_t)i;
+                ++m;
+            }
+    }
+    qsort(e, (size_t)m, sizeof(Entry), cmp_entry);
+    const int tiles = tiles_x * tiles_y;
+    for (int t = 0; t < tiles; ++t) { ranges[2 * t] = 0; ranges[2 * t + 1] = 0; }
+    for (int64_t i = 0; i < m; ++i) {
+        keys[i] = e[i].key; idx[i] = e[i].idx;
+        const uint32_t t = (uint32_t)(e[i].key >> 32);
+        if (i == 0 || (uint32_t)(e[i - 1].key >> 32) != t) ranges[2 * t] = (uint32_t)i;
+        if (i == m - 1 || (uint32_t)(e[i + 1].key >> 32) != t) ranges[2 * t + 1] = (uint32_t)(i + 1);
+    }
+    free(e);
+}
+
+/* ---- global compositing order (R2): depth bits of the centre, ties by surfel index ---- */
+typedef struct { uint32_t d; uint32_t i; } OrdKey;
+static int cmp_ord(const void* a, const void* b) {
+    const OrdKey* x = (const OrdKey*)a; const OrdKey* y = (const OrdKey*)b;
+    if (x->d != y->d) return x->d < y->d ? -1 : 1;
+    return x->i < y->i ? -1 : (x->i > y->i ? 1 : 0);
+}
+static uint32_t* global_order(int64_t n, const Prep* P, int64_t* n_vis) {
+    OrdKey* k = (OrdKey*)malloc(sizeof(OrdKey) * (size_t)(n > 0 ? n : 1));
+    int64_t m = 0;
+    for (int64_t i = 0; i < n; ++i)
+        if (!P[i].culled) { k[m].d = P[i].depth_bits; k[m].i = (uint32_t)i; ++m; }
+    qsort(k, (size_t)m, sizeof(OrdKey), cmp_ord);
+    uint32_t* ord = (uint32_t*)malloc(sizeof(uint32_t) * (size_t)(m > 0 ? m : 1));
+    for (int64_t i = 0; i < m; ++i) ord[i] = k[i].i;
+    free(k);
+    *n_vis = m;
+    return ord;
+}
+
+/*
+ * Candidate lists for the "skipping" mode (O4): bucket b (B x B pixels) lists, in global order,
+ * every surfel whose fp64 AABB PADDED BY 1 PIXEL touches the bucket.  A pixel outside the padded
+ * AABB has rho^2 > c^2 by a margin no rounding can close, so skipping it cannot change the result.
+ * Bit 31 of an entry marks "also inside the UNPADDED tile rect of stage O2" (used only to count
+ * Q_t, the pairs a tile-list traversal tests).  B equals the tile size so the flag is meaningful.
+ */
+typedef struct { int bx, by, B; int64_t* start; uint32_t* list; } Buckets;
+static void build_buckets(const Prep* P, const uint32_t* ord, int64_t n_vis, const Cam* cam, int B, Buckets* bk) {
+    bk->B = B; bk->bx = (cam->W + B - 1) / B; bk->by = (cam->H + B - 1) / B;
+    const int nb = bk->bx * bk->by;
+    bk->start = (int64_t*)calloc((size_t)nb + 1, sizeof(int64_t));
+    for (int pass = 0; pass < 2; ++pass) {
+        int64_t* fill = NULL;
+        if (pass == 1) {
+            int64_t acc = 0;
+            for (int b = 0; b < nb; ++b) { int64_t c = bk->start[b]; bk->start[b] = acc; acc += c; }
+            bk->start[nb] = acc;
+            bk->list = (uint32_t*)malloc(sizeof(uint32_t) * (size_t)(acc > 0 ? acc : 1));
+            fill = (int64_t*)malloc(sizeof(int64_t) * (size_t)nb);
+            memcpy(fill, bk->start, sizeof(int64_t) * (size_t)nb);
+        }
+        for (int64_t j = 0; j < n_vis; ++j) {
+            const Prep* p = P + ord[j];
+            double x0 = floor((p->aabb[0] - 1.0) / B), x1 = floor((p->aabb[1] + 1.0) / B);
+            double y0 = floor((p->aabb[2] - 1.0) / B), y1 = floor((p->aabb[3] + 1.0) / B);
+            if (x0 < 0) x0 = 0;
+            if (y0 < 0) y0 = 0;
+            if (x1 > bk->bx - 1) x1 = bk->bx - 1;
+            if (y1 > bk->by - 1) y1 = bk->by - 1;
+            for (int by = (int)y0; by <= (int)y1; ++by)
+                for (int bx = (int)x0; bx <= (int)x1; ++bx) {
+                    const int b = by * bk->bx + bx;
+                    if (pass == 0) { bk->start[b]++; continue; }
+                    const int inside = bx >= p->rect[0] && bx <= p->rect[2] && by >= p->rect[1] && by <= p->rect[3];
+                    bk->list[fill[b]++] = (uint32_t)j | (inside ? 0x80000000u : 0u); /* j = rank in ord */
+                }
+        }
+        if (fill) free(fill);
+    }
+}
+static void free_buckets(Buckets* bk) { free(bk->start); free(bk->list); }
+
+/* ---------------------------------------------------------------------------------------------
+ * O3 + O4: one (pixel, surfel) pair.  Ray-splat intersection derived from Eq. 4 (R1):
+ *   h_u = M0 - x M2,  h_v = M1 - y M2,  k = h_u x h_v,  (u,v) = k_xy / k_z,  z = M2 . (u,v,1)
+ * then Eq. 8 with the truncation conventions R3-R7:
+ *   skip if k_z == 0 or non-finite; skip if rho^2 > c^2; skip if z <= z_near;
+ *   G = exp(-rho^2/2); a = min(alpha_max, o G); skip if a < alpha_min;
+ *   T' = T (1 - a); if T' < t_min: STOP the pixel, this surfel is not composited.
+ * Returns 0 = skipped, 1 = composited, 2 = stop.  *frag is OR-ed with 1 when any decision taken
+ * had relative margin < 1e-4.
+ * ------------------------------------------------------------------------------------------- */
+typedef struct {
+    double hu[3], hv[3], k[3], u, v, z, G, a;
+    int clamped;
+} Pair;
+
+#define FRAG_EPS 1e-4
+static inline int eval_pair(const Prep* p, double opac, double x, double y, double T, const Cfg* cfg,
+                            Pair* r, int* frag, int* covers) {
+    const double* M = p->M;
+    for (int j = 0; j < 3; ++j) { r->hu[j] = M[j] - x * M[6 + j]; r->hv[j] = M[3 + j] - y * M[6 + j]; }
+    r->k[0] = r->hu[1] * r->hv[2] - r->hu[2] * r->hv[1];
+    r->k[1] = r->hu[2] * r->hv[0] - r->hu[0] * r->hv[2];
+    r->k[2] = r->hu[0] * r->hv[1] - r->hu[1] * r->hv[0];
+    *covers = 0;
+    if (r->k[2] == 0.0) return 0;
+    r->u = r->k[0] / r->k[2];
+    r->v = r->k[1] / r->k[2];
+    const double rho2 = r->u * r->u + r->v * r->v;
+    if (!isfinite(rho2)) return 0;
+    const double c2 = cfg->cutoff * cfg->cutoff;
+    if (isfinite(c2) && fabs(rho2 - c2) < FRAG_EPS * c2) *frag |= 1;
+    if (rho2 > c2) return 0;
+    r->z = M[6] * r->u + M[7] * r->v + M[8];
+    if (cfg->z_near > 0.0 && fabs(r->z - cfg->z_near) < FRAG_EPS * cfg->z_near) *frag |= 1;
+    if (!(r->z > cfg->z_near)) return 0;
+    *covers = 1;
+    r->G = exp(-0.5 * rho2);
+    const double og = opac * r->G;
+    if (fabs(og - cfg->alpha_max) < FRAG_EPS * cfg->alpha_max) *frag |= 2; /* matters to gradients only */
+    r->clamped = og > cfg->alpha_max;
+    r->a = r->clamped ? cfg->alpha_max : og;
+    if (cfg->alpha_min > 0.0 && fabs(r->a - cfg->alpha_min) < FRAG_EPS * cfg->alpha_min) *frag |= 1;
+    if (r->a < cfg->alpha_min) return 0;
+    const double Tn = T * (1.0 - r->a);
+    if (cfg->t_min > 0.0 && fabs(Tn - cfg->t_min) < FRAG_EPS * cfg->t_min) *frag |= 1;
+    if (Tn < cfg->t_min) return 2;
+    return 1;
+}
+
+typedef struct {
+    int64_t n;
+    const float *opacity, *rgb;
+    Cam cam; Cfg cfg;
+    Prep* P;
+    uint32_t* ord; int64_t n_vis;
+    Buckets bk; int brute;
+} Ctx;
+
+static void ctx_init(Ctx* c, int64_t n, const float* mean, const float* scale, const float* quat,
+                     const float* opacity, const float* rgb, const uint8_t* active,
+                     const double* camv, const double* cfgv, int brute) {
+    load_cam(camv, &c->cam); load_cfg(cfgv, &c->cfg);
+    c->n = n; c->opacity = opacity; c->rgb = rgb; c->brute = brute;
+    c->P = prep_all(n, mean, scale, quat, active, &c->cam, &c->cfg);
+    c->ord = global_order(n, c->P, &c->n_vis);
+    build_buckets(c->P, c->ord, c->n_vis, &c->cam, c->cfg.tile, &c->bk);
+}
+static void ctx_free(Ctx* c) { free(c->P); free(c->ord); free_buckets(&c->bk); }
+
+/* candidate iteration for pixel (i,j): brute = every visible surfel in global order;
+ * skipping = the pixel's bucket list, further filtered by the padded AABB. */
+static inline int64_t cand_count(const Ctx* c, int i, int j, const uint32_t** lst) {
+    if (c->brute) { *lst = NULL; return c->n_vis; }
+    const int b = (j / c->bk.B) * c->bk.bx + (i / c->bk.B);
+    *lst = c->bk.list + c->bk.start[b];
+    return c->bk.start[b + 1] - c->bk.start[b];
+}
+
+/* ---- public: forward (O4).  img = 8 planes H*W: r,g,b, depth, nx,ny,nz, alpha (un-normalised
+ * blends, R9/R10; background 0, R17).  counters: [0]=Q_t tile-list pairs tested up to and incl.
+ * the stopping entry, [1]=Q_c composited pairs, [2]=covering pairs (rho^2<=c^2, z>z_near) over
+ * ALL surfels ignoring termination (depth complexity), [3]=n_vis, [4]=fragile pixels. */
+void orc_render(int64_t n, const float* mean, const float* scale, const float* quat,
+                const float* opacity, const float* rgb, const uint8_t* active,
+                const double* camv, const double* cfgv, int brute,
+                double* img, double* T_final, int32_t* n_comp, uint8_t* fragile, int64_t* counters) {
+    Ctx c; ctx_init(&c, n, mean, scale, quat, opacity, rgb, active, camv, cfgv, brute);
+    const int W = c.cam.W, H = c.cam.H; const int64_t HW = (int64_t)W * H;
+    int64_t Qt = 0, Qc = 0, Qcover = 0, nfrag = 0;
+    const int count_all = counters != NULL; /* the covering count needs the traversal past termination */
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : Qt, Qc, Qcover, nfrag)
+    for (int j = 0; j < H; ++j) {
+        for (int i = 0; i < W; ++i) {
+            const double x = i + 0.5, y = j + 0.5; /* pixel centres at half integers (R17) */
+            const uint32_t* lst; const int64_t m = cand_count(&c, i, j, &lst);
+            double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, T = 1.0;
+            int frag = 0, stopped = 0, nc = 0;
+            for (int64_t e = 0; e < m; ++e) {
+                const uint32_t raw = lst ? lst[e] : (uint32_t)e;
+                const uint32_t k = c.ord[raw & 0x7fffffffu];
+                const Prep* p = c.P + k;
+                if (lst) {
+                    if (x < p->aabb[0] - 1.0 || x > p->aabb[1] + 1.0 || y < p->aabb[2] - 1.0 || y > p->aabb[3] + 1.0) {
+                        if ((raw >> 31) && !stopped) ++Qt;
+                        continue;
+                    }
+                }
+                Pair r; int covers, f = 0;
+                const int st = eval_pair(p, opacity[k], x, y, T, &c.cfg, &r, &f, &covers);
+                Qcover += covers;
+                if (stopped) continue; /* past termination: only the covering count continues */
+                if (!lst || (raw >> 31)) ++Qt;
+                frag |= f;
+                if (st == 2) { stopped = 1; if (!count_all) break; continue; }
+                if (st == 0) continue;
+                const double w = r.a * T;
+                acc[0] += w * rgb[3 * k]; acc[1] += w * rgb[3 * k + 1]; acc[2] += w * rgb[3 * k + 2];
+                acc[3] += w * r.z;
+                acc[4] += w * p->tnc[0]; acc[5] += w * p->tnc[1]; acc[6] += w * p->tnc[2];
+                acc[7] += w;
+                T *= (1.0 - r.a);
+                ++nc; ++Qc;
+            }
+            const int64_t pix = (int64_t)j * W + i;
+            for (int ch = 0; ch < 8; ++ch) img[ch * HW + pix] = acc[ch];
+            if (T_final) T_final[pix] = T;
+            if (n_comp) n_comp[pix] = nc;
+            if (fragile) fragile[pix] = (uint8_t)frag;
+            nfrag += (frag & 1);
+        }
+    }
+    if (counters) { counters[0] = Qt; counters[1] = Qc; counters[2] = Qcover; counters[3] = c.n_vis; counters[4] = nfrag; }
+    ctx_free(&c);
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O5-O7: analytic backward.
+ * Per pixel, over its composited list i = 0..m-1 (front to back) with w_i = a_i T_i and
+ * v_i = (rgb_k, z_i, t_nc_k, 1) (Eq. 8 and L118-120), g = upstream gradient of the 8 planes:
+ *   dL/dv_i   = g w_i                          -> rgb_k, t_nc_k, z_i
+ *   dL/da_i   = T_i (g.v_i) - (sum_{j>i} w_j (g.v_j)) / (1 - a_i)
+ *   a = min(alpha_max, o G): zero derivative when clamped (R5), else da/do = G, da/dG = o
+ *   dG/du = -u G, dG/dv = -v G;  z = M20 u + M21 v + M22
+ *   dL/dk = (dL/du, dL/dv, -(u dL/du + v dL/dv)) / k_z
+ *   dL/dh_u = h_v x dL/dk,  dL/dh_v = dL/dk x h_u
+ *   dL/dM0 += dL/dh_u, dL/dM1 += dL/dh_v, dL/dM2 -= x dL/dh_u + y dL/dh_v      (this is dL/dT of L130)
+ * Per surfel (O6, Eq. 9-10 with R11, R13, R14):
+ *   G = K^T dL/dM = [dL/d(s_u t_uc), dL/d(s_v t_vc), dL/dmu_c]
+ *   dL/dt_uc = s_u G[:,0], dL/ds_u = t_uc . G[:,0] (same for v); dL/dt_nc from the normal planes
+ *   world: dL/dmu = R_cw^T dL/dmu_c, dL/dR = R_cw^T [dL/dt_uc, dL/dt_vc, dL/dt_nc];
+ *   then the Jacobian of R(q/|q|).
+ * Pose (O7, Eq. 11-13, left perturbation Exp(tau) o T_cw, tau = (rho, theta), R12, R15):
+ *   dL/drho = sum_k dL/dmu_c;  dL/dtheta = sum_k [mu_c x dL/dmu_c + sum_i R_c[:,i] x dL/dR_c[:,i]]
+ * ------------------------------------------------------------------------------------------- */
+typedef struct { uint32_t k; Pair r; double T; } Hit;
+
+static inline void atomic_add(double* p, double v) {
+#pragma omp atomic
+    *p += v;
+}
+static inline void cross3(const double* a, const double* b, double* o) {
+    o[0] = a[1] * b[2] - a[2] * b[1]; o[1] = a[2] * b[0] - a[0] * b[2]; o[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+void orc_backward(int64_t n, const float* mean, const float* scale, const float* quat,
+                  const float* opacity, const float* rgb, const uint8_t* active,
+                  const double* camv, const double* cfgv, int brute, const double* up /* 8*H*W */,
+                  double* d_mean, double* d_scale, double* d_quat, double* d_opacity, double* d_rgb,
+                  double* d_pose /* 6 */, double* dM_out /* n*9, nullable */, double* dnc_out /* n*3, nullable */,
+                  uint8_t* surfel_fragile /* n, nullable */) {
+    Ctx c; ctx_init(&c, n, mean, scale, quat, opacity, rgb, active, camv, cfgv, brute);
+    const int W = c.cam.W, H = c.cam.H; const int64_t HW = (int64_t)W * H;
+    const size_t nn = (size_t)(n > 0 ? n : 1);
+    double* dM = (double*)calloc(nn * 9, sizeof(double));
+    double* dnc = (double*)calloc(nn * 3, sizeof(double));
+    memset(d_mean, 0, sizeof(double) * 3 * (size_t)n); memset(d_scale, 0, sizeof(double) * 2 * (size_t)n);
+    memset(d_quat, 0, sizeof(double) * 4 * (size_t)n); memset(d_opacity, 0, sizeof(double) * (size_t)n);
+    memset(d_rgb, 0, sizeof(double) * 3 * (size_t)n);
+    if (surfel_fragile) memset(surfel_fragile, 0, (size_t)n);
+#pragma omp parallel
+    {
+        size_t cap = 256; Hit* hits = (Hit*)malloc(sizeof(Hit) * cap);
+#pragma omp for schedule(dynamic, 1)
+        for (int j = 0; j < H; ++j) {
+            for (int i = 0; i < W; ++i) {
+                const double x = i + 0.5, y = j + 0.5;
+                const int64_t pix = (int64_t)j * W + i;
+                double g[8];
+                for (int ch = 0; ch < 8; ++ch) g[ch] = up[ch * HW + pix];
+                const uint32_t* lst; const int64_t m = cand_count(&c, i, j, &lst);
+                /* forward replay, storing the composited list */
+                size_t nh = 0; double T = 1.0;
+                for (int64_t e = 0; e < m; ++e) {
+                    const uint32_t raw = lst ? lst[e] : (uint32_t)e;
+                    const uint32_t k = c.ord[raw & 0x7fffffffu];
+                    const Prep* p = c.P + k;
+                    if (lst && (x < p->aabb[0] - 1.0 || x > p->aabb[1] + 1.0 || y < p->aabb[2] - 1.0 || y > p->aabb[3] + 1.0))
+                        continue;
+                    Pair r; int covers, f = 0;
+                    const int st = eval_pair(p, opacity[k], x, y, T, &c.cfg, &r, &f, &covers);
+                    if (f && surfel_fragile) surfel_fragile[k] = 1; /* benign race: any writer stores 1 */
+                    if (st == 2) break;
+                    if (st == 0) continue;
+                    if (nh == cap) { cap *= 2; hits = (Hit*)realloc(hits, sizeof(Hit) * cap); }
+                    hits[nh].k = k; hits[nh].r = r; hits[nh].T = T; ++nh;
+                    T *= (1.0 - r.a);
+                }
+                /* reverse sweep */
+                double suffix = 0.0; /* sum_{j>i} w_j (g . v_j) */
+                for (size_t q = nh; q-- > 0;) {
+                    const Hit* h = hits + q; const uint32_t k = h->k; const Prep* p = c.P + k; const Pair* r = &h->r;
+                    const double w = r->a * h->T;
+                    const double gv = g[0] * rgb[3 * k] + g[1] * rgb[3 * k + 1] + g[2] * rgb[3 * k + 2] + g[3] * r->z +
+                                      g[4] * p->tnc[0] + g[5] * p->tnc[1] + g[6] * p->tnc[2] + g[7];
+                    for (int ch = 0; ch < 3; ++ch) {
+                        atomic_add(d_rgb + 3 * k + ch, g[ch] * w);
+                        atomic_add(dnc + 3 * k + ch, g[4 + ch] * w);
+                    }
+                    const double dz = g[3] * w;
+                    const double da = h->T * gv - suffix / (1.0 - r->a);
+                    suffix += w * gv;
+                    double dG = 0.0;
+                    if (!r->clamped) { atomic_add(d_opacity + k, da * r->G); dG = da * opacity[k]; }
+                    const double du = -r->u * r->G * dG + dz * p->M[6];
+                    const double dv = -r->v * r->G * dG + dz * p->M[7];
+                    const double dk[3] = {du / r->k[2], dv / r->k[2], -(r->u * du + r->v * dv) / r->k[2]};
+                    double dhu[3], dhv[3];
+                    cross3(r->hv, dk, dhu);
+                    cross3(dk, r->hu, dhv);
+                    const double uv1[3] = {r->u, r->v, 1.0};
+                    for (int t = 0; t < 3; ++t) {
+                        atomic_add(dM + 9 * k + t, dhu[t]);
+                        atomic_add(dM + 9 * k + 3 + t, dhv[t]);
+                        atomic_add(dM + 9 * k + 6 + t, dz * uv1[t] - x * dhu[t] - y * dhv[t]);
+                    }
+                }
+            }
+        }
+        free(hits);
+    }
+    /* O6 + O7 */
+    double pose[6] = {0, 0, 0, 0, 0, 0};
+    const double* Rc = c.cam.R;
+    for (int64_t k = 0; k < n; ++k) {
+        const Prep* p = c.P + k;
+        if (p->culled) continue;
+        const double* m = dM + 9 * k;
+        const double su = scale[2 * k], sv = scale[2 * k + 1];
+        double Gc[3][3]; /* Gc[row][col] = dL/dA, A = [s_u t_uc, s_v t_vc, mu_c]  (Eq. 9, K^T dL/dM) */
+        for (int col = 0; col < 3; ++col) {
+            Gc[0][col] = c.cam.fx * m[col];
+            Gc[1][col] = c.cam.fy * m[3 + col];
+            Gc[2][col] = c.cam.cx * m[col] + c.cam.cy * m[3 + col] + m[6 + col];
+        }
+        double dtuc[3], dtvc[3], dtnc[3], dmuc[3];
+        double dsu = 0, dsv = 0;
+        for (int r = 0; r < 3; ++r) {
+            dtuc[r] = su * Gc[r][0]; dtvc[r] = sv * Gc[r][1]; dmuc[r] = Gc[r][2]; dtnc[r] = dnc[3 * k + r];
+            dsu += p->tuc[r] * Gc[r][0]; dsv += p->tvc[r] * Gc[r][1];
+        }
+        d_scale[2 * k] = dsu; d_scale[2 * k + 1] = dsv;
+        /* pose, Eq. 11-13 */
+        double t0[3], t1[3], t2[3], t3[3];
+        cross3(p->muc, dmuc, t0); cross3(p->tuc, dtuc, t1); cross3(p->tvc, dtvc, t2); cross3(p->tnc, dtnc, t3);
+        for (int r = 0; r < 3; ++r) { pose[r] += dmuc[r]; pose[3 + r] += t0[r] + t1[r] + t2[r] + t3[r]; }
+        /* to world: x_c = R_cw x_w  =>  dL/dx_w = R_cw^T dL/dx_c */
+        double GR[3][3]; /* dL/dR (world), columns t_u, t_v, t_n */
+        for (int r = 0; r < 3; ++r) {
+            d_mean[3 * k + r] = Rc[0 + r] * dmuc[0] + Rc[3 + r] * dmuc[1] + Rc[6 + r] * dmuc[2];
+            GR[r][0] = Rc[0 + r] * dtuc[0] + Rc[3 + r] * dtuc[1] + Rc[6 + r] * dtuc[2];
+            GR[r][1] = Rc[0 + r] * dtvc[0] + Rc[3 + r] * dtvc[1] + Rc[6 + r] * dtvc[2];
+            GR[r][2] = Rc[0 + r] * dtnc[0] + Rc[3 + r] * dtnc[1] + Rc[6 + r] * dtnc[2];
+        }
+        const double qw = p->qh[0], qx = p->qh[1], qy = p->qh[2], qz = p->qh[3];
+        double dq[4];
+        dq[0] = 2.0 * (-qz * GR[0][1] + qy * GR[0][2] + qz * GR[1][0] - qx * GR[1][2] - qy * GR[2][0] + qx * GR[2][1]);
+        dq[1] = 2.0 * (qy * GR[0][1] + qz * GR[0][2] + qy * GR[1][0] - 2.0 * qx * GR[1][1] - qw * GR[1][2] + qz * GR[2][0] + qw * GR[2][1] - 2.0 * qx * GR[2][2]);
+        dq[2] = 2.0 * (-2.0 * qy * GR[0][0] + qx * GR[0][1] + qw * GR[0][2] + qx * GR[1][0] + qz * GR[1][2] - qw * GR[2][0] + qz * GR[2][1] - 2.0 * qy * GR[2][2]);
+        dq[3] = 2.0 * (-2.0 * qz * GR[0][0] - qw * GR[0][1] + qx * GR[0][2] + qw * GR[1][0] - 2.0 * qz * GR[1][1] + qy * GR[1][2] + qx * GR[2][0] + qy * GR[2][1]);
+        const double qd = qw * dq[0] + qx * dq[1] + qy * dq[2] + qz * dq[3];
+        for (int r = 0; r < 4; ++r) d_quat[4 * k + r] = (dq[r] - p->qh[r] * qd) / p->qn; /* through q/|q| */
+    }
+    for (int r = 0; r < 6; ++r) d_pose[r] = pose[r];
+    if (dM_out) memcpy(dM_out, dM, sizeof(double) * 9 * (size_t)n);
+    if (dnc_out) memcpy(dnc_out, dnc, sizeof(double) * 3 * (size_t)n);
+    free(dM); free(dnc);
+    ctx_free(&c);
+}
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

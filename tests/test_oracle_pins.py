@@ -1,0 +1,381 @@
+"""Pins of the CPU oracle (P1-P10) against what PAPER.md and the mathematics fix.
+None of these retypes the oracle's formula: they use closed forms, a hand-evaluated fixture, a
+library matrix inverse, scipy rotations, invariants, finite differences and symmetries."""
+import os
+import numpy as np
+import pytest
+from scipy.spatial.transform import Rotation
+
+import oracle
+import scenegen
+from scenegen import Scene, Camera
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def one_surfel(mu, s, q, o=0.8, rgb=(0.2, 0.5, 0.9)):
+    f = lambda a, sh: np.asarray(a, np.float32).reshape(sh)
+    return Scene(f(mu, (1, 3)), f(s, (1, 2)), f(q, (1, 4)), f([o], (1,)), f(rgb, (1, 3)))
+
+
+def cat(*scs):
+    return Scene(*[np.concatenate([getattr(s, k) for s in scs]) for k in ("mean", "scale", "quat", "opacity", "rgb")])
+
+
+CAM = Camera(64, 48, 60.0, 60.0, 32.0, 24.0)
+
+
+def pix_grid(cam):
+    x = np.arange(cam.width) + 0.5
+    y = np.arange(cam.height) + 0.5
+    return np.meshgrid(x, y)  # (H,W) each
+
+
+# ---------------------------------------------------------------- P1: closed-form footprint (Eq. 1-4, 8)
+@pytest.mark.parametrize("mu", [(0.0, 0.0, 2.0), (0.31, -0.17, 1.5)])
+def test_p1_fronto_parallel_footprint(mu):
+    su, sv, o = 0.11, 0.07, 0.8
+    sc = one_surfel(mu, (su, sv), (1, 0, 0, 0), o)
+    r = oracle.render(sc, oracle.make_cam(CAM), oracle.make_cfg())
+    X, Y = pix_grid(CAM)
+    mu32 = np.float32(mu).astype(np.float64); su, sv, o = [float(np.float32(v)) for v in (su, sv, o)]
+    z0 = mu32[2]
+    u = ((X - CAM.cx) * z0 / CAM.fx - mu32[0]) / su
+    v = ((Y - CAM.cy) * z0 / CAM.fy - mu32[1]) / sv
+    a = o * np.exp(-(u * u + v * v) / 2)
+    a[(u * u + v * v > 9.0) | (a < float(np.float32(1 / 255)))] = 0.0
+    assert np.abs(a).max() > 0.5
+    np.testing.assert_allclose(r["img"][7], a, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(r["img"][3], a * z0, rtol=0, atol=1e-12)       # depth plane = a * z0
+    np.testing.assert_allclose(r["img"][0], a * float(np.float32(0.2)), atol=1e-12)
+    np.testing.assert_allclose(r["img"][6], a * 1.0, atol=1e-12)              # normal = +z for R = I
+
+
+# ---------------------------------------------------------------- P2: depth = ray-plane intersection depth
+def test_p2_tilted_plane_depth():
+    rot = Rotation.from_euler("xyz", [25, -35, 10], degrees=True)
+    qx, qy, qz, qw = rot.as_quat()
+    mu = np.array([0.1, -0.05, 1.8])
+    sc = one_surfel(mu, (0.3, 0.2), (qw, qx, qy, qz), 0.9)
+    r = oracle.render(sc, oracle.make_cam(CAM), oracle.make_cfg())
+    q32 = sc.quat[0].astype(np.float64)
+    n = Rotation.from_quat([q32[1], q32[2], q32[3], q32[0]]).as_matrix()[:, 2]
+    X, Y = pix_grid(CAM)
+    d = np.stack([(X - CAM.cx) / CAM.fx, (Y - CAM.cy) / CAM.fy, np.ones_like(X)], axis=-1)
+    z = (n @ sc.mean[0].astype(np.float64)) / (d @ n)
+    O = r["img"][7]
+    m = O > 0
+    assert m.sum() > 100
+    np.testing.assert_allclose(r["img"][3][m] / O[m], z[m], rtol=1e-12)
+    # normal plane = O * t_n in camera space (identity pose)
+    for ch in range(3):
+        np.testing.assert_allclose(r["img"][4 + ch][m], O[m] * n[ch], atol=1e-12)
+
+
+# ---------------------------------------------------------------- P3: hand-evaluated stacks (golden fixture)
+def _read_stack():
+    rows, exp = [], {}
+    for line in open(os.path.join(GOLDEN, "eq8_stack.txt")):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        a, b = line.split()
+        if a.startswith("expected"):
+            exp[a] = float(b)
+        else:
+            rows.append((float(a), float(b)))
+    return rows, exp
+
+
+def _stack_scene(rows, depths):
+    i, j = 40, 13  # pixel whose centre the surfels project onto
+    scs = []
+    for (o, val), z in zip(rows, depths):
+        mu = ((i + 0.5 - CAM.cx) / CAM.fx * z, (j + 0.5 - CAM.cy) / CAM.fy * z, z)
+        scs.append(one_surfel(mu, (0.2, 0.2), (1, 0, 0, 0), o, (val, 0, 0)))
+    return cat(*scs), i, j
+
+
+def test_p3_hand_computed_stack():
+    rows, exp = _read_stack()
+    cfg = oracle.make_cfg(alpha_max=1.0)
+    sc, i, j = _stack_scene(rows, (1.0, 2.0, 3.0))
+    r = oracle.render(sc, oracle.make_cam(CAM), cfg)
+    assert abs(r["img"][0][j, i] - exp["expected_V"]) < 1e-6
+    assert abs(r["img"][7][j, i] - exp["expected_O"]) < 1e-6
+    assert abs(r["T_final"][j, i] - exp["expected_T"]) < 1e-6
+    sc, i, j = _stack_scene(rows, (2.0, 1.0, 3.0))  # first two swapped in depth
+    r = oracle.render(sc, oracle.make_cam(CAM), cfg)
+    assert abs(r["img"][0][j, i] - exp["expected_V_swapped"]) < 1e-6
+    assert abs(r["img"][7][j, i] - exp["expected_O"]) < 1e-6
+
+
+def test_p3_depth_ties_break_by_index():
+    """Equal depth bits: order is the surfel index (R2), so listing order decides the blend."""
+    rows = [(0.5, 1.0), (0.5, 3.0)]
+    sc, i, j = _stack_scene(rows, (2.0, 2.0))
+    r = oracle.render(sc, oracle.make_cam(CAM), oracle.make_cfg())
+    assert abs(r["img"][0][j, i] - (0.5 * 1.0 + 0.25 * 3.0)) < 1e-6
+
+
+# ---------------------------------------------------------------- P4: invariants
+@pytest.fixture(scope="module")
+def c1():
+    sc, cams, _ = scenegen.make_config("C1")
+    camv, cfg = oracle.make_cam(cams[0]), oracle.make_cfg()
+    return sc, cams[0], camv, cfg, oracle.render(sc, camv, cfg)
+
+
+def test_p4_invariants(c1):
+    sc, cam, camv, cfg, r = c1
+    O, T = r["img"][7], r["T_final"]
+    np.testing.assert_allclose(O, 1.0 - T, atol=1e-13)
+    assert O.max() <= 1.0 and O.min() >= 0.0 and T.min() >= float(cfg[4])
+    assert r["counters"]["Q_c"] == r["n_comp"].sum() and r["counters"]["Q_c"] > 5000
+    assert (r["img"][3] >= 0).all()
+
+
+def test_brute_force_equals_skipping_bitwise(c1):
+    sc, cam, camv, cfg, r = c1
+    rb = oracle.render(sc, camv, cfg, brute=True)
+    assert np.array_equal(r["img"], rb["img"]) and np.array_equal(r["T_final"], rb["T_final"])
+    up = scenegen.upstream_normal(1, cam.height, cam.width)
+    g, gb = oracle.backward(sc, camv, cfg, up), oracle.backward(sc, camv, cfg, up, brute=True)
+    for k in ("mean", "scale", "quat", "opacity", "rgb", "pose"):
+        np.testing.assert_allclose(g[k], gb[k], rtol=1e-10, atol=1e-9)  # atomics reorder fp64 sums
+
+
+# ---------------------------------------------------------------- P5: channels are the same blend (L118-120)
+def test_p5_channel_consistency(c1):
+    sc, cam, camv, cfg, r = c1
+    ones = Scene(sc.mean, sc.scale, sc.quat, sc.opacity, np.ones_like(sc.rgb))
+    r1 = oracle.render(ones, camv, cfg)
+    for ch in range(3):
+        np.testing.assert_allclose(r1["img"][ch], r["img"][7], atol=1e-13)
+    q = sc.quat.astype(np.float64)
+    n_c = Rotation.from_quat(q[:, [1, 2, 3, 0]]).as_matrix()[:, :, 2]  # identity pose: t_nc = t_n
+    rn = oracle.render(Scene(sc.mean, sc.scale, sc.quat, sc.opacity, n_c.astype(np.float32)), camv, cfg)
+    np.testing.assert_allclose(rn["img"][0:3], r["img"][4:7], atol=2e-7)  # rgb carries f32-rounded normals
+
+
+# ---------------------------------------------------------------- P6: truncation constants -> plain Eq. 8
+def test_p6_truncation_limit(c1):
+    sc, cam, camv, cfg, r = c1
+    smooth = oracle.render(sc, camv, oracle.smooth_cfg())["img"]
+    errs = []
+    for c, amin, tmin in [(2.0, 1 / 64, 1e-2), (3.0, 1 / 255, 1e-4), (4.0, 1e-4, 1e-6), (6.0, 1e-8, 1e-10), (9.0, 0.0, 0.0)]:
+        cc = oracle.make_cfg(cutoff=c, alpha_min=amin, alpha_max=1.0, t_min=tmin, z_near=0.0)
+        errs.append(np.abs(oracle.render(sc, camv, cc)["img"] - smooth).max())
+    assert all(a > b for a, b in zip(errs, errs[1:])), errs
+    assert errs[-1] < 1e-12
+
+
+# ---------------------------------------------------------------- P7: binning (list structure + conservativeness)
+def _numpy_uv(M, X, Y):
+    """(u,v) by the textbook route the paper avoids: invert the 3x3 homography with a library
+    routine, (u,v,1) ~ M^-1 (x,y,1).  Independent of the oracle's cross-product formula (R1)."""
+    Minv = np.linalg.inv(M)
+    p = np.stack([X, Y, np.ones_like(X)], axis=-1) @ Minv.T
+    return p[..., 0] / p[..., 2], p[..., 1] / p[..., 2]
+
+
+def test_p7_binning_structure_and_conservativeness(c1):
+    sc, cam, camv, cfg, r = c1
+    b = oracle.binning(sc, camv, cfg)
+    E, keys, idx, ranges = b["E"], b["keys"], b["idx"], b["ranges"]
+    assert E == int(b["count"].sum()) == len(keys)
+    assert (np.diff(keys.astype(np.uint64)) >= 0).all() if E > 1 else True
+    # ranges partition the list in tile order
+    nz = ranges[ranges[:, 1] > ranges[:, 0]]
+    assert nz[0, 0] == 0 and nz[-1, 1] == E and (nz[1:, 0] == nz[:-1, 1]).all()
+    for t, (s, e) in enumerate(ranges):
+        assert ((keys[s:e] >> np.uint64(32)) == t).all()
+        same = keys[s:e][1:] == keys[s:e][:-1]
+        assert (idx[s:e][1:][same] > idx[s:e][:-1][same]).all()      # stable: ties by surfel index
+    # depth bits are those of float32(mu_c.z); identity pose => mu_c.z = mean z
+    vis = b["culled"] == 0
+    assert np.array_equal(b["depth_bits"][vis], sc.mean[vis, 2].view(np.uint32))
+    # conservativeness: every covering pair (rho^2 <= c^2 via library inverse) is in the pixel's tile list
+    X, Y = pix_grid(cam)
+    tile = int(cfg[0])
+    tid = (np.arange(cam.height)[:, None] // tile) * b["tiles_x"] + (np.arange(cam.width)[None, :] // tile)
+    members = [set(idx[s:e].tolist()) for s, e in ranges]
+    n_cover = 0
+    tt = np.linspace(0, 2 * np.pi, 20001)
+    for k in np.nonzero(vis)[0]:
+        u, v = _numpy_uv(b["M"][k].reshape(3, 3), X, Y)
+        cover = (u * u + v * v <= 9.0)
+        n_cover += cover.sum()
+        for t in np.unique(tid[cover]):
+            assert k in members[t]
+        # the AABB is exact: forward-map the cutoff circle with Eq. 4, x = (M0.p)/(M2.p), p = (3cos t, 3sin t, 1)
+        xmin, xmax, ymin, ymax = b["aabb"][k]
+        pc = np.stack([3 * np.cos(tt), 3 * np.sin(tt), np.ones_like(tt)], axis=0)
+        Mk = b["M"][k].reshape(3, 3)
+        ex, ey = (Mk[0] @ pc) / (Mk[2] @ pc), (Mk[1] @ pc) / (Mk[2] @ pc)
+        tol = 1e-5 * max(1.0, xmax - xmin, ymax - ymin)
+        assert abs(ex.min() - xmin) < tol and abs(ex.max() - xmax) < tol
+        assert abs(ey.min() - ymin) < tol and abs(ey.max() - ymax) < tol
+    assert n_cover >= r["counters"]["cover"] > 0   # z>z_near and culling only remove pairs
+
+
+def test_p7_full_forward_against_library_inverse(c1):
+    """Whole forward against an independent numpy render: library matrix inverse for (u,v),
+    cumulative product for the transmittance (Eq. 8 written as array ops)."""
+    sc, cam, camv, cfg, r = c1
+    b = oracle.binning(sc, camv, cfg)
+    X, Y = pix_grid(cam)
+    order = np.lexsort((np.arange(sc.n), b["depth_bits"]))
+    order = order[b["culled"][order] == 0]
+    amin, amax, tmin, znear = cfg[2], cfg[3], cfg[4], cfg[5]
+    T = np.ones_like(X); done = np.zeros_like(X, bool); img = np.zeros((8,) + X.shape)
+    n_c = Rotation.from_quat(sc.quat.astype(np.float64)[:, [1, 2, 3, 0]]).as_matrix()[:, :, 2]
+    for k in order:
+        M = b["M"][k].reshape(3, 3)
+        u, v = _numpy_uv(M, X, Y)
+        z = M[2, 0] * u + M[2, 1] * v + M[2, 2]
+        a = np.minimum(amax, float(sc.opacity[k]) * np.exp(-(u * u + v * v) / 2))
+        ok = (u * u + v * v <= 9.0) & (z > znear) & (a >= amin) & ~done
+        stop = ok & (T * (1 - a) < tmin)
+        done |= stop
+        ok &= ~stop
+        w = np.where(ok, a * T, 0.0)
+        vals = list(sc.rgb[k].astype(np.float64)) + [z] + list(n_c[k]) + [1.0]
+        for ch in range(8):
+            img[ch] += w * vals[ch]
+        T = np.where(ok, T * (1 - a), T)
+    good = r["fragile"] == 0
+    assert good.mean() > 0.99
+    np.testing.assert_allclose(img[:, good], r["img"][:, good], rtol=1e-9, atol=1e-11)
+
+
+# ---------------------------------------------------------------- P8: finite differences of every gradient
+def _tiny(seed=7, n=6):
+    g = scenegen.SplitMix(seed)
+    mean = np.stack([g.uniform(n, -0.25, 0.25), g.uniform(n, -0.2, 0.2), g.uniform(n, 0.8, 1.6)], 1)
+    scale = np.exp(np.stack([g.uniform(n, np.log(0.08), np.log(0.2)) for _ in range(2)], 1))
+    quat = np.stack([g.normal(n) for _ in range(4)], 1) * g.uniform(n, 0.5, 2.0)[:, None]   # NOT unit
+    quat[:, 0] += 2.0 * np.sign(quat[:, 0])  # mostly camera-facing
+    sc = Scene(mean.astype(np.float32), scale.astype(np.float32), quat.astype(np.float32),
+               g.uniform(n, 0.3, 0.95).astype(np.float32), np.stack([g.uniform(n) for _ in range(3)], 1).astype(np.float32))
+    cam = Camera(16, 12, 14.0, 15.0, 8.3, 5.6, scenegen.perturb_pose(np.eye(4)[:3], [0.02, -0.03, 0.05, 0.04, -0.03, 0.06]))
+    return sc, cam
+
+
+def _loss(sc, camv, cfg, up):
+    return float((oracle.render(sc, camv, cfg, counters=False)["img"] * up).sum())
+
+
+def _fd_check(cfg, rtol):
+    sc, cam = _tiny()
+    camv = oracle.make_cam(cam, widen_from_f32=False)
+    up = scenegen.upstream_normal(11, cam.height, cam.width).astype(np.float64)
+    g = oracle.backward(sc, camv, cfg, up)
+    worst = 0.0
+    for name in ("mean", "scale", "quat", "opacity", "rgb"):
+        arr = getattr(sc, name)
+        flat = arr.reshape(-1)
+        ga = g[name].reshape(-1)
+        scale_ref = np.abs(ga).max() + 1e-30
+        for e in range(flat.size):
+            x0 = flat[e]
+            h = np.float32(max(abs(float(x0)), 0.05) * 2.0 ** -12)
+            xp, xm = np.float32(x0 + h), np.float32(x0 - h)
+            flat[e] = xp; lp = _loss(sc, camv, cfg, up)
+            flat[e] = xm; lm = _loss(sc, camv, cfg, up)
+            flat[e] = x0
+            fd = (lp - lm) / (float(xp) - float(xm))          # exact step between two float32 inputs
+            err = abs(fd - ga[e]) / scale_ref
+            worst = max(worst, err)
+            assert err < rtol, (name, e, fd, ga[e])
+    # SE(3) pose: central differences of L(Exp(+-eps e_i) o T_cw)   (Eq. 12)
+    eps = 1e-6
+    for i in range(6):
+        tau = np.zeros(6); tau[i] = eps
+        lp = _loss(sc, oracle.make_cam(cam, scenegen.perturb_pose(cam.T_cw, tau), False), cfg, up)
+        lm = _loss(sc, oracle.make_cam(cam, scenegen.perturb_pose(cam.T_cw, -tau), False), cfg, up)
+        fd = (lp - lm) / (2 * eps)
+        assert abs(fd - g["pose"][i]) < rtol * np.abs(g["pose"]).max(), (i, fd, g["pose"])
+    return worst
+
+
+def test_p8_finite_differences_smooth():
+    """Plain Eq. 8 (no truncation): every surfel gradient and the SE(3) pose gradient."""
+    _fd_check(oracle.smooth_cfg(), 2e-6)
+
+
+def test_p8_finite_differences_alpha_clamp():
+    """alpha_max clamp active (true derivative = 0 when clamped, R5), other truncations off."""
+    cfg = oracle.make_cfg(cutoff=np.inf, alpha_min=0.0, alpha_max=0.6, t_min=0.0, z_near=0.0)
+    sc, cam = _tiny()
+    r = oracle.render(sc, oracle.make_cam(cam, widen_from_f32=False), cfg)
+    assert (r["fragile"] & 2).sum() == 0, "pick another seed: a pixel sits on the clamp boundary"
+    _fd_check(cfg, 2e-6)
+
+
+# ---------------------------------------------------------------- P9: rigid-motion identity (no FD)
+def test_p9_rigid_motion_identity():
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = Camera(64, 48, 60.0, 60.0, 32.0, 24.0, scenegen.perturb_pose(np.eye(4)[:3], [0.1, -0.2, 0.15, 0.2, -0.1, 0.3]))
+    camv, cfg = oracle.make_cam(cam), oracle.make_cfg()
+    up = scenegen.upstream_normal(3, cam.height, cam.width)
+    g = oracle.backward(sc, camv, cfg, up)
+    T = camv[6:].reshape(3, 4); R, t = T[:, :3], T[:, 3]
+    c_cam = -R.T @ t
+    gm, gq = g["mean"], g["quat"]
+    q = sc.quat.astype(np.float64); w, v = q[:, :1], q[:, 1:]
+    gw, gv = gq[:, :1], gq[:, 1:]
+    rot_term = 0.5 * (-gw * v + w * gv + np.cross(v, gv))
+    d_rho = R @ gm.sum(0)
+    d_theta = R @ (np.cross(sc.mean.astype(np.float64) - c_cam, gm) + rot_term).sum(0)
+    s = np.abs(g["pose"]).max()
+    np.testing.assert_allclose(g["pose"][:3], d_rho, atol=1e-9 * s)
+    np.testing.assert_allclose(g["pose"][3:], d_theta, atol=1e-9 * s)
+    # scale gradient is invisible to a rigid motion but the quaternion gradient must be tangent to |q|
+    assert np.abs((q * gq).sum(1)).max() < 1e-9 * np.abs(gq).max()
+
+
+# ---------------------------------------------------------------- P10: symmetries
+def test_p10_swap_tangents(c1):
+    sc, cam, camv, cfg, r = c1
+    q = sc.quat.astype(np.float64)
+    s = np.sqrt(0.5)
+    qs = np.array([0.0, s, s, 0.0])  # 180 deg about (1,1,0): t_u <-> t_v, t_n -> -t_n
+    w1, v1 = q[:, :1], q[:, 1:]
+    q2 = np.concatenate([w1 * qs[0] - v1 @ qs[1:, None], w1 * qs[1:] + qs[0] * v1 + np.cross(v1, qs[1:])], axis=1)
+    sw = Scene(sc.mean, sc.scale[:, ::-1].copy(), q2.astype(np.float32), sc.opacity, sc.rgb)
+    r2 = oracle.render(sw, camv, cfg)
+    good = (r["fragile"] == 0) & (r2["fragile"] == 0)
+    np.testing.assert_allclose(r2["img"][[0, 1, 2, 3, 7]][:, good], r["img"][[0, 1, 2, 3, 7]][:, good], rtol=1e-4, atol=2e-5)
+    np.testing.assert_allclose(r2["img"][4:7][:, good], -r["img"][4:7][:, good], rtol=1e-4, atol=2e-5)
+
+
+def test_p10_mask_equals_subset():
+    sc, cams, _ = scenegen.make_config("C1")
+    act = (scenegen.SplitMix(99).uniform(sc.n) < 0.3).astype(np.uint8)
+    camv, cfg = oracle.make_cam(cams[0]), oracle.make_cfg()
+    masked = Scene(sc.mean, sc.scale, sc.quat, sc.opacity, sc.rgb, act)
+    m = act.astype(bool)
+    sub = Scene(sc.mean[m], sc.scale[m], sc.quat[m], sc.opacity[m], sc.rgb[m])
+    ra, rs = oracle.render(masked, camv, cfg), oracle.render(sub, camv, cfg)
+    assert np.array_equal(ra["img"], rs["img"])
+    ba, bs = oracle.binning(masked, camv, cfg), oracle.binning(sub, camv, cfg)
+    remap = np.nonzero(m)[0]
+    assert np.array_equal(ba["keys"], bs["keys"]) and np.array_equal(ba["idx"], remap[bs["idx"]])
+    up = scenegen.upstream_normal(5, 48, 64)
+    ga, gs = oracle.backward(masked, camv, cfg, up), oracle.backward(sub, camv, cfg, up)
+    assert (ga["mean"][~m] == 0).all() and (ga["quat"][~m] == 0).all() and (ga["opacity"][~m] == 0).all()
+    np.testing.assert_allclose(ga["mean"][m], gs["mean"], rtol=1e-10, atol=1e-9)
+    np.testing.assert_allclose(ga["pose"], gs["pose"], rtol=1e-10)
+
+
+def test_no_view_dependence_of_colour():
+    """L128: no spherical harmonics -- rotating the camera about its centre leaves a surfel's
+    blended colour / alpha ratio at its own centre pixel unchanged."""
+    sc = one_surfel((0.0, 0.0, 2.0), (0.3, 0.3), (1, 0, 0, 0), 0.7, (0.3, 0.6, 0.9))
+    for ang in (0.0, 0.1, -0.2):
+        T = scenegen.perturb_pose(np.eye(4)[:3], [0, 0, 0, 0, ang, 0])
+        r = oracle.render(sc, oracle.make_cam(CAM, T), oracle.make_cfg())
+        m = r["img"][7] > 0.05
+        for ch, c in enumerate((0.3, 0.6, 0.9)):
+            np.testing.assert_allclose(r["img"][ch][m] / r["img"][7][m], float(np.float32(c)), rtol=1e-12)
