@@ -1,0 +1,178 @@
+/*
+ * sgs.h -- C ABI of the B200-native differentiable 2D-Gaussian (surfel) splatting renderer,
+ * the hot path of 2DGS-SLAM (arxiv 2506.00970).  Citations are PAPER.md line numbers; "R<n>"
+ * are the readings of the paper listed in DESIGN.md §3.
+ *
+ * The interface follows the paper's statement of the problem: a map of splats
+ * (mu, R, s_u, s_v, c, alpha) (L122) and a camera pose T_cw in SE(3) with a projection W (L95) go
+ * in; colour, depth, normal and opacity images come out (Eq. 8); a rendering loss's
+ * image gradients go in, gradients to the splat parameters (L122) and to the pose in the tangent
+ * space of SE(3) (Eq. 9-13) come out; tracking renders only active splats (L204).
+ *
+ * Conventions
+ *   - Plain pointers and sizes only.  Every pointer says HOST or DEVICE.  All device buffers are
+ *     the caller's (borrowed for the duration of the call / until the matching backward); the
+ *     library never frees them.  The ctx owns its workspace, obtained through the caller's
+ *     allocator callbacks (or cudaMalloc/cudaFree when the callbacks are NULL).
+ *   - Every call returns an int status (SGS_OK = 0).  No exceptions, no abort, no stdout.
+ *   - Work is enqueued on the given CUDA stream (a cudaStream_t passed as void*).  sgs_render in
+ *     the default (safe) mode waits once for the tile-entry count E; with SGS_FLAG_ASYNC it does
+ *     not synchronise at all and a workspace overflow is reported by the NEXT call on the ctx.
+ *   - Scales and opacity are ACTIVATED values (s > 0 metres, opacity in (0,1]) (R16).  The
+ *     quaternion is (w,x,y,z), need not be unit; it is normalised inside and its gradient
+ *     includes the normalisation.
+ *   - Pixel (i,j) samples the image point (i+0.5, j+0.5), x = fx X/Z + cx (R17).  Images are
+ *     channel-planar fp32, background 0.  depth = sum w z, normal = sum w t_nc (camera space,
+ *     not flipped, not normalised), alpha = sum w (R9, R10).
+ *   - Pose gradient: d_pose6 = (dL/drho, dL/dtheta) for the left perturbation
+ *     T <- Exp(tau) o T_cw, tau = (rho, theta), translation first (Eq. 12-13, R15).
+ *   - Gradients are OVERWRITTEN, and are exactly zero for inactive or culled surfels.
+ */
+#ifndef SGS_H
+#define SGS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define SGS_API __attribute__((visibility("default")))
+#else
+#define SGS_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sgs_ctx sgs_ctx; /* opaque; owns workspace + the last forward's saved state */
+
+/* Caller's device allocator (e.g. torch's caching allocator).  stream is a cudaStream_t. */
+typedef void* (*sgs_alloc_fn)(size_t bytes, void* user, void* stream);
+typedef void (*sgs_free_fn)(void* ptr, void* user, void* stream);
+
+enum {
+    SGS_OK = 0,
+    SGS_INVALID_ARGUMENT = 1,
+    SGS_OUT_OF_MEMORY = 2,
+    SGS_WORKSPACE_OVERFLOW = 3, /* async mode: the previous render overflowed; workspace was grown, render again */
+    SGS_NO_FORWARD_STATE = 4,   /* sgs_backward without a preceding successful sgs_render */
+    SGS_CUDA_ERROR = 5
+};
+
+enum {
+    SGS_FLAG_ASYNC = 1 /* never synchronise the host in sgs_render (CUDA-graph capturable) */
+};
+
+/* Truncation conventions of Eq. 8 (R3-R7).  sgs_default_config fills the defaults shown. */
+typedef struct {
+    int tile;        /* 16: tile edge in pixels (only 16 is supported)                       */
+    float cutoff;    /* 3.0: pairs with u^2+v^2 > cutoff^2 contribute nothing (R3)           */
+    float alpha_min; /* 1/255: pairs with a < alpha_min are skipped (R4)                     */
+    float alpha_max; /* 0.99: a = min(alpha_max, o G), true derivative (0 when clamped) (R5) */
+    float t_min;     /* 1e-4: stop the pixel when T(1-a) < t_min, that splat excluded (R6)   */
+    float z_near;    /* 0.2: cull centre depth <= z_near; skip pair with hit depth <= z_near (R7) */
+    int flags;       /* SGS_FLAG_* */
+    sgs_alloc_fn alloc; /* nullable */
+    sgs_free_fn free;   /* nullable */
+    void* user;
+} sgs_config;
+
+/* The map (L122, Eq. 14's g_i and delta_i).  All DEVICE pointers, fp32, borrowed. */
+typedef struct {
+    int64_t n;
+    const float* mean;     /* n x 3  world-space centre mu                       */
+    const float* scale;    /* n x 2  s_u, s_v                                    */
+    const float* quat;     /* n x 4  (w,x,y,z); R = [t_u, t_v, t_n]              */
+    const float* opacity;  /* n                                                   */
+    const float* rgb;      /* n x 3  plain RGB, no spherical harmonics (L128)     */
+    const uint8_t* active; /* n or NULL (= all active); the active flag delta_i (L161, L204) */
+} sgs_surfels;
+
+/* Camera: pinhole intrinsics in pixels standing for W (L95, R14) and T_cw (HOST values). */
+typedef struct {
+    int width, height;
+    float fx, fy, cx, cy;
+    float T_cw[12]; /* row-major 3x4 [R | t], world -> camera */
+} sgs_camera;
+
+/* Output images / upstream gradients, DEVICE, caller-owned, channel-planar fp32.
+ * In sgs_render any pointer may be NULL (that image is not written).
+ * In sgs_backward a NULL pointer means a zero upstream gradient for that image. */
+typedef struct {
+    float* rgb;    /* 3 x H x W */
+    float* depth;  /* H x W     */
+    float* normal; /* 3 x H x W */
+    float* alpha;  /* H x W     */
+} sgs_images;
+
+/* Surfel gradients, DEVICE, caller-owned, overwritten.  Layout as sgs_surfels. */
+typedef struct {
+    float* mean;    /* n x 3 */
+    float* scale;   /* n x 2 */
+    float* quat;    /* n x 4 */
+    float* opacity; /* n     */
+    float* rgb;     /* n x 3 */
+} sgs_surfel_grads;
+
+/* Counters of the last render (HOST struct; reading it synchronises the stream of that render). */
+typedef struct {
+    int64_t n_visible;    /* surfels that passed culling (N_v)                 */
+    int64_t n_entries;    /* tile entries E                                    */
+    int64_t capacity;     /* current entry capacity of the workspace           */
+    int64_t overflow;     /* 1 if the last render dropped entries              */
+    int64_t workspace_bytes;
+} sgs_stats;
+
+SGS_API int sgs_default_config(sgs_config* cfg);
+SGS_API int sgs_create(sgs_ctx** out, const sgs_config* cfg);
+SGS_API int sgs_destroy(sgs_ctx* ctx);
+
+/* Forward (Eq. 1-8): preprocess -> tile binning (64-bit tile|depth keys, radix sort, ranges)
+ * -> per-tile compositing.  Saves the state sgs_backward needs inside ctx. */
+SGS_API int sgs_render(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_camera* cam, const sgs_images* out,
+               void* cuda_stream);
+
+/* Backward of the most recent sgs_render on this ctx (same surfel buffers, unchanged).
+ *   upstream : dL/d(rgb, depth, normal, alpha)                                     DEVICE
+ *   d_surfels: nullable; NULL = pose-only mode (tracking, L204: splats frozen)     DEVICE
+ *   d_pose6  : nullable; 6 floats (rho, theta), Eq. 11-13                          DEVICE */
+SGS_API int sgs_backward(sgs_ctx* ctx, const sgs_images* upstream, const sgs_surfel_grads* d_surfels, float* d_pose6,
+                 void* cuda_stream);
+
+/* Tracking loss of Eq. 15-19 (harness around the renderer; R18, R19):
+ *   L_t = 1/|Omega| sum_p M_n M_o (|I_r - I|_1 + lambda_d |D_r - D|)
+ * with M_o = [alpha > 0.95] and M_n = [normal_sign * N_r . ray > 0].  Writes the upstream
+ * gradients of the rendered images into `upstream` (all four, zeros where masked) and the scalar
+ * loss into loss (DEVICE, 1 float).  rendered/target/upstream are DEVICE; target uses only
+ * rgb and depth. */
+SGS_API int sgs_tracking_loss(sgs_ctx* ctx, const sgs_camera* cam, const sgs_images* rendered, const sgs_images* target,
+                      float lambda_d, float normal_sign, const sgs_images* upstream, float* loss, void* cuda_stream);
+
+/* Debug export of the binning of the last render, for bit-exact parity tests.  Synchronises.
+ * Returned DEVICE pointers stay valid until the next call on ctx.  idx holds ORIGINAL surfel
+ * indices; culled[i] = 1 iff surfel i was inactive or culled. */
+SGS_API int sgs_get_binning(sgs_ctx* ctx, int64_t* n_entries, const uint64_t** keys, const uint32_t** idx,
+                    const uint32_t** tile_ranges /* tiles x 2 */, const uint8_t** culled /* n */);
+
+SGS_API int sgs_get_stats(sgs_ctx* ctx, sgs_stats* out);
+
+/* HOST-buffer convenience path (end-to-end measurement): copies in, runs, copies out, waits.
+ * sgs_upload_surfels copies a HOST map into ctx-owned device memory and makes it the resident
+ * map; the *_host calls use the resident map. */
+SGS_API int sgs_upload_surfels(sgs_ctx* ctx, const sgs_surfels* host_surfels, void* cuda_stream);
+SGS_API int sgs_render_host(sgs_ctx* ctx, const sgs_camera* cam, const sgs_images* host_out, void* cuda_stream);
+SGS_API int sgs_backward_host(sgs_ctx* ctx, const sgs_images* host_upstream, const sgs_surfel_grads* host_d_surfels,
+                      float* host_d_pose6, void* cuda_stream);
+/* One tracking iteration on the resident map against a resident target frame (uploaded by
+ * sgs_upload_target): render, Eq. 15-19 loss, pose-only backward; reads back loss and the 6-vector. */
+SGS_API int sgs_upload_target(sgs_ctx* ctx, const sgs_camera* cam, const float* host_rgb /*3xHxW*/,
+                      const float* host_depth /*HxW*/, void* cuda_stream);
+SGS_API int sgs_track_iter_host(sgs_ctx* ctx, const sgs_camera* cam, float lambda_d, float normal_sign,
+                        float* host_loss, float* host_d_pose6, void* cuda_stream);
+
+SGS_API const char* sgs_status_string(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SGS_H */

@@ -141,3 +141,25 @@ def backward(sc, camv, cfgv, upstream, brute=False, debug=False):
 
 def num_threads():
     return int(lib().orc_num_threads())
+
+
+def tracking_loss(img, target_rgb, target_depth, camv, lambda_d, normal_sign=1.0):
+    """Eq. 15-19 (L180-204) written out in numpy, fp64.  img: (8,H,W) rendered planes; returns
+    (L_t, upstream (8,H,W)).  M_n = [sign * N_r . r > 0] (Eq. 17; R19: the harness scenes use outward
+    normals so sign = -1 there), M_o = [O > 0.95] (Eq. 18); the masks carry no gradient."""
+    img = np.asarray(img, dtype=np.float64)
+    W, H = int(camv[0]), int(camv[1])
+    fx, fy, cx, cy = camv[2:6]
+    X, Y = np.meshgrid(np.arange(W) + 0.5, np.arange(H) + 0.5)
+    rx, ry = (X - cx) / fx, (Y - cy) / fy   # un-normalised ray: only the sign of N.r is used
+    nr = img[4] * rx + img[5] * ry + img[6]
+    m = ((normal_sign * nr > 0) & (img[7] > float(np.float32(0.95)))).astype(np.float64)
+    dI = img[0:3] - np.asarray(target_rgb, dtype=np.float64)
+    dD = img[3] - np.asarray(target_depth, dtype=np.float64)
+    LI = np.abs(dI).sum(0)                   # Eq. 15: element-wise L1 over the colour channels
+    LD = np.abs(dD)                          # Eq. 16
+    L = (m * (LI + lambda_d * LD)).sum() / (W * H)     # Eq. 19
+    up = np.zeros_like(img)
+    up[0:3] = m * np.sign(dI) / (W * H)
+    up[3] = m * lambda_d * np.sign(dD) / (W * H)
+    return float(L), up

@@ -1,0 +1,261 @@
+"""Thin ctypes binding over libsgs.so (include/sgs.h).  Argument marshalling only: every step of
+the path runs in the CUDA kernels behind the C ABI.  torch is used for device memory (the ctx's
+workspace comes from torch's caching allocator through the sgs_alloc_fn callbacks) and streams.
+There is NO CPU fallback: a missing library or device raises."""
+import ctypes as C
+import os
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libsgs.so")
+
+SGS_OK, SGS_INVALID_ARGUMENT, SGS_OUT_OF_MEMORY, SGS_WORKSPACE_OVERFLOW, SGS_NO_FORWARD_STATE, SGS_CUDA_ERROR = range(6)
+SGS_FLAG_ASYNC = 1
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p, C.c_void_p)
+
+
+class sgs_config(C.Structure):
+    _fields_ = [("tile", C.c_int), ("cutoff", C.c_float), ("alpha_min", C.c_float), ("alpha_max", C.c_float),
+                ("t_min", C.c_float), ("z_near", C.c_float), ("flags", C.c_int),
+                ("alloc", ALLOC_FN), ("free", FREE_FN), ("user", C.c_void_p)]
+
+
+class sgs_surfels(C.Structure):
+    _fields_ = [("n", C.c_int64), ("mean", C.c_void_p), ("scale", C.c_void_p), ("quat", C.c_void_p),
+                ("opacity", C.c_void_p), ("rgb", C.c_void_p), ("active", C.c_void_p)]
+
+
+class sgs_camera(C.Structure):
+    _fields_ = [("width", C.c_int), ("height", C.c_int), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float), ("T_cw", C.c_float * 12)]
+
+
+class sgs_images(C.Structure):
+    _fields_ = [("rgb", C.c_void_p), ("depth", C.c_void_p), ("normal", C.c_void_p), ("alpha", C.c_void_p)]
+
+
+class sgs_surfel_grads(C.Structure):
+    _fields_ = [("mean", C.c_void_p), ("scale", C.c_void_p), ("quat", C.c_void_p), ("opacity", C.c_void_p),
+                ("rgb", C.c_void_p)]
+
+
+class sgs_stats(C.Structure):
+    _fields_ = [("n_visible", C.c_int64), ("n_entries", C.c_int64), ("capacity", C.c_int64), ("overflow", C.c_int64),
+                ("workspace_bytes", C.c_int64)]
+
+
+EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_backward", "sgs_tracking_loss",
+           "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
+           "sgs_upload_target", "sgs_track_iter_host", "sgs_status_string"]
+
+_lib = None
+
+
+def load_library():
+    """dlopen libsgs.so (built by build.py).  Fails loudly when it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError(f"{_LIB_PATH} is missing: run `python -m paper_2506_00970_b200.build` "
+                               "(or __graft_entry__.build()); there is no CPU fallback")
+        lib = C.CDLL(_LIB_PATH)
+        for name in EXPORTS:
+            getattr(lib, name)  # AttributeError if a declared symbol is not exported
+        lib.sgs_status_string.restype = C.c_char_p
+        for name in EXPORTS[:-1]:
+            getattr(lib, name).restype = C.c_int
+        _lib = lib
+    return _lib
+
+
+class SgsError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        super().__init__(f"{where}: {load_library().sgs_status_string(status).decode()} (status {status})")
+
+
+def _check(status, where):
+    if status != SGS_OK:
+        raise SgsError(status, where)
+
+
+def _ptr(t, dtype=torch.float32, device_type="cuda"):
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or t.dtype != dtype or not t.is_contiguous() or t.device.type != device_type:
+        raise TypeError(f"expected a contiguous {dtype} {device_type} tensor")
+    return C.c_void_p(t.data_ptr())
+
+
+def make_camera(width, height, fx, fy, cx, cy, T_cw):
+    cam = sgs_camera()
+    cam.width, cam.height, cam.fx, cam.fy, cam.cx, cam.cy = int(width), int(height), fx, fy, cx, cy
+    T = np.asarray(T_cw, dtype=np.float32)[:3].reshape(12)
+    for i in range(12):
+        cam.T_cw[i] = float(T[i])
+    return cam
+
+
+def _images(rgb=None, depth=None, normal=None, alpha=None, device_type="cuda"):
+    im = sgs_images()
+    im.rgb, im.depth = _ptr(rgb, device_type=device_type), _ptr(depth, device_type=device_type)
+    im.normal, im.alpha = _ptr(normal, device_type=device_type), _ptr(alpha, device_type=device_type)
+    return im
+
+
+def _stream_ptr(stream):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+class Renderer:
+    """One sgs_ctx.  Method names follow the C calls (sgs_render -> render, ...)."""
+
+    def __init__(self, tile=16, cutoff=3.0, alpha_min=1.0 / 255.0, alpha_max=0.99, t_min=1e-4, z_near=0.2,
+                 async_mode=False, device="cuda:0", torch_allocator=True):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2506_00970_b200 needs a CUDA device; there is no CPU fallback")
+        self.lib = load_library()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        torch.cuda.current_stream()  # make sure the primary context exists
+        cfg = sgs_config()
+        _check(self.lib.sgs_default_config(C.byref(cfg)), "sgs_default_config")
+        cfg.tile, cfg.cutoff, cfg.alpha_min, cfg.alpha_max = tile, cutoff, alpha_min, alpha_max
+        cfg.t_min, cfg.z_near, cfg.flags = t_min, z_near, (SGS_FLAG_ASYNC if async_mode else 0)
+        if torch_allocator:
+            dev_index = self.device.index or 0
+
+            def _alloc(nbytes, user, stream):
+                try:
+                    return torch.cuda.caching_allocator_alloc(int(nbytes), dev_index, stream)
+                except Exception:
+                    return None
+
+            def _free(ptr, user, stream):
+                torch.cuda.caching_allocator_delete(ptr)
+
+            self._alloc_cb, self._free_cb = ALLOC_FN(_alloc), FREE_FN(_free)  # keep alive
+            cfg.alloc, cfg.free = self._alloc_cb, self._free_cb
+        self._cfg = cfg
+        self._ctx = C.c_void_p()
+        _check(self.lib.sgs_create(C.byref(self._ctx), C.byref(cfg)), "sgs_create")
+        self._keep = None
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx:
+            self.lib.sgs_destroy(self._ctx)
+            self._ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- device path -------------------------------------------------------------------------
+    @staticmethod
+    def surfels(mean, scale, quat, opacity, rgb, active=None):
+        s = sgs_surfels()
+        s.n = mean.shape[0]
+        s.mean, s.scale, s.quat, s.opacity, s.rgb = _ptr(mean), _ptr(scale), _ptr(quat), _ptr(opacity), _ptr(rgb)
+        s.active = _ptr(active, torch.uint8)
+        return s
+
+    def render(self, surfels, cam, rgb=None, depth=None, normal=None, alpha=None, stream=None):
+        """sgs_render.  `surfels` is a sgs_surfels (see Renderer.surfels); images are preallocated
+        device tensors (any may be None)."""
+        im = _images(rgb, depth, normal, alpha)
+        _check(self.lib.sgs_render(self._ctx, C.byref(surfels), C.byref(cam), C.byref(im), _stream_ptr(stream)), "sgs_render")
+
+    def backward(self, d_rgb=None, d_depth=None, d_normal=None, d_alpha=None, grads=None, d_pose6=None, stream=None):
+        """sgs_backward.  grads: dict of preallocated device tensors mean/scale/quat/opacity/rgb, or None
+        (pose-only).  d_pose6: device tensor of 6 floats or None."""
+        up = _images(d_rgb, d_depth, d_normal, d_alpha)
+        g = None
+        if grads is not None:
+            g = sgs_surfel_grads()
+            g.mean, g.scale, g.quat = _ptr(grads.get("mean")), _ptr(grads.get("scale")), _ptr(grads.get("quat"))
+            g.opacity, g.rgb = _ptr(grads.get("opacity")), _ptr(grads.get("rgb"))
+        _check(self.lib.sgs_backward(self._ctx, C.byref(up), C.byref(g) if g is not None else None, _ptr(d_pose6),
+                                     _stream_ptr(stream)), "sgs_backward")
+
+    def tracking_loss(self, cam, ren, target_rgb, target_depth, lambda_d, normal_sign, up, loss, stream=None):
+        """sgs_tracking_loss.  ren/up: dicts with rgb, depth, normal, alpha device tensors."""
+        r = _images(ren["rgb"], ren["depth"], ren["normal"], ren["alpha"])
+        t = _images(target_rgb, target_depth)
+        u = _images(up["rgb"], up["depth"], up["normal"], up["alpha"])
+        _check(self.lib.sgs_tracking_loss(self._ctx, C.byref(cam), C.byref(r), C.byref(t), C.c_float(lambda_d),
+                                          C.c_float(normal_sign), C.byref(u), _ptr(loss), _stream_ptr(stream)),
+               "sgs_tracking_loss")
+
+    def get_binning(self, n, tiles):
+        """sgs_get_binning -> numpy copies: keys (E,) u64, idx (E,) u32, ranges (tiles,2) u32, culled (n,) u8."""
+        E = C.c_int64()
+        keys, idx, rng, cul = C.c_void_p(), C.c_void_p(), C.c_void_p(), C.c_void_p()
+        _check(self.lib.sgs_get_binning(self._ctx, C.byref(E), C.byref(keys), C.byref(idx), C.byref(rng), C.byref(cul)),
+               "sgs_get_binning")
+        e = int(E.value)
+
+        def fetch(ptr, count, dtype):
+            return _device_to_numpy(ptr.value, count, dtype)
+
+        return dict(E=e, keys=fetch(keys, e, np.uint64), idx=fetch(idx, e, np.uint32),
+                    ranges=fetch(rng, tiles * 2, np.uint32).reshape(tiles, 2), culled=fetch(cul, n, np.uint8))
+
+    def stats(self):
+        st = sgs_stats()
+        _check(self.lib.sgs_get_stats(self._ctx, C.byref(st)), "sgs_get_stats")
+        return {k: int(getattr(st, k)) for k, _ in sgs_stats._fields_}
+
+    # ---- host path (end-to-end) --------------------------------------------------------------
+    def upload_surfels(self, mean, scale, quat, opacity, rgb, active=None, stream=None):
+        """sgs_upload_surfels: HOST (ideally pinned) tensors -> ctx-resident device map."""
+        s = sgs_surfels()
+        s.n = mean.shape[0]
+        hp = lambda t, dt=torch.float32: _ptr(t, dt, "cpu")
+        s.mean, s.scale, s.quat, s.opacity, s.rgb, s.active = hp(mean), hp(scale), hp(quat), hp(opacity), hp(rgb), hp(active, torch.uint8)
+        _check(self.lib.sgs_upload_surfels(self._ctx, C.byref(s), _stream_ptr(stream)), "sgs_upload_surfels")
+
+    def render_host(self, cam, rgb=None, depth=None, normal=None, alpha=None, stream=None):
+        im = _images(rgb, depth, normal, alpha, device_type="cpu")
+        _check(self.lib.sgs_render_host(self._ctx, C.byref(cam), C.byref(im), _stream_ptr(stream)), "sgs_render_host")
+
+    def backward_host(self, d_rgb=None, d_depth=None, d_normal=None, d_alpha=None, grads=None, d_pose6=None, stream=None):
+        up = _images(d_rgb, d_depth, d_normal, d_alpha, device_type="cpu")
+        g = None
+        if grads is not None:
+            g = sgs_surfel_grads()
+            hp = lambda t: _ptr(t, torch.float32, "cpu")
+            g.mean, g.scale, g.quat, g.opacity, g.rgb = (hp(grads.get(k)) for k in ("mean", "scale", "quat", "opacity", "rgb"))
+        _check(self.lib.sgs_backward_host(self._ctx, C.byref(up), C.byref(g) if g is not None else None,
+                                          _ptr(d_pose6, torch.float32, "cpu"), _stream_ptr(stream)), "sgs_backward_host")
+
+    def upload_target(self, cam, rgb, depth, stream=None):
+        _check(self.lib.sgs_upload_target(self._ctx, C.byref(cam), _ptr(rgb, torch.float32, "cpu"),
+                                          _ptr(depth, torch.float32, "cpu"), _stream_ptr(stream)), "sgs_upload_target")
+
+    def track_iter_host(self, cam, lambda_d, normal_sign, stream=None):
+        loss = C.c_float()
+        pose = (C.c_float * 6)()
+        _check(self.lib.sgs_track_iter_host(self._ctx, C.byref(cam), C.c_float(lambda_d), C.c_float(normal_sign),
+                                            C.byref(loss), pose, _stream_ptr(stream)), "sgs_track_iter_host")
+        return float(loss.value), np.array(list(pose), dtype=np.float32)
+
+
+class _RawDeviceBytes:
+    """Wraps a library-owned device pointer for torch through __cuda_array_interface__."""
+
+    def __init__(self, ptr, nbytes):
+        self.__cuda_array_interface__ = {"shape": (int(nbytes),), "typestr": "|u1", "data": (int(ptr), True), "version": 2}
+
+
+def _device_to_numpy(dev_ptr, count, dtype):
+    out = np.empty(count, dtype=dtype)
+    if count:
+        t = torch.as_tensor(_RawDeviceBytes(dev_ptr, out.nbytes), device="cuda")
+        out.view(np.uint8)[:] = t.cpu().numpy()
+    return out

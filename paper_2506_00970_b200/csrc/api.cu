@@ -1,0 +1,182 @@
+// api.cu -- the C ABI of include/sgs.h: ctx, workspace, and the launch sequences.
+#include <math.h>
+#include <new>
+#include <string.h>
+#include "sgs_internal.h"
+
+void* sgs_ws_alloc(sgs_ctx* c, size_t bytes, cudaStream_t s) {
+    if (bytes == 0) bytes = 16;
+    void* p = nullptr;
+    if (c->cfg.alloc) {
+        p = c->cfg.alloc(bytes, c->cfg.user, (void*)s);
+    } else if (cudaMalloc(&p, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        p = nullptr;
+    }
+    if (p) c->bytes += (int64_t)bytes;
+    return p;
+}
+void sgs_ws_free(sgs_ctx* c, void* p, cudaStream_t s) {
+    if (!p) return;
+    if (c->cfg.free) c->cfg.free(p, c->cfg.user, (void*)s);
+    else if (!c->cfg.alloc) cudaFree(p);
+}
+template <typename T>
+static bool ws_realloc(sgs_ctx* c, T*& p, size_t count, cudaStream_t s, bool zero = false) {
+    sgs_ws_free(c, p, s);
+    p = (T*)sgs_ws_alloc(c, count * sizeof(T), s);
+    if (!p) return false;
+    if (zero && cudaMemsetAsync(p, 0, count * sizeof(T), s) != cudaSuccess) return false;
+    return true;
+}
+
+// per-surfel workspace
+int sgs_ensure_surfels(sgs_ctx* c, int64_t n, cudaStream_t s) {
+    if (n <= c->n_cap) return SGS_OK;
+    cudaStreamSynchronize(s);
+    const size_t m = (size_t)(n + n / 8 + 1024);
+    const size_t blocks = (m + SGS_PRE_BLOCK - 1) / SGS_PRE_BLOCK + 1;
+    bool ok = ws_realloc(c, c->scan_state, blocks, s) && ws_realloc(c, c->vis_to_surfel, m, s) &&
+              ws_realloc(c, c->culled, m, s) && ws_realloc(c, c->pay.g0, m, s) && ws_realloc(c, c->pay.g1, m, s) &&
+              ws_realloc(c, c->pay.g2, m, s) && ws_realloc(c, c->pay.g3, m, s) && ws_realloc(c, c->pay.g4, m, s) &&
+              ws_realloc(c, c->pay.g5, m, s) && ws_realloc(c, c->pay.g6, m, s) &&
+              ws_realloc(c, c->acc, m * SGS_ACC_STRIDE, s, true);  // invariant: acc is all-zero between backward calls
+    if (!ok) return SGS_OUT_OF_MEMORY;
+    c->n_cap = (int64_t)m;
+    return SGS_OK;
+}
+
+int sgs_ensure_entries(sgs_ctx* c, int64_t e, cudaStream_t s) {
+    if (e <= c->e_cap) return SGS_OK;
+    cudaStreamSynchronize(s);
+    const size_t m = (size_t)(e + e / 4 + 4096);
+    const size_t st = (m + SGS_SORT_TILE - 1) / SGS_SORT_TILE + 1;
+    bool ok = ws_realloc(c, c->keys[0], m, s) && ws_realloc(c, c->keys[1], m, s) && ws_realloc(c, c->vals[0], m, s) &&
+              ws_realloc(c, c->vals[1], m, s) && ws_realloc(c, c->idx_export, m, s) &&
+              ws_realloc(c, c->sort_state, st * 256 * 8, s);
+    if (!ok) return SGS_OUT_OF_MEMORY;
+    c->e_cap = (int64_t)m;
+    c->sort_tiles_cap = (int64_t)st;
+    return SGS_OK;
+}
+
+int sgs_ensure_image(sgs_ctx* c, int tiles, int64_t pixels, cudaStream_t s) {
+    if (tiles > c->tiles_cap) {
+        cudaStreamSynchronize(s);
+        if (!ws_realloc(c, c->ranges, (size_t)tiles * 2, s)) return SGS_OUT_OF_MEMORY;
+        c->tiles_cap = tiles;
+    }
+    if (pixels > c->pix_cap) {
+        cudaStreamSynchronize(s);
+        if (!(ws_realloc(c, c->T_final, (size_t)pixels, s) && ws_realloc(c, c->n_last, (size_t)pixels, s) &&
+              ws_realloc(c, c->img_scratch, (size_t)pixels * 8, s)))
+            return SGS_OUT_OF_MEMORY;
+        c->pix_cap = pixels;
+    }
+    return SGS_OK;
+}
+
+int sgs_ensure_partials(sgs_ctx* c, int64_t blocks, cudaStream_t s) {
+    static_assert(sizeof(float) == 4, "");
+    if (blocks * 8 <= c->partial_cap) return SGS_OK;
+    cudaStreamSynchronize(s);
+    if (!ws_realloc(c, c->pose_partial, (size_t)blocks * 8 + 64, s)) return SGS_OUT_OF_MEMORY;
+    c->partial_cap = blocks * 8 + 64;
+    return SGS_OK;
+}
+
+void sgs_fill_cam(const sgs_camera* cam, SgsCamDev* d) {
+    d->W = cam->width; d->H = cam->height;
+    d->tiles_x = (cam->width + SGS_TILE - 1) / SGS_TILE;
+    d->tiles_y = (cam->height + SGS_TILE - 1) / SGS_TILE;
+    d->fx = cam->fx; d->fy = cam->fy; d->cx = cam->cx; d->cy = cam->cy;
+    d->Kd[0] = cam->fx; d->Kd[1] = cam->fy; d->Kd[2] = cam->cx; d->Kd[3] = cam->cy;
+    for (int i = 0; i < 3; ++i) {
+        for (int j = 0; j < 3; ++j) { d->R[3 * i + j] = cam->T_cw[4 * i + j]; d->Rf[3 * i + j] = cam->T_cw[4 * i + j]; }
+        d->t[i] = cam->T_cw[4 * i + 3]; d->tf[i] = cam->T_cw[4 * i + 3];
+    }
+}
+
+bool sgs_cam_valid(const sgs_camera* cam) {
+    if (!cam || cam->width <= 0 || cam->height <= 0 || cam->width > 16384 || cam->height > 16384) return false;
+    if (!(cam->fx > 0.f) || !(cam->fy > 0.f) || !isfinite(cam->cx) || !isfinite(cam->cy)) return false;
+    for (int i = 0; i < 12; ++i)
+        if (!isfinite(cam->T_cw[i])) return false;
+    return true;
+}
+
+extern "C" {
+
+int sgs_default_config(sgs_config* cfg) {
+    if (!cfg) return SGS_INVALID_ARGUMENT;
+    memset(cfg, 0, sizeof(*cfg));
+    cfg->tile = SGS_TILE; cfg->cutoff = 3.0f; cfg->alpha_min = 1.0f / 255.0f; cfg->alpha_max = 0.99f;
+    cfg->t_min = 1e-4f; cfg->z_near = 0.2f; cfg->flags = 0;
+    return SGS_OK;
+}
+
+int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
+    if (!out) return SGS_INVALID_ARGUMENT;
+    *out = nullptr;
+    sgs_config def;
+    sgs_default_config(&def);
+    if (!cfg) cfg = &def;
+    if (cfg->tile != SGS_TILE || !(cfg->cutoff > 0.f) || !isfinite(cfg->cutoff) || !(cfg->alpha_min >= 0.f) ||
+        !(cfg->alpha_max > 0.f) || !(cfg->alpha_max < 1.f) || !(cfg->t_min >= 0.f) || !(cfg->z_near > 0.f) ||
+        ((cfg->alloc == nullptr) != (cfg->free == nullptr)))
+        return SGS_INVALID_ARGUMENT;
+    sgs_ctx* c = new (std::nothrow) sgs_ctx;
+    if (!c) return SGS_OUT_OF_MEMORY;
+    memset(c, 0, sizeof(*c));
+    c->cfg = *cfg;
+    c->cfgd.cutoff2 = cfg->cutoff * cfg->cutoff;
+    c->cfgd.alpha_min = cfg->alpha_min; c->cfgd.alpha_max = cfg->alpha_max;
+    c->cfgd.t_min = cfg->t_min; c->cfgd.z_near = cfg->z_near;
+    c->cfgd.cutoff2_d = (double)cfg->cutoff * (double)cfg->cutoff;
+    c->cfgd.z_near_d = (double)cfg->z_near;
+    bool ok = cudaMalloc(&c->counters, sizeof(SgsCounters)) == cudaSuccess &&
+              cudaMallocHost(&c->counters_host, sizeof(SgsCounters)) == cudaSuccess &&
+              cudaMallocHost(&c->pinned_small, 8 * sizeof(float)) == cudaSuccess &&
+              cudaMalloc(&c->sort_hist, sizeof(uint32_t) * (8 * 256 + 8)) == cudaSuccess &&
+              cudaMalloc(&c->loss_dev, sizeof(float) * 8) == cudaSuccess &&
+              cudaEventCreateWithFlags(&c->counters_ready, cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) { cudaGetLastError(); sgs_destroy(c); return SGS_CUDA_ERROR; }
+    c->pose6_dev = c->loss_dev + 1;
+    cudaMemset(c->counters, 0, sizeof(SgsCounters));
+    memset(c->counters_host, 0, sizeof(SgsCounters));
+    *out = c;
+    return SGS_OK;
+}
+
+int sgs_destroy(sgs_ctx* c) {
+    if (!c) return SGS_OK;
+    cudaDeviceSynchronize();
+    cudaStream_t s = 0;
+    void* ptrs[] = {c->scan_state, c->vis_to_surfel, c->culled, c->pay.g0, c->pay.g1, c->pay.g2, c->pay.g3, c->pay.g4,
+                    c->pay.g5, c->pay.g6, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
+                    c->sort_state, c->ranges, c->T_final, c->n_last, c->img_scratch, c->pose_partial, c->resident_store,
+                    c->resident_active, c->target_rgb, c->host_img_dev, c->host_up_dev, c->host_grads_dev};
+    for (void* p : ptrs) sgs_ws_free(c, p, s);
+    if (c->counters) cudaFree(c->counters);
+    if (c->counters_host) cudaFreeHost(c->counters_host);
+    if (c->pinned_small) cudaFreeHost(c->pinned_small);
+    if (c->sort_hist) cudaFree(c->sort_hist);
+    if (c->loss_dev) cudaFree(c->loss_dev);
+    if (c->counters_ready) cudaEventDestroy(c->counters_ready);
+    delete c;
+    return SGS_OK;
+}
+
+const char* sgs_status_string(int status) {
+    switch (status) {
+        case SGS_OK: return "ok";
+        case SGS_INVALID_ARGUMENT: return "invalid argument";
+        case SGS_OUT_OF_MEMORY: return "out of memory";
+        case SGS_WORKSPACE_OVERFLOW: return "workspace overflow: the previous render dropped tile entries; render again";
+        case SGS_NO_FORWARD_STATE: return "no forward state: call sgs_render first";
+        case SGS_CUDA_ERROR: return "CUDA error";
+        default: return "unknown status";
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,146 @@
+// api_host.cu -- HOST-buffer entry points of include/sgs.h (end-to-end path: copies in, runs the
+// device path, copies out, waits).  No arithmetic here.
+#include <string.h>
+#include "sgs_internal.h"
+
+template <typename T>
+static bool grow(sgs_ctx* c, T*& p, int64_t& cap, int64_t need, cudaStream_t s) {
+    if (need <= cap) return true;
+    cudaStreamSynchronize(s);
+    sgs_ws_free(c, p, s);
+    p = (T*)sgs_ws_alloc(c, (size_t)need * sizeof(T), s);
+    cap = p ? need : 0;
+    return p != nullptr;
+}
+
+static int ensure_host_images(sgs_ctx* c, int64_t pixels, cudaStream_t s) {
+    int64_t cap2 = c->host_img_cap;
+    if (!grow(c, c->host_img_dev, c->host_img_cap, pixels * 8, s)) return SGS_OUT_OF_MEMORY;
+    if (!grow(c, c->host_up_dev, cap2, pixels * 8, s)) return SGS_OUT_OF_MEMORY;
+    return SGS_OK;
+}
+
+static void dev_images(float* base, int64_t pixels, sgs_images* im) {
+    im->rgb = base; im->depth = base + 3 * pixels; im->normal = base + 4 * pixels; im->alpha = base + 7 * pixels;
+}
+
+extern "C" {
+
+int sgs_upload_surfels(sgs_ctx* c, const sgs_surfels* h, void* stream) {
+    if (!c || !h || h->n < 0 || (h->n > 0 && (!h->mean || !h->scale || !h->quat || !h->opacity || !h->rgb)))
+        return SGS_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int64_t n = h->n;
+    if (n > c->resident_cap) {
+        cudaStreamSynchronize(s);
+        sgs_ws_free(c, c->resident_store, s);
+        sgs_ws_free(c, c->resident_active, s);
+        c->resident_store = (float*)sgs_ws_alloc(c, (size_t)n * 13 * sizeof(float), s);
+        c->resident_active = (uint8_t*)sgs_ws_alloc(c, (size_t)n, s);
+        if (!c->resident_store || !c->resident_active) { c->resident_cap = 0; return SGS_OUT_OF_MEMORY; }
+        c->resident_cap = n;
+    }
+    float* b = c->resident_store;
+    float* d_mean = b; float* d_scale = b + 3 * n; float* d_quat = b + 5 * n; float* d_op = b + 9 * n; float* d_rgb = b + 10 * n;
+    bool ok = cudaMemcpyAsync(d_mean, h->mean, sizeof(float) * 3 * n, cudaMemcpyHostToDevice, s) == cudaSuccess &&
+              cudaMemcpyAsync(d_scale, h->scale, sizeof(float) * 2 * n, cudaMemcpyHostToDevice, s) == cudaSuccess &&
+              cudaMemcpyAsync(d_quat, h->quat, sizeof(float) * 4 * n, cudaMemcpyHostToDevice, s) == cudaSuccess &&
+              cudaMemcpyAsync(d_op, h->opacity, sizeof(float) * n, cudaMemcpyHostToDevice, s) == cudaSuccess &&
+              cudaMemcpyAsync(d_rgb, h->rgb, sizeof(float) * 3 * n, cudaMemcpyHostToDevice, s) == cudaSuccess;
+    if (ok && h->active) ok = cudaMemcpyAsync(c->resident_active, h->active, (size_t)n, cudaMemcpyHostToDevice, s) == cudaSuccess;
+    if (!ok) return SGS_CUDA_ERROR;
+    c->resident.n = n; c->resident.mean = d_mean; c->resident.scale = d_scale; c->resident.quat = d_quat;
+    c->resident.opacity = d_op; c->resident.rgb = d_rgb; c->resident.active = h->active ? c->resident_active : nullptr;
+    return SGS_OK;
+}
+
+int sgs_render_host(sgs_ctx* c, const sgs_camera* cam, const sgs_images* ho, void* stream) {
+    if (!c || !sgs_cam_valid(cam) || !ho) return SGS_INVALID_ARGUMENT;
+    if (!c->resident.mean && c->resident.n != 0) return SGS_NO_FORWARD_STATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int64_t px = (int64_t)cam->width * cam->height;
+    int r = ensure_host_images(c, px, s);
+    if (r != SGS_OK) return r;
+    sgs_images d;
+    dev_images(c->host_img_dev, px, &d);
+    if ((r = sgs_render(c, &c->resident, cam, &d, stream)) != SGS_OK) return r;
+    bool ok = true;
+    if (ho->rgb) ok = ok && cudaMemcpyAsync(ho->rgb, d.rgb, sizeof(float) * 3 * px, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+    if (ho->depth) ok = ok && cudaMemcpyAsync(ho->depth, d.depth, sizeof(float) * px, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+    if (ho->normal) ok = ok && cudaMemcpyAsync(ho->normal, d.normal, sizeof(float) * 3 * px, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+    if (ho->alpha) ok = ok && cudaMemcpyAsync(ho->alpha, d.alpha, sizeof(float) * px, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+    if (!ok || cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
+    return SGS_OK;
+}
+
+int sgs_backward_host(sgs_ctx* c, const sgs_images* hu, const sgs_surfel_grads* hg, float* h_pose6, void* stream) {
+    if (!c || !hu) return SGS_INVALID_ARGUMENT;
+    if (!c->have_forward) return SGS_NO_FORWARD_STATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int64_t px = (int64_t)c->camd.W * c->camd.H, n = c->last_surfels.n;
+    int r = ensure_host_images(c, px, s);
+    if (r != SGS_OK) return r;
+    sgs_images d;
+    dev_images(c->host_up_dev, px, &d);
+    sgs_images du = {nullptr, nullptr, nullptr, nullptr};
+    bool ok = true;
+    if (hu->rgb) { ok = ok && cudaMemcpyAsync(d.rgb, hu->rgb, sizeof(float) * 3 * px, cudaMemcpyHostToDevice, s) == cudaSuccess; du.rgb = d.rgb; }
+    if (hu->depth) { ok = ok && cudaMemcpyAsync(d.depth, hu->depth, sizeof(float) * px, cudaMemcpyHostToDevice, s) == cudaSuccess; du.depth = d.depth; }
+    if (hu->normal) { ok = ok && cudaMemcpyAsync(d.normal, hu->normal, sizeof(float) * 3 * px, cudaMemcpyHostToDevice, s) == cudaSuccess; du.normal = d.normal; }
+    if (hu->alpha) { ok = ok && cudaMemcpyAsync(d.alpha, hu->alpha, sizeof(float) * px, cudaMemcpyHostToDevice, s) == cudaSuccess; du.alpha = d.alpha; }
+    if (!ok) return SGS_CUDA_ERROR;
+    sgs_surfel_grads dg;
+    if (hg) {
+        if (!grow(c, c->host_grads_dev, c->host_grads_cap, n * 13 + 16, s)) return SGS_OUT_OF_MEMORY;
+        float* b = c->host_grads_dev;
+        dg.mean = b; dg.scale = b + 3 * n; dg.quat = b + 5 * n; dg.opacity = b + 9 * n; dg.rgb = b + 10 * n;
+    }
+    if ((r = sgs_backward(c, &du, hg ? &dg : nullptr, h_pose6 ? c->pose6_dev : nullptr, stream)) != SGS_OK) return r;
+    if (hg) {
+        if (hg->mean) ok = ok && cudaMemcpyAsync(hg->mean, dg.mean, sizeof(float) * 3 * n, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+        if (hg->scale) ok = ok && cudaMemcpyAsync(hg->scale, dg.scale, sizeof(float) * 2 * n, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+        if (hg->quat) ok = ok && cudaMemcpyAsync(hg->quat, dg.quat, sizeof(float) * 4 * n, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+        if (hg->opacity) ok = ok && cudaMemcpyAsync(hg->opacity, dg.opacity, sizeof(float) * n, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+        if (hg->rgb) ok = ok && cudaMemcpyAsync(hg->rgb, dg.rgb, sizeof(float) * 3 * n, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+    }
+    if (h_pose6) ok = ok && cudaMemcpyAsync(c->pinned_small, c->pose6_dev, sizeof(float) * 6, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+    if (!ok || cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
+    if (h_pose6) memcpy(h_pose6, c->pinned_small, sizeof(float) * 6);
+    return SGS_OK;
+}
+
+int sgs_upload_target(sgs_ctx* c, const sgs_camera* cam, const float* h_rgb, const float* h_depth, void* stream) {
+    if (!c || !sgs_cam_valid(cam) || !h_rgb || !h_depth) return SGS_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int64_t px = (int64_t)cam->width * cam->height;
+    if (!grow(c, c->target_rgb, c->target_cap, px * 4, s)) return SGS_OUT_OF_MEMORY;
+    c->target_depth = c->target_rgb + 3 * px;
+    if (cudaMemcpyAsync(c->target_rgb, h_rgb, sizeof(float) * 3 * px, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+        cudaMemcpyAsync(c->target_depth, h_depth, sizeof(float) * px, cudaMemcpyHostToDevice, s) != cudaSuccess)
+        return SGS_CUDA_ERROR;
+    return SGS_OK;
+}
+
+int sgs_track_iter_host(sgs_ctx* c, const sgs_camera* cam, float lambda_d, float normal_sign, float* h_loss,
+                        float* h_pose6, void* stream) {
+    if (!c || !sgs_cam_valid(cam)) return SGS_INVALID_ARGUMENT;
+    const int64_t px = (int64_t)cam->width * cam->height;
+    if (!c->target_rgb || c->target_cap < px * 4 || (!c->resident.mean && c->resident.n != 0)) return SGS_NO_FORWARD_STATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    int r = ensure_host_images(c, px, s);
+    if (r != SGS_OK) return r;
+    sgs_images ren, up, tgt = {c->target_rgb, c->target_depth, nullptr, nullptr};
+    dev_images(c->host_img_dev, px, &ren);
+    dev_images(c->host_up_dev, px, &up);
+    if ((r = sgs_render(c, &c->resident, cam, &ren, stream)) != SGS_OK) return r;
+    if ((r = sgs_tracking_loss(c, cam, &ren, &tgt, lambda_d, normal_sign, &up, c->loss_dev, stream)) != SGS_OK) return r;
+    if ((r = sgs_backward(c, &up, nullptr, c->pose6_dev, stream)) != SGS_OK) return r;
+    if (cudaMemcpyAsync(c->pinned_small, c->loss_dev, sizeof(float) * 7, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        cudaStreamSynchronize(s) != cudaSuccess)
+        return SGS_CUDA_ERROR;
+    if (h_loss) *h_loss = c->pinned_small[0];
+    if (h_pose6) memcpy(h_pose6, c->pinned_small + 1, sizeof(float) * 6);
+    return SGS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,153 @@
+// api_run.cu -- sgs_render / sgs_backward / sgs_tracking_loss / debug export (include/sgs.h).
+#include <string.h>
+#include "sgs_internal.h"
+
+// async mode: examine the counters of the previous render (already copied to pinned memory)
+static int check_pending(sgs_ctx* c, cudaStream_t s) {
+    if (!c->pending_check) return SGS_OK;
+    if (cudaEventSynchronize(c->counters_ready) != cudaSuccess) return SGS_CUDA_ERROR;
+    c->pending_check = false;
+    const int64_t E = (int64_t)c->counters_host->n_entries;
+    c->last_entries = E;
+    if (c->counters_host->overflow) {
+        c->have_forward = false;
+        const int r = sgs_ensure_entries(c, E, s);
+        return r != SGS_OK ? r : SGS_WORKSPACE_OVERFLOW;
+    }
+    return SGS_OK;
+}
+
+extern "C" {
+
+int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* out, void* stream) {
+    if (!c || !sf || !sgs_cam_valid(cam) || sf->n < 0 || sf->n >= (1ll << 24)) return SGS_INVALID_ARGUMENT;
+    if (sf->n > 0 && (!sf->mean || !sf->scale || !sf->quat || !sf->opacity || !sf->rgb)) return SGS_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int r = check_pending(c, s);
+    if (r != SGS_OK) return r;
+    c->have_forward = false;
+    sgs_fill_cam(cam, &c->camd);
+    const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    const int64_t pixels = (int64_t)cam->width * cam->height;
+    if ((r = sgs_ensure_surfels(c, sf->n, s)) != SGS_OK) return r;
+    if ((r = sgs_ensure_image(c, tiles, pixels, s)) != SGS_OK) return r;
+    if (c->e_cap == 0) {
+        int64_t guess = 2 * sf->n;
+        if (guess < (1 << 20)) guess = 1 << 20;
+        if ((r = sgs_ensure_entries(c, guess, s)) != SGS_OK) return r;
+    }
+    const bool async = (c->cfg.flags & SGS_FLAG_ASYNC) != 0;
+    c->launch_entries = c->e_cap;
+    if (async && c->last_entries > 0) {
+        const int64_t hint = c->last_entries + c->last_entries / 4 + 4096;
+        if (hint < c->launch_entries) c->launch_entries = hint;
+    }
+    c->last_surfels = *sf;
+    c->last_cam = *cam;
+    if (sgs_launch_preprocess(c, sf, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    if (cudaMemcpyAsync(c->counters_host, c->counters, sizeof(SgsCounters), cudaMemcpyDeviceToHost, s) != cudaSuccess)
+        return SGS_CUDA_ERROR;
+    if (!async) {
+        if (cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
+        const int64_t E = (int64_t)c->counters_host->n_entries;
+        c->last_entries = E;
+        if (E > c->e_cap) {  // grow and emit again
+            if ((r = sgs_ensure_entries(c, E, s)) != SGS_OK) return r;
+            c->launch_entries = c->e_cap;
+            if (sgs_launch_preprocess(c, sf, s) != cudaSuccess) return SGS_CUDA_ERROR;
+            if (cudaMemcpyAsync(c->counters_host, c->counters, sizeof(SgsCounters), cudaMemcpyDeviceToHost, s) !=
+                    cudaSuccess ||
+                cudaStreamSynchronize(s) != cudaSuccess)
+                return SGS_CUDA_ERROR;
+        }
+        c->launch_entries = E;  // exact grids
+    } else {
+        cudaEventRecord(c->counters_ready, s);
+        c->pending_check = true;
+    }
+    if (sgs_launch_sort_and_ranges(c, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    float* planes[8];
+    for (int i = 0; i < 8; ++i) planes[i] = c->img_scratch + (size_t)i * pixels;
+    if (out) {
+        if (out->rgb) for (int i = 0; i < 3; ++i) planes[i] = out->rgb + (size_t)i * pixels;
+        if (out->depth) planes[3] = out->depth;
+        if (out->normal) for (int i = 0; i < 3; ++i) planes[4 + i] = out->normal + (size_t)i * pixels;
+        if (out->alpha) planes[7] = out->alpha;
+    }
+    for (int i = 0; i < 8; ++i) c->last_img[i] = planes[i];
+    if (sgs_launch_forward(c, planes, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    c->have_forward = true;
+    return SGS_OK;
+}
+
+int sgs_backward(sgs_ctx* c, const sgs_images* upstream, const sgs_surfel_grads* dg, float* d_pose6, void* stream) {
+    if (!c) return SGS_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int r = check_pending(c, s);
+    if (r != SGS_OK) return r;
+    if (!c->have_forward) return SGS_NO_FORWARD_STATE;
+    const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    const int64_t pixels = (int64_t)c->camd.W * c->camd.H;
+    int64_t blocks = (c->last_surfels.n + 255) / 256;
+    if (blocks < tiles) blocks = tiles;
+    if ((r = sgs_ensure_partials(c, blocks, s)) != SGS_OK) return r;
+    const float* up[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    if (upstream) {
+        if (upstream->rgb) for (int i = 0; i < 3; ++i) up[i] = upstream->rgb + (size_t)i * pixels;
+        if (upstream->depth) up[3] = upstream->depth;
+        if (upstream->normal) for (int i = 0; i < 3; ++i) up[4 + i] = upstream->normal + (size_t)i * pixels;
+        if (upstream->alpha) up[7] = upstream->alpha;
+    }
+    if (sgs_launch_backward(c, up, dg, d_pose6, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    return SGS_OK;
+}
+
+int sgs_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const sgs_images* ren, const sgs_images* target, float lambda_d,
+                      float normal_sign, const sgs_images* upstream, float* loss, void* stream) {
+    if (!c || !sgs_cam_valid(cam) || !ren || !target || !upstream) return SGS_INVALID_ARGUMENT;
+    if (!ren->rgb || !ren->depth || !ren->normal || !ren->alpha || !target->rgb || !target->depth)
+        return SGS_INVALID_ARGUMENT;
+    const int64_t pixels = (int64_t)cam->width * cam->height;
+    const float* rp[8];
+    float* upp[8];
+    for (int i = 0; i < 3; ++i) {
+        rp[i] = ren->rgb + (size_t)i * pixels;
+        rp[4 + i] = ren->normal + (size_t)i * pixels;
+        upp[i] = upstream->rgb ? upstream->rgb + (size_t)i * pixels : nullptr;
+        upp[4 + i] = upstream->normal ? upstream->normal + (size_t)i * pixels : nullptr;
+    }
+    rp[3] = ren->depth; rp[7] = ren->alpha; upp[3] = upstream->depth; upp[7] = upstream->alpha;
+    if (sgs_launch_tracking_loss(c, cam, rp, target->rgb, target->depth, lambda_d, normal_sign, upp, loss,
+                                 (cudaStream_t)stream) != cudaSuccess)
+        return SGS_CUDA_ERROR;
+    return SGS_OK;
+}
+
+int sgs_get_binning(sgs_ctx* c, int64_t* n_entries, const uint64_t** keys, const uint32_t** idx,
+                    const uint32_t** tile_ranges, const uint8_t** culled) {
+    if (!c) return SGS_INVALID_ARGUMENT;
+    int r = check_pending(c, 0);
+    if (r != SGS_OK) return r;
+    if (!c->have_forward) return SGS_NO_FORWARD_STATE;
+    if (cudaDeviceSynchronize() != cudaSuccess) return SGS_CUDA_ERROR;
+    if (sgs_launch_export_idx(c, 0) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) return SGS_CUDA_ERROR;
+    if (n_entries) *n_entries = (int64_t)c->counters_host->n_entries;
+    if (keys) *keys = c->keys[c->sorted_buf];
+    if (idx) *idx = c->idx_export;
+    if (tile_ranges) *tile_ranges = c->ranges;
+    if (culled) *culled = c->culled;
+    return SGS_OK;
+}
+
+int sgs_get_stats(sgs_ctx* c, sgs_stats* out) {
+    if (!c || !out) return SGS_INVALID_ARGUMENT;
+    if (c->pending_check && cudaEventSynchronize(c->counters_ready) != cudaSuccess) return SGS_CUDA_ERROR;
+    out->n_visible = c->counters_host->n_visible;
+    out->n_entries = (int64_t)c->counters_host->n_entries;
+    out->capacity = c->e_cap;
+    out->overflow = c->counters_host->overflow;
+    out->workspace_bytes = c->bytes;
+    return SGS_OK;
+}
+
+}  // extern "C"

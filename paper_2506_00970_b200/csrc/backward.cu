@@ -1,0 +1,380 @@
+// backward.cu -- K-bwd, K-sbwd and the pose reductions.
+//
+// K-bwd walks each tile's list in REVERSE from the last composited entry of each pixel, recomputes
+// the pair with the forward's exact instruction sequence (pair.cuh), recovers T_i = T_{i+1}/(1-a_i)
+// and keeps one scalar suffix  sum_{j>i} w_j (g.v_j)  so that
+//     dL/da_i = T_i (g.v_i) - suffix / (1 - a_i)                       (derivative of Eq. 8).
+// The geometric chain is taken in camera space as a "force" on the splat's plane:
+// the constraint  mu_c + a_u u + a_v v = z r  (Eq. 1, 3-4; r = pixel ray, a_u = s_u t_uc) gives
+//     f = [ r x (a_v g_u - a_u g_v) + (a_u x a_v) g_z ] / (r . (a_u x a_v))
+//     dL/dmu_c = sum f,  dL/d(s_u t_uc) = sum u f,  dL/d(s_v t_vc) = sum v f
+// which IS the matrix dL/dH_c of Eq. 9 (= W^T dL/dT) accumulated directly.
+//   full mode     : 16 values per (warp, surfel) are reduced with a transposed butterfly (16 shuffles
+//                   instead of 80) and land as ONE 64-byte red.global.add per warp.
+//   pose-only mode: Eq. 11-13 applied per pixel: dL/drho = sum f, dL/dtheta = r x sum z f + N x g_N;
+//                   no per-surfel traffic at all -- registers -> block -> grid reduction to 6 values.
+#include "pair.cuh"
+#include "sgs_internal.h"
+
+namespace {
+
+struct CPlanes { const float* p[8]; };
+
+struct StagedBwd {
+    float4 s0, s1, s2, s3, s4;  // as StagedFwd
+    float4 s5;                  // a_u.xyz, a_v.x
+    float4 s6;                  // a_v.yz, m.xy      (m = a_u x a_v)
+    float4 s7;                  // m.z, bits(v), -, -
+};
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Transposed butterfly: 16 per-lane values -> lane l ends with the warp-wide sum of value (l>>1)&15.
+__device__ __forceinline__ float reduce16_transposed(float (&x)[16], int lane) {
+    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4, b1 = lane & 2;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float send = b4 ? x[i] : x[i + 8], keep = b4 ? x[i + 8] : x[i];
+        x[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float send = b3 ? x[i] : x[i + 4], keep = b3 ? x[i + 4] : x[i];
+        x[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const float send = b2 ? x[i] : x[i + 2], keep = b2 ? x[i + 2] : x[i];
+        x[i] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    }
+    {
+        const float send = b1 ? x[0] : x[1], keep = b1 ? x[1] : x[0];
+        x[0] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+    }
+    return x[0] + __shfl_xor_sync(0xffffffffu, x[0], 1);
+}
+
+// Grid reduction: every block has written 6 partial sums at partial[block*8 ..]; the block that
+// draws the last ticket adds them all in fp64 and writes the pose gradient (block-then-grid).
+__device__ __forceinline__ void finish_pose(const float* __restrict__ partial, unsigned int n_blocks,
+                                            SgsCounters* __restrict__ counters, float* __restrict__ d_pose6) {
+    __shared__ bool s_is_last;
+    __shared__ double s_sum[8][6];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        const unsigned int t = atomicAdd(&counters->ticket_bwd, 1u);
+        s_is_last = (t == n_blocks - 1);
+    }
+    __syncthreads();
+    if (!s_is_last) return;
+    __threadfence();
+    double a[6] = {0, 0, 0, 0, 0, 0};
+    for (unsigned int b = tid; b < n_blocks; b += blockDim.x) {
+        const float4 lo = __ldcg(reinterpret_cast<const float4*>(partial + (size_t)b * 8));
+        const float4 hi = __ldcg(reinterpret_cast<const float4*>(partial + (size_t)b * 8 + 4));
+        a[0] += lo.x; a[1] += lo.y; a[2] += lo.z; a[3] += lo.w; a[4] += hi.x; a[5] += hi.y;
+    }
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        double v = a[c];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) s_sum[wid][c] = v;
+    }
+    __syncthreads();
+    if (tid < 6) {
+        double v = 0;
+        for (int w2 = 0; w2 < (int)(blockDim.x >> 5); ++w2) v += s_sum[w2][tid];
+        d_pose6[tid] = (float)v;
+    }
+    if (tid == 0) counters->ticket_bwd = 0;  // self-cleaning: backward may run again on the same render
+}
+
+template <bool POSE_ONLY>
+__global__ void __launch_bounds__(SGS_BLOCK)
+k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, SgsPayload pay, int W, int H,
+           int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg, CPlanes up,
+           const float* __restrict__ T_final, const uint32_t* __restrict__ n_last, float* __restrict__ acc,
+           float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6) {
+    __shared__ StagedBwd sh[SGS_BLOCK];
+    __shared__ float s_red[8][6];
+    const int tile = blockIdx.x;
+    const int tx = tile % tiles_x, ty = tile / tiles_x;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int lxi = (wid & 1) * 8 + (lane & 7), lyi = (wid >> 1) * 4 + (lane >> 3);
+    const int px = tx * SGS_TILE + lxi, py = ty * SGS_TILE + lyi;
+    const bool inside = px < W && py < H;
+    const float lx = (float)lxi, ly = (float)lyi;
+    const double px0 = (double)(tx * SGS_TILE) + 0.5, py0 = (double)(ty * SGS_TILE) + 0.5;
+    const uint32_t start = ranges[2 * tile];
+
+    float g[8];
+    float T_after = 1.f;
+    uint32_t last = 0;
+    if (inside) {
+        const size_t pix = (size_t)py * W + px;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) g[c] = up.p[c] ? up.p[c][pix] : 0.f;
+        T_after = T_final[pix];
+        last = n_last[pix];
+    } else {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) g[c] = 0.f;
+    }
+    const float rx = ((float)px + 0.5f - cx) / fx, ry = ((float)py + 0.5f - cy) / fy;  // pixel ray (rx, ry, 1)
+    float suffix = 0.f;
+    float F0 = 0.f, F1 = 0.f, F2 = 0.f, Z0 = 0.f, Z1 = 0.f, Z2 = 0.f, Nn0 = 0.f, Nn1 = 0.f, Nn2 = 0.f;
+
+    // block-wide maximum of `last` decides how many batches exist
+    uint32_t wmax = last;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
+    __shared__ uint32_t s_wmax[8];
+    if (lane == 0) s_wmax[wid] = wmax;
+    __syncthreads();
+    uint32_t bmax = 0;
+#pragma unroll
+    for (int w2 = 0; w2 < 8; ++w2) bmax = max(bmax, s_wmax[w2]);
+
+    const int n_batches = (int)((bmax + SGS_BLOCK - 1) / SGS_BLOCK);
+    for (int b = n_batches - 1; b >= 0; --b) {
+        const uint32_t boff = (uint32_t)b * SGS_BLOCK;
+        const uint32_t nb = min((uint32_t)SGS_BLOCK, bmax - boff);
+        __syncthreads();  // previous batch fully consumed
+        if ((uint32_t)tid < nb) {
+            const uint32_t v = vals[start + boff + tid];
+            const float4 g0 = pay.g0[v], g1 = pay.g1[v], g3 = pay.g3[v], g4 = pay.g4[v], g5 = pay.g5[v], g6 = pay.g6[v];
+            const double2 g2 = pay.g2[v];
+            StagedBwd st;
+            stage_entry(g0, g1, g2, g3, px0, py0, st.s0, st.s1, st.s2);
+            st.s3 = make_float4(g1.w, g3.w, g4.x, g4.y);
+            st.s4 = make_float4(g4.z, g4.w, g5.x, 0.f);
+            const float aux = g5.y, auy = g5.z, auz = g5.w, avx = g6.x, avy = g6.y, avz = g6.z;
+            st.s5 = make_float4(aux, auy, auz, avx);
+            st.s6 = make_float4(avy, avz, auy * avz - auz * avy, auz * avx - aux * avz);
+            st.s7 = make_float4(aux * avy - auy * avx, __uint_as_float(v), 0.f, 0.f);
+            sh[tid] = st;
+        }
+        __syncthreads();
+        // entries at or after the warp's largest `last` were composited by none of its pixels
+        int jstart = (int)min(nb, wmax > boff ? wmax - boff : 0u) - 1;
+        for (int j = jstart; j >= 0; --j) {
+            const float4 s0 = sh[j].s0, s1 = sh[j].s1, s2 = sh[j].s2, s3 = sh[j].s3;
+            PairResult r;
+            bool hit = (boff + (uint32_t)j) < last;
+            if (hit) hit = eval_pair(s0, s1, s2, s3.x, lx, ly, cfg.cutoff2, cfg.alpha_min, cfg.alpha_max, cfg.z_near, r);
+            if (!__any_sync(0xffffffffu, hit)) continue;
+            float x[16];
+#pragma unroll
+            for (int c = 0; c < 16; ++c) x[c] = 0.f;
+            if (hit) {
+                const float4 s4 = sh[j].s4, s5 = sh[j].s5, s6 = sh[j].s6, s7 = sh[j].s7;
+                const float inv1ma = fast_rcp(1.f - r.a);
+                const float Ti = T_after * inv1ma;  // transmittance in front of this splat
+                const float w = r.a * Ti;
+                const float gv = g[0] * s3.y + g[1] * s3.z + g[2] * s3.w + g[3] * r.z + g[4] * s4.x + g[5] * s4.y +
+                                 g[6] * s4.z + g[7];
+                const float da = Ti * gv - suffix * inv1ma;
+                suffix = fmaf(w, gv, suffix);
+                T_after = Ti;
+                const bool clamped = s3.x * r.G > cfg.alpha_max;  // R5: true derivative, zero when clamped
+                const float dG = clamped ? 0.f : da * s3.x;
+                const float gu = -r.u * r.G * dG, gvv = -r.v * r.G * dG, gz = g[3] * w;
+                // f = [ r x (a_v gu - a_u gv) + m gz ] / (r . m)
+                const float q0 = s5.w * gu - s5.x * gvv, q1 = s6.x * gu - s5.y * gvv, q2 = s6.y * gu - s5.z * gvv;
+                const float m0 = s6.z, m1 = s6.w, m2 = s7.x;
+                const float inv_rm = fast_rcp(rx * m0 + ry * m1 + m2);
+                const float f0 = (ry * q2 - q1 + m0 * gz) * inv_rm;
+                const float f1 = (q0 - rx * q2 + m1 * gz) * inv_rm;
+                const float f2 = (rx * q1 - ry * q0 + m2 * gz) * inv_rm;
+                if (POSE_ONLY) {
+                    F0 += f0; F1 += f1; F2 += f2;
+                    Z0 = fmaf(r.z, f0, Z0); Z1 = fmaf(r.z, f1, Z1); Z2 = fmaf(r.z, f2, Z2);
+                    Nn0 = fmaf(w, s4.x, Nn0); Nn1 = fmaf(w, s4.y, Nn1); Nn2 = fmaf(w, s4.z, Nn2);
+                } else {
+                    x[0] = f0; x[1] = f1; x[2] = f2;
+                    x[3] = r.u * f0; x[4] = r.u * f1; x[5] = r.u * f2;
+                    x[6] = r.v * f0; x[7] = r.v * f1; x[8] = r.v * f2;
+                    x[9] = w * g[4]; x[10] = w * g[5]; x[11] = w * g[6];
+                    x[12] = w * g[0]; x[13] = w * g[1]; x[14] = w * g[2];
+                    x[15] = clamped ? 0.f : da * r.G;
+                }
+            }
+            if (!POSE_ONLY) {
+                const float red = reduce16_transposed(x, lane);
+                if ((lane & 1) == 0) {
+                    const uint32_t v = __float_as_uint(sh[j].s7.y);
+                    atomicAdd(acc + (size_t)v * SGS_ACC_STRIDE + (lane >> 1), red);
+                }
+            }
+        }
+    }
+    if (POSE_ONLY) {
+        // Eq. 11-13 per pixel: rho += sum f; theta += X x f summed = r x sum(z f), plus t_nc x dL/dt_nc = N x g_N
+        float p6[6];
+        p6[0] = F0; p6[1] = F1; p6[2] = F2;
+        p6[3] = (ry * Z2 - Z1) + (Nn1 * g[6] - Nn2 * g[5]);
+        p6[4] = (Z0 - rx * Z2) + (Nn2 * g[4] - Nn0 * g[6]);
+        p6[5] = (rx * Z1 - ry * Z0) + (Nn0 * g[5] - Nn1 * g[4]);
+#pragma unroll
+        for (int c = 0; c < 6; ++c) {
+            const float s = warp_sum(inside ? p6[c] : 0.f);
+            if (lane == 0) s_red[wid][c] = s;
+        }
+        __syncthreads();
+        if (tid < 6) {
+            float s = 0.f;
+#pragma unroll
+            for (int w2 = 0; w2 < 8; ++w2) s += s_red[w2][tid];
+            pose_partial[(size_t)tile * 8 + tid] = s;
+        }
+        finish_pose(pose_partial, gridDim.x, counters, d_pose6);
+    }
+}
+
+
+// K-sbwd: one thread per VISIBLE surfel.  Eq. 9-10 (with R11, R13): the accumulator already holds
+// dL/dH_c = [dL/d(s_u t_uc), dL/d(s_v t_vc), dL/dmu_c] and dL/dt_nc; this applies the product rule
+// to (s, t), rotates to world space, goes through R(q/|q|), and forms the surfel's share of the
+// pose gradient (Eq. 11-13).  Leaves acc[v] zeroed for the next backward.
+__global__ void __launch_bounds__(256)
+k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __restrict__ vis_to_surfel,
+                  float* __restrict__ acc, const float* __restrict__ mean, const float* __restrict__ scale,
+                  const float* __restrict__ quat, SgsCamDev cam, sgs_surfel_grads out,
+                  float* __restrict__ pose_partial, SgsCounters* __restrict__ counters_rw,
+                  float* __restrict__ d_pose6) {
+    __shared__ float s_red[8][6];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const unsigned int nv = counters->n_visible;
+    const unsigned int v = blockIdx.x * blockDim.x + tid;
+    float p6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (v < nv) {
+        const uint32_t i = vis_to_surfel[v];
+        float a[16];
+        float4* ap = reinterpret_cast<float4*>(acc + (size_t)v * SGS_ACC_STRIDE);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const float4 t = ap[c];
+            a[4 * c] = t.x; a[4 * c + 1] = t.y; a[4 * c + 2] = t.z; a[4 * c + 3] = t.w;
+            ap[c] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        const float qw0 = quat[4 * i], qx0 = quat[4 * i + 1], qy0 = quat[4 * i + 2], qz0 = quat[4 * i + 3];
+        const float qn = sqrtf(qw0 * qw0 + qx0 * qx0 + qy0 * qy0 + qz0 * qz0);
+        const float qi = 1.f / qn;
+        const float qw = qw0 * qi, qx = qx0 * qi, qy = qy0 * qi, qz = qz0 * qi;
+        const float tu[3] = {1.f - 2.f * (qy * qy + qz * qz), 2.f * (qx * qy + qw * qz), 2.f * (qx * qz - qw * qy)};
+        const float tv[3] = {2.f * (qx * qy - qw * qz), 1.f - 2.f * (qx * qx + qz * qz), 2.f * (qy * qz + qw * qx)};
+        const float tn[3] = {2.f * (qx * qz + qw * qy), 2.f * (qy * qz - qw * qx), 1.f - 2.f * (qx * qx + qy * qy)};
+        const float su = scale[2 * i], sv = scale[2 * i + 1];
+        const float m[3] = {mean[3 * i], mean[3 * i + 1], mean[3 * i + 2]};
+        float tuc[3], tvc[3], tnc[3], muc[3];
+#pragma unroll
+        for (int r = 0; r < 3; ++r) {
+            const float r0 = cam.Rf[3 * r], r1 = cam.Rf[3 * r + 1], r2 = cam.Rf[3 * r + 2];
+            tuc[r] = r0 * tu[0] + r1 * tu[1] + r2 * tu[2];
+            tvc[r] = r0 * tv[0] + r1 * tv[1] + r2 * tv[2];
+            tnc[r] = r0 * tn[0] + r1 * tn[1] + r2 * tn[2];
+            muc[r] = r0 * m[0] + r1 * m[1] + r2 * m[2] + cam.tf[r];
+        }
+        const float* dmu = a;        // dL/dmu_c
+        const float* dau = a + 3;    // dL/d(s_u t_uc)
+        const float* dav = a + 6;    // dL/d(s_v t_vc)
+        const float* dtn = a + 9;    // dL/dt_nc
+        float dtu[3], dtv[3];
+#pragma unroll
+        for (int r = 0; r < 3; ++r) { dtu[r] = su * dau[r]; dtv[r] = sv * dav[r]; }
+        if (out.scale) {
+            out.scale[2 * i] = tuc[0] * dau[0] + tuc[1] * dau[1] + tuc[2] * dau[2];
+            out.scale[2 * i + 1] = tvc[0] * dav[0] + tvc[1] * dav[1] + tvc[2] * dav[2];
+        }
+        if (out.opacity) out.opacity[i] = a[15];
+        if (out.rgb) { out.rgb[3 * i] = a[12]; out.rgb[3 * i + 1] = a[13]; out.rgb[3 * i + 2] = a[14]; }
+        // pose share: rho += dmu; theta += mu_c x dmu + t_uc x dtu + t_vc x dtv + t_nc x dtn   (Eq. 13)
+        p6[0] = dmu[0]; p6[1] = dmu[1]; p6[2] = dmu[2];
+        p6[3] = (muc[1] * dmu[2] - muc[2] * dmu[1]) + (tuc[1] * dtu[2] - tuc[2] * dtu[1]) +
+                (tvc[1] * dtv[2] - tvc[2] * dtv[1]) + (tnc[1] * dtn[2] - tnc[2] * dtn[1]);
+        p6[4] = (muc[2] * dmu[0] - muc[0] * dmu[2]) + (tuc[2] * dtu[0] - tuc[0] * dtu[2]) +
+                (tvc[2] * dtv[0] - tvc[0] * dtv[2]) + (tnc[2] * dtn[0] - tnc[0] * dtn[2]);
+        p6[5] = (muc[0] * dmu[1] - muc[1] * dmu[0]) + (tuc[0] * dtu[1] - tuc[1] * dtu[0]) +
+                (tvc[0] * dtv[1] - tvc[1] * dtv[0]) + (tnc[0] * dtn[1] - tnc[1] * dtn[0]);
+        // world space: x_c = R_cw x_w  =>  dL/dx_w = R_cw^T dL/dx_c
+        float G[3][3];  // dL/dR (world), columns t_u, t_v, t_n
+#pragma unroll
+        for (int r = 0; r < 3; ++r) {
+            const float c0 = cam.Rf[r], c1 = cam.Rf[3 + r], c2 = cam.Rf[6 + r];
+            if (out.mean) out.mean[3 * i + r] = c0 * dmu[0] + c1 * dmu[1] + c2 * dmu[2];
+            G[r][0] = c0 * dtu[0] + c1 * dtu[1] + c2 * dtu[2];
+            G[r][1] = c0 * dtv[0] + c1 * dtv[1] + c2 * dtv[2];
+            G[r][2] = c0 * dtn[0] + c1 * dtn[1] + c2 * dtn[2];
+        }
+        if (out.quat) {
+            float dq[4];
+            dq[0] = 2.f * (-qz * G[0][1] + qy * G[0][2] + qz * G[1][0] - qx * G[1][2] - qy * G[2][0] + qx * G[2][1]);
+            dq[1] = 2.f * (qy * G[0][1] + qz * G[0][2] + qy * G[1][0] - 2.f * qx * G[1][1] - qw * G[1][2] + qz * G[2][0] +
+                           qw * G[2][1] - 2.f * qx * G[2][2]);
+            dq[2] = 2.f * (-2.f * qy * G[0][0] + qx * G[0][1] + qw * G[0][2] + qx * G[1][0] + qz * G[1][2] - qw * G[2][0] +
+                           qz * G[2][1] - 2.f * qy * G[2][2]);
+            dq[3] = 2.f * (-2.f * qz * G[0][0] - qw * G[0][1] + qx * G[0][2] + qw * G[1][0] - 2.f * qz * G[1][1] +
+                           qy * G[1][2] + qx * G[2][0] + qy * G[2][1]);
+            const float qd = qw * dq[0] + qx * dq[1] + qy * dq[2] + qz * dq[3];
+            out.quat[4 * i] = (dq[0] - qw * qd) * qi;
+            out.quat[4 * i + 1] = (dq[1] - qx * qd) * qi;
+            out.quat[4 * i + 2] = (dq[2] - qy * qd) * qi;
+            out.quat[4 * i + 3] = (dq[3] - qz * qd) * qi;
+        }
+    }
+    if (d_pose6 == nullptr) return;
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        const float s = warp_sum(p6[c]);
+        if (lane == 0) s_red[wid][c] = s;
+    }
+    __syncthreads();
+    if (tid < 6) {
+        float s = 0.f;
+#pragma unroll
+        for (int w2 = 0; w2 < 8; ++w2) s += s_red[w2][tid];
+        pose_partial[(size_t)blockIdx.x * 8 + tid] = s;
+    }
+    finish_pose(pose_partial, gridDim.x, counters_rw, d_pose6);
+}
+
+}  // namespace
+
+cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_surfel_grads* dg, float* d_pose6,
+                                cudaStream_t s) {
+    const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    CPlanes u;
+    for (int i = 0; i < 8; ++i) u.p[i] = up[i];
+    const SgsCamDev& cam = c->camd;
+    if (dg == nullptr) {  // pose-only (tracking, L204)
+        if (d_pose6 == nullptr) return cudaSuccess;
+        k_backward<true><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->vals[c->sorted_buf], c->pay, cam.W, cam.H, cam.tiles_x,
+                                                     cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
+                                                     c->acc, c->pose_partial, c->counters, d_pose6);
+        return cudaGetLastError();
+    }
+    const int64_t n = c->last_surfels.n;
+    cudaError_t e = cudaSuccess;
+    if (dg->mean && e == cudaSuccess) e = cudaMemsetAsync(dg->mean, 0, sizeof(float) * 3 * (size_t)n, s);
+    if (dg->scale && e == cudaSuccess) e = cudaMemsetAsync(dg->scale, 0, sizeof(float) * 2 * (size_t)n, s);
+    if (dg->quat && e == cudaSuccess) e = cudaMemsetAsync(dg->quat, 0, sizeof(float) * 4 * (size_t)n, s);
+    if (dg->opacity && e == cudaSuccess) e = cudaMemsetAsync(dg->opacity, 0, sizeof(float) * (size_t)n, s);
+    if (dg->rgb && e == cudaSuccess) e = cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * (size_t)n, s);
+    if (e != cudaSuccess) return e;
+    k_backward<false><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->vals[c->sorted_buf], c->pay, cam.W, cam.H, cam.tiles_x,
+                                                  cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
+                                                  c->acc, c->pose_partial, c->counters, nullptr);
+    const int blocks = (int)((n + 255) / 256);  // bound on N_v; blocks past it only join the pose reduction
+    if (blocks > 0)
+        k_surfel_backward<<<blocks, 256, 0, s>>>(c->counters, c->vis_to_surfel, c->acc, c->last_surfels.mean,
+                                                 c->last_surfels.scale, c->last_surfels.quat, cam, *dg, c->pose_partial,
+                                                 c->counters, d_pose6);
+    return cudaGetLastError();
+}

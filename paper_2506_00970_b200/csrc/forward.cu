@@ -1,0 +1,89 @@
+// forward.cu -- K-fwd: per-tile front-to-back alpha compositing (Eq. 8;
+// SURVEY §8(a) step 3).  One block per 16x16 tile, one thread per pixel, a warp covers an 8x4 pixel
+// patch (better footprint coherence than 32x1).  The tile's depth-sorted entries are staged through
+// shared memory in batches of 256: one thread per entry gathers the surfel's payload (float4 loads,
+// L2-resident) and converts it to the tile-relative form of pair.cuh; all threads then read the
+// staged records as warp-wide broadcasts.  A warp leaves the batch loop when all its pixels are
+// saturated; the block stops fetching batches when every pixel is.
+#include "pair.cuh"
+#include "sgs_internal.h"
+
+namespace {
+
+struct Planes { float* p[8]; };
+
+__global__ void __launch_bounds__(SGS_BLOCK)
+k_forward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, SgsPayload pay, int W, int H,
+          int tiles_x, SgsCfgDev cfg, Planes out, float* __restrict__ T_final, uint32_t* __restrict__ n_last) {
+    __shared__ StagedFwd sh[SGS_BLOCK];
+    const int tile = blockIdx.x;
+    const int tx = tile % tiles_x, ty = tile / tiles_x;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int lxi = (wid & 1) * 8 + (lane & 7), lyi = (wid >> 1) * 4 + (lane >> 3);
+    const int px = tx * SGS_TILE + lxi, py = ty * SGS_TILE + lyi;
+    const bool inside = px < W && py < H;
+    const float lx = (float)lxi, ly = (float)lyi;
+    const double px0 = (double)(tx * SGS_TILE) + 0.5, py0 = (double)(ty * SGS_TILE) + 0.5;
+    const uint32_t start = ranges[2 * tile], end = ranges[2 * tile + 1];
+
+    float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dp = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f, O = 0.f;
+    uint32_t last = 0;  // entries [0, last) of the tile list contain every composited pair of this pixel
+    bool done = !inside;
+
+    for (uint32_t base = start; base < end; base += SGS_BLOCK) {
+        if (__syncthreads_and(done)) break;
+        const uint32_t nb = min((uint32_t)SGS_BLOCK, end - base);
+        if ((uint32_t)tid < nb) {
+            const uint32_t v = vals[base + tid];
+            const float4 g0 = pay.g0[v], g1 = pay.g1[v], g3 = pay.g3[v], g4 = pay.g4[v], g5 = pay.g5[v];
+            const double2 g2 = pay.g2[v];
+            StagedFwd st;
+            stage_entry(g0, g1, g2, g3, px0, py0, st.s0, st.s1, st.s2);
+            st.s3 = make_float4(g1.w, g3.w, g4.x, g4.y);
+            st.s4 = make_float4(g4.z, g4.w, g5.x, 0.f);
+            sh[tid] = st;
+        }
+        __syncthreads();
+        for (uint32_t j = 0; j < nb; ++j) {
+            if (__all_sync(0xffffffffu, done)) break;  // per-warp early stop on saturation
+            if (done) continue;
+            const float4 s0 = sh[j].s0, s1 = sh[j].s1, s2 = sh[j].s2, s3 = sh[j].s3;
+            PairResult r;
+            if (!eval_pair(s0, s1, s2, s3.x, lx, ly, cfg.cutoff2, cfg.alpha_min, cfg.alpha_max, cfg.z_near, r)) continue;
+            const float Tn = __fmul_rn(T, 1.f - r.a);
+            if (Tn < cfg.t_min) { done = true; continue; }  // R6: stop, this splat is not composited
+            const float w = __fmul_rn(r.a, T);
+            const float4 s4 = sh[j].s4;
+            C0 = __fmaf_rn(w, s3.y, C0); C1 = __fmaf_rn(w, s3.z, C1); C2 = __fmaf_rn(w, s3.w, C2);
+            Dp = __fmaf_rn(w, r.z, Dp);
+            N0 = __fmaf_rn(w, s4.x, N0); N1 = __fmaf_rn(w, s4.y, N1); N2 = __fmaf_rn(w, s4.z, N2);
+            O += w;
+            T = Tn;
+            last = base - start + j + 1;
+        }
+    }
+    if (inside) {
+        const size_t pix = (size_t)py * W + px;
+        if (out.p[0]) out.p[0][pix] = C0;
+        if (out.p[1]) out.p[1][pix] = C1;
+        if (out.p[2]) out.p[2][pix] = C2;
+        if (out.p[3]) out.p[3][pix] = Dp;
+        if (out.p[4]) out.p[4][pix] = N0;
+        if (out.p[5]) out.p[5][pix] = N1;
+        if (out.p[6]) out.p[6][pix] = N2;
+        if (out.p[7]) out.p[7][pix] = O;
+        T_final[pix] = T;
+        n_last[pix] = last;
+    }
+}
+
+}  // namespace
+
+cudaError_t sgs_launch_forward(sgs_ctx* c, float* const planes[8], cudaStream_t s) {
+    const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    Planes out;
+    for (int i = 0; i < 8; ++i) out.p[i] = planes[i];
+    k_forward<<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->vals[c->sorted_buf], c->pay, c->camd.W, c->camd.H, c->camd.tiles_x,
+                                          c->cfgd, out, c->T_final, c->n_last);
+    return cudaGetLastError();
+}

@@ -1,0 +1,68 @@
+// loss.cu -- tracking loss of PAPER.md Eq. 15-19 (L180-204): the harness around the renderer that
+// turns a rendered frame and a target RGB-D frame into the upstream image gradients of the
+// pose-only backward.  Element-wise, HBM-bound (reads 8+4 planes, writes 8 planes).
+//   L_I = |I_r - I|_1 (Eq. 15), L_D = |D_r - D| (Eq. 16), M_n = [sign * N_r . r > 0] (Eq. 17, R19),
+//   M_o = [O > 0.95] (Eq. 18), L_t = mean(M_n M_o (L_I + lambda_d L_D)) (Eq. 19).
+#include "sgs_internal.h"
+
+namespace {
+
+struct LP { const float* ren[8]; float* up[8]; };
+
+__global__ void __launch_bounds__(256)
+k_tracking_loss(LP p, const float* __restrict__ trgb, const float* __restrict__ tdepth, int W, int H, float fx,
+                float fy, float cx, float cy, float lambda_d, float nsign, float* __restrict__ loss) {
+    __shared__ float s_part[8];
+    const int64_t HW = (int64_t)W * H;
+    const float inv = 1.f / (float)HW;
+    float acc = 0.f;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < HW; i += (int64_t)gridDim.x * blockDim.x) {
+        const int px = (int)(i % W), py = (int)(i / W);
+        const float rx = ((float)px + 0.5f - cx) / fx, ry = ((float)py + 0.5f - cy) / fy;
+        const float nr = p.ren[4][i] * rx + p.ren[5][i] * ry + p.ren[6][i];
+        const bool m = (nsign * nr > 0.f) && (p.ren[7][i] > 0.95f);
+        float g[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        if (m) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const float d = p.ren[c][i] - trgb[c * HW + i];
+                acc += fabsf(d);
+                g[c] = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
+            }
+            const float d = p.ren[3][i] - tdepth[i];
+            acc += lambda_d * fabsf(d);
+            g[3] = d > 0.f ? lambda_d * inv : (d < 0.f ? -lambda_d * inv : 0.f);
+        }
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+            if (p.up[c]) p.up[c][i] = g[c];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float s = 0.f;
+        for (int w = 0; w < 8; ++w) s += s_part[w];
+        if (loss) atomicAdd(loss, s * inv);
+    }
+}
+
+}  // namespace
+
+cudaError_t sgs_launch_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const float* const ren[8], const float* trgb,
+                                     const float* tdepth, float lambda_d, float nsign, float* const up[8], float* loss,
+                                     cudaStream_t s) {
+    (void)c;
+    LP p;
+    for (int i = 0; i < 8; ++i) { p.ren[i] = ren[i]; p.up[i] = up[i]; }
+    const int64_t HW = (int64_t)cam->width * cam->height;
+    int blocks = (int)((HW + 255) / 256);
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    cudaError_t e = cudaSuccess;
+    if (loss) e = cudaMemsetAsync(loss, 0, sizeof(float), s);
+    if (e != cudaSuccess) return e;
+    k_tracking_loss<<<blocks, 256, 0, s>>>(p, trgb, tdepth, cam->width, cam->height, cam->fx, cam->fy, cam->cx, cam->cy,
+                                           lambda_d, nsign, loss);
+    return cudaGetLastError();
+}

@@ -1,0 +1,66 @@
+// pair.cuh -- one (pixel, surfel) pair, shared by the forward and backward compositing kernels so
+// that both take bit-identical decisions (explicit _rn intrinsics pin the instruction sequence).
+//
+// Ray-splat intersection (Eq. 4) in the screen-centred adjugate form:
+// with the tile-relative staged coefficients
+//   un = U0 + lx P + ly Q,  vn = V0 + lx R + ly S,  dn = D0 + lx E' + ly F'
+//   (u, v) = (un, vn) / dn,   z = a u + b v + c
+// which is algebraically (u,v,1) ~ (M0 - x M2) x (M1 - y M2) with the pixel-independent factors of
+// the cross product hoisted per surfel and the pixel coordinate taken relative to the surfel's
+// projected centre, the well-conditioned choice in fp32.
+#pragma once
+#include <cuda_runtime.h>
+
+// Staged per-(tile, entry) record in shared memory: 5 x float4, read as warp-wide broadcasts.
+struct StagedFwd {
+    float4 s0;  // P, Q, U0, E'
+    float4 s1;  // R, S, V0, F'
+    float4 s2;  // D0, a, b, c
+    float4 s3;  // opacity, r, g, b
+    float4 s4;  // nx, ny, nz, unused
+};
+
+struct PairResult {
+    float u, v, z, G, a;
+};
+
+__device__ __forceinline__ float fast_rcp(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float fast_ex2(float x) {
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// Returns true when the pair passes the geometric tests (rho^2 <= c^2, finite, z > z_near) and
+// a >= alpha_min.  The saturation stop is the caller's (it needs T).
+__device__ __forceinline__ bool eval_pair(const float4 s0, const float4 s1, const float4 s2, const float opacity,
+                                          const float lx, const float ly, const float cutoff2, const float alpha_min,
+                                          const float alpha_max, const float z_near, PairResult& r) {
+    const float un = __fmaf_rn(ly, s0.y, __fmaf_rn(lx, s0.x, s0.z));
+    const float vn = __fmaf_rn(ly, s1.y, __fmaf_rn(lx, s1.x, s1.z));
+    const float dn = __fmaf_rn(ly, s1.w, __fmaf_rn(lx, s0.w, s2.x));
+    const float inv = fast_rcp(dn);
+    r.u = __fmul_rn(un, inv);
+    r.v = __fmul_rn(vn, inv);
+    const float rho2 = __fmaf_rn(r.v, r.v, __fmul_rn(r.u, r.u));
+    if (!(rho2 <= cutoff2)) return false;  // also rejects NaN/inf (dn == 0)
+    r.z = __fmaf_rn(s2.z, r.v, __fmaf_rn(s2.y, r.u, s2.w));
+    if (!(r.z > z_near)) return false;
+    r.G = fast_ex2(__fmul_rn(rho2, -0.72134752044448170368f));  // exp(-rho2/2) = 2^(-rho2 / (2 ln 2))
+    r.a = fminf(alpha_max, __fmul_rn(opacity, r.G));
+    return r.a >= alpha_min;
+}
+
+// Builds the staged record of entry `v` for the tile whose first pixel centre is (px0, py0).
+__device__ __forceinline__ void stage_entry(const float4 g0, const float4 g1, const double2 g2, const float4 g3,
+                                            const double px0, const double py0, float4& s0, float4& s1, float4& s2) {
+    const float X0 = (float)(px0 - g2.x), Y0 = (float)(py0 - g2.y);  // xt, yt of the tile's first pixel
+    const float P = g0.x, Q = g0.y, R = g0.z, S = g0.w, D = g1.x, E = g1.y, F = g1.z;
+    s0 = make_float4(P, Q, __fmaf_rn(Y0, Q, __fmul_rn(X0, P)), -E);
+    s1 = make_float4(R, S, __fmaf_rn(Y0, S, __fmul_rn(X0, R)), -F);
+    s2 = make_float4(__fmaf_rn(-Y0, F, __fmaf_rn(-X0, E, D)), g3.x, g3.y, g3.z);
+}

@@ -1,0 +1,222 @@
+// preprocess.cu -- K-pre: one thread per surfel (SURVEY §8(a) step 1 + the emit half of step 2).
+//
+// Builds the ray-splat homography M = K [s_u t_uc, s_v t_vc, mu_c] (Eq. 5-7), culls,
+// derives the screen AABB of the cutoff ellipse and the tile rectangle, and -- fused in the same
+// kernel through a single-pass chained scan (decoupled look-back over dynamically numbered blocks)
+// -- compacts the visible surfels and emits their 64-bit (tile id << 32 | depth bits) keys in
+// surfel-major, tile row-major order.
+//
+// THIS FILE IS COMPILED WITH -fmad=false.  Everything that takes a binning decision (cull flag,
+// depth bits, tile rectangle) is evaluated in IEEE-754 binary64 in the operation order DESIGN.md §3
+// (O2) fixes, so that the list is bit-identical to the CPU oracle's.  B200 has full-rate-enough
+// FP64 for this: the kernel is HBM-bound (52 B in, ~130 B out per visible surfel).
+#include "sgs_internal.h"
+
+namespace {
+
+constexpr unsigned long long FLAG_AGG = 1ull << 62;
+constexpr unsigned long long FLAG_INC = 2ull << 62;
+constexpr unsigned long long FLAG_MASK = 3ull << 62;
+constexpr int VIS_SHIFT = 38;  // value = vis (24 bits) << 38 | entries (38 bits)
+
+__device__ __forceinline__ unsigned long long warp_incl_scan(unsigned long long v, int lane) {
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        unsigned long long t = __shfl_up_sync(0xffffffffu, v, o);
+        if (lane >= o) v += t;
+    }
+    return v;
+}
+
+struct PreOut {
+    bool vis;
+    uint32_t depth_bits;
+    int tx0, ty0, tx1, ty1;
+    // payload
+    float P, Q, R, S, D, E, F;
+    double xc, yc;
+    float a, b, c;
+    float n[3], au[3], av[3];
+};
+
+__device__ __forceinline__ void preprocess_one(const float* __restrict__ mean, const float* __restrict__ scale,
+                                               const float* __restrict__ quat, const SgsCamDev& cam,
+                                               const SgsCfgDev& cfg, PreOut& o) {
+    o.vis = false;
+    const double w = quat[0], x = quat[1], y = quat[2], z = quat[3];
+    const double qn = sqrt(((w * w + x * x) + y * y) + z * z);
+    if (!(qn > 0.0) || !isfinite(qn)) return;
+    const double qw = w / qn, qx = x / qn, qy = y / qn, qz = z / qn;
+    double Rw[9];
+    Rw[0] = 1.0 - 2.0 * (qy * qy + qz * qz); Rw[1] = 2.0 * (qx * qy - qw * qz); Rw[2] = 2.0 * (qx * qz + qw * qy);
+    Rw[3] = 2.0 * (qx * qy + qw * qz); Rw[4] = 1.0 - 2.0 * (qx * qx + qz * qz); Rw[5] = 2.0 * (qy * qz - qw * qx);
+    Rw[6] = 2.0 * (qx * qz - qw * qy); Rw[7] = 2.0 * (qy * qz + qw * qx); Rw[8] = 1.0 - 2.0 * (qx * qx + qy * qy);
+    const double m0 = mean[0], m1 = mean[1], m2 = mean[2];
+    double tuc[3], tvc[3], tnc[3], muc[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const double r0 = cam.R[3 * i], r1 = cam.R[3 * i + 1], r2 = cam.R[3 * i + 2];
+        tuc[i] = (r0 * Rw[0] + r1 * Rw[3]) + r2 * Rw[6];
+        tvc[i] = (r0 * Rw[1] + r1 * Rw[4]) + r2 * Rw[7];
+        tnc[i] = (r0 * Rw[2] + r1 * Rw[5]) + r2 * Rw[8];
+        muc[i] = ((r0 * m0 + r1 * m1) + r2 * m2) + cam.t[i];
+    }
+    const double su = scale[0], sv = scale[1];
+    const double A0[3] = {su * tuc[0], sv * tvc[0], muc[0]};
+    const double A1[3] = {su * tuc[1], sv * tvc[1], muc[1]};
+    const double A2[3] = {su * tuc[2], sv * tvc[2], muc[2]};
+    double M[9];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        M[j] = cam.Kd[0] * A0[j] + cam.Kd[2] * A2[j];
+        M[3 + j] = cam.Kd[1] * A1[j] + cam.Kd[3] * A2[j];
+        M[6 + j] = A2[j];
+    }
+    o.depth_bits = __float_as_uint((float)muc[2]);
+    if (!(muc[2] > cfg.z_near_d)) return;
+    const double c2 = cfg.cutoff2_d;
+    const double den = c2 * (M[6] * M[6] + M[7] * M[7]) - M[8] * M[8];
+    if (!(den < 0.0)) return;
+    const double ctrx = (c2 * (M[0] * M[6] + M[1] * M[7]) - M[2] * M[8]) / den;
+    const double ctry = (c2 * (M[3] * M[6] + M[4] * M[7]) - M[5] * M[8]) / den;
+    const double hx = sqrt(ctrx * ctrx - (c2 * (M[0] * M[0] + M[1] * M[1]) - M[2] * M[2]) / den);
+    const double hy = sqrt(ctry * ctry - (c2 * (M[3] * M[3] + M[4] * M[4]) - M[5] * M[5]) / den);
+    const double xmin = ctrx - hx, xmax = ctrx + hx, ymin = ctry - hy, ymax = ctry + hy;
+    if (!(isfinite(xmin) && isfinite(xmax) && isfinite(ymin) && isfinite(ymax))) return;
+    if (!(xmax > 0.0 && xmin < (double)cam.W && ymax > 0.0 && ymin < (double)cam.H)) return;
+    const double ts = (double)SGS_TILE;
+    double fx0 = floor(xmin / ts), fx1 = floor(xmax / ts), fy0 = floor(ymin / ts), fy1 = floor(ymax / ts);
+    if (fx0 < 0.0) fx0 = 0.0;
+    if (fy0 < 0.0) fy0 = 0.0;
+    if (fx1 > (double)(cam.tiles_x - 1)) fx1 = (double)(cam.tiles_x - 1);
+    if (fy1 > (double)(cam.tiles_y - 1)) fy1 = (double)(cam.tiles_y - 1);
+    o.tx0 = (int)fx0; o.tx1 = (int)fx1; o.ty0 = (int)fy0; o.ty1 = (int)fy1;
+    o.vis = true;
+    // ---- payload (no decision depends on it; rounded to fp32 at the end) ----
+    const double xc = M[2] / M[8], yc = M[5] / M[8];
+    const double B00 = M[0] - xc * M[6], B01 = M[1] - xc * M[7];
+    const double B10 = M[3] - yc * M[6], B11 = M[4] - yc * M[7];
+    const double a = M[6], b = M[7], c = M[8];
+    o.P = (float)(c * B11); o.Q = (float)(-(c * B01)); o.R = (float)(-(c * B10)); o.S = (float)(c * B00);
+    o.D = (float)(B00 * B11 - B01 * B10);
+    o.E = (float)(a * B11 - b * B10);
+    o.F = (float)(b * B00 - a * B01);
+    o.xc = xc; o.yc = yc;
+    o.a = (float)a; o.b = (float)b; o.c = (float)c;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        o.n[i] = (float)tnc[i];
+        o.au[i] = (float)(su * tuc[i]);
+        o.av[i] = (float)(sv * tvc[i]);
+    }
+}
+
+__global__ void __launch_bounds__(SGS_PRE_BLOCK)
+k_preprocess(int64_t n, const float* __restrict__ mean, const float* __restrict__ scale,
+             const float* __restrict__ quat, const float* __restrict__ opacity, const float* __restrict__ rgb,
+             const uint8_t* __restrict__ active, SgsCamDev cam, SgsCfgDev cfg, SgsPayload pay,
+             uint32_t* __restrict__ vis_to_surfel, uint8_t* __restrict__ culled,
+             unsigned long long* __restrict__ scan_state, SgsCounters* __restrict__ counters,
+             uint64_t* __restrict__ keys, uint32_t* __restrict__ vals, unsigned long long e_cap) {
+    __shared__ unsigned int s_bid;
+    __shared__ unsigned long long s_warp[SGS_PRE_BLOCK / 32];
+    __shared__ unsigned long long s_prefix;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid == 0) s_bid = atomicAdd(&counters->ticket_pre, 1u);  // dynamic id: predecessors are running or done
+    __syncthreads();
+    const unsigned int bid = s_bid;
+    const int64_t i = (int64_t)bid * SGS_PRE_BLOCK + tid;
+
+    PreOut o;
+    o.vis = false;
+    if (i < n && (active == nullptr || active[i] != 0)) preprocess_one(mean + 3 * i, scale + 2 * i, quat + 4 * i, cam, cfg, o);
+    unsigned int cnt = 0;
+    if (o.vis) cnt = (unsigned int)((o.tx1 - o.tx0 + 1) * (o.ty1 - o.ty0 + 1));
+    if (i < n) culled[i] = o.vis ? 0 : 1;
+
+    // block-exclusive scan of (visible, entries) packed in one 64-bit word
+    const unsigned long long mine = ((unsigned long long)(o.vis ? 1 : 0) << VIS_SHIFT) | cnt;
+    const unsigned long long incl = warp_incl_scan(mine, lane);
+    if (lane == 31) s_warp[wid] = incl;
+    __syncthreads();
+    if (wid == 0) {
+        unsigned long long wv = lane < SGS_PRE_BLOCK / 32 ? s_warp[lane] : 0ull;
+        const unsigned long long wi = warp_incl_scan(wv, lane);
+        if (lane < SGS_PRE_BLOCK / 32) s_warp[lane] = wi - wv;  // exclusive warp offsets
+        const unsigned long long block_total = __shfl_sync(0xffffffffu, wi, SGS_PRE_BLOCK / 32 - 1);
+        // chained scan: publish the aggregate, look back over predecessors 32 at a time
+        unsigned long long prefix = 0;
+        if (bid == 0) {
+            if (lane == 0) atomicExch(&scan_state[0], FLAG_INC | block_total);
+        } else {
+            if (lane == 0) atomicExch(&scan_state[bid], FLAG_AGG | block_total);
+            int64_t look = (int64_t)bid - 1;
+            while (true) {
+                const int64_t j = look - lane;
+                unsigned long long st = FLAG_INC;  // lanes before block 0 read as "inclusive 0"
+                if (j >= 0) {
+                    do { st = *((volatile unsigned long long*)&scan_state[j]); } while ((st & FLAG_MASK) == 0);
+                }
+                const unsigned int inc_mask = __ballot_sync(0xffffffffu, (st & FLAG_MASK) == FLAG_INC);
+                const int first_inc = inc_mask ? __ffs(inc_mask) - 1 : 32;
+                unsigned long long v = (lane <= first_inc) ? (st & ~FLAG_MASK) : 0ull;
+#pragma unroll
+                for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+                prefix += v;
+                if (inc_mask) break;
+                look -= 32;
+            }
+            if (lane == 0) atomicExch(&scan_state[bid], FLAG_INC | (prefix + block_total));
+        }
+        if (lane == 0) {
+            s_prefix = prefix;
+            if (bid == gridDim.x - 1) {  // totals: E, N_v, overflow
+                const unsigned long long tot = prefix + block_total;
+                const unsigned long long E = tot & ((1ull << VIS_SHIFT) - 1);
+                counters->n_entries = E;
+                counters->n_visible = (unsigned int)(tot >> VIS_SHIFT);
+                counters->overflow = E > e_cap ? 1u : 0u;
+            }
+        }
+    }
+    __syncthreads();
+    if (!o.vis) return;
+    const unsigned long long excl = s_prefix + s_warp[wid] + (incl - mine);
+    const uint32_t v = (uint32_t)(excl >> VIS_SHIFT);
+    unsigned long long pos = excl & ((1ull << VIS_SHIFT) - 1);
+
+    vis_to_surfel[v] = (uint32_t)i;
+    pay.g0[v] = make_float4(o.P, o.Q, o.R, o.S);
+    pay.g1[v] = make_float4(o.D, o.E, o.F, opacity[i]);
+    pay.g2[v] = make_double2(o.xc, o.yc);
+    pay.g3[v] = make_float4(o.a, o.b, o.c, rgb[3 * i]);
+    pay.g4[v] = make_float4(rgb[3 * i + 1], rgb[3 * i + 2], o.n[0], o.n[1]);
+    pay.g5[v] = make_float4(o.n[2], o.au[0], o.au[1], o.au[2]);
+    pay.g6[v] = make_float4(o.av[0], o.av[1], o.av[2], 0.f);
+
+    // emit keys: tile row-major within the surfel (R2: key = tile id << 32 | depth bits)
+    for (int ty = o.ty0; ty <= o.ty1; ++ty)
+        for (int tx = o.tx0; tx <= o.tx1; ++tx) {
+            if (pos < e_cap) {
+                keys[pos] = ((unsigned long long)(uint32_t)(ty * cam.tiles_x + tx) << 32) | o.depth_bits;
+                vals[pos] = v;
+            }
+            ++pos;
+        }
+}
+
+}  // namespace
+
+cudaError_t sgs_launch_preprocess(sgs_ctx* c, const sgs_surfels* sf, cudaStream_t s) {
+    const int64_t n = sf->n;
+    const int blocks = (int)((n + SGS_PRE_BLOCK - 1) / SGS_PRE_BLOCK);
+    cudaError_t e = cudaMemsetAsync(c->counters, 0, sizeof(SgsCounters), s);
+    if (e != cudaSuccess) return e;
+    if (blocks == 0) return cudaSuccess;
+    e = cudaMemsetAsync(c->scan_state, 0, sizeof(unsigned long long) * (size_t)blocks, s);
+    if (e != cudaSuccess) return e;
+    k_preprocess<<<blocks, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, sf->active,
+                                                  c->camd, c->cfgd, c->pay, c->vis_to_surfel, c->culled, c->scan_state,
+                                                  c->counters, c->keys[0], c->vals[0], (unsigned long long)c->e_cap);
+    return cudaGetLastError();
+}

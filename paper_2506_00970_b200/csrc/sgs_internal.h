@@ -1,0 +1,132 @@
+// sgs_internal.h -- shared declarations of the CUDA path (ctx, workspace layout, launchers).
+// Nothing here is used by the oracle.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/sgs.h"
+
+#define SGS_TILE 16
+#define SGS_BLOCK 256                // threads per compositing block = pixels per tile
+#define SGS_SORT_ITEMS 8             // items per thread in the radix sort
+#define SGS_SORT_TILE (256 * SGS_SORT_ITEMS)
+#define SGS_PRE_BLOCK 256
+#define SGS_ACC_STRIDE 16            // floats per visible surfel in the backward accumulator
+
+// Per-visible-surfel payload, structure of float4 arrays indexed by the compact visible index v.
+// Screen-centred adjugate form of the ray-splat intersection:
+//   xt = x - x_c, yt = y - y_c  (x_c, y_c = projected centre, kept in fp64)
+//   u = (xt P + yt Q) / den,  v = (xt R + yt S) / den,  den = D - xt E - yt F,  z = a u + b v + c
+struct SgsPayload {
+    float4* g0;   // P, Q, R, S
+    float4* g1;   // D, E, F, opacity
+    double2* g2;  // x_c, y_c
+    float4* g3;   // a, b, c (= M20, M21, M22), rgb.r
+    float4* g4;   // rgb.g, rgb.b, n_c.x, n_c.y
+    float4* g5;   // n_c.z, a_u.x, a_u.y, a_u.z      (a_u = s_u t_uc, camera space)
+    float4* g6;   // a_v.x, a_v.y, a_v.z, unused     (a_v = s_v t_vc)
+};
+
+struct SgsCamDev {
+    int W, H, tiles_x, tiles_y;
+    float fx, fy, cx, cy;
+    double Kd[4];   // fx, fy, cx, cy widened
+    double R[9];    // R_cw row-major
+    double t[3];
+    float Rf[9];
+    float tf[3];
+};
+
+struct SgsCfgDev {
+    float cutoff2, alpha_min, alpha_max, t_min, z_near;
+    double cutoff2_d, z_near_d;
+};
+
+// Device-side counters of one render (also copied to pinned host memory).
+struct SgsCounters {
+    unsigned long long n_entries;   // E (may exceed capacity -> overflow)
+    unsigned int n_visible;
+    unsigned int overflow;
+    unsigned int ticket_pre;        // dynamic block ids for the chained scan in K-pre
+    unsigned int ticket_bwd;        // last-block-done ticket for the pose reduction
+    unsigned int pad[2];
+};
+
+struct sgs_ctx {
+    sgs_config cfg;
+    SgsCfgDev cfgd;
+    // sizes
+    int64_t n_cap;        // surfel capacity of per-surfel workspace
+    int64_t e_cap;        // entry capacity
+    int64_t tiles_cap;
+    int64_t pix_cap;
+    int64_t bytes;
+    // per-surfel
+    unsigned long long* scan_state;  // chained-scan status words, one per K-pre block
+    uint32_t* vis_to_surfel;         // n_cap
+    uint8_t* culled;                 // n_cap
+    SgsPayload pay;                  // n_cap each
+    float* acc;                      // n_cap x 16 backward accumulators
+    // per-entry (double buffered for the sort)
+    uint64_t* keys[2];
+    uint32_t* vals[2];
+    uint32_t* idx_export;            // e_cap, original indices for sgs_get_binning
+    uint32_t* sort_hist;             // passes x 256 global digit histograms
+    uint32_t* sort_state;            // passes x sort_tiles x 256 look-back words
+    uint32_t* sort_ticket;           // passes
+    int64_t sort_tiles_cap;
+    // per-tile / per-pixel
+    uint32_t* ranges;                // tiles x 2
+    float* T_final;                  // pixels
+    uint32_t* n_last;                // pixels: index (within the tile list) after the last composited entry
+    float* pose_partial;             // tiles x 8 (pose-only) or blocks x 8 (per-surfel)
+    float* img_saved[8];             // planes the backward needs when the caller did not ask for them
+    float* img_scratch;              // 8 planes, pix_cap each
+    SgsCounters* counters;           // device
+    SgsCounters* counters_host;      // pinned
+    cudaEvent_t counters_ready;
+    // last forward
+    bool have_forward;
+    bool pending_check;              // async mode: counters_host not yet examined
+    sgs_surfels last_surfels;
+    sgs_camera last_cam;
+    SgsCamDev camd;
+    const float* last_img[8];        // device planes of the last render: rgb(3), depth, normal(3), alpha
+    int sorted_buf;                  // which of keys[]/vals[] holds the sorted list
+    int64_t launch_entries;          // entries bound used for this render's launches
+    // resident (host-path) state
+    sgs_surfels resident;            // ctx-owned device copy
+    int64_t resident_cap;
+    float* resident_store;           // one allocation
+    uint8_t* resident_active;
+    float* target_rgb; float* target_depth; int64_t target_cap;
+    float* host_img_dev;             // 8 planes staging for *_host
+    float* host_up_dev;              // 8 planes staging
+    float* host_grads_dev;           // n x 13 staging
+    float* loss_dev; float* pose6_dev;
+    float* pinned_small;             // 8 floats pinned
+    int64_t host_img_cap, host_grads_cap;
+    int64_t partial_cap;             // floats in pose_partial
+    int64_t last_entries;            // E of the last checked render (async launch bound hint), 0 = unknown
+};
+
+// ---- launchers (each enqueues on `s`, returns the last CUDA error) ----
+cudaError_t sgs_launch_preprocess(sgs_ctx* c, const sgs_surfels* sf, cudaStream_t s);
+cudaError_t sgs_launch_sort_and_ranges(sgs_ctx* c, cudaStream_t s);
+cudaError_t sgs_launch_forward(sgs_ctx* c, float* const planes[8], cudaStream_t s);
+cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_surfel_grads* dg, float* d_pose6,
+                                cudaStream_t s);
+cudaError_t sgs_launch_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const float* const ren[8], const float* trgb,
+                                     const float* tdepth, float lambda_d, float nsign, float* const up[8], float* loss,
+                                     cudaStream_t s);
+cudaError_t sgs_launch_export_idx(sgs_ctx* c, cudaStream_t s);
+int sgs_sort_passes(int tiles);
+
+// ---- workspace helpers (api.cu) ----
+void* sgs_ws_alloc(sgs_ctx* c, size_t bytes, cudaStream_t s);
+void sgs_ws_free(sgs_ctx* c, void* p, cudaStream_t s);
+int sgs_ensure_surfels(sgs_ctx* c, int64_t n, cudaStream_t s);
+int sgs_ensure_entries(sgs_ctx* c, int64_t e, cudaStream_t s);
+int sgs_ensure_image(sgs_ctx* c, int tiles, int64_t pixels, cudaStream_t s);
+int sgs_ensure_partials(sgs_ctx* c, int64_t blocks, cudaStream_t s);
+void sgs_fill_cam(const sgs_camera* cam, SgsCamDev* d);
+bool sgs_cam_valid(const sgs_camera* cam);

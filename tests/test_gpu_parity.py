@@ -1,0 +1,244 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the CPU oracle, element by element,
+on the same seeded inputs.  Bars (BASELINE.json north_star): binning bit-exact; images
+1e-4 rel / 1e-5 abs outside the oracle's fragile mask; gradients 1e-3 rel (+1e-3 RMS(group) floor)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import scenegen
+from scenegen import Scene, Camera
+
+pytestmark = pytest.mark.gpu
+
+sgs = pytest.importorskip("paper_2506_00970_b200")
+from gpu_common import (to_device, camera, alloc_images, planes, alloc_grads, split_upstream, image_check,  # noqa: E402
+                        grad_check)
+
+
+@pytest.fixture(scope="module")
+def ren():
+    r = sgs.Renderer()
+    yield r
+    r.close()
+
+
+def run_gpu(ren, sc, cam, up=None, full=True, pose=True, T_cw=None):
+    t, sf = to_device(sc)
+    c = camera(cam, T_cw)
+    im = alloc_images(cam)
+    ren.render(sf, c, **im)
+    tiles = ((cam.width + 15) // 16) * ((cam.height + 15) // 16)
+    out = dict(img=planes(im), bin=ren.get_binning(sc.n, tiles), stats=ren.stats())
+    if up is not None:
+        g = alloc_grads(sc.n) if full else None
+        p6 = torch.full((6,), 3.0, device="cuda") if pose else None
+        ren.backward(**split_upstream(up), grads=g, d_pose6=p6)
+        torch.cuda.synchronize()
+        if g is not None:
+            out["grads"] = {k: v.cpu().numpy() for k, v in g.items()}
+        if p6 is not None:
+            out["pose"] = p6.cpu().numpy().astype(np.float64)
+    return out
+
+
+def assert_binning(gb, ob):
+    assert gb["E"] == ob["E"]
+    assert np.array_equal(gb["culled"], ob["culled"])
+    assert np.array_equal(gb["keys"], ob["keys"])
+    assert np.array_equal(gb["idx"], ob["idx"])
+    assert np.array_equal(gb["ranges"], ob["ranges"])
+
+
+def assert_images(gpu_img, o):
+    chk = image_check(gpu_img, o["img"], o["fragile"])
+    assert chk["n_bad"] == 0, chk
+    assert chk["fragile_ok"], chk
+    assert chk["fragile_frac"] < 0.05, chk
+
+
+def assert_grads(g, og, max_bad=2e-3):
+    for k in ("mean", "scale", "quat", "opacity", "rgb"):
+        chk = grad_check(g[k], og[k])
+        assert chk["frac_bad"] <= max_bad, (k, chk)
+
+
+def assert_pose(p, op, rtol=1e-3):
+    assert np.abs(p - op).max() <= rtol * np.abs(op).max(), (p, op)
+
+
+POSES = [None, [0.1, -0.2, 0.15, 0.2, -0.1, 0.3]]
+
+
+@pytest.mark.parametrize("tau", POSES)
+def test_c1_full(ren, tau):
+    """Config 1: binning bit-exact, images, all surfel gradients and the pose gradient."""
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    T = None if tau is None else scenegen.perturb_pose(cam.T_cw, tau)
+    camv, cfg = oracle.make_cam(cam, T), oracle.make_cfg()
+    up = scenegen.upstream_normal(1, cam.height, cam.width)
+    out = run_gpu(ren, sc, cam, up, T_cw=T)
+    assert_binning(out["bin"], oracle.binning(sc, camv, cfg))
+    o = oracle.render(sc, camv, cfg)
+    assert_images(out["img"], o)
+    og = oracle.backward(sc, camv, cfg, up)
+    assert_grads(out["grads"], og)
+    assert_pose(out["pose"], og["pose"])
+    # pose-only mode (per-pixel Eq. 11-13) against the same oracle
+    out2 = run_gpu(ren, sc, cam, up, full=False, T_cw=T)
+    assert_pose(out2["pose"], og["pose"])
+
+
+def test_c2_tracking_shape(ren):
+    """Config 2 (200k surfels, 640x480): binning, images, tracking loss (Eq. 15-19), pose-only backward."""
+    sc, cams, info = scenegen.make_config("C2")
+    cam = cams[0]
+    camv, cfg = oracle.make_cam(cam), oracle.make_cfg()
+    # target frame: the oracle's own render at the perturbed pose Exp(tau0) T
+    g = scenegen.SplitMix(info["tau0_seed"])
+    d = np.stack([g.normal(3), g.normal(3)])
+    tau0 = np.concatenate([0.02 * d[0] / np.linalg.norm(d[0]), np.deg2rad(1.0) * d[1] / np.linalg.norm(d[1])])
+    T_tgt = scenegen.perturb_pose(cam.T_cw, tau0)
+    tgt = oracle.render(sc, oracle.make_cam(cam, T_tgt), cfg, counters=False)["img"]
+    t, sf = to_device(sc)
+    c = camera(cam)
+    im, upi = alloc_images(cam), alloc_images(cam)
+    ren.render(sf, c, **im)
+    tiles = ((cam.width + 15) // 16) * ((cam.height + 15) // 16)
+    assert_binning(ren.get_binning(sc.n, tiles), oracle.binning(sc, camv, cfg))
+    o = oracle.render(sc, camv, cfg)
+    gimg = planes(im)
+    assert_images(gimg, o)
+    # loss kernel on the GPU's own images vs the numpy definition on the same images
+    trgb = torch.from_numpy(tgt[0:3].astype(np.float32)).cuda()
+    tdep = torch.from_numpy(tgt[3:4].astype(np.float32)).cuda()
+    loss = torch.zeros(1, device="cuda")
+    ren.tracking_loss(c, im, trgb, tdep, 0.5, -1.0, upi, loss)
+    L_ref, up_ref = oracle.tracking_loss(gimg, trgb.cpu().numpy(), tdep.cpu().numpy()[0], camv, 0.5, -1.0)
+    assert abs(float(loss.item()) - L_ref) <= 1e-4 * abs(L_ref)
+    up_gpu = planes(upi)
+    assert np.abs(up_gpu - up_ref).max() <= 1e-6 * np.abs(up_ref).max()
+    assert (up_ref != 0).mean() > 0.05
+    # pose-only backward on those upstream gradients vs the oracle's analytic backward
+    p6 = torch.zeros(6, device="cuda")
+    ren.backward(d_rgb=upi["rgb"], d_depth=upi["depth"], d_normal=upi["normal"], d_alpha=upi["alpha"], d_pose6=p6)
+    og = oracle.backward(sc, camv, cfg, up_gpu)
+    assert_pose(p6.cpu().numpy().astype(np.float64), og["pose"])
+
+
+def test_backward_is_repeatable_and_overwrites(ren):
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    up = scenegen.upstream_normal(4, cam.height, cam.width)
+    t, sf = to_device(sc)
+    ren.render(sf, camera(cam), **alloc_images(cam))
+    res = []
+    for _ in range(2):
+        g, p6 = alloc_grads(sc.n), torch.full((6,), 9.0, device="cuda")
+        ren.backward(**split_upstream(up), grads=g, d_pose6=p6)
+        res.append(({k: v.cpu().numpy() for k, v in g.items()}, p6.cpu().numpy()))
+    for k in res[0][0]:
+        np.testing.assert_allclose(res[0][0][k], res[1][0][k], rtol=1e-4, atol=1e-4 * np.abs(res[0][0][k]).max())
+    np.testing.assert_allclose(res[0][1], res[1][1], rtol=1e-4)
+    culled = ren.get_binning(sc.n, 12)["culled"].astype(bool)
+    assert culled.any()
+    for k in res[0][0]:
+        assert (res[0][0][k][culled] == 0).all()     # exactly zero for culled surfels
+
+
+def test_mask_equals_compacted_subset(ren):
+    """L204/L161: inactive splats contribute nothing -- render(all, mask) == render(active subset) bit for bit."""
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    act = (scenegen.SplitMix(99).uniform(sc.n) < 0.3).astype(np.uint8)
+    m = act.astype(bool)
+    masked = Scene(sc.mean, sc.scale, sc.quat, sc.opacity, sc.rgb, act)
+    sub = Scene(sc.mean[m], sc.scale[m], sc.quat[m], sc.opacity[m], sc.rgb[m])
+    up = scenegen.upstream_normal(5, cam.height, cam.width)
+    a, b = run_gpu(ren, masked, cam, up), run_gpu(ren, sub, cam, up)
+    assert np.array_equal(a["img"], b["img"])
+    assert np.array_equal(a["bin"]["keys"], b["bin"]["keys"])
+    assert np.array_equal(a["bin"]["idx"], np.nonzero(m)[0][b["bin"]["idx"]])
+    for k in a["grads"]:
+        assert (a["grads"][k][~m] == 0).all()
+    assert_binning(a["bin"], oracle.binning(masked, oracle.make_cam(cam), oracle.make_cfg()))
+
+
+def test_edge_cases(ren):
+    cam = Camera(70, 50, 60.0, 60.0, 35.0, 25.0)     # ragged: 70 = 4.375 tiles, 50 = 3.125 tiles
+    cfg = oracle.make_cfg()
+    # empty map
+    empty = Scene(*[np.zeros(s, np.float32) for s in ((0, 3), (0, 2), (0, 4), (0,), (0, 3))])
+    out = run_gpu(ren, empty, cam, scenegen.upstream_normal(1, 50, 70), full=True)
+    assert out["bin"]["E"] == 0 and (out["img"] == 0).all() and (out["pose"] == 0).all()
+    # everything behind the camera / off-screen -> all culled
+    sc = scenegen.tiny_scene(3, 500)
+    behind = Scene(sc.mean * np.float32([1, 1, -1]), sc.scale, sc.quat, sc.opacity, sc.rgb)
+    out = run_gpu(ren, behind, cam, scenegen.upstream_normal(1, 50, 70))
+    assert out["bin"]["E"] == 0 and out["bin"]["culled"].all() and (out["img"] == 0).all()
+    assert all((v == 0).all() for v in out["grads"].values())
+    # ragged image, degenerate inputs: zero quaternion, NaN mean, huge and tiny scales, opacity 1 (clamp)
+    sc = scenegen.tiny_scene(7, 3000)
+    sc.quat[5] = 0; sc.mean[6] = np.nan; sc.scale[7] = 5.0; sc.scale[8] = 1e-5; sc.opacity[:50] = 1.0
+    sc.mean[9] = [0.0, 0.0, 0.25]; sc.scale[9] = 0.5   # disk crossing the camera plane
+    camv = oracle.make_cam(cam)
+    up = scenegen.upstream_normal(2, 50, 70)
+    out = run_gpu(ren, sc, cam, up)
+    ob = oracle.binning(sc, camv, cfg)
+    assert_binning(out["bin"], ob)
+    assert ob["culled"][5] and ob["culled"][6]
+    assert_images(out["img"], oracle.render(sc, camv, cfg))
+    og = oracle.backward(sc, camv, cfg, up)
+    assert_grads(out["grads"], og, max_bad=5e-3)
+    assert_pose(out["pose"], og["pose"])
+
+
+def test_invalid_arguments(ren):
+    sc, cams, _ = scenegen.make_config("C1")
+    t, sf = to_device(sc)
+    bad = sgs.make_camera(0, 48, 60, 60, 32, 24, np.eye(4)[:3])
+    with pytest.raises(sgs.SgsError) as e:
+        ren.render(sf, bad)
+    assert e.value.status == sgs.SGS_INVALID_ARGUMENT
+    fresh = sgs.Renderer()
+    with pytest.raises(sgs.SgsError) as e:
+        fresh.backward(d_pose6=torch.zeros(6, device="cuda"))
+    assert e.value.status == sgs.SGS_NO_FORWARD_STATE
+    fresh.close()
+
+
+def test_async_mode_and_host_path():
+    """SGS_FLAG_ASYNC gives the same result without a host sync; the HOST-buffer calls equal the device calls."""
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    up = scenegen.upstream_normal(6, cam.height, cam.width)
+    sync = sgs.Renderer()
+    ref = run_gpu(sync, sc, cam, up)
+    a = sgs.Renderer(async_mode=True)
+    for _ in range(3):
+        out = run_gpu(a, sc, cam, up)
+    assert np.array_equal(out["img"], ref["img"]) and np.array_equal(out["bin"]["keys"], ref["bin"]["keys"])
+    # host path
+    pin = lambda x, dt=torch.float32: torch.from_numpy(np.ascontiguousarray(x)).to(dt).pin_memory()
+    a.upload_surfels(pin(sc.mean), pin(sc.scale), pin(sc.quat), pin(sc.opacity), pin(sc.rgb))
+    c = camera(cam)
+    H, W = cam.height, cam.width
+    h = dict(rgb=torch.zeros(3, H, W).pin_memory(), depth=torch.zeros(1, H, W).pin_memory(),
+             normal=torch.zeros(3, H, W).pin_memory(), alpha=torch.zeros(1, H, W).pin_memory())
+    a.render_host(c, **h)
+    himg = torch.cat([h["rgb"], h["depth"], h["normal"], h["alpha"]], 0).numpy().astype(np.float64)
+    assert np.array_equal(himg, ref["img"])
+    u = torch.from_numpy(up)
+    hg = {k: torch.zeros(v.shape).pin_memory() for k, v in ref["grads"].items()}
+    hp = torch.zeros(6).pin_memory()
+    a.backward_host(d_rgb=u[0:3].contiguous(), d_depth=u[3:4].contiguous(), d_normal=u[4:7].contiguous(),
+                    d_alpha=u[7:8].contiguous(), grads=hg, d_pose6=hp)
+    for k in hg:
+        np.testing.assert_allclose(hg[k].numpy(), ref["grads"][k], rtol=1e-4, atol=1e-4 * np.abs(ref["grads"][k]).max())
+    np.testing.assert_allclose(hp.numpy(), ref["pose"], rtol=1e-4)
+    # tracking iteration on resident map/target
+    a.upload_target(c, h["rgb"] * 0.9, h["depth"] * 1.01)
+    loss, p6 = a.track_iter_host(c, 0.5, 1.0)
+    assert np.isfinite(loss) and np.isfinite(p6).all()
+    sync.close(); a.close()
