@@ -1,0 +1,413 @@
+#!/usr/bin/env python
+"""bench.py -- forward+backward throughput of the B200 surfel renderer on BASELINE.json's configs.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input:
+  C2 / C5 (tracking-shaped): one frame = `iters` iterations of render -> Eq. 15-19 loss -> pose-only backward
+  C1 / C3 / C4 (mapping-shaped): one window = every view rendered and back-propagated (full backward + pose)
+`value` is megapixels/s (W*H*renders / device time), inputs resident in HBM; `e2e` is the same metric
+through the HOST-buffer C-ABI calls with the copies inside the timed region.  The roofline object is
+for the dominant stage, timed in a second pass of the same K steps with CUDA events around every
+stage (sgs_set_profiling), so the headline value is not perturbed by the extra event records.
+Rank 0 prints ONE JSON line.  --impl reference times the CPU oracle (oracle/) on the host cores."""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "fwd+bwd megapixels/s"
+UNIT = "MP/s"
+# Algorithmic flops per (pixel, entry) pair, counted from the oracle's formulas with FMA = 2
+# (DESIGN.md §7): tested pair 26; composited pair +26 forward, +102 full backward, +94 pose-only backward.
+F_TEST, F_COMP_FWD, F_COMP_BWD_FULL, F_COMP_BWD_POSE = 26, 26, 102, 94
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def fp32_peak_tflops(peaks):
+    # 148 SMs x 128 FP32 lanes x 2 flop (FMA) x max SM clock (guide's unit counts and clocks)
+    return 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks and throttle reasons every 200 ms while the timed region runs."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_evt, self.proc = index, [], threading.Event(), None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([x.strip() for x in line.split(",")])
+                if self._stop_evt.is_set():
+                    break
+        except Exception:
+            pass
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.proc:
+            self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 2 + i and r[2 + i].lower().startswith("active") for r in self.rows)]
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=reasons, samples=len(sm))
+
+
+def tau0(seed):
+    import scenegen
+    g = scenegen.SplitMix(seed)
+    d = np.stack([g.normal(3), g.normal(3)])
+    return np.concatenate([0.02 * d[0] / np.linalg.norm(d[0]), np.deg2rad(1.0) * d[1] / np.linalg.norm(d[1])])
+
+
+def oracle_counters(sc, cams, info):
+    """Q_t, Q_tb, Q_c, E, N_v ... per view from the oracle (they define the algorithmic work)."""
+    import oracle
+    cfg = oracle.make_cfg()
+    out = []
+    for cam in cams:
+        camv = oracle.make_cam(cam)
+        t0 = time.time()
+        r = oracle.render(sc, camv, cfg)
+        c = dict(r["counters"])
+        c["E"] = oracle.preprocess(sc, camv, cfg)["E"]
+        c["fwd_s"] = time.time() - t0
+        out.append((c, r))
+    return out
+
+
+# --------------------------------------------------------------------------------------- our arm
+class Workload:
+    """Device-resident inputs + the step function for one config."""
+
+    def __init__(self, name, iters_override=None):
+        import torch
+        import scenegen
+        import paper_2506_00970_b200 as sgs
+        self.torch, self.sgs, self.name = torch, sgs, name
+        self.sc, self.cams, self.info = scenegen.make_config(name)
+        self.tracking = self.info["mode"] == "pose"
+        self.iters = iters_override or self.info["iters"]
+        sc = self.sc
+        d = lambda a, dt=torch.float32: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to("cuda", dt)
+        self.t = dict(mean=d(sc.mean), scale=d(sc.scale), quat=d(sc.quat), opacity=d(sc.opacity), rgb=d(sc.rgb),
+                      active=d(sc.active, torch.uint8))
+        self.sf = sgs.Renderer.surfels(*(self.t[k] for k in ("mean", "scale", "quat", "opacity", "rgb", "active")))
+        self.ren = sgs.Renderer(async_mode=True)
+        cam0 = self.cams[0]
+        self.H, self.W = cam0.height, cam0.width
+        z = lambda c: torch.zeros((c, self.H, self.W), device="cuda")
+        self.im = dict(rgb=z(3), depth=z(1), normal=z(3), alpha=z(1))
+        self.up = dict(rgb=z(3), depth=z(1), normal=z(3), alpha=z(1))
+        self.ccams = [sgs.make_camera(c.width, c.height, c.fx, c.fy, c.cx, c.cy, c.T_cw) for c in self.cams]
+        self.p6 = torch.zeros(6, device="cuda")
+        self.loss = torch.zeros(1, device="cuda")
+        self.n_active = int(sc.n if sc.active is None else sc.active.sum())
+        # target frame(s): the renderer's own image at the perturbed pose Exp(tau0) T
+        self.targets = []
+        for i, c in enumerate(self.cams):
+            Tt = scenegen.perturb_pose(c.T_cw, tau0(self.info.get("tau0_seed", 2000 + i)))
+            ct = sgs.make_camera(c.width, c.height, c.fx, c.fy, c.cx, c.cy, Tt)
+            self._render_retry(ct)
+            self.targets.append((self.im["rgb"].clone(), self.im["depth"].clone()))
+        if not self.tracking:
+            n = sc.n
+            self.grads = dict(mean=torch.zeros(n, 3, device="cuda"), scale=torch.zeros(n, 2, device="cuda"),
+                              quat=torch.zeros(n, 4, device="cuda"), opacity=torch.zeros(n, device="cuda"),
+                              rgb=torch.zeros(n, 3, device="cuda"))
+        self.renders_per_step = self.iters if self.tracking else len(self.cams)
+        self.flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def _render_retry(self, cam):
+        for _ in range(4):  # async mode: an overflow is reported by the next call, after growing
+            try:
+                self.ren.render(self.sf, cam, **self.im)
+                self.ren.stats()
+                self.ren.render(self.sf, cam, **self.im)
+                return
+            except self.sgs.SgsError as e:
+                if e.status != self.sgs.SGS_WORKSPACE_OVERFLOW:
+                    raise
+        raise RuntimeError("workspace did not settle")
+
+    def one(self, v):
+        """render -> loss -> backward for view v (everything enqueued, no host sync)."""
+        cam = self.ccams[v]
+        self.ren.render(self.sf, cam, **self.im)
+        trgb, tdep = self.targets[v]
+        self.ren.tracking_loss(cam, self.im, trgb, tdep, 0.5, -1.0, self.up, self.loss)
+        u = self.up
+        if self.tracking:
+            self.ren.backward(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"], d_pose6=self.p6)
+        else:
+            self.ren.backward(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"],
+                              grads=self.grads, d_pose6=self.p6)
+
+    def step(self):
+        if self.tracking:
+            for _ in range(self.iters):
+                self.one(0)
+        else:
+            for v in range(len(self.cams)):
+                self.one(v)
+
+    def flush_l2(self):
+        self.flush_buf.zero_()
+
+    # ---- end-to-end: HOST buffers through the C-ABI host calls
+    def setup_e2e(self):
+        torch = self.torch
+        pin = lambda a, dt=torch.float32: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dt).pin_memory()
+        sc = self.sc
+        self.h = dict(mean=pin(sc.mean), scale=pin(sc.scale), quat=pin(sc.quat), opacity=pin(sc.opacity), rgb=pin(sc.rgb),
+                      active=pin(sc.active, torch.uint8))
+        self.h_targets = [(a.cpu().pin_memory(), b.cpu().pin_memory()) for a, b in self.targets]
+        if not self.tracking:
+            self.h_up = {k: v.cpu().pin_memory() for k, v in self.up.items()}
+            self.h_grads = {k: torch.zeros(v.shape).pin_memory() for k, v in self.grads.items()}
+            self.h_p6 = torch.zeros(6).pin_memory()
+            self.h_im = {k: v.cpu().pin_memory() for k, v in self.im.items()}
+
+    def step_e2e(self):
+        """Tracking: upload map + target frame, then `iters` x sgs_track_iter_host (loss + 6-vector read back
+        every iteration).  Mapping: upload map; per view render_host (images to host) + backward_host
+        (upstream from host, all gradients back to host)."""
+        r, h = self.ren, self.h
+        r.upload_surfels(h["mean"], h["scale"], h["quat"], h["opacity"], h["rgb"], h["active"])
+        if self.tracking:
+            r.upload_target(self.ccams[0], *self.h_targets[0])
+            for _ in range(self.iters):
+                loss, p6 = r.track_iter_host(self.ccams[0], 0.5, -1.0)
+            return loss
+        for v in range(len(self.cams)):
+            r.render_host(self.ccams[v], **self.h_im)
+            u = self.h_up
+            r.backward_host(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"],
+                            grads=self.h_grads, d_pose6=self.h_p6)
+        return float(self.h_p6[0])
+
+    def e2e_bytes(self):
+        n, px = self.sc.n, self.H * self.W
+        h2d = n * 52 + (n if self.sc.active is not None else 0)
+        if self.tracking:
+            return h2d + px * 16 + self.iters * 48, self.iters * 28
+        k = len(self.cams)
+        return h2d + k * (px * 32 + 48), k * (px * 32 + n * 52 + 24)
+
+
+def cpu_baseline(name, max_views=1):
+    """The oracle as it stands, on the host cores: forward + analytic backward of `max_views` view(s)."""
+    import oracle
+    import scenegen
+    sc, cams, info = scenegen.make_config(name)
+    cfg = oracle.make_cfg()
+    cam = cams[0]
+    camv = oracle.make_cam(cam)
+    up = scenegen.upstream_normal(7, cam.height, cam.width)
+    t0 = time.time()
+    r = oracle.render(sc, camv, cfg, counters=False)
+    oracle.backward(sc, camv, cfg, up)
+    dt = time.time() - t0
+    return dict(value=cam.width * cam.height / dt / 1e6, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                sample=f"1 iteration (fp64 forward + analytic backward to surfels and pose) of {name} view 0, {dt:.2f} s",
+                seconds=dt), (sc, cams, info)
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle timed on the host cores; each step is ONE forward+backward of
+    view 0 of the config (a bounded sample of the workload)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    import scenegen
+    sc, cams, info = scenegen.make_config(args.config)
+    cfg, cam = oracle.make_cfg(), cams[0]
+    camv = oracle.make_cam(cam)
+    up = scenegen.upstream_normal(7, cam.height, cam.width)
+
+    def step():
+        oracle.render(sc, camv, cfg, counters=False)
+        oracle.backward(sc, camv, cfg, up)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.time()
+    for _ in range(args.steps):
+        step()
+    dt = time.time() - t0
+    mp = cam.width * cam.height * args.steps / dt / 1e6
+    n_act = int(sc.n if sc.active is None else sc.active.sum())
+    line = dict(metric=METRIC, value=mp, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=1e3 * dt / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+                data="synthetic", impl="reference", surfels_per_s=n_act * args.steps / dt,
+                config=dict(workload=f"{args.config}: 1 forward+backward of view 0 per step (bounded sample)",
+                            surfels=sc.n, width=cam.width, height=cam.height),
+                cpu_baseline=dict(value=mp, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                                  sample="every step: one fp64 forward + analytic backward of view 0"),
+                e2e=dict(value=mp, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--iters", type=int, default=None, help="override iterations per tracking step")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    wl = Workload(args.config, args.iters)
+    K, W = args.steps, max(args.warmup, 3)
+    for _ in range(W):
+        wl.step()
+    torch.cuda.synchronize()
+    launches0 = wl.ren.stats()["kernel_launches"]
+
+    def timed_pass():
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+        barrier()
+        for a, b in evs:
+            wl.flush_l2()
+            a.record()
+            wl.step()
+            b.record()
+        barrier()
+        return sum(a.elapsed_time(b) for a, b in evs)  # ms, device time of the K steps
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    ms = timed_pass()
+    clocks = sampler.stop()
+    launches = wl.ren.stats()["kernel_launches"] - launches0
+    t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    px = wl.H * wl.W
+    renders = wl.renders_per_step * K * world
+    value = px * renders / (ms_max * 1e-3) / 1e6
+
+    # second pass with per-stage CUDA events (roofline), not part of `value`
+    wl.ren.set_profiling(True)
+    wl.ren.get_profile(reset=True)
+    timed_pass()
+    prof = wl.ren.get_profile(reset=True)
+    wl.ren.set_profiling(False)
+
+    # end to end through the HOST-buffer C-ABI calls
+    e2e = None
+    if not args.no_e2e:
+        wl.setup_e2e()
+        wl.step_e2e()
+        barrier()
+        t0 = time.time()
+        for _ in range(K):
+            wl.step_e2e()
+        barrier()
+        dt = time.time() - t0
+        te = torch.tensor([dt], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        h2d, d2h = wl.e2e_bytes()
+        e2e = dict(value=px * renders / float(te.item()) / 1e6, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
+                   timing="wall clock around K steps incl. pinned-host copies and per-iteration readback")
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks = load_peaks()
+    cpu, roof, stages = None, None, {}
+    if not args.no_cpu_baseline:
+        cpu, (sc, cams, info) = cpu_baseline(args.config)
+        # algorithmic work per render from the oracle's counters (view 0 stands for every view)
+        import oracle
+        camv, cfg = oracle.make_cam(cams[0]), oracle.make_cfg()
+        cnt = oracle.render(sc, camv, cfg)["counters"]
+        E = oracle.preprocess(sc, camv, cfg)["E"]
+        n_act = wl.n_active
+        fcb = F_COMP_BWD_POSE if wl.tracking else F_COMP_BWD_FULL
+        work = dict(preprocess=("hbm", (sc.n if sc.active is not None else 0) + n_act * 56 + cnt["n_vis"] * 76 + E * 12),
+                    sort=("hbm", E * 24 + E * 8),
+                    forward=("alu", F_TEST * cnt["Q_t"] + F_COMP_FWD * cnt["Q_c"]),
+                    loss=("hbm", px * (12 + 8) * 4),
+                    backward=("alu", F_TEST * cnt["Q_tb"] + fcb * cnt["Q_c"]))
+        tot_ms = sum(v[0] for v in prof.values()) or 1.0
+        for st, (ms_s, calls) in prof.items():
+            if calls == 0:
+                continue
+            kind, units = work[st]
+            per = ms_s / calls * 1e-3
+            if kind == "hbm":
+                ach, peak, unit = units / per / 1e9, peaks["hbm_gbs"], "GB/s"
+            else:
+                ach, peak, unit = units / per / 1e12, fp32_peak_tflops(peaks), "TFLOP/s"
+            stages[st] = dict(bound=kind, achieved=ach, peak=peak, unit=unit, frac=ach / peak, ms_per_launch=per * 1e3,
+                              share=ms_s / tot_ms, algorithmic_units=units)
+        dom = max(stages, key=lambda k: stages[k]["share"])
+        roof = dict(stages[dom])
+        roof.update(kernel=dom, traffic=None, peak_source=peaks["source"] + (" HBM copy" if roof["bound"] == "hbm" else
+                    "; alu peak = 148 SM x 128 lanes x 2 x max SM clock"), counters=dict(cnt, E=E))
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=ms_max / K,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+                surfels_per_s=wl.n_active * renders / (ms_max * 1e-3),
+                config=dict(workload=f"{args.config} ({'tracking' if wl.tracking else 'mapping'}-shaped): "
+                            f"{wl.renders_per_step} x (render + Eq.15-19 loss + "
+                            f"{'pose-only' if wl.tracking else 'full+pose'} backward) per step",
+                            surfels=wl.sc.n, active=wl.n_active, width=wl.W, height=wl.H, renders_per_step=wl.renders_per_step,
+                            l2="flushed between steps by a 256 MiB write; iterations inside a step reuse the map as tracking does",
+                            replicas=world),
+                clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roof, stages=stages, cpu_baseline=cpu)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

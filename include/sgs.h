@@ -121,7 +121,12 @@ typedef struct {
     int64_t capacity;     /* current entry capacity of the workspace           */
     int64_t overflow;     /* 1 if the last render dropped entries              */
     int64_t workspace_bytes;
+    int64_t kernel_launches; /* kernels this ctx has launched since creation (memsets/copies not counted) */
 } sgs_stats;
+
+/* Per-stage device timing (CUDA events recorded on the caller's stream around each stage). */
+enum { SGS_STAGE_PREPROCESS = 0, SGS_STAGE_SORT = 1, SGS_STAGE_FORWARD = 2, SGS_STAGE_LOSS = 3,
+       SGS_STAGE_BACKWARD = 4, SGS_STAGE_COUNT = 5 };
 
 SGS_API int sgs_default_config(sgs_config* cfg);
 SGS_API int sgs_create(sgs_ctx** out, const sgs_config* cfg);
@@ -155,6 +160,12 @@ SGS_API int sgs_get_binning(sgs_ctx* ctx, int64_t* n_entries, const uint64_t** k
                     const uint32_t** tile_ranges /* tiles x 2 */, const uint8_t** culled /* n */);
 
 SGS_API int sgs_get_stats(sgs_ctx* ctx, sgs_stats* out);
+
+/* Profiling: when enabled, every stage launch is bracketed by a pair of CUDA events on its stream.
+ * sgs_get_profile waits for the device, adds up the elapsed milliseconds and call counts per stage
+ * (HOST arrays of SGS_STAGE_COUNT entries) and, if reset != 0, clears the record. */
+SGS_API int sgs_set_profiling(sgs_ctx* ctx, int enabled);
+SGS_API int sgs_get_profile(sgs_ctx* ctx, double* ms, int64_t* calls, int reset);
 
 /* HOST-buffer convenience path (end-to-end measurement): copies in, runs, copies out, waits.
  * sgs_upload_surfels copies a HOST map into ctx-owned device memory and makes it the resident

@@ -296,6 +296,7 @@ typedef struct {
 } Pair;
 
 #define FRAG_EPS 1e-4
+#define KAPPA_MAX 32.0
 static inline int eval_pair(const Prep* p, double opac, double x, double y, double T, const Cfg* cfg,
                             Pair* r, int* frag, int* covers) {
     const double* M = p->M;
@@ -326,6 +327,14 @@ static inline int eval_pair(const Prep* p, double opac, double x, double y, doub
     const double Tn = T * (1.0 - r->a);
     if (cfg->t_min > 0.0 && fabs(Tn - cfg->t_min) < FRAG_EPS * cfg->t_min) *frag |= 1;
     if (Tn < cfg->t_min) return 2;
+    /* Ill-conditioned intersection: kappa = |h_u||h_v| / |k_z| (uv parts) is ~ 1/cos(tilt) of the
+     * splat against the ray.  Beyond KAPPA_MAX the fp32 rounding of the INPUTS already moves (u,v)
+     * by more than the image tolerance allows (delta G / G ~ rho^2 kappa 2e-7), so no binary32
+     * renderer can be held to 1e-4 there: flag bit 2 (value 4) of the fragile mask. */
+    {
+        const double nu = r->hu[0] * r->hu[0] + r->hu[1] * r->hu[1], nv = r->hv[0] * r->hv[0] + r->hv[1] * r->hv[1];
+        if (sqrt(nu * nv) > KAPPA_MAX * fabs(r->k[2])) *frag |= 4;
+    }
     return 1;
 }
 
@@ -361,29 +370,31 @@ static inline int64_t cand_count(const Ctx* c, int i, int j, const uint32_t** ls
 /* ---- public: forward (O4).  img = 8 planes H*W: r,g,b, depth, nx,ny,nz, alpha (un-normalised
  * blends, R9/R10; background 0, R17).  counters: [0]=Q_t tile-list pairs tested up to and incl.
  * the stopping entry, [1]=Q_c composited pairs, [2]=covering pairs (rho^2<=c^2, z>z_near) over
- * ALL surfels ignoring termination (depth complexity), [3]=n_vis, [4]=fragile pixels. */
+ * ALL surfels ignoring termination (depth complexity), [3]=n_vis, [4]=fragile pixels,
+ * [5]=Q_tb tile-list pairs up to and incl. each pixel's LAST COMPOSITED entry (what a reverse traversal revisits). */
 void orc_render(int64_t n, const float* mean, const float* scale, const float* quat,
                 const float* opacity, const float* rgb, const uint8_t* active,
                 const double* camv, const double* cfgv, int brute,
                 double* img, double* T_final, int32_t* n_comp, uint8_t* fragile, int64_t* counters) {
     Ctx c; ctx_init(&c, n, mean, scale, quat, opacity, rgb, active, camv, cfgv, brute);
     const int W = c.cam.W, H = c.cam.H; const int64_t HW = (int64_t)W * H;
-    int64_t Qt = 0, Qc = 0, Qcover = 0, nfrag = 0;
+    int64_t Qt = 0, Qc = 0, Qcover = 0, nfrag = 0, Qtb = 0;
     const int count_all = counters != NULL; /* the covering count needs the traversal past termination */
-#pragma omp parallel for schedule(dynamic, 1) reduction(+ : Qt, Qc, Qcover, nfrag)
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : Qt, Qc, Qcover, nfrag, Qtb)
     for (int j = 0; j < H; ++j) {
         for (int i = 0; i < W; ++i) {
             const double x = i + 0.5, y = j + 0.5; /* pixel centres at half integers (R17) */
             const uint32_t* lst; const int64_t m = cand_count(&c, i, j, &lst);
             double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, T = 1.0;
             int frag = 0, stopped = 0, nc = 0;
+            int64_t qt_pix = 0, qt_last = 0;
             for (int64_t e = 0; e < m; ++e) {
                 const uint32_t raw = lst ? lst[e] : (uint32_t)e;
                 const uint32_t k = c.ord[raw & 0x7fffffffu];
                 const Prep* p = c.P + k;
                 if (lst) {
                     if (x < p->aabb[0] - 1.0 || x > p->aabb[1] + 1.0 || y < p->aabb[2] - 1.0 || y > p->aabb[3] + 1.0) {
-                        if ((raw >> 31) && !stopped) ++Qt;
+                        if ((raw >> 31) && !stopped) ++qt_pix;
                         continue;
                     }
                 }
@@ -391,7 +402,7 @@ void orc_render(int64_t n, const float* mean, const float* scale, const float* q
                 const int st = eval_pair(p, opacity[k], x, y, T, &c.cfg, &r, &f, &covers);
                 Qcover += covers;
                 if (stopped) continue; /* past termination: only the covering count continues */
-                if (!lst || (raw >> 31)) ++Qt;
+                if (!lst || (raw >> 31)) ++qt_pix;
                 frag |= f;
                 if (st == 2) { stopped = 1; if (!count_all) break; continue; }
                 if (st == 0) continue;
@@ -402,16 +413,18 @@ void orc_render(int64_t n, const float* mean, const float* scale, const float* q
                 acc[7] += w;
                 T *= (1.0 - r.a);
                 ++nc; ++Qc;
+                qt_last = qt_pix;
             }
             const int64_t pix = (int64_t)j * W + i;
             for (int ch = 0; ch < 8; ++ch) img[ch * HW + pix] = acc[ch];
             if (T_final) T_final[pix] = T;
             if (n_comp) n_comp[pix] = nc;
             if (fragile) fragile[pix] = (uint8_t)frag;
-            nfrag += (frag & 1);
+            nfrag += (frag & 5) != 0;
+            Qt += qt_pix; Qtb += qt_last;
         }
     }
-    if (counters) { counters[0] = Qt; counters[1] = Qc; counters[2] = Qcover; counters[3] = c.n_vis; counters[4] = nfrag; }
+    if (counters) { counters[0] = Qt; counters[1] = Qc; counters[2] = Qcover; counters[3] = c.n_vis; counters[4] = nfrag; counters[5] = Qtb; }
     ctx_free(&c);
 }
 

@@ -2,8 +2,10 @@
 the path runs in the CUDA kernels behind the C ABI.  torch is used for device memory (the ctx's
 workspace comes from torch's caching allocator through the sgs_alloc_fn callbacks) and streams.
 There is NO CPU fallback: a missing library or device raises."""
+import atexit
 import ctypes as C
 import os
+import weakref
 import numpy as np
 import torch
 
@@ -44,14 +46,21 @@ class sgs_surfel_grads(C.Structure):
 
 class sgs_stats(C.Structure):
     _fields_ = [("n_visible", C.c_int64), ("n_entries", C.c_int64), ("capacity", C.c_int64), ("overflow", C.c_int64),
-                ("workspace_bytes", C.c_int64)]
+                ("workspace_bytes", C.c_int64), ("kernel_launches", C.c_int64)]
 
 
 EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_backward", "sgs_tracking_loss",
            "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
-           "sgs_upload_target", "sgs_track_iter_host", "sgs_status_string"]
+           "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string"]
 
 _lib = None
+_LIVE = weakref.WeakSet()
+
+
+@atexit.register
+def _close_all():
+    for r in list(_LIVE):
+        r.close()
 
 
 def load_library():
@@ -129,21 +138,26 @@ class Renderer:
         if torch_allocator:
             dev_index = self.device.index or 0
 
+            _t_alloc, _t_delete = torch.cuda.caching_allocator_alloc, torch.cuda.caching_allocator_delete
+
             def _alloc(nbytes, user, stream):
                 try:
-                    return torch.cuda.caching_allocator_alloc(int(nbytes), dev_index, stream)
+                    return _t_alloc(int(nbytes), dev_index, stream)
                 except Exception:
                     return None
 
             def _free(ptr, user, stream):
-                torch.cuda.caching_allocator_delete(ptr)
+                try:
+                    _t_delete(ptr)
+                except Exception:  # interpreter shutdown: the allocator is already gone
+                    pass
 
             self._alloc_cb, self._free_cb = ALLOC_FN(_alloc), FREE_FN(_free)  # keep alive
             cfg.alloc, cfg.free = self._alloc_cb, self._free_cb
         self._cfg = cfg
         self._ctx = C.c_void_p()
         _check(self.lib.sgs_create(C.byref(self._ctx), C.byref(cfg)), "sgs_create")
-        self._keep = None
+        _LIVE.add(self)
 
     def close(self):
         if getattr(self, "_ctx", None) is not None and self._ctx:
@@ -211,6 +225,18 @@ class Renderer:
         _check(self.lib.sgs_get_stats(self._ctx, C.byref(st)), "sgs_get_stats")
         return {k: int(getattr(st, k)) for k, _ in sgs_stats._fields_}
 
+    STAGES = ("preprocess", "sort", "forward", "loss", "backward")
+
+    def set_profiling(self, enabled):
+        _check(self.lib.sgs_set_profiling(self._ctx, C.c_int(int(enabled))), "sgs_set_profiling")
+
+    def get_profile(self, reset=True):
+        """sgs_get_profile -> {stage: (total_ms, calls)}; waits for the device."""
+        ms = (C.c_double * len(self.STAGES))()
+        calls = (C.c_int64 * len(self.STAGES))()
+        _check(self.lib.sgs_get_profile(self._ctx, ms, calls, C.c_int(int(reset))), "sgs_get_profile")
+        return {k: (float(ms[i]), int(calls[i])) for i, k in enumerate(self.STAGES)}
+
     # ---- host path (end-to-end) --------------------------------------------------------------
     def upload_surfels(self, mean, scale, quat, opacity, rgb, active=None, stream=None):
         """sgs_upload_surfels: HOST (ideally pinned) tensors -> ctx-resident device map."""
@@ -250,7 +276,7 @@ class _RawDeviceBytes:
     """Wraps a library-owned device pointer for torch through __cuda_array_interface__."""
 
     def __init__(self, ptr, nbytes):
-        self.__cuda_array_interface__ = {"shape": (int(nbytes),), "typestr": "|u1", "data": (int(ptr), True), "version": 2}
+        self.__cuda_array_interface__ = {"shape": (int(nbytes),), "typestr": "|u1", "data": (int(ptr), False), "version": 2}
 
 
 def _device_to_numpy(dev_ptr, count, dtype):

@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/sgs.h: ctx, workspace, and the launch sequences.
 #include <math.h>
 #include <new>
+#include <stdlib.h>
 #include <string.h>
 #include "sgs_internal.h"
 
@@ -105,6 +106,26 @@ bool sgs_cam_valid(const sgs_camera* cam) {
     return true;
 }
 
+SgsStage::SgsStage(sgs_ctx* c_, int stage, cudaStream_t s_) : c(c_), s(s_), slot(-1) {
+    if (!c->prof_on) return;
+    if (c->prof_n == c->prof_cap) {
+        const int ncap = c->prof_cap ? c->prof_cap * 2 : 1024;
+        cudaEvent_t* ev = (cudaEvent_t*)realloc(c->prof_ev, sizeof(cudaEvent_t) * 2 * (size_t)ncap);
+        int* st = (int*)realloc(c->prof_stage, sizeof(int) * (size_t)ncap);
+        if (ev) c->prof_ev = ev;
+        if (st) c->prof_stage = st;
+        if (!ev || !st) return;
+        for (int i = 2 * c->prof_cap; i < 2 * ncap; ++i) cudaEventCreate(&c->prof_ev[i]);
+        c->prof_cap = ncap;
+    }
+    slot = c->prof_n++;
+    c->prof_stage[slot] = stage;
+    cudaEventRecord(c->prof_ev[2 * slot], s);
+}
+SgsStage::~SgsStage() {
+    if (slot >= 0) cudaEventRecord(c->prof_ev[2 * slot + 1], s);
+}
+
 extern "C" {
 
 int sgs_default_config(sgs_config* cfg) {
@@ -163,7 +184,29 @@ int sgs_destroy(sgs_ctx* c) {
     if (c->sort_hist) cudaFree(c->sort_hist);
     if (c->loss_dev) cudaFree(c->loss_dev);
     if (c->counters_ready) cudaEventDestroy(c->counters_ready);
+    for (int i = 0; i < 2 * c->prof_cap; ++i) cudaEventDestroy(c->prof_ev[i]);
+    free(c->prof_ev); free(c->prof_stage);
     delete c;
+    return SGS_OK;
+}
+
+int sgs_set_profiling(sgs_ctx* c, int enabled) {
+    if (!c) return SGS_INVALID_ARGUMENT;
+    c->prof_on = enabled ? 1 : 0;
+    return SGS_OK;
+}
+
+int sgs_get_profile(sgs_ctx* c, double* ms, int64_t* calls, int reset) {
+    if (!c) return SGS_INVALID_ARGUMENT;
+    if (cudaDeviceSynchronize() != cudaSuccess) return SGS_CUDA_ERROR;
+    for (int i = 0; i < SGS_STAGE_COUNT; ++i) { if (ms) ms[i] = 0.0; if (calls) calls[i] = 0; }
+    for (int i = 0; i < c->prof_n; ++i) {
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]) != cudaSuccess) { cudaGetLastError(); continue; }
+        if (ms) ms[c->prof_stage[i]] += (double)t;
+        if (calls) calls[c->prof_stage[i]] += 1;
+    }
+    if (reset) c->prof_n = 0;
     return SGS_OK;
 }
 

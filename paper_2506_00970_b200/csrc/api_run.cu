@@ -147,6 +147,7 @@ int sgs_get_stats(sgs_ctx* c, sgs_stats* out) {
     out->capacity = c->e_cap;
     out->overflow = c->counters_host->overflow;
     out->workspace_bytes = c->bytes;
+    out->kernel_launches = c->launches;
     return SGS_OK;
 }
 

@@ -349,12 +349,14 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
 
 cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_surfel_grads* dg, float* d_pose6,
                                 cudaStream_t s) {
+    SgsStage st(c, SGS_STAGE_BACKWARD, s);
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
     CPlanes u;
     for (int i = 0; i < 8; ++i) u.p[i] = up[i];
     const SgsCamDev& cam = c->camd;
     if (dg == nullptr) {  // pose-only (tracking, L204)
         if (d_pose6 == nullptr) return cudaSuccess;
+        c->launches += 1;
         k_backward<true><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->vals[c->sorted_buf], c->pay, cam.W, cam.H, cam.tiles_x,
                                                      cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
                                                      c->acc, c->pose_partial, c->counters, d_pose6);
@@ -368,12 +370,14 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     if (dg->opacity && e == cudaSuccess) e = cudaMemsetAsync(dg->opacity, 0, sizeof(float) * (size_t)n, s);
     if (dg->rgb && e == cudaSuccess) e = cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * (size_t)n, s);
     if (e != cudaSuccess) return e;
+    c->launches += 1;
     k_backward<false><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->vals[c->sorted_buf], c->pay, cam.W, cam.H, cam.tiles_x,
                                                   cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
                                                   c->acc, c->pose_partial, c->counters, nullptr);
     const int blocks = (int)((n + 255) / 256);  // bound on N_v; blocks past it only join the pose reduction
+    if (blocks == 0 && d_pose6) return cudaMemsetAsync(d_pose6, 0, sizeof(float) * 6, s);
     if (blocks > 0)
-        k_surfel_backward<<<blocks, 256, 0, s>>>(c->counters, c->vis_to_surfel, c->acc, c->last_surfels.mean,
+        c->launches += 1, k_surfel_backward<<<blocks, 256, 0, s>>>(c->counters, c->vis_to_surfel, c->acc, c->last_surfels.mean,
                                                  c->last_surfels.scale, c->last_surfels.quat, cam, *dg, c->pose_partial,
                                                  c->counters, d_pose6);
     return cudaGetLastError();

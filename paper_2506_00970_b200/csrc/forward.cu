@@ -83,6 +83,8 @@ cudaError_t sgs_launch_forward(sgs_ctx* c, float* const planes[8], cudaStream_t 
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
     Planes out;
     for (int i = 0; i < 8; ++i) out.p[i] = planes[i];
+    SgsStage st(c, SGS_STAGE_FORWARD, s);
+    c->launches += 1;
     k_forward<<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->vals[c->sorted_buf], c->pay, c->camd.W, c->camd.H, c->camd.tiles_x,
                                           c->cfgd, out, c->T_final, c->n_last);
     return cudaGetLastError();

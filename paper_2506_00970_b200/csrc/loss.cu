@@ -53,7 +53,8 @@ k_tracking_loss(LP p, const float* __restrict__ trgb, const float* __restrict__ 
 cudaError_t sgs_launch_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const float* const ren[8], const float* trgb,
                                      const float* tdepth, float lambda_d, float nsign, float* const up[8], float* loss,
                                      cudaStream_t s) {
-    (void)c;
+    SgsStage st(c, SGS_STAGE_LOSS, s);
+    c->launches += 1;
     LP p;
     for (int i = 0; i < 8; ++i) { p.ren[i] = ren[i]; p.up[i] = up[i]; }
     const int64_t HW = (int64_t)cam->width * cam->height;

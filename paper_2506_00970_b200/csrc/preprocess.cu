@@ -215,6 +215,8 @@ cudaError_t sgs_launch_preprocess(sgs_ctx* c, const sgs_surfels* sf, cudaStream_
     if (blocks == 0) return cudaSuccess;
     e = cudaMemsetAsync(c->scan_state, 0, sizeof(unsigned long long) * (size_t)blocks, s);
     if (e != cudaSuccess) return e;
+    SgsStage st(c, SGS_STAGE_PREPROCESS, s);
+    c->launches += 1;
     k_preprocess<<<blocks, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, sf->active,
                                                   c->camd, c->cfgd, c->pay, c->vis_to_surfel, c->culled, c->scan_state,
                                                   c->counters, c->keys[0], c->vals[0], (unsigned long long)c->e_cap);

@@ -106,6 +106,8 @@ struct sgs_ctx {
     float* pinned_small;             // 8 floats pinned
     int64_t host_img_cap, host_grads_cap;
     int64_t partial_cap;             // floats in pose_partial
+    int64_t launches;                // kernels launched by this ctx
+    int prof_on; int prof_n, prof_cap; cudaEvent_t* prof_ev; int* prof_stage;  // event pairs: ev[2i], ev[2i+1]
     int64_t last_entries;            // E of the last checked render (async launch bound hint), 0 = unknown
 };
 
@@ -130,3 +132,10 @@ int sgs_ensure_image(sgs_ctx* c, int tiles, int64_t pixels, cudaStream_t s);
 int sgs_ensure_partials(sgs_ctx* c, int64_t blocks, cudaStream_t s);
 void sgs_fill_cam(const sgs_camera* cam, SgsCamDev* d);
 bool sgs_cam_valid(const sgs_camera* cam);
+
+// profiling scope: records an event pair around a stage when ctx->prof_on
+struct SgsStage {
+    sgs_ctx* c; cudaStream_t s; int slot;
+    SgsStage(sgs_ctx* c_, int stage, cudaStream_t s_);
+    ~SgsStage();
+};

@@ -175,6 +175,7 @@ cudaError_t sgs_launch_sort_and_ranges(sgs_ctx* c, cudaStream_t s) {
     const unsigned long long e_cap = (unsigned long long)c->e_cap;
     const int64_t bound = c->launch_entries;  // upper bound on E used to size the grids
     const int sort_tiles = (int)((bound + SGS_SORT_TILE - 1) / SGS_SORT_TILE);
+    SgsStage stg(c, SGS_STAGE_SORT, s);
     cudaError_t e;
     e = cudaMemsetAsync(c->ranges, 0, sizeof(uint32_t) * 2 * (size_t)tiles, s);
     if (e != cudaSuccess) return e;
@@ -185,6 +186,7 @@ cudaError_t sgs_launch_sort_and_ranges(sgs_ctx* c, cudaStream_t s) {
         e = cudaMemsetAsync(c->sort_state, 0, sizeof(uint32_t) * (size_t)passes * sort_tiles * RADIX, s);
         if (e != cudaSuccess) return e;
         int hb = sort_tiles < 148 * 4 ? sort_tiles : 148 * 4;
+        c->launches += 2 + passes;
         k_histogram<<<hb, 256, 0, s>>>(c->keys[0], c->counters, e_cap, passes, c->sort_hist);
         int cur = 0;
         for (int p = 0; p < passes; ++p) {
@@ -206,7 +208,7 @@ cudaError_t sgs_launch_export_idx(sgs_ctx* c, cudaStream_t s) {
     int b = (int)((c->launch_entries + 255) / 256);
     if (b > 148 * 8) b = 148 * 8;
     if (b > 0)
-        k_export_idx<<<b, 256, 0, s>>>(c->vals[c->sorted_buf], c->vis_to_surfel, c->counters, (unsigned long long)c->e_cap,
+        c->launches += 1, k_export_idx<<<b, 256, 0, s>>>(c->vals[c->sorted_buf], c->vis_to_surfel, c->counters, (unsigned long long)c->e_cap,
                                        c->idx_export);
     return cudaGetLastError();
 }
