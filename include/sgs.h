@@ -60,7 +60,9 @@ enum {
 };
 
 enum {
-    SGS_FLAG_ASYNC = 1 /* never synchronise the host in sgs_render (CUDA-graph capturable) */
+    SGS_FLAG_ASYNC = 1,         /* never synchronise the host in sgs_render (CUDA-graph capturable) */
+    SGS_FLAG_RADIX_BINNING = 2  /* bin with the global LSD radix sort of the 64-bit keys instead of the
+                                   default per-tile buckets + in-tile sort; same list, kept for A/B checks */
 };
 
 /* Truncation conventions of Eq. 8 (R3-R7).  sgs_default_config fills the defaults shown. */

@@ -14,6 +14,7 @@ _LIB_PATH = os.path.join(_HERE, "libsgs.so")
 
 SGS_OK, SGS_INVALID_ARGUMENT, SGS_OUT_OF_MEMORY, SGS_WORKSPACE_OVERFLOW, SGS_NO_FORWARD_STATE, SGS_CUDA_ERROR = range(6)
 SGS_FLAG_ASYNC = 1
+SGS_FLAG_RADIX_BINNING = 2
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
 FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p, C.c_void_p)
@@ -124,7 +125,7 @@ class Renderer:
     """One sgs_ctx.  Method names follow the C calls (sgs_render -> render, ...)."""
 
     def __init__(self, tile=16, cutoff=3.0, alpha_min=1.0 / 255.0, alpha_max=0.99, t_min=1e-4, z_near=0.2,
-                 async_mode=False, device="cuda:0", torch_allocator=True):
+                 async_mode=False, radix_binning=False, device="cuda:0", torch_allocator=True):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2506_00970_b200 needs a CUDA device; there is no CPU fallback")
         self.lib = load_library()
@@ -134,7 +135,8 @@ class Renderer:
         cfg = sgs_config()
         _check(self.lib.sgs_default_config(C.byref(cfg)), "sgs_default_config")
         cfg.tile, cfg.cutoff, cfg.alpha_min, cfg.alpha_max = tile, cutoff, alpha_min, alpha_max
-        cfg.t_min, cfg.z_near, cfg.flags = t_min, z_near, (SGS_FLAG_ASYNC if async_mode else 0)
+        cfg.t_min, cfg.z_near = t_min, z_near
+        cfg.flags = (SGS_FLAG_ASYNC if async_mode else 0) | (SGS_FLAG_RADIX_BINNING if radix_binning else 0)
         if torch_allocator:
             dev_index = self.device.index or 0
 

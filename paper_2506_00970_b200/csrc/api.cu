@@ -40,7 +40,7 @@ int sgs_ensure_surfels(sgs_ctx* c, int64_t n, cudaStream_t s) {
     bool ok = ws_realloc(c, c->scan_state, blocks, s) && ws_realloc(c, c->vis_to_surfel, m, s) &&
               ws_realloc(c, c->culled, m, s) && ws_realloc(c, c->pay.g0, m, s) && ws_realloc(c, c->pay.g1, m, s) &&
               ws_realloc(c, c->pay.g2, m, s) && ws_realloc(c, c->pay.g3, m, s) && ws_realloc(c, c->pay.g4, m, s) &&
-              ws_realloc(c, c->pay.g5, m, s) && ws_realloc(c, c->pay.g6, m, s) &&
+              ws_realloc(c, c->pay.g5, m, s) && ws_realloc(c, c->pay.g6, m, s) && ws_realloc(c, c->pay.g7, m, s) &&
               ws_realloc(c, c->acc, m * SGS_ACC_STRIDE, s, true);  // invariant: acc is all-zero between backward calls
     if (!ok) return SGS_OUT_OF_MEMORY;
     c->n_cap = (int64_t)m;
@@ -83,6 +83,32 @@ int sgs_ensure_partials(sgs_ctx* c, int64_t blocks, cudaStream_t s) {
     cudaStreamSynchronize(s);
     if (!ws_realloc(c, c->pose_partial, (size_t)blocks * 8 + 64, s)) return SGS_OUT_OF_MEMORY;
     c->partial_cap = blocks * 8 + 64;
+    return SGS_OK;
+}
+
+int sgs_ensure_buckets(sgs_ctx* c, int tiles, int64_t tile_cap, cudaStream_t s) {
+    int64_t cap = 256;
+    while (cap < tile_cap) cap <<= 1;  // power of two (the bitonic network pads to it)
+    if ((int64_t)tiles * cap >= (1ll << 32)) return SGS_OUT_OF_MEMORY;
+    if (cap == c->tile_cap && (int64_t)tiles * cap <= c->bucket_cap) return SGS_OK;
+    cudaStreamSynchronize(s);
+    if ((int64_t)tiles * cap > c->bucket_cap) {
+        const size_t m = (size_t)tiles * (size_t)cap;
+        if (!(ws_realloc(c, c->bucket, m, s) && ws_realloc(c, c->cursor, (size_t)tiles + 64, s))) return SGS_OUT_OF_MEMORY;
+        c->bucket_cap = (int64_t)m;
+    }
+    c->tile_cap = cap;
+    return SGS_OK;
+}
+
+int sgs_ensure_export(sgs_ctx* c, int tiles, int64_t entries, cudaStream_t s) {
+    if (entries + 2 * tiles <= c->export_cap) return SGS_OK;
+    cudaStreamSynchronize(s);
+    const size_t m = (size_t)entries + 1024;
+    if (!(ws_realloc(c, c->export_keys, m, s) && ws_realloc(c, c->idx_export, m, s) &&
+          ws_realloc(c, c->export_ranges, (size_t)tiles * 2 + 64, s)))
+        return SGS_OUT_OF_MEMORY;
+    c->export_cap = (int64_t)m + 2 * tiles;
     return SGS_OK;
 }
 
@@ -174,9 +200,10 @@ int sgs_destroy(sgs_ctx* c) {
     cudaDeviceSynchronize();
     cudaStream_t s = 0;
     void* ptrs[] = {c->scan_state, c->vis_to_surfel, c->culled, c->pay.g0, c->pay.g1, c->pay.g2, c->pay.g3, c->pay.g4,
-                    c->pay.g5, c->pay.g6, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
+                    c->pay.g5, c->pay.g6, c->pay.g7, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
                     c->sort_state, c->ranges, c->T_final, c->n_last, c->img_scratch, c->pose_partial, c->resident_store,
-                    c->resident_active, c->target_rgb, c->host_img_dev, c->host_up_dev, c->host_grads_dev};
+                    c->resident_active, c->target_rgb, c->host_img_dev, c->host_up_dev, c->host_grads_dev,
+                    c->bucket, c->cursor, c->export_keys, c->export_ranges};
     for (void* p : ptrs) sgs_ws_free(c, p, s);
     if (c->counters) cudaFree(c->counters);
     if (c->counters_host) cudaFreeHost(c->counters_host);

@@ -2,6 +2,10 @@
 #include <string.h>
 #include "sgs_internal.h"
 
+static inline bool radix_mode(const sgs_ctx* c) { return (c->cfg.flags & SGS_FLAG_RADIX_BINNING) != 0; }
+
+static int64_t grown_tile_cap(int64_t max_tile) { return max_tile + max_tile / 2 + 64; }
+
 // async mode: examine the counters of the previous render (already copied to pinned memory)
 static int check_pending(sgs_ctx* c, cudaStream_t s) {
     if (!c->pending_check) return SGS_OK;
@@ -9,12 +13,80 @@ static int check_pending(sgs_ctx* c, cudaStream_t s) {
     c->pending_check = false;
     const int64_t E = (int64_t)c->counters_host->n_entries;
     c->last_entries = E;
-    if (c->counters_host->overflow) {
+    if (radix_mode(c)) {
+        if (c->counters_host->overflow) {
+            c->have_forward = false;
+            const int r = sgs_ensure_entries(c, E, s);
+            return r != SGS_OK ? r : SGS_WORKSPACE_OVERFLOW;
+        }
+    } else if (c->counters_host->max_tile > (unsigned)c->tile_cap) {
         c->have_forward = false;
-        const int r = sgs_ensure_entries(c, E, s);
+        const int r = sgs_ensure_buckets(c, c->camd.tiles_x * c->camd.tiles_y, grown_tile_cap(c->counters_host->max_tile), s);
         return r != SGS_OK ? r : SGS_WORKSPACE_OVERFLOW;
     }
     return SGS_OK;
+}
+
+static int copy_counters(sgs_ctx* c, cudaStream_t s) {
+    return cudaMemcpyAsync(c->counters_host, c->counters, sizeof(SgsCounters), cudaMemcpyDeviceToHost, s) == cudaSuccess
+               ? SGS_OK : SGS_CUDA_ERROR;
+}
+
+// binning through per-tile buckets + in-tile sort (default)
+static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, cudaStream_t s) {
+    const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    int r = sgs_ensure_buckets(c, tiles, c->tile_cap ? c->tile_cap : 2048, s);
+    if (r != SGS_OK) return r;
+    if (sgs_launch_preprocess_bucket(c, sf, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    if ((r = copy_counters(c, s)) != SGS_OK) return r;
+    if (!async) {
+        if (cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
+        if (c->counters_host->max_tile > (unsigned)c->tile_cap) {  // grow and emit again
+            if ((r = sgs_ensure_buckets(c, tiles, grown_tile_cap(c->counters_host->max_tile), s)) != SGS_OK) return r;
+            if (sgs_launch_preprocess_bucket(c, sf, s) != cudaSuccess) return SGS_CUDA_ERROR;
+            if ((r = copy_counters(c, s)) != SGS_OK) return r;
+            if (cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
+        }
+        c->last_entries = (int64_t)c->counters_host->n_entries;
+    } else {
+        cudaEventRecord(c->counters_ready, s);
+        c->pending_check = true;
+    }
+    return sgs_launch_tilesort(c, s) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
+}
+
+// binning through the global LSD radix sort of (tile << 32 | depth) keys (SGS_FLAG_RADIX_BINNING)
+static int bin_radix(sgs_ctx* c, const sgs_surfels* sf, bool async, cudaStream_t s) {
+    int r;
+    if (c->e_cap == 0) {
+        int64_t guess = 2 * sf->n;
+        if (guess < (1 << 20)) guess = 1 << 20;
+        if ((r = sgs_ensure_entries(c, guess, s)) != SGS_OK) return r;
+    }
+    c->launch_entries = c->e_cap;
+    if (async && c->last_entries > 0) {
+        const int64_t hint = c->last_entries + c->last_entries / 4 + 4096;
+        if (hint < c->launch_entries) c->launch_entries = hint;
+    }
+    if (sgs_launch_preprocess(c, sf, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    if ((r = copy_counters(c, s)) != SGS_OK) return r;
+    if (!async) {
+        if (cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
+        const int64_t E = (int64_t)c->counters_host->n_entries;
+        c->last_entries = E;
+        if (E > c->e_cap) {  // grow and emit again
+            if ((r = sgs_ensure_entries(c, E, s)) != SGS_OK) return r;
+            c->launch_entries = c->e_cap;
+            if (sgs_launch_preprocess(c, sf, s) != cudaSuccess) return SGS_CUDA_ERROR;
+            if ((r = copy_counters(c, s)) != SGS_OK) return r;
+            if (cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
+        }
+        c->launch_entries = E;  // exact grids
+    } else {
+        cudaEventRecord(c->counters_ready, s);
+        c->pending_check = true;
+    }
+    return sgs_launch_sort_and_ranges(c, s) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
 }
 
 extern "C" {
@@ -31,41 +103,11 @@ int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const s
     const int64_t pixels = (int64_t)cam->width * cam->height;
     if ((r = sgs_ensure_surfels(c, sf->n, s)) != SGS_OK) return r;
     if ((r = sgs_ensure_image(c, tiles, pixels, s)) != SGS_OK) return r;
-    if (c->e_cap == 0) {
-        int64_t guess = 2 * sf->n;
-        if (guess < (1 << 20)) guess = 1 << 20;
-        if ((r = sgs_ensure_entries(c, guess, s)) != SGS_OK) return r;
-    }
     const bool async = (c->cfg.flags & SGS_FLAG_ASYNC) != 0;
-    c->launch_entries = c->e_cap;
-    if (async && c->last_entries > 0) {
-        const int64_t hint = c->last_entries + c->last_entries / 4 + 4096;
-        if (hint < c->launch_entries) c->launch_entries = hint;
-    }
     c->last_surfels = *sf;
     c->last_cam = *cam;
-    if (sgs_launch_preprocess(c, sf, s) != cudaSuccess) return SGS_CUDA_ERROR;
-    if (cudaMemcpyAsync(c->counters_host, c->counters, sizeof(SgsCounters), cudaMemcpyDeviceToHost, s) != cudaSuccess)
-        return SGS_CUDA_ERROR;
-    if (!async) {
-        if (cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
-        const int64_t E = (int64_t)c->counters_host->n_entries;
-        c->last_entries = E;
-        if (E > c->e_cap) {  // grow and emit again
-            if ((r = sgs_ensure_entries(c, E, s)) != SGS_OK) return r;
-            c->launch_entries = c->e_cap;
-            if (sgs_launch_preprocess(c, sf, s) != cudaSuccess) return SGS_CUDA_ERROR;
-            if (cudaMemcpyAsync(c->counters_host, c->counters, sizeof(SgsCounters), cudaMemcpyDeviceToHost, s) !=
-                    cudaSuccess ||
-                cudaStreamSynchronize(s) != cudaSuccess)
-                return SGS_CUDA_ERROR;
-        }
-        c->launch_entries = E;  // exact grids
-    } else {
-        cudaEventRecord(c->counters_ready, s);
-        c->pending_check = true;
-    }
-    if (sgs_launch_sort_and_ranges(c, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    r = radix_mode(c) ? bin_radix(c, sf, async, s) : bin_buckets(c, sf, async, s);
+    if (r != SGS_OK) return r;
     float* planes[8];
     for (int i = 0; i < 8; ++i) planes[i] = c->img_scratch + (size_t)i * pixels;
     if (out) {
@@ -130,12 +172,22 @@ int sgs_get_binning(sgs_ctx* c, int64_t* n_entries, const uint64_t** keys, const
     if (r != SGS_OK) return r;
     if (!c->have_forward) return SGS_NO_FORWARD_STATE;
     if (cudaDeviceSynchronize() != cudaSuccess) return SGS_CUDA_ERROR;
+    const int64_t E = (int64_t)c->counters_host->n_entries;
+    if (n_entries) *n_entries = E;
+    if (culled) *culled = c->culled;
+    if (!radix_mode(c)) {
+        const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+        if ((r = sgs_ensure_export(c, tiles, E, 0)) != SGS_OK) return r;
+        if (sgs_launch_export_bucket(c, E, 0) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) return SGS_CUDA_ERROR;
+        if (keys) *keys = c->export_keys;
+        if (idx) *idx = c->idx_export;
+        if (tile_ranges) *tile_ranges = c->export_ranges;
+        return SGS_OK;
+    }
     if (sgs_launch_export_idx(c, 0) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) return SGS_CUDA_ERROR;
-    if (n_entries) *n_entries = (int64_t)c->counters_host->n_entries;
     if (keys) *keys = c->keys[c->sorted_buf];
     if (idx) *idx = c->idx_export;
     if (tile_ranges) *tile_ranges = c->ranges;
-    if (culled) *culled = c->culled;
     return SGS_OK;
 }
 
@@ -144,8 +196,8 @@ int sgs_get_stats(sgs_ctx* c, sgs_stats* out) {
     if (c->pending_check && cudaEventSynchronize(c->counters_ready) != cudaSuccess) return SGS_CUDA_ERROR;
     out->n_visible = c->counters_host->n_visible;
     out->n_entries = (int64_t)c->counters_host->n_entries;
-    out->capacity = c->e_cap;
-    out->overflow = c->counters_host->overflow;
+    out->capacity = radix_mode(c) ? c->e_cap : c->tile_cap;
+    out->overflow = radix_mode(c) ? c->counters_host->overflow : (c->counters_host->max_tile > (unsigned)c->tile_cap);
     out->workspace_bytes = c->bytes;
     out->kernel_launches = c->launches;
     return SGS_OK;

@@ -98,11 +98,12 @@ __device__ __forceinline__ void finish_pose(const float* __restrict__ partial, u
 
 template <bool POSE_ONLY>
 __global__ void __launch_bounds__(SGS_BLOCK)
-k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, SgsPayload pay, int W, int H,
+k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
            int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg, CPlanes up,
            const float* __restrict__ T_final, const uint32_t* __restrict__ n_last, float* __restrict__ acc,
            float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6) {
     __shared__ StagedBwd sh[SGS_BLOCK];
+    __shared__ unsigned char sh_mask[SGS_BLOCK];
     __shared__ float s_red[8][6];
     const int tile = blockIdx.x;
     const int tx = tile % tiles_x, ty = tile / tiles_x;
@@ -147,9 +148,11 @@ k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ val
         const uint32_t boff = (uint32_t)b * SGS_BLOCK;
         const uint32_t nb = min((uint32_t)SGS_BLOCK, bmax - boff);
         __syncthreads();  // previous batch fully consumed
+        unsigned pmask = 0;
         if ((uint32_t)tid < nb) {
-            const uint32_t v = vals[start + boff + tid];
+            const uint32_t v = vals[(size_t)(start + boff + tid) * vstride];
             const float4 g0 = pay.g0[v], g1 = pay.g1[v], g3 = pay.g3[v], g4 = pay.g4[v], g5 = pay.g5[v], g6 = pay.g6[v];
+            pmask = warp_patch_mask(pay.g7[v], (float)(tx * SGS_TILE), (float)(ty * SGS_TILE));
             const double2 g2 = pay.g2[v];
             StagedBwd st;
             stage_entry(g0, g1, g2, g3, px0, py0, st.s0, st.s1, st.s2);
@@ -161,10 +164,17 @@ k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ val
             st.s7 = make_float4(aux * avy - auy * avx, __uint_as_float(v), 0.f, 0.f);
             sh[tid] = st;
         }
+        sh_mask[tid] = (unsigned char)pmask;
         __syncthreads();
         // entries at or after the warp's largest `last` were composited by none of its pixels
-        int jstart = (int)min(nb, wmax > boff ? wmax - boff : 0u) - 1;
-        for (int j = jstart; j >= 0; --j) {
+        const int jend = (int)min(nb, wmax > boff ? wmax - boff : 0u);  // exclusive
+        for (int c0 = ((jend - 1) >> 5) << 5; c0 >= 0 && jend > 0; c0 -= 32) {
+          // this chunk's entries whose AABB reaches the warp's patch, walked from the back
+          unsigned m = __ballot_sync(0xffffffffu, (c0 + lane < jend) && ((sh_mask[c0 + lane] >> wid) & 1u));
+          while (m) {
+            const int hb = 31 - __clz(m);
+            m &= ~(1u << hb);
+            const int j = c0 + hb;
             const float4 s0 = sh[j].s0, s1 = sh[j].s1, s2 = sh[j].s2, s3 = sh[j].s3;
             PairResult r;
             bool hit = (boff + (uint32_t)j) < last;
@@ -213,6 +223,7 @@ k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ val
                     atomicAdd(acc + (size_t)v * SGS_ACC_STRIDE + (lane >> 1), red);
                 }
             }
+          }
         }
     }
     if (POSE_ONLY) {
@@ -245,17 +256,19 @@ k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ val
 // pose gradient (Eq. 11-13).  Leaves acc[v] zeroed for the next backward.
 __global__ void __launch_bounds__(256)
 k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __restrict__ vis_to_surfel,
+                  const uint8_t* __restrict__ culled, unsigned int n_all,
                   float* __restrict__ acc, const float* __restrict__ mean, const float* __restrict__ scale,
                   const float* __restrict__ quat, SgsCamDev cam, sgs_surfel_grads out,
                   float* __restrict__ pose_partial, SgsCounters* __restrict__ counters_rw,
                   float* __restrict__ d_pose6) {
     __shared__ float s_red[8][6];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const unsigned int nv = counters->n_visible;
+    // compacted mode: v < N_v, surfel = vis_to_surfel[v]; bucket mode (no compaction): v = surfel index
     const unsigned int v = blockIdx.x * blockDim.x + tid;
     float p6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    if (v < nv) {
-        const uint32_t i = vis_to_surfel[v];
+    const bool live = vis_to_surfel ? (v < counters->n_visible) : (v < n_all && culled[v] == 0);
+    if (live) {
+        const uint32_t i = vis_to_surfel ? vis_to_surfel[v] : v;
         float a[16];
         float4* ap = reinterpret_cast<float4*>(acc + (size_t)v * SGS_ACC_STRIDE);
 #pragma unroll
@@ -357,7 +370,7 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     if (dg == nullptr) {  // pose-only (tracking, L204)
         if (d_pose6 == nullptr) return cudaSuccess;
         c->launches += 1;
-        k_backward<true><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->vals[c->sorted_buf], c->pay, cam.W, cam.H, cam.tiles_x,
+        k_backward<true><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                      cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
                                                      c->acc, c->pose_partial, c->counters, d_pose6);
         return cudaGetLastError();
@@ -371,13 +384,14 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     if (dg->rgb && e == cudaSuccess) e = cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * (size_t)n, s);
     if (e != cudaSuccess) return e;
     c->launches += 1;
-    k_backward<false><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->vals[c->sorted_buf], c->pay, cam.W, cam.H, cam.tiles_x,
+    k_backward<false><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                   cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
                                                   c->acc, c->pose_partial, c->counters, nullptr);
     const int blocks = (int)((n + 255) / 256);  // bound on N_v; blocks past it only join the pose reduction
     if (blocks == 0 && d_pose6) return cudaMemsetAsync(d_pose6, 0, sizeof(float) * 6, s);
     if (blocks > 0)
-        c->launches += 1, k_surfel_backward<<<blocks, 256, 0, s>>>(c->counters, c->vis_to_surfel, c->acc, c->last_surfels.mean,
+        c->launches += 1, k_surfel_backward<<<blocks, 256, 0, s>>>(c->counters, c->list_stride == 2 ? nullptr : c->vis_to_surfel, c->culled,
+                                                 (unsigned int)n, c->acc, c->last_surfels.mean,
                                                  c->last_surfels.scale, c->last_surfels.quat, cam, *dg, c->pose_partial,
                                                  c->counters, d_pose6);
     return cudaGetLastError();

@@ -2,8 +2,9 @@
 // SURVEY §8(a) step 3).  One block per 16x16 tile, one thread per pixel, a warp covers an 8x4 pixel
 // patch (better footprint coherence than 32x1).  The tile's depth-sorted entries are staged through
 // shared memory in batches of 256: one thread per entry gathers the surfel's payload (float4 loads,
-// L2-resident) and converts it to the tile-relative form of pair.cuh; all threads then read the
-// staged records as warp-wide broadcasts.  A warp leaves the batch loop when all its pixels are
+// L2-resident), converts it to the tile-relative form of pair.cuh and records which of the 8 warp
+// patches the surfel's screen AABB reaches; each warp then walks only its own entries (a ballot over
+// the mask bytes, then find-first-set), reading the staged records as warp-wide broadcasts.  A warp leaves the batch loop when all its pixels are
 // saturated; the block stops fetching batches when every pixel is.
 #include "pair.cuh"
 #include "sgs_internal.h"
@@ -13,9 +14,13 @@ namespace {
 struct Planes { float* p[8]; };
 
 __global__ void __launch_bounds__(SGS_BLOCK)
-k_forward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, SgsPayload pay, int W, int H,
+k_forward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
           int tiles_x, SgsCfgDev cfg, Planes out, float* __restrict__ T_final, uint32_t* __restrict__ n_last) {
-    __shared__ StagedFwd sh[SGS_BLOCK];
+    // staged batch, structure of float4 arrays (one base register, immediate offsets, broadcast reads)
+    __shared__ float4 sh[5][SGS_BLOCK];
+    __shared__ unsigned char sh_mask[SGS_BLOCK];
+    const uint32_t sa = smem_addr(&sh[0][0]), sm_a = smem_addr(sh_mask);
+    constexpr uint32_t PL = SGS_BLOCK * 16;  // bytes per staged plane
     const int tile = blockIdx.x;
     const int tx = tile % tiles_x, ty = tile / tiles_x;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -33,33 +38,43 @@ k_forward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals
     for (uint32_t base = start; base < end; base += SGS_BLOCK) {
         if (__syncthreads_and(done)) break;
         const uint32_t nb = min((uint32_t)SGS_BLOCK, end - base);
+        unsigned mask = 0;
         if ((uint32_t)tid < nb) {
-            const uint32_t v = vals[base + tid];
-            const float4 g0 = pay.g0[v], g1 = pay.g1[v], g3 = pay.g3[v], g4 = pay.g4[v], g5 = pay.g5[v];
+            const uint32_t v = vals[(size_t)(base + tid) * vstride];
+            const float4 g0 = pay.g0[v], g1 = pay.g1[v], g3 = pay.g3[v], g4 = pay.g4[v], g5 = pay.g5[v], g7 = pay.g7[v];
             const double2 g2 = pay.g2[v];
-            StagedFwd st;
-            stage_entry(g0, g1, g2, g3, px0, py0, st.s0, st.s1, st.s2);
-            st.s3 = make_float4(g1.w, g3.w, g4.x, g4.y);
-            st.s4 = make_float4(g4.z, g4.w, g5.x, 0.f);
-            sh[tid] = st;
+            float4 s0, s1, s2;
+            stage_entry(g0, g1, g2, g3, px0, py0, s0, s1, s2);
+            sh[0][tid] = s0; sh[1][tid] = s1; sh[2][tid] = s2;
+            sh[3][tid] = make_float4(g1.w, g3.w, g4.x, g4.y);
+            sh[4][tid] = make_float4(g4.z, g4.w, g5.x, 0.f);
+            mask = warp_patch_mask(g7, (float)(tx * SGS_TILE), (float)(ty * SGS_TILE));
         }
+        sh_mask[tid] = (unsigned char)mask;
         __syncthreads();
-        for (uint32_t j = 0; j < nb; ++j) {
+        for (uint32_t c0 = 0; c0 < nb; c0 += 32) {
             if (__all_sync(0xffffffffu, done)) break;  // per-warp early stop on saturation
-            if (done) continue;
-            const float4 s0 = sh[j].s0, s1 = sh[j].s1, s2 = sh[j].s2, s3 = sh[j].s3;
-            PairResult r;
-            if (!eval_pair(s0, s1, s2, s3.x, lx, ly, cfg.cutoff2, cfg.alpha_min, cfg.alpha_max, cfg.z_near, r)) continue;
-            const float Tn = __fmul_rn(T, 1.f - r.a);
-            if (Tn < cfg.t_min) { done = true; continue; }  // R6: stop, this splat is not composited
-            const float w = __fmul_rn(r.a, T);
-            const float4 s4 = sh[j].s4;
-            C0 = __fmaf_rn(w, s3.y, C0); C1 = __fmaf_rn(w, s3.z, C1); C2 = __fmaf_rn(w, s3.w, C2);
-            Dp = __fmaf_rn(w, r.z, Dp);
-            N0 = __fmaf_rn(w, s4.x, N0); N1 = __fmaf_rn(w, s4.y, N1); N2 = __fmaf_rn(w, s4.z, N2);
-            O += w;
-            T = Tn;
-            last = base - start + j + 1;
+            // entries of this chunk whose AABB reaches this warp's 8x4 patch, in list order
+            unsigned m = __ballot_sync(0xffffffffu, (lds_u8(sm_a + c0 + lane) >> wid) & 1u);
+            while (m) {
+                const uint32_t j = c0 + (uint32_t)__ffs(m) - 1u;
+                m &= m - 1u;
+                if (done) continue;
+                const uint32_t ea = sa + j * 16u;
+                const float4 s0 = lds128(ea), s1 = lds128(ea + PL), s2 = lds128(ea + 2 * PL), s3 = lds128(ea + 3 * PL);
+                PairResult r;
+                if (!eval_pair(s0, s1, s2, s3.x, lx, ly, cfg.cutoff2, cfg.alpha_min, cfg.alpha_max, cfg.z_near, r)) continue;
+                const float Tn = __fmul_rn(T, 1.f - r.a);
+                if (Tn < cfg.t_min) { done = true; continue; }  // R6: stop, this splat is not composited
+                const float w = __fmul_rn(r.a, T);
+                const float4 s4 = lds128(ea + 4 * PL);
+                C0 = __fmaf_rn(w, s3.y, C0); C1 = __fmaf_rn(w, s3.z, C1); C2 = __fmaf_rn(w, s3.w, C2);
+                Dp = __fmaf_rn(w, r.z, Dp);
+                N0 = __fmaf_rn(w, s4.x, N0); N1 = __fmaf_rn(w, s4.y, N1); N2 = __fmaf_rn(w, s4.z, N2);
+                O += w;
+                T = Tn;
+                last = base - start + j + 1;
+            }
         }
     }
     if (inside) {
@@ -85,7 +100,7 @@ cudaError_t sgs_launch_forward(sgs_ctx* c, float* const planes[8], cudaStream_t 
     for (int i = 0; i < 8; ++i) out.p[i] = planes[i];
     SgsStage st(c, SGS_STAGE_FORWARD, s);
     c->launches += 1;
-    k_forward<<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->vals[c->sorted_buf], c->pay, c->camd.W, c->camd.H, c->camd.tiles_x,
+    k_forward<<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, c->camd.W, c->camd.H, c->camd.tiles_x,
                                           c->cfgd, out, c->T_final, c->n_last);
     return cudaGetLastError();
 }

@@ -10,6 +10,7 @@
 // projected centre, the well-conditioned choice in fp32.
 #pragma once
 #include <cuda_runtime.h>
+#include <stdint.h>
 
 // Staged per-(tile, entry) record in shared memory: 5 x float4, read as warp-wide broadcasts.
 struct StagedFwd {
@@ -19,6 +20,20 @@ struct StagedFwd {
     float4 s3;  // opacity, r, g, b
     float4 s4;  // nx, ny, nz, unused
 };
+
+// Shared-memory access by 32-bit shared-window address (computed once per kernel): keeps the
+// address arithmetic of the inner loops to one multiply-add.
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint32_t lds_u8(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
 
 struct PairResult {
     float u, v, z, G, a;
@@ -53,6 +68,20 @@ __device__ __forceinline__ bool eval_pair(const float4 s0, const float4 s1, cons
     r.G = fast_ex2(__fmul_rn(rho2, -0.72134752044448170368f));  // exp(-rho2/2) = 2^(-rho2 / (2 ln 2))
     r.a = fminf(alpha_max, __fmul_rn(opacity, r.G));
     return r.a >= alpha_min;
+}
+
+// 8-bit mask of the warps (8x4 pixel patches, warp w at x0 = (w&1)*8, y0 = (w>>1)*4 inside the tile)
+// whose pixel CENTRES the surfel's screen AABB can reach.  Pixels outside the AABB have rho^2 > c^2,
+// so a warp whose bit is clear would reject the entry at every lane: it skips it without testing.
+__device__ __forceinline__ unsigned warp_patch_mask(const float4 bb, const float tile_x0, const float tile_y0) {
+    unsigned m = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+        const float xl = tile_x0 + (float)((w & 1) * 8) + 0.5f, yl = tile_y0 + (float)((w >> 1) * 4) + 0.5f;
+        const bool hit = bb.y >= xl && bb.x <= xl + 7.f && bb.w >= yl && bb.z <= yl + 3.f;
+        m |= hit ? (1u << w) : 0u;
+    }
+    return m;
 }
 
 // Builds the staged record of entry `v` for the tile whose first pixel centre is (px0, py0).

@@ -37,6 +37,7 @@ struct PreOut {
     double xc, yc;
     float a, b, c;
     float n[3], au[3], av[3];
+    float bb[4];
 };
 
 __device__ __forceinline__ void preprocess_one(const float* __restrict__ mean, const float* __restrict__ scale,
@@ -92,6 +93,8 @@ __device__ __forceinline__ void preprocess_one(const float* __restrict__ mean, c
     if (fy1 > (double)(cam.tiles_y - 1)) fy1 = (double)(cam.tiles_y - 1);
     o.tx0 = (int)fx0; o.tx1 = (int)fx1; o.ty0 = (int)fy0; o.ty1 = (int)fy1;
     o.vis = true;
+    o.bb[0] = __double2float_rd(xmin); o.bb[1] = __double2float_ru(xmax);
+    o.bb[2] = __double2float_rd(ymin); o.bb[3] = __double2float_ru(ymax);
     // ---- payload (no decision depends on it; rounded to fp32 at the end) ----
     const double xc = M[2] / M[8], yc = M[5] / M[8];
     const double B00 = M[0] - xc * M[6], B01 = M[1] - xc * M[7];
@@ -109,6 +112,35 @@ __device__ __forceinline__ void preprocess_one(const float* __restrict__ mean, c
         o.au[i] = (float)(su * tuc[i]);
         o.av[i] = (float)(sv * tvc[i]);
     }
+}
+
+// Conservative binary32 pre-cull.  Returns true only when the strict binary64 path above is CERTAIN to
+// cull the surfel, so the cull flags stay bit-identical to the oracle's while ~80-90 % of a room-scale
+// map never touches the FP64 pipe.  The surfel's cutoff disk lies inside the sphere of radius
+// r = cutoff * max(s_u, s_v) around mu_c.  (i) mu_c.z + d < z_near  =>  mu_c.z <= z_near (culled).
+// (ii) sphere entirely beyond a frustum side plane (through the eye and an image border): every disk
+// point in front of the camera projects off that border, so either the disk crosses the camera plane
+// (den >= 0, culled) or its AABB misses the screen (culled).  d = 1e-5 (|mu|_1 + |t|_1 + 1) metres
+// covers the binary32 rounding of mu_c (~20x its bound) and dwarfs the oracle's own 1e-10 px.
+__device__ __forceinline__ bool precull_f32(const float* __restrict__ mean, const float* __restrict__ scale,
+                                            const SgsCamDev& cam, const SgsCfgDev& cfg) {
+    const float m0 = mean[0], m1 = mean[1], m2 = mean[2];
+    const float X = cam.Rf[0] * m0 + cam.Rf[1] * m1 + cam.Rf[2] * m2 + cam.tf[0];
+    const float Y = cam.Rf[3] * m0 + cam.Rf[4] * m1 + cam.Rf[5] * m2 + cam.tf[1];
+    const float Z = cam.Rf[6] * m0 + cam.Rf[7] * m1 + cam.Rf[8] * m2 + cam.tf[2];
+    const float d = 1e-5f * (fabsf(m0) + fabsf(m1) + fabsf(m2) + fabsf(cam.tf[0]) + fabsf(cam.tf[1]) + fabsf(cam.tf[2]) + 1.f);
+    if (Z + d < cfg.z_near) return true;
+    const float r = sqrtf(cfg.cutoff2) * fmaxf(fabsf(scale[0]), fabsf(scale[1])) * 1.00001f + d;
+    const float cxr = cam.cx - (float)cam.W, cyr = cam.cy - (float)cam.H;
+    // left: fx X + cx Z < 0 ; right: fx X + (cx - W) Z > 0 ; top / bottom alike.  Normals un-normalised:
+    // compare against r * |normal| (rounded up by the 1.00001 factor above and a second one here).
+    const float nl = sqrtf(cam.fx * cam.fx + cam.cx * cam.cx) * 1.00001f, nr = sqrtf(cam.fx * cam.fx + cxr * cxr) * 1.00001f;
+    const float nt = sqrtf(cam.fy * cam.fy + cam.cy * cam.cy) * 1.00001f, nb = sqrtf(cam.fy * cam.fy + cyr * cyr) * 1.00001f;
+    if (cam.fx * X + cam.cx * Z < -r * nl) return true;
+    if (cam.fx * X + cxr * Z > r * nr) return true;
+    if (cam.fy * Y + cam.cy * Z < -r * nt) return true;
+    if (cam.fy * Y + cyr * Z > r * nb) return true;
+    return false;
 }
 
 __global__ void __launch_bounds__(SGS_PRE_BLOCK)
@@ -129,7 +161,8 @@ k_preprocess(int64_t n, const float* __restrict__ mean, const float* __restrict_
 
     PreOut o;
     o.vis = false;
-    if (i < n && (active == nullptr || active[i] != 0)) preprocess_one(mean + 3 * i, scale + 2 * i, quat + 4 * i, cam, cfg, o);
+    if (i < n && (active == nullptr || active[i] != 0) && !precull_f32(mean + 3 * i, scale + 2 * i, cam, cfg))
+        preprocess_one(mean + 3 * i, scale + 2 * i, quat + 4 * i, cam, cfg, o);
     unsigned int cnt = 0;
     if (o.vis) cnt = (unsigned int)((o.tx1 - o.tx0 + 1) * (o.ty1 - o.ty0 + 1));
     if (i < n) culled[i] = o.vis ? 0 : 1;
@@ -193,6 +226,7 @@ k_preprocess(int64_t n, const float* __restrict__ mean, const float* __restrict_
     pay.g4[v] = make_float4(rgb[3 * i + 1], rgb[3 * i + 2], o.n[0], o.n[1]);
     pay.g5[v] = make_float4(o.n[2], o.au[0], o.au[1], o.au[2]);
     pay.g6[v] = make_float4(o.av[0], o.av[1], o.av[2], 0.f);
+    pay.g7[v] = make_float4(o.bb[0], o.bb[1], o.bb[2], o.bb[3]);
 
     // emit keys: tile row-major within the surfel (R2: key = tile id << 32 | depth bits)
     for (int ty = o.ty0; ty <= o.ty1; ++ty)
@@ -203,6 +237,91 @@ k_preprocess(int64_t n, const float* __restrict__ mean, const float* __restrict_
             }
             ++pos;
         }
+}
+
+// Bucket variant (default path): no scan at all.  Tile t owns a fixed-capacity bucket; a visible surfel
+// appends (depth bits << 32 | surfel index) to every tile of its rectangle through an atomic cursor.
+// Arrival order is irrelevant: k_tilesort orders each bucket by the full 64-bit key, which is unique
+// inside a tile, so the result is the stable (tile, depth, index) order of the contract.  The payload
+// is indexed by the surfel index itself (no compaction).
+__global__ void __launch_bounds__(SGS_PRE_BLOCK)
+k_preprocess_bucket(int64_t n, const float* __restrict__ mean, const float* __restrict__ scale,
+                    const float* __restrict__ quat, const float* __restrict__ opacity, const float* __restrict__ rgb,
+                    const uint8_t* __restrict__ active, SgsCamDev cam, SgsCfgDev cfg, SgsPayload pay,
+                    uint8_t* __restrict__ culled, SgsCounters* __restrict__ counters, uint32_t* __restrict__ cursor,
+                    uint64_t* __restrict__ bucket, uint32_t tile_cap) {
+    const int64_t i = (int64_t)blockIdx.x * SGS_PRE_BLOCK + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    PreOut o;
+    o.vis = false;
+    if (i < n && (active == nullptr || active[i] != 0) && !precull_f32(mean + 3 * i, scale + 2 * i, cam, cfg))
+        preprocess_one(mean + 3 * i, scale + 2 * i, quat + 4 * i, cam, cfg, o);
+    if (i < n) culled[i] = o.vis ? 0 : 1;
+    unsigned int cnt = o.vis ? (unsigned int)((o.tx1 - o.tx0 + 1) * (o.ty1 - o.ty0 + 1)) : 0u;
+    // totals: one atomic per warp
+    const unsigned int vis_mask = __ballot_sync(0xffffffffu, o.vis);
+    unsigned int wcnt = cnt;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) wcnt += __shfl_xor_sync(0xffffffffu, wcnt, off);
+    if (lane == 0 && vis_mask) {
+        atomicAdd(&counters->n_visible, (unsigned int)__popc(vis_mask));
+        atomicAdd(&counters->n_entries, (unsigned long long)wcnt);
+    }
+    if (o.vis) {
+        pay.g0[i] = make_float4(o.P, o.Q, o.R, o.S);
+        pay.g1[i] = make_float4(o.D, o.E, o.F, opacity[i]);
+        pay.g2[i] = make_double2(o.xc, o.yc);
+        pay.g3[i] = make_float4(o.a, o.b, o.c, rgb[3 * i]);
+        pay.g4[i] = make_float4(rgb[3 * i + 1], rgb[3 * i + 2], o.n[0], o.n[1]);
+        pay.g5[i] = make_float4(o.n[2], o.au[0], o.au[1], o.au[2]);
+        pay.g6[i] = make_float4(o.av[0], o.av[1], o.av[2], 0.f);
+        pay.g7[i] = make_float4(o.bb[0], o.bb[1], o.bb[2], o.bb[3]);
+    }
+    // Cooperative emission: the block's entries (sum of tile counts) are spread over its threads, one
+    // (surfel, tile) pair each, so the cursor atomics of a block are all in flight together instead of
+    // one thread walking its rectangle serially (and a surfel covering hundreds of tiles costs no more
+    // than hundreds of small ones).
+    __shared__ unsigned int s_off[SGS_PRE_BLOCK + 1];
+    __shared__ unsigned long long s_key[SGS_PRE_BLOCK];
+    __shared__ unsigned int s_rect[SGS_PRE_BLOCK];   // tile index of the rectangle's first tile
+    __shared__ unsigned int s_w[SGS_PRE_BLOCK];      // rectangle width in tiles
+    __shared__ unsigned int s_wsum[SGS_PRE_BLOCK / 32];
+    const int tid = threadIdx.x, wid = tid >> 5;
+    unsigned int incl = cnt;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const unsigned int t2 = __shfl_up_sync(0xffffffffu, incl, off);
+        if (lane >= off) incl += t2;
+    }
+    if (lane == 31) s_wsum[wid] = incl;
+    s_key[tid] = ((unsigned long long)o.depth_bits << 32) | (unsigned long long)(uint32_t)i;
+    s_rect[tid] = o.vis ? (unsigned int)(o.ty0 * cam.tiles_x + o.tx0) : 0u;
+    s_w[tid] = o.vis ? (unsigned int)(o.tx1 - o.tx0 + 1) : 1u;
+    __syncthreads();
+    unsigned int wbase = 0, total = 0;
+#pragma unroll
+    for (int w2 = 0; w2 < SGS_PRE_BLOCK / 32; ++w2) {
+        const unsigned int x = s_wsum[w2];
+        wbase += (w2 < wid) ? x : 0u;
+        total += x;
+    }
+    s_off[tid] = wbase + incl - cnt;  // exclusive
+    if (tid == 0) s_off[SGS_PRE_BLOCK] = total;
+    __syncthreads();
+    for (unsigned int e = tid; e < total; e += SGS_PRE_BLOCK) {
+        // owner = last thread whose exclusive offset is <= e (and whose count is non-zero by construction)
+        int lo = 0, hi = SGS_PRE_BLOCK;  // invariant: s_off[lo] <= e < s_off[hi]
+#pragma unroll
+        for (int it = 0; it < 8; ++it) {
+            const int mid = (lo + hi) >> 1;
+            if (s_off[mid] <= e) lo = mid; else hi = mid;
+        }
+        const unsigned int local = e - s_off[lo], w = s_w[lo];
+        const uint32_t t = s_rect[lo] + (local / w) * (unsigned int)cam.tiles_x + (local % w);
+        const uint32_t pos = atomicAdd(&cursor[t], 1u);
+        if (pos < tile_cap) bucket[(size_t)t * tile_cap + pos] = s_key[lo];
+        else atomicMax(&counters->max_tile, pos + 1u);
+    }
 }
 
 }  // namespace
@@ -220,5 +339,21 @@ cudaError_t sgs_launch_preprocess(sgs_ctx* c, const sgs_surfels* sf, cudaStream_
     k_preprocess<<<blocks, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, sf->active,
                                                   c->camd, c->cfgd, c->pay, c->vis_to_surfel, c->culled, c->scan_state,
                                                   c->counters, c->keys[0], c->vals[0], (unsigned long long)c->e_cap);
+    return cudaGetLastError();
+}
+
+cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cudaStream_t s) {
+    const int64_t n = sf->n;
+    const int blocks = (int)((n + SGS_PRE_BLOCK - 1) / SGS_PRE_BLOCK);
+    const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    cudaError_t e = cudaMemsetAsync(c->counters, 0, sizeof(SgsCounters), s);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(c->cursor, 0, sizeof(uint32_t) * (size_t)tiles, s);
+    if (e != cudaSuccess || blocks == 0) return e;
+    SgsStage st(c, SGS_STAGE_PREPROCESS, s);
+    c->launches += 1;
+    k_preprocess_bucket<<<blocks, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb,
+                                                         sf->active, c->camd, c->cfgd, c->pay, c->culled, c->counters,
+                                                         c->cursor, c->bucket, (uint32_t)c->tile_cap);
     return cudaGetLastError();
 }

@@ -24,6 +24,7 @@ struct SgsPayload {
     float4* g4;   // rgb.g, rgb.b, n_c.x, n_c.y
     float4* g5;   // n_c.z, a_u.x, a_u.y, a_u.z      (a_u = s_u t_uc, camera space)
     float4* g6;   // a_v.x, a_v.y, a_v.z, unused     (a_v = s_v t_vc)
+    float4* g7;   // screen AABB of the cutoff ellipse: xmin, xmax, ymin, ymax (rounded outward)
 };
 
 struct SgsCamDev {
@@ -48,7 +49,8 @@ struct SgsCounters {
     unsigned int overflow;
     unsigned int ticket_pre;        // dynamic block ids for the chained scan in K-pre
     unsigned int ticket_bwd;        // last-block-done ticket for the pose reduction
-    unsigned int pad[2];
+    unsigned int max_tile;          // bucket mode: largest per-tile entry count seen (> tile_cap => overflow)
+    unsigned int pad;
 };
 
 struct sgs_ctx {
@@ -74,6 +76,14 @@ struct sgs_ctx {
     uint32_t* sort_state;            // passes x sort_tiles x 256 look-back words
     uint32_t* sort_ticket;           // passes
     int64_t sort_tiles_cap;
+    // bucket binning (default): tile t owns bucket[t * tile_cap .. ), filled through cursor[t]
+    uint64_t* bucket;                // tiles x tile_cap keys: depth bits << 32 | surfel index
+    uint32_t* cursor;                // tiles
+    int64_t tile_cap, bucket_cap;    // entries per tile; allocated keys
+    uint64_t* export_keys;           // contiguous (tile << 32 | depth) list for sgs_get_binning
+    uint32_t* export_ranges;
+    int64_t export_cap;
+    const uint32_t* list_vals; int list_stride;   // the sorted per-tile lists the compositing kernels walk
     // per-tile / per-pixel
     uint32_t* ranges;                // tiles x 2
     float* T_final;                  // pixels
@@ -122,6 +132,11 @@ cudaError_t sgs_launch_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const fl
                                      cudaStream_t s);
 cudaError_t sgs_launch_export_idx(sgs_ctx* c, cudaStream_t s);
 int sgs_sort_passes(int tiles);
+cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cudaStream_t s);
+cudaError_t sgs_launch_tilesort(sgs_ctx* c, cudaStream_t s);
+cudaError_t sgs_launch_export_bucket(sgs_ctx* c, int64_t n_entries, cudaStream_t s);
+int sgs_ensure_buckets(sgs_ctx* c, int tiles, int64_t tile_cap, cudaStream_t s);
+int sgs_ensure_export(sgs_ctx* c, int tiles, int64_t entries, cudaStream_t s);
 
 // ---- workspace helpers (api.cu) ----
 void* sgs_ws_alloc(sgs_ctx* c, size_t bytes, cudaStream_t s);

@@ -104,26 +104,42 @@ k_onesweep(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ va
             atomicExch(st, ST_INC | total);
         } else {
             atomicExch(st, ST_AGG | total);
-            for (int64_t t = (int64_t)tile - 1; t >= 0; --t) {
-                uint32_t sv;
-                do { sv = *((volatile uint32_t*)(state + (size_t)t * RADIX + d)); } while ((sv & ST_MASK) == 0);
-                prefix += sv & ~ST_MASK;
-                if ((sv & ST_MASK) == ST_INC) break;
+            // Look back LB predecessors at a time: the loads are independent (one L2 round trip per
+            // batch instead of one per predecessor); a word that is not published yet is re-read.
+            constexpr int LB = 16;
+            bool found = false;
+            for (int64_t t = (int64_t)tile - 1; !found; t -= LB) {
+                uint32_t sv[LB];
+#pragma unroll
+                for (int k = 0; k < LB; ++k)
+                    sv[k] = (t - k >= 0) ? *((volatile uint32_t*)(state + (size_t)(t - k) * RADIX + d)) : (2u << 30);
+#pragma unroll
+                for (int k = 0; k < LB; ++k) {
+                    if (!found) {
+                        uint32_t x = sv[k];
+                        while ((x & ST_MASK) == 0) x = *((volatile uint32_t*)(state + (size_t)(t - k) * RADIX + d));
+                        prefix += x & ~ST_MASK;
+                        found = (x & ST_MASK) == ST_INC;
+                    }
+                }
             }
             atomicExch(st, ST_INC | (prefix + total));
         }
-        // global digit base = exclusive scan of the histogram (256 values, done redundantly per tile)
-        __shared__ uint32_t s_scan[RADIX];
+        // global digit base = exclusive scan of the histogram: warp shuffles + one smem hop
+        __shared__ uint32_t s_wsum[8];
         const uint32_t h = hist[d];
-        s_scan[d] = h;
-        __syncthreads();
-        for (int off = 1; off < RADIX; off <<= 1) {
-            const uint32_t t2 = d >= off ? s_scan[d - off] : 0u;
-            __syncthreads();
-            s_scan[d] += t2;
-            __syncthreads();
+        uint32_t incl = h;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const uint32_t t2 = __shfl_up_sync(0xffffffffu, incl, off);
+            if (lane >= off) incl += t2;
         }
-        s_base[d] = s_scan[d] - h + prefix;
+        if (lane == 31) s_wsum[wid] = incl;
+        __syncthreads();
+        uint32_t wbase = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) wbase += (w < wid) ? s_wsum[w] : 0u;
+        s_base[d] = wbase + incl - h + prefix;
     }
     __syncthreads();
 #pragma unroll
@@ -185,7 +201,8 @@ cudaError_t sgs_launch_sort_and_ranges(sgs_ctx* c, cudaStream_t s) {
         if (e != cudaSuccess) return e;
         e = cudaMemsetAsync(c->sort_state, 0, sizeof(uint32_t) * (size_t)passes * sort_tiles * RADIX, s);
         if (e != cudaSuccess) return e;
-        int hb = sort_tiles < 148 * 4 ? sort_tiles : 148 * 4;
+        int hb = (int)((bound + 1023) / 1024);
+        if (hb > 148 * 8) hb = 148 * 8;
         c->launches += 2 + passes;
         k_histogram<<<hb, 256, 0, s>>>(c->keys[0], c->counters, e_cap, passes, c->sort_hist);
         int cur = 0;
@@ -201,6 +218,8 @@ cudaError_t sgs_launch_sort_and_ranges(sgs_ctx* c, cudaStream_t s) {
         if (rb > 148 * 8) rb = 148 * 8;
         k_ranges<<<rb, 256, 0, s>>>(c->keys[cur], c->counters, e_cap, c->ranges);
     }
+    c->list_vals = c->vals[c->sorted_buf];
+    c->list_stride = 1;
     return cudaGetLastError();
 }
 

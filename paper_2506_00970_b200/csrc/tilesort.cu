@@ -1,0 +1,117 @@
+// tilesort.cu -- tile binning, second half, default path (hard part H7: "the
+// contract is the resulting list, not the sorting algorithm").
+//
+// The binning is a most-significant-digit-first radix sort of the 64-bit (tile id | depth bits) keys
+// whose first digit IS the tile id: k_preprocess_bucket has already distributed the entries to their
+// tile's bucket (a counting pass with an atomic cursor per tile), so what remains is to order each
+// bucket by (depth bits, surfel index).  One block per tile does that entirely in shared memory with
+// a bitonic network over the unique keys  depth_bits << 32 | index  -- entries move through HBM once
+// instead of once per 8-bit digit, and there is no chained look-back (the global LSD radix sort of
+// sort.cu spent 10 us per pass on it at E = 83 k; ncu, profiles/r01_*).  Buckets too large for shared
+// memory are sorted in place in global memory by the same network.
+// The per-tile ranges fall out of the cursors; the sorted list the forward/backward kernels walk is
+// the low 32 bits of each key.
+#include "sgs_internal.h"
+
+namespace {
+
+template <typename P>
+__device__ __forceinline__ void bitonic_sort(P keys, uint32_t npad) {
+    for (uint32_t k = 2; k <= npad; k <<= 1) {
+        for (uint32_t j = k >> 1; j > 0; j >>= 1) {
+            for (uint32_t t = threadIdx.x; t < (npad >> 1); t += blockDim.x) {
+                const uint32_t i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
+                const uint32_t p = i | j;
+                const unsigned long long a = keys[i], b = keys[p];
+                const bool up = (i & k) == 0;
+                if ((a > b) == up) { keys[i] = b; keys[p] = a; }
+            }
+            __syncthreads();
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_tilesort(uint64_t* __restrict__ bucket, const uint32_t* __restrict__ cursor, uint32_t tile_cap,
+           uint32_t smem_keys, uint32_t* __restrict__ ranges, SgsCounters* __restrict__ counters) {
+    extern __shared__ unsigned long long sk[];
+    const uint32_t t = blockIdx.x;
+    const uint32_t raw = cursor[t];
+    const uint32_t n = raw < tile_cap ? raw : tile_cap;
+    unsigned long long* g = reinterpret_cast<unsigned long long*>(bucket) + (size_t)t * tile_cap;
+    if (threadIdx.x == 0) {
+        ranges[2 * t] = t * tile_cap;  // index into the bucket array; host guarantees tiles * tile_cap < 2^32
+        ranges[2 * t + 1] = t * tile_cap + n;
+        if (raw > tile_cap) counters->overflow = 1u;
+    }
+    if (n < 2) return;
+    uint32_t npad = 2;
+    while (npad < n) npad <<= 1;
+    if (npad <= smem_keys) {
+        for (uint32_t i = threadIdx.x; i < npad; i += blockDim.x) sk[i] = i < n ? g[i] : ~0ull;
+        __syncthreads();
+        bitonic_sort(sk, npad);
+        for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) g[i] = sk[i];
+    } else {
+        // rare: in place in global memory; npad <= tile_cap because tile_cap is a power of two
+        for (uint32_t i = n + threadIdx.x; i < npad; i += blockDim.x) g[i] = ~0ull;
+        __syncthreads();
+        bitonic_sort(g, npad);
+    }
+}
+
+// ---- debug export for sgs_get_binning: contiguous (tile << 32 | depth) keys, indices and ranges ----
+__global__ void k_export_scan(const uint32_t* __restrict__ ranges, int tiles, uint32_t* __restrict__ xr) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        uint32_t acc = 0;
+        for (int t = 0; t < tiles; ++t) {
+            const uint32_t n = ranges[2 * t + 1] - ranges[2 * t];
+            xr[2 * t] = n ? acc : 0u;
+            xr[2 * t + 1] = n ? acc + n : 0u;
+            acc += n;
+        }
+    }
+}
+__global__ void k_export_copy(const uint64_t* __restrict__ bucket, const uint32_t* __restrict__ ranges,
+                              const uint32_t* __restrict__ xr, uint64_t* __restrict__ keys, uint32_t* __restrict__ idx) {
+    const uint32_t t = blockIdx.x;
+    const uint32_t s = ranges[2 * t], n = ranges[2 * t + 1] - s, d = xr[2 * t];
+    for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+        const uint64_t k = bucket[s + i];
+        keys[d + i] = ((uint64_t)t << 32) | (k >> 32);
+        idx[d + i] = (uint32_t)k;
+    }
+}
+
+}  // namespace
+
+cudaError_t sgs_launch_tilesort(sgs_ctx* c, cudaStream_t s) {
+    const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    uint32_t smem_keys = (uint32_t)c->tile_cap;
+    const uint32_t max_keys = (200u << 10) / 8u;  // 200 KB of dynamic shared memory
+    if (smem_keys > max_keys) {
+        smem_keys = 1;
+        while (smem_keys * 2 <= max_keys) smem_keys <<= 1;
+    }
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_tilesort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(max_keys * 8));
+        attr_set = true;
+    }
+    SgsStage st(c, SGS_STAGE_SORT, s);
+    c->launches += 1;
+    k_tilesort<<<tiles, 256, smem_keys * 8, s>>>(c->bucket, c->cursor, (uint32_t)c->tile_cap, smem_keys, c->ranges,
+                                                c->counters);
+    c->list_vals = reinterpret_cast<const uint32_t*>(c->bucket);
+    c->list_stride = 2;
+    return cudaGetLastError();
+}
+
+cudaError_t sgs_launch_export_bucket(sgs_ctx* c, int64_t n_entries, cudaStream_t s) {
+    (void)n_entries;
+    const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    c->launches += 2;
+    k_export_scan<<<1, 32, 0, s>>>(c->ranges, tiles, c->export_ranges);
+    k_export_copy<<<tiles, 256, 0, s>>>(c->bucket, c->ranges, c->export_ranges, c->export_keys, c->idx_export);
+    return cudaGetLastError();
+}

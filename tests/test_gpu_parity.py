@@ -242,3 +242,48 @@ def test_async_mode_and_host_path():
     loss, p6 = a.track_iter_host(c, 0.5, 1.0)
     assert np.isfinite(loss) and np.isfinite(p6).all()
     sync.close(); a.close()
+
+
+def test_radix_binning_path_gives_the_same_list():
+    """SGS_FLAG_RADIX_BINNING (global LSD radix sort of the 64-bit tile|depth keys) and the default
+    per-tile buckets + in-tile sort produce the identical sorted list, images and gradients."""
+    sc, cams, _ = scenegen.make_config("C2", n_override=60000)
+    cam = cams[0]
+    up = scenegen.upstream_normal(8, cam.height, cam.width)
+    a, b = sgs.Renderer(), sgs.Renderer(radix_binning=True)
+    ra, rb = run_gpu(a, sc, cam, up), run_gpu(b, sc, cam, up)
+    assert_binning(ra["bin"], rb["bin"])
+    assert_binning(rb["bin"], oracle.binning(sc, oracle.make_cam(cam), oracle.make_cfg()))
+    assert np.array_equal(ra["img"], rb["img"])
+    np.testing.assert_allclose(ra["pose"], rb["pose"], rtol=1e-4)
+    for k in ra["grads"]:
+        np.testing.assert_allclose(ra["grads"][k], rb["grads"][k], rtol=1e-3, atol=1e-4 * np.abs(ra["grads"][k]).max())
+    a.close(); b.close()
+
+
+def test_tile_bucket_overflow_grows(ren):
+    """Many surfels stacked on one tile overflow the initial per-tile capacity: the sync path regrows and
+    re-emits; the async path reports SGS_WORKSPACE_OVERFLOW on the next call and then succeeds."""
+    g = scenegen.SplitMix(5)
+    n = 6000
+    mean = np.stack([g.uniform(n, -0.02, 0.02), g.uniform(n, -0.02, 0.02), g.uniform(n, 1.0, 3.0)], 1).astype(np.float32)
+    sc = Scene(mean, np.full((n, 2), 0.01, np.float32), np.tile(np.float32([1, 0, 0, 0]), (n, 1)),
+               np.full(n, 0.05, np.float32), np.full((n, 3), 0.5, np.float32))
+    cam = Camera(64, 48, 60.0, 60.0, 32.0, 24.0)
+    camv, cfg = oracle.make_cam(cam), oracle.make_cfg()
+    out = run_gpu(sgs.Renderer(), sc, cam)
+    ob = oracle.binning(sc, camv, cfg)
+    assert (ob["ranges"][:, 1] - ob["ranges"][:, 0]).max() > 2048
+    assert_binning(out["bin"], ob)
+    assert_images(out["img"], oracle.render(sc, camv, cfg))
+    a = sgs.Renderer(async_mode=True)
+    t, sf = to_device(sc)
+    im = alloc_images(cam)
+    a.render(sf, camera(cam), **im)
+    with pytest.raises(sgs.SgsError) as e:
+        a.render(sf, camera(cam), **im)
+    assert e.value.status == sgs.SGS_WORKSPACE_OVERFLOW
+    a.render(sf, camera(cam), **im)
+    a.stats()
+    assert np.array_equal(planes(im), out["img"])
+    a.close()
