@@ -59,21 +59,33 @@ k_forward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals
             while (m) {
                 const uint32_t j = c0 + (uint32_t)__ffs(m) - 1u;
                 m &= m - 1u;
-                if (done) continue;
                 const uint32_t ea = sa + j * 16u;
-                const float4 s0 = lds128(ea), s1 = lds128(ea + PL), s2 = lds128(ea + 2 * PL), s3 = lds128(ea + 3 * PL);
-                PairResult r;
-                if (!eval_pair(s0, s1, s2, s3.x, lx, ly, cfg.cutoff2, cfg.alpha_min, cfg.alpha_max, cfg.z_near, r)) continue;
-                const float Tn = __fmul_rn(T, 1.f - r.a);
-                if (Tn < cfg.t_min) { done = true; continue; }  // R6: stop, this splat is not composited
-                const float w = __fmul_rn(r.a, T);
-                const float4 s4 = lds128(ea + 4 * PL);
+                const float4 s0 = lds128(ea), s1 = lds128(ea + PL), s2 = lds128(ea + 2 * PL);
+                // pair test (pair.cuh sequence); control flow is kept warp-uniform: one vote, no divergence
+                const float un = __fmaf_rn(ly, s0.y, __fmaf_rn(lx, s0.x, s0.z));
+                const float vn = __fmaf_rn(ly, s1.y, __fmaf_rn(lx, s1.x, s1.z));
+                const float dn = __fmaf_rn(ly, s1.w, __fmaf_rn(lx, s0.w, s2.x));
+                const float inv = fast_rcp(dn);
+                const float u = __fmul_rn(un, inv), v = __fmul_rn(vn, inv);
+                const float rho2 = __fmaf_rn(v, v, __fmul_rn(u, u));
+                bool pass = !done && (rho2 <= cfg.cutoff2);
+                if (!__any_sync(0xffffffffu, pass)) continue;
+                const float4 s3 = lds128(ea + 3 * PL), s4 = lds128(ea + 4 * PL);
+                const float z = __fmaf_rn(s2.z, v, __fmaf_rn(s2.y, u, s2.w));
+                const float G = fast_ex2(__fmul_rn(rho2, -0.72134752044448170368f));
+                const float a = fminf(cfg.alpha_max, __fmul_rn(s3.x, G));
+                pass = pass && (z > cfg.z_near) && (a >= cfg.alpha_min);
+                const float Tn = __fmul_rn(T, 1.f - a);
+                const bool stop = pass && (Tn < cfg.t_min);  // R6: stop, this splat is not composited
+                done = done || stop;
+                pass = pass && !stop;
+                const float w = pass ? __fmul_rn(a, T) : 0.f;
                 C0 = __fmaf_rn(w, s3.y, C0); C1 = __fmaf_rn(w, s3.z, C1); C2 = __fmaf_rn(w, s3.w, C2);
-                Dp = __fmaf_rn(w, r.z, Dp);
+                Dp = __fmaf_rn(w, z, Dp);
                 N0 = __fmaf_rn(w, s4.x, N0); N1 = __fmaf_rn(w, s4.y, N1); N2 = __fmaf_rn(w, s4.z, N2);
                 O += w;
-                T = Tn;
-                last = base - start + j + 1;
+                T = pass ? Tn : T;
+                last = pass ? base - start + j + 1 : last;
             }
         }
     }
