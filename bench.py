@@ -159,11 +159,12 @@ class Workload:
         cam = self.ccams[v]
         self.ren.render(self.sf, cam, **self.im)
         trgb, tdep = self.targets[v]
+        if self.tracking:  # Eq. 15-19 loss fused into the pose-only backward
+            self.ren.backward_tracking(trgb, tdep, 0.5, -1.0, self.p6, self.loss)
+            return
         self.ren.tracking_loss(cam, self.im, trgb, tdep, 0.5, -1.0, self.up, self.loss)
         u = self.up
-        if self.tracking:
-            self.ren.backward(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"], d_pose6=self.p6)
-        else:
+        if True:
             self.ren.backward(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"],
                               grads=self.grads, d_pose6=self.p6)
 

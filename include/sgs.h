@@ -155,6 +155,14 @@ SGS_API int sgs_backward(sgs_ctx* ctx, const sgs_images* upstream, const sgs_sur
 SGS_API int sgs_tracking_loss(sgs_ctx* ctx, const sgs_camera* cam, const sgs_images* rendered, const sgs_images* target,
                       float lambda_d, float normal_sign, const sgs_images* upstream, float* loss, void* cuda_stream);
 
+/* Tracking iteration backward (L180-204): the Eq. 15-19 loss of sgs_tracking_loss evaluated INSIDE the
+ * pose-only backward on the images of the most recent sgs_render (whose output buffers must still hold
+ * them), so neither the upstream gradients nor a loss kernel touch HBM.  target: DEVICE rgb + depth.
+ * d_pose6 (6 floats) and loss (1 float, nullable): DEVICE.  Same result as sgs_tracking_loss followed
+ * by sgs_backward(upstream, NULL, d_pose6). */
+SGS_API int sgs_backward_tracking(sgs_ctx* ctx, const sgs_images* target, float lambda_d, float normal_sign,
+                                  float* d_pose6, float* loss, void* cuda_stream);
+
 /* Debug export of the binning of the last render, for bit-exact parity tests.  Synchronises.
  * Returned DEVICE pointers stay valid until the next call on ctx.  idx holds ORIGINAL surfel
  * indices; culled[i] = 1 iff surfel i was inactive or culled. */

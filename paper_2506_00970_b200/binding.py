@@ -51,7 +51,7 @@ class sgs_stats(C.Structure):
 
 
 EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_backward", "sgs_tracking_loss",
-           "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
+           "sgs_backward_tracking", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
            "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string"]
 
 _lib = None
@@ -207,6 +207,12 @@ class Renderer:
         _check(self.lib.sgs_tracking_loss(self._ctx, C.byref(cam), C.byref(r), C.byref(t), C.c_float(lambda_d),
                                           C.c_float(normal_sign), C.byref(u), _ptr(loss), _stream_ptr(stream)),
                "sgs_tracking_loss")
+
+    def backward_tracking(self, target_rgb, target_depth, lambda_d, normal_sign, d_pose6, loss=None, stream=None):
+        """sgs_backward_tracking: pose-only backward with the Eq. 15-19 loss fused in."""
+        t = _images(target_rgb, target_depth)
+        _check(self.lib.sgs_backward_tracking(self._ctx, C.byref(t), C.c_float(lambda_d), C.c_float(normal_sign),
+                                              _ptr(d_pose6), _ptr(loss), _stream_ptr(stream)), "sgs_backward_tracking")
 
     def get_binning(self, n, tiles):
         """sgs_get_binning -> numpy copies: keys (E,) u64, idx (E,) u32, ranges (tiles,2) u32, culled (n,) u8."""

@@ -129,12 +129,10 @@ int sgs_track_iter_host(sgs_ctx* c, const sgs_camera* cam, float lambda_d, float
     cudaStream_t s = (cudaStream_t)stream;
     int r = ensure_host_images(c, px, s);
     if (r != SGS_OK) return r;
-    sgs_images ren, up, tgt = {c->target_rgb, c->target_depth, nullptr, nullptr};
+    sgs_images ren, tgt = {c->target_rgb, c->target_depth, nullptr, nullptr};
     dev_images(c->host_img_dev, px, &ren);
-    dev_images(c->host_up_dev, px, &up);
     if ((r = sgs_render(c, &c->resident, cam, &ren, stream)) != SGS_OK) return r;
-    if ((r = sgs_tracking_loss(c, cam, &ren, &tgt, lambda_d, normal_sign, &up, c->loss_dev, stream)) != SGS_OK) return r;
-    if ((r = sgs_backward(c, &up, nullptr, c->pose6_dev, stream)) != SGS_OK) return r;
+    if ((r = sgs_backward_tracking(c, &tgt, lambda_d, normal_sign, c->pose6_dev, c->loss_dev, stream)) != SGS_OK) return r;
     if (cudaMemcpyAsync(c->pinned_small, c->loss_dev, sizeof(float) * 7, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
         cudaStreamSynchronize(s) != cudaSuccess)
         return SGS_CUDA_ERROR;

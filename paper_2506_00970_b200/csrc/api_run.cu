@@ -144,6 +144,19 @@ int sgs_backward(sgs_ctx* c, const sgs_images* upstream, const sgs_surfel_grads*
     return SGS_OK;
 }
 
+int sgs_backward_tracking(sgs_ctx* c, const sgs_images* target, float lambda_d, float normal_sign, float* d_pose6,
+                          float* loss, void* stream) {
+    if (!c || !target || !target->rgb || !target->depth || !d_pose6) return SGS_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int r = check_pending(c, s);
+    if (r != SGS_OK) return r;
+    if (!c->have_forward) return SGS_NO_FORWARD_STATE;
+    if ((r = sgs_ensure_partials(c, c->camd.tiles_x * c->camd.tiles_y, s)) != SGS_OK) return r;
+    if (sgs_launch_backward_tracking(c, target->rgb, target->depth, lambda_d, normal_sign, d_pose6, loss, s) != cudaSuccess)
+        return SGS_CUDA_ERROR;
+    return SGS_OK;
+}
+
 int sgs_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const sgs_images* ren, const sgs_images* target, float lambda_d,
                       float normal_sign, const sgs_images* upstream, float* loss, void* stream) {
     if (!c || !sgs_cam_valid(cam) || !ren || !target || !upstream) return SGS_INVALID_ARGUMENT;

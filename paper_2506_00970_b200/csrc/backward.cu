@@ -61,9 +61,10 @@ __device__ __forceinline__ float reduce16_transposed(float (&x)[16], int lane) {
 // Grid reduction: every block has written 6 partial sums at partial[block*8 ..]; the block that
 // draws the last ticket adds them all in fp64 and writes the pose gradient (block-then-grid).
 __device__ __forceinline__ void finish_pose(const float* __restrict__ partial, unsigned int n_blocks,
-                                            SgsCounters* __restrict__ counters, float* __restrict__ d_pose6) {
+                                            SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
+                                            float* __restrict__ loss_out = nullptr) {
     __shared__ bool s_is_last;
-    __shared__ double s_sum[8][6];
+    __shared__ double s_sum[8][7];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     __syncthreads();
     if (tid == 0) {
@@ -74,37 +75,44 @@ __device__ __forceinline__ void finish_pose(const float* __restrict__ partial, u
     __syncthreads();
     if (!s_is_last) return;
     __threadfence();
-    double a[6] = {0, 0, 0, 0, 0, 0};
+    double a[7] = {0, 0, 0, 0, 0, 0, 0};
     for (unsigned int b = tid; b < n_blocks; b += blockDim.x) {
         const float4 lo = __ldcg(reinterpret_cast<const float4*>(partial + (size_t)b * 8));
         const float4 hi = __ldcg(reinterpret_cast<const float4*>(partial + (size_t)b * 8 + 4));
-        a[0] += lo.x; a[1] += lo.y; a[2] += lo.z; a[3] += lo.w; a[4] += hi.x; a[5] += hi.y;
+        a[0] += lo.x; a[1] += lo.y; a[2] += lo.z; a[3] += lo.w; a[4] += hi.x; a[5] += hi.y; a[6] += hi.z;
     }
 #pragma unroll
-    for (int c = 0; c < 6; ++c) {
+    for (int c = 0; c < 7; ++c) {
         double v = a[c];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
         if (lane == 0) s_sum[wid][c] = v;
     }
     __syncthreads();
-    if (tid < 6) {
+    if (tid < 7) {
         double v = 0;
         for (int w2 = 0; w2 < (int)(blockDim.x >> 5); ++w2) v += s_sum[w2][tid];
-        d_pose6[tid] = (float)v;
+        if (tid < 6) d_pose6[tid] = (float)v;
+        else if (loss_out) *loss_out = (float)v;
     }
     if (tid == 0) counters->ticket_bwd = 0;  // self-cleaning: backward may run again on the same render
 }
 
-template <bool POSE_ONLY>
+// FUSED (pose-only only): `up` holds the RENDERED planes of the last forward and the upstream gradients of the
+// tracking loss (Eq. 15-19, same arithmetic as loss.cu) are formed in registers -- no loss kernel, no
+// upstream images through HBM; the loss itself rides in slot 6 of the pose partials.
+struct FusedLoss { const float* trgb; const float* tdepth; float lambda_d, nsign; float* loss; };
+
+template <bool POSE_ONLY, bool FUSED>
 __global__ void __launch_bounds__(SGS_BLOCK)
 k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
            int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg, CPlanes up,
            const float* __restrict__ T_final, const uint32_t* __restrict__ n_last, float* __restrict__ acc,
-           float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6) {
+           float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
+           FusedLoss fl) {
     __shared__ StagedBwd sh[SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
-    __shared__ float s_red[8][6];
+    __shared__ float s_red[8][7];
     const int tile = blockIdx.x;
     const int tx = tile % tiles_x, ty = tile / tiles_x;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -118,17 +126,35 @@ k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ val
     float g[8];
     float T_after = 1.f;
     uint32_t last = 0;
+    float my_loss = 0.f;
+    const float rx = ((float)px + 0.5f - cx) / fx, ry = ((float)py + 0.5f - cy) / fy;  // pixel ray (rx, ry, 1)
+#pragma unroll
+    for (int c = 0; c < 8; ++c) g[c] = 0.f;
     if (inside) {
         const size_t pix = (size_t)py * W + px;
+        if (FUSED) {
+            const size_t HW = (size_t)W * H;
+            const float inv = 1.f / (float)HW;
+            const float nr = up.p[4][pix] * rx + up.p[5][pix] * ry + up.p[6][pix];
+            if ((fl.nsign * nr > 0.f) && (up.p[7][pix] > 0.95f)) {   // M_n M_o (Eq. 17-18)
 #pragma unroll
-        for (int c = 0; c < 8; ++c) g[c] = up.p[c] ? up.p[c][pix] : 0.f;
+                for (int c = 0; c < 3; ++c) {
+                    const float d = up.p[c][pix] - fl.trgb[c * HW + pix];
+                    my_loss += fabsf(d);
+                    g[c] = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
+                }
+                const float d = up.p[3][pix] - fl.tdepth[pix];
+                my_loss += fl.lambda_d * fabsf(d);
+                g[3] = d > 0.f ? fl.lambda_d * inv : (d < 0.f ? -fl.lambda_d * inv : 0.f);
+            }
+            my_loss *= inv;
+        } else {
+#pragma unroll
+            for (int c = 0; c < 8; ++c) g[c] = up.p[c] ? up.p[c][pix] : 0.f;
+        }
         T_after = T_final[pix];
         last = n_last[pix];
-    } else {
-#pragma unroll
-        for (int c = 0; c < 8; ++c) g[c] = 0.f;
     }
-    const float rx = ((float)px + 0.5f - cx) / fx, ry = ((float)py + 0.5f - cy) / fy;  // pixel ray (rx, ry, 1)
     float suffix = 0.f;
     float F0 = 0.f, F1 = 0.f, F2 = 0.f, Z0 = 0.f, Z1 = 0.f, Z2 = 0.f, Nn0 = 0.f, Nn1 = 0.f, Nn2 = 0.f;
 
@@ -228,24 +254,25 @@ k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ val
     }
     if (POSE_ONLY) {
         // Eq. 11-13 per pixel: rho += sum f; theta += X x f summed = r x sum(z f), plus t_nc x dL/dt_nc = N x g_N
-        float p6[6];
+        float p6[7];
+        p6[6] = my_loss;
         p6[0] = F0; p6[1] = F1; p6[2] = F2;
         p6[3] = (ry * Z2 - Z1) + (Nn1 * g[6] - Nn2 * g[5]);
         p6[4] = (Z0 - rx * Z2) + (Nn2 * g[4] - Nn0 * g[6]);
         p6[5] = (rx * Z1 - ry * Z0) + (Nn0 * g[5] - Nn1 * g[4]);
 #pragma unroll
-        for (int c = 0; c < 6; ++c) {
+        for (int c = 0; c < 7; ++c) {
             const float s = warp_sum(inside ? p6[c] : 0.f);
             if (lane == 0) s_red[wid][c] = s;
         }
         __syncthreads();
-        if (tid < 6) {
+        if (tid < 7) {
             float s = 0.f;
 #pragma unroll
             for (int w2 = 0; w2 < 8; ++w2) s += s_red[w2][tid];
             pose_partial[(size_t)tile * 8 + tid] = s;
         }
-        finish_pose(pose_partial, gridDim.x, counters, d_pose6);
+        finish_pose(pose_partial, gridDim.x, counters, d_pose6, FUSED ? fl.loss : nullptr);
     }
 }
 
@@ -370,9 +397,9 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     if (dg == nullptr) {  // pose-only (tracking, L204)
         if (d_pose6 == nullptr) return cudaSuccess;
         c->launches += 1;
-        k_backward<true><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
+        k_backward<true, false><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                      cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
-                                                     c->acc, c->pose_partial, c->counters, d_pose6);
+                                                     c->acc, c->pose_partial, c->counters, d_pose6, FusedLoss{});
         return cudaGetLastError();
     }
     const int64_t n = c->last_surfels.n;
@@ -384,9 +411,9 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     if (dg->rgb && e == cudaSuccess) e = cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * (size_t)n, s);
     if (e != cudaSuccess) return e;
     c->launches += 1;
-    k_backward<false><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
+    k_backward<false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                   cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
-                                                  c->acc, c->pose_partial, c->counters, nullptr);
+                                                  c->acc, c->pose_partial, c->counters, nullptr, FusedLoss{});
     const int blocks = (int)((n + 255) / 256);  // bound on N_v; blocks past it only join the pose reduction
     if (blocks == 0 && d_pose6) return cudaMemsetAsync(d_pose6, 0, sizeof(float) * 6, s);
     if (blocks > 0)
@@ -394,5 +421,21 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
                                                  (unsigned int)n, c->acc, c->last_surfels.mean,
                                                  c->last_surfels.scale, c->last_surfels.quat, cam, *dg, c->pose_partial,
                                                  c->counters, d_pose6);
+    return cudaGetLastError();
+}
+
+// Tracking iteration backward with the Eq. 15-19 loss fused in (pose-only): see FusedLoss.
+cudaError_t sgs_launch_backward_tracking(sgs_ctx* c, const float* trgb, const float* tdepth, float lambda_d, float nsign,
+                                         float* d_pose6, float* loss, cudaStream_t s) {
+    SgsStage st(c, SGS_STAGE_BACKWARD, s);
+    const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    CPlanes u;
+    for (int i = 0; i < 8; ++i) u.p[i] = c->last_img[i];
+    const SgsCamDev& cam = c->camd;
+    FusedLoss fl{trgb, tdepth, lambda_d, nsign, loss};
+    c->launches += 1;
+    k_backward<true, true><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H,
+                                                       cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final,
+                                                       c->n_last, c->acc, c->pose_partial, c->counters, d_pose6, fl);
     return cudaGetLastError();
 }

@@ -131,6 +131,8 @@ cudaError_t sgs_launch_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const fl
                                      const float* tdepth, float lambda_d, float nsign, float* const up[8], float* loss,
                                      cudaStream_t s);
 cudaError_t sgs_launch_export_idx(sgs_ctx* c, cudaStream_t s);
+cudaError_t sgs_launch_backward_tracking(sgs_ctx* c, const float* trgb, const float* tdepth, float lambda_d, float nsign,
+                                         float* d_pose6, float* loss, cudaStream_t s);
 int sgs_sort_passes(int tiles);
 cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cudaStream_t s);
 cudaError_t sgs_launch_tilesort(sgs_ctx* c, cudaStream_t s);

@@ -125,6 +125,12 @@ def test_c2_tracking_shape(ren):
     ren.backward(d_rgb=upi["rgb"], d_depth=upi["depth"], d_normal=upi["normal"], d_alpha=upi["alpha"], d_pose6=p6)
     og = oracle.backward(sc, camv, cfg, up_gpu)
     assert_pose(p6.cpu().numpy().astype(np.float64), og["pose"])
+    # fused loss + backward (sgs_backward_tracking) == loss kernel followed by backward, and == the oracle
+    p6f, lossf = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+    ren.backward_tracking(trgb, tdep, 0.5, -1.0, p6f, lossf)
+    assert abs(float(lossf.item()) - L_ref) <= 1e-4 * abs(L_ref)
+    assert_pose(p6f.cpu().numpy().astype(np.float64), og["pose"])
+    np.testing.assert_allclose(p6f.cpu().numpy(), p6.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(p6.abs().max()))
 
 
 def test_backward_is_repeatable_and_overwrites(ren):
