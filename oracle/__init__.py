@@ -112,11 +112,12 @@ def render(sc, camv, cfgv, brute=False, counters=True):
     mean, scale, quat, opac, rgb, act = _scene_arrays(sc)
     W, H = int(camv[0]), int(camv[1])
     img = np.zeros((8, H, W)); T = np.zeros((H, W)); nc = np.zeros((H, W), np.int32)
-    frag = np.zeros((H, W), np.uint8); cnt = np.zeros(6, np.int64)
+    frag = np.zeros((H, W), np.uint8); cnt = np.zeros(6, np.int64); qtb = np.zeros((H, W), np.int32)
     lib().orc_render(ctypes.c_int64(sc.n), _p(mean, C_F32), _p(scale, C_F32), _p(quat, C_F32), _p(opac, C_F32),
                      _p(rgb, C_F32), _p(act, C_U8), _p(camv, C_F64), _p(cfgv, C_F64), ctypes.c_int(int(brute)),
-                     _p(img, C_F64), _p(T, C_F64), _p(nc, C_I32), _p(frag, C_U8), _p(cnt if counters else None, C_I64))
-    return dict(img=img, T_final=T, n_comp=nc, fragile=frag,
+                     _p(img, C_F64), _p(T, C_F64), _p(nc, C_I32), _p(frag, C_U8), _p(cnt if counters else None, C_I64),
+                     _p(qtb if counters else None, C_I32))
+    return dict(img=img, T_final=T, n_comp=nc, fragile=frag, qtb_pix=qtb,
                 counters=dict(Q_t=int(cnt[0]), Q_c=int(cnt[1]), cover=int(cnt[2]), n_vis=int(cnt[3]), n_fragile=int(cnt[4]), Q_tb=int(cnt[5])))
 
 

@@ -375,7 +375,8 @@ static inline int64_t cand_count(const Ctx* c, int i, int j, const uint32_t** ls
 void orc_render(int64_t n, const float* mean, const float* scale, const float* quat,
                 const float* opacity, const float* rgb, const uint8_t* active,
                 const double* camv, const double* cfgv, int brute,
-                double* img, double* T_final, int32_t* n_comp, uint8_t* fragile, int64_t* counters) {
+                double* img, double* T_final, int32_t* n_comp, uint8_t* fragile, int64_t* counters,
+                int32_t* qtb_pix /* nullable: per-pixel Q_tb */) {
     Ctx c; ctx_init(&c, n, mean, scale, quat, opacity, rgb, active, camv, cfgv, brute);
     const int W = c.cam.W, H = c.cam.H; const int64_t HW = (int64_t)W * H;
     int64_t Qt = 0, Qc = 0, Qcover = 0, nfrag = 0, Qtb = 0;
@@ -419,6 +420,7 @@ void orc_render(int64_t n, const float* mean, const float* scale, const float* q
             for (int ch = 0; ch < 8; ++ch) img[ch * HW + pix] = acc[ch];
             if (T_final) T_final[pix] = T;
             if (n_comp) n_comp[pix] = nc;
+            if (qtb_pix) qtb_pix[pix] = (int32_t)qt_last;
             if (fragile) fragile[pix] = (uint8_t)frag;
             nfrag += (frag & 5) != 0;
             Qt += qt_pix; Qtb += qt_last;

@@ -52,6 +52,12 @@ static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, cudaStream
         cudaEventRecord(c->counters_ready, s);
         c->pending_check = true;
     }
+    c->fused_sort = c->tile_cap <= 2048;
+    if (c->fused_sort) {  // k_forward orders each bucket itself
+        c->list_vals = reinterpret_cast<const uint32_t*>(c->bucket);
+        c->list_stride = 2;
+        return SGS_OK;
+    }
     return sgs_launch_tilesort(c, s) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
 }
 
@@ -86,6 +92,7 @@ static int bin_radix(sgs_ctx* c, const sgs_surfels* sf, bool async, cudaStream_t
         cudaEventRecord(c->counters_ready, s);
         c->pending_check = true;
     }
+    c->fused_sort = false;
     return sgs_launch_sort_and_ranges(c, s) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
 }
 

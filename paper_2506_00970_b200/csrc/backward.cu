@@ -154,6 +154,12 @@ k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ val
         }
         T_after = T_final[pix];
         last = n_last[pix];
+        // every term of the backward carries a factor g: a pixel whose upstream gradient is exactly zero
+        // (e.g. masked out by M_n M_o in tracking, Eq. 17-19) contributes exactly nothing -- skip its list
+        bool nz = false;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) nz = nz || (g[c] != 0.f);
+        if (!nz) last = 0;
     }
     float suffix = 0.f;
     float F0 = 0.f, F1 = 0.f, F2 = 0.f, Z0 = 0.f, Z1 = 0.f, Z2 = 0.f, Nn0 = 0.f, Nn1 = 0.f, Nn2 = 0.f;

@@ -14,8 +14,9 @@ namespace {
 struct Planes { float* p[8]; };
 
 __global__ void __launch_bounds__(SGS_BLOCK)
-k_forward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
-          int tiles_x, SgsCfgDev cfg, Planes out, float* __restrict__ T_final, uint32_t* __restrict__ n_last) {
+k_forward(uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
+          int tiles_x, SgsCfgDev cfg, Planes out, float* __restrict__ T_final, uint32_t* __restrict__ n_last,
+          const uint32_t* __restrict__ cursor, unsigned long long* bucket, uint32_t tile_cap) {
     // staged batch, structure of float4 arrays (one base register, immediate offsets, broadcast reads)
     __shared__ float4 sh[5][SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
@@ -29,7 +30,45 @@ k_forward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals
     const bool inside = px < W && py < H;
     const float lx = (float)lxi, ly = (float)lyi;
     const double px0 = (double)(tx * SGS_TILE) + 0.5, py0 = (double)(ty * SGS_TILE) + 0.5;
-    const uint32_t start = ranges[2 * tile], end = ranges[2 * tile + 1];
+    uint32_t start, end;
+    if (cursor != nullptr) {
+        // Fused in-tile sort (bucket binning, tile_cap <= 2048): order this tile's bucket by the unique key
+        // depth_bits << 32 | index in the staging memory before compositing, write it back for the
+        // backward pass and publish the range.  See tilesort.cu for the rationale and the large-bucket path.
+        const uint32_t raw = cursor[tile];
+        const uint32_t n = raw < tile_cap ? raw : tile_cap;
+        start = tile * tile_cap; end = start + n;
+        if (tid == 0) { ranges[2 * tile] = start; ranges[2 * tile + 1] = end; }
+        unsigned long long* g = bucket + (size_t)start;
+        unsigned long long* sk = reinterpret_cast<unsigned long long*>(&sh[0][0]);
+        if (n >= 2 && n <= 256) {
+            const bool mine = (uint32_t)tid < n;
+            const unsigned long long key = mine ? g[tid] : ~0ull;
+            if (mine) sk[tid] = key;
+            __syncthreads();
+            uint32_t rank = 0;
+            for (uint32_t k = 0; k < n; ++k) rank += sk[k] < key ? 1u : 0u;
+            if (mine) g[rank] = key;
+        } else if (n > 256) {
+            uint32_t npad = 512;
+            while (npad < n) npad <<= 1;
+            for (uint32_t i = tid; i < npad; i += SGS_BLOCK) sk[i] = i < n ? g[i] : ~0ull;
+            __syncthreads();
+            for (uint32_t k = 2; k <= npad; k <<= 1)
+                for (uint32_t j = k >> 1; j > 0; j >>= 1) {
+                    for (uint32_t t = tid; t < (npad >> 1); t += SGS_BLOCK) {
+                        const uint32_t i = ((t & ~(j - 1)) << 1) | (t & (j - 1)), p = i | j;
+                        const unsigned long long a = sk[i], b = sk[p];
+                        if ((a > b) == ((i & k) == 0)) { sk[i] = b; sk[p] = a; }
+                    }
+                    __syncthreads();
+                }
+            for (uint32_t i = tid; i < n; i += SGS_BLOCK) g[i] = sk[i];
+        }
+        __syncthreads();  // sorted bucket visible to the block; staging memory free again
+    } else {
+        start = ranges[2 * tile]; end = ranges[2 * tile + 1];
+    }
 
     float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dp = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f, O = 0.f;
     uint32_t last = 0;  // entries [0, last) of the tile list contain every composited pair of this pixel
@@ -40,7 +79,8 @@ k_forward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals
         const uint32_t nb = min((uint32_t)SGS_BLOCK, end - base);
         unsigned mask = 0;
         if ((uint32_t)tid < nb) {
-            const uint32_t v = vals[(size_t)(base + tid) * vstride];
+            // fused mode: the bucket was just rewritten by this block -- plain loads, not the read-only path
+            const uint32_t v = cursor != nullptr ? (uint32_t)bucket[base + tid] : vals[(size_t)(base + tid) * vstride];
             const float4 g0 = pay.g0[v], g1 = pay.g1[v], g3 = pay.g3[v], g4 = pay.g4[v], g5 = pay.g5[v], g7 = pay.g7[v];
             const double2 g2 = pay.g2[v];
             float4 s0, s1, s2;
@@ -113,6 +153,7 @@ cudaError_t sgs_launch_forward(sgs_ctx* c, float* const planes[8], cudaStream_t 
     SgsStage st(c, SGS_STAGE_FORWARD, s);
     c->launches += 1;
     k_forward<<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, c->camd.W, c->camd.H, c->camd.tiles_x,
-                                          c->cfgd, out, c->T_final, c->n_last);
+                                          c->cfgd, out, c->T_final, c->n_last, c->fused_sort ? c->cursor : nullptr,
+                                          reinterpret_cast<unsigned long long*>(c->bucket), (uint32_t)c->tile_cap);
     return cudaGetLastError();
 }

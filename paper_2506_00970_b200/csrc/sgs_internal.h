@@ -83,7 +83,8 @@ struct sgs_ctx {
     uint64_t* export_keys;           // contiguous (tile << 32 | depth) list for sgs_get_binning
     uint32_t* export_ranges;
     int64_t export_cap;
-    const uint32_t* list_vals; int list_stride;   // the sorted per-tile lists the compositing kernels walk
+    const uint32_t* list_vals; int list_stride;
+    bool fused_sort;                 // bucket mode with tile_cap <= 2048: k_forward sorts its own bucket   // the sorted per-tile lists the compositing kernels walk
     // per-tile / per-pixel
     uint32_t* ranges;                // tiles x 2
     float* T_final;                  // pixels
