@@ -15,6 +15,7 @@
 //                   no per-surfel traffic at all -- registers -> block -> grid reduction to 6 values.
 #include "pair.cuh"
 #include "sgs_internal.h"
+#include "reduce.cuh"
 
 namespace {
 
@@ -26,12 +27,6 @@ struct StagedBwd {
     float4 s6;                  // a_v.yz, m.xy      (m = a_u x a_v)
     float4 s7;                  // m.z, bits(v), -, -
 };
-
-__device__ __forceinline__ float warp_sum(float v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
 
 // Transposed butterfly: 16 per-lane values -> lane l ends with the warp-wide sum of value (l>>1)&15.
 __device__ __forceinline__ float reduce16_transposed(float (&x)[16], int lane) {
@@ -56,46 +51,6 @@ __device__ __forceinline__ float reduce16_transposed(float (&x)[16], int lane) {
         x[0] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
     }
     return x[0] + __shfl_xor_sync(0xffffffffu, x[0], 1);
-}
-
-// Grid reduction: every block has written 6 partial sums at partial[block*8 ..]; the block that
-// draws the last ticket adds them all in fp64 and writes the pose gradient (block-then-grid).
-__device__ __forceinline__ void finish_pose(const float* __restrict__ partial, unsigned int n_blocks,
-                                            SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
-                                            float* __restrict__ loss_out = nullptr) {
-    __shared__ bool s_is_last;
-    __shared__ double s_sum[8][7];
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    __syncthreads();
-    if (tid == 0) {
-        __threadfence();
-        const unsigned int t = atomicAdd(&counters->ticket_bwd, 1u);
-        s_is_last = (t == n_blocks - 1);
-    }
-    __syncthreads();
-    if (!s_is_last) return;
-    __threadfence();
-    double a[7] = {0, 0, 0, 0, 0, 0, 0};
-    for (unsigned int b = tid; b < n_blocks; b += blockDim.x) {
-        const float4 lo = __ldcg(reinterpret_cast<const float4*>(partial + (size_t)b * 8));
-        const float4 hi = __ldcg(reinterpret_cast<const float4*>(partial + (size_t)b * 8 + 4));
-        a[0] += lo.x; a[1] += lo.y; a[2] += lo.z; a[3] += lo.w; a[4] += hi.x; a[5] += hi.y; a[6] += hi.z;
-    }
-#pragma unroll
-    for (int c = 0; c < 7; ++c) {
-        double v = a[c];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if (lane == 0) s_sum[wid][c] = v;
-    }
-    __syncthreads();
-    if (tid < 7) {
-        double v = 0;
-        for (int w2 = 0; w2 < (int)(blockDim.x >> 5); ++w2) v += s_sum[w2][tid];
-        if (tid < 6) d_pose6[tid] = (float)v;
-        else if (loss_out) *loss_out = (float)v;
-    }
-    if (tid == 0) counters->ticket_bwd = 0;  // self-cleaning: backward may run again on the same render
 }
 
 // FUSED (pose-only only): `up` holds the RENDERED planes of the last forward and the upstream gradients of the
