@@ -157,11 +157,11 @@ class Workload:
     def one(self, v):
         """render -> loss -> backward for view v (everything enqueued, no host sync)."""
         cam = self.ccams[v]
-        self.ren.render(self.sf, cam, **self.im)
         trgb, tdep = self.targets[v]
-        if self.tracking:  # Eq. 15-19 loss fused into the pose-only backward
-            self.ren.backward_tracking(trgb, tdep, 0.5, -1.0, self.p6, self.loss)
+        if self.tracking:  # one tracking iteration: K-pre + K-track (render, Eq. 15-19 loss, pose-only backward); images written
+            self.ren.track_iter(self.sf, cam, trgb, tdep, 0.5, -1.0, self.p6, self.loss, **self.im)
             return
+        self.ren.render(self.sf, cam, **self.im)
         self.ren.tracking_loss(cam, self.im, trgb, tdep, 0.5, -1.0, self.up, self.loss)
         u = self.up
         if True:

@@ -163,6 +163,20 @@ SGS_API int sgs_tracking_loss(sgs_ctx* ctx, const sgs_camera* cam, const sgs_ima
 SGS_API int sgs_backward_tracking(sgs_ctx* ctx, const sgs_images* target, float lambda_d, float normal_sign,
                                   float* d_pose6, float* loss, void* cuda_stream);
 
+/* One whole tracking iteration (L180-204) in two launches: preprocess + tile binning, then ONE kernel that
+ * composites each tile (Eq. 8), evaluates Eq. 15-19 against the current frame in registers and walks the
+ * tile's list back for the pose gradient (Eq. 11-13); images, T and the upstream gradients never leave the
+ * SM.  Same result as sgs_render + sgs_backward_tracking (bit-identical images, loss and 6-vector up to
+ * the order of the block sums).
+ *   surfels : DEVICE map; only active splats are rendered (L204)
+ *   target  : DEVICE rgb (3xHxW) + depth (HxW) of the current frame
+ *   out     : nullable; DEVICE images to write (any pointer may be NULL = not written)
+ *   d_pose6 : DEVICE, 6 floats (rho, theta); loss: DEVICE, 1 float, nullable
+ * Leaves no state for sgs_backward (SGS_NO_FORWARD_STATE); sgs_get_binning works. */
+SGS_API int sgs_track_iter(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_camera* cam, const sgs_images* target,
+                           float lambda_d, float normal_sign, const sgs_images* out, float* d_pose6, float* loss,
+                           void* cuda_stream);
+
 /* Debug export of the binning of the last render, for bit-exact parity tests.  Synchronises.
  * Returned DEVICE pointers stay valid until the next call on ctx.  idx holds ORIGINAL surfel
  * indices; culled[i] = 1 iff surfel i was inactive or culled. */

@@ -51,7 +51,7 @@ class sgs_stats(C.Structure):
 
 
 EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_backward", "sgs_tracking_loss",
-           "sgs_backward_tracking", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
+           "sgs_backward_tracking", "sgs_track_iter", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
            "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string"]
 
 _lib = None
@@ -213,6 +213,15 @@ class Renderer:
         t = _images(target_rgb, target_depth)
         _check(self.lib.sgs_backward_tracking(self._ctx, C.byref(t), C.c_float(lambda_d), C.c_float(normal_sign),
                                               _ptr(d_pose6), _ptr(loss), _stream_ptr(stream)), "sgs_backward_tracking")
+
+    def track_iter(self, surfels, cam, target_rgb, target_depth, lambda_d, normal_sign, d_pose6, loss=None,
+                   rgb=None, depth=None, normal=None, alpha=None, stream=None):
+        """sgs_track_iter: preprocess + binning, then ONE kernel for render + Eq. 15-19 loss + pose-only backward."""
+        t = _images(rgb=target_rgb, depth=target_depth)
+        out = _images(rgb, depth, normal, alpha)
+        _check(self.lib.sgs_track_iter(self._ctx, C.byref(surfels), C.byref(cam), C.byref(t), C.c_float(lambda_d),
+                                       C.c_float(normal_sign), C.byref(out), _ptr(d_pose6), _ptr(loss),
+                                       _stream_ptr(stream)), "sgs_track_iter")
 
     def get_binning(self, n, tiles):
         """sgs_get_binning -> numpy copies: keys (E,) u64, idx (E,) u32, ranges (tiles,2) u32, culled (n,) u8."""

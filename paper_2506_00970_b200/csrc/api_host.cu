@@ -131,8 +131,8 @@ int sgs_track_iter_host(sgs_ctx* c, const sgs_camera* cam, float lambda_d, float
     if (r != SGS_OK) return r;
     sgs_images ren, tgt = {c->target_rgb, c->target_depth, nullptr, nullptr};
     dev_images(c->host_img_dev, px, &ren);
-    if ((r = sgs_render(c, &c->resident, cam, &ren, stream)) != SGS_OK) return r;
-    if ((r = sgs_backward_tracking(c, &tgt, lambda_d, normal_sign, c->pose6_dev, c->loss_dev, stream)) != SGS_OK) return r;
+    if ((r = sgs_track_iter(c, &c->resident, cam, &tgt, lambda_d, normal_sign, &ren, c->pose6_dev, c->loss_dev, stream)) != SGS_OK)
+        return r;
     if (cudaMemcpyAsync(c->pinned_small, c->loss_dev, sizeof(float) * 7, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
         cudaStreamSynchronize(s) != cudaSuccess)
         return SGS_CUDA_ERROR;

@@ -15,12 +15,12 @@ static int check_pending(sgs_ctx* c, cudaStream_t s) {
     c->last_entries = E;
     if (radix_mode(c)) {
         if (c->counters_host->overflow) {
-            c->have_forward = false;
+            c->have_forward = c->have_binning = false;
             const int r = sgs_ensure_entries(c, E, s);
             return r != SGS_OK ? r : SGS_WORKSPACE_OVERFLOW;
         }
     } else if (c->counters_host->max_tile > (unsigned)c->tile_cap) {
-        c->have_forward = false;
+        c->have_forward = c->have_binning = false;
         const int r = sgs_ensure_buckets(c, c->camd.tiles_x * c->camd.tiles_y, grown_tile_cap(c->counters_host->max_tile), s);
         return r != SGS_OK ? r : SGS_WORKSPACE_OVERFLOW;
     }
@@ -98,13 +98,14 @@ static int bin_radix(sgs_ctx* c, const sgs_surfels* sf, bool async, cudaStream_t
 
 extern "C" {
 
-int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* out, void* stream) {
+// preprocess + tile binning of one view (shared by sgs_render and sgs_track_iter)
+static int bin_view(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, cudaStream_t s) {
     if (!c || !sf || !sgs_cam_valid(cam) || sf->n < 0 || sf->n >= (1ll << 24)) return SGS_INVALID_ARGUMENT;
     if (sf->n > 0 && (!sf->mean || !sf->scale || !sf->quat || !sf->opacity || !sf->rgb)) return SGS_INVALID_ARGUMENT;
-    cudaStream_t s = (cudaStream_t)stream;
     int r = check_pending(c, s);
     if (r != SGS_OK) return r;
     c->have_forward = false;
+    c->have_binning = false;
     sgs_fill_cam(cam, &c->camd);
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
     const int64_t pixels = (int64_t)cam->width * cam->height;
@@ -113,19 +114,53 @@ int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const s
     const bool async = (c->cfg.flags & SGS_FLAG_ASYNC) != 0;
     c->last_surfels = *sf;
     c->last_cam = *cam;
-    r = radix_mode(c) ? bin_radix(c, sf, async, s) : bin_buckets(c, sf, async, s);
-    if (r != SGS_OK) return r;
-    float* planes[8];
-    for (int i = 0; i < 8; ++i) planes[i] = c->img_scratch + (size_t)i * pixels;
+    return radix_mode(c) ? bin_radix(c, sf, async, s) : bin_buckets(c, sf, async, s);
+}
+
+static void pick_planes(sgs_ctx* c, const sgs_images* out, int64_t pixels, bool scratch, float* planes[8]) {
+    for (int i = 0; i < 8; ++i) planes[i] = scratch ? c->img_scratch + (size_t)i * pixels : nullptr;
     if (out) {
         if (out->rgb) for (int i = 0; i < 3; ++i) planes[i] = out->rgb + (size_t)i * pixels;
         if (out->depth) planes[3] = out->depth;
         if (out->normal) for (int i = 0; i < 3; ++i) planes[4 + i] = out->normal + (size_t)i * pixels;
         if (out->alpha) planes[7] = out->alpha;
     }
+}
+
+int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* out, void* stream) {
+    cudaStream_t s = (cudaStream_t)stream;
+    int r = bin_view(c, sf, cam, s);
+    if (r != SGS_OK) return r;
+    const int64_t pixels = (int64_t)cam->width * cam->height;
+    float* planes[8];
+    pick_planes(c, out, pixels, true, planes);
     for (int i = 0; i < 8; ++i) c->last_img[i] = planes[i];
     if (sgs_launch_forward(c, planes, s) != cudaSuccess) return SGS_CUDA_ERROR;
     c->have_forward = true;
+    c->have_binning = true;
+    return SGS_OK;
+}
+
+int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* target, float lambda_d,
+                   float normal_sign, const sgs_images* out, float* d_pose6, float* loss, void* stream) {
+    if (!c || !target || !target->rgb || !target->depth || !d_pose6) return SGS_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (radix_mode(c)) {  // A/B binning path: the unfused sequence
+        int r = sgs_render(c, sf, cam, out, stream);
+        if (r != SGS_OK) return r;
+        r = sgs_backward_tracking(c, target, lambda_d, normal_sign, d_pose6, loss, stream);
+        c->have_forward = false;
+        return r;
+    }
+    int r = bin_view(c, sf, cam, s);
+    if (r != SGS_OK) return r;
+    const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    if ((r = sgs_ensure_partials(c, tiles, s)) != SGS_OK) return r;
+    float* planes[8];
+    pick_planes(c, out, (int64_t)cam->width * cam->height, false, planes);
+    if (sgs_launch_track(c, planes, target->rgb, target->depth, lambda_d, normal_sign, d_pose6, loss, s) != cudaSuccess)
+        return SGS_CUDA_ERROR;
+    c->have_binning = true;
     return SGS_OK;
 }
 
@@ -190,7 +225,7 @@ int sgs_get_binning(sgs_ctx* c, int64_t* n_entries, const uint64_t** keys, const
     if (!c) return SGS_INVALID_ARGUMENT;
     int r = check_pending(c, 0);
     if (r != SGS_OK) return r;
-    if (!c->have_forward) return SGS_NO_FORWARD_STATE;
+    if (!c->have_binning) return SGS_NO_FORWARD_STATE;
     if (cudaDeviceSynchronize() != cudaSuccess) return SGS_CUDA_ERROR;
     const int64_t E = (int64_t)c->counters_host->n_entries;
     if (n_entries) *n_entries = E;

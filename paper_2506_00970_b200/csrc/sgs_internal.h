@@ -97,6 +97,7 @@ struct sgs_ctx {
     cudaEvent_t counters_ready;
     // last forward
     bool have_forward;
+    bool have_binning;               // sorted lists + ranges of the last render / track_iter are valid
     bool pending_check;              // async mode: counters_host not yet examined
     sgs_surfels last_surfels;
     sgs_camera last_cam;
@@ -134,6 +135,8 @@ cudaError_t sgs_launch_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const fl
 cudaError_t sgs_launch_export_idx(sgs_ctx* c, cudaStream_t s);
 cudaError_t sgs_launch_backward_tracking(sgs_ctx* c, const float* trgb, const float* tdepth, float lambda_d, float nsign,
                                          float* d_pose6, float* loss, cudaStream_t s);
+cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* trgb, const float* tdepth, float lambda_d,
+                             float nsign, float* d_pose6, float* loss, cudaStream_t s);
 int sgs_sort_passes(int tiles);
 cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cudaStream_t s);
 cudaError_t sgs_launch_tilesort(sgs_ctx* c, cudaStream_t s);

@@ -1,0 +1,335 @@
+// track.cu -- K-track: ONE launch per tracking iteration after K-pre.
+//
+// A tracking iteration renders the active map (Eq. 8), evaluates the masked L1 colour + depth loss of
+// Eq. 15-19 against the current frame, and back-propagates to the 6-DoF pose only (Eq. 11-13; the splats
+// are frozen, L204).  The loss couples nothing across pixels, so the whole chain runs per tile inside one
+// block:  in-tile sort -> forward compositing -> loss and upstream gradients in registers -> reverse
+// traversal -> block reduction -> grid reduction.  Compared with k_forward + k_backward<pose-only> this
+// removes a launch, the T_final / n_last / image round trip through L2, the backward's prologue loads and
+// -- for tiles whose list fits one 256-entry batch (the common case in tracking) -- the second staging
+// gather: the staged records of the forward walk are walked again in reverse.
+// Arithmetic is pair.cuh's (identical decisions to k_forward / k_backward); the tracking loss has no
+// normal / alpha gradient, so those terms of the general backward are dropped at compile time.
+#include "pair.cuh"
+#include "reduce.cuh"
+#include "sgs_internal.h"
+
+namespace {
+
+struct TrackPlanes { float* p[8]; };
+
+constexpr uint32_t TRK_PL = SGS_BLOCK * 16;  // bytes per staged plane
+constexpr int TRK_MAX_SORT = 2048;           // largest bucket ordered inside the kernel (= fused-sort tile_cap bound)
+
+// One thread stages entry `v` of the tile: forward record (s0..s4) plus the backward's a_u, a_v, m = a_u x a_v.
+__device__ __forceinline__ unsigned stage_track(const SgsPayload& pay, uint32_t v, double px0, double py0, float tx0,
+                                                float ty0, float4 (*sh)[SGS_BLOCK], int tid) {
+    const float4 g0 = pay.g0[v], g1 = pay.g1[v], g3 = pay.g3[v], g4 = pay.g4[v], g5 = pay.g5[v], g6 = pay.g6[v];
+    const float4 g7 = pay.g7[v];
+    const double2 g2 = pay.g2[v];
+    float4 s0, s1, s2;
+    stage_entry(g0, g1, g2, g3, px0, py0, s0, s1, s2);
+    sh[0][tid] = s0; sh[1][tid] = s1; sh[2][tid] = s2;
+    sh[3][tid] = make_float4(g1.w, g3.w, g4.x, g4.y);
+    sh[4][tid] = make_float4(g4.z, g4.w, g5.x, 0.f);
+    const float aux = g5.y, auy = g5.z, auz = g5.w, avx = g6.x, avy = g6.y, avz = g6.z;
+    sh[5][tid] = make_float4(aux, auy, auz, avx);
+    sh[6][tid] = make_float4(avy, avz, auy * avz - auz * avy, auz * avx - aux * avz);
+    sh[7][tid] = make_float4(aux * avy - auy * avx, 0.f, 0.f, 0.f);
+    return warp_patch_mask(g7, tx0, ty0);
+}
+
+// (u, v) and rho^2 of one pair (pair.cuh's sequence)
+__device__ __forceinline__ float pair_rho2(const float4 s0, const float4 s1, const float4 s2, float lx, float ly, float& u,
+                                           float& v) {
+    const float un = __fmaf_rn(ly, s0.y, __fmaf_rn(lx, s0.x, s0.z));
+    const float vn = __fmaf_rn(ly, s1.y, __fmaf_rn(lx, s1.x, s1.z));
+    const float dn = __fmaf_rn(ly, s1.w, __fmaf_rn(lx, s0.w, s2.x));
+    const float inv = fast_rcp(dn);
+    u = __fmul_rn(un, inv); v = __fmul_rn(vn, inv);
+    return __fmaf_rn(v, v, __fmul_rn(u, u));
+}
+
+// Eq. 8 for one pair that passed the cutoff somewhere in the warp (k_forward's sequence)
+__device__ __forceinline__ void fwd_composite(uint32_t ea, const float4 s2, float u, float v, float rho2, bool pass,
+                                              uint32_t last_if, const SgsCfgDev& cfg, float& T, bool& done, uint32_t& last,
+                                              float& C0, float& C1, float& C2, float& Dp, float& N0, float& N1, float& N2,
+                                              float& O) {
+    const float4 s3 = lds128(ea + 3 * TRK_PL), s4 = lds128(ea + 4 * TRK_PL);
+    const float z = __fmaf_rn(s2.z, v, __fmaf_rn(s2.y, u, s2.w));
+    const float G = fast_ex2(__fmul_rn(rho2, -0.72134752044448170368f));
+    const float a = fminf(cfg.alpha_max, __fmul_rn(s3.x, G));
+    pass = pass && (z > cfg.z_near) && (a >= cfg.alpha_min);
+    const float Tn = __fmul_rn(T, 1.f - a);
+    const bool stop = pass && (Tn < cfg.t_min);  // R6: stop, this splat is not composited
+    done = done || stop;
+    pass = pass && !stop;
+    const float w = pass ? __fmul_rn(a, T) : 0.f;
+    C0 = __fmaf_rn(w, s3.y, C0); C1 = __fmaf_rn(w, s3.z, C1); C2 = __fmaf_rn(w, s3.w, C2);
+    Dp = __fmaf_rn(w, z, Dp);
+    N0 = __fmaf_rn(w, s4.x, N0); N1 = __fmaf_rn(w, s4.y, N1); N2 = __fmaf_rn(w, s4.z, N2);
+    O += w;
+    T = pass ? Tn : T;
+    last = pass ? last_if : last;
+}
+
+// Backward of one composited pair, pose-only, tracking loss (g_normal = g_alpha = 0): k_backward's sequence.
+__device__ __forceinline__ void bwd_pair(uint32_t ea, const float4 s3, const PairResult& r, float g0, float g1, float g2,
+                                         float g3, float rx, float ry, float alpha_max, float& T_after, float& suffix,
+                                         float& F0, float& F1, float& F2, float& Z0, float& Z1, float& Z2) {
+    const float4 s5 = lds128(ea + 5 * TRK_PL), s6 = lds128(ea + 6 * TRK_PL), s7 = lds128(ea + 7 * TRK_PL);
+    const float inv1ma = fast_rcp(1.f - r.a);
+    const float Ti = T_after * inv1ma;  // transmittance in front of this splat
+    const float w = r.a * Ti;
+    const float gv = g0 * s3.y + g1 * s3.z + g2 * s3.w + g3 * r.z;
+    const float da = Ti * gv - suffix * inv1ma;
+    suffix = fmaf(w, gv, suffix);
+    T_after = Ti;
+    const bool clamped = s3.x * r.G > alpha_max;  // R5: true derivative, zero when clamped
+    const float dG = clamped ? 0.f : da * s3.x;
+    const float gu = -r.u * r.G * dG, gvv = -r.v * r.G * dG, gz = g3 * w;
+    // f = [ r x (a_v gu - a_u gv) + m gz ] / (r . m)
+    const float q0 = s5.w * gu - s5.x * gvv, q1 = s6.x * gu - s5.y * gvv, q2 = s6.y * gu - s5.z * gvv;
+    const float m0 = s6.z, m1 = s6.w, m2 = s7.x;
+    const float inv_rm = fast_rcp(rx * m0 + ry * m1 + m2);
+    const float f0 = (ry * q2 - q1 + m0 * gz) * inv_rm;
+    const float f1 = (q0 - rx * q2 + m1 * gz) * inv_rm;
+    const float f2 = (rx * q1 - ry * q0 + m2 * gz) * inv_rm;
+    F0 += f0; F1 += f1; F2 += f2;
+    Z0 = fmaf(r.z, f0, Z0); Z1 = fmaf(r.z, f1, Z1); Z2 = fmaf(r.z, f2, Z2);
+}
+
+template <bool WRITE_IMAGES>
+__global__ void __launch_bounds__(SGS_BLOCK, 3)
+k_track(uint32_t* __restrict__ ranges, const uint32_t* __restrict__ cursor, unsigned long long* bucket, uint32_t tile_cap,
+        int presorted, SgsPayload pay, int W, int H, int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg,
+        TrackPlanes out, const float* __restrict__ trgb, const float* __restrict__ tdepth, float lambda_d, float nsign,
+        float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
+        float* __restrict__ loss_out) {
+    __shared__ float4 sh[8][SGS_BLOCK];
+    __shared__ uint32_t s_idx[TRK_MAX_SORT];
+    __shared__ unsigned char sh_mask[SGS_BLOCK];
+    __shared__ float s_red[8][7];
+    __shared__ uint32_t s_wmax[8];
+    const uint32_t sa = smem_addr(&sh[0][0]), sm_a = smem_addr(sh_mask);
+    const int tile = blockIdx.x;
+    const int tx = tile % tiles_x, ty = tile / tiles_x;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int lxi = (wid & 1) * 8 + (lane & 7), lyi = (wid >> 1) * 4 + (lane >> 3);
+    const int px = tx * SGS_TILE + lxi, py = ty * SGS_TILE + lyi;
+    const bool inside = px < W && py < H;
+    const float lx = (float)lxi, ly = (float)lyi;
+    const float tx0 = (float)(tx * SGS_TILE), ty0 = (float)(ty * SGS_TILE);
+    const double px0 = (double)(tx * SGS_TILE) + 0.5, py0 = (double)(ty * SGS_TILE) + 0.5;
+    const size_t pix = (size_t)py * W + px, HW = (size_t)W * H;
+
+    // the current frame's pixel: issued first, consumed after the forward walk
+    float tr = 0.f, tg = 0.f, tb = 0.f, td = 0.f;
+    if (inside) { tr = __ldg(trgb + pix); tg = __ldg(trgb + HW + pix); tb = __ldg(trgb + 2 * HW + pix); td = __ldg(tdepth + pix); }
+
+    // ---- tile list: order the bucket by (depth bits, index) (tilesort.cu's contract) ----
+    const uint32_t raw = cursor[tile];
+    const uint32_t n = raw < tile_cap ? raw : tile_cap;
+    const uint32_t start = tile * tile_cap;
+    unsigned long long* g = bucket + (size_t)start;
+    if (tid == 0) { ranges[2 * tile] = start; ranges[2 * tile + 1] = start + n; }
+    const bool in_smem = !presorted && n <= TRK_MAX_SORT;  // sorted indices live in s_idx
+    if (!presorted) {
+        unsigned long long* sk = reinterpret_cast<unsigned long long*>(&sh[0][0]);
+        if (n == 1) {
+            if (tid == 0) s_idx[0] = (uint32_t)g[0];
+        } else if (n <= SGS_BLOCK) {
+            // rank by counting (keys are unique); only warps that own keys walk the list
+            const bool mine = (uint32_t)tid < n;
+            const unsigned long long key = mine ? g[tid] : ~0ull;
+            if (mine) sk[tid] = key;
+            __syncthreads();
+            if ((uint32_t)(wid * 32) < n) {
+                uint32_t rank = 0;
+                for (uint32_t k = 0; k < n; ++k) rank += sk[k] < key ? 1u : 0u;
+                if (mine) { g[rank] = key; s_idx[rank] = (uint32_t)key; }
+            }
+        } else {
+            uint32_t npad = 512;
+            while (npad < n) npad <<= 1;
+            for (uint32_t i = tid; i < npad; i += SGS_BLOCK) sk[i] = i < n ? g[i] : ~0ull;
+            __syncthreads();
+            for (uint32_t k = 2; k <= npad; k <<= 1)
+                for (uint32_t j = k >> 1; j > 0; j >>= 1) {
+                    for (uint32_t t = tid; t < (npad >> 1); t += SGS_BLOCK) {
+                        const uint32_t i = ((t & ~(j - 1)) << 1) | (t & (j - 1)), p = i | j;
+                        const unsigned long long a = sk[i], b = sk[p];
+                        if ((a > b) == ((i & k) == 0)) { sk[i] = b; sk[p] = a; }
+                    }
+                    __syncthreads();
+                }
+            for (uint32_t i = tid; i < n; i += SGS_BLOCK) { const unsigned long long k2 = sk[i]; g[i] = k2; s_idx[i] = (uint32_t)k2; }
+        }
+        __syncthreads();  // s_idx complete; staging memory free
+    }
+
+    // ---- forward compositing (Eq. 8), as k_forward ----
+    float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dp = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f, O = 0.f;
+    uint32_t last = 0;
+    bool done = !inside;
+    int staged_b = -1;  // batch currently held in shared memory
+    for (uint32_t boff = 0; boff < n; boff += SGS_BLOCK) {
+        if (__syncthreads_and(done)) break;
+        const uint32_t nb = min((uint32_t)SGS_BLOCK, n - boff);
+        unsigned mask = 0;
+        if ((uint32_t)tid < nb) {
+            const uint32_t v = in_smem ? s_idx[boff + tid] : (uint32_t)g[boff + tid];
+            mask = stage_track(pay, v, px0, py0, tx0, ty0, sh, tid);
+        }
+        sh_mask[tid] = (unsigned char)mask;
+        staged_b = (int)(boff / SGS_BLOCK);
+        __syncthreads();
+        for (uint32_t c0 = 0; c0 < nb; c0 += 32) {
+            if (__all_sync(0xffffffffu, done)) break;
+            unsigned m = __ballot_sync(0xffffffffu, (lds_u8(sm_a + c0 + lane) >> wid) & 1u);
+            while (m) {
+                // two entries per trip: their LDS -> FMA -> RCP chains are independent and overlap; only the
+                // T / done recurrence is sequential (first A, then B)
+                const uint32_t ja = c0 + (uint32_t)__ffs(m) - 1u;
+                m &= m - 1u;
+                const bool two = m != 0u;
+                const uint32_t jb = two ? c0 + (uint32_t)__ffs(m) - 1u : ja;
+                m &= m - 1u;
+                const uint32_t ea = sa + ja * 16u, eb = sa + jb * 16u;
+                const float4 a0 = lds128(ea), a1 = lds128(ea + TRK_PL), a2 = lds128(ea + 2 * TRK_PL);
+                const float4 b0 = lds128(eb), b1 = lds128(eb + TRK_PL), b2 = lds128(eb + 2 * TRK_PL);
+                float ua, va, ub, vb;
+                const float rho2a = pair_rho2(a0, a1, a2, lx, ly, ua, va);
+                const float rho2b = pair_rho2(b0, b1, b2, lx, ly, ub, vb);
+                const bool pa = !done && (rho2a <= cfg.cutoff2);
+                const bool pb = two && (rho2b <= cfg.cutoff2);
+                const bool anya = __any_sync(0xffffffffu, pa), anyb = __any_sync(0xffffffffu, pb);
+                if (anya) fwd_composite(ea, a2, ua, va, rho2a, pa, boff + ja + 1, cfg, T, done, last, C0, C1, C2, Dp, N0, N1, N2, O);
+                if (anyb) fwd_composite(eb, b2, ub, vb, rho2b, pb && !done, boff + jb + 1, cfg, T, done, last, C0, C1, C2, Dp, N0, N1, N2, O);
+            }
+        }
+    }
+    if (WRITE_IMAGES && inside) {
+        if (out.p[0]) out.p[0][pix] = C0;
+        if (out.p[1]) out.p[1][pix] = C1;
+        if (out.p[2]) out.p[2][pix] = C2;
+        if (out.p[3]) out.p[3][pix] = Dp;
+        if (out.p[4]) out.p[4][pix] = N0;
+        if (out.p[5]) out.p[5][pix] = N1;
+        if (out.p[6]) out.p[6][pix] = N2;
+        if (out.p[7]) out.p[7][pix] = O;
+    }
+
+    // ---- Eq. 15-19 in registers (same arithmetic as loss.cu): loss term and upstream gradients of rgb, depth ----
+    const float rx = ((float)px + 0.5f - cx) / fx, ry = ((float)py + 0.5f - cy) / fy;  // pixel ray (rx, ry, 1)
+    float g0 = 0.f, g1 = 0.f, g2 = 0.f, g3 = 0.f, my_loss = 0.f;
+    if (inside) {
+        const float inv = 1.f / (float)HW;
+        const float nr = N0 * rx + N1 * ry + N2;
+        if ((nsign * nr > 0.f) && (O > 0.95f)) {  // M_n M_o (Eq. 17-18)
+            float d = C0 - tr; my_loss += fabsf(d); g0 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
+            d = C1 - tg; my_loss += fabsf(d); g1 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
+            d = C2 - tb; my_loss += fabsf(d); g2 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
+            d = Dp - td; my_loss += lambda_d * fabsf(d);
+            g3 = d > 0.f ? lambda_d * inv : (d < 0.f ? -lambda_d * inv : 0.f);
+        }
+        my_loss *= inv;
+    }
+    if (!(g0 != 0.f || g1 != 0.f || g2 != 0.f || g3 != 0.f)) last = 0;  // every backward term carries a factor g
+
+    // ---- reverse traversal (as k_backward<POSE_ONLY>, g_normal = g_alpha = 0) ----
+    uint32_t wmax = last;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
+    if (lane == 0) s_wmax[wid] = wmax;
+    __syncthreads();  // also: every warp has left the forward walk
+    uint32_t bmax = 0;
+#pragma unroll
+    for (int w2 = 0; w2 < 8; ++w2) bmax = max(bmax, s_wmax[w2]);
+
+    float T_after = T, suffix = 0.f;
+    float F0 = 0.f, F1 = 0.f, F2 = 0.f, Z0 = 0.f, Z1 = 0.f, Z2 = 0.f;
+    const int n_batches = (int)((bmax + SGS_BLOCK - 1) / SGS_BLOCK);
+    for (int b = n_batches - 1; b >= 0; --b) {
+        const uint32_t boff = (uint32_t)b * SGS_BLOCK;
+        const uint32_t nb = min((uint32_t)SGS_BLOCK, bmax - boff);
+        if (b != staged_b) {  // block-uniform
+            __syncthreads();  // previous batch fully consumed
+            unsigned mask = 0;
+            if ((uint32_t)tid < nb) {
+                const uint32_t v = in_smem ? s_idx[boff + tid] : (uint32_t)g[boff + tid];
+                mask = stage_track(pay, v, px0, py0, tx0, ty0, sh, tid);
+            }
+            sh_mask[tid] = (unsigned char)mask;
+            staged_b = b;
+            __syncthreads();
+        }
+        const int jend = (int)min(nb, wmax > boff ? wmax - boff : 0u);  // exclusive
+        for (int c0 = ((jend - 1) >> 5) << 5; c0 >= 0 && jend > 0; c0 -= 32) {
+            unsigned m = __ballot_sync(0xffffffffu, (c0 + lane < jend) && ((lds_u8(sm_a + c0 + lane) >> wid) & 1u));
+            while (m) {
+                // two entries per trip (back to front: A then B); the pair tests overlap, the T / suffix
+                // recurrence runs A first, then B
+                const int ha = 31 - __clz(m);
+                m &= ~(1u << ha);
+                const bool two = m != 0u;
+                const int hb = two ? 31 - __clz(m) : ha;
+                m &= ~(1u << hb);
+                const uint32_t ja = (uint32_t)(c0 + ha), jb = (uint32_t)(c0 + hb);
+                const uint32_t ea = sa + ja * 16u, eb = sa + jb * 16u;
+                const float4 a0 = lds128(ea), a1 = lds128(ea + TRK_PL), a2 = lds128(ea + 2 * TRK_PL), a3 = lds128(ea + 3 * TRK_PL);
+                const float4 b0 = lds128(eb), b1 = lds128(eb + TRK_PL), b2 = lds128(eb + 2 * TRK_PL), b3 = lds128(eb + 3 * TRK_PL);
+                PairResult ra, rb;
+                bool hita = (boff + ja) < last, hitb = two && (boff + jb) < last;
+                if (hita) hita = eval_pair(a0, a1, a2, a3.x, lx, ly, cfg.cutoff2, cfg.alpha_min, cfg.alpha_max, cfg.z_near, ra);
+                if (hitb) hitb = eval_pair(b0, b1, b2, b3.x, lx, ly, cfg.cutoff2, cfg.alpha_min, cfg.alpha_max, cfg.z_near, rb);
+                if (__any_sync(0xffffffffu, hita) && hita)
+                    bwd_pair(ea, a3, ra, g0, g1, g2, g3, rx, ry, cfg.alpha_max, T_after, suffix, F0, F1, F2, Z0, Z1, Z2);
+                if (__any_sync(0xffffffffu, hitb) && hitb)
+                    bwd_pair(eb, b3, rb, g0, g1, g2, g3, rx, ry, cfg.alpha_max, T_after, suffix, F0, F1, F2, Z0, Z1, Z2);
+            }
+        }
+    }
+    // Eq. 11-13 per pixel: rho += sum f; theta += r x sum(z f)   (g_N = 0 in tracking)
+    float p6[7];
+    p6[0] = F0; p6[1] = F1; p6[2] = F2;
+    p6[3] = ry * Z2 - Z1; p6[4] = Z0 - rx * Z2; p6[5] = rx * Z1 - ry * Z0;
+    p6[6] = my_loss;
+#pragma unroll
+    for (int c = 0; c < 7; ++c) {
+        const float s = warp_sum(inside ? p6[c] : 0.f);
+        if (lane == 0) s_red[wid][c] = s;
+    }
+    __syncthreads();
+    if (tid < 7) {
+        float s = 0.f;
+#pragma unroll
+        for (int w2 = 0; w2 < 8; ++w2) s += s_red[w2][tid];
+        pose_partial[(size_t)tile * 8 + tid] = s;
+    }
+    finish_pose(pose_partial, gridDim.x, counters, d_pose6, loss_out);
+}
+
+}  // namespace
+
+cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* trgb, const float* tdepth, float lambda_d,
+                             float nsign, float* d_pose6, float* loss, cudaStream_t s) {
+    const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    const SgsCamDev& cam = c->camd;
+    TrackPlanes out;
+    bool any = false;
+    for (int i = 0; i < 8; ++i) { out.p[i] = planes ? planes[i] : nullptr; any = any || out.p[i] != nullptr; }
+    SgsStage st(c, SGS_STAGE_FORWARD, s);
+    c->launches += 1;
+    unsigned long long* bucket = reinterpret_cast<unsigned long long*>(c->bucket);
+    const int presorted = c->fused_sort ? 0 : 1;
+    if (any)
+        k_track<true><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->cursor, bucket, (uint32_t)c->tile_cap, presorted, c->pay, cam.W,
+                                                  cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb,
+                                                  tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss);
+    else
+        k_track<false><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->cursor, bucket, (uint32_t)c->tile_cap, presorted, c->pay, cam.W,
+                                                   cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb,
+                                                   tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss);
+    return cudaGetLastError();
+}

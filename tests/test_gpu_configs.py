@@ -108,6 +108,20 @@ def check_config(name, views, full):
                 assert abs(float(lossf.item()) - L_ref) <= 2e-4 * abs(L_ref)
                 posef = p6f.cpu().numpy().astype(np.float64)
                 assert np.abs(posef - og["pose"]).max() <= 2e-3 * np.abs(og["pose"]).max(), (name, v, posef, og["pose"])
+                # ... and the single-launch iteration (sgs_track_iter: sort + render + loss + backward in one kernel)
+                im2 = alloc_images(cam)
+                p6t, losst = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+                for _ in range(2):
+                    ren.track_iter(sf, c, trgb, tdep, LAMBDA_D, NSIGN, p6t, losst, **im2)
+                    ren.stats()
+                assert np.array_equal(planes(im2), gimg)                      # same images, bit for bit
+                assert_binning(ren.get_binning(sc.n, tiles), oracle.binning(sc, camv, cfg))
+                assert abs(float(losst.item()) - float(lossf.item())) <= 1e-6 * abs(L_ref)
+                poset = p6t.cpu().numpy().astype(np.float64)
+                assert np.abs(poset - posef).max() <= 1e-5 * np.abs(posef).max(), (poset, posef)
+                assert np.abs(poset - og["pose"]).max() <= 2e-3 * np.abs(og["pose"]).max(), (name, v, poset, og["pose"])
+                ren.track_iter(sf, c, trgb, tdep, LAMBDA_D, NSIGN, p6t, losst)   # no image outputs
+                np.testing.assert_allclose(p6t.cpu().numpy(), poset, rtol=1e-5, atol=1e-7 * np.abs(poset).max())
     finally:
         ren.close()
 

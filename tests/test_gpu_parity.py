@@ -293,3 +293,39 @@ def test_tile_bucket_overflow_grows(ren):
     a.stats()
     assert np.array_equal(planes(im), out["img"])
     a.close()
+
+
+def test_track_iter_matches_unfused_sequence():
+    """sgs_track_iter == sgs_render + sgs_backward_tracking on C1 (short lists) and on a tile list longer than one
+    256-entry batch and longer than the in-kernel sort bound (bucket regrowth -> pre-sorted path)."""
+    cases = []
+    sc, cams, _ = scenegen.make_config("C1")
+    cases.append((sc, cams[0]))
+    g = scenegen.SplitMix(11)
+    for n in (900, 6000):   # ~n entries on the central tiles: multi-batch; > 2048 -> tilesort pre-pass
+        mean = np.stack([g.uniform(n, -0.05, 0.05), g.uniform(n, -0.05, 0.05), g.uniform(n, 1.0, 3.0)], 1).astype(np.float32)
+        cases.append((Scene(mean, np.full((n, 2), 0.01, np.float32), np.tile(np.float32([1, 0.1, 0, 0]), (n, 1)),
+                            np.full(n, 0.03 if n > 2000 else 0.2, np.float32),
+                            np.stack([g.uniform(n) for _ in range(3)], 1).astype(np.float32)),
+                      Camera(64, 48, 60.0, 60.0, 32.0, 24.0)))
+    for sc, cam in cases:
+        ren = sgs.Renderer()
+        t, sf = to_device(sc)
+        c = camera(cam)
+        im, im2 = alloc_images(cam), alloc_images(cam)
+        ren.render(sf, c, **im)
+        tgt_rgb = (im["rgb"] * 0.9 + 0.01).contiguous()
+        tgt_dep = (im["depth"] * 1.02).contiguous()
+        p6a, la = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+        ren.backward_tracking(tgt_rgb, tgt_dep, 0.5, 1.0, p6a, la)
+        p6b, lb = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+        ren.track_iter(sf, c, tgt_rgb, tgt_dep, 0.5, 1.0, p6b, lb, **im2)
+        torch.cuda.synchronize()
+        assert np.array_equal(planes(im), planes(im2))
+        assert float(la.abs().item()) > 0 and np.abs(p6a.cpu().numpy()).max() > 0
+        np.testing.assert_allclose(lb.cpu().numpy(), la.cpu().numpy(), rtol=1e-5)
+        np.testing.assert_allclose(p6b.cpu().numpy(), p6a.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(p6a.abs().max()))
+        with pytest.raises(sgs.SgsError) as e:   # track_iter leaves no state for sgs_backward
+            ren.backward(d_pose6=p6a)
+        assert e.value.status == sgs.SGS_NO_FORWARD_STATE
+        ren.close()
