@@ -404,7 +404,8 @@ def main():
                             surfels=wl.sc.n, active=wl.n_active, width=wl.W, height=wl.H, renders_per_step=wl.renders_per_step,
                             l2="flushed between steps by a 256 MiB write; iterations inside a step reuse the map as tracking does",
                             replicas=world),
-                clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roof, stages=stages, cpu_baseline=cpu)
+                clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roof, stages=stages, cpu_baseline=cpu,
+                stage_us={k: round(1e3 * v[0] / v[1], 2) for k, v in prof.items() if v[1]})
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

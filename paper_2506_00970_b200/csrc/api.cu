@@ -122,6 +122,12 @@ void sgs_fill_cam(const sgs_camera* cam, SgsCamDev* d) {
         for (int j = 0; j < 3; ++j) { d->R[3 * i + j] = cam->T_cw[4 * i + j]; d->Rf[3 * i + j] = cam->T_cw[4 * i + j]; }
         d->t[i] = cam->T_cw[4 * i + 3]; d->tf[i] = cam->T_cw[4 * i + 3];
     }
+    d->pc_cxr = cam->cx - (float)cam->width; d->pc_cyr = cam->cy - (float)cam->height;
+    d->pc_n[0] = sqrtf(cam->fx * cam->fx + cam->cx * cam->cx) * 1.00001f;
+    d->pc_n[1] = sqrtf(cam->fx * cam->fx + d->pc_cxr * d->pc_cxr) * 1.00001f;
+    d->pc_n[2] = sqrtf(cam->fy * cam->fy + cam->cy * cam->cy) * 1.00001f;
+    d->pc_n[3] = sqrtf(cam->fy * cam->fy + d->pc_cyr * d->pc_cyr) * 1.00001f;
+    d->pc_tabs = fabsf(d->tf[0]) + fabsf(d->tf[1]) + fabsf(d->tf[2]) + 1.f;
 }
 
 bool sgs_cam_valid(const sgs_camera* cam) {
@@ -177,6 +183,7 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
     memset(c, 0, sizeof(*c));
     c->cfg = *cfg;
     c->cfgd.cutoff2 = cfg->cutoff * cfg->cutoff;
+    c->cfgd.cutoff = sqrtf(c->cfgd.cutoff2);
     c->cfgd.alpha_min = cfg->alpha_min; c->cfgd.alpha_max = cfg->alpha_max;
     c->cfgd.t_min = cfg->t_min; c->cfgd.z_near = cfg->z_near;
     c->cfgd.cutoff2_d = (double)cfg->cutoff * (double)cfg->cutoff;

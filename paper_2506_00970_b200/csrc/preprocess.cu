@@ -128,18 +128,15 @@ __device__ __forceinline__ bool precull_f32(const float* __restrict__ mean, cons
     const float X = cam.Rf[0] * m0 + cam.Rf[1] * m1 + cam.Rf[2] * m2 + cam.tf[0];
     const float Y = cam.Rf[3] * m0 + cam.Rf[4] * m1 + cam.Rf[5] * m2 + cam.tf[1];
     const float Z = cam.Rf[6] * m0 + cam.Rf[7] * m1 + cam.Rf[8] * m2 + cam.tf[2];
-    const float d = 1e-5f * (fabsf(m0) + fabsf(m1) + fabsf(m2) + fabsf(cam.tf[0]) + fabsf(cam.tf[1]) + fabsf(cam.tf[2]) + 1.f);
+    const float d = 1e-5f * (fabsf(m0) + fabsf(m1) + fabsf(m2) + cam.pc_tabs);
     if (Z + d < cfg.z_near) return true;
-    const float r = sqrtf(cfg.cutoff2) * fmaxf(fabsf(scale[0]), fabsf(scale[1])) * 1.00001f + d;
-    const float cxr = cam.cx - (float)cam.W, cyr = cam.cy - (float)cam.H;
+    const float r = cfg.cutoff * fmaxf(fabsf(scale[0]), fabsf(scale[1])) * 1.00001f + d;
     // left: fx X + cx Z < 0 ; right: fx X + (cx - W) Z > 0 ; top / bottom alike.  Normals un-normalised:
-    // compare against r * |normal| (rounded up by the 1.00001 factor above and a second one here).
-    const float nl = sqrtf(cam.fx * cam.fx + cam.cx * cam.cx) * 1.00001f, nr = sqrtf(cam.fx * cam.fx + cxr * cxr) * 1.00001f;
-    const float nt = sqrtf(cam.fy * cam.fy + cam.cy * cam.cy) * 1.00001f, nb = sqrtf(cam.fy * cam.fy + cyr * cyr) * 1.00001f;
-    if (cam.fx * X + cam.cx * Z < -r * nl) return true;
-    if (cam.fx * X + cxr * Z > r * nr) return true;
-    if (cam.fy * Y + cam.cy * Z < -r * nt) return true;
-    if (cam.fy * Y + cyr * Z > r * nb) return true;
+    // compare against r * |normal| (|normal| rounded up on the host, cam.pc_n, and r rounded up above).
+    if (cam.fx * X + cam.cx * Z < -r * cam.pc_n[0]) return true;
+    if (cam.fx * X + cam.pc_cxr * Z > r * cam.pc_n[1]) return true;
+    if (cam.fy * Y + cam.cy * Z < -r * cam.pc_n[2]) return true;
+    if (cam.fy * Y + cam.pc_cyr * Z > r * cam.pc_n[3]) return true;
     return false;
 }
 
@@ -241,86 +238,172 @@ k_preprocess(int64_t n, const float* __restrict__ mean, const float* __restrict_
 
 // Bucket variant (default path): no scan at all.  Tile t owns a fixed-capacity bucket; a visible surfel
 // appends (depth bits << 32 | surfel index) to every tile of its rectangle through an atomic cursor.
-// Arrival order is irrelevant: k_tilesort orders each bucket by the full 64-bit key, which is unique
+// Arrival order is irrelevant: the in-tile sort orders each bucket by the full 64-bit key, which is unique
 // inside a tile, so the result is the stable (tile, depth, index) order of the contract.  The payload
-// is indexed by the surfel index itself (no compaction).
+// is indexed by the surfel index itself (no compaction of the payload in HBM).
+//
+// Two kernels (ncu, profiles/r01_*: with one thread per surfel doing everything, 73 % of the warps of a
+// 20 %-active map dragged all 32 lanes through the ~700-instruction binary64 path for one or two
+// survivors, the kernel sat at 3 blocks/SM on its 78 registers and 42 % of the stall samples were
+// dependent global loads):
+//   K-pre-A  light (few registers, full occupancy, 4 surfels per thread with all loads in flight together):
+//            active flag + binary32 pre-cull; writes culled = 1 for the rejected, compacts the survivors of
+//            the block in shared memory and appends them to a global list with ONE atomic per block.
+//   K-pre-B  dense: one thread per survivor runs the binary64 sequence, writes the payload, and the
+//            block's tile entries are spread over its threads (one (surfel, tile) pair each).
+constexpr int SGS_PREA_ITEMS = 4;
+constexpr int SGS_PREA_SPAN = SGS_PREA_ITEMS * SGS_PRE_BLOCK;
+
 __global__ void __launch_bounds__(SGS_PRE_BLOCK)
-k_preprocess_bucket(int64_t n, const float* __restrict__ mean, const float* __restrict__ scale,
-                    const float* __restrict__ quat, const float* __restrict__ opacity, const float* __restrict__ rgb,
-                    const uint8_t* __restrict__ active, SgsCamDev cam, SgsCfgDev cfg, SgsPayload pay,
-                    uint8_t* __restrict__ culled, SgsCounters* __restrict__ counters, uint32_t* __restrict__ cursor,
-                    uint64_t* __restrict__ bucket, uint32_t tile_cap) {
-    const int64_t i = (int64_t)blockIdx.x * SGS_PRE_BLOCK + threadIdx.x;
-    const int lane = threadIdx.x & 31;
-    PreOut o;
-    o.vis = false;
-    if (i < n && (active == nullptr || active[i] != 0) && !precull_f32(mean + 3 * i, scale + 2 * i, cam, cfg))
-        preprocess_one(mean + 3 * i, scale + 2 * i, quat + 4 * i, cam, cfg, o);
-    if (i < n) culled[i] = o.vis ? 0 : 1;
-    unsigned int cnt = o.vis ? (unsigned int)((o.tx1 - o.tx0 + 1) * (o.ty1 - o.ty0 + 1)) : 0u;
-    // totals: one atomic per warp
-    const unsigned int vis_mask = __ballot_sync(0xffffffffu, o.vis);
-    unsigned int wcnt = cnt;
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) wcnt += __shfl_xor_sync(0xffffffffu, wcnt, off);
-    if (lane == 0 && vis_mask) {
-        atomicAdd(&counters->n_visible, (unsigned int)__popc(vis_mask));
-        atomicAdd(&counters->n_entries, (unsigned long long)wcnt);
-    }
-    if (o.vis) {
-        pay.g0[i] = make_float4(o.P, o.Q, o.R, o.S);
-        pay.g1[i] = make_float4(o.D, o.E, o.F, opacity[i]);
-        pay.g2[i] = make_double2(o.xc, o.yc);
-        pay.g3[i] = make_float4(o.a, o.b, o.c, rgb[3 * i]);
-        pay.g4[i] = make_float4(rgb[3 * i + 1], rgb[3 * i + 2], o.n[0], o.n[1]);
-        pay.g5[i] = make_float4(o.n[2], o.au[0], o.au[1], o.au[2]);
-        pay.g6[i] = make_float4(o.av[0], o.av[1], o.av[2], 0.f);
-        pay.g7[i] = make_float4(o.bb[0], o.bb[1], o.bb[2], o.bb[3]);
-    }
-    // Cooperative emission: the block's entries (sum of tile counts) are spread over its threads, one
-    // (surfel, tile) pair each, so the cursor atomics of a block are all in flight together instead of
-    // one thread walking its rectangle serially (and a surfel covering hundreds of tiles costs no more
-    // than hundreds of small ones).
-    __shared__ unsigned int s_off[SGS_PRE_BLOCK + 1];
-    __shared__ unsigned long long s_key[SGS_PRE_BLOCK];
-    __shared__ unsigned int s_rect[SGS_PRE_BLOCK];   // tile index of the rectangle's first tile
-    __shared__ unsigned int s_w[SGS_PRE_BLOCK];      // rectangle width in tiles
-    __shared__ unsigned int s_wsum[SGS_PRE_BLOCK / 32];
-    const int tid = threadIdx.x, wid = tid >> 5;
-    unsigned int incl = cnt;
-#pragma unroll
-    for (int off = 1; off < 32; off <<= 1) {
-        const unsigned int t2 = __shfl_up_sync(0xffffffffu, incl, off);
-        if (lane >= off) incl += t2;
-    }
-    if (lane == 31) s_wsum[wid] = incl;
-    s_key[tid] = ((unsigned long long)o.depth_bits << 32) | (unsigned long long)(uint32_t)i;
-    s_rect[tid] = o.vis ? (unsigned int)(o.ty0 * cam.tiles_x + o.tx0) : 0u;
-    s_w[tid] = o.vis ? (unsigned int)(o.tx1 - o.tx0 + 1) : 1u;
+k_pre_select(int64_t n, const float* __restrict__ mean, const float* __restrict__ scale,
+             const uint8_t* __restrict__ active, SgsCamDev cam, SgsCfgDev cfg, uint8_t* __restrict__ culled,
+             SgsCounters* __restrict__ counters, uint32_t* __restrict__ surv_list) {
+    __shared__ unsigned short s_list[SGS_PREA_SPAN];
+    __shared__ unsigned int s_n, s_base;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int64_t base = (int64_t)blockIdx.x * SGS_PREA_SPAN;
+    if (tid == 0) s_n = 0;
     __syncthreads();
-    unsigned int wbase = 0, total = 0;
+    // all loads of the thread's items are issued before the first use
+    bool act[SGS_PREA_ITEMS];
+    float m[SGS_PREA_ITEMS][3], sc[SGS_PREA_ITEMS][2];
 #pragma unroll
-    for (int w2 = 0; w2 < SGS_PRE_BLOCK / 32; ++w2) {
-        const unsigned int x = s_wsum[w2];
-        wbase += (w2 < wid) ? x : 0u;
-        total += x;
+    for (int it = 0; it < SGS_PREA_ITEMS; ++it) {
+        const int64_t i = base + it * SGS_PRE_BLOCK + tid;
+        act[it] = i < n && (active == nullptr || active[i] != 0);
     }
-    s_off[tid] = wbase + incl - cnt;  // exclusive
-    if (tid == 0) s_off[SGS_PRE_BLOCK] = total;
-    __syncthreads();
-    for (unsigned int e = tid; e < total; e += SGS_PRE_BLOCK) {
-        // owner = last thread whose exclusive offset is <= e (and whose count is non-zero by construction)
-        int lo = 0, hi = SGS_PRE_BLOCK;  // invariant: s_off[lo] <= e < s_off[hi]
 #pragma unroll
-        for (int it = 0; it < 8; ++it) {
-            const int mid = (lo + hi) >> 1;
-            if (s_off[mid] <= e) lo = mid; else hi = mid;
+    for (int it = 0; it < SGS_PREA_ITEMS; ++it) {
+        const int64_t i = base + it * SGS_PRE_BLOCK + tid;
+        m[it][0] = m[it][1] = m[it][2] = 0.f; sc[it][0] = sc[it][1] = 0.f;
+        if (act[it]) {
+            m[it][0] = mean[3 * i]; m[it][1] = mean[3 * i + 1]; m[it][2] = mean[3 * i + 2];
+            sc[it][0] = scale[2 * i]; sc[it][1] = scale[2 * i + 1];
         }
-        const unsigned int local = e - s_off[lo], w = s_w[lo];
-        const uint32_t t = s_rect[lo] + (local / w) * (unsigned int)cam.tiles_x + (local % w);
-        const uint32_t pos = atomicAdd(&cursor[t], 1u);
-        if (pos < tile_cap) bucket[(size_t)t * tile_cap + pos] = s_key[lo];
-        else atomicMax(&counters->max_tile, pos + 1u);
+    }
+#pragma unroll
+    for (int it = 0; it < SGS_PREA_ITEMS; ++it) {
+        const int local = it * SGS_PRE_BLOCK + tid;
+        const int64_t i = base + local;
+        const bool surv = act[it] && !precull_f32(m[it], sc[it], cam, cfg);
+        if (i < n && !surv) culled[i] = 1;
+        const unsigned int bal = __ballot_sync(0xffffffffu, surv);
+        unsigned int wbase = 0;
+        if (lane == 0 && bal) wbase = atomicAdd(&s_n, (unsigned int)__popc(bal));
+        wbase = __shfl_sync(0xffffffffu, wbase, 0);
+        if (surv) s_list[wbase + __popc(bal & ((1u << lane) - 1u))] = (unsigned short)local;
+    }
+    __syncthreads();
+    const unsigned int ns = s_n;
+    if (ns == 0) return;
+    if (tid == 0) s_base = atomicAdd(&counters->n_surv, ns);
+    __syncthreads();
+    const unsigned int gb = s_base;
+    for (unsigned int k = tid; k < ns; k += SGS_PRE_BLOCK) surv_list[gb + k] = (uint32_t)(base + s_list[k]);
+}
+
+constexpr int SGS_PREB_BLOCK = 128, SGS_PREB_LOG2 = 7;  // K-pre-B block: small, so that few survivors still spread over the SMs
+
+__global__ void __launch_bounds__(SGS_PREB_BLOCK)
+k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, const float* __restrict__ quat,
+              const float* __restrict__ opacity, const float* __restrict__ rgb, SgsCamDev cam, SgsCfgDev cfg,
+              SgsPayload pay, uint8_t* __restrict__ culled, SgsCounters* __restrict__ counters,
+              const uint32_t* __restrict__ surv_list, uint32_t* __restrict__ cursor, uint64_t* __restrict__ bucket,
+              uint32_t tile_cap) {
+    __shared__ unsigned int s_off[SGS_PREB_BLOCK + 1];
+    __shared__ unsigned long long s_key[SGS_PREB_BLOCK];
+    __shared__ unsigned int s_rect[SGS_PREB_BLOCK];   // tile index of the rectangle's first tile
+    __shared__ unsigned int s_w[SGS_PREB_BLOCK];      // rectangle width in tiles
+    __shared__ unsigned int s_wsum[SGS_PREB_BLOCK / 32];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const unsigned int n_surv = counters->n_surv;   // written by K-pre-A (previous launch on the stream)
+    for (unsigned int r0 = blockIdx.x * SGS_PREB_BLOCK; r0 < n_surv; r0 += gridDim.x * SGS_PREB_BLOCK) {
+        const bool have = r0 + tid < n_surv;
+        const int64_t i = have ? (int64_t)surv_list[r0 + tid] : 0;
+        PreOut o;
+        o.vis = false;
+        o.depth_bits = 0;
+        if (have) {
+            preprocess_one(mean + 3 * i, scale + 2 * i, quat + 4 * i, cam, cfg, o);
+            culled[i] = o.vis ? 0 : 1;
+        }
+        const unsigned int cnt = o.vis ? (unsigned int)((o.tx1 - o.tx0 + 1) * (o.ty1 - o.ty0 + 1)) : 0u;
+        // totals: one atomic per warp
+        const unsigned int vis_mask = __ballot_sync(0xffffffffu, o.vis);
+        unsigned int wcnt = cnt;
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) wcnt += __shfl_xor_sync(0xffffffffu, wcnt, off);
+        if (lane == 0 && vis_mask) {
+            atomicAdd(&counters->n_visible, (unsigned int)__popc(vis_mask));
+            atomicAdd(&counters->n_entries, (unsigned long long)wcnt);
+        }
+        if (o.vis) {
+            pay.g0[i] = make_float4(o.P, o.Q, o.R, o.S);
+            pay.g1[i] = make_float4(o.D, o.E, o.F, opacity[i]);
+            pay.g2[i] = make_double2(o.xc, o.yc);
+            pay.g3[i] = make_float4(o.a, o.b, o.c, rgb[3 * i]);
+            pay.g4[i] = make_float4(rgb[3 * i + 1], rgb[3 * i + 2], o.n[0], o.n[1]);
+            pay.g5[i] = make_float4(o.n[2], o.au[0], o.au[1], o.au[2]);
+            pay.g6[i] = make_float4(o.av[0], o.av[1], o.av[2], 0.f);
+            pay.g7[i] = make_float4(o.bb[0], o.bb[1], o.bb[2], o.bb[3]);
+        }
+        // Cooperative emission: the round's entries (sum of tile counts) are spread over the block's threads,
+        // one (surfel, tile) pair each, so the cursor atomics are all in flight together instead of one
+        // thread walking its rectangle serially (a surfel covering hundreds of tiles costs no more than
+        // hundreds of small ones).
+        unsigned int incl = cnt;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const unsigned int t2 = __shfl_up_sync(0xffffffffu, incl, off);
+            if (lane >= off) incl += t2;
+        }
+        if (lane == 31) s_wsum[wid] = incl;
+        s_key[tid] = ((unsigned long long)o.depth_bits << 32) | (unsigned long long)(uint32_t)i;
+        s_rect[tid] = o.vis ? (unsigned int)(o.ty0 * cam.tiles_x + o.tx0) : 0u;
+        s_w[tid] = o.vis ? (unsigned int)(o.tx1 - o.tx0 + 1) : 1u;
+        __syncthreads();
+        unsigned int wbase = 0, total = 0;
+#pragma unroll
+        for (int w2 = 0; w2 < SGS_PREB_BLOCK / 32; ++w2) {
+            const unsigned int x = s_wsum[w2];
+            wbase += (w2 < wid) ? x : 0u;
+            total += x;
+        }
+        s_off[tid] = wbase + incl - cnt;  // exclusive
+        if (tid == 0) s_off[SGS_PREB_BLOCK] = total;
+        __syncthreads();
+        for (unsigned int e0 = tid; e0 < total; e0 += 2 * SGS_PREB_BLOCK) {
+            // two entries per trip so that both cursor atomics are in flight before either dependent store
+            uint32_t t[2];
+            unsigned long long key[2];
+            bool ok[2];
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                const unsigned int e = e0 + k * SGS_PREB_BLOCK;
+                ok[k] = e < total;
+                // owner = last thread whose exclusive offset is <= e (and whose count is non-zero by construction)
+                int lo = 0, hi = SGS_PREB_BLOCK;  // invariant: s_off[lo] <= e < s_off[hi]
+#pragma unroll
+                for (int it = 0; it < SGS_PREB_LOG2; ++it) {
+                    const int mid = (lo + hi) >> 1;
+                    if (s_off[mid] <= e) lo = mid; else hi = mid;
+                }
+                const unsigned int local = e - s_off[lo], w = s_w[lo];
+                t[k] = s_rect[lo] + (local / w) * (unsigned int)cam.tiles_x + (local % w);
+                key[k] = s_key[lo];
+            }
+            uint32_t pos[2] = {0u, 0u};
+#pragma unroll
+            for (int k = 0; k < 2; ++k)
+                if (ok[k]) pos[k] = atomicAdd(&cursor[t[k]], 1u);
+#pragma unroll
+            for (int k = 0; k < 2; ++k)
+                if (ok[k]) {
+                    if (pos[k] < tile_cap) bucket[(size_t)t[k] * tile_cap + pos[k]] = key[k];
+                    else atomicMax(&counters->max_tile, pos[k] + 1u);
+                }
+        }
+        __syncthreads();  // the round's shared arrays are free again
     }
 }
 
@@ -344,16 +427,21 @@ cudaError_t sgs_launch_preprocess(sgs_ctx* c, const sgs_surfels* sf, cudaStream_
 
 cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cudaStream_t s) {
     const int64_t n = sf->n;
-    const int blocks = (int)((n + SGS_PRE_BLOCK - 1) / SGS_PRE_BLOCK);
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
     cudaError_t e = cudaMemsetAsync(c->counters, 0, sizeof(SgsCounters), s);
     if (e != cudaSuccess) return e;
     e = cudaMemsetAsync(c->cursor, 0, sizeof(uint32_t) * (size_t)tiles, s);
-    if (e != cudaSuccess || blocks == 0) return e;
+    if (e != cudaSuccess || n == 0) return e;
     SgsStage st(c, SGS_STAGE_PREPROCESS, s);
-    c->launches += 1;
-    k_preprocess_bucket<<<blocks, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb,
-                                                         sf->active, c->camd, c->cfgd, c->pay, c->culled, c->counters,
-                                                         c->cursor, c->bucket, (uint32_t)c->tile_cap);
+    c->launches += 2;
+    const int blocks_a = (int)((n + SGS_PREA_SPAN - 1) / SGS_PREA_SPAN);
+    k_pre_select<<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, c->camd, c->cfgd, c->culled, c->counters,
+                                                    c->vis_to_surfel);
+    // K-pre-B walks the survivor list with a grid-stride loop: the count is only known on the device
+    int64_t blocks_b = (n + SGS_PREB_BLOCK - 1) / SGS_PREB_BLOCK;
+    if (blocks_b > 148 * 8) blocks_b = 148 * 8;
+    k_pre_project<<<(int)blocks_b, SGS_PREB_BLOCK, 0, s>>>(sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd, c->cfgd,
+                                                          c->pay, c->culled, c->counters, c->vis_to_surfel, c->cursor,
+                                                          c->bucket, (uint32_t)c->tile_cap);
     return cudaGetLastError();
 }

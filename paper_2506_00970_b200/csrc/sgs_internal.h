@@ -35,10 +35,14 @@ struct SgsCamDev {
     double t[3];
     float Rf[9];
     float tf[3];
+    // camera-only constants of the binary32 pre-cull (preprocess.cu precull_f32), filled on the host
+    float pc_n[4];   // |(fx, cx)|, |(fx, cx - W)|, |(fy, cy)|, |(fy, cy - H)|, each rounded up by 1.00001
+    float pc_cxr, pc_cyr, pc_tabs;  // cx - W, cy - H, |t|_1 + 1
 };
 
 struct SgsCfgDev {
     float cutoff2, alpha_min, alpha_max, t_min, z_near;
+    float cutoff;   // sqrt(cutoff2)
     double cutoff2_d, z_near_d;
 };
 
@@ -50,7 +54,7 @@ struct SgsCounters {
     unsigned int ticket_pre;        // dynamic block ids for the chained scan in K-pre
     unsigned int ticket_bwd;        // last-block-done ticket for the pose reduction
     unsigned int max_tile;          // bucket mode: largest per-tile entry count seen (> tile_cap => overflow)
-    unsigned int pad;
+    unsigned int n_surv;            // bucket mode: surfels that passed the cheap tests of K-pre-A (the list K-pre-B walks)
 };
 
 struct sgs_ctx {
