@@ -29,6 +29,9 @@ UNIT = "MP/s"
 # Algorithmic flops per (pixel, entry) pair, counted from the oracle's formulas with FMA = 2
 # (DESIGN.md §7): tested pair 26; composited pair +26 forward, +102 full backward, +94 pose-only backward.
 F_TEST, F_COMP_FWD, F_COMP_BWD_FULL, F_COMP_BWD_POSE = 26, 26, 102, 94
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
+# captures (profiles/r01_*.md; ncu flushes L2 before every replay, so these are cold-cache figures)
+NCU_TRAFFIC = {("C2", "track"): 20.9e6, ("C2", "backward"): 30.6e6, ("C2", "forward"): 14.0e6}
 
 
 def load_peaks():
@@ -378,7 +381,9 @@ def main():
                     sort=("hbm", E * 24 + E * 8),
                     forward=("alu", F_TEST * cnt["Q_t"] + F_COMP_FWD * cnt["Q_c"]),
                     loss=("hbm", px * (12 + 8) * 4),
-                    backward=("alu", F_TEST * cnt["Q_tb"] + fcb * cnt["Q_c"]))
+                    backward=("alu", F_TEST * cnt["Q_tb"] + fcb * cnt["Q_c"]),
+                    # sgs_track_iter's single kernel: forward + pose-only backward of the same view
+                    track=("alu", F_TEST * (cnt["Q_t"] + cnt["Q_tb"]) + (F_COMP_FWD + F_COMP_BWD_POSE) * cnt["Q_c"]))
         tot_ms = sum(v[0] for v in prof.values()) or 1.0
         for st, (ms_s, calls) in prof.items():
             if calls == 0:
@@ -393,7 +398,7 @@ def main():
                               share=ms_s / tot_ms, algorithmic_units=units)
         dom = max(stages, key=lambda k: stages[k]["share"])
         roof = dict(stages[dom])
-        roof.update(kernel=dom, traffic=None, peak_source=peaks["source"] + (" HBM copy" if roof["bound"] == "hbm" else
+        roof.update(kernel=dom, traffic=NCU_TRAFFIC.get((args.config, dom)), peak_source=peaks["source"] + (" HBM copy" if roof["bound"] == "hbm" else
                     "; alu peak = 148 SM x 128 lanes x 2 x max SM clock"), counters=dict(cnt, E=E))
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=ms_max / K,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",

@@ -128,7 +128,7 @@ typedef struct {
 
 /* Per-stage device timing (CUDA events recorded on the caller's stream around each stage). */
 enum { SGS_STAGE_PREPROCESS = 0, SGS_STAGE_SORT = 1, SGS_STAGE_FORWARD = 2, SGS_STAGE_LOSS = 3,
-       SGS_STAGE_BACKWARD = 4, SGS_STAGE_COUNT = 5 };
+       SGS_STAGE_BACKWARD = 4, SGS_STAGE_TRACK = 5 /* sgs_track_iter's fused kernel */, SGS_STAGE_COUNT = 6 };
 
 SGS_API int sgs_default_config(sgs_config* cfg);
 SGS_API int sgs_create(sgs_ctx** out, const sgs_config* cfg);

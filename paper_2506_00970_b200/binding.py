@@ -242,7 +242,7 @@ class Renderer:
         _check(self.lib.sgs_get_stats(self._ctx, C.byref(st)), "sgs_get_stats")
         return {k: int(getattr(st, k)) for k, _ in sgs_stats._fields_}
 
-    STAGES = ("preprocess", "sort", "forward", "loss", "backward")
+    STAGES = ("preprocess", "sort", "forward", "loss", "backward", "track")
 
     def set_profiling(self, enabled):
         _check(self.lib.sgs_set_profiling(self._ctx, C.c_int(int(enabled))), "sgs_set_profiling")

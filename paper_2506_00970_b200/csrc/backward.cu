@@ -248,7 +248,7 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
                   float* __restrict__ acc, const float* __restrict__ mean, const float* __restrict__ scale,
                   const float* __restrict__ quat, SgsCamDev cam, sgs_surfel_grads out,
                   float* __restrict__ pose_partial, SgsCounters* __restrict__ counters_rw,
-                  float* __restrict__ d_pose6) {
+                  float* __restrict__ d_pose6, int zero_rest) {
     __shared__ float s_red[8][6];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     // compacted mode: v < N_v, surfel = vis_to_surfel[v]; bucket mode (no compaction): v = surfel index
@@ -330,6 +330,15 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
             out.quat[4 * i + 3] = (dq[3] - qz * qd) * qi;
         }
     }
+    else if (zero_rest && v < n_all) {
+        // inactive / culled surfel: gradients are exactly zero (bucket mode: v IS the surfel index, so the
+        // caller's buffers are overwritten here instead of by five memsets)
+        if (out.mean) { out.mean[3 * v] = 0.f; out.mean[3 * v + 1] = 0.f; out.mean[3 * v + 2] = 0.f; }
+        if (out.scale) { out.scale[2 * v] = 0.f; out.scale[2 * v + 1] = 0.f; }
+        if (out.quat) reinterpret_cast<float4*>(out.quat)[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (out.opacity) out.opacity[v] = 0.f;
+        if (out.rgb) { out.rgb[3 * v] = 0.f; out.rgb[3 * v + 1] = 0.f; out.rgb[3 * v + 2] = 0.f; }
+    }
     if (d_pose6 == nullptr) return;
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
@@ -365,11 +374,16 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     }
     const int64_t n = c->last_surfels.n;
     cudaError_t e = cudaSuccess;
-    if (dg->mean && e == cudaSuccess) e = cudaMemsetAsync(dg->mean, 0, sizeof(float) * 3 * (size_t)n, s);
-    if (dg->scale && e == cudaSuccess) e = cudaMemsetAsync(dg->scale, 0, sizeof(float) * 2 * (size_t)n, s);
-    if (dg->quat && e == cudaSuccess) e = cudaMemsetAsync(dg->quat, 0, sizeof(float) * 4 * (size_t)n, s);
-    if (dg->opacity && e == cudaSuccess) e = cudaMemsetAsync(dg->opacity, 0, sizeof(float) * (size_t)n, s);
-    if (dg->rgb && e == cudaSuccess) e = cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * (size_t)n, s);
+    // bucket mode: k_surfel_backward visits every surfel and writes the zeros itself; the quat store is a float4
+    const bool bucket_mode = c->list_stride == 2;
+    const bool kernel_zeroes = bucket_mode && ((reinterpret_cast<uintptr_t>(dg->quat) & 15u) == 0);
+    if (!kernel_zeroes) {
+        if (dg->mean && e == cudaSuccess) e = cudaMemsetAsync(dg->mean, 0, sizeof(float) * 3 * (size_t)n, s);
+        if (dg->scale && e == cudaSuccess) e = cudaMemsetAsync(dg->scale, 0, sizeof(float) * 2 * (size_t)n, s);
+        if (dg->quat && e == cudaSuccess) e = cudaMemsetAsync(dg->quat, 0, sizeof(float) * 4 * (size_t)n, s);
+        if (dg->opacity && e == cudaSuccess) e = cudaMemsetAsync(dg->opacity, 0, sizeof(float) * (size_t)n, s);
+        if (dg->rgb && e == cudaSuccess) e = cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * (size_t)n, s);
+    }
     if (e != cudaSuccess) return e;
     c->launches += 1;
     k_backward<false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
@@ -381,7 +395,7 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
         c->launches += 1, k_surfel_backward<<<blocks, 256, 0, s>>>(c->counters, c->list_stride == 2 ? nullptr : c->vis_to_surfel, c->culled,
                                                  (unsigned int)n, c->acc, c->last_surfels.mean,
                                                  c->last_surfels.scale, c->last_surfels.quat, cam, *dg, c->pose_partial,
-                                                 c->counters, d_pose6);
+                                                 c->counters, d_pose6, kernel_zeroes ? 1 : 0);
     return cudaGetLastError();
 }
 

@@ -19,7 +19,6 @@ namespace {
 struct TrackPlanes { float* p[8]; };
 
 constexpr uint32_t TRK_PL = SGS_BLOCK * 16;  // bytes per staged plane
-constexpr int TRK_MAX_SORT = 2048;           // largest bucket ordered inside the kernel (= fused-sort tile_cap bound)
 
 // One thread stages entry `v` of the tile: forward record (s0..s4) plus the backward's a_u, a_v, m = a_u x a_v.
 __device__ __forceinline__ unsigned stage_track(const SgsPayload& pay, uint32_t v, double px0, double py0, float tx0,
@@ -107,7 +106,7 @@ k_track(uint32_t* __restrict__ ranges, const uint32_t* __restrict__ cursor, unsi
         float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
         float* __restrict__ loss_out) {
     __shared__ float4 sh[8][SGS_BLOCK];
-    __shared__ uint32_t s_idx[TRK_MAX_SORT];
+    __shared__ unsigned long long s_keys[SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
     __shared__ float s_red[8][7];
     __shared__ uint32_t s_wmax[8];
@@ -127,65 +126,13 @@ k_track(uint32_t* __restrict__ ranges, const uint32_t* __restrict__ cursor, unsi
     float tr = 0.f, tg = 0.f, tb = 0.f, td = 0.f;
     if (inside) { tr = __ldg(trgb + pix); tg = __ldg(trgb + HW + pix); tb = __ldg(trgb + 2 * HW + pix); td = __ldg(tdepth + pix); }
 
-    // ---- tile list: order the bucket by (depth bits, index) (tilesort.cu's contract) ----
-    const uint32_t raw = cursor[tile];
-    const uint32_t n = raw < tile_cap ? raw : tile_cap;
-    const uint32_t start = tile * tile_cap;
-    unsigned long long* g = bucket + (size_t)start;
-    if (tid == 0) { ranges[2 * tile] = start; ranges[2 * tile + 1] = start + n; }
-    const bool in_smem = !presorted && n <= TRK_MAX_SORT;  // sorted indices live in s_idx
-    if (!presorted) {
-        unsigned long long* sk = reinterpret_cast<unsigned long long*>(&sh[0][0]);
-        if (n == 1) {
-            if (tid == 0) s_idx[0] = (uint32_t)g[0];
-        } else if (n <= SGS_BLOCK) {
-            // rank by counting (keys are unique); only warps that own keys walk the list
-            const bool mine = (uint32_t)tid < n;
-            const unsigned long long key = mine ? g[tid] : ~0ull;
-            if (mine) sk[tid] = key;
-            __syncthreads();
-            if ((uint32_t)(wid * 32) < n) {
-                uint32_t rank = 0;
-                for (uint32_t k = 0; k < n; ++k) rank += sk[k] < key ? 1u : 0u;
-                if (mine) { g[rank] = key; s_idx[rank] = (uint32_t)key; }
-            }
-        } else {
-            uint32_t npad = 512;
-            while (npad < n) npad <<= 1;
-            for (uint32_t i = tid; i < npad; i += SGS_BLOCK) sk[i] = i < n ? g[i] : ~0ull;
-            __syncthreads();
-            for (uint32_t k = 2; k <= npad; k <<= 1)
-                for (uint32_t j = k >> 1; j > 0; j >>= 1) {
-                    for (uint32_t t = tid; t < (npad >> 1); t += SGS_BLOCK) {
-                        const uint32_t i = ((t & ~(j - 1)) << 1) | (t & (j - 1)), p = i | j;
-                        const unsigned long long a = sk[i], b = sk[p];
-                        if ((a > b) == ((i & k) == 0)) { sk[i] = b; sk[p] = a; }
-                    }
-                    __syncthreads();
-                }
-            for (uint32_t i = tid; i < n; i += SGS_BLOCK) { const unsigned long long k2 = sk[i]; g[i] = k2; s_idx[i] = (uint32_t)k2; }
-        }
-        __syncthreads();  // s_idx complete; staging memory free
-    }
-
-    // ---- forward compositing (Eq. 8), as k_forward ----
+    // ---- forward walk over the staged batch [boff, boff + nb) (Eq. 8, as k_forward) ----
     float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dp = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f, O = 0.f;
     uint32_t last = 0;
     bool done = !inside;
-    int staged_b = -1;  // batch currently held in shared memory
-    for (uint32_t boff = 0; boff < n; boff += SGS_BLOCK) {
-        if (__syncthreads_and(done)) break;
-        const uint32_t nb = min((uint32_t)SGS_BLOCK, n - boff);
-        unsigned mask = 0;
-        if ((uint32_t)tid < nb) {
-            const uint32_t v = in_smem ? s_idx[boff + tid] : (uint32_t)g[boff + tid];
-            mask = stage_track(pay, v, px0, py0, tx0, ty0, sh, tid);
-        }
-        sh_mask[tid] = (unsigned char)mask;
-        staged_b = (int)(boff / SGS_BLOCK);
-        __syncthreads();
+    auto forward_walk = [&](const uint32_t boff, const uint32_t nb) {
         for (uint32_t c0 = 0; c0 < nb; c0 += 32) {
-            if (__all_sync(0xffffffffu, done)) break;
+            if (__all_sync(0xffffffffu, done)) break;  // per-warp early stop on saturation
             unsigned m = __ballot_sync(0xffffffffu, (lds_u8(sm_a + c0 + lane) >> wid) & 1u);
             while (m) {
                 // two entries per trip: their LDS -> FMA -> RCP chains are independent and overlap; only the
@@ -208,63 +155,41 @@ k_track(uint32_t* __restrict__ ranges, const uint32_t* __restrict__ cursor, unsi
                 if (anyb) fwd_composite(eb, b2, ub, vb, rho2b, pb && !done, boff + jb + 1, cfg, T, done, last, C0, C1, C2, Dp, N0, N1, N2, O);
             }
         }
-    }
-    if (WRITE_IMAGES && inside) {
-        if (out.p[0]) out.p[0][pix] = C0;
-        if (out.p[1]) out.p[1][pix] = C1;
-        if (out.p[2]) out.p[2][pix] = C2;
-        if (out.p[3]) out.p[3][pix] = Dp;
-        if (out.p[4]) out.p[4][pix] = N0;
-        if (out.p[5]) out.p[5][pix] = N1;
-        if (out.p[6]) out.p[6][pix] = N2;
-        if (out.p[7]) out.p[7][pix] = O;
-    }
+    };
 
     // ---- Eq. 15-19 in registers (same arithmetic as loss.cu): loss term and upstream gradients of rgb, depth ----
     const float rx = ((float)px + 0.5f - cx) / fx, ry = ((float)py + 0.5f - cy) / fy;  // pixel ray (rx, ry, 1)
     float g0 = 0.f, g1 = 0.f, g2 = 0.f, g3 = 0.f, my_loss = 0.f;
-    if (inside) {
-        const float inv = 1.f / (float)HW;
-        const float nr = N0 * rx + N1 * ry + N2;
-        if ((nsign * nr > 0.f) && (O > 0.95f)) {  // M_n M_o (Eq. 17-18)
-            float d = C0 - tr; my_loss += fabsf(d); g0 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
-            d = C1 - tg; my_loss += fabsf(d); g1 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
-            d = C2 - tb; my_loss += fabsf(d); g2 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
-            d = Dp - td; my_loss += lambda_d * fabsf(d);
-            g3 = d > 0.f ? lambda_d * inv : (d < 0.f ? -lambda_d * inv : 0.f);
+    auto finish_forward = [&]() {
+        if (WRITE_IMAGES && inside) {
+            if (out.p[0]) out.p[0][pix] = C0;
+            if (out.p[1]) out.p[1][pix] = C1;
+            if (out.p[2]) out.p[2][pix] = C2;
+            if (out.p[3]) out.p[3][pix] = Dp;
+            if (out.p[4]) out.p[4][pix] = N0;
+            if (out.p[5]) out.p[5][pix] = N1;
+            if (out.p[6]) out.p[6][pix] = N2;
+            if (out.p[7]) out.p[7][pix] = O;
         }
-        my_loss *= inv;
-    }
-    if (!(g0 != 0.f || g1 != 0.f || g2 != 0.f || g3 != 0.f)) last = 0;  // every backward term carries a factor g
-
-    // ---- reverse traversal (as k_backward<POSE_ONLY>, g_normal = g_alpha = 0) ----
-    uint32_t wmax = last;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
-    if (lane == 0) s_wmax[wid] = wmax;
-    __syncthreads();  // also: every warp has left the forward walk
-    uint32_t bmax = 0;
-#pragma unroll
-    for (int w2 = 0; w2 < 8; ++w2) bmax = max(bmax, s_wmax[w2]);
-
-    float T_after = T, suffix = 0.f;
-    float F0 = 0.f, F1 = 0.f, F2 = 0.f, Z0 = 0.f, Z1 = 0.f, Z2 = 0.f;
-    const int n_batches = (int)((bmax + SGS_BLOCK - 1) / SGS_BLOCK);
-    for (int b = n_batches - 1; b >= 0; --b) {
-        const uint32_t boff = (uint32_t)b * SGS_BLOCK;
-        const uint32_t nb = min((uint32_t)SGS_BLOCK, bmax - boff);
-        if (b != staged_b) {  // block-uniform
-            __syncthreads();  // previous batch fully consumed
-            unsigned mask = 0;
-            if ((uint32_t)tid < nb) {
-                const uint32_t v = in_smem ? s_idx[boff + tid] : (uint32_t)g[boff + tid];
-                mask = stage_track(pay, v, px0, py0, tx0, ty0, sh, tid);
+        if (inside) {
+            const float inv = 1.f / (float)HW;
+            const float nr = N0 * rx + N1 * ry + N2;
+            if ((nsign * nr > 0.f) && (O > 0.95f)) {  // M_n M_o (Eq. 17-18)
+                float d = C0 - tr; my_loss += fabsf(d); g0 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
+                d = C1 - tg; my_loss += fabsf(d); g1 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
+                d = C2 - tb; my_loss += fabsf(d); g2 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
+                d = Dp - td; my_loss += lambda_d * fabsf(d);
+                g3 = d > 0.f ? lambda_d * inv : (d < 0.f ? -lambda_d * inv : 0.f);
             }
-            sh_mask[tid] = (unsigned char)mask;
-            staged_b = b;
-            __syncthreads();
+            my_loss *= inv;
         }
-        const int jend = (int)min(nb, wmax > boff ? wmax - boff : 0u);  // exclusive
+        if (!(g0 != 0.f || g1 != 0.f || g2 != 0.f || g3 != 0.f)) last = 0;  // every backward term carries a factor g
+    };
+
+    // ---- reverse walk over the staged batch (as k_backward<POSE_ONLY>, g_normal = g_alpha = 0) ----
+    float T_after = 1.f, suffix = 0.f;
+    float F0 = 0.f, F1 = 0.f, F2 = 0.f, Z0 = 0.f, Z1 = 0.f, Z2 = 0.f;
+    auto backward_walk = [&](const uint32_t boff, const int jend) {  // entries [0, jend) of the staged batch, back to front
         for (int c0 = ((jend - 1) >> 5) << 5; c0 >= 0 && jend > 0; c0 -= 32) {
             unsigned m = __ballot_sync(0xffffffffu, (c0 + lane < jend) && ((lds_u8(sm_a + c0 + lane) >> wid) & 1u));
             while (m) {
@@ -288,6 +213,97 @@ k_track(uint32_t* __restrict__ ranges, const uint32_t* __restrict__ cursor, unsi
                 if (__any_sync(0xffffffffu, hitb) && hitb)
                     bwd_pair(eb, b3, rb, g0, g1, g2, g3, rx, ry, cfg.alpha_max, T_after, suffix, F0, F1, F2, Z0, Z1, Z2);
             }
+        }
+    };
+    auto warp_max_last = [&]() {
+        uint32_t wmax = last;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
+        return wmax;
+    };
+
+    // ---- tile list: order the bucket by (depth bits, index) (tilesort.cu's contract) ----
+    const uint32_t raw = cursor[tile];
+    const uint32_t n = raw < tile_cap ? raw : tile_cap;
+    const uint32_t start = tile * tile_cap;
+    unsigned long long* g = bucket + (size_t)start;
+    if (tid == 0) { ranges[2 * tile] = start; ranges[2 * tile + 1] = start + n; }
+
+    if (!presorted && n <= SGS_BLOCK) {
+        // ===== one batch (the common case in tracking): rank the keys by counting (they are unique), stage each
+        // entry straight into the slot of its rank, walk forward, then walk the SAME staged records back.
+        // No barrier between the two walks: a warp needs only its own pixels' state. =====
+        const bool mine = (uint32_t)tid < n;
+        const unsigned long long key = mine ? g[tid] : ~0ull;
+        s_keys[tid] = key;
+        sh_mask[tid] = 0;
+        __syncthreads();
+        if ((uint32_t)(wid * 32) < n) {  // only warps that own keys walk the list
+            uint32_t rank = 0;
+            for (uint32_t k = 0; k < n; ++k) rank += s_keys[k] < key ? 1u : 0u;
+            if (mine) {
+                g[rank] = key;  // sorted list for sgs_get_binning
+                sh_mask[rank] = (unsigned char)stage_track(pay, (uint32_t)key, px0, py0, tx0, ty0, sh, (int)rank);
+            }
+        }
+        __syncthreads();
+        forward_walk(0u, n);
+        finish_forward();
+        T_after = T;
+        backward_walk(0u, (int)min(n, warp_max_last()));
+    } else {
+        // ===== general path: 256-entry batches front to back, then back to front (restaging what was evicted) =====
+        if (!presorted) {  // n > 256: bitonic network in the staging memory, sorted keys back to the bucket
+            unsigned long long* sk = reinterpret_cast<unsigned long long*>(&sh[0][0]);
+            uint32_t npad = 512;
+            while (npad < n) npad <<= 1;
+            for (uint32_t i = tid; i < npad; i += SGS_BLOCK) sk[i] = i < n ? g[i] : ~0ull;
+            __syncthreads();
+            for (uint32_t k = 2; k <= npad; k <<= 1)
+                for (uint32_t j = k >> 1; j > 0; j >>= 1) {
+                    for (uint32_t t = tid; t < (npad >> 1); t += SGS_BLOCK) {
+                        const uint32_t i = ((t & ~(j - 1)) << 1) | (t & (j - 1)), p = i | j;
+                        const unsigned long long a = sk[i], b = sk[p];
+                        if ((a > b) == ((i & k) == 0)) { sk[i] = b; sk[p] = a; }
+                    }
+                    __syncthreads();
+                }
+            for (uint32_t i = tid; i < n; i += SGS_BLOCK) g[i] = sk[i];
+            __syncthreads();  // sorted bucket visible to the block; staging memory free
+        }
+        int staged_b = -1;  // batch currently held in shared memory
+        for (uint32_t boff = 0; boff < n; boff += SGS_BLOCK) {
+            if (__syncthreads_and(done)) break;
+            const uint32_t nb = min((uint32_t)SGS_BLOCK, n - boff);
+            unsigned mask = 0;
+            // plain loads: the bucket may just have been rewritten by this block
+            if ((uint32_t)tid < nb) mask = stage_track(pay, (uint32_t)g[boff + tid], px0, py0, tx0, ty0, sh, tid);
+            sh_mask[tid] = (unsigned char)mask;
+            staged_b = (int)(boff / SGS_BLOCK);
+            __syncthreads();
+            forward_walk(boff, nb);
+        }
+        finish_forward();
+        T_after = T;
+        const uint32_t wmax = warp_max_last();
+        if (lane == 0) s_wmax[wid] = wmax;
+        __syncthreads();  // also: every warp has left the forward walk
+        uint32_t bmax = 0;
+#pragma unroll
+        for (int w2 = 0; w2 < 8; ++w2) bmax = max(bmax, s_wmax[w2]);
+        const int n_batches = (int)((bmax + SGS_BLOCK - 1) / SGS_BLOCK);
+        for (int b = n_batches - 1; b >= 0; --b) {
+            const uint32_t boff = (uint32_t)b * SGS_BLOCK;
+            const uint32_t nb = min((uint32_t)SGS_BLOCK, bmax - boff);
+            if (b != staged_b) {  // block-uniform
+                __syncthreads();  // previous batch fully consumed
+                unsigned mask = 0;
+                if ((uint32_t)tid < nb) mask = stage_track(pay, (uint32_t)g[boff + tid], px0, py0, tx0, ty0, sh, tid);
+                sh_mask[tid] = (unsigned char)mask;
+                staged_b = b;
+                __syncthreads();
+            }
+            backward_walk(boff, (int)min(nb, wmax > boff ? wmax - boff : 0u));
         }
     }
     // Eq. 11-13 per pixel: rho += sum f; theta += r x sum(z f)   (g_N = 0 in tracking)
@@ -319,7 +335,7 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
     TrackPlanes out;
     bool any = false;
     for (int i = 0; i < 8; ++i) { out.p[i] = planes ? planes[i] : nullptr; any = any || out.p[i] != nullptr; }
-    SgsStage st(c, SGS_STAGE_FORWARD, s);
+    SgsStage st(c, SGS_STAGE_TRACK, s);
     c->launches += 1;
     unsigned long long* bucket = reinterpret_cast<unsigned long long*>(c->bucket);
     const int presorted = c->fused_sort ? 0 : 1;
