@@ -103,6 +103,18 @@ def oracle_counters(sc, cams, info):
     return out
 
 
+def aggregate_replicas(ms_local, pixels, renders_per_rank, world, dist=None, device="cpu"):
+    """Weak scaling over independent replicas ("replicas only", no data-path collective): every rank
+    times the same K steps on the device; the job's time is the MAX over ranks and its throughput the work of
+    ALL ranks divided by that time.  Returns (ms_max, megapixels_per_second)."""
+    import torch
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    return ms_max, pixels * renders_per_rank * world / (ms_max * 1e-3) / 1e6
+
+
 # --------------------------------------------------------------------------------------- our arm
 class Workload:
     """Device-resident inputs + the step function for one config."""
@@ -329,13 +341,9 @@ def main():
     ms = timed_pass()
     clocks = sampler.stop()
     launches = wl.ren.stats()["kernel_launches"] - launches0
-    t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
     px = wl.H * wl.W
+    ms_max, value = aggregate_replicas(ms, px, wl.renders_per_step * K, world, dist, "cuda")
     renders = wl.renders_per_step * K * world
-    value = px * renders / (ms_max * 1e-3) / 1e6
 
     # second pass with per-stage CUDA events (roofline), not part of `value`
     wl.ren.set_profiling(True)
