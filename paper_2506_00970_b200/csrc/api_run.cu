@@ -13,6 +13,7 @@ static int check_pending(sgs_ctx* c, cudaStream_t s) {
     c->pending_check = false;
     const int64_t E = (int64_t)c->counters_host->n_entries;
     c->last_entries = E;
+    c->last_surv = (int64_t)c->counters_host->n_surv;
     if (radix_mode(c)) {
         if (c->counters_host->overflow) {
             c->have_forward = c->have_binning = false;
@@ -48,6 +49,7 @@ static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, cudaStream
             if (cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
         }
         c->last_entries = (int64_t)c->counters_host->n_entries;
+        c->last_surv = (int64_t)c->counters_host->n_surv;
     } else {
         cudaEventRecord(c->counters_ready, s);
         c->pending_check = true;

@@ -431,15 +431,22 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     cudaError_t e = cudaMemsetAsync(c->counters, 0, sizeof(SgsCounters), s);
     if (e != cudaSuccess) return e;
     e = cudaMemsetAsync(c->cursor, 0, sizeof(uint32_t) * (size_t)tiles, s);
-    if (e != cudaSuccess || n == 0) return e;
+    if (e != cudaSuccess) return e;
     SgsStage st(c, SGS_STAGE_PREPROCESS, s);
-    c->launches += 2;
     const int blocks_a = (int)((n + SGS_PREA_SPAN - 1) / SGS_PREA_SPAN);
-    k_pre_select<<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, c->camd, c->cfgd, c->culled, c->counters,
-                                                    c->vis_to_surfel);
+    c->launches += blocks_a > 0 ? 2 : 1;
+    if (blocks_a > 0)
+        k_pre_select<<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, c->camd, c->cfgd, c->culled,
+                                                        c->counters, c->vis_to_surfel);
     // K-pre-B walks the survivor list with a grid-stride loop: the count is only known on the device
+    // (the grid follows the last known survivor count)
     int64_t blocks_b = (n + SGS_PREB_BLOCK - 1) / SGS_PREB_BLOCK;
+    if (c->last_surv > 0) {
+        const int64_t hint = (c->last_surv + c->last_surv / 4 + SGS_PREB_BLOCK - 1) / SGS_PREB_BLOCK;
+        if (hint < blocks_b) blocks_b = hint;
+    }
     if (blocks_b > 148 * 8) blocks_b = 148 * 8;
+    if (blocks_b < 1) blocks_b = 1;
     k_pre_project<<<(int)blocks_b, SGS_PREB_BLOCK, 0, s>>>(sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd, c->cfgd,
                                                           c->pay, c->culled, c->counters, c->vis_to_surfel, c->cursor,
                                                           c->bucket, (uint32_t)c->tile_cap);

@@ -12,7 +12,8 @@ __device__ __forceinline__ float warp_sum(float v) {
 
 // Grid reduction: every block has written 6 partial sums at partial[block*8 ..]; the block that
 // draws the last ticket adds them all in fp64 and writes the pose gradient (block-then-grid).
-__device__ __forceinline__ void finish_pose(const float* __restrict__ partial, unsigned int n_blocks,
+// Returns (to every thread of the block) whether this block was the last one.
+__device__ __forceinline__ bool finish_pose(const float* __restrict__ partial, unsigned int n_blocks,
                                             SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
                                             float* __restrict__ loss_out = nullptr) {
     __shared__ bool s_is_last;
@@ -25,7 +26,7 @@ __device__ __forceinline__ void finish_pose(const float* __restrict__ partial, u
         s_is_last = (t == n_blocks - 1);
     }
     __syncthreads();
-    if (!s_is_last) return;
+    if (!s_is_last) return false;
     __threadfence();
     double a[7] = {0, 0, 0, 0, 0, 0, 0};
     for (unsigned int b = tid; b < n_blocks; b += blockDim.x) {
@@ -48,5 +49,6 @@ __device__ __forceinline__ void finish_pose(const float* __restrict__ partial, u
         else if (loss_out) *loss_out = (float)v;
     }
     if (tid == 0) counters->ticket_bwd = 0;  // self-cleaning: backward may run again on the same render
+    return true;
 }
 

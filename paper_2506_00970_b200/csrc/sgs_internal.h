@@ -83,6 +83,8 @@ struct sgs_ctx {
     // bucket binning (default): tile t owns bucket[t * tile_cap .. ), filled through cursor[t]
     uint64_t* bucket;                // tiles x tile_cap keys: depth bits << 32 | surfel index
     uint32_t* cursor;                // tiles
+    uint32_t* tile_order;            // tiles: tile ids by descending entry count (longest first), written by K-pre-B
+    int64_t cursor_cap;              // tiles the cursor / tile_order arrays hold
     int64_t tile_cap, bucket_cap;    // entries per tile; allocated keys
     uint64_t* export_keys;           // contiguous (tile << 32 | depth) list for sgs_get_binning
     uint32_t* export_ranges;
@@ -125,6 +127,9 @@ struct sgs_ctx {
     int64_t launches;                // kernels launched by this ctx
     int prof_on; int prof_n, prof_cap; cudaEvent_t* prof_ev; int* prof_stage;  // event pairs: ev[2i], ev[2i+1]
     int64_t last_entries;            // E of the last checked render (async launch bound hint), 0 = unknown
+    int64_t last_surv;               // K-pre-A survivors of the last checked render (K-pre-B grid hint), 0 = unknown
+    uint32_t* tile_cost;             // tiles: cycles >> 8 each tile's k_track block took last time (scheduling feedback)
+    int cost_tiles, cost_W, cost_H;  // camera the costs were measured for (0 = none)
 };
 
 // ---- launchers (each enqueues on `s`, returns the last CUDA error) ----

@@ -19,6 +19,8 @@ namespace {
 struct TrackPlanes { float* p[8]; };
 
 constexpr uint32_t TRK_PL = SGS_BLOCK * 16;  // bytes per staged plane
+constexpr int TRK_ORDER_BINS = 2048;         // tile costs (cycles >> 8) are binned 0..2047
+constexpr int TRK_K = 2;                     // entries per trip of the walks
 
 // One thread stages entry `v` of the tile: forward record (s0..s4) plus the backward's a_u, a_v, m = a_u x a_v.
 __device__ __forceinline__ unsigned stage_track(const SgsPayload& pay, uint32_t v, double px0, double py0, float tx0,
@@ -100,18 +102,19 @@ __device__ __forceinline__ void bwd_pair(uint32_t ea, const float4 s3, const Pai
 
 template <bool WRITE_IMAGES>
 __global__ void __launch_bounds__(SGS_BLOCK, 3)
-k_track(uint32_t* __restrict__ ranges, const uint32_t* __restrict__ cursor, unsigned long long* bucket, uint32_t tile_cap,
+k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* __restrict__ cursor, unsigned long long* bucket, uint32_t tile_cap,
         int presorted, SgsPayload pay, int W, int H, int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg,
         TrackPlanes out, const float* __restrict__ trgb, const float* __restrict__ tdepth, float lambda_d, float nsign,
         float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
-        float* __restrict__ loss_out) {
+        float* __restrict__ loss_out, uint32_t* __restrict__ tile_cost) {
+    const long long t_start = clock64();
     __shared__ float4 sh[8][SGS_BLOCK];
     __shared__ unsigned long long s_keys[SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
     __shared__ float s_red[8][7];
     __shared__ uint32_t s_wmax[8];
     const uint32_t sa = smem_addr(&sh[0][0]), sm_a = smem_addr(sh_mask);
-    const int tile = blockIdx.x;
+    const int tile = (int)tile_order[blockIdx.x];  // longest tiles first (order written by the previous launch)
     const int tx = tile % tiles_x, ty = tile / tiles_x;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int lxi = (wid & 1) * 8 + (lane & 7), lyi = (wid >> 1) * 4 + (lane >> 3);
@@ -135,24 +138,52 @@ k_track(uint32_t* __restrict__ ranges, const uint32_t* __restrict__ cursor, unsi
             if (__all_sync(0xffffffffu, done)) break;  // per-warp early stop on saturation
             unsigned m = __ballot_sync(0xffffffffu, (lds_u8(sm_a + c0 + lane) >> wid) & 1u);
             while (m) {
-                // two entries per trip: their LDS -> FMA -> RCP chains are independent and overlap; only the
-                // T / done recurrence is sequential (first A, then B)
-                const uint32_t ja = c0 + (uint32_t)__ffs(m) - 1u;
-                m &= m - 1u;
-                const bool two = m != 0u;
-                const uint32_t jb = two ? c0 + (uint32_t)__ffs(m) - 1u : ja;
-                m &= m - 1u;
-                const uint32_t ea = sa + ja * 16u, eb = sa + jb * 16u;
-                const float4 a0 = lds128(ea), a1 = lds128(ea + TRK_PL), a2 = lds128(ea + 2 * TRK_PL);
-                const float4 b0 = lds128(eb), b1 = lds128(eb + TRK_PL), b2 = lds128(eb + 2 * TRK_PL);
-                float ua, va, ub, vb;
-                const float rho2a = pair_rho2(a0, a1, a2, lx, ly, ua, va);
-                const float rho2b = pair_rho2(b0, b1, b2, lx, ly, ub, vb);
-                const bool pa = !done && (rho2a <= cfg.cutoff2);
-                const bool pb = two && (rho2b <= cfg.cutoff2);
-                const bool anya = __any_sync(0xffffffffu, pa), anyb = __any_sync(0xffffffffu, pb);
-                if (anya) fwd_composite(ea, a2, ua, va, rho2a, pa, boff + ja + 1, cfg, T, done, last, C0, C1, C2, Dp, N0, N1, N2, O);
-                if (anyb) fwd_composite(eb, b2, ub, vb, rho2b, pb && !done, boff + jb + 1, cfg, T, done, last, C0, C1, C2, Dp, N0, N1, N2, O);
+                // TRK_K entries per trip, in three phases.  The time of a tile is the serial walk of its slowest
+                // warp (profiles/r01_c2_track.md: a handful of 230-entry tiles set the whole kernel's duration at
+                // ~180 cycles per entry), so everything that does not depend on the running transmittance --
+                // loads, intersection, rho^2, z, G, alpha -- is evaluated for all TRK_K entries side by side
+                // (phase 1), the T / stop recurrence is a few dependent instructions per entry (phase 2), and
+                // the eight accumulations follow (phase 3).  Operations and their order per pixel are k_forward's.
+                uint32_t ea[TRK_K], jl[TRK_K];
+                float al[TRK_K], zz[TRK_K];
+                bool anyv = false;
+#pragma unroll
+                for (int k = 0; k < TRK_K; ++k) {
+                    const bool has = m != 0u;
+                    const uint32_t j = has ? c0 + (uint32_t)__ffs(m) - 1u : c0;
+                    m &= m - 1u;
+                    jl[k] = boff + j + 1u;
+                    ea[k] = sa + j * 16u;
+                    const float4 s0 = lds128(ea[k]), s1 = lds128(ea[k] + TRK_PL), s2 = lds128(ea[k] + 2 * TRK_PL);
+                    const float opac = lds32(ea[k] + 3 * TRK_PL);
+                    float u, v;
+                    const float rho2 = pair_rho2(s0, s1, s2, lx, ly, u, v);
+                    const float z = __fmaf_rn(s2.z, v, __fmaf_rn(s2.y, u, s2.w));
+                    const float G = fast_ex2(__fmul_rn(rho2, -0.72134752044448170368f));
+                    const float a = fminf(cfg.alpha_max, __fmul_rn(opac, G));
+                    const bool valid = has && (rho2 <= cfg.cutoff2) && (z > cfg.z_near) && (a >= cfg.alpha_min);
+                    al[k] = valid ? a : 0.f;  // alpha_min > 0 or not, a valid pair has a > 0 or contributes nothing
+                    zz[k] = z;
+                    anyv = anyv || valid;
+                }
+                if (!__any_sync(0xffffffffu, anyv && !done)) continue;
+#pragma unroll
+                for (int k = 0; k < TRK_K; ++k) {
+                    const float a = al[k];
+                    bool pass = !done && (a > 0.f);
+                    const float Tn = __fmul_rn(T, 1.f - a);
+                    const bool stop = pass && (Tn < cfg.t_min);  // R6: stop, this splat is not composited
+                    done = done || stop;
+                    pass = pass && !stop;
+                    const float w = pass ? __fmul_rn(a, T) : 0.f;
+                    T = pass ? Tn : T;
+                    last = pass ? jl[k] : last;
+                    const float4 s3 = lds128(ea[k] + 3 * TRK_PL), s4 = lds128(ea[k] + 4 * TRK_PL);
+                    C0 = __fmaf_rn(w, s3.y, C0); C1 = __fmaf_rn(w, s3.z, C1); C2 = __fmaf_rn(w, s3.w, C2);
+                    Dp = __fmaf_rn(w, zz[k], Dp);
+                    N0 = __fmaf_rn(w, s4.x, N0); N1 = __fmaf_rn(w, s4.y, N1); N2 = __fmaf_rn(w, s4.z, N2);
+                    O += w;
+                }
             }
         }
     };
@@ -193,25 +224,64 @@ k_track(uint32_t* __restrict__ ranges, const uint32_t* __restrict__ cursor, unsi
         for (int c0 = ((jend - 1) >> 5) << 5; c0 >= 0 && jend > 0; c0 -= 32) {
             unsigned m = __ballot_sync(0xffffffffu, (c0 + lane < jend) && ((lds_u8(sm_a + c0 + lane) >> wid) & 1u));
             while (m) {
-                // two entries per trip (back to front: A then B); the pair tests overlap, the T / suffix
-                // recurrence runs A first, then B
-                const int ha = 31 - __clz(m);
-                m &= ~(1u << ha);
-                const bool two = m != 0u;
-                const int hb = two ? 31 - __clz(m) : ha;
-                m &= ~(1u << hb);
-                const uint32_t ja = (uint32_t)(c0 + ha), jb = (uint32_t)(c0 + hb);
-                const uint32_t ea = sa + ja * 16u, eb = sa + jb * 16u;
-                const float4 a0 = lds128(ea), a1 = lds128(ea + TRK_PL), a2 = lds128(ea + 2 * TRK_PL), a3 = lds128(ea + 3 * TRK_PL);
-                const float4 b0 = lds128(eb), b1 = lds128(eb + TRK_PL), b2 = lds128(eb + 2 * TRK_PL), b3 = lds128(eb + 3 * TRK_PL);
-                PairResult ra, rb;
-                bool hita = (boff + ja) < last, hitb = two && (boff + jb) < last;
-                if (hita) hita = eval_pair(a0, a1, a2, a3.x, lx, ly, cfg.cutoff2, cfg.alpha_min, cfg.alpha_max, cfg.z_near, ra);
-                if (hitb) hitb = eval_pair(b0, b1, b2, b3.x, lx, ly, cfg.cutoff2, cfg.alpha_min, cfg.alpha_max, cfg.z_near, rb);
-                if (__any_sync(0xffffffffu, hita) && hita)
-                    bwd_pair(ea, a3, ra, g0, g1, g2, g3, rx, ry, cfg.alpha_max, T_after, suffix, F0, F1, F2, Z0, Z1, Z2);
-                if (__any_sync(0xffffffffu, hitb) && hitb)
-                    bwd_pair(eb, b3, rb, g0, g1, g2, g3, rx, ry, cfg.alpha_max, T_after, suffix, F0, F1, F2, Z0, Z1, Z2);
+                // TRK_K entries per trip, back to front, phases as in the forward walk: pair evaluation, 1/(1-a)
+                // and g.v side by side; then the T_i / suffix recurrence (4 dependent instructions per entry);
+                // then the geometric chain of each hit.
+                uint32_t ea[TRK_K];
+                PairResult r[TRK_K];
+                float inv1ma[TRK_K], gv[TRK_K], opac[TRK_K], da[TRK_K], w[TRK_K];
+                bool hit[TRK_K];
+                bool anyh = false;
+#pragma unroll
+                for (int k = 0; k < TRK_K; ++k) {
+                    const bool has = m != 0u;
+                    const int hb = has ? 31 - __clz(m) : 0;
+                    m &= ~(1u << hb);
+                    const uint32_t j = (uint32_t)(c0 + hb);
+                    ea[k] = sa + j * 16u;
+                    const float4 s0 = lds128(ea[k]), s1 = lds128(ea[k] + TRK_PL), s2 = lds128(ea[k] + 2 * TRK_PL);
+                    const float4 s3 = lds128(ea[k] + 3 * TRK_PL);
+                    // branch-free pair evaluation (pair.cuh's sequence and decisions, no early exits) so that the four
+                    // LDS -> FMA -> RCP -> EX2 chains of the trip are scheduled side by side
+                    const float rho2 = pair_rho2(s0, s1, s2, lx, ly, r[k].u, r[k].v);
+                    r[k].z = __fmaf_rn(s2.z, r[k].v, __fmaf_rn(s2.y, r[k].u, s2.w));
+                    r[k].G = fast_ex2(__fmul_rn(rho2, -0.72134752044448170368f));
+                    r[k].a = fminf(cfg.alpha_max, __fmul_rn(s3.x, r[k].G));
+                    hit[k] = has && (boff + j) < last && (rho2 <= cfg.cutoff2) && (r[k].z > cfg.z_near) && (r[k].a >= cfg.alpha_min);
+                    opac[k] = s3.x;
+                    inv1ma[k] = fast_rcp(1.f - r[k].a);
+                    gv[k] = g0 * s3.y + g1 * s3.z + g2 * s3.w + g3 * r[k].z;
+                    anyh = anyh || hit[k];
+                }
+                if (!__any_sync(0xffffffffu, anyh)) continue;
+#pragma unroll
+                for (int k = 0; k < TRK_K; ++k) {  // the recurrence: 4 dependent instructions per hit
+                    const float Ti = T_after * inv1ma[k];  // transmittance in front of this splat
+                    const float wk = r[k].a * Ti;
+                    const float dak = Ti * gv[k] - suffix * inv1ma[k];
+                    w[k] = hit[k] ? wk : 0.f;
+                    da[k] = hit[k] ? dak : 0.f;
+                    suffix = hit[k] ? fmaf(wk, gv[k], suffix) : suffix;
+                    T_after = hit[k] ? Ti : T_after;
+                }
+#pragma unroll
+                for (int k = 0; k < TRK_K; ++k) {  // the geometric chain, predicated per lane (no divergent branches)
+                    const float4 s5 = lds128(ea[k] + 5 * TRK_PL), s6 = lds128(ea[k] + 6 * TRK_PL);
+                    const float m2 = lds32(ea[k] + 7 * TRK_PL);
+                    const bool clamped = opac[k] * r[k].G > cfg.alpha_max;  // R5: true derivative, zero when clamped
+                    const float dG = clamped ? 0.f : da[k] * opac[k];
+                    const float gu = -r[k].u * r[k].G * dG, gvv = -r[k].v * r[k].G * dG, gz = g3 * w[k];
+                    // f = [ r x (a_v gu - a_u gv) + m gz ] / (r . m)
+                    const float q0 = s5.w * gu - s5.x * gvv, q1 = s6.x * gu - s5.y * gvv, q2 = s6.y * gu - s5.z * gvv;
+                    const float m0 = s6.z, m1 = s6.w;
+                    const float inv_rm = fast_rcp(rx * m0 + ry * m1 + m2);
+                    const float f0 = hit[k] ? (ry * q2 - q1 + m0 * gz) * inv_rm : 0.f;
+                    const float f1 = hit[k] ? (q0 - rx * q2 + m1 * gz) * inv_rm : 0.f;
+                    const float f2 = hit[k] ? (rx * q1 - ry * q0 + m2 * gz) * inv_rm : 0.f;
+                    const float zk = hit[k] ? r[k].z : 0.f;  // a rejected pair may carry inf / NaN
+                    F0 += f0; F1 += f1; F2 += f2;
+                    Z0 = fmaf(zk, f0, Z0); Z1 = fmaf(zk, f1, Z1); Z2 = fmaf(zk, f2, Z2);
+                }
             }
         }
     };
@@ -323,7 +393,70 @@ k_track(uint32_t* __restrict__ ranges, const uint32_t* __restrict__ cursor, unsi
         for (int w2 = 0; w2 < 8; ++w2) s += s_red[w2][tid];
         pose_partial[(size_t)tile * 8 + tid] = s;
     }
-    finish_pose(pose_partial, gridDim.x, counters, d_pose6, loss_out);
+    if (tid == 0) tile_cost[tile] = (uint32_t)((clock64() - t_start) >> 8);  // feedback for the next iteration's order
+    if (!finish_pose(pose_partial, gridDim.x, counters, d_pose6, loss_out)) return;
+    // ---- last block: longest-first tile order for the NEXT iteration ----
+    // One block per tile, and tiles differ several-fold in work (C2: 20 k .. 130 k cycles), so the tail of this
+    // kernel is set by when the long tiles start.  Every block has stored the cycles it took (tile_cost) before
+    // drawing its ticket; consecutive tracking iterations differ by a small pose step, so those costs predict the
+    // next iteration's.  Counting sort of the tiles by cost, descending, into tile_order (in place: every block
+    // of this launch has read its entry).  Ties land in arbitrary order; the order steers scheduling, never a result.
+    unsigned int* s_hist = reinterpret_cast<unsigned int*>(&sh[0][0]);  // staging memory is free now
+    const int tiles = (int)gridDim.x;
+    __syncthreads();
+    for (int b = tid; b < TRK_ORDER_BINS; b += SGS_BLOCK) s_hist[b] = 0;
+    __syncthreads();
+    constexpr int ORD_U = 8;  // one pass covers ORD_U * 256 = 2048 tiles with the keys kept in registers
+    unsigned int kb[ORD_U];
+    auto load_keys = [&](int t0) {
+#pragma unroll
+        for (int k = 0; k < ORD_U; ++k) {
+            const int t = t0 + k * SGS_BLOCK;
+            kb[k] = t < tiles ? min(__ldcg(tile_cost + t), (unsigned int)(TRK_ORDER_BINS - 1)) : 0xffffffffu;
+        }
+    };
+    for (int t0 = tid; t0 < tiles; t0 += ORD_U * SGS_BLOCK) {
+        load_keys(t0);
+#pragma unroll
+        for (int k = 0; k < ORD_U; ++k)
+            if (kb[k] != 0xffffffffu) atomicAdd(&s_hist[kb[k]], 1u);
+    }
+    __syncthreads();
+    // exclusive scan over the bins from the largest cost down: thread k owns a contiguous run of bins
+    constexpr int PER = TRK_ORDER_BINS / SGS_BLOCK;
+    unsigned int local = 0;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) local += s_hist[TRK_ORDER_BINS - 1 - (tid * PER + k)];
+    unsigned int incl = local;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const unsigned int t2 = __shfl_up_sync(0xffffffffu, incl, off);
+        if (lane >= off) incl += t2;
+    }
+    if (lane == 31) s_wmax[wid] = incl;
+    __syncthreads();
+    unsigned int run = incl - local;
+    for (int w2 = 0; w2 < wid; ++w2) run += s_wmax[w2];
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        const int b = TRK_ORDER_BINS - 1 - (tid * PER + k);
+        const unsigned int c2 = s_hist[b];
+        s_hist[b] = run;  // first output slot of this bin
+        run += c2;
+    }
+    __syncthreads();
+    const bool one_pass = tiles <= ORD_U * SGS_BLOCK;
+    for (int t0 = tid; t0 < tiles; t0 += ORD_U * SGS_BLOCK) {
+        if (!one_pass) load_keys(t0);
+#pragma unroll
+        for (int k = 0; k < ORD_U; ++k)
+            if (kb[k] != 0xffffffffu) tile_order[atomicAdd(&s_hist[kb[k]], 1u)] = (uint32_t)(t0 + k * SGS_BLOCK);
+    }
+}
+
+__global__ void k_iota(uint32_t* __restrict__ p, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = (uint32_t)i;
 }
 
 }  // namespace
@@ -335,17 +468,22 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
     TrackPlanes out;
     bool any = false;
     for (int i = 0; i < 8; ++i) { out.p[i] = planes ? planes[i] : nullptr; any = any || out.p[i] != nullptr; }
+    if (!(c->cost_tiles == tiles && c->cost_W == cam.W && c->cost_H == cam.H)) {  // no order yet for this camera
+        k_iota<<<(tiles + 255) / 256, 256, 0, s>>>(c->tile_order, tiles);
+        c->launches += 1;
+    }
     SgsStage st(c, SGS_STAGE_TRACK, s);
     c->launches += 1;
     unsigned long long* bucket = reinterpret_cast<unsigned long long*>(c->bucket);
     const int presorted = c->fused_sort ? 0 : 1;
     if (any)
-        k_track<true><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->cursor, bucket, (uint32_t)c->tile_cap, presorted, c->pay, cam.W,
+        k_track<true><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, (uint32_t)c->tile_cap, presorted, c->pay, cam.W,
                                                   cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb,
-                                                  tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss);
+                                                  tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost);
     else
-        k_track<false><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->cursor, bucket, (uint32_t)c->tile_cap, presorted, c->pay, cam.W,
+        k_track<false><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, (uint32_t)c->tile_cap, presorted, c->pay, cam.W,
                                                    cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb,
-                                                   tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss);
+                                                   tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost);
+    c->cost_tiles = tiles; c->cost_W = cam.W; c->cost_H = cam.H;
     return cudaGetLastError();
 }
