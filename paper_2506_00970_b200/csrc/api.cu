@@ -93,7 +93,7 @@ int sgs_ensure_buckets(sgs_ctx* c, int tiles, int64_t tile_cap, cudaStream_t s) 
     if (cap == c->tile_cap && (int64_t)tiles * cap <= c->bucket_cap && tiles <= c->cursor_cap) return SGS_OK;
     cudaStreamSynchronize(s);
     if (tiles > c->cursor_cap) {
-        if (!(ws_realloc(c, c->cursor, (size_t)tiles + 64, s) && ws_realloc(c, c->tile_order, (size_t)tiles + 64, s) &&
+        if (!(ws_realloc(c, c->cursor, (size_t)tiles + 64, s) && ws_realloc(c, c->tile_order, (size_t)tiles + 64, s) && ws_realloc(c, c->render_order, (size_t)tiles + 64, s) &&
               ws_realloc(c, c->tile_cost, (size_t)tiles + 64, s)))
             return SGS_OUT_OF_MEMORY;
         c->cursor_cap = tiles;
@@ -217,7 +217,7 @@ int sgs_destroy(sgs_ctx* c) {
                     c->pay.g5, c->pay.g6, c->pay.g7, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
                     c->sort_state, c->ranges, c->T_final, c->n_last, c->img_scratch, c->pose_partial, c->resident_store,
                     c->resident_active, c->target_rgb, c->host_img_dev, c->host_up_dev, c->host_grads_dev,
-                    c->bucket, c->cursor, c->tile_order, c->tile_cost, c->export_keys, c->export_ranges};
+                    c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->export_keys, c->export_ranges};
     for (void* p : ptrs) sgs_ws_free(c, p, s);
     if (c->counters) cudaFree(c->counters);
     if (c->counters_host) cudaFreeHost(c->counters_host);

@@ -34,7 +34,7 @@ static int copy_counters(sgs_ctx* c, cudaStream_t s) {
 }
 
 // binning through per-tile buckets + in-tile sort (default)
-static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, cudaStream_t s) {
+static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, bool want_order, cudaStream_t s) {
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
     int r = sgs_ensure_buckets(c, tiles, c->tile_cap ? c->tile_cap : 2048, s);
     if (r != SGS_OK) return r;
@@ -55,6 +55,8 @@ static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, cudaStream
         c->pending_check = true;
     }
     c->fused_sort = c->tile_cap <= 2048;
+    c->render_order_valid = false;
+    if (want_order && sgs_launch_tile_order(c, s) != cudaSuccess) return SGS_CUDA_ERROR;
     if (c->fused_sort) {  // k_forward orders each bucket itself
         c->list_vals = reinterpret_cast<const uint32_t*>(c->bucket);
         c->list_stride = 2;
@@ -95,13 +97,14 @@ static int bin_radix(sgs_ctx* c, const sgs_surfels* sf, bool async, cudaStream_t
         c->pending_check = true;
     }
     c->fused_sort = false;
+    c->render_order_valid = false;
     return sgs_launch_sort_and_ranges(c, s) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
 }
 
 extern "C" {
 
 // preprocess + tile binning of one view (shared by sgs_render and sgs_track_iter)
-static int bin_view(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, cudaStream_t s) {
+static int bin_view(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, bool want_order, cudaStream_t s) {
     if (!c || !sf || !sgs_cam_valid(cam) || sf->n < 0 || sf->n >= (1ll << 24)) return SGS_INVALID_ARGUMENT;
     if (sf->n > 0 && (!sf->mean || !sf->scale || !sf->quat || !sf->opacity || !sf->rgb)) return SGS_INVALID_ARGUMENT;
     int r = check_pending(c, s);
@@ -116,7 +119,7 @@ static int bin_view(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, cu
     const bool async = (c->cfg.flags & SGS_FLAG_ASYNC) != 0;
     c->last_surfels = *sf;
     c->last_cam = *cam;
-    return radix_mode(c) ? bin_radix(c, sf, async, s) : bin_buckets(c, sf, async, s);
+    return radix_mode(c) ? bin_radix(c, sf, async, s) : bin_buckets(c, sf, async, want_order, s);
 }
 
 static void pick_planes(sgs_ctx* c, const sgs_images* out, int64_t pixels, bool scratch, float* planes[8]) {
@@ -131,7 +134,7 @@ static void pick_planes(sgs_ctx* c, const sgs_images* out, int64_t pixels, bool 
 
 int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* out, void* stream) {
     cudaStream_t s = (cudaStream_t)stream;
-    int r = bin_view(c, sf, cam, s);
+    int r = bin_view(c, sf, cam, true, s);
     if (r != SGS_OK) return r;
     const int64_t pixels = (int64_t)cam->width * cam->height;
     float* planes[8];
@@ -154,7 +157,7 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
         c->have_forward = false;
         return r;
     }
-    int r = bin_view(c, sf, cam, s);
+    int r = bin_view(c, sf, cam, false, s);
     if (r != SGS_OK) return r;
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
     if ((r = sgs_ensure_partials(c, tiles, s)) != SGS_OK) return r;

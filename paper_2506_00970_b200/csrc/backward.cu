@@ -21,6 +21,8 @@ namespace {
 
 struct CPlanes { const float* p[8]; };
 
+constexpr int BWD_K = 2;  // entries per trip of the reverse walk
+
 struct StagedBwd {
     float4 s0, s1, s2, s3, s4;  // as StagedFwd
     float4 s5;                  // a_u.xyz, a_v.x
@@ -60,7 +62,7 @@ struct FusedLoss { const float* trgb; const float* tdepth; float lambda_d, nsign
 
 template <bool POSE_ONLY, bool FUSED>
 __global__ void __launch_bounds__(SGS_BLOCK)
-k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
+k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
            int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg, CPlanes up,
            const float* __restrict__ T_final, const uint32_t* __restrict__ n_last, float* __restrict__ acc,
            float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
@@ -68,7 +70,7 @@ k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ val
     __shared__ StagedBwd sh[SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
     __shared__ float s_red[8][7];
-    const int tile = blockIdx.x;
+    const int tile = tile_order ? (int)tile_order[blockIdx.x] : (int)blockIdx.x;  // longest tiles first
     const int tx = tile % tiles_x, ty = tile / tiles_x;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int lxi = (wid & 1) * 8 + (lane & 7), lyi = (wid >> 1) * 4 + (lane >> 3);
@@ -159,55 +161,80 @@ k_backward(const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ val
           // this chunk's entries whose AABB reaches the warp's patch, walked from the back
           unsigned m = __ballot_sync(0xffffffffu, (c0 + lane < jend) && ((sh_mask[c0 + lane] >> wid) & 1u));
           while (m) {
-            const int hb = 31 - __clz(m);
-            m &= ~(1u << hb);
-            const int j = c0 + hb;
-            const float4 s0 = sh[j].s0, s1 = sh[j].s1, s2 = sh[j].s2, s3 = sh[j].s3;
-            PairResult r;
-            bool hit = (boff + (uint32_t)j) < last;
-            if (hit) hit = eval_pair(s0, s1, s2, s3.x, lx, ly, cfg.cutoff2, cfg.alpha_min, cfg.alpha_max, cfg.z_near, r);
-            if (!__any_sync(0xffffffffu, hit)) continue;
-            float x[16];
+            // BWD_K entries per trip, back to front, in phases (see track.cu): branch-free pair evaluation,
+            // 1/(1-a) and g.v of all entries side by side; then the T_i / suffix recurrence (4 dependent
+            // instructions per hit); then the geometric chain of each entry some lane hit.
+            int jj[BWD_K];
+            PairResult r[BWD_K];
+            float inv1ma[BWD_K], gv[BWD_K], opac[BWD_K], da[BWD_K], w[BWD_K];
+            bool hit[BWD_K];
 #pragma unroll
-            for (int c = 0; c < 16; ++c) x[c] = 0.f;
-            if (hit) {
+            for (int k = 0; k < BWD_K; ++k) {
+                const bool has = m != 0u;
+                const int hb = has ? 31 - __clz(m) : 0;
+                m &= ~(1u << hb);
+                const int j = c0 + hb;
+                jj[k] = j;
+                const float4 s0 = sh[j].s0, s1 = sh[j].s1, s2 = sh[j].s2, s3 = sh[j].s3, s4 = sh[j].s4;
+                const float un = __fmaf_rn(ly, s0.y, __fmaf_rn(lx, s0.x, s0.z));
+                const float vn = __fmaf_rn(ly, s1.y, __fmaf_rn(lx, s1.x, s1.z));
+                const float dn = __fmaf_rn(ly, s1.w, __fmaf_rn(lx, s0.w, s2.x));
+                const float inv = fast_rcp(dn);
+                r[k].u = __fmul_rn(un, inv); r[k].v = __fmul_rn(vn, inv);
+                const float rho2 = __fmaf_rn(r[k].v, r[k].v, __fmul_rn(r[k].u, r[k].u));
+                r[k].z = __fmaf_rn(s2.z, r[k].v, __fmaf_rn(s2.y, r[k].u, s2.w));
+                r[k].G = fast_ex2(__fmul_rn(rho2, -0.72134752044448170368f));
+                r[k].a = fminf(cfg.alpha_max, __fmul_rn(s3.x, r[k].G));
+                hit[k] = has && (boff + (uint32_t)j) < last && (rho2 <= cfg.cutoff2) && (r[k].z > cfg.z_near) &&
+                         (r[k].a >= cfg.alpha_min);
+                opac[k] = s3.x;
+                inv1ma[k] = fast_rcp(1.f - r[k].a);
+                gv[k] = g[0] * s3.y + g[1] * s3.z + g[2] * s3.w + g[3] * r[k].z + g[4] * s4.x + g[5] * s4.y + g[6] * s4.z + g[7];
+            }
+#pragma unroll
+            for (int k = 0; k < BWD_K; ++k) {
+                const float Ti = T_after * inv1ma[k];  // transmittance in front of this splat
+                const float wk = r[k].a * Ti;
+                const float dak = Ti * gv[k] - suffix * inv1ma[k];
+                w[k] = hit[k] ? wk : 0.f;
+                da[k] = hit[k] ? dak : 0.f;
+                suffix = hit[k] ? fmaf(wk, gv[k], suffix) : suffix;
+                T_after = hit[k] ? Ti : T_after;
+            }
+#pragma unroll
+            for (int k = 0; k < BWD_K; ++k) {
+                if (!__any_sync(0xffffffffu, hit[k])) continue;
+                const int j = jj[k];
                 const float4 s4 = sh[j].s4, s5 = sh[j].s5, s6 = sh[j].s6, s7 = sh[j].s7;
-                const float inv1ma = fast_rcp(1.f - r.a);
-                const float Ti = T_after * inv1ma;  // transmittance in front of this splat
-                const float w = r.a * Ti;
-                const float gv = g[0] * s3.y + g[1] * s3.z + g[2] * s3.w + g[3] * r.z + g[4] * s4.x + g[5] * s4.y +
-                                 g[6] * s4.z + g[7];
-                const float da = Ti * gv - suffix * inv1ma;
-                suffix = fmaf(w, gv, suffix);
-                T_after = Ti;
-                const bool clamped = s3.x * r.G > cfg.alpha_max;  // R5: true derivative, zero when clamped
-                const float dG = clamped ? 0.f : da * s3.x;
-                const float gu = -r.u * r.G * dG, gvv = -r.v * r.G * dG, gz = g[3] * w;
+                const bool clamped = opac[k] * r[k].G > cfg.alpha_max;  // R5: true derivative, zero when clamped
+                const float dG = clamped ? 0.f : da[k] * opac[k];
+                const float gu = -r[k].u * r[k].G * dG, gvv = -r[k].v * r[k].G * dG, gz = g[3] * w[k];
                 // f = [ r x (a_v gu - a_u gv) + m gz ] / (r . m)
                 const float q0 = s5.w * gu - s5.x * gvv, q1 = s6.x * gu - s5.y * gvv, q2 = s6.y * gu - s5.z * gvv;
                 const float m0 = s6.z, m1 = s6.w, m2 = s7.x;
                 const float inv_rm = fast_rcp(rx * m0 + ry * m1 + m2);
-                const float f0 = (ry * q2 - q1 + m0 * gz) * inv_rm;
-                const float f1 = (q0 - rx * q2 + m1 * gz) * inv_rm;
-                const float f2 = (rx * q1 - ry * q0 + m2 * gz) * inv_rm;
+                // a rejected pair may carry inf / NaN: its lanes contribute exact zeros
+                const float f0 = hit[k] ? (ry * q2 - q1 + m0 * gz) * inv_rm : 0.f;
+                const float f1 = hit[k] ? (q0 - rx * q2 + m1 * gz) * inv_rm : 0.f;
+                const float f2 = hit[k] ? (rx * q1 - ry * q0 + m2 * gz) * inv_rm : 0.f;
+                const float uk = hit[k] ? r[k].u : 0.f, vk = hit[k] ? r[k].v : 0.f, zk = hit[k] ? r[k].z : 0.f;
                 if (POSE_ONLY) {
                     F0 += f0; F1 += f1; F2 += f2;
-                    Z0 = fmaf(r.z, f0, Z0); Z1 = fmaf(r.z, f1, Z1); Z2 = fmaf(r.z, f2, Z2);
-                    Nn0 = fmaf(w, s4.x, Nn0); Nn1 = fmaf(w, s4.y, Nn1); Nn2 = fmaf(w, s4.z, Nn2);
+                    Z0 = fmaf(zk, f0, Z0); Z1 = fmaf(zk, f1, Z1); Z2 = fmaf(zk, f2, Z2);
+                    Nn0 = fmaf(w[k], s4.x, Nn0); Nn1 = fmaf(w[k], s4.y, Nn1); Nn2 = fmaf(w[k], s4.z, Nn2);
                 } else {
+                    float x[16];
                     x[0] = f0; x[1] = f1; x[2] = f2;
-                    x[3] = r.u * f0; x[4] = r.u * f1; x[5] = r.u * f2;
-                    x[6] = r.v * f0; x[7] = r.v * f1; x[8] = r.v * f2;
-                    x[9] = w * g[4]; x[10] = w * g[5]; x[11] = w * g[6];
-                    x[12] = w * g[0]; x[13] = w * g[1]; x[14] = w * g[2];
-                    x[15] = clamped ? 0.f : da * r.G;
-                }
-            }
-            if (!POSE_ONLY) {
-                const float red = reduce16_transposed(x, lane);
-                if ((lane & 1) == 0) {
-                    const uint32_t v = __float_as_uint(sh[j].s7.y);
-                    atomicAdd(acc + (size_t)v * SGS_ACC_STRIDE + (lane >> 1), red);
+                    x[3] = uk * f0; x[4] = uk * f1; x[5] = uk * f2;
+                    x[6] = vk * f0; x[7] = vk * f1; x[8] = vk * f2;
+                    x[9] = w[k] * g[4]; x[10] = w[k] * g[5]; x[11] = w[k] * g[6];
+                    x[12] = w[k] * g[0]; x[13] = w[k] * g[1]; x[14] = w[k] * g[2];
+                    x[15] = (clamped || !hit[k]) ? 0.f : da[k] * r[k].G;
+                    const float red = reduce16_transposed(x, lane);
+                    if ((lane & 1) == 0) {
+                        const uint32_t v = __float_as_uint(sh[j].s7.y);
+                        atomicAdd(acc + (size_t)v * SGS_ACC_STRIDE + (lane >> 1), red);
+                    }
                 }
             }
           }
@@ -367,7 +394,7 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     if (dg == nullptr) {  // pose-only (tracking, L204)
         if (d_pose6 == nullptr) return cudaSuccess;
         c->launches += 1;
-        k_backward<true, false><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
+        k_backward<true, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                      cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
                                                      c->acc, c->pose_partial, c->counters, d_pose6, FusedLoss{});
         return cudaGetLastError();
@@ -386,7 +413,7 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     }
     if (e != cudaSuccess) return e;
     c->launches += 1;
-    k_backward<false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
+    k_backward<false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                   cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
                                                   c->acc, c->pose_partial, c->counters, nullptr, FusedLoss{});
     const int blocks = (int)((n + 255) / 256);  // bound on N_v; blocks past it only join the pose reduction
@@ -409,7 +436,7 @@ cudaError_t sgs_launch_backward_tracking(sgs_ctx* c, const float* trgb, const fl
     const SgsCamDev& cam = c->camd;
     FusedLoss fl{trgb, tdepth, lambda_d, nsign, loss};
     c->launches += 1;
-    k_backward<true, true><<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H,
+    k_backward<true, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H,
                                                        cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final,
                                                        c->n_last, c->acc, c->pose_partial, c->counters, d_pose6, fl);
     return cudaGetLastError();

@@ -14,7 +14,7 @@ namespace {
 struct Planes { float* p[8]; };
 
 __global__ void __launch_bounds__(SGS_BLOCK)
-k_forward(uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
+k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
           int tiles_x, SgsCfgDev cfg, Planes out, float* __restrict__ T_final, uint32_t* __restrict__ n_last,
           const uint32_t* __restrict__ cursor, unsigned long long* bucket, uint32_t tile_cap) {
     // staged batch, structure of float4 arrays (one base register, immediate offsets, broadcast reads)
@@ -22,7 +22,7 @@ k_forward(uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int 
     __shared__ unsigned char sh_mask[SGS_BLOCK];
     const uint32_t sa = smem_addr(&sh[0][0]), sm_a = smem_addr(sh_mask);
     constexpr uint32_t PL = SGS_BLOCK * 16;  // bytes per staged plane
-    const int tile = blockIdx.x;
+    const int tile = tile_order ? (int)tile_order[blockIdx.x] : (int)blockIdx.x;  // longest tiles first
     const int tx = tile % tiles_x, ty = tile / tiles_x;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int lxi = (wid & 1) * 8 + (lane & 7), lyi = (wid >> 1) * 4 + (lane >> 3);
@@ -152,7 +152,7 @@ cudaError_t sgs_launch_forward(sgs_ctx* c, float* const planes[8], cudaStream_t 
     for (int i = 0; i < 8; ++i) out.p[i] = planes[i];
     SgsStage st(c, SGS_STAGE_FORWARD, s);
     c->launches += 1;
-    k_forward<<<tiles, SGS_BLOCK, 0, s>>>(c->ranges, c->list_vals, c->list_stride, c->pay, c->camd.W, c->camd.H, c->camd.tiles_x,
+    k_forward<<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, c->camd.W, c->camd.H, c->camd.tiles_x,
                                           c->cfgd, out, c->T_final, c->n_last, c->fused_sort ? c->cursor : nullptr,
                                           reinterpret_cast<unsigned long long*>(c->bucket), (uint32_t)c->tile_cap);
     return cudaGetLastError();

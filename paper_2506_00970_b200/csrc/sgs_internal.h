@@ -84,6 +84,8 @@ struct sgs_ctx {
     uint64_t* bucket;                // tiles x tile_cap keys: depth bits << 32 | surfel index
     uint32_t* cursor;                // tiles
     uint32_t* tile_order;            // tiles: tile ids by descending entry count (longest first), written by K-pre-B
+    uint32_t* render_order;          // tiles: longest-first order of the last sgs_render's tiles (by entry count), or unused
+    bool render_order_valid;
     int64_t cursor_cap;              // tiles the cursor / tile_order arrays hold
     int64_t tile_cap, bucket_cap;    // entries per tile; allocated keys
     uint64_t* export_keys;           // contiguous (tile << 32 | depth) list for sgs_get_binning
@@ -149,6 +151,7 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
 int sgs_sort_passes(int tiles);
 cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cudaStream_t s);
 cudaError_t sgs_launch_tilesort(sgs_ctx* c, cudaStream_t s);
+cudaError_t sgs_launch_tile_order(sgs_ctx* c, cudaStream_t s);
 cudaError_t sgs_launch_export_bucket(sgs_ctx* c, int64_t n_entries, cudaStream_t s);
 int sgs_ensure_buckets(sgs_ctx* c, int tiles, int64_t tile_cap, cudaStream_t s);
 int sgs_ensure_export(sgs_ctx* c, int tiles, int64_t entries, cudaStream_t s);

@@ -70,6 +70,65 @@ k_tilesort(uint64_t* __restrict__ bucket, const uint32_t* __restrict__ cursor, u
     }
 }
 
+// Longest-first tile order for the compositing kernels of sgs_render / sgs_backward (one block per tile; ncu,
+// profiles/r01_c3_c4_c5.md: SMs were active 80 % of k_forward's and k_backward's duration because the long tiles
+// started late).  One block: counting sort of the tiles by entry count, descending.  Ties land in arbitrary
+// order; the order steers scheduling only, never a result.
+constexpr int ORDER_BINS = 2048, ORDER_THREADS = 1024;
+__global__ void __launch_bounds__(ORDER_THREADS)
+k_tile_order(const uint32_t* __restrict__ cursor, int tiles, uint32_t* __restrict__ order) {
+    __shared__ unsigned int s_hist[ORDER_BINS];
+    __shared__ unsigned int s_wsum[ORDER_THREADS / 32];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    for (int b = tid; b < ORDER_BINS; b += ORDER_THREADS) s_hist[b] = 0;
+    __syncthreads();
+    constexpr int U = 4;  // keys of one pass (U * 1024 = 4096 tiles) stay in registers for the scatter
+    unsigned int kb[U];
+    auto load_keys = [&](int t0) {
+#pragma unroll
+        for (int k = 0; k < U; ++k) {
+            const int t = t0 + k * ORDER_THREADS;
+            kb[k] = t < tiles ? min(cursor[t], (unsigned int)(ORDER_BINS - 1)) : 0xffffffffu;
+        }
+    };
+    for (int t0 = tid; t0 < tiles; t0 += U * ORDER_THREADS) {
+        load_keys(t0);
+#pragma unroll
+        for (int k = 0; k < U; ++k)
+            if (kb[k] != 0xffffffffu) atomicAdd(&s_hist[kb[k]], 1u);
+    }
+    __syncthreads();
+    constexpr int PER = ORDER_BINS / ORDER_THREADS;
+    unsigned int local = 0;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) local += s_hist[ORDER_BINS - 1 - (tid * PER + k)];
+    unsigned int incl = local;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const unsigned int t2 = __shfl_up_sync(0xffffffffu, incl, off);
+        if (lane >= off) incl += t2;
+    }
+    if (lane == 31) s_wsum[wid] = incl;
+    __syncthreads();
+    unsigned int run = incl - local;
+    for (int w2 = 0; w2 < wid; ++w2) run += s_wsum[w2];
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        const int b = ORDER_BINS - 1 - (tid * PER + k);
+        const unsigned int c2 = s_hist[b];
+        s_hist[b] = run;
+        run += c2;
+    }
+    __syncthreads();
+    const bool one_pass = tiles <= U * ORDER_THREADS;
+    for (int t0 = tid; t0 < tiles; t0 += U * ORDER_THREADS) {
+        if (!one_pass) load_keys(t0);
+#pragma unroll
+        for (int k = 0; k < U; ++k)
+            if (kb[k] != 0xffffffffu) order[atomicAdd(&s_hist[kb[k]], 1u)] = (uint32_t)(t0 + k * ORDER_THREADS);
+    }
+}
+
 // ---- debug export for sgs_get_binning: contiguous (tile << 32 | depth) keys, indices and ranges ----
 __global__ void k_export_scan(const uint32_t* __restrict__ ranges, int tiles, uint32_t* __restrict__ xr) {
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -114,6 +173,15 @@ cudaError_t sgs_launch_tilesort(sgs_ctx* c, cudaStream_t s) {
                                                 c->counters);
     c->list_vals = reinterpret_cast<const uint32_t*>(c->bucket);
     c->list_stride = 2;
+    return cudaGetLastError();
+}
+
+cudaError_t sgs_launch_tile_order(sgs_ctx* c, cudaStream_t s) {
+    const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    SgsStage st(c, SGS_STAGE_SORT, s);
+    c->launches += 1;
+    k_tile_order<<<1, ORDER_THREADS, 0, s>>>(c->cursor, tiles, c->render_order);
+    c->render_order_valid = true;
     return cudaGetLastError();
 }
 
