@@ -121,6 +121,31 @@ def render(sc, camv, cfgv, brute=False, counters=True):
                 counters=dict(Q_t=int(cnt[0]), Q_c=int(cnt[1]), cover=int(cnt[2]), n_vis=int(cnt[3]), n_fragile=int(cnt[4]), Q_tb=int(cnt[5])))
 
 
+def contribution(sc, camv, cfgv, brute=False):
+    """Eq. 20-21 (L208-214): C_k^V = sum_p w_k(p), the sum of splat k's blending coefficients over the pixels of
+    the view (fp64, (n,)); zero for inactive, culled or never-composited splats."""
+    mean, scale, quat, opac, rgb, act = _scene_arrays(sc)
+    W, H = int(camv[0]), int(camv[1])
+    img = np.zeros((8, H, W))
+    contrib = np.zeros(sc.n)
+    lib().orc_render_ex(ctypes.c_int64(sc.n), _p(mean, C_F32), _p(scale, C_F32), _p(quat, C_F32), _p(opac, C_F32),
+                        _p(rgb, C_F32), _p(act, C_U8), _p(camv, C_F64), _p(cfgv, C_F64), ctypes.c_int(int(brute)),
+                        _p(img, C_F64), None, None, None, None, None, _p(contrib, C_F64))
+    return contrib
+
+
+def covisibility(contrib_a, contrib_b, active=None, threshold=0.5):
+    """Eq. 22 (L216-221): |G_A n G_B| / |G_A u G_B| with G_V = {k in M_A : C_k^V > 0.5}.  Returns
+    (score, n_intersection, n_union); the score of two empty sets is 0."""
+    a = np.asarray(contrib_a) > threshold
+    b = np.asarray(contrib_b) > threshold
+    if active is not None:
+        m = np.asarray(active).astype(bool)
+        a, b = a & m, b & m
+    inter, union = int((a & b).sum()), int((a | b).sum())
+    return (inter / union if union else 0.0), inter, union
+
+
 def backward(sc, camv, cfgv, upstream, brute=False, debug=False):
     """Analytic backward (O5-O7).  upstream: (8,H,W).  Returns fp64 grads for mean, scale, quat,
     opacity, rgb, and pose (6,) = (rho, theta) under T <- Exp(tau) o T_cw (Eq. 11-13)."""

@@ -372,11 +372,18 @@ static inline int64_t cand_count(const Ctx* c, int i, int j, const uint32_t** ls
  * the stopping entry, [1]=Q_c composited pairs, [2]=covering pairs (rho^2<=c^2, z>z_near) over
  * ALL surfels ignoring termination (depth complexity), [3]=n_vis, [4]=fragile pixels,
  * [5]=Q_tb tile-list pairs up to and incl. each pixel's LAST COMPOSITED entry (what a reverse traversal revisits). */
-void orc_render(int64_t n, const float* mean, const float* scale, const float* quat,
-                const float* opacity, const float* rgb, const uint8_t* active,
-                const double* camv, const double* cfgv, int brute,
-                double* img, double* T_final, int32_t* n_comp, uint8_t* fragile, int64_t* counters,
-                int32_t* qtb_pix /* nullable: per-pixel Q_tb */) {
+static inline void atomic_add_fwd(double* p, double v) {
+#pragma omp atomic
+    *p += v;
+}
+
+/* contrib (nullable, n doubles, zero-initialised by the caller): the contribution of splat k to the view,
+ * C_k^V = sum over pixels of its blending coefficient w_k(p) = a_k T_k (Eq. 20-21). */
+void orc_render_ex(int64_t n, const float* mean, const float* scale, const float* quat,
+                   const float* opacity, const float* rgb, const uint8_t* active,
+                   const double* camv, const double* cfgv, int brute,
+                   double* img, double* T_final, int32_t* n_comp, uint8_t* fragile, int64_t* counters,
+                   int32_t* qtb_pix /* nullable: per-pixel Q_tb */, double* contrib) {
     Ctx c; ctx_init(&c, n, mean, scale, quat, opacity, rgb, active, camv, cfgv, brute);
     const int W = c.cam.W, H = c.cam.H; const int64_t HW = (int64_t)W * H;
     int64_t Qt = 0, Qc = 0, Qcover = 0, nfrag = 0, Qtb = 0;
@@ -412,6 +419,7 @@ void orc_render(int64_t n, const float* mean, const float* scale, const float* q
                 acc[3] += w * r.z;
                 acc[4] += w * p->tnc[0]; acc[5] += w * p->tnc[1]; acc[6] += w * p->tnc[2];
                 acc[7] += w;
+                if (contrib) atomic_add_fwd(contrib + k, w); /* Eq. 21 */
                 T *= (1.0 - r.a);
                 ++nc; ++Qc;
                 qt_last = qt_pix;
@@ -428,6 +436,15 @@ void orc_render(int64_t n, const float* mean, const float* scale, const float* q
     }
     if (counters) { counters[0] = Qt; counters[1] = Qc; counters[2] = Qcover; counters[3] = c.n_vis; counters[4] = nfrag; counters[5] = Qtb; }
     ctx_free(&c);
+}
+
+void orc_render(int64_t n, const float* mean, const float* scale, const float* quat,
+                const float* opacity, const float* rgb, const uint8_t* active,
+                const double* camv, const double* cfgv, int brute,
+                double* img, double* T_final, int32_t* n_comp, uint8_t* fragile, int64_t* counters,
+                int32_t* qtb_pix) {
+    orc_render_ex(n, mean, scale, quat, opacity, rgb, active, camv, cfgv, brute, img, T_final, n_comp, fragile, counters,
+                  qtb_pix, NULL);
 }
 
 /* ---------------------------------------------------------------------------------------------

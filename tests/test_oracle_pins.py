@@ -379,3 +379,60 @@ def test_no_view_dependence_of_colour():
         m = r["img"][7] > 0.05
         for ch, c in enumerate((0.3, 0.6, 0.9)):
             np.testing.assert_allclose(r["img"][ch][m] / r["img"][7][m], float(np.float32(c)), rtol=1e-12)
+
+
+# ---------------------------------------------------------------- P11: per-splat contribution and covisibility (Eq. 20-22)
+def _footprint_alpha(mu, su, sv, o, cam=CAM):
+    """Closed-form alpha image of a fronto-parallel surfel (as P1), fp64, with the truncation conventions."""
+    X, Y = pix_grid(cam)
+    mu32 = np.float32(mu).astype(np.float64); su, sv, o = [float(np.float32(v)) for v in (su, sv, o)]
+    u = ((X - cam.cx) * mu32[2] / cam.fx - mu32[0]) / su
+    v = ((Y - cam.cy) * mu32[2] / cam.fy - mu32[1]) / sv
+    a = np.minimum(o * np.exp(-(u * u + v * v) / 2), float(np.float32(0.99)))
+    a[(u * u + v * v > 9.0) | (a < float(np.float32(1 / 255)))] = 0.0
+    return a
+
+
+def test_p11_contribution_sums_to_the_alpha_image(c1):
+    """Eq. 21 summed over k is Eq. 8's accumulated opacity summed over the pixels: sum_k C_k = sum_p O(p)."""
+    sc, cam, camv, cfg, r = c1
+    C = oracle.contribution(sc, camv, cfg)
+    assert abs(C.sum() - r["img"][7].sum()) <= 1e-10 * C.sum()
+    assert (C >= 0).all() and (C[oracle.binning(sc, camv, cfg)["culled"].astype(bool)] == 0).all()
+    assert np.abs(C - oracle.contribution(sc, camv, cfg, brute=True)).max() <= 1e-12 * C.max()
+
+
+def test_p11_single_surfel_and_occlusion_closed_forms():
+    """C of a lone fronto-parallel splat is the sum of its closed-form footprint; behind a second splat with the same
+    footprint every coefficient is scaled by that pixel's (1 - a_front) (Eq. 20)."""
+    a_front = _footprint_alpha((0.1, -0.05, 1.5), 0.09, 0.06, 0.7)
+    sc1 = one_surfel((0.1, -0.05, 1.5), (0.09, 0.06), (1, 0, 0, 0), 0.7)
+    camv, cfg = oracle.make_cam(CAM), oracle.make_cfg()
+    np.testing.assert_allclose(oracle.contribution(sc1, camv, cfg), [a_front.sum()], rtol=1e-12)
+    a_back = _footprint_alpha((0.0, 0.0, 2.5), 0.2, 0.2, 0.9)
+    sc2 = cat(one_surfel((0.0, 0.0, 2.5), (0.2, 0.2), (1, 0, 0, 0), 0.9), sc1)   # index order != depth order
+    C = oracle.contribution(sc2, camv, cfg)
+    np.testing.assert_allclose(C, [(a_back * (1 - a_front)).sum(), a_front.sum()], rtol=1e-12)
+
+
+def test_p11_contribution_approaches_the_footprint_integral():
+    """"How many pixels the splat contributes to" (L214): for a footprint of many pixels C tends to the integral of
+    o exp(-rho^2/2) over the cutoff ellipse, 2 pi o sx sy (1 - exp(-c^2/2)) with s = f s_world / z pixels."""
+    cam = Camera(400, 300, 300.0, 300.0, 200.0, 150.0)
+    su, sv, o, z0 = 0.12, 0.08, 0.6, 2.0
+    sc = one_surfel((0.0, 0.0, z0), (su, sv), (1, 0, 0, 0), o)
+    C = oracle.contribution(sc, oracle.make_cam(cam), oracle.make_cfg())[0]
+    sx, sy = 300.0 * float(np.float32(su)) / z0, 300.0 * float(np.float32(sv)) / z0
+    expect = 2 * np.pi * float(np.float32(o)) * sx * sy * (1 - np.exp(-4.5))
+    assert abs(C - expect) <= 2e-3 * expect
+
+
+def test_p11_covisibility_hand_example():
+    """Eq. 22 on a hand example: G_A = {0,1,2}, G_B = {1,2,3} -> 2/4; identical views -> 1; disjoint -> 0."""
+    CA = np.array([0.9, 3.0, 0.51, 0.5, 0.0]); CB = np.array([0.2, 0.6, 7.0, 0.7, 0.5])
+    assert oracle.covisibility(CA, CB) == (0.5, 2, 4)
+    assert oracle.covisibility(CA, CA)[0] == 1.0
+    assert oracle.covisibility(CA, np.zeros(5)) == (0.0, 0, 3)
+    act = np.array([1, 0, 1, 1, 1], np.uint8)                       # only splats of the active map count (L216)
+    assert oracle.covisibility(CA, CB, active=act) == (1 / 3, 1, 3)
+    assert oracle.covisibility(np.zeros(3), np.zeros(3)) == (0.0, 0, 0)
