@@ -119,7 +119,8 @@ def aggregate_replicas(ms_local, pixels, renders_per_rank, world, dist=None, dev
 class Workload:
     """Device-resident inputs + the step function for one config."""
 
-    def __init__(self, name, iters_override=None):
+    def __init__(self, name, iters_override=None, contrib=False):
+        self.contrib = contrib
         import torch
         import scenegen
         import paper_2506_00970_b200 as sgs
@@ -140,6 +141,7 @@ class Workload:
         self.up = dict(rgb=z(3), depth=z(1), normal=z(3), alpha=z(1))
         self.ccams = [sgs.make_camera(c.width, c.height, c.fx, c.fy, c.cx, c.cy, c.T_cw) for c in self.cams]
         self.p6 = torch.zeros(6, device="cuda")
+        self.contrib_buf = torch.zeros(sc.n, device="cuda") if contrib else None
         self.loss = torch.zeros(1, device="cuda")
         self.n_active = int(sc.n if sc.active is None else sc.active.sum())
         # target frame(s): the renderer's own image at the perturbed pose Exp(tau0) T
@@ -176,7 +178,10 @@ class Workload:
         if self.tracking:  # one tracking iteration: K-pre + K-track (render, Eq. 15-19 loss, pose-only backward); images written
             self.ren.track_iter(self.sf, cam, trgb, tdep, 0.5, -1.0, self.p6, self.loss, **self.im)
             return
-        self.ren.render(self.sf, cam, **self.im)
+        if self.contrib:  # forward with the per-splat contribution output (Eq. 20-21) switched on
+            self.ren.render_contrib(self.sf, cam, self.contrib_buf, **self.im)
+        else:
+            self.ren.render(self.sf, cam, **self.im)
         self.ren.tracking_loss(cam, self.im, trgb, tdep, 0.5, -1.0, self.up, self.loss)
         u = self.up
         if True:
@@ -299,6 +304,7 @@ def main():
     ap.add_argument("--iters", type=int, default=None, help="override iterations per tracking step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--contrib", action="store_true", help="mapping configs: render with sgs_render_contrib (C_k output on)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -317,7 +323,7 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    wl = Workload(args.config, args.iters)
+    wl = Workload(args.config, args.iters, args.contrib)
     K, W = args.steps, max(args.warmup, 3)
     for _ in range(W):
         wl.step()

@@ -139,6 +139,20 @@ SGS_API int sgs_destroy(sgs_ctx* ctx);
 SGS_API int sgs_render(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_camera* cam, const sgs_images* out,
                void* cuda_stream);
 
+/* sgs_render that additionally returns the contribution of every splat to the view (Eq. 20-21):
+ * contrib[k] = C_k^V = sum over pixels of w_k(p) = a_k T_k, "how many pixels the splat contributes to"; the
+ * paper calls a splat visible in the view when C_k^V > 0.5 (keyframe selection, state update, pruning).
+ *   contrib: DEVICE, n floats, overwritten; exactly 0 for inactive, culled or never-composited splats. */
+SGS_API int sgs_render_contrib(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_camera* cam, const sgs_images* out,
+                               float* contrib, void* cuda_stream);
+
+/* Covisibility score of two views (Eq. 22): |G_A n G_B| / |G_A u G_B| with
+ * G_V = {k : active[k] != 0 and C_k^V > threshold} (paper: threshold 0.5).
+ *   contrib_a, contrib_b: DEVICE, n floats (outputs of sgs_render_contrib);  active: DEVICE n bytes or NULL
+ *   result3: DEVICE, 3 floats, overwritten: score (0 when the union is empty), |intersection|, |union| */
+SGS_API int sgs_covisibility(sgs_ctx* ctx, const float* contrib_a, const float* contrib_b, int64_t n, const uint8_t* active,
+                             float threshold, float* result3, void* cuda_stream);
+
 /* Backward of the most recent sgs_render on this ctx (same surfel buffers, unchanged).
  *   upstream : dL/d(rgb, depth, normal, alpha)                                     DEVICE
  *   d_surfels: nullable; NULL = pose-only mode (tracking, L204: splats frozen)     DEVICE

@@ -51,7 +51,7 @@ class sgs_stats(C.Structure):
 
 
 EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_backward", "sgs_tracking_loss",
-           "sgs_backward_tracking", "sgs_track_iter", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
+           "sgs_backward_tracking", "sgs_track_iter", "sgs_render_contrib", "sgs_covisibility", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
            "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string"]
 
 _lib = None
@@ -186,6 +186,18 @@ class Renderer:
         device tensors (any may be None)."""
         im = _images(rgb, depth, normal, alpha)
         _check(self.lib.sgs_render(self._ctx, C.byref(surfels), C.byref(cam), C.byref(im), _stream_ptr(stream)), "sgs_render")
+
+    def render_contrib(self, surfels, cam, contrib, rgb=None, depth=None, normal=None, alpha=None, stream=None):
+        """sgs_render_contrib: render + per-splat contribution C_k^V (Eq. 20-21) into `contrib` (n floats, device)."""
+        out = _images(rgb, depth, normal, alpha)
+        _check(self.lib.sgs_render_contrib(self._ctx, C.byref(surfels), C.byref(cam), C.byref(out), _ptr(contrib),
+                                           _stream_ptr(stream)), "sgs_render_contrib")
+
+    def covisibility(self, contrib_a, contrib_b, result3, active=None, threshold=0.5, stream=None):
+        """sgs_covisibility (Eq. 22): result3 <- (score, |intersection|, |union|)."""
+        _check(self.lib.sgs_covisibility(self._ctx, _ptr(contrib_a), _ptr(contrib_b), C.c_int64(contrib_a.numel()),
+                                         _ptr(active, torch.uint8), C.c_float(threshold), _ptr(result3),
+                                         _stream_ptr(stream)), "sgs_covisibility")
 
     def backward(self, d_rgb=None, d_depth=None, d_normal=None, d_alpha=None, grads=None, d_pose6=None, stream=None):
         """sgs_backward.  grads: dict of preallocated device tensors mean/scale/quat/opacity/rgb, or None

@@ -224,6 +224,7 @@ int sgs_destroy(sgs_ctx* c) {
     if (c->pinned_small) cudaFreeHost(c->pinned_small);
     if (c->sort_hist) cudaFree(c->sort_hist);
     if (c->loss_dev) cudaFree(c->loss_dev);
+    if (c->covis_cnt) cudaFree(c->covis_cnt);
     if (c->counters_ready) cudaEventDestroy(c->counters_ready);
     for (int i = 0; i < 2 * c->prof_cap; ++i) cudaEventDestroy(c->prof_ev[i]);
     free(c->prof_ev); free(c->prof_stage);

@@ -146,6 +146,24 @@ int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const s
     return SGS_OK;
 }
 
+int sgs_render_contrib(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* out, float* contrib,
+                       void* stream) {
+    if (!c || !sf || !contrib) return SGS_INVALID_ARGUMENT;
+    if (sf->n > 0 && cudaMemsetAsync(contrib, 0, sizeof(float) * (size_t)sf->n, (cudaStream_t)stream) != cudaSuccess)
+        return SGS_CUDA_ERROR;
+    c->contrib_out = contrib;
+    const int r = sgs_render(c, sf, cam, out, stream);
+    c->contrib_out = nullptr;
+    return r;
+}
+
+int sgs_covisibility(sgs_ctx* c, const float* ca, const float* cb, int64_t n, const uint8_t* active, float threshold,
+                     float* result3, void* stream) {
+    if (!c || !ca || !cb || !result3 || n < 0) return SGS_INVALID_ARGUMENT;
+    return sgs_launch_covisibility(c, ca, cb, n, active, threshold, result3, (cudaStream_t)stream) == cudaSuccess
+               ? SGS_OK : SGS_CUDA_ERROR;
+}
+
 int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* target, float lambda_d,
                    float normal_sign, const sgs_images* out, float* d_pose6, float* loss, void* stream) {
     if (!c || !target || !target->rgb || !target->depth || !d_pose6) return SGS_INVALID_ARGUMENT;

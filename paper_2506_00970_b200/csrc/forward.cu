@@ -13,10 +13,12 @@ namespace {
 
 struct Planes { float* p[8]; };
 
+template <bool CONTRIB>
 __global__ void __launch_bounds__(SGS_BLOCK)
 k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
           int tiles_x, SgsCfgDev cfg, Planes out, float* __restrict__ T_final, uint32_t* __restrict__ n_last,
-          const uint32_t* __restrict__ cursor, unsigned long long* bucket, uint32_t tile_cap) {
+          const uint32_t* __restrict__ cursor, unsigned long long* bucket, uint32_t tile_cap,
+          float* __restrict__ contrib) {
     // staged batch, structure of float4 arrays (one base register, immediate offsets, broadcast reads)
     __shared__ float4 sh[5][SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
@@ -87,7 +89,7 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
             stage_entry(g0, g1, g2, g3, px0, py0, s0, s1, s2);
             sh[0][tid] = s0; sh[1][tid] = s1; sh[2][tid] = s2;
             sh[3][tid] = make_float4(g1.w, g3.w, g4.x, g4.y);
-            sh[4][tid] = make_float4(g4.z, g4.w, g5.x, 0.f);
+            sh[4][tid] = make_float4(g4.z, g4.w, g5.x, __uint_as_float(v));
             mask = warp_patch_mask(g7, (float)(tx * SGS_TILE), (float)(ty * SGS_TILE));
         }
         sh_mask[tid] = (unsigned char)mask;
@@ -124,6 +126,12 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
                 Dp = __fmaf_rn(w, z, Dp);
                 N0 = __fmaf_rn(w, s4.x, N0); N1 = __fmaf_rn(w, s4.y, N1); N2 = __fmaf_rn(w, s4.z, N2);
                 O += w;
+                if (CONTRIB) {  // Eq. 20-21: C_k += sum over the warp's pixels of w_k(p); one atomic per (warp, entry)
+                    // w in [0, 1] as 24-bit fixed point: the warp sum is ONE redux.sync instead of five shuffle-adds
+                    // (quantisation 6e-8 per pixel, far below the 1e-4 bar); 32 x 2^24 fits 32 bits
+                    const unsigned ws = __reduce_add_sync(0xffffffffu, (unsigned)__float2uint_rn(w * 16777216.f));
+                    if (lane == 0 && ws != 0u) atomicAdd(contrib + __float_as_uint(s4.w), (float)ws * (1.f / 16777216.f));
+                }
                 T = pass ? Tn : T;
                 last = pass ? base - start + j + 1 : last;
             }
@@ -152,8 +160,11 @@ cudaError_t sgs_launch_forward(sgs_ctx* c, float* const planes[8], cudaStream_t 
     for (int i = 0; i < 8; ++i) out.p[i] = planes[i];
     SgsStage st(c, SGS_STAGE_FORWARD, s);
     c->launches += 1;
-    k_forward<<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, c->camd.W, c->camd.H, c->camd.tiles_x,
-                                          c->cfgd, out, c->T_final, c->n_last, c->fused_sort ? c->cursor : nullptr,
-                                          reinterpret_cast<unsigned long long*>(c->bucket), (uint32_t)c->tile_cap);
+#define SGS_FWD_ARGS c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, c->camd.W, \
+                     c->camd.H, c->camd.tiles_x, c->cfgd, out, c->T_final, c->n_last, c->fused_sort ? c->cursor : nullptr,     \
+                     reinterpret_cast<unsigned long long*>(c->bucket), (uint32_t)c->tile_cap, c->contrib_out
+    if (c->contrib_out) k_forward<true><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+    else k_forward<false><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+#undef SGS_FWD_ARGS
     return cudaGetLastError();
 }

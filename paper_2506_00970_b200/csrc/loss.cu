@@ -48,7 +48,59 @@ k_tracking_loss(LP p, const float* __restrict__ trgb, const float* __restrict__ 
     }
 }
 
+// Covisibility of two views (Eq. 22): counts of the intersection and the union of the visible
+// sets G_V = {k active : C_k^V > threshold}; the last block forms the score.  Integer counts: exact.
+__global__ void __launch_bounds__(256)
+k_covisibility(const float* __restrict__ ca, const float* __restrict__ cb, long long n, const uint8_t* __restrict__ active,
+               float thr, unsigned int* __restrict__ cnt /* inter, union, ticket */, float* __restrict__ result3) {
+    unsigned int inter = 0, uni = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const bool act = active == nullptr || active[i] != 0;
+        const bool a = act && ca[i] > thr, b = act && cb[i] > thr;
+        inter += (a && b) ? 1u : 0u;
+        uni += (a || b) ? 1u : 0u;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        inter += __shfl_xor_sync(0xffffffffu, inter, o);
+        uni += __shfl_xor_sync(0xffffffffu, uni, o);
+    }
+    __shared__ bool s_last;
+    if ((threadIdx.x & 31) == 0) {
+        if (inter) atomicAdd(&cnt[0], inter);
+        if (uni) atomicAdd(&cnt[1], uni);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        s_last = atomicAdd(&cnt[2], 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (s_last && threadIdx.x == 0) {
+        __threadfence();
+        const unsigned int it = atomicAdd(&cnt[0], 0u), un = atomicAdd(&cnt[1], 0u);
+        result3[0] = un ? (float)it / (float)un : 0.f;
+        result3[1] = (float)it;
+        result3[2] = (float)un;
+        cnt[0] = 0; cnt[1] = 0; cnt[2] = 0;  // self-cleaning
+    }
+}
+
 }  // namespace
+
+cudaError_t sgs_launch_covisibility(sgs_ctx* c, const float* ca, const float* cb, int64_t n, const uint8_t* active, float thr,
+                                    float* result3, cudaStream_t s) {
+    if (!c->covis_cnt) {
+        if (cudaMalloc(&c->covis_cnt, 4 * sizeof(unsigned int)) != cudaSuccess) return cudaErrorMemoryAllocation;
+        cudaMemset(c->covis_cnt, 0, 4 * sizeof(unsigned int));
+    }
+    int blocks = (int)((n + 255) / 256);
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks < 1) blocks = 1;
+    c->launches += 1;
+    k_covisibility<<<blocks, 256, 0, s>>>(ca, cb, (long long)n, active, thr, c->covis_cnt, result3);
+    return cudaGetLastError();
+}
 
 cudaError_t sgs_launch_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const float* const ren[8], const float* trgb,
                                      const float* tdepth, float lambda_d, float nsign, float* const up[8], float* loss,

@@ -86,6 +86,8 @@ struct sgs_ctx {
     uint32_t* tile_order;            // tiles: tile ids by descending entry count (longest first), written by K-pre-B
     uint32_t* render_order;          // tiles: longest-first order of the last sgs_render's tiles (by entry count), or unused
     bool render_order_valid;
+    unsigned int* covis_cnt;         // 4 counters of k_covisibility (cudaMalloc, lazily)
+    float* contrib_out;              // sgs_render_contrib: per-splat contribution output of the current forward, or NULL
     int64_t cursor_cap;              // tiles the cursor / tile_order arrays hold
     int64_t tile_cap, bucket_cap;    // entries per tile; allocated keys
     uint64_t* export_keys;           // contiguous (tile << 32 | depth) list for sgs_get_binning
@@ -152,6 +154,8 @@ int sgs_sort_passes(int tiles);
 cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cudaStream_t s);
 cudaError_t sgs_launch_tilesort(sgs_ctx* c, cudaStream_t s);
 cudaError_t sgs_launch_tile_order(sgs_ctx* c, cudaStream_t s);
+cudaError_t sgs_launch_covisibility(sgs_ctx* c, const float* ca, const float* cb, int64_t n, const uint8_t* active, float thr,
+                                    float* result3, cudaStream_t s);
 cudaError_t sgs_launch_export_bucket(sgs_ctx* c, int64_t n_entries, cudaStream_t s);
 int sgs_ensure_buckets(sgs_ctx* c, int tiles, int64_t tile_cap, cudaStream_t s);
 int sgs_ensure_export(sgs_ctx* c, int tiles, int64_t entries, cudaStream_t s);
