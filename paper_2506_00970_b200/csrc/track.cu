@@ -22,7 +22,8 @@ constexpr uint32_t TRK_PL = SGS_BLOCK * 16;  // bytes per staged plane
 constexpr int TRK_ORDER_BINS = 2048;         // tile costs (cycles >> 8) are binned 0..2047
 constexpr int TRK_K = 2;                     // entries per trip of the walks
 
-// One thread stages entry `v` of the tile: forward record (s0..s4) plus the backward's a_u, a_v, m = a_u x a_v.
+// One thread stages entry `v` of the tile: forward record (s0..s4; s4.w carries m.z) plus the backward's a_u, a_v and
+// m = a_u x a_v: 7 planes of float4.
 __device__ __forceinline__ unsigned stage_track(const SgsPayload& pay, uint32_t v, double px0, double py0, float tx0,
                                                 float ty0, float4 (*sh)[SGS_BLOCK], int tid) {
     const float4 g0 = pay.g0[v], g1 = pay.g1[v], g3 = pay.g3[v], g4 = pay.g4[v], g5 = pay.g5[v], g6 = pay.g6[v];
@@ -32,11 +33,10 @@ __device__ __forceinline__ unsigned stage_track(const SgsPayload& pay, uint32_t 
     stage_entry(g0, g1, g2, g3, px0, py0, s0, s1, s2);
     sh[0][tid] = s0; sh[1][tid] = s1; sh[2][tid] = s2;
     sh[3][tid] = make_float4(g1.w, g3.w, g4.x, g4.y);
-    sh[4][tid] = make_float4(g4.z, g4.w, g5.x, 0.f);
     const float aux = g5.y, auy = g5.z, auz = g5.w, avx = g6.x, avy = g6.y, avz = g6.z;
     sh[5][tid] = make_float4(aux, auy, auz, avx);
     sh[6][tid] = make_float4(avy, avz, auy * avz - auz * avy, auz * avx - aux * avz);
-    sh[7][tid] = make_float4(aux * avy - auy * avx, 0.f, 0.f, 0.f);
+    sh[4][tid] = make_float4(g4.z, g4.w, g5.x, aux * avy - auy * avx);  // n_c.y, n_c.z (with g4.w), ..., m.z
     return warp_patch_mask(g7, tx0, ty0);
 }
 
@@ -51,55 +51,6 @@ __device__ __forceinline__ float pair_rho2(const float4 s0, const float4 s1, con
     return __fmaf_rn(v, v, __fmul_rn(u, u));
 }
 
-// Eq. 8 for one pair that passed the cutoff somewhere in the warp (k_forward's sequence)
-__device__ __forceinline__ void fwd_composite(uint32_t ea, const float4 s2, float u, float v, float rho2, bool pass,
-                                              uint32_t last_if, const SgsCfgDev& cfg, float& T, bool& done, uint32_t& last,
-                                              float& C0, float& C1, float& C2, float& Dp, float& N0, float& N1, float& N2,
-                                              float& O) {
-    const float4 s3 = lds128(ea + 3 * TRK_PL), s4 = lds128(ea + 4 * TRK_PL);
-    const float z = __fmaf_rn(s2.z, v, __fmaf_rn(s2.y, u, s2.w));
-    const float G = fast_ex2(__fmul_rn(rho2, -0.72134752044448170368f));
-    const float a = fminf(cfg.alpha_max, __fmul_rn(s3.x, G));
-    pass = pass && (z > cfg.z_near) && (a >= cfg.alpha_min);
-    const float Tn = __fmul_rn(T, 1.f - a);
-    const bool stop = pass && (Tn < cfg.t_min);  // R6: stop, this splat is not composited
-    done = done || stop;
-    pass = pass && !stop;
-    const float w = pass ? __fmul_rn(a, T) : 0.f;
-    C0 = __fmaf_rn(w, s3.y, C0); C1 = __fmaf_rn(w, s3.z, C1); C2 = __fmaf_rn(w, s3.w, C2);
-    Dp = __fmaf_rn(w, z, Dp);
-    N0 = __fmaf_rn(w, s4.x, N0); N1 = __fmaf_rn(w, s4.y, N1); N2 = __fmaf_rn(w, s4.z, N2);
-    O += w;
-    T = pass ? Tn : T;
-    last = pass ? last_if : last;
-}
-
-// Backward of one composited pair, pose-only, tracking loss (g_normal = g_alpha = 0): k_backward's sequence.
-__device__ __forceinline__ void bwd_pair(uint32_t ea, const float4 s3, const PairResult& r, float g0, float g1, float g2,
-                                         float g3, float rx, float ry, float alpha_max, float& T_after, float& suffix,
-                                         float& F0, float& F1, float& F2, float& Z0, float& Z1, float& Z2) {
-    const float4 s5 = lds128(ea + 5 * TRK_PL), s6 = lds128(ea + 6 * TRK_PL), s7 = lds128(ea + 7 * TRK_PL);
-    const float inv1ma = fast_rcp(1.f - r.a);
-    const float Ti = T_after * inv1ma;  // transmittance in front of this splat
-    const float w = r.a * Ti;
-    const float gv = g0 * s3.y + g1 * s3.z + g2 * s3.w + g3 * r.z;
-    const float da = Ti * gv - suffix * inv1ma;
-    suffix = fmaf(w, gv, suffix);
-    T_after = Ti;
-    const bool clamped = s3.x * r.G > alpha_max;  // R5: true derivative, zero when clamped
-    const float dG = clamped ? 0.f : da * s3.x;
-    const float gu = -r.u * r.G * dG, gvv = -r.v * r.G * dG, gz = g3 * w;
-    // f = [ r x (a_v gu - a_u gv) + m gz ] / (r . m)
-    const float q0 = s5.w * gu - s5.x * gvv, q1 = s6.x * gu - s5.y * gvv, q2 = s6.y * gu - s5.z * gvv;
-    const float m0 = s6.z, m1 = s6.w, m2 = s7.x;
-    const float inv_rm = fast_rcp(rx * m0 + ry * m1 + m2);
-    const float f0 = (ry * q2 - q1 + m0 * gz) * inv_rm;
-    const float f1 = (q0 - rx * q2 + m1 * gz) * inv_rm;
-    const float f2 = (rx * q1 - ry * q0 + m2 * gz) * inv_rm;
-    F0 += f0; F1 += f1; F2 += f2;
-    Z0 = fmaf(r.z, f0, Z0); Z1 = fmaf(r.z, f1, Z1); Z2 = fmaf(r.z, f2, Z2);
-}
-
 template <bool WRITE_IMAGES>
 __global__ void __launch_bounds__(SGS_BLOCK, 3)
 k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* __restrict__ cursor, unsigned long long* bucket, uint32_t tile_cap,
@@ -108,7 +59,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* __r
         float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
         float* __restrict__ loss_out, uint32_t* __restrict__ tile_cost) {
     const long long t_start = clock64();
-    __shared__ float4 sh[8][SGS_BLOCK];
+    __shared__ float4 sh[7][SGS_BLOCK];
     __shared__ unsigned long long s_keys[SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
     __shared__ float s_red[8][7];
@@ -267,7 +218,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* __r
 #pragma unroll
                 for (int k = 0; k < TRK_K; ++k) {  // the geometric chain, predicated per lane (no divergent branches)
                     const float4 s5 = lds128(ea[k] + 5 * TRK_PL), s6 = lds128(ea[k] + 6 * TRK_PL);
-                    const float m2 = lds32(ea[k] + 7 * TRK_PL);
+                    const float m2 = lds32(ea[k] + 4 * TRK_PL + 12);
                     const bool clamped = opac[k] * r[k].G > cfg.alpha_max;  // R5: true derivative, zero when clamped
                     const float dG = clamped ? 0.f : da[k] * opac[k];
                     const float gu = -r[k].u * r[k].G * dG, gvv = -r[k].v * r[k].G * dG, gz = g3 * w[k];
