@@ -251,13 +251,12 @@ k_preprocess(int64_t n, const float* __restrict__ mean, const float* __restrict_
 //            the block in shared memory and appends them to a global list with ONE atomic per block.
 //   K-pre-B  dense: one thread per survivor runs the binary64 sequence, writes the payload, and the
 //            block's tile entries are spread over its threads (one (surfel, tile) pair each).
-constexpr int SGS_PREA_ITEMS = 4;
-constexpr int SGS_PREA_SPAN = SGS_PREA_ITEMS * SGS_PRE_BLOCK;
-
+template <int SGS_PREA_ITEMS>
 __global__ void __launch_bounds__(SGS_PRE_BLOCK)
 k_pre_select(int64_t n, const float* __restrict__ mean, const float* __restrict__ scale,
              const uint8_t* __restrict__ active, SgsCamDev cam, SgsCfgDev cfg, uint8_t* __restrict__ culled,
              SgsCounters* __restrict__ counters, uint32_t* __restrict__ surv_list) {
+    constexpr int SGS_PREA_SPAN = SGS_PREA_ITEMS * SGS_PRE_BLOCK;
     __shared__ unsigned short s_list[SGS_PREA_SPAN];
     __shared__ unsigned int s_n, s_base;
     const int tid = threadIdx.x, lane = tid & 31;
@@ -433,11 +432,19 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     e = cudaMemsetAsync(c->cursor, 0, sizeof(uint32_t) * (size_t)tiles, s);
     if (e != cudaSuccess) return e;
     SgsStage st(c, SGS_STAGE_PREPROCESS, s);
-    const int blocks_a = (int)((n + SGS_PREA_SPAN - 1) / SGS_PREA_SPAN);
+    // K-pre-A: 4 surfels per thread once that still gives every SM several blocks (large maps), else 1
+    const bool wide = (n + 1023) / 1024 >= 4 * 148;
+    const int span = wide ? 1024 : 256;
+    const int blocks_a = (int)((n + span - 1) / span);
     c->launches += blocks_a > 0 ? 2 : 1;
-    if (blocks_a > 0)
-        k_pre_select<<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, c->camd, c->cfgd, c->culled,
-                                                        c->counters, c->vis_to_surfel);
+    if (blocks_a > 0) {
+        if (wide)
+            k_pre_select<4><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, c->camd, c->cfgd, c->culled,
+                                                               c->counters, c->vis_to_surfel);
+        else
+            k_pre_select<1><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, c->camd, c->cfgd, c->culled,
+                                                               c->counters, c->vis_to_surfel);
+    }
     // K-pre-B walks the survivor list with a grid-stride loop: the count is only known on the device
     // (the grid follows the last known survivor count)
     int64_t blocks_b = (n + SGS_PREB_BLOCK - 1) / SGS_PREB_BLOCK;
