@@ -436,3 +436,47 @@ def test_p11_covisibility_hand_example():
     act = np.array([1, 0, 1, 1, 1], np.uint8)                       # only splats of the active map count (L216)
     assert oracle.covisibility(CA, CB, active=act) == (1 / 3, 1, 3)
     assert oracle.covisibility(np.zeros(3), np.zeros(3)) == (0.0, 0, 0)
+
+
+# ---------------------------------------------------------------- P12: tracking loss harness (Eq. 15-19)
+def test_p12_tracking_loss_hand_example_masks_and_gradient():
+    """Eq. 15-19 on a 2x2 frame evaluated by hand: pixel (0,0) passes both masks, (1,0) fails M_o (alpha 0.9),
+    (0,1) fails M_n (normal faces away), (1,1) passes.  L_t = (1/4) sum M_n M_o (|dI|_1 + lambda_d |dD|)."""
+    cam = Camera(2, 2, 1.0, 1.0, 1.0, 1.0)
+    camv = oracle.make_cam(cam)
+    img = np.zeros((8, 2, 2))
+    img[0:3] = [[[0.5, 0.2], [0.3, 0.9]], [[0.1, 0.2], [0.3, 0.4]], [[0.0, 0.2], [0.3, 0.6]]]
+    img[3] = [[2.0, 1.0], [1.5, 3.0]]
+    img[6] = [[1.0, 1.0], [-1.0, 1.0]]                  # N_r = (0, 0, +-1): N.r = +-1 for every ray (r_z = 1)
+    img[7] = [[0.99, 0.9], [0.99, 0.96]]
+    trgb = np.zeros((3, 2, 2)); trgb[:, 0, 0] = [0.4, 0.3, 0.0]; trgb[:, 1, 1] = [1.0, 0.1, 0.6]
+    tdep = np.array([[2.5, 0.0], [0.0, 2.0]])
+    L, up = oracle.tracking_loss(img, trgb, tdep, camv, 0.5, 1.0)
+    # (0,0): |0.1| + |-0.2| + 0 + 0.5 |-0.5| = 0.55 ; (1,1): |-0.1| + |0.3| + 0 + 0.5 |1.0| = 0.9
+    assert abs(L - (0.55 + 0.9) / 4) < 1e-15
+    assert (up[:, 0, 1] == 0).all() and (up[:, 1, 0] == 0).all() and (up[4:] == 0).all()
+    np.testing.assert_allclose(up[0:4, 0, 0], np.array([1, -1, 0, -0.5]) / 4)
+    np.testing.assert_allclose(up[0:4, 1, 1], np.array([-1, 1, 0, 0.5]) / 4)
+    # the other sign convention (R19) swaps which pixels pass M_n
+    L2, _ = oracle.tracking_loss(img, trgb, tdep, camv, 0.5, -1.0)
+    assert abs(L2 - (0.3 + 0.3 + 0.3 + 0.5 * 1.5) / 4) < 1e-15     # only (0,1): rgb 0.3 each, depth 1.5
+
+
+def test_p12_tracking_loss_gradient_is_its_finite_difference(c1):
+    """`up` is dL_t/d(image) wherever L_t is differentiable (central differences on the C1 render)."""
+    sc, cam, camv, cfg, r = c1
+    img = r["img"].copy()
+    img[7] = np.where(img[7] > 0.5, 0.97, img[7])       # let a good share of pixels pass M_o = [O > 0.95]
+    g = scenegen.SplitMix(5)
+    trgb = img[0:3] + 0.05 * g.normal(img[0:3].size).reshape(img[0:3].shape)
+    tdep = img[3] + 0.1 * g.normal(img[3].size).reshape(img[3].shape)
+    for nsign in (1.0, -1.0):
+        L, up = oracle.tracking_loss(img, trgb, tdep, camv, 0.5, nsign)
+        nz = np.argwhere(up != 0)
+        assert len(nz) > 50
+        for ch, j, i in nz[:: max(1, len(nz) // 40)]:
+            d = np.zeros_like(img); d[ch, j, i] = 1e-6
+            fd = (oracle.tracking_loss(img + d, trgb, tdep, camv, 0.5, nsign)[0] -
+                  oracle.tracking_loss(img - d, trgb, tdep, camv, 0.5, nsign)[0]) / 2e-6
+            assert abs(fd - up[ch, j, i]) <= 1e-6 * abs(up[ch, j, i]) + 1e-12
+    assert oracle.tracking_loss(img, img[0:3], img[3], camv, 0.5, 1.0)[0] == 0.0
