@@ -279,9 +279,12 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
     __shared__ float s_red[8][6];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     // compacted mode: v < N_v, surfel = vis_to_surfel[v]; bucket mode (no compaction): v = surfel index
-    const unsigned int v = blockIdx.x * blockDim.x + tid;
+    // grid-stride over the surfels: a bounded grid keeps the per-block ticket of the pose reduction off the
+    // critical path (one same-address atomic per block)
     float p6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    const bool live = vis_to_surfel ? (v < counters->n_visible) : (v < n_all && culled[v] == 0);
+    const unsigned int n_loop = vis_to_surfel ? counters->n_visible : n_all;
+    for (unsigned int v = blockIdx.x * blockDim.x + tid; v < n_loop; v += gridDim.x * blockDim.x) {
+    const bool live = vis_to_surfel ? true : (culled[v] == 0);
     if (live) {
         const uint32_t i = vis_to_surfel ? vis_to_surfel[v] : v;
         float a[16];
@@ -324,12 +327,12 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
         if (out.opacity) out.opacity[i] = a[15];
         if (out.rgb) { out.rgb[3 * i] = a[12]; out.rgb[3 * i + 1] = a[13]; out.rgb[3 * i + 2] = a[14]; }
         // pose share: rho += dmu; theta += mu_c x dmu + t_uc x dtu + t_vc x dtv + t_nc x dtn   (Eq. 13)
-        p6[0] = dmu[0]; p6[1] = dmu[1]; p6[2] = dmu[2];
-        p6[3] = (muc[1] * dmu[2] - muc[2] * dmu[1]) + (tuc[1] * dtu[2] - tuc[2] * dtu[1]) +
+        p6[0] += dmu[0]; p6[1] += dmu[1]; p6[2] += dmu[2];
+        p6[3] += (muc[1] * dmu[2] - muc[2] * dmu[1]) + (tuc[1] * dtu[2] - tuc[2] * dtu[1]) +
                 (tvc[1] * dtv[2] - tvc[2] * dtv[1]) + (tnc[1] * dtn[2] - tnc[2] * dtn[1]);
-        p6[4] = (muc[2] * dmu[0] - muc[0] * dmu[2]) + (tuc[2] * dtu[0] - tuc[0] * dtu[2]) +
+        p6[4] += (muc[2] * dmu[0] - muc[0] * dmu[2]) + (tuc[2] * dtu[0] - tuc[0] * dtu[2]) +
                 (tvc[2] * dtv[0] - tvc[0] * dtv[2]) + (tnc[2] * dtn[0] - tnc[0] * dtn[2]);
-        p6[5] = (muc[0] * dmu[1] - muc[1] * dmu[0]) + (tuc[0] * dtu[1] - tuc[1] * dtu[0]) +
+        p6[5] += (muc[0] * dmu[1] - muc[1] * dmu[0]) + (tuc[0] * dtu[1] - tuc[1] * dtu[0]) +
                 (tvc[0] * dtv[1] - tvc[1] * dtv[0]) + (tnc[0] * dtn[1] - tnc[1] * dtn[0]);
         // world space: x_c = R_cw x_w  =>  dL/dx_w = R_cw^T dL/dx_c
         float G[3][3];  // dL/dR (world), columns t_u, t_v, t_n
@@ -357,7 +360,7 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
             out.quat[4 * i + 3] = (dq[3] - qz * qd) * qi;
         }
     }
-    else if (zero_rest && v < n_all) {
+    else if (zero_rest) {
         // inactive / culled surfel: gradients are exactly zero (bucket mode: v IS the surfel index, so the
         // caller's buffers are overwritten here instead of by five memsets)
         if (out.mean) { out.mean[3 * v] = 0.f; out.mean[3 * v + 1] = 0.f; out.mean[3 * v + 2] = 0.f; }
@@ -365,6 +368,7 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
         if (out.quat) reinterpret_cast<float4*>(out.quat)[v] = make_float4(0.f, 0.f, 0.f, 0.f);
         if (out.opacity) out.opacity[v] = 0.f;
         if (out.rgb) { out.rgb[3 * v] = 0.f; out.rgb[3 * v + 1] = 0.f; out.rgb[3 * v + 2] = 0.f; }
+    }
     }
     if (d_pose6 == nullptr) return;
 #pragma unroll
@@ -416,7 +420,8 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     k_backward<false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                   cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
                                                   c->acc, c->pose_partial, c->counters, nullptr, FusedLoss{});
-    const int blocks = (int)((n + 255) / 256);  // bound on N_v; blocks past it only join the pose reduction
+    int blocks = (int)((n + 255) / 256);  // bound on N_v
+    if (blocks > 148 * 8) blocks = 148 * 8;
     if (blocks == 0 && d_pose6) return cudaMemsetAsync(d_pose6, 0, sizeof(float) * 6, s);
     if (blocks > 0)
         c->launches += 1, k_surfel_backward<<<blocks, 256, 0, s>>>(c->counters, c->list_stride == 2 ? nullptr : c->vis_to_surfel, c->culled,
