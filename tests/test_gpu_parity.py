@@ -329,3 +329,29 @@ def test_track_iter_matches_unfused_sequence():
             ren.backward(d_pose6=p6a)
         assert e.value.status == sgs.SGS_NO_FORWARD_STATE
         ren.close()
+
+
+def test_random_poses_binning_and_images(ren):
+    """Eight seeded random camera poses inside a 30 k-surfel room (looking at every wall, rolled, close to
+    surfaces): binning bit-exact and images within the bar at each -- guards the conservative binary32 pre-cull
+    and the two-kernel preprocess against view-dependent mistakes."""
+    sc, _, _ = scenegen.make_config("C2", n_override=30000)
+    g = scenegen.SplitMix(4242)
+    cfg = oracle.make_cfg()
+    t, sf = to_device(sc)
+    for k in range(8):
+        eye = np.array([g.uniform(1, 0.3, 4.7)[0], g.uniform(1, 0.3, 3.7)[0], g.uniform(1, 0.3, 2.7)[0]])
+        tgt = np.array([g.uniform(1, -1.0, 6.0)[0], g.uniform(1, -1.0, 5.0)[0], g.uniform(1, -1.0, 4.0)[0]])
+        T = scenegen.look_at(eye, tgt).astype(np.float64)
+        roll = scenegen.se3_exp(np.array([0, 0, 0, 0, 0, g.uniform(1, -np.pi, np.pi)[0]]))[:3, :3]
+        T = np.concatenate([roll @ T[:, :3], (roll @ T[:, 3])[:, None]], axis=1)
+        cam = Camera(200 + 16 * k + (k % 3), 150 + 7 * k, 180.0 + 10 * k, 175.0 + 9 * k, 100.0 + 3 * k, 75.0 - 2 * k,
+                     T.astype(np.float32))
+        camv = oracle.make_cam(cam)
+        im = alloc_images(cam)
+        ren.render(sf, camera(cam), **im)
+        tiles = ((cam.width + 15) // 16) * ((cam.height + 15) // 16)
+        ob = oracle.binning(sc, camv, cfg)
+        assert ob["E"] > 1000
+        assert_binning(ren.get_binning(sc.n, tiles), ob)
+        assert_images(planes(im), oracle.render(sc, camv, cfg))
