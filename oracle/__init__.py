@@ -190,3 +190,68 @@ def tracking_loss(img, target_rgb, target_depth, camv, lambda_d, normal_sign=1.0
     up[0:3] = m * np.sign(dI) / (W * H)
     up[3] = m * lambda_d * np.sign(dD) / (W * H)
     return float(L), up
+
+
+def normal_from_depth(depth, camv):
+    """Eq. 23 (L226-228): N_D = (grad_x D x grad_y D) / |.|, "the cross product of neighbouring pixel differences in
+    D" -- reading R23: the differences are those of the back-projected points
+    P(x,y) = D(x,y) ((x+0.5-cx)/fx, (y+0.5-cy)/fy, 1), central: grad_x P = P(x+1,y) - P(x-1,y), grad_y P = P(x,y+1) -
+    P(x,y-1).  Defined on interior pixels with a non-zero cross product; N_D = 0 elsewhere.  Returns (3,H,W) fp64."""
+    D = np.asarray(depth, dtype=np.float64)
+    W, H = int(camv[0]), int(camv[1])
+    fx, fy, cx, cy = camv[2:6]
+    X, Y = np.meshgrid(np.arange(W) + 0.5, np.arange(H) + 0.5)
+    P = np.stack([D * (X - cx) / fx, D * (Y - cy) / fy, D], 0)
+    N = np.zeros((3, H, W))
+    a = P[:, 1:-1, 2:] - P[:, 1:-1, :-2]
+    b = P[:, 2:, 1:-1] - P[:, :-2, 1:-1]
+    c = np.cross(a, b, axis=0)
+    nrm = np.sqrt((c * c).sum(0))
+    ok = nrm > 0
+    N[:, 1:-1, 1:-1] = np.where(ok, c / np.where(ok, nrm, 1.0), 0.0)
+    return N
+
+
+def mapping_loss(img, target_rgb, target_depth, camv, lambda_c, w_d, w_n, normal_sign=1.0):
+    """Mapping loss of Eq. 24-26 (L232-248) WITHOUT the SSIM term (stated in DESIGN.md):
+        L = 1/|Omega| sum_p [ lambda_c |I_r - I|_1 + w_d |D_r - D| + w_n (1 - sign N_{D_r} . N_r) ]
+    with N_{D_r} = normal_from_depth(D_r) (Eq. 23, 25).  Returns (L, upstream (8,H,W)): dL/d(rgb, depth, normal, alpha)
+    of the rendered planes, the depth gradient including the chain through N_{D_r}."""
+    img = np.asarray(img, dtype=np.float64)
+    W, H = int(camv[0]), int(camv[1])
+    fx, fy, cx, cy = camv[2:6]
+    HW = W * H
+    dI = img[0:3] - np.asarray(target_rgb, dtype=np.float64)
+    dD = img[3] - np.asarray(target_depth, dtype=np.float64)
+    ND = normal_from_depth(img[3], camv)
+    Nr = img[4:7]
+    Ln = 1.0 - normal_sign * (ND * Nr).sum(0)
+    L = (lambda_c * np.abs(dI).sum(0) + w_d * np.abs(dD) + w_n * Ln).sum() / HW
+    up = np.zeros_like(img)
+    up[0:3] = lambda_c * np.sign(dI) / HW
+    up[3] = w_d * np.sign(dD) / HW
+    up[4:7] = -normal_sign * w_n * ND / HW
+    # chain through N_D: f = N.m with N = c/|c|, c = a x b  =>  df/dc = (m - N (N.m))/|c|, df/da = b x df/dc,
+    # df/db = df/dc x a; a, b are differences of P = D ray, so each interior pixel scatters to its four neighbours
+    X, Y = np.meshgrid(np.arange(W) + 0.5, np.arange(H) + 0.5)
+    ray = np.stack([(X - cx) / fx, (Y - cy) / fy, np.ones_like(X)], 0)
+    P = img[3][None] * ray
+    a = P[:, 1:-1, 2:] - P[:, 1:-1, :-2]
+    b = P[:, 2:, 1:-1] - P[:, :-2, 1:-1]
+    c = np.cross(a, b, axis=0)
+    nrm = np.sqrt((c * c).sum(0))
+    ok = nrm > 0
+    inv = np.where(ok, 1.0 / np.where(ok, nrm, 1.0), 0.0)
+    Nc = c * inv
+    m = Nr[:, 1:-1, 1:-1]
+    q = (m - Nc * (Nc * m).sum(0)) * inv
+    coef = -normal_sign * w_n / HW
+    dfa = np.cross(b, q, axis=0) * coef
+    dfb = np.cross(q, a, axis=0) * coef
+    gP = np.zeros((3, H, W))
+    gP[:, 1:-1, 2:] += dfa
+    gP[:, 1:-1, :-2] -= dfa
+    gP[:, 2:, 1:-1] += dfb
+    gP[:, :-2, 1:-1] -= dfb
+    up[3] += (gP * ray).sum(0)
+    return float(L), up

@@ -480,3 +480,56 @@ def test_p12_tracking_loss_gradient_is_its_finite_difference(c1):
                   oracle.tracking_loss(img - d, trgb, tdep, camv, 0.5, nsign)[0]) / 2e-6
             assert abs(fd - up[ch, j, i]) <= 1e-6 * abs(up[ch, j, i]) + 1e-12
     assert oracle.tracking_loss(img, img[0:3], img[3], camv, 0.5, 1.0)[0] == 0.0
+
+
+# ---------------------------------------------------------------- P13: normal from depth and the mapping loss (Eq. 23-26)
+def _plane_depth(cam, n, d):
+    """Depth image of the plane n.X = d seen by `cam` (closed form: z = d / (n . ray))."""
+    X, Y = pix_grid(cam)
+    ray = np.stack([(X - cam.cx) / cam.fx, (Y - cam.cy) / cam.fy, np.ones_like(X)], 0)
+    return d / (n[:, None, None] * ray).sum(0), ray
+
+
+def test_p13_normal_from_depth_of_a_plane_is_the_plane_normal():
+    """Differences of points of a plane lie in the plane: Eq. 23 returns the plane's unit normal exactly (interior)."""
+    cam = Camera(40, 30, 50.0, 45.0, 19.0, 16.0)
+    camv = oracle.make_cam(cam)
+    for n in ([0.0, 0.0, 1.0], [0.3, -0.2, 0.9], [-0.5, 0.4, 0.6]):
+        n = np.array(n) / np.linalg.norm(n)
+        D, _ = _plane_depth(cam, n, 2.0)
+        assert (D > 0).all()
+        N = oracle.normal_from_depth(D, camv)
+        np.testing.assert_allclose(N[:, 1:-1, 1:-1], np.broadcast_to(n[:, None, None], (3, 28, 38)), atol=1e-10)
+        assert (N[:, 0] == 0).all() and (N[:, :, -1] == 0).all()      # border: undefined -> 0
+
+
+def test_p13_mapping_loss_values_and_gradient():
+    """Eq. 24-26 (no SSIM): exact values on a plane (L_n = 0 where N_r = N_D, 2 where N_r = -N_D), and `up` equals
+    central finite differences of L on a bumpy depth image."""
+    cam = Camera(24, 18, 30.0, 28.0, 12.5, 8.0)
+    camv = oracle.make_cam(cam)
+    n = np.array([0.2, -0.3, 0.93]); n /= np.linalg.norm(n)
+    D, _ = _plane_depth(cam, n, 1.7)
+    img = np.zeros((8, 18, 24)); img[3] = D; img[4:7] = n[:, None, None]
+    HW = 24 * 18
+    L, _ = oracle.mapping_loss(img, img[0:3], D, camv, 0.875, 0.5, 0.02, 1.0)
+    border = HW - 22 * 16
+    assert abs(L - 0.02 * border / HW) < 1e-12                       # interior consistent; the border keeps L_n = 1
+    L, _ = oracle.mapping_loss(img, img[0:3], D, camv, 0.875, 0.5, 0.02, -1.0)
+    assert abs(L - 0.02 * (border + 2 * 22 * 16) / HW) < 1e-12
+    L, _ = oracle.mapping_loss(img, img[0:3] + 0.1, D - 0.25, camv, 0.875, 0.5, 0.0)
+    assert abs(L - (0.875 * 0.3 + 0.5 * 0.25)) < 1e-12
+    # gradient check on a generic image
+    g = scenegen.SplitMix(9)
+    img[3] = D + 0.05 * g.normal(HW).reshape(18, 24)
+    img[4:7] = g.normal(3 * HW).reshape(3, 18, 24)
+    img[0:3] = g.uniform(3 * HW).reshape(3, 18, 24)
+    trgb, tdep = g.uniform(3 * HW).reshape(3, 18, 24), D
+    args = (trgb, tdep, camv, 0.875, 0.5, 0.3, -1.0)
+    L, up = oracle.mapping_loss(img, *args)
+    assert (up[7] == 0).all()
+    for ch, j, i in [(3, 5, 7), (3, 1, 1), (3, 0, 4), (3, 9, 23), (3, 16, 12), (4, 6, 6), (5, 3, 20), (6, 10, 2), (0, 2, 2),
+                     (2, 17, 23), (3, 8, 11), (3, 2, 21)]:
+        d = np.zeros_like(img); d[ch, j, i] = 1e-6
+        fd = (oracle.mapping_loss(img + d, *args)[0] - oracle.mapping_loss(img - d, *args)[0]) / 2e-6
+        assert abs(fd - up[ch, j, i]) <= 2e-6 * abs(up[ch, j, i]) + 1e-11, (ch, j, i, fd, up[ch, j, i])
