@@ -182,7 +182,8 @@ class Workload:
             self.ren.render_contrib(self.sf, cam, self.contrib_buf, **self.im)
         else:
             self.ren.render(self.sf, cam, **self.im)
-        self.ren.tracking_loss(cam, self.im, trgb, tdep, 0.5, -1.0, self.up, self.loss)
+        # mapping iteration: Eq. 24-26 (lambda_c, w_d, w_n of Tab. I; SSIM term not built) -> upstream of all planes
+        self.ren.mapping_loss(cam, self.im, trgb, tdep, 0.875, 0.5, 0.02, -1.0, self.up, self.loss)
         u = self.up
         if True:
             self.ren.backward(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"],
@@ -418,7 +419,7 @@ def main():
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
                 surfels_per_s=wl.n_active * renders / (ms_max * 1e-3),
                 config=dict(workload=f"{args.config} ({'tracking' if wl.tracking else 'mapping'}-shaped): "
-                            f"{wl.renders_per_step} x (render + Eq.15-19 loss + "
+                            f"{wl.renders_per_step} x (render + {'Eq.15-19' if wl.tracking else 'Eq.24-26 (no SSIM)'} loss + "
                             f"{'pose-only' if wl.tracking else 'full+pose'} backward) per step",
                             surfels=wl.sc.n, active=wl.n_active, width=wl.W, height=wl.H, renders_per_step=wl.renders_per_step,
                             l2="flushed between steps by a 256 MiB write; iterations inside a step reuse the map as tracking does",

@@ -169,6 +169,17 @@ SGS_API int sgs_backward(sgs_ctx* ctx, const sgs_images* upstream, const sgs_sur
 SGS_API int sgs_tracking_loss(sgs_ctx* ctx, const sgs_camera* cam, const sgs_images* rendered, const sgs_images* target,
                       float lambda_d, float normal_sign, const sgs_images* upstream, float* loss, void* cuda_stream);
 
+/* Mapping loss of Eq. 24-26 (L232-248) WITHOUT its SSIM term (out of this round's scope), harness around
+ * the renderer for the mapping-shaped configs:
+ *   L = 1/|Omega| sum_p [ lambda_c |I_r - I|_1 + w_d |D_r - D| + w_n (1 - normal_sign N_{D_r} . N_r) ]
+ * N_{D_r}: unit cross product of the central differences of the points back-projected from the RENDERED depth
+ * (Eq. 23, 25; reading R23), interior pixels only.  Writes dL/d(rgb, depth, normal, alpha) of the rendered images
+ * into `upstream` (the depth gradient includes the chain through N_{D_r}; alpha gets 0) and L into loss
+ * (DEVICE, 1 float).  rendered / target / upstream: DEVICE; target uses rgb and depth. */
+SGS_API int sgs_mapping_loss(sgs_ctx* ctx, const sgs_camera* cam, const sgs_images* rendered, const sgs_images* target,
+                             float lambda_c, float w_d, float w_n, float normal_sign, const sgs_images* upstream,
+                             float* loss, void* cuda_stream);
+
 /* Tracking iteration backward (L180-204): the Eq. 15-19 loss of sgs_tracking_loss evaluated INSIDE the
  * pose-only backward on the images of the most recent sgs_render (whose output buffers must still hold
  * them), so neither the upstream gradients nor a loss kernel touch HBM.  target: DEVICE rgb + depth.

@@ -51,7 +51,7 @@ class sgs_stats(C.Structure):
 
 
 EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_backward", "sgs_tracking_loss",
-           "sgs_backward_tracking", "sgs_track_iter", "sgs_render_contrib", "sgs_covisibility", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
+           "sgs_backward_tracking", "sgs_track_iter", "sgs_render_contrib", "sgs_covisibility", "sgs_mapping_loss", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
            "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string"]
 
 _lib = None
@@ -219,6 +219,15 @@ class Renderer:
         _check(self.lib.sgs_tracking_loss(self._ctx, C.byref(cam), C.byref(r), C.byref(t), C.c_float(lambda_d),
                                           C.c_float(normal_sign), C.byref(u), _ptr(loss), _stream_ptr(stream)),
                "sgs_tracking_loss")
+
+    def mapping_loss(self, cam, ren, target_rgb, target_depth, lambda_c, w_d, w_n, normal_sign, up, loss, stream=None):
+        """sgs_mapping_loss (Eq. 24-26 without SSIM).  ren/up: dicts with rgb, depth, normal, alpha device tensors."""
+        r = _images(ren["rgb"], ren["depth"], ren["normal"], ren["alpha"])
+        t = _images(rgb=target_rgb, depth=target_depth)
+        u = _images(up["rgb"], up["depth"], up["normal"], up["alpha"])
+        _check(self.lib.sgs_mapping_loss(self._ctx, C.byref(cam), C.byref(r), C.byref(t), C.c_float(lambda_c), C.c_float(w_d),
+                                         C.c_float(w_n), C.c_float(normal_sign), C.byref(u), _ptr(loss), _stream_ptr(stream)),
+               "sgs_mapping_loss")
 
     def backward_tracking(self, target_rgb, target_depth, lambda_d, normal_sign, d_pose6, loss=None, stream=None):
         """sgs_backward_tracking: pose-only backward with the Eq. 15-19 loss fused in."""

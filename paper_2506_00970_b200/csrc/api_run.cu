@@ -243,6 +243,24 @@ int sgs_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const sgs_images* ren, 
     return SGS_OK;
 }
 
+int sgs_mapping_loss(sgs_ctx* c, const sgs_camera* cam, const sgs_images* ren, const sgs_images* target, float lambda_c,
+                     float w_d, float w_n, float normal_sign, const sgs_images* upstream, float* loss, void* stream) {
+    if (!c || !sgs_cam_valid(cam) || !ren || !target || !upstream) return SGS_INVALID_ARGUMENT;
+    if (!ren->rgb || !ren->depth || !ren->normal || !target->rgb || !target->depth) return SGS_INVALID_ARGUMENT;
+    const int64_t pixels = (int64_t)cam->width * cam->height;
+    const float* rp[8];
+    float* upp[8];
+    for (int i = 0; i < 3; ++i) {
+        rp[i] = ren->rgb + (size_t)i * pixels;
+        rp[4 + i] = ren->normal + (size_t)i * pixels;
+        upp[i] = upstream->rgb ? upstream->rgb + (size_t)i * pixels : nullptr;
+        upp[4 + i] = upstream->normal ? upstream->normal + (size_t)i * pixels : nullptr;
+    }
+    rp[3] = ren->depth; rp[7] = ren->alpha; upp[3] = upstream->depth; upp[7] = upstream->alpha;
+    return sgs_launch_mapping_loss(c, cam, rp, target->rgb, target->depth, lambda_c, w_d, w_n, normal_sign, upp, loss,
+                                   (cudaStream_t)stream) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
+}
+
 int sgs_get_binning(sgs_ctx* c, int64_t* n_entries, const uint64_t** keys, const uint32_t** idx,
                     const uint32_t** tile_ranges, const uint8_t** culled) {
     if (!c) return SGS_INVALID_ARGUMENT;

@@ -48,6 +48,108 @@ k_tracking_loss(LP p, const float* __restrict__ trgb, const float* __restrict__ 
     }
 }
 
+// ---- mapping loss of PAPER.md Eq. 24-26 (L232-248) without the SSIM term, and Eq. 23's normal from depth ----
+//   L = 1/|Omega| sum_p [ lambda_c |I_r - I|_1 + w_d |D_r - D| + w_n (1 - sign N_{D_r} . N_r) ]
+// N_D (Eq. 23, reading R23): unit cross product of the central differences of the back-projected points
+// P = D ray; interior pixels only (0 elsewhere).  One thread per pixel; the depth gradient through N_D is taken
+// in GATHER form: pixel X receives  ray(X) . [ A(X - e_x) - A(X + e_x) + B(X - e_y) - B(X + e_y) ]  with
+// A(p) = b_p x q_p, B(p) = q_p x a_p, q_p = (m - N (N.m)) / |a_p x b_p|  (the oracle scatters the same terms).
+struct MapImg { const float* ren[8]; float* up[8]; const float* depth; int W, H; float ifx, ify, cx, cy; };
+
+// normal chain at stencil position p from the four back-projected neighbours of p (l, r, u, d) and p's rendered
+// normal m: N = a x b / |a x b| with a = r - l, b = d - u;  A = b x q, B = q x a, q = (m - N (N.m)) / |a x b|.
+// `ok` = p is an interior pixel.  Outputs are zero where N_D is undefined.
+__device__ __forceinline__ void normal_chain(bool ok, const float (&l)[3], const float (&r)[3], const float (&u)[3],
+                                             const float (&d)[3], const float (&m)[3], float (&N)[3], float (&A)[3],
+                                             float (&B)[3]) {
+    float a[3], b[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { a[k] = r[k] - l[k]; b[k] = d[k] - u[k]; N[k] = 0.f; A[k] = 0.f; B[k] = 0.f; }
+    const float c0 = a[1] * b[2] - a[2] * b[1], c1 = a[2] * b[0] - a[0] * b[2], c2 = a[0] * b[1] - a[1] * b[0];
+    const float n2 = c0 * c0 + c1 * c1 + c2 * c2;
+    if (!ok || !(n2 > 0.f)) return;
+    const float inv = rsqrtf(n2);
+    N[0] = c0 * inv; N[1] = c1 * inv; N[2] = c2 * inv;
+    const float nm = N[0] * m[0] + N[1] * m[1] + N[2] * m[2];
+    const float q0 = (m[0] - N[0] * nm) * inv, q1 = (m[1] - N[1] * nm) * inv, q2 = (m[2] - N[2] * nm) * inv;
+    A[0] = b[1] * q2 - b[2] * q1; A[1] = b[2] * q0 - b[0] * q2; A[2] = b[0] * q1 - b[1] * q0;
+    B[0] = q1 * a[2] - q2 * a[1]; B[1] = q2 * a[0] - q0 * a[2]; B[2] = q0 * a[1] - q1 * a[0];
+}
+
+__global__ void __launch_bounds__(256)
+k_mapping_loss(MapImg im, const float* __restrict__ trgb, const float* __restrict__ tdepth, float lambda_c, float w_d,
+               float w_n, float nsign, float* __restrict__ loss) {
+    __shared__ float s_part[8];
+    const int x = blockIdx.x * 32 + (threadIdx.x & 31), y = blockIdx.y * 8 + (threadIdx.x >> 5);
+    float acc = 0.f;
+    if (x < im.W && y < im.H) {
+        const size_t HW = (size_t)im.W * im.H, pix = (size_t)y * im.W + x;
+        const float inv = 1.f / (float)HW;
+        // every load of the radius-2 diamond is issued before the arithmetic: 13 depths -> 13 points, 5 normals
+        auto inimg = [&](int ox, int oy) { return x + ox >= 0 && x + ox < im.W && y + oy >= 0 && y + oy < im.H; };
+        auto interior = [&](int ox, int oy) { return x + ox >= 1 && x + ox < im.W - 1 && y + oy >= 1 && y + oy < im.H - 1; };
+        auto depth_at = [&](int ox, int oy) { return inimg(ox, oy) ? im.depth[(size_t)(y + oy) * im.W + (x + ox)] : 0.f; };
+        const float d00 = depth_at(0, 0), dl = depth_at(-1, 0), dr = depth_at(1, 0), du = depth_at(0, -1), dd_ = depth_at(0, 1);
+        const float dll = depth_at(-2, 0), drr = depth_at(2, 0), duu = depth_at(0, -2), ddd = depth_at(0, 2);
+        const float dul = depth_at(-1, -1), dur = depth_at(1, -1), ddl = depth_at(-1, 1), ddr = depth_at(1, 1);
+        float m[5][3];  // rendered normal at centre, left, right, up, down
+        const int ox5[5] = {0, -1, 1, 0, 0}, oy5[5] = {0, 0, 0, -1, 1};
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const bool in = inimg(ox5[k], oy5[k]);
+            const size_t q = (size_t)(y + oy5[k]) * im.W + (x + ox5[k]);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) m[k][c] = in ? im.ren[4 + c][q] : 0.f;
+        }
+        float rgb[3], tr[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { rgb[c] = im.ren[c][pix]; tr[c] = trgb[c * HW + pix]; }
+        const float td = tdepth[pix];
+        auto pt = [&](float dv, int ox, int oy, float (&P)[3]) {
+            P[0] = dv * (((float)(x + ox) + 0.5f - im.cx) * im.ifx); P[1] = dv * (((float)(y + oy) + 0.5f - im.cy) * im.ify); P[2] = dv;
+        };
+        float P00[3], Pl[3], Pr[3], Pu[3], Pd[3], Pll[3], Prr[3], Puu[3], Pdd[3], Pul[3], Pur[3], Pdl[3], Pdr[3];
+        pt(d00, 0, 0, P00); pt(dl, -1, 0, Pl); pt(dr, 1, 0, Pr); pt(du, 0, -1, Pu); pt(dd_, 0, 1, Pd);
+        pt(dll, -2, 0, Pll); pt(drr, 2, 0, Prr); pt(duu, 0, -2, Puu); pt(ddd, 0, 2, Pdd);
+        pt(dul, -1, -1, Pul); pt(dur, 1, -1, Pur); pt(ddl, -1, 1, Pdl); pt(ddr, 1, 1, Pdr);
+        float N[3], Nt[3], A0[3], B0[3], Al[3], Ar[3], Bu[3], Bd[3], tmp[3];
+        normal_chain(interior(0, 0), Pl, Pr, Pu, Pd, m[0], N, A0, B0);
+        normal_chain(interior(-1, 0), Pll, P00, Pul, Pdl, m[1], Nt, Al, tmp);
+        normal_chain(interior(1, 0), P00, Prr, Pur, Pdr, m[2], Nt, Ar, tmp);
+        normal_chain(interior(0, -1), Pul, Pur, Puu, P00, m[3], Nt, tmp, Bu);
+        normal_chain(interior(0, 1), Pdl, Pdr, P00, Pdd, m[4], Nt, tmp, Bd);
+        float g[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float d = rgb[c] - tr[c];
+            acc += lambda_c * fabsf(d);
+            g[c] = d > 0.f ? lambda_c * inv : (d < 0.f ? -lambda_c * inv : 0.f);
+        }
+        const float dd = d00 - td;
+        acc += w_d * fabsf(dd);
+        g[3] = dd > 0.f ? w_d * inv : (dd < 0.f ? -w_d * inv : 0.f);
+        acc += w_n * (1.f - nsign * (N[0] * m[0][0] + N[1] * m[0][1] + N[2] * m[0][2]));
+        const float coef = -nsign * w_n * inv;
+        g[4] = coef * N[0]; g[5] = coef * N[1]; g[6] = coef * N[2];
+        const float r0 = ((float)x + 0.5f - im.cx) * im.ifx, r1 = ((float)y + 0.5f - im.cy) * im.ify;
+        g[3] += coef * (r0 * (Al[0] - Ar[0] + Bu[0] - Bd[0]) + r1 * (Al[1] - Ar[1] + Bu[1] - Bd[1]) +
+                        (Al[2] - Ar[2] + Bu[2] - Bd[2]));
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+            if (im.up[c]) im.up[c][pix] = g[c];
+        acc *= inv;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0 && loss) {
+        float t = 0.f;
+        for (int w = 0; w < 8; ++w) t += s_part[w];
+        atomicAdd(loss, t);
+    }
+}
+
 // Covisibility of two views (Eq. 22): counts of the intersection and the union of the visible
 // sets G_V = {k active : C_k^V > threshold}; the last block forms the score.  Integer counts: exact.
 __global__ void __launch_bounds__(256)
@@ -117,5 +219,21 @@ cudaError_t sgs_launch_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const fl
     if (e != cudaSuccess) return e;
     k_tracking_loss<<<blocks, 256, 0, s>>>(p, trgb, tdepth, cam->width, cam->height, cam->fx, cam->fy, cam->cx, cam->cy,
                                            lambda_d, nsign, loss);
+    return cudaGetLastError();
+}
+
+cudaError_t sgs_launch_mapping_loss(sgs_ctx* c, const sgs_camera* cam, const float* const ren[8], const float* trgb,
+                                    const float* tdepth, float lambda_c, float w_d, float w_n, float nsign, float* const up[8],
+                                    float* loss, cudaStream_t s) {
+    SgsStage st(c, SGS_STAGE_LOSS, s);
+    c->launches += 1;
+    MapImg im;
+    for (int i = 0; i < 8; ++i) { im.ren[i] = ren[i]; im.up[i] = up[i]; }
+    im.depth = ren[3]; im.W = cam->width; im.H = cam->height; im.ifx = 1.f / cam->fx; im.ify = 1.f / cam->fy; im.cx = cam->cx; im.cy = cam->cy;
+    cudaError_t e = cudaSuccess;
+    if (loss) e = cudaMemsetAsync(loss, 0, sizeof(float), s);
+    if (e != cudaSuccess) return e;
+    const dim3 grid((cam->width + 31) / 32, (cam->height + 7) / 8);
+    k_mapping_loss<<<grid, 256, 0, s>>>(im, trgb, tdepth, lambda_c, w_d, w_n, nsign, loss);
     return cudaGetLastError();
 }
