@@ -271,24 +271,27 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
 // pose gradient (Eq. 11-13).  Leaves acc[v] zeroed for the next backward.
 __global__ void __launch_bounds__(256)
 k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __restrict__ vis_to_surfel,
-                  const uint8_t* __restrict__ culled, unsigned int n_all,
+                  const uint8_t* __restrict__ culled,
                   float* __restrict__ acc, const float* __restrict__ mean, const float* __restrict__ scale,
                   const float* __restrict__ quat, SgsCamDev cam, sgs_surfel_grads out,
                   float* __restrict__ pose_partial, SgsCounters* __restrict__ counters_rw,
-                  float* __restrict__ d_pose6, int zero_rest) {
+                  float* __restrict__ d_pose6, int survivors) {
     __shared__ float s_red[8][6];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     // compacted mode: v < N_v, surfel = vis_to_surfel[v]; bucket mode (no compaction): v = surfel index
     // grid-stride over the surfels: a bounded grid keeps the per-block ticket of the pose reduction off the
     // critical path (one same-address atomic per block)
     float p6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    const unsigned int n_loop = vis_to_surfel ? counters->n_visible : n_all;
+    // list: the compacted visible surfels (radix binning: acc is indexed by the list position) or K-pre-A's survivor
+    // list (bucket binning: a superset of the visible surfels; acc is indexed by the surfel itself).  Everything
+    // else -- inactive, pre-culled -- keeps the zeros the launcher's memsets wrote.
+    const unsigned int n_loop = survivors ? counters->n_surv : counters->n_visible;
     for (unsigned int v = blockIdx.x * blockDim.x + tid; v < n_loop; v += gridDim.x * blockDim.x) {
-    const bool live = vis_to_surfel ? true : (culled[v] == 0);
+    const uint32_t i = vis_to_surfel[v];
+    const bool live = survivors ? (culled[i] == 0) : true;
     if (live) {
-        const uint32_t i = vis_to_surfel ? vis_to_surfel[v] : v;
         float a[16];
-        float4* ap = reinterpret_cast<float4*>(acc + (size_t)v * SGS_ACC_STRIDE);
+        float4* ap = reinterpret_cast<float4*>(acc + (size_t)(survivors ? i : v) * SGS_ACC_STRIDE);
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             const float4 t = ap[c];
@@ -360,15 +363,6 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
             out.quat[4 * i + 3] = (dq[3] - qz * qd) * qi;
         }
     }
-    else if (zero_rest) {
-        // inactive / culled surfel: gradients are exactly zero (bucket mode: v IS the surfel index, so the
-        // caller's buffers are overwritten here instead of by five memsets)
-        if (out.mean) { out.mean[3 * v] = 0.f; out.mean[3 * v + 1] = 0.f; out.mean[3 * v + 2] = 0.f; }
-        if (out.scale) { out.scale[2 * v] = 0.f; out.scale[2 * v + 1] = 0.f; }
-        if (out.quat) reinterpret_cast<float4*>(out.quat)[v] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (out.opacity) out.opacity[v] = 0.f;
-        if (out.rgb) { out.rgb[3 * v] = 0.f; out.rgb[3 * v + 1] = 0.f; out.rgb[3 * v + 2] = 0.f; }
-    }
     }
     if (d_pose6 == nullptr) return;
 #pragma unroll
@@ -405,29 +399,29 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     }
     const int64_t n = c->last_surfels.n;
     cudaError_t e = cudaSuccess;
-    // bucket mode: k_surfel_backward visits every surfel and writes the zeros itself; the quat store is a float4
-    const bool bucket_mode = c->list_stride == 2;
-    const bool kernel_zeroes = bucket_mode && ((reinterpret_cast<uintptr_t>(dg->quat) & 15u) == 0);
-    if (!kernel_zeroes) {
-        if (dg->mean && e == cudaSuccess) e = cudaMemsetAsync(dg->mean, 0, sizeof(float) * 3 * (size_t)n, s);
-        if (dg->scale && e == cudaSuccess) e = cudaMemsetAsync(dg->scale, 0, sizeof(float) * 2 * (size_t)n, s);
-        if (dg->quat && e == cudaSuccess) e = cudaMemsetAsync(dg->quat, 0, sizeof(float) * 4 * (size_t)n, s);
-        if (dg->opacity && e == cudaSuccess) e = cudaMemsetAsync(dg->opacity, 0, sizeof(float) * (size_t)n, s);
-        if (dg->rgb && e == cudaSuccess) e = cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * (size_t)n, s);
-    }
+    // exact zeros for every surfel the per-surfel kernel does not visit (inactive, culled)
+    if (dg->mean && e == cudaSuccess) e = cudaMemsetAsync(dg->mean, 0, sizeof(float) * 3 * (size_t)n, s);
+    if (dg->scale && e == cudaSuccess) e = cudaMemsetAsync(dg->scale, 0, sizeof(float) * 2 * (size_t)n, s);
+    if (dg->quat && e == cudaSuccess) e = cudaMemsetAsync(dg->quat, 0, sizeof(float) * 4 * (size_t)n, s);
+    if (dg->opacity && e == cudaSuccess) e = cudaMemsetAsync(dg->opacity, 0, sizeof(float) * (size_t)n, s);
+    if (dg->rgb && e == cudaSuccess) e = cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * (size_t)n, s);
     if (e != cudaSuccess) return e;
     c->launches += 1;
     k_backward<false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                   cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
                                                   c->acc, c->pose_partial, c->counters, nullptr, FusedLoss{});
-    int blocks = (int)((n + 255) / 256);  // bound on N_v
+    // one thread per listed surfel; the list length is only known on the device: grid-stride from a hinted grid
+    const bool bucket_mode = c->list_stride == 2;
+    int64_t want = n;
+    if (bucket_mode && c->last_surv > 0 && c->last_surv + c->last_surv / 4 < want) want = c->last_surv + c->last_surv / 4;
+    int blocks = (int)((want + 255) / 256);
     if (blocks > 148 * 8) blocks = 148 * 8;
-    if (blocks == 0 && d_pose6) return cudaMemsetAsync(d_pose6, 0, sizeof(float) * 6, s);
-    if (blocks > 0)
-        c->launches += 1, k_surfel_backward<<<blocks, 256, 0, s>>>(c->counters, c->list_stride == 2 ? nullptr : c->vis_to_surfel, c->culled,
-                                                 (unsigned int)n, c->acc, c->last_surfels.mean,
-                                                 c->last_surfels.scale, c->last_surfels.quat, cam, *dg, c->pose_partial,
-                                                 c->counters, d_pose6, kernel_zeroes ? 1 : 0);
+    if (n == 0) return d_pose6 ? cudaMemsetAsync(d_pose6, 0, sizeof(float) * 6, s) : cudaSuccess;
+    if (blocks < 1) blocks = 1;
+    c->launches += 1;
+    k_surfel_backward<<<blocks, 256, 0, s>>>(c->counters, c->vis_to_surfel, c->culled, c->acc, c->last_surfels.mean,
+                                             c->last_surfels.scale, c->last_surfels.quat, cam, *dg, c->pose_partial,
+                                             c->counters, d_pose6, bucket_mode ? 1 : 0);
     return cudaGetLastError();
 }
 
