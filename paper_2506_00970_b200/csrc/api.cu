@@ -98,6 +98,7 @@ int sgs_ensure_buckets(sgs_ctx* c, int tiles, int64_t tile_cap, cudaStream_t s) 
             return SGS_OUT_OF_MEMORY;
         c->cursor_cap = tiles;
         c->cost_tiles = 0;
+        c->prezero_tiles = 0;
     }
     if ((int64_t)tiles * cap > c->bucket_cap) {
         const size_t m = (size_t)tiles * (size_t)cap;

@@ -427,10 +427,14 @@ cudaError_t sgs_launch_preprocess(sgs_ctx* c, const sgs_surfels* sf, cudaStream_
 cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cudaStream_t s) {
     const int64_t n = sf->n;
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
-    cudaError_t e = cudaMemsetAsync(c->counters, 0, sizeof(SgsCounters), s);
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(c->cursor, 0, sizeof(uint32_t) * (size_t)tiles, s);
-    if (e != cudaSuccess) return e;
+    cudaError_t e = cudaSuccess;
+    if (c->prezero_tiles < tiles) {  // else: the previous sgs_track_iter's kernel already zeroed both (two stream ops saved)
+        e = cudaMemsetAsync(c->counters, 0, sizeof(SgsCounters), s);
+        if (e != cudaSuccess) return e;
+        e = cudaMemsetAsync(c->cursor, 0, sizeof(uint32_t) * (size_t)tiles, s);
+        if (e != cudaSuccess) return e;
+    }
+    c->prezero_tiles = 0;
     SgsStage st(c, SGS_STAGE_PREPROCESS, s);
     // K-pre-A: 4 surfels per thread once that still gives every SM several blocks (large maps), else 1
     const bool wide = (n + 1023) / 1024 >= 4 * 148;

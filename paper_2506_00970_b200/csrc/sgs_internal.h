@@ -134,6 +134,7 @@ struct sgs_ctx {
     int64_t last_surv;               // K-pre-A survivors of the last checked render (K-pre-B grid hint), 0 = unknown
     uint32_t* tile_cost;             // tiles: cycles >> 8 each tile's k_track block took last time (scheduling feedback)
     int cost_tiles, cost_W, cost_H;  // camera the costs were measured for (0 = none)
+    int prezero_tiles;               // k_track's last block left counters and cursor[0..prezero_tiles) zeroed for the next preprocess
 };
 
 // ---- launchers (each enqueues on `s`, returns the last CUDA error) ----

@@ -53,11 +53,11 @@ __device__ __forceinline__ float pair_rho2(const float4 s0, const float4 s1, con
 
 template <bool WRITE_IMAGES>
 __global__ void __launch_bounds__(SGS_BLOCK, 3)
-k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* __restrict__ cursor, unsigned long long* bucket, uint32_t tile_cap,
+k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cursor, unsigned long long* bucket, uint32_t tile_cap,
         int presorted, SgsPayload pay, int W, int H, int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg,
         TrackPlanes out, const float* __restrict__ trgb, const float* __restrict__ tdepth, float lambda_d, float nsign,
         float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
-        float* __restrict__ loss_out, uint32_t* __restrict__ tile_cost) {
+        float* __restrict__ loss_out, uint32_t* __restrict__ tile_cost, uint32_t* cursor_rw) {
     const long long t_start = clock64();
     __shared__ float4 sh[7][SGS_BLOCK];
     __shared__ unsigned long long s_keys[SGS_BLOCK];
@@ -354,6 +354,13 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* __r
     // of this launch has read its entry).  Ties land in arbitrary order; the order steers scheduling, never a result.
     unsigned int* s_hist = reinterpret_cast<unsigned int*>(&sh[0][0]);  // staging memory is free now
     const int tiles = (int)gridDim.x;
+    // ... and the next preprocess finds its counters and per-tile cursors already zeroed (every block of this launch
+    // has read its cursor; the host copied the counters before this kernel started)
+    for (int t = tid; t < tiles; t += SGS_BLOCK) cursor_rw[t] = 0u;
+    if (tid == 0) {
+        counters->n_entries = 0ull; counters->n_visible = 0u; counters->overflow = 0u; counters->ticket_pre = 0u;
+        counters->max_tile = 0u; counters->n_surv = 0u;
+    }
     __syncthreads();
     for (int b = tid; b < TRK_ORDER_BINS; b += SGS_BLOCK) s_hist[b] = 0;
     __syncthreads();
@@ -430,11 +437,12 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
     if (any)
         k_track<true><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, (uint32_t)c->tile_cap, presorted, c->pay, cam.W,
                                                   cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb,
-                                                  tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost);
+                                                  tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost, c->cursor);
     else
         k_track<false><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, (uint32_t)c->tile_cap, presorted, c->pay, cam.W,
                                                    cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb,
-                                                   tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost);
+                                                   tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost, c->cursor);
     c->cost_tiles = tiles; c->cost_W = cam.W; c->cost_H = cam.H;
+    c->prezero_tiles = tiles;
     return cudaGetLastError();
 }
