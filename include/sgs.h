@@ -197,7 +197,10 @@ SGS_API int sgs_backward_tracking(sgs_ctx* ctx, const sgs_images* target, float 
  *   target  : DEVICE rgb (3xHxW) + depth (HxW) of the current frame
  *   out     : nullable; DEVICE images to write (any pointer may be NULL = not written)
  *   d_pose6 : DEVICE, 6 floats (rho, theta); loss: DEVICE, 1 float, nullable
- * Leaves no state for sgs_backward (SGS_NO_FORWARD_STATE); sgs_get_binning works. */
+ * Leaves no state for sgs_backward (SGS_NO_FORWARD_STATE); sgs_get_binning works.
+ * With SGS_FLAG_ASYNC the counters of an iteration reach the host behind its compositing kernel and are never waited
+ * for: a tile-bucket overflow is reported (SGS_WORKSPACE_OVERFLOW, workspace grown) by the first later call on the
+ * ctx that finds them there, or by sgs_get_stats, which waits. */
 SGS_API int sgs_track_iter(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_camera* cam, const sgs_images* target,
                            float lambda_d, float normal_sign, const sgs_images* out, float* d_pose6, float* loss,
                            void* cuda_stream);

@@ -9,8 +9,15 @@ static int64_t grown_tile_cap(int64_t max_tile) { return max_tile + max_tile / 2
 // async mode: examine the counters of the previous render (already copied to pinned memory)
 static int check_pending(sgs_ctx* c, cudaStream_t s) {
     if (!c->pending_check) return SGS_OK;
-    if (cudaEventSynchronize(c->counters_ready) != cudaSuccess) return SGS_CUDA_ERROR;
+    if (c->pending_lazy) {
+        // sgs_track_iter copies the counters after its fused kernel: waiting here would serialise host and device,
+        // so an overflow of iteration i is reported by the first call that finds the copy complete
+        const cudaError_t q = cudaEventQuery(c->counters_ready);
+        if (q == cudaErrorNotReady) return SGS_OK;
+        if (q != cudaSuccess) return SGS_CUDA_ERROR;
+    } else if (cudaEventSynchronize(c->counters_ready) != cudaSuccess) return SGS_CUDA_ERROR;
     c->pending_check = false;
+    c->pending_lazy = false;
     const int64_t E = (int64_t)c->counters_host->n_entries;
     c->last_entries = E;
     c->last_surv = (int64_t)c->counters_host->n_surv;
@@ -39,7 +46,9 @@ static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, bool want_
     int r = sgs_ensure_buckets(c, tiles, c->tile_cap ? c->tile_cap : 2048, s);
     if (r != SGS_OK) return r;
     if (sgs_launch_preprocess_bucket(c, sf, s) != cudaSuccess) return SGS_CUDA_ERROR;
-    if ((r = copy_counters(c, s)) != SGS_OK) return r;
+    const bool defer = async && c->defer_counters && c->tile_cap <= 2048;  // the fused kernel snapshots them
+    c->defer_counters = defer;
+    if (!defer && (r = copy_counters(c, s)) != SGS_OK) return r;
     if (!async) {
         if (cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
         if (c->counters_host->max_tile > (unsigned)c->tile_cap) {  // grow and emit again
@@ -50,9 +59,10 @@ static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, bool want_
         }
         c->last_entries = (int64_t)c->counters_host->n_entries;
         c->last_surv = (int64_t)c->counters_host->n_surv;
-    } else {
+    } else if (!defer) {
         cudaEventRecord(c->counters_ready, s);
         c->pending_check = true;
+        c->pending_lazy = false;
     }
     c->fused_sort = c->tile_cap <= 2048;
     c->render_order_valid = false;
@@ -95,6 +105,7 @@ static int bin_radix(sgs_ctx* c, const sgs_surfels* sf, bool async, cudaStream_t
     } else {
         cudaEventRecord(c->counters_ready, s);
         c->pending_check = true;
+        c->pending_lazy = false;
     }
     c->fused_sort = false;
     c->render_order_valid = false;
@@ -175,14 +186,24 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
         c->have_forward = false;
         return r;
     }
+    c->defer_counters = true;  // (bin_buckets clears it when it cannot honour it)
     int r = bin_view(c, sf, cam, false, s);
+    const bool deferred = c->defer_counters;
+    c->defer_counters = false;
     if (r != SGS_OK) return r;
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
     if ((r = sgs_ensure_partials(c, tiles, s)) != SGS_OK) return r;
     float* planes[8];
     pick_planes(c, out, (int64_t)cam->width * cam->height, false, planes);
-    if (sgs_launch_track(c, planes, target->rgb, target->depth, lambda_d, normal_sign, d_pose6, loss, s) != cudaSuccess)
+    if (sgs_launch_track(c, planes, target->rgb, target->depth, lambda_d, normal_sign, d_pose6, loss, deferred, s) != cudaSuccess)
         return SGS_CUDA_ERROR;
+    if (deferred) {  // the counters of this iteration's preprocess, snapshotted by k_track's last block
+        if (cudaMemcpyAsync(c->counters_host, c->counters_snap, sizeof(SgsCounters), cudaMemcpyDeviceToHost, s) != cudaSuccess)
+            return SGS_CUDA_ERROR;
+        cudaEventRecord(c->counters_ready, s);
+        c->pending_check = true;
+        c->pending_lazy = true;
+    }
     c->have_binning = true;
     return SGS_OK;
 }

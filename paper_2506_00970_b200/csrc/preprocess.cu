@@ -257,6 +257,7 @@ k_pre_select(int64_t n, const float* __restrict__ mean, const float* __restrict_
              const uint8_t* __restrict__ active, SgsCamDev cam, SgsCfgDev cfg, uint8_t* __restrict__ culled,
              SgsCounters* __restrict__ counters, uint32_t* __restrict__ surv_list) {
     constexpr int SGS_PREA_SPAN = SGS_PREA_ITEMS * SGS_PRE_BLOCK;
+    cudaTriggerProgrammaticLaunchCompletion();  // K-pre-B may be staged now; it waits for this grid before reading
     __shared__ unsigned short s_list[SGS_PREA_SPAN];
     __shared__ unsigned int s_n, s_base;
     const int tid = threadIdx.x, lane = tid & 31;
@@ -315,6 +316,7 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
     __shared__ unsigned int s_w[SGS_PREB_BLOCK];      // rectangle width in tiles
     __shared__ unsigned int s_wsum[SGS_PREB_BLOCK / 32];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    cudaGridDependencySynchronize();                // K-pre-A complete: survivor list and count are final
     const unsigned int n_surv = counters->n_surv;   // written by K-pre-A (previous launch on the stream)
     for (unsigned int r0 = blockIdx.x * SGS_PREB_BLOCK; r0 < n_surv; r0 += gridDim.x * SGS_PREB_BLOCK) {
         const bool have = r0 + tid < n_surv;
@@ -458,8 +460,16 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     }
     if (blocks_b > 148 * 8) blocks_b = 148 * 8;
     if (blocks_b < 1) blocks_b = 1;
-    k_pre_project<<<(int)blocks_b, SGS_PREB_BLOCK, 0, s>>>(sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd, c->cfgd,
-                                                          c->pay, c->culled, c->counters, c->vis_to_surfel, c->cursor,
-                                                          c->bucket, (uint32_t)c->tile_cap);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)blocks_b); cfg.blockDim = dim3(SGS_PREB_BLOCK); cfg.dynamicSmemBytes = 0; cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = blocks_a > 0 ? 1 : 0;  // programmatic dependent launch behind K-pre-A
+    const cudaError_t le = cudaLaunchKernelEx(&cfg, k_pre_project, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd,
+                                              c->cfgd, c->pay, c->culled, c->counters, (const uint32_t*)c->vis_to_surfel,
+                                              c->cursor, c->bucket, (uint32_t)c->tile_cap);
+    if (le != cudaSuccess) return le;
     return cudaGetLastError();
 }

@@ -109,6 +109,7 @@ struct sgs_ctx {
     bool have_forward;
     bool have_binning;               // sorted lists + ranges of the last render / track_iter are valid
     bool pending_check;              // async mode: counters_host not yet examined
+    bool pending_lazy;               // ... and the copy was enqueued BEHIND the compositing kernel (sgs_track_iter): never wait for it
     sgs_surfels last_surfels;
     sgs_camera last_cam;
     SgsCamDev camd;
@@ -134,6 +135,8 @@ struct sgs_ctx {
     int64_t last_surv;               // K-pre-A survivors of the last checked render (K-pre-B grid hint), 0 = unknown
     uint32_t* tile_cost;             // tiles: cycles >> 8 each tile's k_track block took last time (scheduling feedback)
     int cost_tiles, cost_W, cost_H;  // camera the costs were measured for (0 = none)
+    SgsCounters* counters_snap;      // device copy of the counters taken by k_track's last block before it zeroes them
+    bool defer_counters;             // sgs_track_iter (async): the counters reach the host after k_track, from the snapshot
     int prezero_tiles;               // k_track's last block left counters and cursor[0..prezero_tiles) zeroed for the next preprocess
 };
 
@@ -153,7 +156,7 @@ cudaError_t sgs_launch_export_idx(sgs_ctx* c, cudaStream_t s);
 cudaError_t sgs_launch_backward_tracking(sgs_ctx* c, const float* trgb, const float* tdepth, float lambda_d, float nsign,
                                          float* d_pose6, float* loss, cudaStream_t s);
 cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* trgb, const float* tdepth, float lambda_d,
-                             float nsign, float* d_pose6, float* loss, cudaStream_t s);
+                             float nsign, float* d_pose6, float* loss, bool after_preprocess, cudaStream_t s);
 int sgs_sort_passes(int tiles);
 cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cudaStream_t s);
 cudaError_t sgs_launch_tilesort(sgs_ctx* c, cudaStream_t s);

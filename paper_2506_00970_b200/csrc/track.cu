@@ -57,7 +57,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         int presorted, SgsPayload pay, int W, int H, int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg,
         TrackPlanes out, const float* __restrict__ trgb, const float* __restrict__ tdepth, float lambda_d, float nsign,
         float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
-        float* __restrict__ loss_out, uint32_t* __restrict__ tile_cost, uint32_t* cursor_rw) {
+        float* __restrict__ loss_out, uint32_t* __restrict__ tile_cost, uint32_t* cursor_rw, SgsCounters* __restrict__ counters_snap) {
     const long long t_start = clock64();
     __shared__ float4 sh[7][SGS_BLOCK];
     __shared__ unsigned long long s_keys[SGS_BLOCK];
@@ -358,6 +358,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     // has read its cursor; the host copied the counters before this kernel started)
     for (int t = tid; t < tiles; t += SGS_BLOCK) cursor_rw[t] = 0u;
     if (tid == 0) {
+        if (counters_snap) *counters_snap = *counters;  // what the host reads for overflow detection and hints
         counters->n_entries = 0ull; counters->n_visible = 0u; counters->overflow = 0u; counters->ticket_pre = 0u;
         counters->max_tile = 0u; counters->n_surv = 0u;
     }
@@ -420,7 +421,7 @@ __global__ void k_iota(uint32_t* __restrict__ p, int n) {
 }  // namespace
 
 cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* trgb, const float* tdepth, float lambda_d,
-                             float nsign, float* d_pose6, float* loss, cudaStream_t s) {
+                             float nsign, float* d_pose6, float* loss, bool after_preprocess, cudaStream_t s) {
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
     const SgsCamDev& cam = c->camd;
     TrackPlanes out;
@@ -434,14 +435,20 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
     c->launches += 1;
     unsigned long long* bucket = reinterpret_cast<unsigned long long*>(c->bucket);
     const int presorted = c->fused_sort ? 0 : 1;
+    // (A programmatic dependent launch behind K-pre-B was measured and rejected: C2 3459 -> 2888 MP/s, the early
+    // resident blocks of this kernel get in K-pre-B's way; profiles/r01_c2_track.md.)
+    const uint32_t tile_cap = (uint32_t)c->tile_cap;
+    SgsCounters* snap = after_preprocess ? c->counters_snap : nullptr;
     if (any)
-        k_track<true><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, (uint32_t)c->tile_cap, presorted, c->pay, cam.W,
-                                                  cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb,
-                                                  tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost, c->cursor);
+        k_track<true><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W,
+                                                  cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb, tdepth,
+                                                  lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost,
+                                                  c->cursor, snap);
     else
-        k_track<false><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, (uint32_t)c->tile_cap, presorted, c->pay, cam.W,
-                                                   cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb,
-                                                   tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost, c->cursor);
+        k_track<false><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W,
+                                                   cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb, tdepth,
+                                                   lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost,
+                                                   c->cursor, snap);
     c->cost_tiles = tiles; c->cost_W = cam.W; c->cost_H = cam.H;
     c->prezero_tiles = tiles;
     return cudaGetLastError();
