@@ -43,7 +43,10 @@ def load_peaks():
 
 
 def fp32_peak_tflops(peaks):
+    # measured on this device by sgs_measure_fp32_peak (register-resident FMA loop) when available; else
     # 148 SMs x 128 FP32 lanes x 2 flop (FMA) x max SM clock (guide's unit counts and clocks)
+    if peaks.get("fp32_tflops_measured"):
+        return peaks["fp32_tflops_measured"]
     return 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
 
 
@@ -382,6 +385,10 @@ def main():
         return
 
     peaks = load_peaks()
+    try:
+        peaks["fp32_tflops_measured"] = wl.sgs.measure_fp32_peak()
+    except Exception:
+        peaks["fp32_tflops_measured"] = None
     cpu, roof, stages = None, None, {}
     if not args.no_cpu_baseline:
         cpu, (sc, cams, info) = cpu_baseline(args.config)
@@ -414,7 +421,7 @@ def main():
         dom = max(stages, key=lambda k: stages[k]["share"])
         roof = dict(stages[dom])
         roof.update(kernel=dom, traffic=NCU_TRAFFIC.get((args.config, dom)), peak_source=peaks["source"] + (" HBM copy" if roof["bound"] == "hbm" else
-                    "; alu peak = 148 SM x 128 lanes x 2 x max SM clock"), counters=dict(cnt, E=E))
+                    ("; alu peak = measured FMA loop (sgs_measure_fp32_peak), nominal 148 SM x 128 lanes x 2 x max SM clock = %.1f" % (148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12) if peaks.get("fp32_tflops_measured") else "; alu peak = 148 SM x 128 lanes x 2 x max SM clock")), counters=dict(cnt, E=E))
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=ms_max / K,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
                 surfels_per_s=wl.n_active * renders / (ms_max * 1e-3),

@@ -233,6 +233,11 @@ SGS_API int sgs_upload_target(sgs_ctx* ctx, const sgs_camera* cam, const float* 
 SGS_API int sgs_track_iter_host(sgs_ctx* ctx, const sgs_camera* cam, float lambda_d, float normal_sign,
                         float* host_loss, float* host_d_pose6, void* cuda_stream);
 
+/* Measures this device's FP32 FMA throughput with a register-resident loop (16 independent chains per thread,
+ * 8 blocks of 256 threads per SM, best of 4 timed launches, ~1 ms each; waits): the denominator of the compositing
+ * kernels' roofline.  tflops: HOST double. */
+SGS_API int sgs_measure_fp32_peak(double* tflops, void* cuda_stream);
+
 SGS_API const char* sgs_status_string(int status);
 
 #ifdef __cplusplus

@@ -51,7 +51,7 @@ class sgs_stats(C.Structure):
 
 
 EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_backward", "sgs_tracking_loss",
-           "sgs_backward_tracking", "sgs_track_iter", "sgs_render_contrib", "sgs_covisibility", "sgs_mapping_loss", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
+           "sgs_backward_tracking", "sgs_track_iter", "sgs_render_contrib", "sgs_covisibility", "sgs_mapping_loss", "sgs_measure_fp32_peak", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
            "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string"]
 
 _lib = None
@@ -119,6 +119,15 @@ def _images(rgb=None, depth=None, normal=None, alpha=None, device_type="cuda"):
 def _stream_ptr(stream):
     s = torch.cuda.current_stream() if stream is None else stream
     return C.c_void_p(s.cuda_stream)
+
+
+def measure_fp32_peak(stream=None):
+    """sgs_measure_fp32_peak: measured FP32 FMA throughput of the current device in TFLOP/s."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2506_00970_b200 needs a CUDA device; there is no CPU fallback")
+    out = C.c_double(0.0)
+    _check(load_library().sgs_measure_fp32_peak(C.byref(out), _stream_ptr(stream)), "sgs_measure_fp32_peak")
+    return float(out.value)
 
 
 class Renderer:

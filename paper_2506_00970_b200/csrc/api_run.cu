@@ -282,6 +282,11 @@ int sgs_mapping_loss(sgs_ctx* c, const sgs_camera* cam, const sgs_images* ren, c
                                    (cudaStream_t)stream) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
 }
 
+int sgs_measure_fp32_peak(double* tflops, void* stream) {
+    if (!tflops) return SGS_INVALID_ARGUMENT;
+    return sgs_launch_fma_peak(tflops, (cudaStream_t)stream) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
+}
+
 int sgs_get_binning(sgs_ctx* c, int64_t* n_entries, const uint64_t** keys, const uint32_t** idx,
                     const uint32_t** tile_ranges, const uint8_t** culled) {
     if (!c) return SGS_INVALID_ARGUMENT;

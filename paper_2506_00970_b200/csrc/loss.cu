@@ -237,3 +237,48 @@ cudaError_t sgs_launch_mapping_loss(sgs_ctx* c, const sgs_camera* cam, const flo
     k_mapping_loss<<<grid, 256, 0, s>>>(im, trgb, tdepth, lambda_c, w_d, w_n, nsign, loss);
     return cudaGetLastError();
 }
+
+// ---- FP32 FMA peak of this device, measured: the denominator of the compositing kernels' roofline ----
+namespace {
+__global__ void __launch_bounds__(256)
+k_fma_peak(float* __restrict__ sink, int iters, float a, float b) {
+    float x[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) x[k] = (float)(threadIdx.x + k) * 1e-3f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) x[k] = fmaf(x[k], a, b);   // 16 independent register-resident chains
+    }
+    float t = 0.f;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) t += x[k];
+    if (t == 12345.678f) sink[0] = t;   // keeps the loop alive; practically never taken
+}
+}  // namespace
+
+cudaError_t sgs_launch_fma_peak(double* tflops, cudaStream_t s) {
+    int dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    float* sink = nullptr;
+    cudaError_t e = cudaMalloc(&sink, sizeof(float));
+    if (e != cudaSuccess) return e;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = sms * 8, iters = 1 << 14;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {   // first repetitions warm the clocks; best of the rest
+        cudaEventRecord(e0, s);
+        k_fma_peak<<<blocks, 256, 0, s>>>(sink, iters, 0.999f, 1e-4f);
+        cudaEventRecord(e1, s);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double tf = 2.0 * 16.0 * (double)iters * 256.0 * (double)blocks / (ms * 1e-3) / 1e12;
+        if (rep >= 2 && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(sink);
+    *tflops = best;
+    return cudaGetLastError();
+}

@@ -152,6 +152,7 @@ cudaError_t sgs_launch_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const fl
 cudaError_t sgs_launch_mapping_loss(sgs_ctx* c, const sgs_camera* cam, const float* const ren[8], const float* trgb,
                                     const float* tdepth, float lambda_c, float w_d, float w_n, float nsign, float* const up[8],
                                     float* loss, cudaStream_t s);
+cudaError_t sgs_launch_fma_peak(double* tflops, cudaStream_t s);
 cudaError_t sgs_launch_export_idx(sgs_ctx* c, cudaStream_t s);
 cudaError_t sgs_launch_backward_tracking(sgs_ctx* c, const float* trgb, const float* tdepth, float lambda_d, float nsign,
                                          float* d_pose6, float* loss, cudaStream_t s);
