@@ -255,3 +255,33 @@ def mapping_loss(img, target_rgb, target_depth, camv, lambda_c, w_d, w_n, normal
     gP[:, :-2, 1:-1] -= dfb
     up[3] += (gP * ray).sum(0)
     return float(L), up
+
+
+def quat_to_matrix(q):
+    """R(q/|q|) for (n,4) quaternions (w,x,y,z), fp64 -- the unit-quaternion formula of Eq. 5-6's R."""
+    q = np.asarray(q, dtype=np.float64)
+    q = q / np.linalg.norm(q, axis=-1, keepdims=True)
+    w, x, y, z = q[..., 0], q[..., 1], q[..., 2], q[..., 3]
+    return np.stack([np.stack([1 - 2 * (y * y + z * z), 2 * (x * y - w * z), 2 * (x * z + w * y)], -1),
+                     np.stack([2 * (x * y + w * z), 1 - 2 * (x * x + z * z), 2 * (y * z - w * x)], -1),
+                     np.stack([2 * (x * z - w * y), 2 * (y * z + w * x), 1 - 2 * (x * x + y * y)], -1)], -2)
+
+
+def map_correction(mean, quat, frame_id, T_orig, T_opt):
+    """Map correction after pose-graph optimisation (Eq. 31-32, L302-312): Delta T_i = T_i^o T_i^{-1} per keyframe;
+    each splat moves with the increment of its closest observed keyframe f: mu' = Delta T_f mu, R' = Delta R_f R.
+    T_orig, T_opt: (K,3,4) rigid transforms [R|t].  Returns (mu' (n,3), R' (n,3,3)) in fp64 -- the rotation as a MATRIX
+    (a quaternion is unique only up to sign)."""
+    To = np.asarray(T_orig, dtype=np.float64).reshape(-1, 3, 4)
+    Tn = np.asarray(T_opt, dtype=np.float64).reshape(-1, 3, 4)
+    K = To.shape[0]
+    dT = np.zeros((K, 4, 4))
+    for i in range(K):
+        A = np.eye(4); A[:3] = To[i]
+        B = np.eye(4); B[:3] = Tn[i]
+        dT[i] = B @ np.linalg.inv(A)                 # Eq. 31
+    f = np.asarray(frame_id).astype(np.int64)
+    mu = np.asarray(mean, dtype=np.float64)
+    mu2 = np.einsum("nij,nj->ni", dT[f, :3, :3], mu) + dT[f, :3, 3]      # Eq. 32
+    R2 = np.einsum("nij,njk->nik", dT[f, :3, :3], quat_to_matrix(quat))
+    return mu2, R2

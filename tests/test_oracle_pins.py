@@ -533,3 +533,35 @@ def test_p13_mapping_loss_values_and_gradient():
         d = np.zeros_like(img); d[ch, j, i] = 1e-6
         fd = (oracle.mapping_loss(img + d, *args)[0] - oracle.mapping_loss(img - d, *args)[0]) / 2e-6
         assert abs(fd - up[ch, j, i]) <= 2e-6 * abs(up[ch, j, i]) + 1e-11, (ch, j, i, fd, up[ch, j, i])
+
+
+# ---------------------------------------------------------------- P14: map correction (Eq. 31-32)
+def _rand_poses(g, k, scale=1.0):
+    rot = Rotation.from_rotvec(scale * np.stack([g.normal(3) for _ in range(k)]))
+    T = np.zeros((k, 3, 4)); T[:, :, :3] = rot.as_matrix(); T[:, :, 3] = 2.0 * np.stack([g.normal(3) for _ in range(k)])
+    return T
+
+
+def test_p14_map_correction_moves_splats_rigidly_with_their_keyframe():
+    """A splat expressed in its keyframe's frame keeps those coordinates: T_o^{-1} (mu', R') = T^{-1} (mu, R) (what Eq.
+    31-32 mean), checked with scipy rotations; identity increments leave the map unchanged; two splats of one keyframe
+    keep their distance."""
+    g = scenegen.SplitMix(31)
+    n, K = 200, 7
+    To, Tn = _rand_poses(g, K), _rand_poses(g, K)
+    mean = np.stack([g.normal(n) for _ in range(3)], 1)
+    quat = np.stack([g.normal(n) for _ in range(4)], 1) * 1.7          # not unit
+    fid = (g.uniform(n) * K).astype(np.int32)
+    mu2, R2 = oracle.map_correction(mean, quat, fid, To, Tn)
+    qx = quat / np.linalg.norm(quat, axis=1, keepdims=True)
+    R = Rotation.from_quat(np.stack([qx[:, 1], qx[:, 2], qx[:, 3], qx[:, 0]], 1)).as_matrix()   # scipy: (x,y,z,w)
+    np.testing.assert_allclose(oracle.quat_to_matrix(quat), R, atol=1e-12)
+    for k in range(n):
+        Ro, to, Rn, tn = To[fid[k], :, :3], To[fid[k], :, 3], Tn[fid[k], :, :3], Tn[fid[k], :, 3]
+        np.testing.assert_allclose(Rn.T @ (mu2[k] - tn), Ro.T @ (mean[k] - to), atol=1e-10)   # same local coordinates
+        np.testing.assert_allclose(Rn.T @ R2[k], Ro.T @ R[k], atol=1e-10)                      # same local orientation
+        assert abs(np.linalg.det(R2[k]) - 1) < 1e-10
+    mu3, R3 = oracle.map_correction(mean, quat, fid, To, To)
+    np.testing.assert_allclose(mu3, mean, atol=1e-12); np.testing.assert_allclose(R3, R, atol=1e-12)
+    a, b = np.nonzero(fid == fid[0])[0][:2]
+    assert abs(np.linalg.norm(mu2[a] - mu2[b]) - np.linalg.norm(mean[a] - mean[b])) < 1e-10
