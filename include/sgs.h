@@ -233,6 +233,13 @@ SGS_API int sgs_upload_target(sgs_ctx* ctx, const sgs_camera* cam, const float* 
 SGS_API int sgs_track_iter_host(sgs_ctx* ctx, const sgs_camera* cam, float lambda_d, float normal_sign,
                         float* host_loss, float* host_d_pose6, void* cuda_stream);
 
+/* Map correction after pose-graph optimisation (Eq. 31-32), in place: Delta T_f = T_f^o T_f^{-1} and
+ * mu_k <- Delta T_f mu_k, R_k <- Delta R_f R_k with f = frame_id[k], the splat's closest observed keyframe.
+ *   mean (n x 3), quat (n x 4, (w,x,y,z), 16-byte aligned), frame_id (n x int32; ids outside [0, n_frames) leave the
+ *   splat untouched), T_orig / T_opt (n_frames x 12, row-major 3x4 [R|t] of T_f and T_f^o): all DEVICE. */
+SGS_API int sgs_map_correction(sgs_ctx* ctx, int64_t n, float* mean, float* quat, const int32_t* frame_id, int n_frames,
+                               const float* T_orig, const float* T_opt, void* cuda_stream);
+
 /* Measures this device's FP32 FMA throughput with a register-resident loop (16 independent chains per thread,
  * 8 blocks of 256 threads per SM, best of 4 timed launches, ~1 ms each; waits): the denominator of the compositing
  * kernels' roofline.  tflops: HOST double. */

@@ -282,6 +282,15 @@ int sgs_mapping_loss(sgs_ctx* c, const sgs_camera* cam, const sgs_images* ren, c
                                    (cudaStream_t)stream) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
 }
 
+int sgs_map_correction(sgs_ctx* c, int64_t n, float* mean, float* quat, const int32_t* frame_id, int n_frames,
+                       const float* T_orig, const float* T_opt, void* stream) {
+    if (!c || n < 0 || n_frames < 0) return SGS_INVALID_ARGUMENT;
+    if (n > 0 && (!mean || !quat || !frame_id || (n_frames > 0 && (!T_orig || !T_opt)))) return SGS_INVALID_ARGUMENT;
+    if (reinterpret_cast<uintptr_t>(quat) & 15u) return SGS_INVALID_ARGUMENT;
+    return sgs_launch_map_correction(c, n, mean, quat, frame_id, n_frames, T_orig, T_opt, (cudaStream_t)stream) == cudaSuccess
+               ? SGS_OK : SGS_CUDA_ERROR;
+}
+
 int sgs_measure_fp32_peak(double* tflops, void* stream) {
     if (!tflops) return SGS_INVALID_ARGUMENT;
     return sgs_launch_fma_peak(tflops, (cudaStream_t)stream) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;

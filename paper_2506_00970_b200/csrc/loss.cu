@@ -282,3 +282,86 @@ cudaError_t sgs_launch_fma_peak(double* tflops, cudaStream_t s) {
     *tflops = best;
     return cudaGetLastError();
 }
+
+// ---- map correction after pose-graph optimisation (Eq. 31-32) ----
+// Delta T_f = T_f^o T_f^{-1}; mu' = Delta T_f mu, R' = Delta R_f R for the splat's closest observed keyframe f.
+// k_pose_increments: one thread per keyframe (Delta R, Delta t, q_Delta -> 64 B); k_map_correction: one thread per splat,
+// in place, HBM-bound (32 B read + 28 B written per splat; the 64-byte increments sit in L2).
+// The rotation is applied to the stored quaternion as q' = q_Delta (x) q  (|q'| = |q|: R(q'/|q'|) = Delta R R(q/|q|)).
+namespace {
+// one thread per keyframe: Delta R (9), Delta t (3) and Delta R as a unit quaternion (4) -> 16 floats per frame
+__global__ void k_pose_increments(int n_frames, const float* __restrict__ T_orig, const float* __restrict__ T_opt,
+                                  float4* __restrict__ inc) {
+    const int f = blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= n_frames) return;
+    float A[12], B[12];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) { A[k] = T_orig[12 * f + k]; B[k] = T_opt[12 * f + k]; }
+    // Delta R = R_o R^T, Delta t = t_o - Delta R t   (T^{-1} = [R^T | -R^T t])
+    float D[9], dt[3];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) D[3 * r + c] = B[4 * r] * A[4 * c] + B[4 * r + 1] * A[4 * c + 1] + B[4 * r + 2] * A[4 * c + 2];
+#pragma unroll
+    for (int r = 0; r < 3; ++r) dt[r] = B[4 * r + 3] - (D[3 * r] * A[3] + D[3 * r + 1] * A[7] + D[3 * r + 2] * A[11]);
+    // Delta R -> unit quaternion (largest-component branch)
+    float qw, qx, qy, qz;
+    const float tr = D[0] + D[4] + D[8];
+    if (tr > 0.f) {
+        const float s = sqrtf(tr + 1.f) * 2.f;
+        qw = 0.25f * s; qx = (D[7] - D[5]) / s; qy = (D[2] - D[6]) / s; qz = (D[3] - D[1]) / s;
+    } else if (D[0] > D[4] && D[0] > D[8]) {
+        const float s = sqrtf(1.f + D[0] - D[4] - D[8]) * 2.f;
+        qw = (D[7] - D[5]) / s; qx = 0.25f * s; qy = (D[1] + D[3]) / s; qz = (D[2] + D[6]) / s;
+    } else if (D[4] > D[8]) {
+        const float s = sqrtf(1.f + D[4] - D[0] - D[8]) * 2.f;
+        qw = (D[2] - D[6]) / s; qx = (D[1] + D[3]) / s; qy = 0.25f * s; qz = (D[5] + D[7]) / s;
+    } else {
+        const float s = sqrtf(1.f + D[8] - D[0] - D[4]) * 2.f;
+        qw = (D[3] - D[1]) / s; qx = (D[2] + D[6]) / s; qy = (D[5] + D[7]) / s; qz = 0.25f * s;
+    }
+    inc[4 * f] = make_float4(D[0], D[1], D[2], dt[0]);
+    inc[4 * f + 1] = make_float4(D[3], D[4], D[5], dt[1]);
+    inc[4 * f + 2] = make_float4(D[6], D[7], D[8], dt[2]);
+    inc[4 * f + 3] = make_float4(qw, qx, qy, qz);
+}
+
+__global__ void __launch_bounds__(256)
+k_map_correction(long long n, float* __restrict__ mean, float* __restrict__ quat, const int* __restrict__ frame_id,
+                 int n_frames, const float4* __restrict__ inc) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int f = frame_id[i];
+        if (f < 0 || f >= n_frames) continue;   // no keyframe: left as it is
+        const float4 r0 = inc[4 * f], r1 = inc[4 * f + 1], r2 = inc[4 * f + 2], qd = inc[4 * f + 3];
+        const float m0 = mean[3 * i], m1 = mean[3 * i + 1], m2 = mean[3 * i + 2];
+        mean[3 * i] = r0.x * m0 + r0.y * m1 + r0.z * m2 + r0.w;
+        mean[3 * i + 1] = r1.x * m0 + r1.y * m1 + r1.z * m2 + r1.w;
+        mean[3 * i + 2] = r2.x * m0 + r2.y * m1 + r2.z * m2 + r2.w;
+        const float4 q = reinterpret_cast<const float4*>(quat)[i];   // (w, x, y, z);  q' = q_Delta (x) q
+        float4 o;
+        o.x = qd.x * q.x - qd.y * q.y - qd.z * q.z - qd.w * q.w;
+        o.y = qd.x * q.y + qd.y * q.x + qd.z * q.w - qd.w * q.z;
+        o.z = qd.x * q.z - qd.y * q.w + qd.z * q.x + qd.w * q.y;
+        o.w = qd.x * q.w + qd.y * q.z - qd.z * q.y + qd.w * q.x;
+        reinterpret_cast<float4*>(quat)[i] = o;
+    }
+}
+}  // namespace
+
+cudaError_t sgs_launch_map_correction(sgs_ctx* c, int64_t n, float* mean, float* quat, const int* frame_id, int n_frames,
+                                      const float* T_orig, const float* T_opt, cudaStream_t s) {
+    if (n == 0 || n_frames == 0) return cudaSuccess;
+    if (n_frames > c->inc_cap) {
+        if (c->pose_inc) sgs_ws_free(c, c->pose_inc, s);
+        c->pose_inc = (float*)sgs_ws_alloc(c, sizeof(float) * 16 * (size_t)n_frames, s);
+        if (!c->pose_inc) { c->inc_cap = 0; return cudaErrorMemoryAllocation; }
+        c->inc_cap = n_frames;
+    }
+    int blocks = (int)((n + 255) / 256);
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    c->launches += 2;
+    k_pose_increments<<<(n_frames + 127) / 128, 128, 0, s>>>(n_frames, T_orig, T_opt, reinterpret_cast<float4*>(c->pose_inc));
+    k_map_correction<<<blocks, 256, 0, s>>>((long long)n, mean, quat, frame_id, n_frames, reinterpret_cast<const float4*>(c->pose_inc));
+    return cudaGetLastError();
+}

@@ -86,6 +86,7 @@ struct sgs_ctx {
     uint32_t* tile_order;            // tiles: tile ids by descending entry count (longest first), written by K-pre-B
     uint32_t* render_order;          // tiles: longest-first order of the last sgs_render's tiles (by entry count), or unused
     bool render_order_valid;
+    float* pose_inc; int inc_cap;    // per-keyframe increments of sgs_map_correction (16 floats each)
     unsigned int* covis_cnt;         // 4 counters of k_covisibility (cudaMalloc, lazily)
     float* contrib_out;              // sgs_render_contrib: per-splat contribution output of the current forward, or NULL
     int64_t cursor_cap;              // tiles the cursor / tile_order arrays hold
@@ -153,6 +154,8 @@ cudaError_t sgs_launch_mapping_loss(sgs_ctx* c, const sgs_camera* cam, const flo
                                     const float* tdepth, float lambda_c, float w_d, float w_n, float nsign, float* const up[8],
                                     float* loss, cudaStream_t s);
 cudaError_t sgs_launch_fma_peak(double* tflops, cudaStream_t s);
+cudaError_t sgs_launch_map_correction(sgs_ctx* c, int64_t n, float* mean, float* quat, const int* frame_id, int n_frames,
+                                      const float* T_orig, const float* T_opt, cudaStream_t s);
 cudaError_t sgs_launch_export_idx(sgs_ctx* c, cudaStream_t s);
 cudaError_t sgs_launch_backward_tracking(sgs_ctx* c, const float* trgb, const float* tdepth, float lambda_d, float nsign,
                                          float* d_pose6, float* loss, cudaStream_t s);
