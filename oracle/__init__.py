@@ -285,3 +285,39 @@ def map_correction(mean, quat, frame_id, T_orig, T_opt):
     mu2 = np.einsum("nij,nj->ni", dT[f, :3, :3], mu) + dT[f, :3, 3]      # Eq. 32
     R2 = np.einsum("nij,njk->nik", dT[f, :3, :3], quat_to_matrix(quat))
     return mu2, R2
+
+
+def ssim_window(size=11, sigma=1.5):
+    """The normalised Gaussian window of SSIM [87] (11 x 11, sigma 1.5), as a 1-D kernel; the 2-D window is its outer product."""
+    x = np.arange(size, dtype=np.float64) - (size - 1) / 2.0
+    g = np.exp(-x * x / (2.0 * sigma * sigma))
+    return g / g.sum()
+
+
+def ssim_loss(rgb_r, rgb_t, weight):
+    """SSIM term of Eq. 24 (L236-238), reading R24: per channel the structural similarity index of [87]
+    with the 11 x 11 Gaussian window (sigma 1.5), zero padding, C1 = 0.01^2, C2 = 0.03^2 (unit dynamic range);
+    L_SSIM(p) = 1 - mean_c SSIM_c(p);  returns (weight/|Omega| sum_p L_SSIM(p), d/d rgb_r of that (3,H,W)), fp64."""
+    from scipy.signal import convolve2d
+    x = np.asarray(rgb_r, dtype=np.float64); y = np.asarray(rgb_t, dtype=np.float64)
+    Cn, H, W = x.shape
+    g = ssim_window()
+    win = np.outer(g, g)
+    conv = lambda a: convolve2d(a, win, mode="same", boundary="fill", fillvalue=0.0)
+    C1, C2 = 0.01 ** 2, 0.03 ** 2
+    L = 0.0
+    grad = np.zeros_like(x)
+    G = -weight / (Cn * H * W)          # dL/dSSIM_c(p)
+    for c in range(Cn):
+        mu1, mu2 = conv(x[c]), conv(y[c])
+        e11, e22, e12 = conv(x[c] * x[c]), conv(y[c] * y[c]), conv(x[c] * y[c])
+        s1, s2, s12 = e11 - mu1 * mu1, e22 - mu2 * mu2, e12 - mu1 * mu2
+        a1, a2 = 2 * mu1 * mu2 + C1, 2 * s12 + C2
+        b1, b2 = mu1 * mu1 + mu2 * mu2 + C1, s1 + s2 + C2
+        S = a1 * a2 / (b1 * b2)
+        L += weight * (1.0 - S).sum() / (Cn * H * W)
+        dS_dmu1 = 2 * mu2 * (a2 - a1) / (b1 * b2) - S * (2 * mu1 / b1 - 2 * mu1 / b2)
+        dS_de11 = -S / b2
+        dS_de12 = 2 * a1 / (b1 * b2)
+        grad[c] = conv(G * dS_dmu1) + 2 * x[c] * conv(G * dS_de11) + y[c] * conv(G * dS_de12)
+    return float(L), grad

@@ -565,3 +565,39 @@ def test_p14_map_correction_moves_splats_rigidly_with_their_keyframe():
     np.testing.assert_allclose(mu3, mean, atol=1e-12); np.testing.assert_allclose(R3, R, atol=1e-12)
     a, b = np.nonzero(fid == fid[0])[0][:2]
     assert abs(np.linalg.norm(mu2[a] - mu2[b]) - np.linalg.norm(mean[a] - mean[b])) < 1e-10
+
+
+# ---------------------------------------------------------------- P15: SSIM term of Eq. 24
+def test_p15_ssim_closed_forms_brute_force_and_gradient():
+    g = scenegen.SplitMix(15)
+    H, W = 17, 23
+    x = g.uniform(3 * H * W).reshape(3, H, W); y = np.clip(x + 0.1 * g.normal(3 * H * W).reshape(3, H, W), 0, 1)
+    # identical images: SSIM = 1 everywhere -> loss 0, gradient 0
+    L, gr = oracle.ssim_loss(x, x, 0.125)
+    assert abs(L) < 1e-14 and np.abs(gr).max() < 1e-12
+    # constant images (far from the zero-padded border): SSIM = (2 c1 c2 + C1) / (c1^2 + c2^2 + C1), variances are 0
+    c1, c2 = 0.3, 0.7
+    Lc, _ = oracle.ssim_loss(np.full((1, 41, 41), c1), np.full((1, 41, 41), c2), 1.0)
+    s_int = (2 * c1 * c2 + 1e-4) / (c1 * c1 + c2 * c2 + 1e-4)
+    big = np.full((1, 41, 41), c1); bigy = np.full((1, 41, 41), c2)
+    # interior pixel value through the brute-force definition below
+    def ssim_at(xx, yy, j, i):
+        w1 = oracle.ssim_window(); acc = dict(m1=0, m2=0, e11=0, e22=0, e12=0)
+        for dj in range(-5, 6):
+            for di in range(-5, 6):
+                jj, ii = j + dj, i + di
+                if 0 <= jj < xx.shape[0] and 0 <= ii < xx.shape[1]:
+                    ww = w1[dj + 5] * w1[di + 5]; a, b = xx[jj, ii], yy[jj, ii]
+                    acc["m1"] += ww * a; acc["m2"] += ww * b; acc["e11"] += ww * a * a; acc["e22"] += ww * b * b; acc["e12"] += ww * a * b
+        m1, m2 = acc["m1"], acc["m2"]; s1, s2, s12 = acc["e11"] - m1 * m1, acc["e22"] - m2 * m2, acc["e12"] - m1 * m2
+        return (2 * m1 * m2 + 1e-4) * (2 * s12 + 9e-4) / ((m1 * m1 + m2 * m2 + 1e-4) * (s1 + s2 + 9e-4))
+    assert abs(ssim_at(big[0], bigy[0], 20, 20) - s_int) < 1e-12
+    # loss = mean over pixels and channels of 1 - SSIM, against the brute-force window sums (incl. border pixels)
+    L, gr = oracle.ssim_loss(x, y, 0.2)
+    brute = np.mean([[1 - ssim_at(x[c], y[c], j, i) for j in range(H) for i in range(W)] for c in range(3)])
+    assert abs(L - 0.2 * brute) < 1e-12
+    # gradient = central finite differences
+    for c, j, i in [(0, 0, 0), (1, 8, 11), (2, 16, 22), (0, 5, 1), (1, 3, 19), (2, 10, 4)]:
+        d = np.zeros_like(x); d[c, j, i] = 1e-6
+        fd = (oracle.ssim_loss(x + d, y, 0.2)[0] - oracle.ssim_loss(x - d, y, 0.2)[0]) / 2e-6
+        assert abs(fd - gr[c, j, i]) <= 1e-6 * abs(gr[c, j, i]) + 1e-11
