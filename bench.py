@@ -185,8 +185,9 @@ class Workload:
             self.ren.render_contrib(self.sf, cam, self.contrib_buf, **self.im)
         else:
             self.ren.render(self.sf, cam, **self.im)
-        # mapping iteration: Eq. 24-26 (lambda_c, w_d, w_n of Tab. I; SSIM term not built) -> upstream of all planes
+        # mapping iteration: Eq. 24-26 with Tab. I's lambda_c, w_d, w_n -> upstream gradients of all planes
         self.ren.mapping_loss(cam, self.im, trgb, tdep, 0.875, 0.5, 0.02, -1.0, self.up, self.loss)
+        self.ren.ssim_loss(self.im["rgb"], trgb, 0.125, self.up["rgb"], self.loss)   # + (1 - lambda_c) L_SSIM: Eq. 24 complete
         u = self.up
         if True:
             self.ren.backward(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"],
@@ -402,7 +403,7 @@ def main():
         work = dict(preprocess=("hbm", (sc.n if sc.active is not None else 0) + n_act * 56 + cnt["n_vis"] * 76 + E * 12),
                     sort=("hbm", E * 24 + E * 8),
                     forward=("alu", F_TEST * cnt["Q_t"] + F_COMP_FWD * cnt["Q_c"]),
-                    loss=("hbm", px * (12 + 8) * 4),
+                    loss=("hbm", px * (12 + 8) * 4 + (0 if wl.tracking else px * 3 * 4 * 12)),
                     backward=("alu", F_TEST * cnt["Q_tb"] + fcb * cnt["Q_c"]),
                     # sgs_track_iter's single kernel: forward + pose-only backward of the same view
                     track=("alu", F_TEST * (cnt["Q_t"] + cnt["Q_tb"]) + (F_COMP_FWD + F_COMP_BWD_POSE) * cnt["Q_c"]))
@@ -426,7 +427,7 @@ def main():
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
                 surfels_per_s=wl.n_active * renders / (ms_max * 1e-3),
                 config=dict(workload=f"{args.config} ({'tracking' if wl.tracking else 'mapping'}-shaped): "
-                            f"{wl.renders_per_step} x (render + {'Eq.15-19' if wl.tracking else 'Eq.24-26 (no SSIM)'} loss + "
+                            f"{wl.renders_per_step} x (render + {'Eq.15-19' if wl.tracking else 'Eq.24-26'} loss + "
                             f"{'pose-only' if wl.tracking else 'full+pose'} backward) per step",
                             surfels=wl.sc.n, active=wl.n_active, width=wl.W, height=wl.H, renders_per_step=wl.renders_per_step,
                             l2="flushed between steps by a 256 MiB write; iterations inside a step reuse the map as tracking does",

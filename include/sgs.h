@@ -233,6 +233,15 @@ SGS_API int sgs_upload_target(sgs_ctx* ctx, const sgs_camera* cam, const float* 
 SGS_API int sgs_track_iter_host(sgs_ctx* ctx, const sgs_camera* cam, float lambda_d, float normal_sign,
                         float* host_loss, float* host_d_pose6, void* cuda_stream);
 
+/* SSIM term of the colour loss (Eq. 24; reading R24): per channel the structural similarity index of [87],
+ * 11 x 11 Gaussian window (sigma 1.5), zero padding, C1 = 0.01^2, C2 = 0.03^2;
+ *   L = weight / (3 |Omega|) sum_c sum_p (1 - SSIM_c(p)).
+ * ACCUMULATES: dL/d(rendered rgb) is added to upstream_rgb and L to *loss, so that it composes with
+ * sgs_mapping_loss (call that first; Eq. 24's weights: sgs_mapping_loss(lambda_c, ...) then sgs_ssim_loss(1 - lambda_c)).
+ *   rendered_rgb, target_rgb, upstream_rgb: DEVICE 3 x H x W;  loss: DEVICE 1 float, nullable. */
+SGS_API int sgs_ssim_loss(sgs_ctx* ctx, int width, int height, const float* rendered_rgb, const float* target_rgb,
+                          float weight, float* upstream_rgb, float* loss, void* cuda_stream);
+
 /* Map correction after pose-graph optimisation (Eq. 31-32), in place: Delta T_f = T_f^o T_f^{-1} and
  * mu_k <- Delta T_f mu_k, R_k <- Delta R_f R_k with f = frame_id[k], the splat's closest observed keyframe.
  *   mean (n x 3), quat (n x 4, (w,x,y,z), 16-byte aligned), frame_id (n x int32; ids outside [0, n_frames) leave the

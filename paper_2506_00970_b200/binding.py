@@ -51,7 +51,7 @@ class sgs_stats(C.Structure):
 
 
 EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_backward", "sgs_tracking_loss",
-           "sgs_backward_tracking", "sgs_track_iter", "sgs_render_contrib", "sgs_covisibility", "sgs_mapping_loss", "sgs_map_correction", "sgs_measure_fp32_peak", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
+           "sgs_backward_tracking", "sgs_track_iter", "sgs_render_contrib", "sgs_covisibility", "sgs_mapping_loss", "sgs_ssim_loss", "sgs_map_correction", "sgs_measure_fp32_peak", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
            "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string"]
 
 _lib = None
@@ -237,6 +237,12 @@ class Renderer:
         _check(self.lib.sgs_mapping_loss(self._ctx, C.byref(cam), C.byref(r), C.byref(t), C.c_float(lambda_c), C.c_float(w_d),
                                          C.c_float(w_n), C.c_float(normal_sign), C.byref(u), _ptr(loss), _stream_ptr(stream)),
                "sgs_mapping_loss")
+
+    def ssim_loss(self, rendered_rgb, target_rgb, weight, upstream_rgb, loss=None, stream=None):
+        """sgs_ssim_loss (SSIM term of Eq. 24): ACCUMULATES into upstream_rgb and loss."""
+        H, W = rendered_rgb.shape[-2], rendered_rgb.shape[-1]
+        _check(self.lib.sgs_ssim_loss(self._ctx, C.c_int(W), C.c_int(H), _ptr(rendered_rgb), _ptr(target_rgb),
+                                      C.c_float(weight), _ptr(upstream_rgb), _ptr(loss), _stream_ptr(stream)), "sgs_ssim_loss")
 
     def map_correction(self, mean, quat, frame_id, T_orig, T_opt, stream=None):
         """sgs_map_correction (Eq. 31-32), in place on mean / quat."""

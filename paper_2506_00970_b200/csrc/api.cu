@@ -219,7 +219,7 @@ int sgs_destroy(sgs_ctx* c) {
                     c->pay.g5, c->pay.g6, c->pay.g7, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
                     c->sort_state, c->ranges, c->T_final, c->n_last, c->img_scratch, c->pose_partial, c->resident_store,
                     c->resident_active, c->target_rgb, c->host_img_dev, c->host_up_dev, c->host_grads_dev,
-                    c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->pose_inc, c->export_keys, c->export_ranges};
+                    c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->pose_inc, c->ssim_maps, c->export_keys, c->export_ranges};
     for (void* p : ptrs) sgs_ws_free(c, p, s);
     if (c->counters) cudaFree(c->counters);
     if (c->counters_snap) cudaFree(c->counters_snap);

@@ -282,6 +282,13 @@ int sgs_mapping_loss(sgs_ctx* c, const sgs_camera* cam, const sgs_images* ren, c
                                    (cudaStream_t)stream) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
 }
 
+int sgs_ssim_loss(sgs_ctx* c, int width, int height, const float* rendered_rgb, const float* target_rgb, float weight,
+                  float* upstream_rgb, float* loss, void* stream) {
+    if (!c || width <= 0 || height <= 0 || !rendered_rgb || !target_rgb || !upstream_rgb) return SGS_INVALID_ARGUMENT;
+    return sgs_launch_ssim_loss(c, width, height, rendered_rgb, target_rgb, weight, upstream_rgb, loss,
+                                (cudaStream_t)stream) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
+}
+
 int sgs_map_correction(sgs_ctx* c, int64_t n, float* mean, float* quat, const int32_t* frame_id, int n_frames,
                        const float* T_orig, const float* T_opt, void* stream) {
     if (!c || n < 0 || n_frames < 0) return SGS_INVALID_ARGUMENT;

@@ -86,6 +86,7 @@ struct sgs_ctx {
     uint32_t* tile_order;            // tiles: tile ids by descending entry count (longest first), written by K-pre-B
     uint32_t* render_order;          // tiles: longest-first order of the last sgs_render's tiles (by entry count), or unused
     bool render_order_valid;
+    float* ssim_maps; int64_t ssim_cap;  // 9 derivative planes of sgs_ssim_loss
     float* pose_inc; int inc_cap;    // per-keyframe increments of sgs_map_correction (16 floats each)
     unsigned int* covis_cnt;         // 4 counters of k_covisibility (cudaMalloc, lazily)
     float* contrib_out;              // sgs_render_contrib: per-splat contribution output of the current forward, or NULL
@@ -154,6 +155,8 @@ cudaError_t sgs_launch_mapping_loss(sgs_ctx* c, const sgs_camera* cam, const flo
                                     const float* tdepth, float lambda_c, float w_d, float w_n, float nsign, float* const up[8],
                                     float* loss, cudaStream_t s);
 cudaError_t sgs_launch_fma_peak(double* tflops, cudaStream_t s);
+cudaError_t sgs_launch_ssim_loss(sgs_ctx* c, int W, int H, const float* rgb_r, const float* rgb_t, float weight, float* up_rgb,
+                                 float* loss, cudaStream_t s);
 cudaError_t sgs_launch_map_correction(sgs_ctx* c, int64_t n, float* mean, float* quat, const int* frame_id, int n_frames,
                                       const float* T_orig, const float* T_opt, cudaStream_t s);
 cudaError_t sgs_launch_export_idx(sgs_ctx* c, cudaStream_t s);
