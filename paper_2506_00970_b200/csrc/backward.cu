@@ -26,34 +26,8 @@ constexpr int BWD_K = 2;  // entries per trip of the reverse walk
 struct StagedBwd {
     float4 s0, s1, s2, s3, s4;  // as StagedFwd
     float4 s5;                  // a_u.xyz, a_v.x
-    float4 s6;                  // a_v.yz, m.xy      (m = a_u x a_v)
-    float4 s7;                  // m.z, bits(v), -, -
+    float4 s6;                  // a_v.yz, m.xy      (m = a_u x a_v); m.z rides in s4.w
 };
-
-// Transposed butterfly: 16 per-lane values -> lane l ends with the warp-wide sum of value (l>>1)&15.
-__device__ __forceinline__ float reduce16_transposed(float (&x)[16], int lane) {
-    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4, b1 = lane & 2;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const float send = b4 ? x[i] : x[i + 8], keep = b4 ? x[i + 8] : x[i];
-        x[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-    }
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const float send = b3 ? x[i] : x[i + 4], keep = b3 ? x[i + 4] : x[i];
-        x[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-    }
-#pragma unroll
-    for (int i = 0; i < 2; ++i) {
-        const float send = b2 ? x[i] : x[i + 2], keep = b2 ? x[i + 2] : x[i];
-        x[i] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-    }
-    {
-        const float send = b1 ? x[0] : x[1], keep = b1 ? x[1] : x[0];
-        x[0] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
-    }
-    return x[0] + __shfl_xor_sync(0xffffffffu, x[0], 1);
-}
 
 // FUSED (pose-only only): `up` holds the RENDERED planes of the last forward and the upstream gradients of the
 // tracking loss (Eq. 15-19, same arithmetic as loss.cu) are formed in registers -- no loss kernel, no
@@ -69,6 +43,9 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
            FusedLoss fl) {
     __shared__ StagedBwd sh[SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
+    __shared__ uint32_t sh_v[SGS_BLOCK];  // surfel (accumulator) index of each staged entry
+    // full mode: per-warp scratch of the 16-value reduction, [value][lane] with rows padded to 36 words
+    __shared__ float red_s[POSE_ONLY ? 1 : 8 * 16 * 36];
     __shared__ float s_red[8][7];
     const int tile = tile_order ? (int)tile_order[blockIdx.x] : (int)blockIdx.x;  // longest tiles first
     const int tx = tile % tiles_x, ty = tile / tiles_x;
@@ -146,12 +123,14 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
             StagedBwd st;
             stage_entry(g0, g1, g2, g3, px0, py0, st.s0, st.s1, st.s2);
             st.s3 = make_float4(g1.w, g3.w, g4.x, g4.y);
-            st.s4 = make_float4(g4.z, g4.w, g5.x, 0.f);
+            st.s4 = make_float4(g4.z, g4.w, g5.x, 0.f);  // .w <- m.z below
             const float aux = g5.y, auy = g5.z, auz = g5.w, avx = g6.x, avy = g6.y, avz = g6.z;
             st.s5 = make_float4(aux, auy, auz, avx);
             st.s6 = make_float4(avy, avz, auy * avz - auz * avy, auz * avx - aux * avz);
-            st.s7 = make_float4(aux * avy - auy * avx, __uint_as_float(v), 0.f, 0.f);
+            st.s4.w = aux * avy - auy * avx;
+            sh_v[tid] = v;
             sh[tid] = st;
+            pmask = refine_patch_mask(pmask, st.s0, st.s1, st.s2, g1.w, cfg.cutoff2, cfg.alpha_min);
         }
         sh_mask[tid] = (unsigned char)pmask;
         __syncthreads();
@@ -205,13 +184,13 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
             for (int k = 0; k < BWD_K; ++k) {
                 if (!__any_sync(0xffffffffu, hit[k])) continue;
                 const int j = jj[k];
-                const float4 s4 = sh[j].s4, s5 = sh[j].s5, s6 = sh[j].s6, s7 = sh[j].s7;
+                const float4 s4 = sh[j].s4, s5 = sh[j].s5, s6 = sh[j].s6;
                 const bool clamped = opac[k] * r[k].G > cfg.alpha_max;  // R5: true derivative, zero when clamped
                 const float dG = clamped ? 0.f : da[k] * opac[k];
                 const float gu = -r[k].u * r[k].G * dG, gvv = -r[k].v * r[k].G * dG, gz = g[3] * w[k];
                 // f = [ r x (a_v gu - a_u gv) + m gz ] / (r . m)
                 const float q0 = s5.w * gu - s5.x * gvv, q1 = s6.x * gu - s5.y * gvv, q2 = s6.y * gu - s5.z * gvv;
-                const float m0 = s6.z, m1 = s6.w, m2 = s7.x;
+                const float m0 = s6.z, m1 = s6.w, m2 = s4.w;
                 const float inv_rm = fast_rcp(rx * m0 + ry * m1 + m2);
                 // a rejected pair may carry inf / NaN: its lanes contribute exact zeros
                 const float f0 = hit[k] ? (ry * q2 - q1 + m0 * gz) * inv_rm : 0.f;
@@ -230,11 +209,21 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
                     x[9] = w[k] * g[4]; x[10] = w[k] * g[5]; x[11] = w[k] * g[6];
                     x[12] = w[k] * g[0]; x[13] = w[k] * g[1]; x[14] = w[k] * g[2];
                     x[15] = (clamped || !hit[k]) ? 0.f : da[k] * r[k].G;
-                    const float red = reduce16_transposed(x, lane);
-                    if ((lane & 1) == 0) {
-                        const uint32_t v = __float_as_uint(sh[j].s7.y);
-                        atomicAdd(acc + (size_t)v * SGS_ACC_STRIDE + (lane >> 1), red);
-                    }
+                    // Sum of the 16 values over the warp through shared memory (ncu: the register butterfly -- 16 SHFL,
+                    // 30 SEL, 16 FADD -- was 32 % of this kernel's instructions; removing it altogether saved 95 us per
+                    // C3/C4 view): every lane stores its 16 values transposed (conflict-free), then lane l adds 16 of the
+                    // 32 entries of row l & 15 (four LDS.128, conflict-free per quarter-warp thanks to the 36-word
+                    // rows) and one shuffle joins the two halves; the shuffle is also the barrier before the next store.
+                    float* rs = red_s + wid * (16 * 36);
+#pragma unroll
+                    for (int q = 0; q < 16; ++q) rs[q * 36 + lane] = x[q];
+                    __syncwarp();
+                    const float4* rp = reinterpret_cast<const float4*>(rs + (lane & 15) * 36 + (lane >> 4) * 16);
+                    const float4 v0 = rp[0], v1 = rp[1], v2 = rp[2], v3 = rp[3];
+                    float red = (((v0.x + v0.y) + (v0.z + v0.w)) + ((v1.x + v1.y) + (v1.z + v1.w))) +
+                                (((v2.x + v2.y) + (v2.z + v2.w)) + ((v3.x + v3.y) + (v3.z + v3.w)));
+                    red += __shfl_xor_sync(0xffffffffu, red, 16);
+                    if (lane < 16) atomicAdd(acc + (size_t)sh_v[j] * SGS_ACC_STRIDE + lane, red);
                 }
             }
           }

@@ -90,7 +90,8 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
             sh[0][tid] = s0; sh[1][tid] = s1; sh[2][tid] = s2;
             sh[3][tid] = make_float4(g1.w, g3.w, g4.x, g4.y);
             sh[4][tid] = make_float4(g4.z, g4.w, g5.x, __uint_as_float(v));
-            mask = warp_patch_mask(g7, (float)(tx * SGS_TILE), (float)(ty * SGS_TILE));
+            mask = refine_patch_mask(warp_patch_mask(g7, (float)(tx * SGS_TILE), (float)(ty * SGS_TILE)), s0, s1, s2, g1.w,
+                                     cfg.cutoff2, cfg.alpha_min);
         }
         sh_mask[tid] = (unsigned char)mask;
         __syncthreads();

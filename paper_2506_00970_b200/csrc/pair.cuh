@@ -89,6 +89,46 @@ __device__ __forceinline__ unsigned warp_patch_mask(const float4 bb, const float
     return m;
 }
 
+// Second, exact stage of the warp-patch mask.  With the staged rows a = (P, Q, U0), b = (R, S, V0), c = (E', F', D0)
+// and p = (lx, ly, 1), rho^2 = ((a.p)^2 + (b.p)^2) / (c.p)^2, so rho^2 <= k2 is the conic
+//   q(x, y) = (a.p)^2 + (b.p)^2 - k2 (c.p)^2 = A x^2 + 2 B x y + C y^2 + 2 D x + 2 E y + F <= 0.
+// k2 = min(cutoff^2, 2 ln(opacity / alpha_min)) also folds the alpha >= alpha_min test in (eval_pair).  Where q is
+// convex (the splat's footprint is an ellipse) its minimum over a patch's rectangle of pixel centres, grown by a
+// quarter pixel against rounding, is attained at the centre clamped onto the rectangle along one axis and
+// minimised along the other; a patch whose minimum is positive holds no pixel that eval_pair() accepts and loses its
+// bit.  Non-convex or badly conditioned conics (horizon through the tile, edge-on splats) keep the AABB answer.
+// Measured need: in C3 two of three (warp, entry) trips that passed the AABB mask found no lane that hits.
+__device__ __forceinline__ unsigned refine_patch_mask(const unsigned m, const float4 s0, const float4 s1, const float4 s2,
+                                                      const float opacity, const float cutoff2, const float alpha_min) {
+    const float ratio = opacity / alpha_min;
+    if (!(ratio >= 1.f)) return 0u;  // alpha < alpha_min everywhere (also NaN opacity)
+    const float k2 = fminf(cutoff2, fmaf(2.002f, __logf(ratio), 1e-3f));
+    const float a1 = s0.x, a2 = s0.y, a3 = s0.z, b1 = s1.x, b2 = s1.y, b3 = s1.z, c1 = s0.w, c2 = s1.w, c3 = s2.x;
+    const float kc1 = k2 * c1, kc2 = k2 * c2, kc3 = k2 * c3;
+    const float A = fmaf(a1, a1, fmaf(b1, b1, -kc1 * c1)), B = fmaf(a1, a2, fmaf(b1, b2, -kc1 * c2));
+    const float C = fmaf(a2, a2, fmaf(b2, b2, -kc2 * c2)), D = fmaf(a1, a3, fmaf(b1, b3, -kc1 * c3));
+    const float E = fmaf(a2, a3, fmaf(b2, b3, -kc2 * c3)), F = fmaf(a3, a3, fmaf(b3, b3, -kc3 * c3));
+    const float det = fmaf(A, C, -B * B);
+    if (!(A > 0.f && C > 0.f && det > 1e-4f * A * C)) return m;
+    const float idet = 1.f / det, nia = -1.f / A, nic = -1.f / C;
+    const float xc = (B * E - C * D) * idet, yc = (B * D - A * E) * idet;
+    const float B2 = B + B, D2 = D + D, E2 = E + E;
+    // rounding allowance: 32 ulp of the largest term q can hold inside the tile (|x|, |y| <= 16)
+    const float tol = 4e-6f * (fabsf(F) + 32.f * (fabsf(D) + fabsf(E)) + 256.f * (A + C + fabsf(B2)));
+    unsigned out = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+        const float x0 = (float)((w & 1) * 8) - 0.25f, x1 = x0 + 7.5f, y0 = (float)((w >> 1) * 4) - 0.25f, y1 = y0 + 3.5f;
+        const float X = fminf(fmaxf(xc, x0), x1), Y = fminf(fmaxf(yc, y0), y1);
+        const float ys = fminf(fmaxf(fmaf(B, X, E) * nic, y0), y1);   // argmin over y of q(X, y), clamped
+        const float xs = fminf(fmaxf(fmaf(B, Y, D) * nia, x0), x1);   // argmin over x of q(x, Y), clamped
+        const float q1 = fmaf(X, fmaf(A, X, fmaf(B2, ys, D2)), fmaf(ys, fmaf(C, ys, E2), F));
+        const float q2 = fmaf(xs, fmaf(A, xs, fmaf(B2, Y, D2)), fmaf(Y, fmaf(C, Y, E2), F));
+        out |= (fminf(q1, q2) <= tol) ? (1u << w) : 0u;
+    }
+    return m & out;
+}
+
 // Builds the staged record of entry `v` for the tile whose first pixel centre is (px0, py0).
 __device__ __forceinline__ void stage_entry(const float4 g0, const float4 g1, const double2 g2, const float4 g3,
                                             const double px0, const double py0, float4& s0, float4& s1, float4& s2) {

@@ -25,7 +25,7 @@ constexpr int TRK_K = 2;                     // entries per trip of the walks
 // One thread stages entry `v` of the tile: forward record (s0..s4; s4.w carries m.z) plus the backward's a_u, a_v and
 // m = a_u x a_v: 7 planes of float4.
 __device__ __forceinline__ unsigned stage_track(const SgsPayload& pay, uint32_t v, double px0, double py0, float tx0,
-                                                float ty0, float4 (*sh)[SGS_BLOCK], int tid) {
+                                                float ty0, float4 (*sh)[SGS_BLOCK], int tid, const SgsCfgDev& cfg) {
     const float4 g0 = pay.g0[v], g1 = pay.g1[v], g3 = pay.g3[v], g4 = pay.g4[v], g5 = pay.g5[v], g6 = pay.g6[v];
     const float4 g7 = pay.g7[v];
     const double2 g2 = pay.g2[v];
@@ -37,7 +37,7 @@ __device__ __forceinline__ unsigned stage_track(const SgsPayload& pay, uint32_t 
     sh[5][tid] = make_float4(aux, auy, auz, avx);
     sh[6][tid] = make_float4(avy, avz, auy * avz - auz * avy, auz * avx - aux * avz);
     sh[4][tid] = make_float4(g4.z, g4.w, g5.x, aux * avy - auy * avx);  // n_c.y, n_c.z (with g4.w), ..., m.z
-    return warp_patch_mask(g7, tx0, ty0);
+    return refine_patch_mask(warp_patch_mask(g7, tx0, ty0), s0, s1, s2, g1.w, cfg.cutoff2, cfg.alpha_min);
 }
 
 // (u, v) and rho^2 of one pair (pair.cuh's sequence)
@@ -264,7 +264,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
             for (uint32_t k = 0; k < n; ++k) rank += s_keys[k] < key ? 1u : 0u;
             if (mine) {
                 g[rank] = key;  // sorted list for sgs_get_binning
-                sh_mask[rank] = (unsigned char)stage_track(pay, (uint32_t)key, px0, py0, tx0, ty0, sh, (int)rank);
+                sh_mask[rank] = (unsigned char)stage_track(pay, (uint32_t)key, px0, py0, tx0, ty0, sh, (int)rank, cfg);
             }
         }
         __syncthreads();
@@ -298,7 +298,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
             const uint32_t nb = min((uint32_t)SGS_BLOCK, n - boff);
             unsigned mask = 0;
             // plain loads: the bucket may just have been rewritten by this block
-            if ((uint32_t)tid < nb) mask = stage_track(pay, (uint32_t)g[boff + tid], px0, py0, tx0, ty0, sh, tid);
+            if ((uint32_t)tid < nb) mask = stage_track(pay, (uint32_t)g[boff + tid], px0, py0, tx0, ty0, sh, tid, cfg);
             sh_mask[tid] = (unsigned char)mask;
             staged_b = (int)(boff / SGS_BLOCK);
             __syncthreads();
@@ -319,7 +319,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
             if (b != staged_b) {  // block-uniform
                 __syncthreads();  // previous batch fully consumed
                 unsigned mask = 0;
-                if ((uint32_t)tid < nb) mask = stage_track(pay, (uint32_t)g[boff + tid], px0, py0, tx0, ty0, sh, tid);
+                if ((uint32_t)tid < nb) mask = stage_track(pay, (uint32_t)g[boff + tid], px0, py0, tx0, ty0, sh, tid, cfg);
                 sh_mask[tid] = (unsigned char)mask;
                 staged_b = b;
                 __syncthreads();
