@@ -220,8 +220,13 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
                     __syncwarp();
                     const float4* rp = reinterpret_cast<const float4*>(rs + (lane & 15) * 36 + (lane >> 4) * 16);
                     const float4 v0 = rp[0], v1 = rp[1], v2 = rp[2], v3 = rp[3];
-                    float red = (((v0.x + v0.y) + (v0.z + v0.w)) + ((v1.x + v1.y) + (v1.z + v1.w))) +
-                                (((v2.x + v2.y) + (v2.z + v2.w)) + ((v3.x + v3.y) + (v3.z + v3.w)));
+                    // packed adds (FADD2: two binary32 sums per issue slot; the kernel is issue-bound): 7 + 1 instead of 15
+                    const float2 h0 = __fadd2_rn(__fadd2_rn(make_float2(v0.x, v0.y), make_float2(v0.z, v0.w)),
+                                                 __fadd2_rn(make_float2(v1.x, v1.y), make_float2(v1.z, v1.w)));
+                    const float2 h1 = __fadd2_rn(__fadd2_rn(make_float2(v2.x, v2.y), make_float2(v2.z, v2.w)),
+                                                 __fadd2_rn(make_float2(v3.x, v3.y), make_float2(v3.z, v3.w)));
+                    const float2 hs = __fadd2_rn(h0, h1);
+                    float red = hs.x + hs.y;
                     red += __shfl_xor_sync(0xffffffffu, red, 16);
                     if (lane < 16) atomicAdd(acc + (size_t)sh_v[j] * SGS_ACC_STRIDE + lane, red);
                 }

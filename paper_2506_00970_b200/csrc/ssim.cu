@@ -2,147 +2,226 @@
 // DESIGN.md): per channel the structural similarity index of [87] with the 11 x 11 Gaussian window (sigma 1.5),
 // zero padding, C1 = 0.01^2, C2 = 0.03^2;  L = weight / (3 |Omega|) sum_c sum_p (1 - SSIM_c(p)).
 //
-// Two kernels, one block per 16 x 16 output tile and channel, the 26 x 26 input tile (halo 5) staged in shared memory
-// and convolved separably there (11 taps across, then 11 taps down), so every input pixel crosses HBM once:
+// Two kernels of the same shape.  A block of 64 threads owns a strip 64 pixels wide and `rows` pixels tall of one
+// channel and marches down it one input row at a time: the row (64 + 10 halo pixels, zero outside the image) is
+// staged in shared memory by `cp.async`, three rows ahead; every thread takes the 11
+// taps ACROSS for its column from shared memory, and the 11 taps DOWN never leave registers: each finished row is
+// scattered with the window's weights into the 11 pending output rows' accumulators (a ring indexed statically by
+// unrolling the march 11-fold), and the row that has just received its last tap is emitted.
 //   k_ssim_forward : window sums of x, y, x^2, y^2, xy -> SSIM -> loss; writes the three derivative maps
 //                    G dS/dmu1, G dS/de11, G dS/de12  (G = dL/dSSIM = -weight / (3 |Omega|))
 //   k_ssim_backward: the same window over the three maps;  dL/dx = conv(m0) + 2 x conv(m1) + y conv(m2)  is ADDED to
 //                    the caller's upstream colour gradient (the window is symmetric: correlation = convolution).
+// The first version (16 x 16 output tiles, 26 x 26 inputs, both passes through shared memory) spent 99 shared-memory
+// accesses per output pixel and channel and ran 52 + 46 us at 1200 x 680; this one spends 12, and its arithmetic is
+// packed two binary32 lanes per instruction (FFMA2 / FMUL2 / FADD2: same flops per clock, half the issue slots).
 #include "sgs_internal.h"
 
 namespace {
 
-constexpr int SS_T = 16, SS_R = 5, SS_IN = SS_T + 2 * SS_R;  // 16 x 16 outputs, 26 x 26 inputs
-// Row strides chosen against bank conflicts: a warp works on two consecutive tile rows x 16 columns, so a stride of
-// 16 (mod 32) words puts its 32 accesses on 32 banks (ncu before: half of all shared-memory wavefronts were conflicts).
-constexpr int SS_IS = 48, SS_HS = 16;
-__constant__ float c_win[2 * SS_R + 1];
+constexpr int SB_W = 64, SS_R = 5, SS_TAPS = 2 * SS_R + 1, SB_IN = SB_W + 2 * SS_R, SB_ST = 4;  // 4 staged rows in flight
+__constant__ float c_win[SS_TAPS];
 
-__global__ void __launch_bounds__(SS_T * SS_T)
-k_ssim_forward(const float* __restrict__ xr, const float* __restrict__ yt, int W, int H, float G, float lscale,
+// 4-byte asynchronous global -> shared copy; `valid == false` writes a zero (the zero padding) without touching src
+__device__ __forceinline__ void cp_async4(void* dst, const float* src, bool valid) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst);
+    const int sz = valid ? 4 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(d), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait2() { asm volatile("cp.async.wait_group 2;" ::: "memory"); }
+
+__global__ void __launch_bounds__(SB_W)
+k_ssim_forward(const float* __restrict__ xr, const float* __restrict__ yt, int W, int H, int rows, float G, float lscale,
                float* __restrict__ maps /* 3 channels x 3 maps x HW */, float* __restrict__ slots /* 64 partial sums */) {
-    __shared__ float sx[SS_IN][SS_IS], sy[SS_IN][SS_IS];
-    __shared__ float hs[5][SS_IN][SS_HS];
-    __shared__ float s_part[8];
-    const int c = blockIdx.z, tid = threadIdx.x;
+    __shared__ float2 sxy[SB_ST][SB_IN + 2];  // (x, y) interleaved: one LDS.64 per tap feeds the packed FMAs
+    __shared__ float s_part[SB_W / 32];
+    const int c = blockIdx.z, tx = threadIdx.x;
     const size_t HW = (size_t)W * H;
     const float* x = xr + (size_t)c * HW;
     const float* y = yt + (size_t)c * HW;
-    const int x0 = blockIdx.x * SS_T - SS_R, y0 = blockIdx.y * SS_T - SS_R;
-    {   // 26 x 26 inputs by 16 x 16 threads: up to four (row, column) positions each, no division
-        const int tx = tid & 15, tyy = tid >> 4;
+    float* m = maps + (size_t)c * 3 * HW;
+    const int px = blockIdx.x * SB_W + tx, yb = blockIdx.y * rows, gx0 = blockIdx.x * SB_W - SS_R;
+    const int nrow = min(rows, H - yb), nin = nrow + 2 * SS_R;
+    const int gxa = gx0 + tx, gxb = gx0 + SB_W + tx;               // this thread's one or two columns of a staged row
+    const bool ina = gxa >= 0 && gxa < W, inb = gxb < W;
+    // running source pointers of this thread's column(s): one row further per issue_row() call
+    int gy_n = yb - SS_R;
+    const float* xa = x + (ptrdiff_t)gy_n * W + gxa;
+    const float* ya = y + (ptrdiff_t)gy_n * W + gxa;
+    auto issue_row = [&](int j) {  // input row j of the strip -> stage j % 4
+        if (j < nin) {
+            const bool rin = (unsigned)gy_n < (unsigned)H;
+            float2* d = sxy[j & (SB_ST - 1)];
+            cp_async4(&d[tx].x, (rin && ina) ? xa : x, rin && ina);
+            cp_async4(&d[tx].y, (rin && ina) ? ya : y, rin && ina);
+            if (tx < 2 * SS_R) {
+                cp_async4(&d[SB_W + tx].x, (rin && inb) ? xa + SB_W : x, rin && inb);
+                cp_async4(&d[SB_W + tx].y, (rin && inb) ? ya + SB_W : y, rin && inb);
+            }
+        }
+        cp_async_commit();
+        ++gy_n; xa += W; ya += W;
+    };
+    issue_row(0); issue_row(1); issue_row(2);
+    float2 w2[SS_TAPS];
 #pragma unroll
-        for (int j = 0; j < 2; ++j)
+    for (int t = 0; t < SS_TAPS; ++t) w2[t] = make_float2(c_win[t], c_win[t]);
+    float2 A01[SS_TAPS], A23[SS_TAPS];
+    float A4[SS_TAPS];
 #pragma unroll
-            for (int i = 0; i < 2; ++i) {
-                const int r = tyy + 16 * j, q = tx + 16 * i;
-                if (r < SS_IN && q < SS_IN) {
-                    const int gx = x0 + q, gy = y0 + r;
-                    const bool in = gx >= 0 && gx < W && gy >= 0 && gy < H;
-                    sx[r][q] = in ? x[(size_t)gy * W + gx] : 0.f;
-                    sy[r][q] = in ? y[(size_t)gy * W + gx] : 0.f;
+    for (int k = 0; k < SS_TAPS; ++k) { A01[k] = make_float2(0.f, 0.f); A23[k] = make_float2(0.f, 0.f); A4[k] = 0.f; }
+    float lsum = 0.f;
+    for (int j0 = 0; j0 < nin; j0 += SS_TAPS) {
+#pragma unroll
+        for (int s = 0; s < SS_TAPS; ++s) {
+            const int j = j0 + s;
+            if (j < nin) {  // block-uniform
+                cp_async_wait2();   // row j has landed (rows j+1, j+2 may still be in flight)
+                __syncthreads();    // ... for every thread; and stage (j+3) % 4, read at step j-1, is free again
+                issue_row(j + 3);
+                const int gy = yb - SS_R + j;
+                if (gy >= 0 && gy < H) {  // rows outside the image are zero padding: nothing to add
+                    const float2* row = sxy[j & (SB_ST - 1)] + tx;
+                    float2 h01 = make_float2(0.f, 0.f), h23 = make_float2(0.f, 0.f);
+                    float h4 = 0.f;
+#pragma unroll
+                    for (int t = 0; t < SS_TAPS; ++t) {  // 11 taps across: sums of x, y | x^2, y^2 | xy
+                        const float2 ab = row[t];
+                        const float2 wab = __fmul2_rn(w2[t], ab);
+                        h01 = __fadd2_rn(h01, wab);
+                        h23 = __ffma2_rn(wab, ab, h23);
+                        h4 = fmaf(wab.x, ab.y, h4);
+                    }
+#pragma unroll
+                    for (int t = 1; t < SS_TAPS; ++t) {  // 11 taps down: this row is tap t of output row j - t
+                        const int k = (s - t + SS_TAPS) % SS_TAPS;
+                        A01[k] = __ffma2_rn(w2[t], h01, A01[k]);
+                        A23[k] = __ffma2_rn(w2[t], h23, A23[k]);
+                        A4[k] = fmaf(w2[t].x, h4, A4[k]);
+                    }
+                    // tap 0 opens output row j in the slot that row j - 11 left at the previous step
+                    A01[s] = __fmul2_rn(w2[0], h01); A23[s] = __fmul2_rn(w2[0], h23); A4[s] = w2[0].x * h4;
+                } else {
+                    A01[s] = make_float2(0.f, 0.f); A23[s] = make_float2(0.f, 0.f); A4[s] = 0.f;
+                }
+                {   // output row j - 10 has all its taps
+                    const int k = (s + 1) % SS_TAPS, o = j - 2 * SS_R;
+                    if (o >= 0 && px < W) {
+                        const float mu1 = A01[k].x, mu2 = A01[k].y, e11 = A23[k].x, e22 = A23[k].y, e12 = A4[k];
+                        const float C1 = 1e-4f, C2 = 9e-4f;
+                        const float s1 = e11 - mu1 * mu1, s2 = e22 - mu2 * mu2, s12 = e12 - mu1 * mu2;
+                        const float a1 = 2.f * mu1 * mu2 + C1, a2 = 2.f * s12 + C2, b1 = mu1 * mu1 + mu2 * mu2 + C1, b2 = s1 + s2 + C2;
+                        const float ib = 1.f / (b1 * b2);  // b1, b2 > 0; 1/b1 = b2 ib and 1/b2 = b1 ib below
+                        const float S = a1 * a2 * ib;
+                        lsum += 1.f - S;
+                        float* mo = m + (size_t)(yb + o) * W + px;
+                        mo[0] = G * (2.f * ib * (mu2 * (a2 - a1) - S * mu1 * (b2 - b1)));  // G dS/dmu1
+                        mo[HW] = -G * S * b1 * ib;                                           // G dS/de11 = -G S / b2
+                        mo[2 * HW] = G * (2.f * a1 * ib);                                    // G dS/de12
+                    }
                 }
             }
-    }
-    __syncthreads();
-    for (int k = tid; k < SS_IN * SS_T; k += SS_T * SS_T) {  // 11 taps across
-        const int r = k / SS_T, q = k % SS_T;
-        float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, a4 = 0.f;
-#pragma unroll
-        for (int t = 0; t <= 2 * SS_R; ++t) {
-            const float w = c_win[t], a = sx[r][q + t], b = sy[r][q + t];
-            a0 = fmaf(w, a, a0); a1 = fmaf(w, b, a1); a2 = fmaf(w * a, a, a2); a3 = fmaf(w * b, b, a3); a4 = fmaf(w * a, b, a4);
         }
-        hs[0][r][q] = a0; hs[1][r][q] = a1; hs[2][r][q] = a2; hs[3][r][q] = a3; hs[4][r][q] = a4;
-    }
-    __syncthreads();
-    const int lx = tid % SS_T, ly = tid / SS_T, px = blockIdx.x * SS_T + lx, py = blockIdx.y * SS_T + ly;
-    float one_minus = 0.f;
-    if (px < W && py < H) {
-        float mu1 = 0.f, mu2 = 0.f, e11 = 0.f, e22 = 0.f, e12 = 0.f;
-#pragma unroll
-        for (int t = 0; t <= 2 * SS_R; ++t) {  // 11 taps down
-            const float w = c_win[t];
-            mu1 = fmaf(w, hs[0][ly + t][lx], mu1); mu2 = fmaf(w, hs[1][ly + t][lx], mu2);
-            e11 = fmaf(w, hs[2][ly + t][lx], e11); e22 = fmaf(w, hs[3][ly + t][lx], e22); e12 = fmaf(w, hs[4][ly + t][lx], e12);
-        }
-        const float C1 = 1e-4f, C2 = 9e-4f;
-        const float s1 = e11 - mu1 * mu1, s2 = e22 - mu2 * mu2, s12 = e12 - mu1 * mu2;
-        const float a1 = 2.f * mu1 * mu2 + C1, a2 = 2.f * s12 + C2, b1 = mu1 * mu1 + mu2 * mu2 + C1, b2 = s1 + s2 + C2;
-        const float ib = 1.f / (b1 * b2);
-        const float S = a1 * a2 * ib;
-        one_minus = 1.f - S;
-        const size_t pix = (size_t)py * W + px;
-        float* m = maps + (size_t)c * 3 * HW;
-        m[pix] = G * (2.f * mu2 * (a2 - a1) * ib - S * (2.f * mu1 / b1 - 2.f * mu1 / b2));  // G dS/dmu1
-        m[HW + pix] = G * (-S / b2);                                                          // G dS/de11
-        m[2 * HW + pix] = G * (2.f * a1 * ib);                                                // G dS/de12
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) one_minus += __shfl_xor_sync(0xffffffffu, one_minus, o);
-    if ((tid & 31) == 0) s_part[tid >> 5] = one_minus;
+    for (int o = 16; o > 0; o >>= 1) lsum += __shfl_xor_sync(0xffffffffu, lsum, o);
+    if ((tx & 31) == 0) s_part[tx >> 5] = lsum;
     __syncthreads();
-    if (tid == 0) {  // 64 slots instead of one address: ~10 k blocks would serialise on a single atomic
+    if (tx == 0) {  // 64 slots instead of one address: a thousand blocks would serialise on a single atomic
         float t = 0.f;
-        for (int w = 0; w < 8; ++w) t += s_part[w];
+#pragma unroll
+        for (int w = 0; w < SB_W / 32; ++w) t += s_part[w];
         atomicAdd(slots + ((blockIdx.x + 7 * blockIdx.y + 13 * blockIdx.z) & 63), t * lscale);
     }
 }
 
-__global__ void __launch_bounds__(SS_T * SS_T)
-k_ssim_backward(const float* __restrict__ xr, const float* __restrict__ yt, int W, int H, const float* __restrict__ maps,
-                float* __restrict__ up_rgb, float* __restrict__ slots, float* __restrict__ loss) {
-    __shared__ float sm[3][SS_IN][SS_IS];
-    __shared__ float hs[3][SS_IN][SS_HS];
-    const int c = blockIdx.z, tid = threadIdx.x;
-    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && tid < 32) {  // the forward's loss: 64 slots -> *loss, slots re-zeroed
-        float t = slots[tid] + slots[tid + 32];
-        slots[tid] = 0.f; slots[tid + 32] = 0.f;
+__global__ void __launch_bounds__(SB_W)
+k_ssim_backward(const float* __restrict__ xr, const float* __restrict__ yt, int W, int H, int rows,
+                const float* __restrict__ maps, float* __restrict__ up_rgb, float* __restrict__ slots, float* __restrict__ loss) {
+    __shared__ float2 s01[SB_ST][SB_IN + 2];  // maps 0 and 1 interleaved
+    __shared__ float s2[SB_ST][SB_IN + 2];
+    const int c = blockIdx.z, tx = threadIdx.x;
+    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && tx < 32) {  // the forward's loss: 64 slots -> *loss, slots re-zeroed
+        float t = slots[tx] + slots[tx + 32];
+        slots[tx] = 0.f; slots[tx + 32] = 0.f;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-        if (tid == 0 && loss) atomicAdd(loss, t);
+        if (tx == 0 && loss) atomicAdd(loss, t);
     }
     const size_t HW = (size_t)W * H;
     const float* m = maps + (size_t)c * 3 * HW;
-    const int x0 = blockIdx.x * SS_T - SS_R, y0 = blockIdx.y * SS_T - SS_R;
-    {
-        const int tx = tid & 15, tyy = tid >> 4;
-#pragma unroll
-        for (int j = 0; j < 2; ++j)
-#pragma unroll
-            for (int i = 0; i < 2; ++i) {
-                const int r = tyy + 16 * j, q = tx + 16 * i;
-                if (r < SS_IN && q < SS_IN) {
-                    const int gx = x0 + q, gy = y0 + r;
-                    const bool in = gx >= 0 && gx < W && gy >= 0 && gy < H;
-                    const size_t p = (size_t)gy * W + gx;
-                    sm[0][r][q] = in ? m[p] : 0.f; sm[1][r][q] = in ? m[HW + p] : 0.f; sm[2][r][q] = in ? m[2 * HW + p] : 0.f;
-                }
+    const int px = blockIdx.x * SB_W + tx, yb = blockIdx.y * rows, gx0 = blockIdx.x * SB_W - SS_R;
+    const int nrow = min(rows, H - yb), nin = nrow + 2 * SS_R;
+    const int gxa = gx0 + tx, gxb = gx0 + SB_W + tx;
+    const bool ina = gxa >= 0 && gxa < W, inb = gxb < W;
+    int gy_n = yb - SS_R;
+    const float* ma = m + (ptrdiff_t)gy_n * W + gxa;
+    auto issue_row = [&](int j) {
+        if (j < nin) {
+            const bool rin = (unsigned)gy_n < (unsigned)H;
+            const int st = j & (SB_ST - 1);
+            const float* pa = (rin && ina) ? ma : m;
+            cp_async4(&s01[st][tx].x, pa, rin && ina);
+            cp_async4(&s01[st][tx].y, pa + HW, rin && ina);
+            cp_async4(&s2[st][tx], pa + 2 * HW, rin && ina);
+            if (tx < 2 * SS_R) {
+                const float* pb = (rin && inb) ? ma + SB_W : m;
+                cp_async4(&s01[st][SB_W + tx].x, pb, rin && inb);
+                cp_async4(&s01[st][SB_W + tx].y, pb + HW, rin && inb);
+                cp_async4(&s2[st][SB_W + tx], pb + 2 * HW, rin && inb);
             }
-    }
-    __syncthreads();
-    for (int k = tid; k < SS_IN * SS_T; k += SS_T * SS_T) {
-        const int r = k / SS_T, q = k % SS_T;
-        float a0 = 0.f, a1 = 0.f, a2 = 0.f;
-#pragma unroll
-        for (int t = 0; t <= 2 * SS_R; ++t) {
-            const float w = c_win[t];
-            a0 = fmaf(w, sm[0][r][q + t], a0); a1 = fmaf(w, sm[1][r][q + t], a1); a2 = fmaf(w, sm[2][r][q + t], a2);
         }
-        hs[0][r][q] = a0; hs[1][r][q] = a1; hs[2][r][q] = a2;
-    }
-    __syncthreads();
-    const int lx = tid % SS_T, ly = tid / SS_T, px = blockIdx.x * SS_T + lx, py = blockIdx.y * SS_T + ly;
-    if (px < W && py < H) {
-        float c0 = 0.f, c1 = 0.f, c2 = 0.f;
+        cp_async_commit();
+        ++gy_n; ma += W;
+    };
+    issue_row(0); issue_row(1); issue_row(2);
+    float2 w2[SS_TAPS];
 #pragma unroll
-        for (int t = 0; t <= 2 * SS_R; ++t) {
-            const float w = c_win[t];
-            c0 = fmaf(w, hs[0][ly + t][lx], c0); c1 = fmaf(w, hs[1][ly + t][lx], c1); c2 = fmaf(w, hs[2][ly + t][lx], c2);
+    for (int t = 0; t < SS_TAPS; ++t) w2[t] = make_float2(c_win[t], c_win[t]);
+    float2 A01[SS_TAPS];
+    float A2[SS_TAPS];
+#pragma unroll
+    for (int k = 0; k < SS_TAPS; ++k) { A01[k] = make_float2(0.f, 0.f); A2[k] = 0.f; }
+    for (int j0 = 0; j0 < nin; j0 += SS_TAPS) {
+#pragma unroll
+        for (int s = 0; s < SS_TAPS; ++s) {
+            const int j = j0 + s;
+            if (j < nin) {
+                cp_async_wait2();
+                __syncthreads();
+                issue_row(j + 3);
+                // the output row that completes at this step: its pixel values are needed for the final combination
+                const int k = (s + 1) % SS_TAPS, o = j - 2 * SS_R;
+                const bool emit = o >= 0 && px < W;
+                const size_t pix = emit ? (size_t)c * HW + (size_t)(yb + o) * W + px : 0;
+                float xv = 0.f, yv = 0.f, uv = 0.f;
+                if (emit) { xv = xr[pix]; yv = yt[pix]; uv = up_rgb[pix]; }
+                const int gy = yb - SS_R + j;
+                if (gy >= 0 && gy < H) {
+                    const int st = j & (SB_ST - 1);
+                    const float2* r01 = s01[st] + tx;
+                    const float* r2 = s2[st] + tx;
+                    float2 h01 = make_float2(0.f, 0.f);
+                    float h2 = 0.f;
+#pragma unroll
+                    for (int t = 0; t < SS_TAPS; ++t) {
+                        h01 = __ffma2_rn(w2[t], r01[t], h01);
+                        h2 = fmaf(w2[t].x, r2[t], h2);
+                    }
+#pragma unroll
+                    for (int t = 1; t < SS_TAPS; ++t) {
+                        const int kk = (s - t + SS_TAPS) % SS_TAPS;
+                        A01[kk] = __ffma2_rn(w2[t], h01, A01[kk]);
+                        A2[kk] = fmaf(w2[t].x, h2, A2[kk]);
+                    }
+                    A01[s] = __fmul2_rn(w2[0], h01); A2[s] = w2[0].x * h2;  // tap 0 opens output row j in the freed slot
+                } else {
+                    A01[s] = make_float2(0.f, 0.f); A2[s] = 0.f;
+                }
+                if (emit) up_rgb[pix] = uv + (A01[k].x + 2.f * xv * A01[k].y + yv * A2[k]);
+            }
         }
-        const size_t pix = (size_t)py * W + px;
-        const float xv = xr[(size_t)c * HW + pix], yv = yt[(size_t)c * HW + pix];
-        up_rgb[(size_t)c * HW + pix] += c0 + 2.f * xv * c1 + yv * c2;
     }
 }
 
@@ -154,7 +233,7 @@ cudaError_t sgs_launch_ssim_loss(sgs_ctx* c, int W, int H, const float* rgb_r, c
     if (!win_set) {  // normalised Gaussian, sigma 1.5, evaluated in double and rounded once (as the oracle's)
         double g[2 * SS_R + 1], sum = 0.0;
         for (int t = 0; t <= 2 * SS_R; ++t) { const double d = t - SS_R; g[t] = exp(-d * d / (2.0 * 1.5 * 1.5)); sum += g[t]; }
-        float gf[2 * SS_R + 1];
+        float gf[SS_TAPS];
         for (int t = 0; t <= 2 * SS_R; ++t) gf[t] = (float)(g[t] / sum);
         const cudaError_t e = cudaMemcpyToSymbol(c_win, gf, sizeof(gf));
         if (e != cudaSuccess) return e;
@@ -172,9 +251,13 @@ cudaError_t sgs_launch_ssim_loss(sgs_ctx* c, int W, int H, const float* rgb_r, c
     float* slots = c->ssim_maps + c->ssim_cap;
     SgsStage st(c, SGS_STAGE_LOSS, s);
     c->launches += 2;
-    const dim3 grid((W + SS_T - 1) / SS_T, (H + SS_T - 1) / SS_T, 3);
+    // strip height: 10 halo rows are re-convolved per strip, so tall strips waste less, but the grid should still
+    // hold a few blocks per SM (2 warps each)
+    int rows = 68;
+    while (rows > 17 && (int64_t)((W + SB_W - 1) / SB_W) * ((H + rows - 1) / rows) * 3 < 148 * 6) rows = (rows + 1) / 2;
+    const dim3 grid((W + SB_W - 1) / SB_W, (H + rows - 1) / rows, 3);
     const float inv = 1.f / (3.f * (float)HW);
-    k_ssim_forward<<<grid, SS_T * SS_T, 0, s>>>(rgb_r, rgb_t, W, H, -weight * inv, weight * inv, c->ssim_maps, slots);
-    k_ssim_backward<<<grid, SS_T * SS_T, 0, s>>>(rgb_r, rgb_t, W, H, c->ssim_maps, up_rgb, slots, loss);
+    k_ssim_forward<<<grid, SB_W, 0, s>>>(rgb_r, rgb_t, W, H, rows, -weight * inv, weight * inv, c->ssim_maps, slots);
+    k_ssim_backward<<<grid, SB_W, 0, s>>>(rgb_r, rgb_t, W, H, rows, c->ssim_maps, up_rgb, slots, loss);
     return cudaGetLastError();
 }
