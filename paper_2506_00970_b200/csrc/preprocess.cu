@@ -302,7 +302,7 @@ k_pre_select(int64_t n, const float* __restrict__ mean, const float* __restrict_
     for (unsigned int k = tid; k < ns; k += SGS_PRE_BLOCK) surv_list[gb + k] = (uint32_t)(base + s_list[k]);
 }
 
-constexpr int SGS_PREB_BLOCK = 128, SGS_PREB_LOG2 = 7;  // K-pre-B block: small, so that few survivors still spread over the SMs
+constexpr int SGS_PREB_BLOCK = 128, SGS_PREB_LOG2 = 7, PREB_EMIT = 4;  // K-pre-B block: small, so that few survivors still spread over the SMs
 
 __global__ void __launch_bounds__(SGS_PREB_BLOCK)
 k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, const float* __restrict__ quat,
@@ -373,13 +373,13 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
         s_off[tid] = wbase + incl - cnt;  // exclusive
         if (tid == 0) s_off[SGS_PREB_BLOCK] = total;
         __syncthreads();
-        for (unsigned int e0 = tid; e0 < total; e0 += 2 * SGS_PREB_BLOCK) {
-            // two entries per trip so that both cursor atomics are in flight before either dependent store
-            uint32_t t[2];
-            unsigned long long key[2];
-            bool ok[2];
+        for (unsigned int e0 = tid; e0 < total; e0 += PREB_EMIT * SGS_PREB_BLOCK) {
+            // PREB_EMIT entries per trip so that their cursor atomics are all in flight before the first dependent store
+            uint32_t t[PREB_EMIT];
+            unsigned long long key[PREB_EMIT];
+            bool ok[PREB_EMIT];
 #pragma unroll
-            for (int k = 0; k < 2; ++k) {
+            for (int k = 0; k < PREB_EMIT; ++k) {
                 const unsigned int e = e0 + k * SGS_PREB_BLOCK;
                 ok[k] = e < total;
                 // owner = last thread whose exclusive offset is <= e (and whose count is non-zero by construction)
@@ -393,12 +393,12 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
                 t[k] = s_rect[lo] + (local / w) * (unsigned int)cam.tiles_x + (local % w);
                 key[k] = s_key[lo];
             }
-            uint32_t pos[2] = {0u, 0u};
+            uint32_t pos[PREB_EMIT];
 #pragma unroll
-            for (int k = 0; k < 2; ++k)
-                if (ok[k]) pos[k] = atomicAdd(&cursor[t[k]], 1u);
+            for (int k = 0; k < PREB_EMIT; ++k)
+                pos[k] = ok[k] ? atomicAdd(&cursor[t[k]], 1u) : 0u;
 #pragma unroll
-            for (int k = 0; k < 2; ++k)
+            for (int k = 0; k < PREB_EMIT; ++k)
                 if (ok[k]) {
                     if (pos[k] < tile_cap) bucket[(size_t)t[k] * tile_cap + pos[k]] = key[k];
                     else atomicMax(&counters->max_tile, pos[k] + 1u);
