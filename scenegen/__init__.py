@@ -11,8 +11,8 @@ available; these scenes take only their shapes (image sizes, intrinsics,
 room-scale geometry, centimetre-scale surface-aligned splats).
 """
 from .rng import SplitMix
-from .scenes import (Scene, Camera, make_config, tiny_scene, room_scene,
+from .scenes import (Scene, Camera, make_config, tiny_scene, room_scene, stress_scene, stress_camera,
                      upstream_normal, look_at, se3_exp, perturb_pose, CONFIG_NAMES)
 
-__all__ = ["SplitMix", "Scene", "Camera", "make_config", "tiny_scene", "room_scene",
+__all__ = ["SplitMix", "Scene", "Camera", "make_config", "tiny_scene", "room_scene", "stress_scene", "stress_camera",
            "upstream_normal", "look_at", "se3_exp", "perturb_pose", "CONFIG_NAMES"]

@@ -142,6 +142,57 @@ def tiny_camera():
     return Camera(64, 48, 60.0, 60.0, 32.0, 24.0)
 
 
+def stress_scene(seed=11, n=1600):
+    """Splats chosen to strain the renderer's conservative culling and masking, not to look like a room (camera at the
+    origin looking down +z, `stress_camera`): slivers (axis ratio up to 200:1), edge-on splats (normal within a few
+    degrees of perpendicular to the view ray), sub-pixel splats, splats larger than the screen, opacities around the
+    1/255 threshold, and splats close to the near plane.  Eight equal groups, parameters only (no method arithmetic)."""
+    g = SplitMix(seed)
+    k = n // 8
+    n = 8 * k
+    grp = np.repeat(np.arange(8), k)
+    mean = np.stack([g.uniform(n, -1.2, 1.2), g.uniform(n, -1.0, 1.0), g.uniform(n, 1.0, 3.0)], axis=1)
+    ls = np.stack([g.uniform(n, np.log(0.01), np.log(0.05)), g.uniform(n, np.log(0.01), np.log(0.05))], axis=1)
+    quat = np.stack([g.normal(n) for _ in range(4)], axis=1)
+    quat /= np.linalg.norm(quat, axis=1, keepdims=True)
+    opacity = g.uniform(n, 0.1, 0.99)
+    rgb = np.stack([g.uniform(n) for _ in range(3)], axis=1)
+    m = grp == 0                                   # slivers: 5-40 cm by 0.2-2 mm
+    ls[m, 0] = g.uniform(n, np.log(0.05), np.log(0.4))[m]; ls[m, 1] = g.uniform(n, np.log(0.0002), np.log(0.002))[m]
+    m = grp == 1                                   # edge-on: t_u along the view ray to the centre, tilted by < 3 degrees
+    ang = g.uniform(n, -0.05, 0.05); roll = g.uniform(n, 0.0, 2 * np.pi)
+    for i in np.nonzero(m)[0]:
+        ez0 = mean[i] / np.linalg.norm(mean[i])                      # view ray
+        a = np.cross(ez0, [0.0, 1.0, 0.0]); a /= np.linalg.norm(a)
+        b = np.cross(ez0, a)
+        side = np.cos(roll[i]) * a + np.sin(roll[i]) * b             # in-plane axis perpendicular to the ray
+        tn = np.cos(ang[i]) * np.cross(ez0, side) + np.sin(ang[i]) * ez0   # normal: almost perpendicular to the ray
+        tn /= np.linalg.norm(tn)
+        tu = np.cross(side, tn)
+        quat[i] = _quat_from_frame(tu, side, tn)
+    m = grp == 2                                   # sub-pixel: 0.1-2 mm
+    ls[m] = np.stack([g.uniform(n, np.log(0.0001), np.log(0.002)), g.uniform(n, np.log(0.0001), np.log(0.002))], axis=1)[m]
+    m = grp == 3                                   # larger than the screen: 1-3 m
+    ls[m] = np.stack([g.uniform(n, np.log(1.0), np.log(3.0)), g.uniform(n, np.log(1.0), np.log(3.0))], axis=1)[m]
+    opacity[m] = g.uniform(n, 0.02, 0.2)[m]
+    m = grp == 4                                   # opacity around 1/255
+    opacity[m] = g.uniform(n, 0.002, 0.02)[m]
+    ls[m] = np.stack([g.uniform(n, np.log(0.03), np.log(0.2)), g.uniform(n, np.log(0.03), np.log(0.2))], axis=1)[m]
+    m = grp == 5                                   # close to the near plane (z_near = 0.2)
+    mean[m, 2] = g.uniform(n, 0.15, 0.45)[m]; mean[m, 0] *= 0.2; mean[m, 1] *= 0.2
+    m = grp == 6                                   # far outside the frustum sideways, large enough to reach in
+    mean[m, 0] = (np.sign(mean[m, 0]) + (mean[m, 0] == 0)) * g.uniform(n, 2.0, 6.0)[m]
+    ls[m] = np.stack([g.uniform(n, np.log(0.3), np.log(2.0)), g.uniform(n, np.log(0.02), np.log(0.3))], axis=1)[m]
+    # group 7: plain splats (the C1 recipe) as filler
+    return Scene(mean.astype(np.float32), np.exp(ls).astype(np.float32), quat.astype(np.float32),
+                 opacity.astype(np.float32), rgb.astype(np.float32))
+
+
+def stress_camera():
+    """104 x 72 (7 x 5 tiles, both edges ragged), f = 70 px."""
+    return Camera(104, 72, 70.0, 70.0, 51.3, 36.7)
+
+
 # ----------------------------------------------------------------------------- rooms
 ROOM = np.array([5.0, 4.0, 3.0])
 

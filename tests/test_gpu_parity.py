@@ -390,3 +390,41 @@ def test_track_iter_edge_cases():
     np.testing.assert_allclose(lb.cpu().numpy(), la.cpu().numpy(), rtol=1e-5)
     np.testing.assert_allclose(pb.cpu().numpy(), pa.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(pa.abs().max()))
     ren.close()
+
+
+def test_stress_scene_masks_stay_conservative(ren):
+    """Splats built to strain the culling and the two-stage warp-patch masks (slivers of 200:1, edge-on splats,
+    sub-pixel and screen-filling splats, opacities around 1/255, splats at the near plane, splats reaching in from
+    far outside the frustum): binning bit-exact, images, every gradient and both pose paths against the oracle, and
+    the fused tracking kernel against the unfused sequence.  A mask that dropped one pair that eval_pair() accepts
+    would show as an image error of a whole blending weight."""
+    sc, cam = scenegen.stress_scene(), scenegen.stress_camera()
+    for tau in (None, [0.05, -0.08, 0.1, 0.3, -0.2, 0.4]):
+        T = None if tau is None else scenegen.perturb_pose(cam.T_cw, tau)
+        camv, cfg = oracle.make_cam(cam, T), oracle.make_cfg()
+        up = scenegen.upstream_normal(3, cam.height, cam.width)
+        out = run_gpu(ren, sc, cam, up, T_cw=T)
+        assert_binning(out["bin"], oracle.binning(sc, camv, cfg))
+        o = oracle.render(sc, camv, cfg)
+        chk = image_check(out["img"], o["img"], o["fragile"])
+        assert chk["n_bad"] == 0 and chk["fragile_ok"] and chk["fragile_frac"] < 0.12, chk
+        og = oracle.backward(sc, camv, cfg, up)
+        assert_grads(out["grads"], og, max_bad=5e-3)
+        assert_pose(out["pose"], og["pose"], rtol=2e-3)
+        out2 = run_gpu(ren, sc, cam, up, full=False, T_cw=T)
+        assert_pose(out2["pose"], og["pose"], rtol=2e-3)
+    r2 = sgs.Renderer()
+    t, sf = to_device(sc)
+    c = camera(cam)
+    im, im2 = alloc_images(cam), alloc_images(cam)
+    r2.render(sf, c, **im)
+    tgt_rgb, tgt_dep = (im["rgb"] * 0.9 + 0.01).contiguous(), (im["depth"] * 1.02).contiguous()
+    p6a, la = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+    r2.backward_tracking(tgt_rgb, tgt_dep, 0.5, 1.0, p6a, la)
+    p6b, lb = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+    r2.track_iter(sf, c, tgt_rgb, tgt_dep, 0.5, 1.0, p6b, lb, **im2)
+    torch.cuda.synchronize()
+    assert np.array_equal(planes(im), planes(im2))
+    np.testing.assert_allclose(lb.cpu().numpy(), la.cpu().numpy(), rtol=1e-5)
+    np.testing.assert_allclose(p6b.cpu().numpy(), p6a.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(p6a.abs().max()))
+    r2.close()
