@@ -122,7 +122,7 @@ def aggregate_replicas(ms_local, pixels, renders_per_rank, world, dist=None, dev
 class Workload:
     """Device-resident inputs + the step function for one config."""
 
-    def __init__(self, name, iters_override=None, contrib=False):
+    def __init__(self, name, iters_override=None, contrib=False, prefetch=True):
         self.contrib = contrib
         import torch
         import scenegen
@@ -137,6 +137,10 @@ class Workload:
                       active=d(sc.active, torch.uint8))
         self.sf = sgs.Renderer.surfels(*(self.t[k] for k in ("mean", "scale", "quat", "opacity", "rgb", "active")))
         self.ren = sgs.Renderer(async_mode=True)
+        # mapping window: a second context + a side stream, so that sgs_prepare (binning) of view v+1 runs under the
+        # compositing kernels of view v (include/sgs.h); tracking iterations depend on one another and use one context
+        self.rens = [self.ren] + ([sgs.Renderer(async_mode=True)] if (prefetch and not self.tracking and len(self.cams) > 1) else [])
+        self.side = torch.cuda.Stream(priority=-1) if len(self.rens) > 1 else None
         cam0 = self.cams[0]
         self.H, self.W = cam0.height, cam0.width
         z = lambda c: torch.zeros((c, self.H, self.W), device="cuda")
@@ -160,46 +164,61 @@ class Workload:
                               quat=torch.zeros(n, 4, device="cuda"), opacity=torch.zeros(n, device="cuda"),
                               rgb=torch.zeros(n, 3, device="cuda"))
         self.renders_per_step = self.iters if self.tracking else len(self.cams)
+        for r in self.rens[1:]:   # the second context's workspace settles on the same views
+            for c in self.ccams:
+                self._render_retry(c, r)
         self.flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
-    def _render_retry(self, cam):
+    def _render_retry(self, cam, ren=None):
+        ren = ren or self.ren
         for _ in range(4):  # async mode: an overflow is reported by the next call, after growing
             try:
-                self.ren.render(self.sf, cam, **self.im)
-                self.ren.stats()
-                self.ren.render(self.sf, cam, **self.im)
+                ren.render(self.sf, cam, **self.im)
+                ren.stats()
+                ren.render(self.sf, cam, **self.im)
                 return
             except self.sgs.SgsError as e:
                 if e.status != self.sgs.SGS_WORKSPACE_OVERFLOW:
                     raise
         raise RuntimeError("workspace did not settle")
 
-    def one(self, v):
+    def one(self, v, ren=None):
         """render -> loss -> backward for view v (everything enqueued, no host sync)."""
+        ren = ren or self.ren
         cam = self.ccams[v]
         trgb, tdep = self.targets[v]
         if self.tracking:  # one tracking iteration: K-pre + K-track (render, Eq. 15-19 loss, pose-only backward); images written
-            self.ren.track_iter(self.sf, cam, trgb, tdep, 0.5, -1.0, self.p6, self.loss, **self.im)
+            ren.track_iter(self.sf, cam, trgb, tdep, 0.5, -1.0, self.p6, self.loss, **self.im)
             return
         if self.contrib:  # forward with the per-splat contribution output (Eq. 20-21) switched on
-            self.ren.render_contrib(self.sf, cam, self.contrib_buf, **self.im)
+            ren.render_contrib(self.sf, cam, self.contrib_buf, **self.im)
         else:
-            self.ren.render(self.sf, cam, **self.im)
+            ren.render(self.sf, cam, **self.im)
         # mapping iteration: Eq. 24-26 with Tab. I's lambda_c, w_d, w_n -> upstream gradients of all planes
-        self.ren.mapping_loss(cam, self.im, trgb, tdep, 0.875, 0.5, 0.02, -1.0, self.up, self.loss)
-        self.ren.ssim_loss(self.im["rgb"], trgb, 0.125, self.up["rgb"], self.loss)   # + (1 - lambda_c) L_SSIM: Eq. 24 complete
+        ren.mapping_loss(cam, self.im, trgb, tdep, 0.875, 0.5, 0.02, -1.0, self.up, self.loss)
+        ren.ssim_loss(self.im["rgb"], trgb, 0.125, self.up["rgb"], self.loss)   # + (1 - lambda_c) L_SSIM: Eq. 24 complete
         u = self.up
         if True:
-            self.ren.backward(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"],
+            ren.backward(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"],
                               grads=self.grads, d_pose6=self.p6)
 
     def step(self):
         if self.tracking:
             for _ in range(self.iters):
                 self.one(0)
-        else:
+        elif len(self.rens) == 1:
             for v in range(len(self.cams)):
                 self.one(v)
+        else:
+            main = self.torch.cuda.current_stream()
+            self.side.wait_stream(main)   # the step's first launch stays behind the timed region's start event
+            nv = len(self.cams)
+            self.rens[0].prepare(self.sf, self.ccams[0], stream=self.side)
+            for v in range(nv):
+                if v + 1 < nv:
+                    self.rens[(v + 1) % 2].prepare(self.sf, self.ccams[v + 1], stream=self.side)
+                self.one(v, self.rens[v % 2])   # its render finds the binning prepared and orders itself behind it
+            main.wait_stream(self.side)
 
     def flush_l2(self):
         self.flush_buf.zero_()
@@ -309,6 +328,7 @@ def main():
     ap.add_argument("--iters", type=int, default=None, help="override iterations per tracking step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-prefetch", action="store_true", help="mapping configs: one context, binning of each view in line")
     ap.add_argument("--contrib", action="store_true", help="mapping configs: render with sgs_render_contrib (C_k output on)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -328,12 +348,12 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    wl = Workload(args.config, args.iters, args.contrib)
+    wl = Workload(args.config, args.iters, args.contrib, not args.no_prefetch)
     K, W = args.steps, max(args.warmup, 3)
     for _ in range(W):
         wl.step()
     torch.cuda.synchronize()
-    launches0 = wl.ren.stats()["kernel_launches"]
+    launches0 = sum(r.stats()["kernel_launches"] for r in wl.rens)
 
     def timed_pass():
         evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
@@ -351,17 +371,22 @@ def main():
     time.sleep(0.3)
     ms = timed_pass()
     clocks = sampler.stop()
-    launches = wl.ren.stats()["kernel_launches"] - launches0
+    launches = sum(r.stats()["kernel_launches"] for r in wl.rens) - launches0
     px = wl.H * wl.W
     ms_max, value = aggregate_replicas(ms, px, wl.renders_per_step * K, world, dist, "cuda")
     renders = wl.renders_per_step * K * world
 
     # second pass with per-stage CUDA events (roofline), not part of `value`
-    wl.ren.set_profiling(True)
-    wl.ren.get_profile(reset=True)
+    for r in wl.rens:
+        r.set_profiling(True)
+        r.get_profile(reset=True)
     timed_pass()
-    prof = wl.ren.get_profile(reset=True)
-    wl.ren.set_profiling(False)
+    prof = {}
+    for r in wl.rens:
+        for st, (ms_s, calls) in r.get_profile(reset=True).items():
+            a, b = prof.get(st, (0.0, 0))
+            prof[st] = (a + ms_s, b + calls)
+        r.set_profiling(False)
 
     # end to end through the HOST-buffer C-ABI calls
     e2e = None
@@ -431,7 +456,9 @@ def main():
                             f"{'pose-only' if wl.tracking else 'full+pose'} backward) per step",
                             surfels=wl.sc.n, active=wl.n_active, width=wl.W, height=wl.H, renders_per_step=wl.renders_per_step,
                             l2="flushed between steps by a 256 MiB write; iterations inside a step reuse the map as tracking does",
-                            replicas=world),
+                            replicas=world,
+                            binning=("sgs_prepare of view v+1 on a second context and a side stream, under view v's compositing"
+                                     if len(wl.rens) > 1 else "in line (sgs_render / sgs_track_iter)")),
                 clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roof, stages=stages, cpu_baseline=cpu,
                 stage_us={k: round(1e3 * v[0] / v[1], 2) for k, v in prof.items() if v[1]})
     print(json.dumps(line))

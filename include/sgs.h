@@ -139,6 +139,16 @@ SGS_API int sgs_destroy(sgs_ctx* ctx);
 SGS_API int sgs_render(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_camera* cam, const sgs_images* out,
                void* cuda_stream);
 
+/* First half of sgs_render on its own: preprocess + tile binning of (surfels, cam), enqueued on `stream`, nothing
+ * rendered.  The next sgs_render on this ctx with the SAME surfels struct and camera (compared bytewise) skips its
+ * own binning, orders its stream behind this call's work (an internal event; the two streams may differ) and goes
+ * straight to compositing; any other call in between drops the prepared state.  The call itself is ordered behind
+ * the ctx's last sgs_render / sgs_backward, whose stream may differ as well.  Purpose: in a mapping window (L248-252:
+ * several keyframes rendered against one map) the latency-bound binning of view v+1, on a second ctx and a side
+ * stream, hides under the compositing kernels of view v.  Same arguments, status codes and async-mode overflow
+ * reporting as sgs_render. */
+SGS_API int sgs_prepare(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_camera* cam, void* cuda_stream);
+
 /* sgs_render that additionally returns the contribution of every splat to the view (Eq. 20-21):
  * contrib[k] = C_k^V = sum over pixels of w_k(p) = a_k T_k, "how many pixels the splat contributes to"; the
  * paper calls a splat visible in the view when C_k^V > 0.5 (keyframe selection, state update, pruning).

@@ -50,7 +50,7 @@ class sgs_stats(C.Structure):
                 ("workspace_bytes", C.c_int64), ("kernel_launches", C.c_int64)]
 
 
-EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_backward", "sgs_tracking_loss",
+EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_prepare", "sgs_backward", "sgs_tracking_loss",
            "sgs_backward_tracking", "sgs_track_iter", "sgs_render_contrib", "sgs_covisibility", "sgs_mapping_loss", "sgs_ssim_loss", "sgs_map_correction", "sgs_measure_fp32_peak", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
            "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string"]
 
@@ -195,6 +195,11 @@ class Renderer:
         device tensors (any may be None)."""
         im = _images(rgb, depth, normal, alpha)
         _check(self.lib.sgs_render(self._ctx, C.byref(surfels), C.byref(cam), C.byref(im), _stream_ptr(stream)), "sgs_render")
+
+    def prepare(self, surfels, cam, stream=None):
+        """sgs_prepare: preprocess + tile binning only; the next render() of the same (surfels, cam) objects on this
+        Renderer skips its binning and orders itself behind this call (the streams may differ)."""
+        _check(self.lib.sgs_prepare(self._ctx, C.byref(surfels), C.byref(cam), _stream_ptr(stream)), "sgs_prepare")
 
     def render_contrib(self, surfels, cam, contrib, rgb=None, depth=None, normal=None, alpha=None, stream=None):
         """sgs_render_contrib: render + per-splat contribution C_k^V (Eq. 20-21) into `contrib` (n floats, device)."""

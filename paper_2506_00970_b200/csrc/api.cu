@@ -202,7 +202,9 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
               cudaMallocHost(&c->pinned_small, 8 * sizeof(float)) == cudaSuccess &&
               cudaMalloc(&c->sort_hist, sizeof(uint32_t) * (8 * 256 + 8)) == cudaSuccess &&
               cudaMalloc(&c->loss_dev, sizeof(float) * 8) == cudaSuccess &&
-              cudaEventCreateWithFlags(&c->counters_ready, cudaEventDisableTiming) == cudaSuccess;
+              cudaEventCreateWithFlags(&c->counters_ready, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreateWithFlags(&c->prepared_ev, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreateWithFlags(&c->work_ev, cudaEventDisableTiming) == cudaSuccess;
     if (!ok) { cudaGetLastError(); sgs_destroy(c); return SGS_CUDA_ERROR; }
     c->pose6_dev = c->loss_dev + 1;
     cudaMemset(c->counters, 0, sizeof(SgsCounters));
@@ -229,6 +231,8 @@ int sgs_destroy(sgs_ctx* c) {
     if (c->loss_dev) cudaFree(c->loss_dev);
     if (c->covis_cnt) cudaFree(c->covis_cnt);
     if (c->counters_ready) cudaEventDestroy(c->counters_ready);
+    if (c->prepared_ev) cudaEventDestroy(c->prepared_ev);
+    if (c->work_ev) cudaEventDestroy(c->work_ev);
     for (int i = 0; i < 2 * c->prof_cap; ++i) cudaEventDestroy(c->prof_ev[i]);
     free(c->prof_ev); free(c->prof_stage);
     delete c;

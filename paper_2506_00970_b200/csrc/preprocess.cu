@@ -459,6 +459,9 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
         if (hint < blocks_b) blocks_b = hint;
     }
     if (blocks_b > 148 * 8) blocks_b = 148 * 8;
+    // sgs_prepare: the binning runs under another view's compositing kernels and has a whole view's time to finish;
+    // a narrow grid (one block per SM) keeps it from displacing their blocks (each of these holds 13.8 k registers)
+    if (c->narrow_prepare && blocks_b > 148 * c->narrow_prepare) blocks_b = 148 * c->narrow_prepare;
     if (blocks_b < 1) blocks_b = 1;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)blocks_b); cfg.blockDim = dim3(SGS_PREB_BLOCK); cfg.dynamicSmemBytes = 0; cfg.stream = s;

@@ -428,3 +428,57 @@ def test_stress_scene_masks_stay_conservative(ren):
     np.testing.assert_allclose(lb.cpu().numpy(), la.cpu().numpy(), rtol=1e-5)
     np.testing.assert_allclose(p6b.cpu().numpy(), p6a.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(p6a.abs().max()))
     r2.close()
+
+
+def test_prepare_then_render_equals_render():
+    """sgs_prepare (binning only, on a side stream) followed by sgs_render of the same view == plain sgs_render:
+    binning and images bit-identical, gradients equal up to the order of the atomic sums; a render of ANOTHER view
+    after a prepare bins again; two contexts alternating over a window of views reproduce the in-line sequence."""
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    t, sf = to_device(sc)
+    tiles = ((cam.width + 15) // 16) * ((cam.height + 15) // 16)
+    up = scenegen.upstream_normal(5, cam.height, cam.width)
+    taus = [None, [0.05, 0.02, -0.04, 0.1, -0.05, 0.2], [-0.1, 0.05, 0.02, -0.2, 0.1, 0.05]]
+    cs = [camera(cam, None if tau is None else scenegen.perturb_pose(cam.T_cw, tau)) for tau in taus]
+    side = torch.cuda.Stream()
+
+    def full(ren, c, prepared_on=None):
+        im, g, p6 = alloc_images(cam), alloc_grads(sc.n), torch.zeros(6, device="cuda")
+        if prepared_on is not None:
+            ren.prepare(sf, prepared_on, stream=side)
+        ren.render(sf, c, **im)
+        b = ren.get_binning(sc.n, tiles)
+        ren.backward(**split_upstream(up), grads=g, d_pose6=p6)
+        torch.cuda.synchronize()
+        return planes(im), b, {k: v.cpu().numpy() for k, v in g.items()}, p6.cpu().numpy()
+
+    ref_ren = sgs.Renderer()
+    refs = [full(ref_ren, c) for c in cs]
+    ra, rb = sgs.Renderer(), sgs.Renderer()
+    # same view prepared; another view prepared (the render must bin again)
+    for c_prep, k in ((cs[1], 1), (cs[2], 1)):
+        img, b, g, p6 = full(ra, cs[k], prepared_on=c_prep)
+        assert np.array_equal(img, refs[k][0])
+        assert_binning(b, refs[k][1])
+        for name in g:
+            np.testing.assert_allclose(g[name], refs[k][2][name], rtol=2e-4, atol=1e-5 * np.abs(refs[k][2][name]).max())
+        np.testing.assert_allclose(p6, refs[k][3], rtol=1e-4, atol=1e-5 * np.abs(refs[k][3]).max())
+    # a window of views over two contexts: binning of view v+1 enqueued on the side stream before view v is rendered
+    rens = [ra, rb]
+    ims = [alloc_images(cam) for _ in cs]
+    p6s = [torch.zeros(6, device="cuda") for _ in cs]
+    main = torch.cuda.current_stream()
+    side.wait_stream(main)
+    rens[0].prepare(sf, cs[0], stream=side)
+    for v, c in enumerate(cs):
+        if v + 1 < len(cs):
+            rens[(v + 1) % 2].prepare(sf, cs[v + 1], stream=side)
+        rens[v % 2].render(sf, c, **ims[v])
+        rens[v % 2].backward(**split_upstream(up), grads=None, d_pose6=p6s[v])
+    torch.cuda.synchronize()
+    for v in range(len(cs)):
+        assert np.array_equal(planes(ims[v]), refs[v][0])
+        np.testing.assert_allclose(p6s[v].cpu().numpy(), refs[v][3], rtol=1e-4, atol=1e-5 * np.abs(refs[v][3]).max())
+    for r in (ref_ren, ra, rb):
+        r.close()
