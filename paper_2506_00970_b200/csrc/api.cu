@@ -204,7 +204,10 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
               cudaMalloc(&c->loss_dev, sizeof(float) * 8) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->counters_ready, cudaEventDisableTiming) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->prepared_ev, cudaEventDisableTiming) == cudaSuccess &&
-              cudaEventCreateWithFlags(&c->work_ev, cudaEventDisableTiming) == cudaSuccess;
+              cudaEventCreateWithFlags(&c->work_ev, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreateWithFlags(&c->fork_ev, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreateWithFlags(&c->join_ev, cudaEventDisableTiming) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking) == cudaSuccess;
     if (!ok) { cudaGetLastError(); sgs_destroy(c); return SGS_CUDA_ERROR; }
     c->pose6_dev = c->loss_dev + 1;
     cudaMemset(c->counters, 0, sizeof(SgsCounters));
@@ -233,6 +236,9 @@ int sgs_destroy(sgs_ctx* c) {
     if (c->counters_ready) cudaEventDestroy(c->counters_ready);
     if (c->prepared_ev) cudaEventDestroy(c->prepared_ev);
     if (c->work_ev) cudaEventDestroy(c->work_ev);
+    if (c->fork_ev) cudaEventDestroy(c->fork_ev);
+    if (c->join_ev) cudaEventDestroy(c->join_ev);
+    if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
     for (int i = 0; i < 2 * c->prof_cap; ++i) cudaEventDestroy(c->prof_ev[i]);
     free(c->prof_ev); free(c->prof_stage);
     delete c;

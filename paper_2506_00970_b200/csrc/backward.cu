@@ -393,17 +393,26 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     }
     const int64_t n = c->last_surfels.n;
     cudaError_t e = cudaSuccess;
-    // exact zeros for every surfel the per-surfel kernel does not visit (inactive, culled)
-    if (dg->mean && e == cudaSuccess) e = cudaMemsetAsync(dg->mean, 0, sizeof(float) * 3 * (size_t)n, s);
-    if (dg->scale && e == cudaSuccess) e = cudaMemsetAsync(dg->scale, 0, sizeof(float) * 2 * (size_t)n, s);
-    if (dg->quat && e == cudaSuccess) e = cudaMemsetAsync(dg->quat, 0, sizeof(float) * 4 * (size_t)n, s);
-    if (dg->opacity && e == cudaSuccess) e = cudaMemsetAsync(dg->opacity, 0, sizeof(float) * (size_t)n, s);
-    if (dg->rgb && e == cudaSuccess) e = cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * (size_t)n, s);
+    // exact zeros for every surfel the per-surfel kernel does not visit (inactive, culled): 52 B per surfel of plain
+    // HBM writes that nothing before k_surfel_backward depends on -- forked onto the ctx's own stream so that they run
+    // beside the issue-bound k_backward, joined in front of k_surfel_backward
+    cudaStream_t ms = c->aux_stream ? c->aux_stream : s;
+    if (ms != s) {
+        if ((e = cudaEventRecord(c->fork_ev, s)) != cudaSuccess) return e;
+        if ((e = cudaStreamWaitEvent(ms, c->fork_ev, 0)) != cudaSuccess) return e;
+    }
+    if (dg->mean && e == cudaSuccess) e = cudaMemsetAsync(dg->mean, 0, sizeof(float) * 3 * (size_t)n, ms);
+    if (dg->scale && e == cudaSuccess) e = cudaMemsetAsync(dg->scale, 0, sizeof(float) * 2 * (size_t)n, ms);
+    if (dg->quat && e == cudaSuccess) e = cudaMemsetAsync(dg->quat, 0, sizeof(float) * 4 * (size_t)n, ms);
+    if (dg->opacity && e == cudaSuccess) e = cudaMemsetAsync(dg->opacity, 0, sizeof(float) * (size_t)n, ms);
+    if (dg->rgb && e == cudaSuccess) e = cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * (size_t)n, ms);
     if (e != cudaSuccess) return e;
+    if (ms != s && (e = cudaEventRecord(c->join_ev, ms)) != cudaSuccess) return e;
     c->launches += 1;
     k_backward<false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                   cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
                                                   c->acc, c->pose_partial, c->counters, nullptr, FusedLoss{});
+    if (ms != s && (e = cudaStreamWaitEvent(s, c->join_ev, 0)) != cudaSuccess) return e;
     // one thread per listed surfel; the list length is only known on the device: grid-stride from a hinted grid
     const bool bucket_mode = c->list_stride == 2;
     int64_t want = n;

@@ -107,6 +107,8 @@ struct sgs_ctx {
     SgsCounters* counters;           // device
     SgsCounters* counters_host;      // pinned
     cudaEvent_t counters_ready;
+    cudaStream_t aux_stream;           // sgs_backward: the gradient memsets run beside k_backward (fork / join by events)
+    cudaEvent_t fork_ev, join_ev;
     cudaEvent_t prepared_ev, work_ev;   // sgs_prepare: binning enqueued / the ctx's last render or backward enqueued
     int narrow_prepare;                // > 0 inside sgs_prepare: K-pre-B blocks per SM
     bool prepared, work_recorded;      // binning of (last_surfels, last_cam) enqueued by sgs_prepare, not yet rendered
