@@ -134,8 +134,13 @@ SGS_API int sgs_default_config(sgs_config* cfg);
 SGS_API int sgs_create(sgs_ctx** out, const sgs_config* cfg);
 SGS_API int sgs_destroy(sgs_ctx* ctx);
 
-/* Forward (Eq. 1-8): preprocess -> tile binning (64-bit tile|depth keys, radix sort, ranges)
- * -> per-tile compositing.  Saves the state sgs_backward needs inside ctx. */
+/* Forward (Eq. 1-8): preprocess (Eq. 5-7, culling, screen AABB) -> tile binning (the list of (tile, depth, surfel)
+ * entries in the order of the 64-bit key tile << 32 | depth bits, ties by surfel index: per-tile buckets + an in-tile
+ * sort by default, one global radix sort with SGS_FLAG_RADIX_BINNING -- the same list either way) -> per-tile
+ * front-to-back compositing (Eq. 8 with the truncation rules R3-R7).  Saves the state sgs_backward needs inside ctx.
+ *   surfels: DEVICE map, borrowed until the matching sgs_backward;  cam: HOST;  out: DEVICE images, any may be NULL.
+ * Errors: SGS_INVALID_ARGUMENT (NULL / non-positive sizes / n >= 2^24), SGS_OUT_OF_MEMORY (workspace),
+ * SGS_WORKSPACE_OVERFLOW (async mode, see above), SGS_CUDA_ERROR. */
 SGS_API int sgs_render(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_camera* cam, const sgs_images* out,
                void* cuda_stream);
 
@@ -163,10 +168,14 @@ SGS_API int sgs_render_contrib(sgs_ctx* ctx, const sgs_surfels* surfels, const s
 SGS_API int sgs_covisibility(sgs_ctx* ctx, const float* contrib_a, const float* contrib_b, int64_t n, const uint8_t* active,
                              float threshold, float* result3, void* cuda_stream);
 
-/* Backward of the most recent sgs_render on this ctx (same surfel buffers, unchanged).
+/* Backward of the most recent sgs_render on this ctx (same surfel buffers, unchanged) (Eq. 9-13).
  *   upstream : dL/d(rgb, depth, normal, alpha)                                     DEVICE
  *   d_surfels: nullable; NULL = pose-only mode (tracking, L204: splats frozen)     DEVICE
- *   d_pose6  : nullable; 6 floats (rho, theta), Eq. 11-13                          DEVICE */
+ *   d_pose6  : nullable; 6 floats (rho, theta), Eq. 11-13                          DEVICE
+ * All results are complete in the order of `cuda_stream` (the zero-fill of d_surfels runs on a stream of the ctx
+ * beside the compositing kernel and is joined before the call's last kernel).
+ * Errors: SGS_NO_FORWARD_STATE without a preceding successful sgs_render (also after sgs_track_iter, sgs_prepare),
+ * SGS_WORKSPACE_OVERFLOW (async mode: that render had overflowed; render again), SGS_OUT_OF_MEMORY, SGS_CUDA_ERROR. */
 SGS_API int sgs_backward(sgs_ctx* ctx, const sgs_images* upstream, const sgs_surfel_grads* d_surfels, float* d_pose6,
                  void* cuda_stream);
 
@@ -179,8 +188,8 @@ SGS_API int sgs_backward(sgs_ctx* ctx, const sgs_images* upstream, const sgs_sur
 SGS_API int sgs_tracking_loss(sgs_ctx* ctx, const sgs_camera* cam, const sgs_images* rendered, const sgs_images* target,
                       float lambda_d, float normal_sign, const sgs_images* upstream, float* loss, void* cuda_stream);
 
-/* Mapping loss of Eq. 24-26 (L232-248) WITHOUT its SSIM term (out of this round's scope), harness around
- * the renderer for the mapping-shaped configs:
+/* Mapping loss of Eq. 24-26 (L232-248) without the SSIM term of Eq. 24, which sgs_ssim_loss adds on top; harness
+ * around the renderer for the mapping-shaped configs:
  *   L = 1/|Omega| sum_p [ lambda_c |I_r - I|_1 + w_d |D_r - D| + w_n (1 - normal_sign N_{D_r} . N_r) ]
  * N_{D_r}: unit cross product of the central differences of the points back-projected from the RENDERED depth
  * (Eq. 23, 25; reading R23), interior pixels only.  Writes dL/d(rgb, depth, normal, alpha) of the rendered images
@@ -198,7 +207,7 @@ SGS_API int sgs_mapping_loss(sgs_ctx* ctx, const sgs_camera* cam, const sgs_imag
 SGS_API int sgs_backward_tracking(sgs_ctx* ctx, const sgs_images* target, float lambda_d, float normal_sign,
                                   float* d_pose6, float* loss, void* cuda_stream);
 
-/* One whole tracking iteration (L180-204) in two launches: preprocess + tile binning, then ONE kernel that
+/* One whole tracking iteration (L180-204) in three launches: preprocess + tile binning (two), then ONE kernel that
  * composites each tile (Eq. 8), evaluates Eq. 15-19 against the current frame in registers and walks the
  * tile's list back for the pose gradient (Eq. 11-13); images, T and the upstream gradients never leave the
  * SM.  Same result as sgs_render + sgs_backward_tracking (bit-identical images, loss and 6-vector up to
