@@ -122,7 +122,7 @@ def aggregate_replicas(ms_local, pixels, renders_per_rank, world, dist=None, dev
 class Workload:
     """Device-resident inputs + the step function for one config."""
 
-    def __init__(self, name, iters_override=None, contrib=False, prefetch=True):
+    def __init__(self, name, iters_override=None, contrib=False, prefetch=True, reuse=True):
         self.contrib = contrib
         import torch
         import scenegen
@@ -136,7 +136,7 @@ class Workload:
         self.t = dict(mean=d(sc.mean), scale=d(sc.scale), quat=d(sc.quat), opacity=d(sc.opacity), rgb=d(sc.rgb),
                       active=d(sc.active, torch.uint8))
         self.sf = sgs.Renderer.surfels(*(self.t[k] for k in ("mean", "scale", "quat", "opacity", "rgb", "active")))
-        self.ren = sgs.Renderer(async_mode=True)
+        self.ren = sgs.Renderer(async_mode=True, track_reuse=self.tracking and reuse)
         # mapping window: a second context + a side stream, so that sgs_prepare (binning) of view v+1 runs under the
         # compositing kernels of view v (include/sgs.h); tracking iterations depend on one another and use one context
         self.rens = [self.ren] + ([sgs.Renderer(async_mode=True)] if (prefetch and not self.tracking and len(self.cams) > 1) else [])
@@ -204,6 +204,7 @@ class Workload:
 
     def step(self):
         if self.tracking:
+            self.ren.track_new_frame()   # a step is the tracking of one frame: the survivor list is built once per step
             for _ in range(self.iters):
                 self.one(0)
         elif len(self.rens) == 1:
@@ -328,6 +329,7 @@ def main():
     ap.add_argument("--iters", type=int, default=None, help="override iterations per tracking step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-reuse", action="store_true", help="tracking configs: run the pre-cull over the whole map every iteration")
     ap.add_argument("--no-prefetch", action="store_true", help="mapping configs: one context, binning of each view in line")
     ap.add_argument("--contrib", action="store_true", help="mapping configs: render with sgs_render_contrib (C_k output on)")
     args = ap.parse_args()
@@ -348,7 +350,7 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    wl = Workload(args.config, args.iters, args.contrib, not args.no_prefetch)
+    wl = Workload(args.config, args.iters, args.contrib, not args.no_prefetch, not args.no_reuse)
     K, W = args.steps, max(args.warmup, 3)
     for _ in range(W):
         wl.step()
@@ -457,6 +459,8 @@ def main():
                             surfels=wl.sc.n, active=wl.n_active, width=wl.W, height=wl.H, renders_per_step=wl.renders_per_step,
                             l2="flushed between steps by a 256 MiB write; iterations inside a step reuse the map as tracking does",
                             replicas=world,
+                            survivor_list=("built once per step (frame) with a 3 cm / 0.02 rad pose margin, SGS_FLAG_TRACK_REUSE"
+                                           if (wl.tracking and not args.no_reuse) else "every render"),
                             binning=("sgs_prepare of view v+1 on a second context and a side stream, under view v's compositing"
                                      if len(wl.rens) > 1 else "in line (sgs_render / sgs_track_iter)")),
                 clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roof, stages=stages, cpu_baseline=cpu,

@@ -61,8 +61,9 @@ enum {
 
 enum {
     SGS_FLAG_ASYNC = 1,         /* never synchronise the host in sgs_render (CUDA-graph capturable) */
-    SGS_FLAG_RADIX_BINNING = 2  /* bin with the global LSD radix sort of the 64-bit keys instead of the
+    SGS_FLAG_RADIX_BINNING = 2, /* bin with the global LSD radix sort of the 64-bit keys instead of the
                                    default per-tile buckets + in-tile sort; same list, kept for A/B checks */
+    SGS_FLAG_TRACK_REUSE = 4    /* sgs_track_iter: the map is frozen between sgs_track_new_frame calls, see there */
 };
 
 /* Truncation conventions of Eq. 8 (R3-R7).  sgs_default_config fills the defaults shown. */
@@ -223,6 +224,17 @@ SGS_API int sgs_backward_tracking(sgs_ctx* ctx, const sgs_images* target, float 
 SGS_API int sgs_track_iter(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_camera* cam, const sgs_images* target,
                            float lambda_d, float normal_sign, const sgs_images* out, float* d_pose6, float* loss,
                            void* cuda_stream);
+
+/* SGS_FLAG_TRACK_REUSE.  Tracking optimises the pose of ONE frame over many iterations against a frozen map (L204).
+ * With the flag set, the caller promises that between two sgs_track_new_frame calls the arrays behind a bytewise-equal
+ * sgs_surfels struct (means, scales, active flags) do not change.  sgs_track_iter then keeps the survivor list of its
+ * conservative pre-cull (active and possibly inside the frustum), built with a margin of 3 cm / 0.02 rad around the
+ * pose of the iteration that built it, and skips that pass over the whole map while the pose stays inside 80 % of the
+ * margin; a pose outside, another surfels struct, or any other binning call on the ctx rebuilds it.  The exact
+ * culling and everything after it run every iteration on the listed splats, so results are unchanged
+ * (tests: binning bit-identical to the oracle's along a pose trajectory that leaves the margin).
+ * sgs_track_new_frame drops the list (call it when the map may have changed, i.e. at every new frame). */
+SGS_API int sgs_track_new_frame(sgs_ctx* ctx);
 
 /* Debug export of the binning of the last render, for bit-exact parity tests.  Synchronises.
  * Returned DEVICE pointers stay valid until the next call on ctx.  idx holds ORIGINAL surfel

@@ -136,6 +136,7 @@ void sgs_fill_cam(const sgs_camera* cam, SgsCamDev* d) {
     d->pc_n[2] = sqrtf(cam->fy * cam->fy + cam->cy * cam->cy) * 1.00001f;
     d->pc_n[3] = sqrtf(cam->fy * cam->fy + d->pc_cyr * d->pc_cyr) * 1.00001f;
     d->pc_tabs = fabsf(d->tf[0]) + fabsf(d->tf[1]) + fabsf(d->tf[2]) + 1.f;
+    d->pm_t = 0.f; d->pm_r = 0.f;
 }
 
 bool sgs_cam_valid(const sgs_camera* cam) {
@@ -224,7 +225,7 @@ int sgs_destroy(sgs_ctx* c) {
                     c->pay.g5, c->pay.g6, c->pay.g7, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
                     c->sort_state, c->ranges, c->T_final, c->n_last, c->img_scratch, c->pose_partial, c->resident_store,
                     c->resident_active, c->target_rgb, c->host_img_dev, c->host_up_dev, c->host_grads_dev,
-                    c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->pose_inc, c->ssim_maps, c->export_keys, c->export_ranges};
+                    c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->pose_inc, c->ssim_maps, c->surv_cnt, c->export_keys, c->export_ranges};
     for (void* p : ptrs) sgs_ws_free(c, p, s);
     if (c->counters) cudaFree(c->counters);
     if (c->counters_snap) cudaFree(c->counters_snap);

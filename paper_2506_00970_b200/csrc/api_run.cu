@@ -1,4 +1,5 @@
 // api_run.cu -- sgs_render / sgs_backward / sgs_tracking_loss / debug export (include/sgs.h).
+#include <math.h>
 #include <string.h>
 #include "sgs_internal.h"
 
@@ -122,6 +123,7 @@ static int bin_view(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, bo
     if (r != SGS_OK) return r;
     c->have_forward = false;
     c->have_binning = false;
+    if (!c->use_surv_cache) c->surv_valid = false;  // K-pre-A is about to overwrite the list
     sgs_fill_cam(cam, &c->camd);
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
     const int64_t pixels = (int64_t)cam->width * cam->height;
@@ -141,6 +143,31 @@ static void pick_planes(sgs_ctx* c, const sgs_images* out, int64_t pixels, bool 
         if (out->normal) for (int i = 0; i < 3; ++i) planes[4 + i] = out->normal + (size_t)i * pixels;
         if (out->alpha) planes[7] = out->alpha;
     }
+}
+
+// cam = Exp(tau) o ref with |rho| and |theta| inside 80 % of the survivor list's margins (same image and intrinsics)
+static bool pose_within_margin(const sgs_camera* ref, const sgs_camera* cam) {
+    if (ref->width != cam->width || ref->height != cam->height || ref->fx != cam->fx || ref->fy != cam->fy ||
+        ref->cx != cam->cx || ref->cy != cam->cy) return false;
+    const float* A = cam->T_cw; const float* B = ref->T_cw;  // rows [R | t]
+    double Rd[9], tr = 0.0;
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {  // R_d = R_cam R_ref^T
+            double v = 0.0;
+            for (int k = 0; k < 3; ++k) v += (double)A[4 * i + k] * (double)B[4 * j + k];
+            Rd[3 * i + j] = v;
+        }
+    tr = Rd[0] + Rd[4] + Rd[8];
+    double cosang = 0.5 * (tr - 1.0);
+    if (!(cosang <= 1.0)) cosang = 1.0;
+    if (!(cosang >= -1.0)) return false;
+    double d2 = 0.0;
+    for (int i = 0; i < 3; ++i) {  // t_d = t_cam - R_d t_ref
+        const double v = (double)A[4 * i + 3] - (Rd[3 * i] * B[3] + Rd[3 * i + 1] * B[7] + Rd[3 * i + 2] * B[11]);
+        d2 += v * v;
+    }
+    const double mt = 0.8 * SGS_REUSE_MARGIN_T, mr = 0.8 * SGS_REUSE_MARGIN_R;
+    return d2 <= mt * mt && cosang >= cos(mr);
 }
 
 static bool same_view(const sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam) {
@@ -213,8 +240,15 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
         c->have_forward = false;
         return r;
     }
+    if ((c->cfg.flags & SGS_FLAG_TRACK_REUSE) && sf && sgs_cam_valid(cam)) {
+        if (!c->surv_cnt && !(c->surv_cnt = (unsigned int*)sgs_ws_alloc(c, sizeof(unsigned int), s))) return SGS_OUT_OF_MEMORY;
+        if (c->surv_valid && !(memcmp(&c->surv_sf, sf, sizeof(*sf)) == 0 && pose_within_margin(&c->surv_cam, cam)))
+            c->surv_valid = false;  // another map, or the pose has left the list's margin: build it again, centred here
+        c->use_surv_cache = true;
+    }
     c->defer_counters = true;  // (bin_buckets clears it when it cannot honour it)
     int r = bin_view(c, sf, cam, false, s);
+    c->use_surv_cache = false;
     const bool deferred = c->defer_counters;
     c->defer_counters = false;
     if (r != SGS_OK) return r;
@@ -232,6 +266,12 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
         c->pending_lazy = true;
     }
     c->have_binning = true;
+    return SGS_OK;
+}
+
+int sgs_track_new_frame(sgs_ctx* c) {
+    if (!c) return SGS_INVALID_ARGUMENT;
+    c->surv_valid = false;
     return SGS_OK;
 }
 

@@ -128,7 +128,10 @@ __device__ __forceinline__ bool precull_f32(const float* __restrict__ mean, cons
     const float X = cam.Rf[0] * m0 + cam.Rf[1] * m1 + cam.Rf[2] * m2 + cam.tf[0];
     const float Y = cam.Rf[3] * m0 + cam.Rf[4] * m1 + cam.Rf[5] * m2 + cam.tf[1];
     const float Z = cam.Rf[6] * m0 + cam.Rf[7] * m1 + cam.Rf[8] * m2 + cam.tf[2];
-    const float d = 1e-5f * (fabsf(m0) + fabsf(m1) + fabsf(m2) + cam.pc_tabs);
+    // pm_t, pm_r > 0 (survivor list kept for later poses T' = Exp(tau) T with |rho| <= pm_t, |theta| <= pm_r): the
+    // camera-space centre moves by at most pm_r |X_c| + pm_t, and every test below is linear in it with a unit normal
+    const float d = 1e-5f * (fabsf(m0) + fabsf(m1) + fabsf(m2) + cam.pc_tabs) + cam.pm_t +
+                    cam.pm_r * (fabsf(X) + fabsf(Y) + fabsf(Z));
     if (Z + d < cfg.z_near) return true;
     const float r = cfg.cutoff * fmaxf(fabsf(scale[0]), fabsf(scale[1])) * 1.00001f + d;
     // left: fx X + cx Z < 0 ; right: fx X + (cx - W) Z > 0 ; top / bottom alike.  Normals un-normalised:
@@ -255,7 +258,7 @@ template <int SGS_PREA_ITEMS>
 __global__ void __launch_bounds__(SGS_PRE_BLOCK)
 k_pre_select(int64_t n, const float* __restrict__ mean, const float* __restrict__ scale,
              const uint8_t* __restrict__ active, SgsCamDev cam, SgsCfgDev cfg, uint8_t* __restrict__ culled,
-             SgsCounters* __restrict__ counters, uint32_t* __restrict__ surv_list) {
+             unsigned int* __restrict__ n_surv, uint32_t* __restrict__ surv_list) {
     constexpr int SGS_PREA_SPAN = SGS_PREA_ITEMS * SGS_PRE_BLOCK;
     cudaTriggerProgrammaticLaunchCompletion();  // K-pre-B may be staged now; it waits for this grid before reading
     __shared__ unsigned short s_list[SGS_PREA_SPAN];
@@ -296,7 +299,7 @@ k_pre_select(int64_t n, const float* __restrict__ mean, const float* __restrict_
     __syncthreads();
     const unsigned int ns = s_n;
     if (ns == 0) return;
-    if (tid == 0) s_base = atomicAdd(&counters->n_surv, ns);
+    if (tid == 0) s_base = atomicAdd(n_surv, ns);
     __syncthreads();
     const unsigned int gb = s_base;
     for (unsigned int k = tid; k < ns; k += SGS_PRE_BLOCK) surv_list[gb + k] = (uint32_t)(base + s_list[k]);
@@ -308,8 +311,8 @@ __global__ void __launch_bounds__(SGS_PREB_BLOCK)
 k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, const float* __restrict__ quat,
               const float* __restrict__ opacity, const float* __restrict__ rgb, SgsCamDev cam, SgsCfgDev cfg,
               SgsPayload pay, uint8_t* __restrict__ culled, SgsCounters* __restrict__ counters,
-              const uint32_t* __restrict__ surv_list, uint32_t* __restrict__ cursor, uint64_t* __restrict__ bucket,
-              uint32_t tile_cap) {
+              const uint32_t* __restrict__ surv_list, const unsigned int* __restrict__ n_surv_in,
+              uint32_t* __restrict__ cursor, uint64_t* __restrict__ bucket, uint32_t tile_cap) {
     __shared__ unsigned int s_off[SGS_PREB_BLOCK + 1];
     __shared__ unsigned long long s_key[SGS_PREB_BLOCK];
     __shared__ unsigned int s_rect[SGS_PREB_BLOCK];   // tile index of the rectangle's first tile
@@ -317,7 +320,8 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
     __shared__ unsigned int s_wsum[SGS_PREB_BLOCK / 32];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     cudaGridDependencySynchronize();                // K-pre-A complete: survivor list and count are final
-    const unsigned int n_surv = counters->n_surv;   // written by K-pre-A (previous launch on the stream)
+    const unsigned int n_surv = *n_surv_in;   // written by K-pre-A (previous launch on the stream, or an earlier iteration)
+    if (n_surv_in != &counters->n_surv && blockIdx.x == 0 && tid == 0) counters->n_surv = n_surv;  // for the host's grid hint
     for (unsigned int r0 = blockIdx.x * SGS_PREB_BLOCK; r0 < n_surv; r0 += gridDim.x * SGS_PREB_BLOCK) {
         const bool have = r0 + tid < n_surv;
         const int64_t i = have ? (int64_t)surv_list[r0 + tid] : 0;
@@ -442,14 +446,24 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     const bool wide = (n + 1023) / 1024 >= 4 * 148;
     const int span = wide ? 1024 : 256;
     const int blocks_a = (int)((n + span - 1) / span);
-    c->launches += blocks_a > 0 ? 2 : 1;
-    if (blocks_a > 0) {
+    // SGS_FLAG_TRACK_REUSE: the list built (with pose margins) by an earlier iteration still covers this pose
+    const bool cached = c->use_surv_cache && c->surv_valid;
+    unsigned int* n_surv = c->use_surv_cache ? c->surv_cnt : &c->counters->n_surv;
+    const bool run_a = blocks_a > 0 && !cached;
+    c->launches += run_a ? 2 : 1;
+    SgsCamDev cam_a = c->camd;
+    if (run_a && c->use_surv_cache) {  // this list has to cover the poses of the coming iterations too
+        if ((e = cudaMemsetAsync(c->surv_cnt, 0, sizeof(unsigned int), s)) != cudaSuccess) return e;
+        cam_a.pm_t = SGS_REUSE_MARGIN_T; cam_a.pm_r = SGS_REUSE_MARGIN_R;
+        c->surv_valid = true; c->surv_sf = *sf; c->surv_cam = c->last_cam;
+    }
+    if (run_a) {
         if (wide)
-            k_pre_select<4><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, c->camd, c->cfgd, c->culled,
-                                                               c->counters, c->vis_to_surfel);
+            k_pre_select<4><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, cam_a, c->cfgd, c->culled,
+                                                               n_surv, c->vis_to_surfel);
         else
-            k_pre_select<1><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, c->camd, c->cfgd, c->culled,
-                                                               c->counters, c->vis_to_surfel);
+            k_pre_select<1><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, cam_a, c->cfgd, c->culled,
+                                                               n_surv, c->vis_to_surfel);
     }
     // K-pre-B walks the survivor list with a grid-stride loop: the count is only known on the device
     // (the grid follows the last known survivor count)
@@ -469,10 +483,10 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = blocks_a > 0 ? 1 : 0;  // programmatic dependent launch behind K-pre-A
+    cfg.numAttrs = run_a ? 1 : 0;  // programmatic dependent launch behind K-pre-A
     const cudaError_t le = cudaLaunchKernelEx(&cfg, k_pre_project, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd,
                                               c->cfgd, c->pay, c->culled, c->counters, (const uint32_t*)c->vis_to_surfel,
-                                              c->cursor, c->bucket, (uint32_t)c->tile_cap);
+                                              (const unsigned int*)n_surv, c->cursor, c->bucket, (uint32_t)c->tile_cap);
     if (le != cudaSuccess) return le;
     return cudaGetLastError();
 }

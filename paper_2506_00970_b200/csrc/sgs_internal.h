@@ -38,7 +38,11 @@ struct SgsCamDev {
     // camera-only constants of the binary32 pre-cull (preprocess.cu precull_f32), filled on the host
     float pc_n[4];   // |(fx, cx)|, |(fx, cx - W)|, |(fy, cy)|, |(fy, cy - H)|, each rounded up by 1.00001
     float pc_cxr, pc_cyr, pc_tabs;  // cx - W, cy - H, |t|_1 + 1
+    float pm_t, pm_r;  // pose margin of the pre-cull (metres, radians): 0 unless a survivor list is built for reuse
 };
+
+// SGS_FLAG_TRACK_REUSE: a survivor list stays valid for poses within this translation / rotation of the pose it was built for
+constexpr float SGS_REUSE_MARGIN_T = 0.03f, SGS_REUSE_MARGIN_R = 0.02f;
 
 struct SgsCfgDev {
     float cutoff2, alpha_min, alpha_max, t_min, z_near;
@@ -110,6 +114,11 @@ struct sgs_ctx {
     cudaStream_t aux_stream;           // sgs_backward: the gradient memsets run beside k_backward (fork / join by events)
     cudaEvent_t fork_ev, join_ev;
     cudaEvent_t prepared_ev, work_ev;   // sgs_prepare: binning enqueued / the ctx's last render or backward enqueued
+    // SGS_FLAG_TRACK_REUSE: K-pre-A's survivor list (vis_to_surfel) outlives the iteration it was built in
+    unsigned int* surv_cnt;            // device: its length
+    bool surv_valid, use_surv_cache;   // list valid for (surv_sf, poses near surv_cam) / this preprocess launch uses it
+    sgs_surfels surv_sf;
+    sgs_camera surv_cam;
     int narrow_prepare;                // > 0 inside sgs_prepare: K-pre-B blocks per SM
     bool prepared, work_recorded;      // binning of (last_surfels, last_cam) enqueued by sgs_prepare, not yet rendered
     // last forward

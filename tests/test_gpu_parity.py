@@ -482,3 +482,56 @@ def test_prepare_then_render_equals_render():
         np.testing.assert_allclose(p6s[v].cpu().numpy(), refs[v][3], rtol=1e-4, atol=1e-5 * np.abs(refs[v][3]).max())
     for r in (ref_ren, ra, rb):
         r.close()
+
+
+def test_track_reuse_keeps_the_binning_exact():
+    """SGS_FLAG_TRACK_REUSE: along a pose trajectory (steps inside the survivor list's 3 cm / 0.02 rad margin, a step
+    that leaves it, another map, a new frame) every iteration's binning is bit-identical to the oracle's and images,
+    loss and pose gradient equal those of a context without the flag; the list is rebuilt exactly when it has to be
+    (kernel launch counts: 3 launches with K-pre-A, 2 without)."""
+    sc, _, _ = scenegen.make_config("C2", n_override=30000)
+    sc2 = Scene(sc.mean + np.float32(0.01), sc.scale, sc.quat, sc.opacity, sc.rgb, sc.active)
+    cfg = oracle.make_cfg()
+    t, sf = to_device(sc)
+    t2, sf2 = to_device(sc2)
+    T0 = scenegen.look_at(np.array([2.4, 0.6, 1.5]), np.array([2.6, 3.9, 1.2])).astype(np.float32)
+    base = Camera(208, 150, 150.0, 150.0, 104.0, 75.0, T0)
+    ra, rb = sgs.Renderer(track_reuse=True), sgs.Renderer()
+    im0 = alloc_images(base)
+    rb.render(sf, camera(base), **im0)
+    tgt_rgb, tgt_dep = (im0["rgb"] * 0.9 + 0.01).contiguous(), (im0["depth"] * 1.02).contiguous()
+    tiles = ((base.width + 15) // 16) * ((base.height + 15) // 16)
+    p0, l0_ = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+    ra.track_iter(sf, camera(base), tgt_rgb, tgt_dep, 0.5, -1.0, p0, l0_)   # first call: workspace + tile order set up
+    ra.track_new_frame()
+    # (tau relative to T0, which map, new frame first?, expected number of kernel launches of the iteration)
+    steps = [([0, 0, 0, 0, 0, 0], 0, False, 3),
+             ([0.01, -0.005, 0.008, 0.004, -0.006, 0.005], 0, False, 2),        # inside the margin: list reused
+             ([-0.015, 0.01, 0.005, -0.008, 0.004, -0.007], 0, False, 2),
+             ([0.05, 0.0, 0.02, 0.0, 0.03, 0.0], 0, False, 3),                   # outside: rebuilt around this pose
+             ([0.055, 0.004, 0.018, 0.003, 0.033, -0.004], 0, False, 2),        # inside the NEW list's margin
+             ([0.055, 0.004, 0.018, 0.003, 0.033, -0.004], 1, False, 3),        # another map
+             ([0.055, 0.004, 0.018, 0.003, 0.033, -0.004], 1, False, 2),
+             ([0.055, 0.004, 0.018, 0.003, 0.033, -0.004], 1, True, 3)]         # new frame
+    for tau, which, new_frame, want_launches in steps:
+        T = scenegen.perturb_pose(T0, tau)
+        cam = Camera(base.width, base.height, base.fx, base.fy, base.cx, base.cy, T)
+        c = camera(cam)
+        scene, s_dev = (sc, sf) if which == 0 else (sc2, sf2)
+        if new_frame:
+            ra.track_new_frame()
+        ima, imb = alloc_images(cam), alloc_images(cam)
+        pa, la = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+        pb, lb = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+        l0 = ra.stats()["kernel_launches"]
+        ra.track_iter(s_dev, c, tgt_rgb, tgt_dep, 0.5, -1.0, pa, la, **ima)
+        assert ra.stats()["kernel_launches"] - l0 == want_launches, (tau, which, new_frame)
+        rb.track_iter(s_dev, c, tgt_rgb, tgt_dep, 0.5, -1.0, pb, lb, **imb)
+        torch.cuda.synchronize()
+        ob = oracle.binning(scene, oracle.make_cam(cam), cfg)
+        assert ob["E"] > 1000
+        assert_binning(ra.get_binning(scene.n, tiles), ob)
+        assert np.array_equal(planes(ima), planes(imb))
+        np.testing.assert_allclose(la.cpu().numpy(), lb.cpu().numpy(), rtol=1e-5)
+        np.testing.assert_allclose(pa.cpu().numpy(), pb.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(pb.abs().max()))
+    ra.close(); rb.close()
