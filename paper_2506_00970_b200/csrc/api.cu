@@ -38,11 +38,12 @@ int sgs_ensure_surfels(sgs_ctx* c, int64_t n, cudaStream_t s) {
     const size_t m = (size_t)(n + n / 8 + 1024);
     const size_t blocks = (m + SGS_PRE_BLOCK - 1) / SGS_PRE_BLOCK + 1;
     bool ok = ws_realloc(c, c->scan_state, blocks, s) && ws_realloc(c, c->vis_to_surfel, m, s) &&
-              ws_realloc(c, c->culled, m, s) && ws_realloc(c, c->pay.g0, m, s) && ws_realloc(c, c->pay.g1, m, s) &&
-              ws_realloc(c, c->pay.g2, m, s) && ws_realloc(c, c->pay.g3, m, s) && ws_realloc(c, c->pay.g4, m, s) &&
-              ws_realloc(c, c->pay.g5, m, s) && ws_realloc(c, c->pay.g6, m, s) && ws_realloc(c, c->pay.g7, m, s) &&
+              ws_realloc(c, c->culled, m, s) && ws_realloc(c, c->pay.store, m * 8, s) &&
               ws_realloc(c, c->acc, m * SGS_ACC_STRIDE, s, true);  // invariant: acc is all-zero between backward calls
     if (!ok) return SGS_OUT_OF_MEMORY;
+    float4* st = c->pay.store;
+    c->pay.g0.base = st; c->pay.g1.base = st + 1; c->pay.g2.base = st + 2; c->pay.g3.base = st + 3;
+    c->pay.g4.base = st + 4; c->pay.g5.base = st + 5; c->pay.g6.base = st + 6; c->pay.g7.base = st + 7;
     c->n_cap = (int64_t)m;
     return SGS_OK;
 }
@@ -221,11 +222,10 @@ int sgs_destroy(sgs_ctx* c) {
     if (!c) return SGS_OK;
     cudaDeviceSynchronize();
     cudaStream_t s = 0;
-    void* ptrs[] = {c->scan_state, c->vis_to_surfel, c->culled, c->pay.g0, c->pay.g1, c->pay.g2, c->pay.g3, c->pay.g4,
-                    c->pay.g5, c->pay.g6, c->pay.g7, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
+    void* ptrs[] = {c->scan_state, c->vis_to_surfel, c->culled, c->pay.store, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
                     c->sort_state, c->ranges, c->T_final, c->n_last, c->img_scratch, c->pose_partial, c->resident_store,
                     c->resident_active, c->target_rgb, c->host_img_dev, c->host_up_dev, c->host_grads_dev,
-                    c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->pose_inc, c->ssim_maps, c->surv_cnt, c->export_keys, c->export_ranges};
+                    c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->pose_inc, c->ssim_maps, c->surv_cnt, c->surv_in, c->export_keys, c->export_ranges};
     for (void* p : ptrs) sgs_ws_free(c, p, s);
     if (c->counters) cudaFree(c->counters);
     if (c->counters_snap) cudaFree(c->counters_snap);

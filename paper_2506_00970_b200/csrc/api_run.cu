@@ -242,6 +242,12 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
     }
     if ((c->cfg.flags & SGS_FLAG_TRACK_REUSE) && sf && sgs_cam_valid(cam)) {
         if (!c->surv_cnt && !(c->surv_cnt = (unsigned int*)sgs_ws_alloc(c, sizeof(unsigned int), s))) return SGS_OUT_OF_MEMORY;
+        if (c->surv_in_cap < sf->n) {  // 52 B per splat of the map at most; every survivor list fits
+            if (c->surv_in) sgs_ws_free(c, c->surv_in, s);
+            c->surv_in_cap = 0; c->surv_valid = false;
+            if (!(c->surv_in = sgs_ws_alloc(c, 52 * (size_t)sf->n + 64, s))) return SGS_OUT_OF_MEMORY;
+            c->surv_in_cap = sf->n;
+        }
         if (c->surv_valid && !(memcmp(&c->surv_sf, sf, sizeof(*sf)) == 0 && pose_within_margin(&c->surv_cam, cam)))
             c->surv_valid = false;  // another map, or the pose has left the list's margin: build it again, centred here
         c->use_surv_cache = true;

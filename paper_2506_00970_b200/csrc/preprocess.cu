@@ -305,6 +305,24 @@ k_pre_select(int64_t n, const float* __restrict__ mean, const float* __restrict_
     for (unsigned int k = tid; k < ns; k += SGS_PRE_BLOCK) surv_list[gb + k] = (uint32_t)(base + s_list[k]);
 }
 
+// SGS_FLAG_TRACK_REUSE: one copy of the listed splats' parameters in list order (52 B each, 7.8 MB for 150 k survivors:
+// resident in L2 across the iterations of a frame), so that K-pre-B reads coalesced lines instead of gathering 12-16 B
+// pieces of a map that does not fit the L2 (ncu, C5: 43 % of its stall samples were those gathers, L2 hit rate 7 %).
+__global__ void __launch_bounds__(256)
+k_surv_gather(const uint32_t* __restrict__ surv_list, const unsigned int* __restrict__ n_surv_in,
+              const float* __restrict__ mean, const float* __restrict__ scale, const float* __restrict__ quat,
+              const float* __restrict__ opacity, const float* __restrict__ rgb, float4* __restrict__ p0,
+              float4* __restrict__ p1, float4* __restrict__ p2, float* __restrict__ p3) {
+    const unsigned int n = *n_surv_in;
+    for (unsigned int j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+        const size_t i = surv_list[j];
+        p0[j] = make_float4(mean[3 * i], mean[3 * i + 1], mean[3 * i + 2], opacity[i]);
+        p1[j] = make_float4(quat[4 * i], quat[4 * i + 1], quat[4 * i + 2], quat[4 * i + 3]);
+        p2[j] = make_float4(scale[2 * i], scale[2 * i + 1], rgb[3 * i], rgb[3 * i + 1]);
+        p3[j] = rgb[3 * i + 2];
+    }
+}
+
 constexpr int SGS_PREB_BLOCK = 128, SGS_PREB_LOG2 = 7, PREB_EMIT = 4;  // K-pre-B block: small, so that few survivors still spread over the SMs
 
 __global__ void __launch_bounds__(SGS_PREB_BLOCK)
@@ -312,7 +330,7 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
               const float* __restrict__ opacity, const float* __restrict__ rgb, SgsCamDev cam, SgsCfgDev cfg,
               SgsPayload pay, uint8_t* __restrict__ culled, SgsCounters* __restrict__ counters,
               const uint32_t* __restrict__ surv_list, const unsigned int* __restrict__ n_surv_in,
-              uint32_t* __restrict__ cursor, uint64_t* __restrict__ bucket, uint32_t tile_cap) {
+              uint32_t* __restrict__ cursor, uint64_t* __restrict__ bucket, uint32_t tile_cap, SurvInputs cin) {
     __shared__ unsigned int s_off[SGS_PREB_BLOCK + 1];
     __shared__ unsigned long long s_key[SGS_PREB_BLOCK];
     __shared__ unsigned int s_rect[SGS_PREB_BLOCK];   // tile index of the rectangle's first tile
@@ -328,8 +346,19 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
         PreOut o;
         o.vis = false;
         o.depth_bits = 0;
+        float in_m[3] = {0.f, 0.f, 0.f}, in_s[2] = {0.f, 0.f}, in_q[4] = {0.f, 0.f, 0.f, 0.f}, in_o = 0.f, in_c[3] = {0.f, 0.f, 0.f};
         if (have) {
-            preprocess_one(mean + 3 * i, scale + 2 * i, quat + 4 * i, cam, cfg, o);
+            if (cin.p0) {  // SGS_FLAG_TRACK_REUSE: the survivors' parameters, copied in list order when the list was built
+                const float4 a = cin.p0[r0 + tid], q = cin.p1[r0 + tid], c2 = cin.p2[r0 + tid];
+                in_m[0] = a.x; in_m[1] = a.y; in_m[2] = a.z; in_o = a.w;
+                in_q[0] = q.x; in_q[1] = q.y; in_q[2] = q.z; in_q[3] = q.w;
+                in_s[0] = c2.x; in_s[1] = c2.y; in_c[0] = c2.z; in_c[1] = c2.w; in_c[2] = cin.p3[r0 + tid];
+            } else {
+                in_m[0] = mean[3 * i]; in_m[1] = mean[3 * i + 1]; in_m[2] = mean[3 * i + 2];
+                in_s[0] = scale[2 * i]; in_s[1] = scale[2 * i + 1];
+                in_q[0] = quat[4 * i]; in_q[1] = quat[4 * i + 1]; in_q[2] = quat[4 * i + 2]; in_q[3] = quat[4 * i + 3];
+            }
+            preprocess_one(in_m, in_s, in_q, cam, cfg, o);
             culled[i] = o.vis ? 0 : 1;
         }
         const unsigned int cnt = o.vis ? (unsigned int)((o.tx1 - o.tx0 + 1) * (o.ty1 - o.ty0 + 1)) : 0u;
@@ -343,11 +372,12 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
             atomicAdd(&counters->n_entries, (unsigned long long)wcnt);
         }
         if (o.vis) {
+            if (!cin.p0) { in_o = opacity[i]; in_c[0] = rgb[3 * i]; in_c[1] = rgb[3 * i + 1]; in_c[2] = rgb[3 * i + 2]; }
             pay.g0[i] = make_float4(o.P, o.Q, o.R, o.S);
-            pay.g1[i] = make_float4(o.D, o.E, o.F, opacity[i]);
+            pay.g1[i] = make_float4(o.D, o.E, o.F, in_o);
             pay.g2[i] = make_double2(o.xc, o.yc);
-            pay.g3[i] = make_float4(o.a, o.b, o.c, rgb[3 * i]);
-            pay.g4[i] = make_float4(rgb[3 * i + 1], rgb[3 * i + 2], o.n[0], o.n[1]);
+            pay.g3[i] = make_float4(o.a, o.b, o.c, in_c[0]);
+            pay.g4[i] = make_float4(in_c[1], in_c[2], o.n[0], o.n[1]);
             pay.g5[i] = make_float4(o.n[2], o.au[0], o.au[1], o.au[2]);
             pay.g6[i] = make_float4(o.av[0], o.av[1], o.av[2], 0.f);
             pay.g7[i] = make_float4(o.bb[0], o.bb[1], o.bb[2], o.bb[3]);
@@ -465,6 +495,17 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
             k_pre_select<1><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, cam_a, c->cfgd, c->culled,
                                                                n_surv, c->vis_to_surfel);
     }
+    SurvInputs cin = {nullptr, nullptr, nullptr, nullptr};
+    if (c->use_surv_cache && c->surv_in) {
+        cin.p0 = reinterpret_cast<float4*>(c->surv_in);
+        cin.p1 = cin.p0 + c->surv_in_cap; cin.p2 = cin.p1 + c->surv_in_cap;
+        cin.p3 = reinterpret_cast<float*>(cin.p2 + c->surv_in_cap);
+        if (run_a) {
+            c->launches += 1;
+            k_surv_gather<<<148 * 4, 256, 0, s>>>(c->vis_to_surfel, n_surv, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb,
+                                                 cin.p0, cin.p1, cin.p2, cin.p3);
+        }
+    }
     // K-pre-B walks the survivor list with a grid-stride loop: the count is only known on the device
     // (the grid follows the last known survivor count)
     int64_t blocks_b = (n + SGS_PREB_BLOCK - 1) / SGS_PREB_BLOCK;
@@ -483,10 +524,10 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = run_a ? 1 : 0;  // programmatic dependent launch behind K-pre-A
+    cfg.numAttrs = (run_a && !cin.p0) ? 1 : 0;  // programmatic dependent launch behind K-pre-A
     const cudaError_t le = cudaLaunchKernelEx(&cfg, k_pre_project, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd,
                                               c->cfgd, c->pay, c->culled, c->counters, (const uint32_t*)c->vis_to_surfel,
-                                              (const unsigned int*)n_surv, c->cursor, c->bucket, (uint32_t)c->tile_cap);
+                                              (const unsigned int*)n_surv, c->cursor, c->bucket, (uint32_t)c->tile_cap, cin);
     if (le != cudaSuccess) return le;
     return cudaGetLastError();
 }

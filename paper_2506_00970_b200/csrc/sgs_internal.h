@@ -16,15 +16,25 @@
 // Screen-centred adjugate form of the ray-splat intersection:
 //   xt = x - x_c, yt = y - y_c  (x_c, y_c = projected centre, kept in fp64)
 //   u = (xt P + yt Q) / den,  v = (xt R + yt S) / den,  den = D - xt E - yt F,  z = a u + b v + c
+// Per-surfel payload written by the preprocess and gathered by the compositing kernels: ONE 128-byte record per surfel
+// (eight 16-byte fields), so that a record is four whole 32-byte sectors.  As eight separate planes every field was
+// half a sector: K-pre-B's stores cost a read-fill each (ncu, C5: 145 MB read for 17 MB of inputs) and the gathers
+// fetched seven half-used sectors per entry.  g<k>[v] addresses field k of surfel v as before.
+template <typename T>
+struct PayField {
+    float4* base;  // record 0's field
+    __device__ __forceinline__ T& operator[](size_t v) const { return reinterpret_cast<T*>(base)[v * 8]; }
+};
 struct SgsPayload {
-    float4* g0;   // P, Q, R, S
-    float4* g1;   // D, E, F, opacity
-    double2* g2;  // x_c, y_c
-    float4* g3;   // a, b, c (= M20, M21, M22), rgb.r
-    float4* g4;   // rgb.g, rgb.b, n_c.x, n_c.y
-    float4* g5;   // n_c.z, a_u.x, a_u.y, a_u.z      (a_u = s_u t_uc, camera space)
-    float4* g6;   // a_v.x, a_v.y, a_v.z, unused     (a_v = s_v t_vc)
-    float4* g7;   // screen AABB of the cutoff ellipse: xmin, xmax, ymin, ymax (rounded outward)
+    PayField<float4> g0;   // P, Q, R, S
+    PayField<float4> g1;   // D, E, F, opacity
+    PayField<double2> g2;  // x_c, y_c
+    PayField<float4> g3;   // a, b, c (= M20, M21, M22), rgb.r
+    PayField<float4> g4;   // rgb.g, rgb.b, n_c.x, n_c.y
+    PayField<float4> g5;   // n_c.z, a_u.x, a_u.y, a_u.z      (a_u = s_u t_uc, camera space)
+    PayField<float4> g6;   // a_v.x, a_v.y, a_v.z, unused     (a_v = s_v t_vc)
+    PayField<float4> g7;   // screen AABB of the cutoff ellipse: xmin, xmax, ymin, ymax (rounded outward)
+    float4* store;         // n x 8 float4
 };
 
 struct SgsCamDev {
@@ -43,6 +53,8 @@ struct SgsCamDev {
 
 // SGS_FLAG_TRACK_REUSE: a survivor list stays valid for poses within this translation / rotation of the pose it was built for
 constexpr float SGS_REUSE_MARGIN_T = 0.03f, SGS_REUSE_MARGIN_R = 0.02f;
+
+struct SurvInputs { float4 *p0, *p1, *p2; float* p3; };  // (mean, opacity), quat, (scale, r, g), b
 
 struct SgsCfgDev {
     float cutoff2, alpha_min, alpha_max, t_min, z_near;
@@ -116,6 +128,7 @@ struct sgs_ctx {
     cudaEvent_t prepared_ev, work_ev;   // sgs_prepare: binning enqueued / the ctx's last render or backward enqueued
     // SGS_FLAG_TRACK_REUSE: K-pre-A's survivor list (vis_to_surfel) outlives the iteration it was built in
     unsigned int* surv_cnt;            // device: its length
+    void* surv_in; int64_t surv_in_cap; // the listed splats' parameters in list order (3 float4 planes + 1 float plane)
     bool surv_valid, use_surv_cache;   // list valid for (surv_sf, poses near surv_cam) / this preprocess launch uses it
     sgs_surfels surv_sf;
     sgs_camera surv_cam;
