@@ -31,6 +31,7 @@ int sgs_upload_surfels(sgs_ctx* c, const sgs_surfels* h, void* stream) {
         return SGS_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     const int64_t n = h->n;
+    c->surv_valid = false;  // SGS_FLAG_TRACK_REUSE: the resident map is being rewritten
     if (n > c->resident_cap) {
         cudaStreamSynchronize(s);
         sgs_ws_free(c, c->resident_store, s);
