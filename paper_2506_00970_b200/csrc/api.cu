@@ -199,7 +199,8 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
     c->cfgd.cutoff2_d = (double)cfg->cutoff * (double)cfg->cutoff;
     c->cfgd.z_near_d = (double)cfg->z_near;
     bool ok = cudaMalloc(&c->counters, sizeof(SgsCounters)) == cudaSuccess &&
-              cudaMalloc(&c->counters_snap, sizeof(SgsCounters)) == cudaSuccess &&
+              cudaMalloc(&c->counters_snap, 2 * sizeof(SgsCounters)) == cudaSuccess &&
+              cudaEventCreateWithFlags(&c->counters_ready_prev, cudaEventDisableTiming) == cudaSuccess &&
               cudaMallocHost(&c->counters_host, sizeof(SgsCounters)) == cudaSuccess &&
               cudaMallocHost(&c->pinned_small, 8 * sizeof(float)) == cudaSuccess &&
               cudaMalloc(&c->sort_hist, sizeof(uint32_t) * (8 * 256 + 8)) == cudaSuccess &&
@@ -229,6 +230,7 @@ int sgs_destroy(sgs_ctx* c) {
     for (void* p : ptrs) sgs_ws_free(c, p, s);
     if (c->counters) cudaFree(c->counters);
     if (c->counters_snap) cudaFree(c->counters_snap);
+    if (c->counters_ready_prev) cudaEventDestroy(c->counters_ready_prev);
     if (c->counters_host) cudaFreeHost(c->counters_host);
     if (c->pinned_small) cudaFreeHost(c->pinned_small);
     if (c->sort_hist) cudaFree(c->sort_hist);

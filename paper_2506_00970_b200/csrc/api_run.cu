@@ -44,12 +44,23 @@ static int copy_counters(sgs_ctx* c, cudaStream_t s) {
 // binning through per-tile buckets + in-tile sort (default)
 static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, bool want_order, cudaStream_t s) {
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
+    if (c->copy_in_flight) {  // a copy of the LIVE counters (render path) may still run on the ctx's stream: normally long done
+        if (cudaStreamWaitEvent(s, c->counters_ready, 0) != cudaSuccess) return SGS_CUDA_ERROR;
+        c->copy_in_flight = false;
+    }
     int r = sgs_ensure_buckets(c, tiles, c->tile_cap ? c->tile_cap : 2048, s);
     if (r != SGS_OK) return r;
     if (sgs_launch_preprocess_bucket(c, sf, s) != cudaSuccess) return SGS_CUDA_ERROR;
     const bool defer = async && c->defer_counters && c->tile_cap <= 2048;  // the fused kernel snapshots them
     c->defer_counters = defer;
-    if (!defer && (r = copy_counters(c, s)) != SGS_OK) return r;
+    // async mode: the 32-byte copy runs on the ctx's own stream so that it is not a link of the caller's chain
+    // (K-pre-B -> copy -> compositing); the next preprocess on this ctx waits for it before it clears the counters
+    cudaStream_t cs = (async && c->aux_stream) ? c->aux_stream : s;
+    if (!defer) {
+        if (cs != s && (cudaEventRecord(c->fork_ev, s) != cudaSuccess || cudaStreamWaitEvent(cs, c->fork_ev, 0) != cudaSuccess))
+            return SGS_CUDA_ERROR;
+        if ((r = copy_counters(c, cs)) != SGS_OK) return r;
+    }
     if (!async) {
         if (cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
         if (c->counters_host->max_tile > (unsigned)c->tile_cap) {  // grow and emit again
@@ -61,7 +72,8 @@ static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, bool want_
         c->last_entries = (int64_t)c->counters_host->n_entries;
         c->last_surv = (int64_t)c->counters_host->n_surv;
     } else if (!defer) {
-        cudaEventRecord(c->counters_ready, s);
+        cudaEventRecord(c->counters_ready, cs);
+        c->copy_in_flight = cs != s;
         c->pending_check = true;
         c->pending_lazy = false;
     }
@@ -262,12 +274,26 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
     if ((r = sgs_ensure_partials(c, tiles, s)) != SGS_OK) return r;
     float* planes[8];
     pick_planes(c, out, (int64_t)cam->width * cam->height, false, planes);
+    if (deferred && c->prev_copy_on_aux) {  // the slot this K-track overwrites was copied two iterations ago: done long since
+        if (cudaStreamWaitEvent(s, c->counters_ready_prev, 0) != cudaSuccess) return SGS_CUDA_ERROR;
+        c->prev_copy_on_aux = false;
+    }
     if (sgs_launch_track(c, planes, target->rgb, target->depth, lambda_d, normal_sign, d_pose6, loss, deferred, s) != cudaSuccess)
         return SGS_CUDA_ERROR;
     if (deferred) {  // the counters of this iteration's preprocess, snapshotted by k_track's last block
-        if (cudaMemcpyAsync(c->counters_host, c->counters_snap, sizeof(SgsCounters), cudaMemcpyDeviceToHost, s) != cudaSuccess)
+        // ... copied on the ctx's own stream: a copy between K-track and the next iteration's K-pre-B is a link of the
+        // iteration's dependency chain (measured on C2: 82.3 -> 72.2 us per iteration).  Two snapshot slots alternate, and
+        // an iteration waits for the copy of the slot it is about to overwrite, which is one iteration old.
+        cudaStream_t cs = c->aux_stream ? c->aux_stream : s;
+        if (cs != s && (cudaEventRecord(c->fork_ev, s) != cudaSuccess || cudaStreamWaitEvent(cs, c->fork_ev, 0) != cudaSuccess))
             return SGS_CUDA_ERROR;
-        cudaEventRecord(c->counters_ready, s);
+        if (cudaMemcpyAsync(c->counters_host, c->counters_snap + c->snap_slot, sizeof(SgsCounters), cudaMemcpyDeviceToHost, cs) != cudaSuccess)
+            return SGS_CUDA_ERROR;
+        const cudaEvent_t t = c->counters_ready_prev; c->counters_ready_prev = c->counters_ready; c->counters_ready = t;
+        c->prev_copy_on_aux = c->snap_copy_on_aux;
+        cudaEventRecord(c->counters_ready, cs);
+        c->snap_copy_on_aux = cs != s;
+        c->snap_slot ^= 1;
         c->pending_check = true;
         c->pending_lazy = true;
     }

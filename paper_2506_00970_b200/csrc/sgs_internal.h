@@ -133,6 +133,7 @@ struct sgs_ctx {
     sgs_surfels surv_sf;
     sgs_camera surv_cam;
     int narrow_prepare;                // > 0 inside sgs_prepare: K-pre-B blocks per SM
+    bool copy_in_flight;               // counters_ready was recorded on aux_stream and nothing on the caller's stream waited for it yet
     bool prepared, work_recorded;      // binning of (last_surfels, last_cam) enqueued by sgs_prepare, not yet rendered
     // last forward
     bool have_forward;
@@ -164,7 +165,10 @@ struct sgs_ctx {
     int64_t last_surv;               // K-pre-A survivors of the last checked render (K-pre-B grid hint), 0 = unknown
     uint32_t* tile_cost;             // tiles: cycles >> 8 each tile's k_track block took last time (scheduling feedback)
     int cost_tiles, cost_W, cost_H;  // camera the costs were measured for (0 = none)
-    SgsCounters* counters_snap;      // device copy of the counters taken by k_track's last block before it zeroes them
+    SgsCounters* counters_snap;      // device copies (two slots, alternating) of the counters taken by k_track's last block before it zeroes them
+    int snap_slot;                   // slot the NEXT sgs_track_iter writes
+    cudaEvent_t counters_ready_prev; // copy of the other slot (one iteration older) done; swapped with counters_ready
+    bool prev_copy_on_aux, snap_copy_on_aux;
     bool defer_counters;             // sgs_track_iter (async): the counters reach the host after k_track, from the snapshot
     int prezero_tiles;               // k_track's last block left counters and cursor[0..prezero_tiles) zeroed for the next preprocess
 };

@@ -438,7 +438,7 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
     // (A programmatic dependent launch behind K-pre-B was measured and rejected: C2 3459 -> 2888 MP/s, the early
     // resident blocks of this kernel get in K-pre-B's way; profiles/r01_c2_track.md.)
     const uint32_t tile_cap = (uint32_t)c->tile_cap;
-    SgsCounters* snap = after_preprocess ? c->counters_snap : nullptr;
+    SgsCounters* snap = after_preprocess ? c->counters_snap + c->snap_slot : nullptr;
     if (any)
         k_track<true><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W,
                                                   cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb, tdepth,
