@@ -464,7 +464,8 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     const int64_t n = sf->n;
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
     cudaError_t e = cudaSuccess;
-    if (c->prezero_tiles < tiles) {  // else: the previous sgs_track_iter's kernel already zeroed both (two stream ops saved)
+    const bool prezeroed = c->prezero_tiles >= tiles;
+    if (!prezeroed) {  // else: the previous sgs_track_iter's kernel already zeroed both (two stream ops saved)
         e = cudaMemsetAsync(c->counters, 0, sizeof(SgsCounters), s);
         if (e != cudaSuccess) return e;
         e = cudaMemsetAsync(c->cursor, 0, sizeof(uint32_t) * (size_t)tiles, s);
@@ -524,7 +525,8 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = (run_a && !cin.p0) ? 1 : 0;  // programmatic dependent launch behind K-pre-A
+    // programmatic dependent launch behind K-pre-A, or (list reused, previous launch on the stream = K-track) behind K-track
+    cfg.numAttrs = ((run_a && !cin.p0) || (cached && prezeroed)) ? 1 : 0;
     const cudaError_t le = cudaLaunchKernelEx(&cfg, k_pre_project, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd,
                                               c->cfgd, c->pay, c->culled, c->counters, (const uint32_t*)c->vis_to_surfel,
                                               (const unsigned int*)n_surv, c->cursor, c->bucket, (uint32_t)c->tile_cap, cin);

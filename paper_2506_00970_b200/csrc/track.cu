@@ -59,6 +59,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
         float* __restrict__ loss_out, uint32_t* __restrict__ tile_cost, uint32_t* cursor_rw, SgsCounters* __restrict__ counters_snap) {
     const long long t_start = clock64();
+    cudaTriggerProgrammaticLaunchCompletion();  // the next iteration's K-pre-B may be staged; it waits for this grid before it reads anything
     __shared__ float4 sh[7][SGS_BLOCK];
     __shared__ unsigned long long s_keys[SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
