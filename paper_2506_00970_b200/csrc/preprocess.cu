@@ -329,20 +329,24 @@ __global__ void __launch_bounds__(SGS_PREB_BLOCK)
 k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, const float* __restrict__ quat,
               const float* __restrict__ opacity, const float* __restrict__ rgb, SgsCamDev cam, SgsCfgDev cfg,
               SgsPayload pay, uint8_t* __restrict__ culled, SgsCounters* __restrict__ counters,
-              const uint32_t* __restrict__ surv_list, const unsigned int* __restrict__ n_surv_in,
-              uint32_t* __restrict__ cursor, uint64_t* __restrict__ bucket, uint32_t tile_cap, SurvInputs cin) {
+              const uint32_t* surv_list, const unsigned int* n_surv_in,  // written by the PREVIOUS grid: no __restrict__,
+              // or the compiler may hoist their loads above the conditional grid-dependency wait (it did: stale counts)
+              uint32_t* __restrict__ cursor, uint64_t* __restrict__ bucket, uint32_t tile_cap, SurvInputs cin, int early) {
     __shared__ unsigned int s_off[SGS_PREB_BLOCK + 1];
     __shared__ unsigned long long s_key[SGS_PREB_BLOCK];
     __shared__ unsigned int s_rect[SGS_PREB_BLOCK];   // tile index of the rectangle's first tile
     __shared__ unsigned int s_w[SGS_PREB_BLOCK];      // rectangle width in tiles
     __shared__ unsigned int s_wsum[SGS_PREB_BLOCK / 32];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    cudaGridDependencySynchronize();                // K-pre-A complete: survivor list and count are final
-    const unsigned int n_surv = *n_surv_in;   // written by K-pre-A (previous launch on the stream, or an earlier iteration)
-    if (n_surv_in != &counters->n_surv && blockIdx.x == 0 && tid == 0) counters->n_surv = n_surv;  // for the host's grid hint
+    // early (list and inputs kept from an earlier iteration, this grid staged programmatically behind K-track): nothing
+    // the first round reads is written by the previous kernel, so its loads and the projection run before the wait and
+    // only the stores (records K-track still gathers, cursors it zeroes at its end) stay behind it
+    bool must_wait = early != 0;
+    if (!must_wait) cudaGridDependencySynchronize();   // K-pre-A complete: survivor list and count are final
+    const unsigned int n_surv = *(const volatile unsigned int*)n_surv_in;   // written by K-pre-A (previous launch on the stream, or an earlier iteration)
     for (unsigned int r0 = blockIdx.x * SGS_PREB_BLOCK; r0 < n_surv; r0 += gridDim.x * SGS_PREB_BLOCK) {
         const bool have = r0 + tid < n_surv;
-        const int64_t i = have ? (int64_t)surv_list[r0 + tid] : 0;
+        const int64_t i = have ? (int64_t)__ldcg(surv_list + r0 + tid) : 0;
         PreOut o;
         o.vis = false;
         o.depth_bits = 0;
@@ -359,8 +363,10 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
                 in_q[0] = quat[4 * i]; in_q[1] = quat[4 * i + 1]; in_q[2] = quat[4 * i + 2]; in_q[3] = quat[4 * i + 3];
             }
             preprocess_one(in_m, in_s, in_q, cam, cfg, o);
-            culled[i] = o.vis ? 0 : 1;
         }
+        if (must_wait) { cudaGridDependencySynchronize(); must_wait = false; }
+        if (n_surv_in != &counters->n_surv && r0 == 0 && tid == 0) counters->n_surv = n_surv;  // for the host's grid hint
+        if (have) culled[i] = o.vis ? 0 : 1;
         const unsigned int cnt = o.vis ? (unsigned int)((o.tx1 - o.tx0 + 1) * (o.ty1 - o.ty0 + 1)) : 0u;
         // totals: one atomic per warp
         const unsigned int vis_mask = __ballot_sync(0xffffffffu, o.vis);
@@ -529,7 +535,8 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     cfg.numAttrs = ((run_a && !cin.p0) || (cached && prezeroed)) ? 1 : 0;
     const cudaError_t le = cudaLaunchKernelEx(&cfg, k_pre_project, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd,
                                               c->cfgd, c->pay, c->culled, c->counters, (const uint32_t*)c->vis_to_surfel,
-                                              (const unsigned int*)n_surv, c->cursor, c->bucket, (uint32_t)c->tile_cap, cin);
+                                              (const unsigned int*)n_surv, c->cursor, c->bucket, (uint32_t)c->tile_cap, cin,
+                                              (cached && prezeroed && cin.p0) ? 1 : 0);
     if (le != cudaSuccess) return le;
     return cudaGetLastError();
 }
