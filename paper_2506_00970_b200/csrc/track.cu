@@ -436,8 +436,9 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
     c->launches += 1;
     unsigned long long* bucket = reinterpret_cast<unsigned long long*>(c->bucket);
     const int presorted = c->fused_sort ? 0 : 1;
-    // (A programmatic dependent launch behind K-pre-B was measured and rejected: C2 3459 -> 2888 MP/s, the early
-    // resident blocks of this kernel get in K-pre-B's way; profiles/r01_c2_track.md.)
+    // (A programmatic dependent launch of THIS kernel behind K-pre-B was measured twice: 3459 -> 2888 MP/s when K-pre-B
+    // triggered at its start, and no change (4483 vs 4468) with the trigger behind K-pre-B's own wait and the target-pixel
+    // loads in front of this kernel's wait; profiles/r01_c2_track.md.  The other edge, K-pre-B behind this kernel, pays.)
     const uint32_t tile_cap = (uint32_t)c->tile_cap;
     SgsCounters* snap = after_preprocess ? c->counters_snap + c->snap_slot : nullptr;
     if (any)
