@@ -139,7 +139,11 @@ class Workload:
         self.ren = sgs.Renderer(async_mode=True, track_reuse=self.tracking and reuse)
         # mapping window: a second context + a side stream, so that sgs_prepare (binning) of view v+1 runs under the
         # compositing kernels of view v (include/sgs.h); tracking iterations depend on one another and use one context
-        self.rens = [self.ren] + ([sgs.Renderer(async_mode=True)] if (prefetch and not self.tracking and len(self.cams) > 1) else [])
+        two = prefetch and not self.tracking and len(self.cams) > 1
+        if two:  # + SGS_FLAG_LAZY_GRADS: a view's per-surfel kernel runs under the next view's forward; joined at the step's end
+            self.ren.close()
+            self.ren = sgs.Renderer(async_mode=True, lazy_grads=True)
+        self.rens = [self.ren] + ([sgs.Renderer(async_mode=True, lazy_grads=True)] if two else [])
         self.side = torch.cuda.Stream(priority=-1) if len(self.rens) > 1 else None
         cam0 = self.cams[0]
         self.H, self.W = cam0.height, cam0.width
@@ -160,9 +164,13 @@ class Workload:
             self.targets.append((self.im["rgb"].clone(), self.im["depth"].clone()))
         if not self.tracking:
             n = sc.n
-            self.grads = dict(mean=torch.zeros(n, 3, device="cuda"), scale=torch.zeros(n, 2, device="cuda"),
+            mk = lambda: dict(mean=torch.zeros(n, 3, device="cuda"), scale=torch.zeros(n, 2, device="cuda"),
                               quat=torch.zeros(n, 4, device="cuda"), opacity=torch.zeros(n, device="cuda"),
                               rgb=torch.zeros(n, 3, device="cuda"))
+            self.grads = mk()
+            # one set of gradient buffers (and pose gradient) per context: with lazy gradients two views' are in flight
+            self.grads_of = {id(r): (self.grads if k == 0 else mk()) for k, r in enumerate(self.rens)}
+            self.p6_of = {id(r): (self.p6 if k == 0 else torch.zeros(6, device="cuda")) for k, r in enumerate(self.rens)}
         self.renders_per_step = self.iters if self.tracking else len(self.cams)
         for r in self.rens[1:]:   # the second context's workspace settles on the same views
             for c in self.ccams:
@@ -200,7 +208,7 @@ class Workload:
         u = self.up
         if True:
             ren.backward(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"],
-                              grads=self.grads, d_pose6=self.p6)
+                         grads=self.grads_of[id(ren)], d_pose6=self.p6_of[id(ren)])
 
     def step(self):
         if self.tracking:
@@ -220,6 +228,8 @@ class Workload:
                     self.rens[(v + 1) % 2].prepare(self.sf, self.ccams[v + 1], stream=self.side)
                 self.one(v, self.rens[v % 2])   # its render finds the binning prepared and orders itself behind it
             main.wait_stream(self.side)
+            for r in self.rens:
+                r.wait_grads()   # the step ends when every view's gradients are complete
 
     def flush_l2(self):
         self.flush_buf.zero_()

@@ -63,7 +63,8 @@ enum {
     SGS_FLAG_ASYNC = 1,         /* never synchronise the host in sgs_render (CUDA-graph capturable) */
     SGS_FLAG_RADIX_BINNING = 2, /* bin with the global LSD radix sort of the 64-bit keys instead of the
                                    default per-tile buckets + in-tile sort; same list, kept for A/B checks */
-    SGS_FLAG_TRACK_REUSE = 4    /* sgs_track_iter: the map is frozen between sgs_track_new_frame calls, see there */
+    SGS_FLAG_TRACK_REUSE = 4,   /* sgs_track_iter: the map is frozen between sgs_track_new_frame calls, see there */
+    SGS_FLAG_LAZY_GRADS = 8     /* sgs_backward: d_surfels / d_pose6 are complete only behind sgs_wait_grads, see there */
 };
 
 /* Truncation conventions of Eq. 8 (R3-R7).  sgs_default_config fills the defaults shown. */
@@ -179,6 +180,13 @@ SGS_API int sgs_covisibility(sgs_ctx* ctx, const float* contrib_a, const float* 
  * SGS_WORKSPACE_OVERFLOW (async mode: that render had overflowed; render again), SGS_OUT_OF_MEMORY, SGS_CUDA_ERROR. */
 SGS_API int sgs_backward(sgs_ctx* ctx, const sgs_images* upstream, const sgs_surfel_grads* d_surfels, float* d_pose6,
                  void* cuda_stream);
+
+/* SGS_FLAG_LAZY_GRADS.  The last kernel of a full sgs_backward (per-surfel chain rule Eq. 9-10, pose reduction Eq. 13,
+ * latency-bound) then stays on a stream of the ctx and `cuda_stream` does not wait for it, so that the next view's
+ * kernels (another ctx, same caller stream) run meanwhile.  d_surfels and d_pose6 of that call are complete on a stream
+ * only after sgs_wait_grads(ctx, that stream); the ctx orders its own later calls behind the kernel by itself.
+ * Without the flag sgs_wait_grads is a no-op. */
+SGS_API int sgs_wait_grads(sgs_ctx* ctx, void* cuda_stream);
 
 /* Tracking loss of Eq. 15-19 (harness around the renderer; R18, R19):
  *   L_t = 1/|Omega| sum_p M_n M_o (|I_r - I|_1 + lambda_d |D_r - D|)

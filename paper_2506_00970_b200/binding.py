@@ -16,6 +16,7 @@ SGS_OK, SGS_INVALID_ARGUMENT, SGS_OUT_OF_MEMORY, SGS_WORKSPACE_OVERFLOW, SGS_NO_
 SGS_FLAG_ASYNC = 1
 SGS_FLAG_RADIX_BINNING = 2
 SGS_FLAG_TRACK_REUSE = 4
+SGS_FLAG_LAZY_GRADS = 8
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
 FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p, C.c_void_p)
@@ -51,7 +52,7 @@ class sgs_stats(C.Structure):
                 ("workspace_bytes", C.c_int64), ("kernel_launches", C.c_int64)]
 
 
-EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_prepare", "sgs_backward", "sgs_tracking_loss",
+EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_prepare", "sgs_backward", "sgs_wait_grads", "sgs_tracking_loss",
            "sgs_backward_tracking", "sgs_track_iter", "sgs_track_new_frame", "sgs_render_contrib", "sgs_covisibility", "sgs_mapping_loss", "sgs_ssim_loss", "sgs_map_correction", "sgs_measure_fp32_peak", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
            "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string"]
 
@@ -135,7 +136,7 @@ class Renderer:
     """One sgs_ctx.  Method names follow the C calls (sgs_render -> render, ...)."""
 
     def __init__(self, tile=16, cutoff=3.0, alpha_min=1.0 / 255.0, alpha_max=0.99, t_min=1e-4, z_near=0.2,
-                 async_mode=False, radix_binning=False, track_reuse=False, device="cuda:0", torch_allocator=True):
+                 async_mode=False, radix_binning=False, track_reuse=False, lazy_grads=False, device="cuda:0", torch_allocator=True):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2506_00970_b200 needs a CUDA device; there is no CPU fallback")
         self.lib = load_library()
@@ -147,7 +148,7 @@ class Renderer:
         cfg.tile, cfg.cutoff, cfg.alpha_min, cfg.alpha_max = tile, cutoff, alpha_min, alpha_max
         cfg.t_min, cfg.z_near = t_min, z_near
         cfg.flags = ((SGS_FLAG_ASYNC if async_mode else 0) | (SGS_FLAG_RADIX_BINNING if radix_binning else 0) |
-                     (SGS_FLAG_TRACK_REUSE if track_reuse else 0))
+                     (SGS_FLAG_TRACK_REUSE if track_reuse else 0) | (SGS_FLAG_LAZY_GRADS if lazy_grads else 0))
         if torch_allocator:
             dev_index = self.device.index or 0
 
@@ -197,6 +198,10 @@ class Renderer:
         device tensors (any may be None)."""
         im = _images(rgb, depth, normal, alpha)
         _check(self.lib.sgs_render(self._ctx, C.byref(surfels), C.byref(cam), C.byref(im), _stream_ptr(stream)), "sgs_render")
+
+    def wait_grads(self, stream=None):
+        """sgs_wait_grads: with lazy_grads=True, orders `stream` behind the last backward()'s per-surfel kernel."""
+        _check(self.lib.sgs_wait_grads(self._ctx, _stream_ptr(stream)), "sgs_wait_grads")
 
     def track_new_frame(self):
         """sgs_track_new_frame: with track_reuse=True, drops the survivor list kept across tracking iterations (call at

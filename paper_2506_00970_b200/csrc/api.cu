@@ -198,6 +198,8 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
     c->cfgd.t_min = cfg->t_min; c->cfgd.z_near = cfg->z_near;
     c->cfgd.cutoff2_d = (double)cfg->cutoff * (double)cfg->cutoff;
     c->cfgd.z_near_d = (double)cfg->z_near;
+    int prio_lo = 0, prio_hi = 0;  // the ctx's own stream carries short latency-bound work: let it in first
+    cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
     bool ok = cudaMalloc(&c->counters, sizeof(SgsCounters)) == cudaSuccess &&
               cudaMalloc(&c->counters_snap, 2 * sizeof(SgsCounters)) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->counters_ready_prev, cudaEventDisableTiming) == cudaSuccess &&
@@ -210,7 +212,7 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
               cudaEventCreateWithFlags(&c->work_ev, cudaEventDisableTiming) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->fork_ev, cudaEventDisableTiming) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->join_ev, cudaEventDisableTiming) == cudaSuccess &&
-              cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking) == cudaSuccess;
+              cudaStreamCreateWithPriority(&c->aux_stream, cudaStreamNonBlocking, prio_hi) == cudaSuccess;
     if (!ok) { cudaGetLastError(); sgs_destroy(c); return SGS_CUDA_ERROR; }
     c->pose6_dev = c->loss_dev + 1;
     cudaMemset(c->counters, 0, sizeof(SgsCounters));

@@ -97,6 +97,7 @@ int sgs_backward_host(sgs_ctx* c, const sgs_images* hu, const sgs_surfel_grads* 
         dg.mean = b; dg.scale = b + 3 * n; dg.quat = b + 5 * n; dg.opacity = b + 9 * n; dg.rgb = b + 10 * n;
     }
     if ((r = sgs_backward(c, &du, hg ? &dg : nullptr, h_pose6 ? c->pose6_dev : nullptr, stream)) != SGS_OK) return r;
+    if ((r = sgs_wait_grads(c, stream)) != SGS_OK) return r;  // SGS_FLAG_LAZY_GRADS: the copies below need the last kernel
     if (hg) {
         if (hg->mean) ok = ok && cudaMemcpyAsync(hg->mean, dg.mean, sizeof(float) * 3 * n, cudaMemcpyDeviceToHost, s) == cudaSuccess;
         if (hg->scale) ok = ok && cudaMemcpyAsync(hg->scale, dg.scale, sizeof(float) * 2 * n, cudaMemcpyDeviceToHost, s) == cudaSuccess;

@@ -135,6 +135,10 @@ static int bin_view(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, bo
     if (r != SGS_OK) return r;
     c->have_forward = false;
     c->have_binning = false;
+    if (c->grads_on_aux) {  // SGS_FLAG_LAZY_GRADS: the last backward's per-surfel kernel still reads the lists this call rewrites
+        if (c->work_recorded && cudaStreamWaitEvent(s, c->work_ev, 0) != cudaSuccess) return SGS_CUDA_ERROR;
+        c->grads_on_aux = false;
+    }
     if (!c->use_surv_cache) c->surv_valid = false;  // K-pre-A is about to overwrite the list
     sgs_fill_cam(cam, &c->camd);
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
@@ -325,8 +329,16 @@ int sgs_backward(sgs_ctx* c, const sgs_images* upstream, const sgs_surfel_grads*
         if (upstream->normal) for (int i = 0; i < 3; ++i) up[4 + i] = upstream->normal + (size_t)i * pixels;
         if (upstream->alpha) up[7] = upstream->alpha;
     }
+    c->grads_on_aux = false;
     if (sgs_launch_backward(c, up, dg, d_pose6, s) != cudaSuccess) return SGS_CUDA_ERROR;
-    c->work_recorded = cudaEventRecord(c->work_ev, s) == cudaSuccess;
+    c->work_recorded = cudaEventRecord(c->work_ev, c->grads_on_aux ? c->aux_stream : s) == cudaSuccess;
+    return SGS_OK;
+}
+
+int sgs_wait_grads(sgs_ctx* c, void* stream) {
+    if (!c) return SGS_INVALID_ARGUMENT;
+    if (c->grads_on_aux && c->work_recorded && cudaStreamWaitEvent((cudaStream_t)stream, c->work_ev, 0) != cudaSuccess)
+        return SGS_CUDA_ERROR;
     return SGS_OK;
 }
 

@@ -412,17 +412,26 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     k_backward<false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                   cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
                                                   c->acc, c->pose_partial, c->counters, nullptr, FusedLoss{});
-    if (ms != s && (e = cudaStreamWaitEvent(s, c->join_ev, 0)) != cudaSuccess) return e;
+    // SGS_FLAG_LAZY_GRADS: the per-surfel kernel (latency-bound: 12 % issue utilisation) stays on the ctx's stream, behind
+    // k_backward by an event, and the caller's stream does NOT wait for it: sgs_wait_grads does (the next view's kernels
+    // run meanwhile).  Otherwise the caller's stream joins here.
+    const bool lazy = (c->cfg.flags & SGS_FLAG_LAZY_GRADS) != 0 && ms != s;
+    cudaStream_t ks = lazy ? ms : s;
+    if (lazy) {
+        if ((e = cudaEventRecord(c->fork_ev, s)) != cudaSuccess) return e;       // k_backward enqueued
+        if ((e = cudaStreamWaitEvent(ms, c->fork_ev, 0)) != cudaSuccess) return e;
+    } else if (ms != s && (e = cudaStreamWaitEvent(s, c->join_ev, 0)) != cudaSuccess) return e;
     // one thread per listed surfel; the list length is only known on the device: grid-stride from a hinted grid
     const bool bucket_mode = c->list_stride == 2;
     int64_t want = n;
     if (bucket_mode && c->last_surv > 0 && c->last_surv + c->last_surv / 4 < want) want = c->last_surv + c->last_surv / 4;
     int blocks = (int)((want + 255) / 256);
     if (blocks > 148 * 8) blocks = 148 * 8;
-    if (n == 0) return d_pose6 ? cudaMemsetAsync(d_pose6, 0, sizeof(float) * 6, s) : cudaSuccess;
+    if (n == 0) return d_pose6 ? cudaMemsetAsync(d_pose6, 0, sizeof(float) * 6, ks) : cudaSuccess;
     if (blocks < 1) blocks = 1;
     c->launches += 1;
-    k_surfel_backward<<<blocks, 256, 0, s>>>(c->counters, c->vis_to_surfel, c->culled, c->acc, c->last_surfels.mean,
+    c->grads_on_aux = lazy;
+    k_surfel_backward<<<blocks, 256, 0, ks>>>(c->counters, c->vis_to_surfel, c->culled, c->acc, c->last_surfels.mean,
                                              c->last_surfels.scale, c->last_surfels.quat, cam, *dg, c->pose_partial,
                                              c->counters, d_pose6, bucket_mode ? 1 : 0);
     return cudaGetLastError();

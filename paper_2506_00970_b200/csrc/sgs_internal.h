@@ -133,6 +133,7 @@ struct sgs_ctx {
     sgs_surfels surv_sf;
     sgs_camera surv_cam;
     int narrow_prepare;                // > 0 inside sgs_prepare: K-pre-B blocks per SM
+    bool grads_on_aux;                 // SGS_FLAG_LAZY_GRADS: the last sgs_backward left its final kernel on aux_stream
     bool copy_in_flight;               // counters_ready was recorded on aux_stream and nothing on the caller's stream waited for it yet
     bool prepared, work_recorded;      // binning of (last_surfels, last_cam) enqueued by sgs_prepare, not yet rendered
     // last forward

@@ -535,3 +535,39 @@ def test_track_reuse_keeps_the_binning_exact():
         np.testing.assert_allclose(la.cpu().numpy(), lb.cpu().numpy(), rtol=1e-5)
         np.testing.assert_allclose(pa.cpu().numpy(), pb.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(pb.abs().max()))
     ra.close(); rb.close()
+
+
+def test_lazy_grads_equal_after_wait():
+    """SGS_FLAG_LAZY_GRADS: after sgs_wait_grads the surfel and pose gradients equal those of a context without the
+    flag (same kernels; sums of atomics differ in order only), also when the next view is rendered on another context
+    in between and when the same context is reused for a later view (its own calls order themselves)."""
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    t, sf = to_device(sc)
+    up = scenegen.upstream_normal(9, cam.height, cam.width)
+    taus = [None, [0.05, 0.02, -0.04, 0.1, -0.05, 0.2], [-0.1, 0.05, 0.02, -0.2, 0.1, 0.05], [0.02, 0.0, 0.01, 0.0, 0.03, 0.0]]
+    cs = [camera(cam, None if tau is None else scenegen.perturb_pose(cam.T_cw, tau)) for tau in taus]
+    ref = sgs.Renderer()
+    refs = []
+    for c in cs:
+        im, g, p6 = alloc_images(cam), alloc_grads(sc.n), torch.zeros(6, device="cuda")
+        ref.render(sf, c, **im)
+        ref.backward(**split_upstream(up), grads=g, d_pose6=p6)
+        torch.cuda.synchronize()
+        refs.append(({k: v.cpu().numpy() for k, v in g.items()}, p6.cpu().numpy()))
+    rens = [sgs.Renderer(lazy_grads=True), sgs.Renderer(lazy_grads=True)]
+    outs = []
+    for v, c in enumerate(cs):   # two contexts alternate; nothing waits until the end
+        im, g, p6 = alloc_images(cam), alloc_grads(sc.n), torch.full((6,), 7.0, device="cuda")
+        rens[v % 2].render(sf, c, **im)
+        rens[v % 2].backward(**split_upstream(up), grads=g, d_pose6=p6)
+        outs.append((g, p6))
+    for r in rens:
+        r.wait_grads()
+    res = [({k: x.cpu().numpy() for k, x in g.items()}, p6.cpu().numpy()) for g, p6 in outs]   # on the waited stream
+    for (g, p6), (rg, rp6) in zip(res, refs):
+        for name in g:
+            np.testing.assert_allclose(g[name], rg[name], rtol=2e-4, atol=1e-5 * np.abs(rg[name]).max())
+        np.testing.assert_allclose(p6, rp6, rtol=1e-4, atol=1e-5 * np.abs(rp6).max())
+    for r in rens + [ref]:
+        r.close()
