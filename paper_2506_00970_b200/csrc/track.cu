@@ -18,14 +18,18 @@ namespace {
 
 struct TrackPlanes { float* p[8]; };
 
-constexpr uint32_t TRK_PL = SGS_BLOCK * 16;  // bytes per staged plane
+// Staging capacity: lists of up to TRK_CAP entries are walked from ONE staged batch (the fast path below).  384 keeps the
+// kernel's static shared memory under 48 KB; C2's longest tile list (263) used to fall into the general path, and that
+// one tile set the end of the whole launch.
+constexpr int TRK_CAP = 384;
+constexpr uint32_t TRK_PL = TRK_CAP * 16;  // bytes per staged plane
 constexpr int TRK_ORDER_BINS = 2048;         // tile costs (cycles >> 8) are binned 0..2047
 constexpr int TRK_K = 2;                     // entries per trip of the walks
 
 // One thread stages entry `v` of the tile: forward record (s0..s4; s4.w carries m.z) plus the backward's a_u, a_v and
 // m = a_u x a_v: 7 planes of float4.
 __device__ __forceinline__ unsigned stage_track(const SgsPayload& pay, uint32_t v, double px0, double py0, float tx0,
-                                                float ty0, float4 (*sh)[SGS_BLOCK], int tid, const SgsCfgDev& cfg) {
+                                                float ty0, float4 (*sh)[TRK_CAP], int tid, const SgsCfgDev& cfg) {
     const float4 g0 = pay.g0[v], g1 = pay.g1[v], g3 = pay.g3[v], g4 = pay.g4[v], g5 = pay.g5[v], g6 = pay.g6[v];
     const float4 g7 = pay.g7[v];
     const double2 g2 = pay.g2[v];
@@ -60,9 +64,9 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         float* __restrict__ loss_out, uint32_t* __restrict__ tile_cost, uint32_t* cursor_rw, SgsCounters* __restrict__ counters_snap) {
     const long long t_start = clock64();
     cudaTriggerProgrammaticLaunchCompletion();  // the next iteration's K-pre-B may be staged; it waits for this grid before it reads anything
-    __shared__ float4 sh[7][SGS_BLOCK];
-    __shared__ unsigned long long s_keys[SGS_BLOCK];
-    __shared__ unsigned char sh_mask[SGS_BLOCK];
+    __shared__ float4 sh[7][TRK_CAP];
+    __shared__ unsigned long long s_keys[TRK_CAP];
+    __shared__ unsigned char sh_mask[TRK_CAP];
     __shared__ float s_red[8][7];
     __shared__ uint32_t s_wmax[8];
     const uint32_t sa = smem_addr(&sh[0][0]), sm_a = smem_addr(sh_mask);
@@ -251,21 +255,26 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     unsigned long long* g = bucket + (size_t)start;
     if (tid == 0) { ranges[2 * tile] = start; ranges[2 * tile + 1] = start + n; }
 
-    if (!presorted && n <= SGS_BLOCK) {
+    if (!presorted && n <= TRK_CAP) {
         // ===== one batch (the common case in tracking): rank the keys by counting (they are unique), stage each
         // entry straight into the slot of its rank, walk forward, then walk the SAME staged records back.
         // No barrier between the two walks: a warp needs only its own pixels' state. =====
-        const bool mine = (uint32_t)tid < n;
-        const unsigned long long key = mine ? g[tid] : ~0ull;
-        s_keys[tid] = key;
-        sh_mask[tid] = 0;
+        for (uint32_t e = tid; e < (uint32_t)TRK_CAP; e += SGS_BLOCK) {
+            s_keys[e] = e < n ? g[e] : ~0ull;
+            sh_mask[e] = 0;
+        }
         __syncthreads();
-        if ((uint32_t)(wid * 32) < n) {  // only warps that own keys walk the list
-            uint32_t rank = 0;
-            for (uint32_t k = 0; k < n; ++k) rank += s_keys[k] < key ? 1u : 0u;
-            if (mine) {
-                g[rank] = key;  // sorted list for sgs_get_binning
-                sh_mask[rank] = (unsigned char)stage_track(pay, (uint32_t)key, px0, py0, tx0, ty0, sh, (int)rank, cfg);
+        for (uint32_t e0 = 0; e0 < n; e0 += SGS_BLOCK) {
+            if (e0 + (uint32_t)(wid * 32) < n) {  // only warps that own keys walk the list
+                const uint32_t e = e0 + tid;
+                const bool mine = e < n;
+                const unsigned long long key = mine ? s_keys[e] : ~0ull;
+                uint32_t rank = 0;
+                for (uint32_t k = 0; k < n; ++k) rank += s_keys[k] < key ? 1u : 0u;
+                if (mine) {
+                    g[rank] = key;  // sorted list for sgs_get_binning
+                    sh_mask[rank] = (unsigned char)stage_track(pay, (uint32_t)key, px0, py0, tx0, ty0, sh, (int)rank, cfg);
+                }
             }
         }
         __syncthreads();
