@@ -382,6 +382,12 @@ def main():
     sampler.start()
     time.sleep(0.3)
     ms = timed_pass()
+    # the timed region can be shorter than nvidia-smi's start-up: keep the same load running (untimed) until the sampler
+    # has seen it a few times, so that `clocks` is always a reading under this workload
+    t_wait = time.time()
+    while len(sampler.rows) < 3 and time.time() - t_wait < 4.0:
+        wl.step()
+        torch.cuda.synchronize()
     clocks = sampler.stop()
     launches = sum(r.stats()["kernel_launches"] for r in wl.rens) - launches0
     px = wl.H * wl.W
