@@ -31,7 +31,7 @@ UNIT = "MP/s"
 F_TEST, F_COMP_FWD, F_COMP_BWD_FULL, F_COMP_BWD_POSE = 26, 26, 102, 94
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
 # captures (profiles/r01_*.md; ncu flushes L2 before every replay, so these are cold-cache figures)
-NCU_TRAFFIC = {("C2", "track"): 20.9e6, ("C2", "backward"): 30.6e6, ("C2", "forward"): 14.0e6}
+NCU_TRAFFIC = {("C2", "track"): 8.49e6, ("C2", "backward"): 30.6e6, ("C2", "forward"): 14.0e6}
 
 
 def load_peaks():
@@ -382,6 +382,7 @@ def main():
     sampler.start()
     time.sleep(0.3)
     ms = timed_pass()
+    launches = sum(r.stats()["kernel_launches"] for r in wl.rens) - launches0   # of the timed region only
     # the timed region can be shorter than nvidia-smi's start-up: keep the same load running (untimed) until the sampler
     # has seen it a few times, so that `clocks` is always a reading under this workload
     t_wait = time.time()
@@ -389,7 +390,6 @@ def main():
         wl.step()
         torch.cuda.synchronize()
     clocks = sampler.stop()
-    launches = sum(r.stats()["kernel_launches"] for r in wl.rens) - launches0
     px = wl.H * wl.W
     ms_max, value = aggregate_replicas(ms, px, wl.renders_per_step * K, world, dist, "cuda")
     renders = wl.renders_per_step * K * world
