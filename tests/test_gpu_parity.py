@@ -357,13 +357,15 @@ def test_random_poses_binning_and_images(ren):
         assert_images(planes(im), oracle.render(sc, camv, cfg))
 
 
-def test_track_iter_edge_cases():
-    """sgs_track_iter on an empty map, an all-culled map and a ragged image (70x50: partial tiles)."""
+@pytest.mark.parametrize("reuse", [False, True])
+def test_track_iter_edge_cases(reuse):
+    """sgs_track_iter on an empty map, an all-culled map and a ragged image (70x50: partial tiles); with and without
+    SGS_FLAG_TRACK_REUSE (each case twice in a row, so that the second call runs from the kept list)."""
     cam = Camera(70, 50, 60.0, 60.0, 35.0, 25.0)
     c = camera(cam)
     tgt_rgb = torch.full((3, 50, 70), 0.3, device="cuda")
     tgt_dep = torch.full((1, 50, 70), 1.5, device="cuda")
-    ren = sgs.Renderer()
+    ren = sgs.Renderer(track_reuse=reuse)
     empty = Scene(*[np.zeros(s, np.float32) for s in ((0, 3), (0, 2), (0, 4), (0,), (0, 3))])
     sc = scenegen.tiny_scene(3, 500)
     behind = Scene(sc.mean * np.float32([1, 1, -1]), sc.scale, sc.quat, sc.opacity, sc.rgb)
@@ -371,10 +373,12 @@ def test_track_iter_edge_cases():
         t, sf = to_device(scene)
         im = alloc_images(cam)
         im["rgb"].fill_(9.0)
-        p6, loss = torch.full((6,), 3.0, device="cuda"), torch.full((1,), 3.0, device="cuda")
-        ren.track_iter(sf, c, tgt_rgb, tgt_dep, 0.5, 1.0, p6, loss, **im)
-        torch.cuda.synchronize()
-        assert (planes(im) == 0).all() and (p6 == 0).all() and float(loss.item()) == 0.0
+        for _ in range(2):
+            im["rgb"].fill_(9.0)
+            p6, loss = torch.full((6,), 3.0, device="cuda"), torch.full((1,), 3.0, device="cuda")
+            ren.track_iter(sf, c, tgt_rgb, tgt_dep, 0.5, 1.0, p6, loss, **im)
+            torch.cuda.synchronize()
+            assert (planes(im) == 0).all() and (p6 == 0).all() and float(loss.item()) == 0.0
     # ragged image, dense enough that many pixels pass M_o: fused == unfused
     sc = scenegen.tiny_scene(7, 6000)
     sc.opacity[:] = 0.9
@@ -384,11 +388,12 @@ def test_track_iter_edge_cases():
     assert float((im["alpha"] > 0.95).float().mean()) > 0.05
     pa, la = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
     ren.backward_tracking(tgt_rgb, tgt_dep, 0.5, 1.0, pa, la)
-    pb, lb = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
-    ren.track_iter(sf, c, tgt_rgb, tgt_dep, 0.5, 1.0, pb, lb, **im2)
-    assert np.array_equal(planes(im), planes(im2))
-    np.testing.assert_allclose(lb.cpu().numpy(), la.cpu().numpy(), rtol=1e-5)
-    np.testing.assert_allclose(pb.cpu().numpy(), pa.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(pa.abs().max()))
+    for _ in range(2):
+        pb, lb = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+        ren.track_iter(sf, c, tgt_rgb, tgt_dep, 0.5, 1.0, pb, lb, **im2)
+        assert np.array_equal(planes(im), planes(im2))
+        np.testing.assert_allclose(lb.cpu().numpy(), la.cpu().numpy(), rtol=1e-5)
+        np.testing.assert_allclose(pb.cpu().numpy(), pa.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(pa.abs().max()))
     ren.close()
 
 
