@@ -204,7 +204,10 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
               cudaMalloc(&c->counters_snap, 2 * sizeof(SgsCounters)) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->counters_ready_prev, cudaEventDisableTiming) == cudaSuccess &&
               cudaMallocHost(&c->counters_host, sizeof(SgsCounters)) == cudaSuccess &&
-              cudaMallocHost(&c->pinned_small, 8 * sizeof(float)) == cudaSuccess &&
+              cudaHostAlloc(&c->pinned_small, 8 * sizeof(float), cudaHostAllocMapped) == cudaSuccess &&
+              cudaHostAlloc(&c->host_flag, sizeof(unsigned int), cudaHostAllocMapped) == cudaSuccess &&
+              cudaHostGetDevicePointer(&c->pinned_small_dev, c->pinned_small, 0) == cudaSuccess &&
+              cudaHostGetDevicePointer(&c->host_flag_dev, c->host_flag, 0) == cudaSuccess &&
               cudaMalloc(&c->sort_hist, sizeof(uint32_t) * (8 * 256 + 8)) == cudaSuccess &&
               cudaMalloc(&c->loss_dev, sizeof(float) * 8) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->counters_ready, cudaEventDisableTiming) == cudaSuccess &&
@@ -235,6 +238,7 @@ int sgs_destroy(sgs_ctx* c) {
     if (c->counters_ready_prev) cudaEventDestroy(c->counters_ready_prev);
     if (c->counters_host) cudaFreeHost(c->counters_host);
     if (c->pinned_small) cudaFreeHost(c->pinned_small);
+    if (c->host_flag) cudaFreeHost(c->host_flag);
     if (c->sort_hist) cudaFree(c->sort_hist);
     if (c->loss_dev) cudaFree(c->loss_dev);
     if (c->covis_cnt) cudaFree(c->covis_cnt);

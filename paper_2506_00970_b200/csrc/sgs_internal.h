@@ -158,6 +158,10 @@ struct sgs_ctx {
     float* host_grads_dev;           // n x 13 staging
     float* loss_dev; float* pose6_dev;
     float* pinned_small;             // 8 floats pinned
+    // sgs_track_iter_host: K-track writes loss + pose gradient straight into pinned_small and then this flag word (pinned,
+    // device-visible); the host polls it instead of a copy + stream synchronisation
+    unsigned int* host_flag; unsigned int* host_flag_dev; float* pinned_small_dev;
+    unsigned int host_flag_val; bool host_flag_want, host_flag_armed;
     int64_t host_img_cap, host_grads_cap;
     int64_t partial_cap;             // floats in pose_partial
     int64_t launches;                // kernels launched by this ctx

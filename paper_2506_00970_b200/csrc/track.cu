@@ -61,7 +61,8 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         int presorted, SgsPayload pay, int W, int H, int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg,
         TrackPlanes out, const float* __restrict__ trgb, const float* __restrict__ tdepth, float lambda_d, float nsign,
         float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
-        float* __restrict__ loss_out, uint32_t* __restrict__ tile_cost, uint32_t* cursor_rw, SgsCounters* __restrict__ counters_snap) {
+        float* __restrict__ loss_out, uint32_t* __restrict__ tile_cost, uint32_t* cursor_rw, SgsCounters* __restrict__ counters_snap,
+        unsigned int* host_flag, unsigned int flag_val) {
     const long long t_start = clock64();
     cudaTriggerProgrammaticLaunchCompletion();  // the next iteration's K-pre-B may be staged; it waits for this grid before it reads anything
     __shared__ float4 sh[7][TRK_CAP];
@@ -356,6 +357,11 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     }
     if (tid == 0) tile_cost[tile] = (uint32_t)((clock64() - t_start) >> 8);  // feedback for the next iteration's order
     if (!finish_pose(pose_partial, gridDim.x, counters, d_pose6, loss_out)) return;
+    if (host_flag) {  // sgs_track_iter_host: d_pose6 / loss_out are pinned HOST memory; publish them before the housekeeping below
+        if (tid < 7) __threadfence_system();
+        __syncthreads();
+        if (tid == 0) *reinterpret_cast<volatile unsigned int*>(host_flag) = flag_val;
+    }
     // ---- last block: longest-first tile order for the NEXT iteration ----
     // One block per tile, and tiles differ several-fold in work (C2: 20 k .. 130 k cycles), so the tail of this
     // kernel is set by when the long tiles start.  Every block has stored the cycles it took (tile_cost) before
@@ -450,16 +456,18 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
     // loads in front of this kernel's wait; profiles/r01_c2_track.md.  The other edge, K-pre-B behind this kernel, pays.)
     const uint32_t tile_cap = (uint32_t)c->tile_cap;
     SgsCounters* snap = after_preprocess ? c->counters_snap + c->snap_slot : nullptr;
+    unsigned int* hflag = c->host_flag_want ? c->host_flag_dev : nullptr;  // (sgs_track_iter_host)
+    c->host_flag_armed = hflag != nullptr;
     if (any)
         k_track<true><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W,
                                                   cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb, tdepth,
                                                   lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost,
-                                                  c->cursor, snap);
+                                                  c->cursor, snap, hflag, c->host_flag_val);
     else
         k_track<false><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W,
                                                    cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb, tdepth,
                                                    lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost,
-                                                   c->cursor, snap);
+                                                   c->cursor, snap, hflag, c->host_flag_val);
     c->cost_tiles = tiles; c->cost_W = cam.W; c->cost_H = cam.H;
     c->prezero_tiles = tiles;
     return cudaGetLastError();
