@@ -341,11 +341,13 @@ class Renderer:
                                           _ptr(depth, torch.float32, "cpu"), _stream_ptr(stream)), "sgs_upload_target")
 
     def track_iter_host(self, cam, lambda_d, normal_sign, stream=None):
-        loss = C.c_float()
-        pose = (C.c_float * 6)()
+        buf = getattr(self, "_h_track", None)
+        if buf is None:  # one 7-float host buffer for the life of the Renderer: this call sits in a tracker's inner loop
+            buf = self._h_track = (C.c_float * 7)()
+            self._h_track_np = np.frombuffer(buf, dtype=np.float32)
         _check(self.lib.sgs_track_iter_host(self._ctx, C.byref(cam), C.c_float(lambda_d), C.c_float(normal_sign),
-                                            C.byref(loss), pose, _stream_ptr(stream)), "sgs_track_iter_host")
-        return float(loss.value), np.array(list(pose), dtype=np.float32)
+                                            buf, C.byref(buf, 4), _stream_ptr(stream)), "sgs_track_iter_host")
+        return float(self._h_track_np[0]), self._h_track_np[1:].copy()
 
 
 class _RawDeviceBytes:
