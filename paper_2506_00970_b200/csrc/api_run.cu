@@ -24,12 +24,12 @@ static int check_pending(sgs_ctx* c, cudaStream_t s) {
     c->last_surv = (int64_t)c->counters_host->n_surv;
     if (radix_mode(c)) {
         if (c->counters_host->overflow) {
-            c->have_forward = c->have_binning = false;
+            c->have_forward = c->have_binning = c->prepared = false;
             const int r = sgs_ensure_entries(c, E, s);
             return r != SGS_OK ? r : SGS_WORKSPACE_OVERFLOW;
         }
     } else if (c->counters_host->max_tile > (unsigned)c->tile_cap) {
-        c->have_forward = c->have_binning = false;
+        c->have_forward = c->have_binning = c->prepared = false;
         const int r = sgs_ensure_buckets(c, c->camd.tiles_x * c->camd.tiles_y, grown_tile_cap(c->counters_host->max_tile), s);
         return r != SGS_OK ? r : SGS_WORKSPACE_OVERFLOW;
     }
@@ -210,6 +210,9 @@ int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const s
     cudaStream_t s = (cudaStream_t)stream;
     int r;
     if (c->prepared && same_view(c, sf, cam)) {  // binning already enqueued by sgs_prepare: order this stream behind it
+        // async mode: its counters have usually arrived by now; an overflow is reported HERE (workspace grown, nothing
+        // composited from truncated lists) and the caller renders again, which bins in line
+        if ((r = check_pending(c, s)) != SGS_OK) return r;
         c->prepared = false;
         if (cudaStreamWaitEvent(s, c->prepared_ev, 0) != cudaSuccess) return SGS_CUDA_ERROR;
     } else {
