@@ -293,6 +293,20 @@ def test_tile_bucket_overflow_grows(ren):
     a.stats()
     assert np.array_equal(planes(im), out["img"])
     a.close()
+    # the same through sgs_prepare: the render that follows reports the overflow of the prepared binning before it
+    # composites anything; rendering again bins in line with the grown buckets
+    b = sgs.Renderer(async_mode=True)
+    c = camera(cam)
+    im.update(alloc_images(cam))
+    b.prepare(sf, c)
+    with pytest.raises(sgs.SgsError) as e:
+        b.render(sf, c, **im)
+    assert e.value.status == sgs.SGS_WORKSPACE_OVERFLOW
+    assert float(im["alpha"].abs().max()) == 0.0   # nothing was composited
+    b.render(sf, c, **im)
+    b.stats()
+    assert np.array_equal(planes(im), out["img"])
+    b.close()
 
 
 def test_track_iter_matches_unfused_sequence():
