@@ -206,6 +206,9 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
               cudaMallocHost(&c->counters_host, sizeof(SgsCounters)) == cudaSuccess &&
               cudaHostAlloc(&c->pinned_small, 8 * sizeof(float), cudaHostAllocMapped) == cudaSuccess &&
               cudaHostAlloc(&c->host_flag, sizeof(unsigned int), cudaHostAllocMapped) == cudaSuccess &&
+              cudaMalloc(&c->split_state, sizeof(float) * 6 * SGS_BLOCK * SGS_TRACK_HELPERS) == cudaSuccess &&
+              cudaMalloc(&c->split_flag, sizeof(unsigned int) * SGS_TRACK_HELPERS) == cudaSuccess &&
+              cudaMemset(c->split_flag, 0, sizeof(unsigned int) * SGS_TRACK_HELPERS) == cudaSuccess &&
               cudaHostGetDevicePointer(&c->pinned_small_dev, c->pinned_small, 0) == cudaSuccess &&
               cudaHostGetDevicePointer(&c->host_flag_dev, c->host_flag, 0) == cudaSuccess &&
               cudaMalloc(&c->sort_hist, sizeof(uint32_t) * (8 * 256 + 8)) == cudaSuccess &&
@@ -214,6 +217,8 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
               cudaEventCreateWithFlags(&c->prepared_ev, cudaEventDisableTiming) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->work_ev, cudaEventDisableTiming) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->fork_ev, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreateWithFlags(&c->order_fork, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreateWithFlags(&c->order_done, cudaEventDisableTiming) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->join_ev, cudaEventDisableTiming) == cudaSuccess &&
               cudaStreamCreateWithPriority(&c->aux_stream, cudaStreamNonBlocking, prio_hi) == cudaSuccess;
     if (!ok) { cudaGetLastError(); sgs_destroy(c); return SGS_CUDA_ERROR; }
@@ -239,6 +244,8 @@ int sgs_destroy(sgs_ctx* c) {
     if (c->counters_host) cudaFreeHost(c->counters_host);
     if (c->pinned_small) cudaFreeHost(c->pinned_small);
     if (c->host_flag) cudaFreeHost(c->host_flag);
+    if (c->split_state) cudaFree(c->split_state);
+    if (c->split_flag) cudaFree(c->split_flag);
     if (c->sort_hist) cudaFree(c->sort_hist);
     if (c->loss_dev) cudaFree(c->loss_dev);
     if (c->covis_cnt) cudaFree(c->covis_cnt);
@@ -246,6 +253,8 @@ int sgs_destroy(sgs_ctx* c) {
     if (c->prepared_ev) cudaEventDestroy(c->prepared_ev);
     if (c->work_ev) cudaEventDestroy(c->work_ev);
     if (c->fork_ev) cudaEventDestroy(c->fork_ev);
+    if (c->order_fork) cudaEventDestroy(c->order_fork);
+    if (c->order_done) cudaEventDestroy(c->order_done);
     if (c->join_ev) cudaEventDestroy(c->join_ev);
     if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
     for (int i = 0; i < 2 * c->prof_cap; ++i) cudaEventDestroy(c->prof_ev[i]);

@@ -278,7 +278,7 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
     c->defer_counters = false;
     if (r != SGS_OK) return r;
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
-    if ((r = sgs_ensure_partials(c, tiles, s)) != SGS_OK) return r;
+    if ((r = sgs_ensure_partials(c, (int64_t)tiles + SGS_TRACK_HELPERS, s)) != SGS_OK) return r;  // K-track: one row per block, helpers included
     float* planes[8];
     pick_planes(c, out, (int64_t)cam->width * cam->height, false, planes);
     if (deferred && c->prev_copy_on_aux) {  // the slot this K-track overwrites was copied two iterations ago: done long since

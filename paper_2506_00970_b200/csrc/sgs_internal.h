@@ -54,6 +54,8 @@ struct SgsCamDev {
 // SGS_FLAG_TRACK_REUSE: a survivor list stays valid for poses within this translation / rotation of the pose it was built for
 constexpr float SGS_REUSE_MARGIN_T = 0.03f, SGS_REUSE_MARGIN_R = 0.02f;
 
+constexpr int SGS_TRACK_HELPERS = 48;  // K-track: extra blocks that walk back the second half of the longest tile lists
+
 struct SurvInputs { float4 *p0, *p1, *p2; float* p3; };  // (mean, opacity), quat, (scale, r, g), b
 
 struct SgsCfgDev {
@@ -162,6 +164,9 @@ struct sgs_ctx {
     // device-visible); the host polls it instead of a copy + stream synchronisation
     unsigned int* host_flag; unsigned int* host_flag_dev; float* pinned_small_dev;
     unsigned int host_flag_val; bool host_flag_want, host_flag_armed;
+    // K-track helpers (track.cu): per helper 6 x 256 floats of per-pixel state and a flag word, the launch counter they compare with
+    float* split_state; unsigned int* split_flag; unsigned int track_launch_id;
+    cudaEvent_t order_fork, order_done; bool order_pending;  // k_track_order on aux_stream
     int64_t host_img_cap, host_grads_cap;
     int64_t partial_cap;             // floats in pose_partial
     int64_t launches;                // kernels launched by this ctx

@@ -25,6 +25,12 @@ constexpr int TRK_CAP = 384;
 constexpr uint32_t TRK_PL = TRK_CAP * 16;  // bytes per staged plane
 constexpr int TRK_ORDER_BINS = 2048;         // tile costs (cycles >> 8) are binned 0..2047
 constexpr int TRK_K = 2;                     // entries per trip of the walks
+// Lists of TRK_SPLIT_MIN+1 .. TRK_CAP entries are walked BACK by the two blocks of the tile's cluster at once: block 0 the front
+// part [0, m), block 1 the back part [m, n) (m a multiple of 32, n - m <= TRK_CAP / 2).  One warp gets through a trip of two
+// entries in ~340 cycles whatever else the SM does (profiles/r01_c2_track.md), so a long list is a long serial walk and
+// the launch ended with a dozen of them; the forward walk stays with block 0 (bit-identical images), block 1 stages its
+// part meanwhile, receives (g, T_final, last) per pixel through distributed shared memory and takes half of the way back.
+constexpr uint32_t TRK_SPLIT_MIN = 128;
 
 // One thread stages entry `v` of the tile: forward record (s0..s4; s4.w carries m.z) plus the backward's a_u, a_v and
 // m = a_u x a_v: 7 planes of float4.
@@ -62,7 +68,8 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         TrackPlanes out, const float* __restrict__ trgb, const float* __restrict__ tdepth, float lambda_d, float nsign,
         float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
         float* __restrict__ loss_out, uint32_t* __restrict__ tile_cost, uint32_t* cursor_rw, SgsCounters* __restrict__ counters_snap,
-        unsigned int* host_flag, unsigned int flag_val) {
+        unsigned int* host_flag, unsigned int flag_val, float* split_state, unsigned int* split_flag, unsigned int launch_id,
+        int n_help) {
     const long long t_start = clock64();
     cudaTriggerProgrammaticLaunchCompletion();  // the next iteration's K-pre-B may be staged; it waits for this grid before it reads anything
     __shared__ float4 sh[7][TRK_CAP];
@@ -71,7 +78,12 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     __shared__ float s_red[8][7];
     __shared__ uint32_t s_wmax[8];
     const uint32_t sa = smem_addr(&sh[0][0]), sm_a = smem_addr(sh_mask);
-    const int tile = (int)tile_order[blockIdx.x];  // longest tiles first (order written by the previous launch)
+    // blocks [0, n_help) are HELPERS of the n_help tiles predicted longest (tile_order[0 .. n_help)); block n_help + k owns tile_order[k]
+    const bool helper = (int)blockIdx.x < n_help;
+    const int slot = helper ? (int)blockIdx.x : (int)blockIdx.x - n_help;
+    const int tile = (int)tile_order[slot];  // longest tiles first (order written by the previous launch)
+    const int crank = helper ? 1 : 0;
+    const bool has_helper = !helper && slot < n_help;
     const int tx = tile % tiles_x, ty = tile / tiles_x;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int lxi = (wid & 1) * 8 + (lane & 7), lyi = (wid >> 1) * 4 + (lane >> 3);
@@ -90,8 +102,8 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dp = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f, O = 0.f;
     uint32_t last = 0;
     bool done = !inside;
-    auto forward_walk = [&](const uint32_t boff, const uint32_t nb) {
-        for (uint32_t c0 = 0; c0 < nb; c0 += 32) {
+    auto forward_walk = [&](const uint32_t boff, const uint32_t nb, const uint32_t j0 = 0u) {  // slots [j0, nb), j0 % 32 == 0
+        for (uint32_t c0 = j0; c0 < nb; c0 += 32) {
             if (__all_sync(0xffffffffu, done)) break;  // per-warp early stop on saturation
             unsigned m = __ballot_sync(0xffffffffu, (lds_u8(sm_a + c0 + lane) >> wid) & 1u);
             while (m) {
@@ -256,7 +268,43 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     unsigned long long* g = bucket + (size_t)start;
     if (tid == 0) { ranges[2 * tile] = start; ranges[2 * tile + 1] = start + n; }
 
-    if (!presorted && n <= TRK_CAP) {
+    // split tiles: both blocks of the cluster work; otherwise block 1 has nothing to do (it still writes a zero row of
+    // partial sums and draws its ticket below, so that the grid reduction counts every block)
+    const bool split = (helper || has_helper) && !presorted && n > TRK_SPLIT_MIN && n <= (uint32_t)TRK_CAP;
+    const uint32_t msp = split ? (((n + 1u) / 2u + 31u) & ~31u) : n;  // block 0: [0, msp) on the way back, block 1: [msp, n)
+    // per-pixel state the owner hands to its helper: 6 x 256 floats in global memory, published by a flag = this launch's id
+    float* st = split_state + (size_t)slot * (6 * SGS_BLOCK);
+    if (crank == 1) {
+        if (split) {
+            for (uint32_t e = tid; e < (uint32_t)TRK_CAP; e += SGS_BLOCK) {
+                s_keys[e] = e < n ? g[e] : ~0ull;
+                sh_mask[e] = 0;
+            }
+            __syncthreads();
+            for (uint32_t e0 = 0; e0 < n; e0 += SGS_BLOCK) {
+                if (e0 + (uint32_t)(wid * 32) < n) {
+                    const uint32_t e = e0 + tid;
+                    const bool mine = e < n;
+                    const unsigned long long key = mine ? s_keys[e] : ~0ull;
+                    uint32_t rank = 0;
+                    for (uint32_t k = 0; k < n; ++k) rank += s_keys[k] < key ? 1u : 0u;
+                    if (mine && rank >= msp)   // this block's part of the sorted list, at slot rank - msp
+                        sh_mask[rank - msp] = (unsigned char)stage_track(pay, (uint32_t)key, px0, py0, tx0, ty0, sh, (int)(rank - msp), cfg);
+                }
+            }
+            __syncthreads();
+            if (tid == 0) {  // the owner has walked forward and stored these pixels' state
+                while (*reinterpret_cast<volatile unsigned int*>(split_flag + slot) != launch_id) __nanosleep(200);
+                __threadfence();
+            }
+            __syncthreads();
+            g0 = __ldcg(st + tid); g1 = __ldcg(st + SGS_BLOCK + tid); g2 = __ldcg(st + 2 * SGS_BLOCK + tid);
+            g3 = __ldcg(st + 3 * SGS_BLOCK + tid); T_after = __ldcg(st + 4 * SGS_BLOCK + tid);
+            last = __float_as_uint(__ldcg(st + 5 * SGS_BLOCK + tid));
+            const uint32_t wmax = warp_max_last();
+            backward_walk(msp, (int)min(n - msp, wmax > msp ? wmax - msp : 0u));
+        }
+    } else if (!presorted && n <= TRK_CAP) {
         // ===== one batch (the common case in tracking): rank the keys by counting (they are unique), stage each
         // entry straight into the slot of its rank, walk forward, then walk the SAME staged records back.
         // No barrier between the two walks: a warp needs only its own pixels' state. =====
@@ -279,10 +327,28 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
             }
         }
         __syncthreads();
-        forward_walk(0u, n);
-        finish_forward();
-        T_after = T;
-        backward_walk(0u, (int)min(n, warp_max_last()));
+        if (!split) {
+            forward_walk(0u, n);
+            finish_forward();
+            T_after = T;
+            backward_walk(0u, (int)min(n, warp_max_last()));
+        } else {
+            forward_walk(0u, msp);
+            const float Tm = T, C0m = C0, C1m = C1, C2m = C2, Dpm = Dp;  // the pixel's state between the two parts
+            forward_walk(0u, n, msp);
+            finish_forward();
+            // hand (g, T_final, last) of this pixel to the helper
+            st[tid] = g0; st[SGS_BLOCK + tid] = g1; st[2 * SGS_BLOCK + tid] = g2; st[3 * SGS_BLOCK + tid] = g3;
+            st[4 * SGS_BLOCK + tid] = T; st[5 * SGS_BLOCK + tid] = __uint_as_float(last);
+            __threadfence();
+            __syncthreads();
+            if (tid == 0) *reinterpret_cast<volatile unsigned int*>(split_flag + slot) = launch_id;
+            // the way back over [0, msp): transmittance behind entry msp - 1 and the suffix sum of everything behind it,
+            // sum_{j >= msp} w_j (g . v_j) = g . (V_final - V_msp) with V the running accumulators of Eq. 8
+            T_after = Tm;
+            suffix = g0 * (C0 - C0m) + g1 * (C1 - C1m) + g2 * (C2 - C2m) + g3 * (Dp - Dpm);
+            backward_walk(0u, (int)min(msp, warp_max_last()));
+        }
     } else {
         // ===== general path: 256-entry batches front to back, then back to front (restaging what was evicted) =====
         if (!presorted) {  // n > 256: bitonic network in the staging memory, sorted keys back to the bucket
@@ -353,23 +419,17 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         float s = 0.f;
 #pragma unroll
         for (int w2 = 0; w2 < 8; ++w2) s += s_red[w2][tid];
-        pose_partial[(size_t)tile * 8 + tid] = s;
+        pose_partial[(size_t)blockIdx.x * 8 + tid] = s;
     }
-    if (tid == 0) tile_cost[tile] = (uint32_t)((clock64() - t_start) >> 8);  // feedback for the next iteration's order
+    if (tid == 0 && crank == 0) tile_cost[tile] = (uint32_t)((clock64() - t_start) >> 8);  // feedback for the next iteration's order
     if (!finish_pose(pose_partial, gridDim.x, counters, d_pose6, loss_out)) return;
     if (host_flag) {  // sgs_track_iter_host: d_pose6 / loss_out are pinned HOST memory; publish them before the housekeeping below
         if (tid < 7) __threadfence_system();
         __syncthreads();
         if (tid == 0) *reinterpret_cast<volatile unsigned int*>(host_flag) = flag_val;
     }
-    // ---- last block: longest-first tile order for the NEXT iteration ----
-    // One block per tile, and tiles differ several-fold in work (C2: 20 k .. 130 k cycles), so the tail of this
-    // kernel is set by when the long tiles start.  Every block has stored the cycles it took (tile_cost) before
-    // drawing its ticket; consecutive tracking iterations differ by a small pose step, so those costs predict the
-    // next iteration's.  Counting sort of the tiles by cost, descending, into tile_order (in place: every block
-    // of this launch has read its entry).  Ties land in arbitrary order; the order steers scheduling, never a result.
-    unsigned int* s_hist = reinterpret_cast<unsigned int*>(&sh[0][0]);  // staging memory is free now
-    const int tiles = (int)gridDim.x;
+    // ---- last block: housekeeping for the next iteration (the tile order is k_track_order's, off this stream) ----
+    const int tiles = (int)gridDim.x - n_help;
     // ... and the next preprocess finds its counters and per-tile cursors already zeroed (every block of this launch
     // has read its cursor; the host copied the counters before this kernel started)
     for (int t = tid; t < tiles; t += SGS_BLOCK) cursor_rw[t] = 0u;
@@ -378,7 +438,19 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         counters->n_entries = 0ull; counters->n_visible = 0u; counters->overflow = 0u; counters->ticket_pre = 0u;
         counters->max_tile = 0u; counters->n_surv = 0u;
     }
-    __syncthreads();
+}
+
+// Longest-first tile order for the NEXT iteration.  One block per tile, and tiles differ several-fold in work (C2: 20 k ..
+// 100 k cycles), so a launch ends when its long tiles end: they have to start first.  Every block of K-track has stored
+// the cycles it took (tile_cost); consecutive tracking iterations differ by a small pose step, so those costs predict
+// the next iteration's.  Counting sort of the tiles by cost, descending, into tile_order.  Ties land in arbitrary order;
+// the order steers scheduling, never a result.  Its own one-block kernel on the context's stream since the timeline of
+// profiles/r01_c2_track.md: inside K-track's last block these 2.4 us sat between the last tile and the next K-pre-B.
+__global__ void __launch_bounds__(SGS_BLOCK)
+k_track_order(const uint32_t* __restrict__ tile_cost, uint32_t* __restrict__ tile_order, int tiles) {
+    __shared__ unsigned int s_hist[TRK_ORDER_BINS];
+    __shared__ uint32_t s_wmax[8];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     for (int b = tid; b < TRK_ORDER_BINS; b += SGS_BLOCK) s_hist[b] = 0;
     __syncthreads();
     constexpr int ORD_U = 8;  // one pass covers ORD_U * 256 = 2048 tiles with the keys kept in registers
@@ -443,6 +515,11 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
     TrackPlanes out;
     bool any = false;
     for (int i = 0; i < 8; ++i) { out.p[i] = planes ? planes[i] : nullptr; any = any || out.p[i] != nullptr; }
+    // the order written by the previous iteration's k_track_order (on the ctx's stream) must be complete
+    if (c->order_pending) {
+        if (cudaStreamWaitEvent(s, c->order_done, 0) != cudaSuccess) return cudaErrorUnknown;
+        c->order_pending = false;
+    }
     if (!(c->cost_tiles == tiles && c->cost_W == cam.W && c->cost_H == cam.H)) {  // no order yet for this camera
         k_iota<<<(tiles + 255) / 256, 256, 0, s>>>(c->tile_order, tiles);
         c->launches += 1;
@@ -457,17 +534,27 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
     const uint32_t tile_cap = (uint32_t)c->tile_cap;
     SgsCounters* snap = after_preprocess ? c->counters_snap + c->snap_slot : nullptr;
     unsigned int* hflag = c->host_flag_want ? c->host_flag_dev : nullptr;  // (sgs_track_iter_host)
+    const int n_help = (c->split_state && tiles >= 4 * SGS_TRACK_HELPERS) ? SGS_TRACK_HELPERS : 0;
+    c->track_launch_id += 1;
     c->host_flag_armed = hflag != nullptr;
     if (any)
-        k_track<true><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W,
+        k_track<true><<<tiles + n_help, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W,
                                                   cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb, tdepth,
                                                   lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost,
-                                                  c->cursor, snap, hflag, c->host_flag_val);
+                                                  c->cursor, snap, hflag, c->host_flag_val, c->split_state, c->split_flag, c->track_launch_id, n_help);
     else
-        k_track<false><<<tiles, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W,
+        k_track<false><<<tiles + n_help, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W,
                                                    cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb, tdepth,
                                                    lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost,
-                                                   c->cursor, snap, hflag, c->host_flag_val);
+                                                   c->cursor, snap, hflag, c->host_flag_val, c->split_state, c->split_flag, c->track_launch_id, n_help);
+    {   // next iteration's tile order from this launch's measured tile costs, beside the next K-pre-B
+        cudaStream_t os = c->aux_stream ? c->aux_stream : s;
+        if (os != s && (cudaEventRecord(c->order_fork, s) != cudaSuccess || cudaStreamWaitEvent(os, c->order_fork, 0) != cudaSuccess))
+            return cudaErrorUnknown;
+        c->launches += 1;
+        k_track_order<<<1, SGS_BLOCK, 0, os>>>(c->tile_cost, c->tile_order, tiles);
+        if (os != s) { if (cudaEventRecord(c->order_done, os) != cudaSuccess) return cudaErrorUnknown; c->order_pending = true; }
+    }
     c->cost_tiles = tiles; c->cost_W = cam.W; c->cost_H = cam.H;
     c->prezero_tiles = tiles;
     return cudaGetLastError();
