@@ -54,7 +54,7 @@ struct SgsCamDev {
 // SGS_FLAG_TRACK_REUSE: a survivor list stays valid for poses within this translation / rotation of the pose it was built for
 constexpr float SGS_REUSE_MARGIN_T = 0.03f, SGS_REUSE_MARGIN_R = 0.02f;
 
-constexpr int SGS_TRACK_HELPERS = 48;  // K-track: extra blocks that walk back the second half of the longest tile lists
+constexpr int SGS_TRACK_HELPERS = 32;  // K-track: extra blocks that walk back the second half of the longest tile lists
 
 struct SurvInputs { float4 *p0, *p1, *p2; float* p3; };  // (mean, opacity), quat, (scale, r, g), b
 

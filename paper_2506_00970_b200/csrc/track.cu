@@ -30,7 +30,7 @@ constexpr int TRK_K = 2;                     // entries per trip of the walks
 // entries in ~340 cycles whatever else the SM does (profiles/r01_c2_track.md), so a long list is a long serial walk and
 // the launch ended with a dozen of them; the forward walk stays with block 0 (bit-identical images), block 1 stages its
 // part meanwhile, receives (g, T_final, last) per pixel through distributed shared memory and takes half of the way back.
-constexpr uint32_t TRK_SPLIT_MIN = 128;
+constexpr uint32_t TRK_SPLIT_MIN = 160;
 
 // One thread stages entry `v` of the tile: forward record (s0..s4; s4.w carries m.z) plus the backward's a_u, a_v and
 // m = a_u x a_v: 7 planes of float4.
