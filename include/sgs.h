@@ -216,7 +216,7 @@ SGS_API int sgs_mapping_loss(sgs_ctx* ctx, const sgs_camera* cam, const sgs_imag
 SGS_API int sgs_backward_tracking(sgs_ctx* ctx, const sgs_images* target, float lambda_d, float normal_sign,
                                   float* d_pose6, float* loss, void* cuda_stream);
 
-/* One whole tracking iteration (L180-204) in three launches: preprocess + tile binning (two), then ONE kernel that
+/* One whole tracking iteration (L180-204): preprocess + tile binning (two launches; one with SGS_FLAG_TRACK_REUSE), then ONE kernel that
  * composites each tile (Eq. 8), evaluates Eq. 15-19 against the current frame in registers and walks the
  * tile's list back for the pose gradient (Eq. 11-13); images, T and the upstream gradients never leave the
  * SM.  Same result as sgs_render + sgs_backward_tracking (bit-identical images, loss and 6-vector up to
@@ -225,6 +225,7 @@ SGS_API int sgs_backward_tracking(sgs_ctx* ctx, const sgs_images* target, float 
  *   target  : DEVICE rgb (3xHxW) + depth (HxW) of the current frame
  *   out     : nullable; DEVICE images to write (any pointer may be NULL = not written)
  *   d_pose6 : DEVICE, 6 floats (rho, theta); loss: DEVICE, 1 float, nullable
+ * (A one-block kernel that orders the tiles by their measured cost for the next iteration runs on a stream of the ctx.)
  * Leaves no state for sgs_backward (SGS_NO_FORWARD_STATE); sgs_get_binning works.
  * With SGS_FLAG_ASYNC the counters of an iteration reach the host behind its compositing kernel and are never waited
  * for: a tile-bucket overflow is reported (SGS_WORKSPACE_OVERFLOW, workspace grown) by the first later call on the
