@@ -166,6 +166,42 @@ def backward(sc, camv, cfgv, upstream, brute=False, debug=False):
     return g
 
 
+def normalise_depth(img):
+    """Expected depth D_n = D / O (DESIGN R9n; D = sum w z and O = sum w are the depth and opacity
+    images of Eq. 8): the blend weights renormalised to sum to one.  0 where O = 0 (no splat composited).
+    img: (8,H,W) [rgb, depth, normal, alpha]; returns a copy with the depth plane replaced."""
+    out = np.array(img, dtype=np.float64, copy=True)
+    D, O = out[3], out[7]
+    out[3] = np.divide(D, O, out=np.zeros_like(D), where=O > 0)
+    return out
+
+
+def normalised_depth_upstream(img_raw, upstream_n):
+    """Chain rule of D_n = D / O: an upstream gradient on (.., D_n, .., O) becomes one on the raw images of Eq. 8,
+    dL/dD = g_Dn / O and dL/dO = g_O - g_Dn D / O^2 (both contributions of g_Dn vanish where O = 0)."""
+    up = np.array(upstream_n, dtype=np.float64, copy=True)
+    D, O = img_raw[3], img_raw[7]
+    m = O > 0
+    gD = np.divide(up[3], O, out=np.zeros_like(D), where=m)
+    up[7] = up[7] - np.where(m, gD * np.divide(D, O, out=np.zeros_like(D), where=m), 0.0)
+    up[3] = gD
+    return up
+
+
+def render_normalised(sc, camv, cfgv, brute=False, counters=True):
+    """render() with the depth plane normalised; the raw images of Eq. 8 stay under "img_raw"."""
+    r = render(sc, camv, cfgv, brute=brute, counters=counters)
+    r["img_raw"] = r["img"]
+    r["img"] = normalise_depth(r["img"])
+    return r
+
+
+def backward_normalised(sc, camv, cfgv, upstream_n, brute=False):
+    """backward() of a loss on the normalised-depth images: upstream_n[3] is dL/dD_n."""
+    raw = render(sc, camv, cfgv, brute=brute, counters=False)["img"]
+    return backward(sc, camv, cfgv, normalised_depth_upstream(raw, upstream_n), brute=brute)
+
+
 def num_threads():
     return int(lib().orc_num_threads())
 

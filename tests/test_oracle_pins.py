@@ -262,15 +262,19 @@ def _tiny(seed=7, n=6):
     return sc, cam
 
 
+_NORMALISED = [False]   # _loss / _fd_check differentiate the normalised-depth images (P16) when set
+
+
 def _loss(sc, camv, cfg, up):
-    return float((oracle.render(sc, camv, cfg, counters=False)["img"] * up).sum())
+    r = oracle.render_normalised if _NORMALISED[0] else oracle.render
+    return float((r(sc, camv, cfg, counters=False)["img"] * up).sum())
 
 
 def _fd_check(cfg, rtol):
     sc, cam = _tiny()
     camv = oracle.make_cam(cam, widen_from_f32=False)
     up = scenegen.upstream_normal(11, cam.height, cam.width).astype(np.float64)
-    g = oracle.backward(sc, camv, cfg, up)
+    g = (oracle.backward_normalised if _NORMALISED[0] else oracle.backward)(sc, camv, cfg, up)
     worst = 0.0
     for name in ("mean", "scale", "quat", "opacity", "rgb"):
         arr = getattr(sc, name)
@@ -601,3 +605,74 @@ def test_p15_ssim_closed_forms_brute_force_and_gradient():
         d = np.zeros_like(x); d[c, j, i] = 1e-6
         fd = (oracle.ssim_loss(x + d, y, 0.2)[0] - oracle.ssim_loss(x - d, y, 0.2)[0]) / 2e-6
         assert abs(fd - gr[c, j, i]) <= 1e-6 * abs(gr[c, j, i]) + 1e-11
+
+
+# ---------------------------------------------------------------- P16: normalised depth D_n = D / O
+def test_p16_normalised_depth_of_coplanar_splats_is_the_ray_plane_depth():
+    """Five partly transparent splats on ONE tilted plane: whatever their weights, the expected depth of a pixel is
+    the ray-plane intersection depth (closed form), while the plain Eq. 8 depth is O times it."""
+    rot = Rotation.from_euler("xyz", [20, -30, 15], degrees=True)
+    qx, qy, qz, qw = rot.as_quat()
+    R = rot.as_matrix()
+    mu0 = np.array([0.05, -0.02, 1.7])
+    scs = []
+    for k, (a, b, o) in enumerate([(0, 0, 0.3), (0.2, 0.1, 0.6), (-0.15, 0.2, 0.9), (0.1, -0.2, 0.45), (-0.2, -0.1, 0.75)]):
+        scs.append(one_surfel(mu0 + a * R[:, 0] + b * R[:, 1], (0.12 + 0.02 * k, 0.1), (qw, qx, qy, qz), o))
+    sc = cat(*scs)
+    r = oracle.render_normalised(sc, oracle.make_cam(CAM), oracle.make_cfg())
+    # the plane through the float32 centres with the float32 quaternion's normal (centres are coplanar up to 1e-7)
+    q32 = sc.quat[0].astype(np.float64)
+    n = Rotation.from_quat([q32[1], q32[2], q32[3], q32[0]]).as_matrix()[:, 2]
+    X, Y = pix_grid(CAM)
+    d = np.stack([(X - CAM.cx) / CAM.fx, (Y - CAM.cy) / CAM.fy, np.ones_like(X)], axis=-1)
+    z = (n @ mu0) / (d @ n)
+    O = r["img"][7]
+    m = O > 0
+    assert m.sum() > 300 and (r["n_comp"] >= 2).sum() > 50
+    np.testing.assert_allclose(r["img"][3][m], z[m], rtol=1e-6)          # float32 rounding of the five centres
+    np.testing.assert_allclose(r["img_raw"][3][m], O[m] * z[m], rtol=1e-6)
+    assert np.abs(r["img_raw"][3][m] - z[m]).max() > 0.5                   # the un-normalised image is far from metric
+    assert (r["img"][3][~m] == 0).all()
+    for ch in (0, 1, 2, 4, 5, 6, 7):                                       # every other plane untouched
+        assert (r["img"][ch] == r["img_raw"][ch]).all()
+
+
+def test_p16_normalised_depth_two_layers_hand_value():
+    """Two fronto-parallel splats at z1 < z2 on the optical axis: at the principal pixel G = 1 for both (centre pixel
+    ray through both centres), so a1 = o1, a2 = o2 and D_n = (o1 z1 + o2 (1 - o1) z2) / (o1 + o2 (1 - o1))."""
+    cam = Camera(9, 9, 20.0, 20.0, 4.5, 4.5)
+    o1, o2, z1, z2 = 0.5, 0.25, 1.0, 3.0
+    sc = cat(one_surfel((0, 0, z1), (0.2, 0.2), (1, 0, 0, 0), o1), one_surfel((0, 0, z2), (0.5, 0.5), (1, 0, 0, 0), o2))
+    r = oracle.render_normalised(sc, oracle.make_cam(cam), oracle.make_cfg())
+    want = (o1 * z1 + o2 * (1 - o1) * z2) / (o1 + o2 * (1 - o1))            # = 0.875 / 0.625 = 1.4
+    assert abs(want - 1.4) < 1e-15
+    assert abs(r["img"][3][4, 4] - 1.4) < 1e-12
+    assert abs(r["img_raw"][3][4, 4] - 0.875) < 1e-12 and abs(r["img"][7][4, 4] - 0.625) < 1e-12
+
+
+def test_p16_normalised_depth_gradients_are_finite_differences():
+    """Surfel and SE(3) pose gradients of a loss on (rgb, D_n, normal, O) against central differences (smooth Eq. 8:
+    O > 0 at every pixel, D_n smooth), and with the alpha clamp active."""
+    _NORMALISED[0] = True
+    try:
+        _fd_check(oracle.smooth_cfg(), 2e-6)
+        _fd_check(oracle.make_cfg(cutoff=np.inf, alpha_min=0.0, alpha_max=0.6, t_min=0.0, z_near=0.0), 2e-6)
+    finally:
+        _NORMALISED[0] = False
+
+
+def test_p16_upstream_map_is_the_jacobian_transpose_of_the_division():
+    """normalised_depth_upstream against a direct numerical Jacobian of (D, O) -> D / O at random pixels."""
+    g = np.random.default_rng(5)
+    img = g.uniform(0.2, 1.0, (8, 3, 4)); img[7, 0, 0] = 0.0; img[3, 0, 0] = 0.0
+    up = g.normal(size=(8, 3, 4))
+    got = oracle.normalised_depth_upstream(img, up)
+    L = lambda im: float((oracle.normalise_depth(im) * up).sum())
+    for ch in (3, 7):
+        for (i, j) in [(1, 2), (2, 3), (0, 1)]:
+            p, m_ = img.copy(), img.copy()
+            p[ch, i, j] += 1e-6; m_[ch, i, j] -= 1e-6
+            assert abs((L(p) - L(m_)) / 2e-6 - got[ch, i, j]) < 1e-7
+    assert got[3, 0, 0] == 0.0 and got[7, 0, 0] == up[7, 0, 0]               # O = 0: only the opacity upstream survives
+    for ch in (0, 1, 2, 4, 5, 6):
+        assert (got[ch] == up[ch]).all()
