@@ -122,8 +122,9 @@ def aggregate_replicas(ms_local, pixels, renders_per_rank, world, dist=None, dev
 class Workload:
     """Device-resident inputs + the step function for one config."""
 
-    def __init__(self, name, iters_override=None, contrib=False, prefetch=True, reuse=True):
+    def __init__(self, name, iters_override=None, contrib=False, prefetch=True, reuse=True, normalised_depth=False):
         self.contrib = contrib
+        nd = self.normalised_depth = normalised_depth
         import torch
         import scenegen
         import paper_2506_00970_b200 as sgs
@@ -136,14 +137,14 @@ class Workload:
         self.t = dict(mean=d(sc.mean), scale=d(sc.scale), quat=d(sc.quat), opacity=d(sc.opacity), rgb=d(sc.rgb),
                       active=d(sc.active, torch.uint8))
         self.sf = sgs.Renderer.surfels(*(self.t[k] for k in ("mean", "scale", "quat", "opacity", "rgb", "active")))
-        self.ren = sgs.Renderer(async_mode=True, track_reuse=self.tracking and reuse)
+        self.ren = sgs.Renderer(async_mode=True, track_reuse=self.tracking and reuse, normalised_depth=nd)
         # mapping window: a second context + a side stream, so that sgs_prepare (binning) of view v+1 runs under the
         # compositing kernels of view v (include/sgs.h); tracking iterations depend on one another and use one context
         two = prefetch and not self.tracking and len(self.cams) > 1
         if two:  # + SGS_FLAG_LAZY_GRADS: a view's per-surfel kernel runs under the next view's forward; joined at the step's end
             self.ren.close()
-            self.ren = sgs.Renderer(async_mode=True, lazy_grads=True)
-        self.rens = [self.ren] + ([sgs.Renderer(async_mode=True, lazy_grads=True)] if two else [])
+            self.ren = sgs.Renderer(async_mode=True, lazy_grads=True, normalised_depth=nd)
+        self.rens = [self.ren] + ([sgs.Renderer(async_mode=True, lazy_grads=True, normalised_depth=nd)] if two else [])
         self.side = torch.cuda.Stream(priority=-1) if len(self.rens) > 1 else None
         cam0 = self.cams[0]
         self.H, self.W = cam0.height, cam0.width
@@ -341,6 +342,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-reuse", action="store_true", help="tracking configs: run the pre-cull over the whole map every iteration")
     ap.add_argument("--no-prefetch", action="store_true", help="mapping configs: one context, binning of each view in line")
+    ap.add_argument("--normalised-depth", action="store_true", help="SGS_FLAG_NORMALISED_DEPTH: depth image D/O (tracking takes the unfused sequence)")
     ap.add_argument("--contrib", action="store_true", help="mapping configs: render with sgs_render_contrib (C_k output on)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -360,7 +362,7 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    wl = Workload(args.config, args.iters, args.contrib, not args.no_prefetch, not args.no_reuse)
+    wl = Workload(args.config, args.iters, args.contrib, not args.no_prefetch, not args.no_reuse, args.normalised_depth)
     K, W = args.steps, max(args.warmup, 3)
     for _ in range(W):
         wl.step()
@@ -481,6 +483,8 @@ def main():
                                      if len(wl.rens) > 1 else "in line (sgs_render / sgs_track_iter)")),
                 clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roof, stages=stages, cpu_baseline=cpu,
                 stage_us={k: round(1e3 * v[0] / v[1], 2) for k, v in prof.items() if v[1]})
+    if args.normalised_depth:
+        line["config"]["depth"] = "normalised D/O (SGS_FLAG_NORMALISED_DEPTH); not the default workload"
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -64,7 +64,16 @@ enum {
     SGS_FLAG_RADIX_BINNING = 2, /* bin with the global LSD radix sort of the 64-bit keys instead of the
                                    default per-tile buckets + in-tile sort; same list, kept for A/B checks */
     SGS_FLAG_TRACK_REUSE = 4,   /* sgs_track_iter: the map is frozen between sgs_track_new_frame calls, see there */
-    SGS_FLAG_LAZY_GRADS = 8     /* sgs_backward: d_surfels / d_pose6 are complete only behind sgs_wait_grads, see there */
+    SGS_FLAG_LAZY_GRADS = 8,    /* sgs_backward: d_surfels / d_pose6 are complete only behind sgs_wait_grads, see there */
+    SGS_FLAG_NORMALISED_DEPTH = 16 /* SURVEY 8(f) NEXT-3 (variant of R9; Eq. 8 L116-120 renders D = sum w z and
+                                   O = sum w): the depth image is the expected depth D_n = D / O (0 where O = 0), i.e.
+                                   the blend weights renormalised to sum to one, so a partly transparent surface keeps
+                                   its metric depth.  The forward keeps (D_n, 1/O) per pixel in the context; every
+                                   backward (sgs_backward, the tracking backward) then takes the depth upstream as
+                                   dL/dD_n and carries it to dL/dD = g/O and dL/dO -= g D_n/O inside the compositing
+                                   backward's prologue.  Losses computed by this library (Eq. 15-19, Eq. 23-26) see D_n.
+                                   sgs_track_iter runs the unfused sequence (render, then the fused-loss backward)
+                                   under this flag: the one-kernel iteration has no opacity upstream. */
 };
 
 /* Truncation conventions of Eq. 8 (R3-R7).  sgs_default_config fills the defaults shown. */

@@ -73,6 +73,7 @@ int sgs_ensure_image(sgs_ctx* c, int tiles, int64_t pixels, cudaStream_t s) {
         if (!(ws_realloc(c, c->T_final, (size_t)pixels, s) && ws_realloc(c, c->n_last, (size_t)pixels, s) &&
               ws_realloc(c, c->img_scratch, (size_t)pixels * 8, s)))
             return SGS_OUT_OF_MEMORY;
+        if ((c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) && !ws_realloc(c, c->dn_state, (size_t)pixels, s)) return SGS_OUT_OF_MEMORY;
         c->pix_cap = pixels;
     }
     return SGS_OK;
@@ -234,7 +235,7 @@ int sgs_destroy(sgs_ctx* c) {
     cudaDeviceSynchronize();
     cudaStream_t s = 0;
     void* ptrs[] = {c->scan_state, c->vis_to_surfel, c->culled, c->pay.store, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
-                    c->sort_state, c->ranges, c->T_final, c->n_last, c->img_scratch, c->pose_partial, c->resident_store,
+                    c->sort_state, c->ranges, c->T_final, c->n_last, c->dn_state, c->img_scratch, c->pose_partial, c->resident_store,
                     c->resident_active, c->target_rgb, c->host_img_dev, c->host_up_dev, c->host_grads_dev,
                     c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->pose_inc, c->ssim_maps, c->surv_cnt, c->surv_in, c->export_keys, c->export_ranges};
     for (void* p : ptrs) sgs_ws_free(c, p, s);

@@ -34,13 +34,13 @@ struct StagedBwd {
 // upstream images through HBM; the loss itself rides in slot 6 of the pose partials.
 struct FusedLoss { const float* trgb; const float* tdepth; float lambda_d, nsign; float* loss; };
 
-template <bool POSE_ONLY, bool FUSED>
+template <bool POSE_ONLY, bool FUSED, bool NDEPTH>
 __global__ void __launch_bounds__(SGS_BLOCK)
 k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
            int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg, CPlanes up,
            const float* __restrict__ T_final, const uint32_t* __restrict__ n_last, float* __restrict__ acc,
            float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
-           FusedLoss fl) {
+           FusedLoss fl, const float2* __restrict__ dn_state) {
     __shared__ StagedBwd sh[SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
     __shared__ uint32_t sh_v[SGS_BLOCK];  // surfel (accumulator) index of each staged entry
@@ -85,6 +85,11 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
         } else {
 #pragma unroll
             for (int c = 0; c < 8; ++c) g[c] = up.p[c] ? up.p[c][pix] : 0.f;
+        }
+        if (NDEPTH) {  // SGS_FLAG_NORMALISED_DEPTH: g[3] is dL/dD_n; D_n = D / O  =>  dL/dD = g / O, dL/dO -= g D_n / O
+            const float2 dn = dn_state[pix];
+            g[3] *= dn.y;
+            g[7] = __fmaf_rn(-g[3], dn.x, g[7]);
         }
         T_after = T_final[pix];
         last = n_last[pix];
@@ -383,12 +388,16 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     CPlanes u;
     for (int i = 0; i < 8; ++i) u.p[i] = up[i];
     const SgsCamDev& cam = c->camd;
+    const float2* dn = (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) ? c->dn_state : nullptr;
     if (dg == nullptr) {  // pose-only (tracking, L204)
         if (d_pose6 == nullptr) return cudaSuccess;
         c->launches += 1;
-        k_backward<true, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
+        if (dn) k_backward<true, false, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                      cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
-                                                     c->acc, c->pose_partial, c->counters, d_pose6, FusedLoss{});
+                                                     c->acc, c->pose_partial, c->counters, d_pose6, FusedLoss{}, dn);
+        else k_backward<true, false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
+                                                     cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
+                                                     c->acc, c->pose_partial, c->counters, d_pose6, FusedLoss{}, dn);
         return cudaGetLastError();
     }
     const int64_t n = c->last_surfels.n;
@@ -409,9 +418,12 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     if (e != cudaSuccess) return e;
     if (ms != s && (e = cudaEventRecord(c->join_ev, ms)) != cudaSuccess) return e;
     c->launches += 1;
-    k_backward<false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
+    if (dn) k_backward<false, false, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                   cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
-                                                  c->acc, c->pose_partial, c->counters, nullptr, FusedLoss{});
+                                                  c->acc, c->pose_partial, c->counters, nullptr, FusedLoss{}, dn);
+    else k_backward<false, false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
+                                                  cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
+                                                  c->acc, c->pose_partial, c->counters, nullptr, FusedLoss{}, dn);
     // SGS_FLAG_LAZY_GRADS: the per-surfel kernel (latency-bound: 12 % issue utilisation) stays on the ctx's stream, behind
     // k_backward by an event, and the caller's stream does NOT wait for it: sgs_wait_grads does (the next view's kernels
     // run meanwhile).  Otherwise the caller's stream joins here.
@@ -445,10 +457,14 @@ cudaError_t sgs_launch_backward_tracking(sgs_ctx* c, const float* trgb, const fl
     CPlanes u;
     for (int i = 0; i < 8; ++i) u.p[i] = c->last_img[i];
     const SgsCamDev& cam = c->camd;
+    const float2* dn = (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) ? c->dn_state : nullptr;
     FusedLoss fl{trgb, tdepth, lambda_d, nsign, loss};
     c->launches += 1;
-    k_backward<true, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H,
+    if (dn) k_backward<true, true, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H,
                                                        cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final,
-                                                       c->n_last, c->acc, c->pose_partial, c->counters, d_pose6, fl);
+                                                       c->n_last, c->acc, c->pose_partial, c->counters, d_pose6, fl, dn);
+    else k_backward<true, true, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H,
+                                                       cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final,
+                                                       c->n_last, c->acc, c->pose_partial, c->counters, d_pose6, fl, dn);
     return cudaGetLastError();
 }

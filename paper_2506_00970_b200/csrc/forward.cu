@@ -13,12 +13,12 @@ namespace {
 
 struct Planes { float* p[8]; };
 
-template <bool CONTRIB>
-__global__ void __launch_bounds__(SGS_BLOCK)
+template <bool CONTRIB, bool NDEPTH>
+__global__ void __launch_bounds__(SGS_BLOCK, 4)  // 64 registers: four blocks per SM (the D_n variant would take 72 and lose one)
 k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
           int tiles_x, SgsCfgDev cfg, Planes out, float* __restrict__ T_final, uint32_t* __restrict__ n_last,
           const uint32_t* __restrict__ cursor, unsigned long long* bucket, uint32_t tile_cap,
-          float* __restrict__ contrib) {
+          float* __restrict__ contrib, float2* __restrict__ dn_state) {
     // staged batch, structure of float4 arrays (one base register, immediate offsets, broadcast reads)
     __shared__ float4 sh[5][SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
@@ -140,6 +140,11 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
     }
     if (inside) {
         const size_t pix = (size_t)py * W + px;
+        if (NDEPTH) {  // SGS_FLAG_NORMALISED_DEPTH: D_n = D / O, kept with 1 / O for the backward's prologue
+            const float io = O > 0.f ? __frcp_rn(O) : 0.f;
+            Dp = __fmul_rn(Dp, io);
+            dn_state[pix] = make_float2(Dp, io);
+        }
         if (out.p[0]) out.p[0][pix] = C0;
         if (out.p[1]) out.p[1][pix] = C1;
         if (out.p[2]) out.p[2][pix] = C2;
@@ -163,9 +168,16 @@ cudaError_t sgs_launch_forward(sgs_ctx* c, float* const planes[8], cudaStream_t 
     c->launches += 1;
 #define SGS_FWD_ARGS c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, c->camd.W, \
                      c->camd.H, c->camd.tiles_x, c->cfgd, out, c->T_final, c->n_last, c->fused_sort ? c->cursor : nullptr,     \
-                     reinterpret_cast<unsigned long long*>(c->bucket), (uint32_t)c->tile_cap, c->contrib_out
-    if (c->contrib_out) k_forward<true><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
-    else k_forward<false><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+                     reinterpret_cast<unsigned long long*>(c->bucket), (uint32_t)c->tile_cap, c->contrib_out, \
+                     (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) ? c->dn_state : nullptr
+    const bool nd = (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) != 0;
+    if (c->contrib_out) {
+        if (nd) k_forward<true, true><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+        else k_forward<true, false><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+    } else {
+        if (nd) k_forward<false, true><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+        else k_forward<false, false><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+    }
 #undef SGS_FWD_ARGS
     return cudaGetLastError();
 }

@@ -119,6 +119,7 @@ struct sgs_ctx {
     uint32_t* ranges;                // tiles x 2
     float* T_final;                  // pixels
     uint32_t* n_last;                // pixels: index (within the tile list) after the last composited entry
+    float2* dn_state;                // pixels, SGS_FLAG_NORMALISED_DEPTH only: (D / O, 1 / O) of the last forward (0, 0 where O = 0)
     float* pose_partial;             // tiles x 8 (pose-only) or blocks x 8 (per-surfel)
     float* img_saved[8];             // planes the backward needs when the caller did not ask for them
     float* img_scratch;              // 8 planes, pix_cap each

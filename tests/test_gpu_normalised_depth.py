@@ -1,0 +1,135 @@
+"""GPU parity of SGS_FLAG_NORMALISED_DEPTH (depth image D_n = D / O) against the oracle's
+normalise_depth / normalised_depth_upstream (pinned by P16): images, full and pose-only backward, the tracking
+iteration (sgs_track_iter takes the unfused sequence under this flag) and the degenerate cases."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import scenegen
+from scenegen import Scene, Camera
+
+pytestmark = pytest.mark.gpu
+
+sgs = pytest.importorskip("paper_2506_00970_b200")
+from gpu_common import (to_device, camera, alloc_images, planes, alloc_grads, split_upstream, image_check,  # noqa: E402
+                        grad_check)
+
+
+@pytest.fixture(scope="module")
+def ren():
+    r = sgs.Renderer(normalised_depth=True)
+    yield r
+    r.close()
+
+
+def check_images(gimg, o):
+    chk = image_check(gimg, o["img"], o["fragile"])
+    assert chk["n_bad"] == 0, chk
+    assert chk["fragile_ok"], chk
+
+
+@pytest.mark.parametrize("tau", [None, [0.1, -0.2, 0.15, 0.2, -0.1, 0.3]])
+def test_c1_images_and_all_gradients(ren, tau):
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    T = None if tau is None else scenegen.perturb_pose(cam.T_cw, tau)
+    camv, cfg = oracle.make_cam(cam, T), oracle.make_cfg()
+    up = scenegen.upstream_normal(1, cam.height, cam.width)
+    t, sf = to_device(sc)
+    c = camera(cam, T)
+    im = alloc_images(cam)
+    ren.render(sf, c, **im)
+    o = oracle.render_normalised(sc, camv, cfg)
+    gimg = planes(im)
+    check_images(gimg, o)
+    m = o["img"][7] > 0.05
+    assert np.abs(gimg[3][m] - o["img_raw"][3][m]).max() > 0.1      # it is not the Eq. 8 depth any more
+    ob = oracle.binning(sc, camv, cfg)
+    gb = ren.get_binning(sc.n, 12)
+    assert np.array_equal(gb["keys"], ob["keys"]) and np.array_equal(gb["idx"], ob["idx"])
+    og = oracle.backward_normalised(sc, camv, cfg, up)
+    g, p6 = alloc_grads(sc.n), torch.full((6,), 3.0, device="cuda")
+    ren.backward(**split_upstream(up), grads=g, d_pose6=p6)
+    torch.cuda.synchronize()
+    for k in ("mean", "scale", "quat", "opacity", "rgb"):
+        chk = grad_check(g[k].cpu().numpy(), og[k])
+        assert chk["frac_bad"] <= 2e-3, (k, chk)
+    assert np.abs(p6.cpu().numpy() - og["pose"]).max() <= 1e-3 * np.abs(og["pose"]).max()
+    # the normalisation matters to the gradients: the plain backward of the same upstream is far away
+    plain = oracle.backward(sc, camv, cfg, up)
+    assert np.abs(plain["pose"] - og["pose"]).max() > 0.05 * np.abs(og["pose"]).max()
+    # pose-only mode, depth upstream alone (dL/dO comes from the depth term only)
+    up_d = np.zeros_like(up); up_d[3] = up[3]
+    ren.render(sf, c, **im)
+    p6b = torch.zeros(6, device="cuda")
+    ren.backward(**split_upstream(up_d), d_pose6=p6b)
+    ogd = oracle.backward_normalised(sc, camv, cfg, up_d)
+    assert np.abs(p6b.cpu().numpy() - ogd["pose"]).max() <= 1e-3 * np.abs(ogd["pose"]).max()
+
+
+def test_c2_tracking_iteration_at_full_size(ren):
+    """C2 (200k surfels, 640x480): images, then sgs_track_iter (loss Eq. 15-19 on D_n, pose gradient) against the
+    oracle's loss on the GPU's images and its analytic backward through the division."""
+    sc, cams, info = scenegen.make_config("C2")
+    cam = cams[0]
+    camv, cfg = oracle.make_cam(cam), oracle.make_cfg()
+    g = scenegen.SplitMix(info["tau0_seed"])
+    d = np.stack([g.normal(3), g.normal(3)])
+    tau0 = np.concatenate([0.02 * d[0] / np.linalg.norm(d[0]), np.deg2rad(1.0) * d[1] / np.linalg.norm(d[1])])
+    tgt = oracle.render_normalised(sc, oracle.make_cam(cam, scenegen.perturb_pose(cam.T_cw, tau0)), cfg, counters=False)["img"]
+    t, sf = to_device(sc)
+    c = camera(cam)
+    im = alloc_images(cam)
+    trgb = torch.from_numpy(tgt[0:3].astype(np.float32)).cuda()
+    tdep = torch.from_numpy(tgt[3:4].astype(np.float32)).cuda()
+    p6, loss = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+    ren.track_iter(sf, c, trgb, tdep, 0.5, -1.0, p6, loss, **im)
+    torch.cuda.synchronize()
+    o = oracle.render_normalised(sc, camv, cfg)
+    gimg = planes(im)
+    check_images(gimg, o)
+    L_ref, up_ref = oracle.tracking_loss(gimg, trgb.cpu().numpy(), tdep.cpu().numpy()[0], camv, 0.5, -1.0)
+    assert (up_ref[3] != 0).mean() > 0.05
+    assert abs(float(loss.item()) - L_ref) <= 1e-4 * abs(L_ref)
+    og = oracle.backward_normalised(sc, camv, cfg, up_ref)
+    assert np.abs(p6.cpu().numpy() - og["pose"]).max() <= 1e-3 * np.abs(og["pose"]).max(), (p6, og["pose"])
+    # render + backward_tracking gives the same numbers as track_iter
+    im2 = alloc_images(cam)
+    ren.render(sf, c, **im2)
+    p6b, lb = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+    ren.backward_tracking(trgb, tdep, 0.5, -1.0, p6b, lb)
+    torch.cuda.synchronize()
+    assert np.array_equal(planes(im2), gimg)
+    np.testing.assert_allclose(p6b.cpu().numpy(), p6.cpu().numpy(), rtol=1e-5, atol=1e-7 * float(p6.abs().max()))
+
+
+def test_degenerate_cases(ren):
+    cam = Camera(40, 24, 30.0, 30.0, 20.0, 12.0)
+    # no surfels: O = 0 everywhere -> D_n = 0, gradients zero, nothing non-finite
+    z = lambda *s: np.zeros(s, np.float32)
+    sc0 = Scene(z(0, 3), z(0, 2), z(0, 4), z(0), z(0, 3))
+    t, sf = to_device(sc0)
+    im = alloc_images(cam)
+    for v in im.values():
+        v.fill_(5.0)
+    ren.render(sf, camera(cam), **im)
+    assert float(planes(im)[3].max()) == 0.0 and float(planes(im)[7].max()) == 0.0
+    # one small splat: most pixels empty (D_n = 0 there), covered pixels carry the plane's depth
+    sc1 = Scene(np.float32([[0, 0, 2.0]]), np.float32([[0.1, 0.1]]), np.float32([[1, 0, 0, 0]]), np.float32([0.3]),
+                np.float32([[0.2, 0.4, 0.6]]))
+    t, sf = to_device(sc1)
+    ren.render(sf, camera(cam), **im)
+    gi = planes(im)
+    cov = gi[7] > 0
+    assert 0 < cov.sum() < cov.size
+    assert np.abs(gi[3][cov] - 2.0).max() < 1e-5 and (gi[3][~cov] == 0).all()
+    up = scenegen.upstream_normal(3, cam.height, cam.width)
+    g, p6 = alloc_grads(1), torch.zeros(6, device="cuda")
+    ren.backward(**split_upstream(up), grads=g, d_pose6=p6)
+    og = oracle.backward_normalised(sc1, oracle.make_cam(cam), oracle.make_cfg(), up)
+    for k in ("mean", "scale", "quat", "opacity", "rgb"):
+        a = g[k].cpu().numpy().astype(np.float64)
+        assert np.isfinite(a).all()
+        assert np.abs(a - og[k]).max() <= 1e-3 * np.abs(og[k]).max() + 1e-6, (k, a, og[k])
+    assert np.abs(p6.cpu().numpy() - og["pose"]).max() <= 1e-3 * np.abs(og["pose"]).max()
