@@ -31,7 +31,8 @@ UNIT = "MP/s"
 F_TEST, F_COMP_FWD, F_COMP_BWD_FULL, F_COMP_BWD_POSE = 26, 26, 102, 94
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
 # captures (profiles/r01_*.md; ncu flushes L2 before every replay, so these are cold-cache figures)
-NCU_TRAFFIC = {("C2", "track"): 8.49e6, ("C2", "backward"): 30.6e6, ("C2", "forward"): 14.0e6}
+NCU_TRAFFIC = {("C2", "track"): 8.49e6, ("C2", "backward"): 30.6e6, ("C2", "forward"): 14.0e6,
+               ("C4", "backward"): 70.2e6, ("C3", "backward"): 68.3e6, ("C4", "forward"): 31.5e6, ("C5", "track"): 31.3e6}
 
 
 def load_peaks():
