@@ -252,7 +252,7 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
                    float normal_sign, const sgs_images* out, float* d_pose6, float* loss, void* stream) {
     if (!c || !target || !target->rgb || !target->depth || !d_pose6) return SGS_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
-    if (radix_mode(c) || (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH)) {  // A/B binning path, or D_n = D / O (needs an opacity upstream): the unfused sequence
+    if (radix_mode(c)) {  // A/B binning path: the unfused sequence
         int r = sgs_render(c, sf, cam, out, stream);
         if (r != SGS_OK) return r;
         r = sgs_backward_tracking(c, target, lambda_d, normal_sign, d_pose6, loss, stream);

@@ -61,7 +61,7 @@ __device__ __forceinline__ float pair_rho2(const float4 s0, const float4 s1, con
     return __fmaf_rn(v, v, __fmul_rn(u, u));
 }
 
-template <bool WRITE_IMAGES>
+template <bool WRITE_IMAGES, bool NDEPTH>
 __global__ void __launch_bounds__(SGS_BLOCK, 3)
 k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cursor, unsigned long long* bucket, uint32_t tile_cap,
         int presorted, SgsPayload pay, int W, int H, int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg,
@@ -160,7 +160,15 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     // ---- Eq. 15-19 in registers (same arithmetic as loss.cu): loss term and upstream gradients of rgb, depth ----
     const float rx = ((float)px + 0.5f - cx) / fx, ry = ((float)py + 0.5f - cy) / fy;  // pixel ray (rx, ry, 1)
     float g0 = 0.f, g1 = 0.f, g2 = 0.f, g3 = 0.f, my_loss = 0.f;
+    // SGS_FLAG_NORMALISED_DEPTH (launched without helpers): the depth image and the loss take D_n = D / O; its upstream g
+    // becomes dL/dD = g / O (kept in g3) and dL/dO = -g3 D_n, which the walk back carries as g3 (z - zref), zref = D_n
+    float zref = 0.f;
     auto finish_forward = [&]() {
+        if (NDEPTH) {
+            const float io = O > 0.f ? __frcp_rn(O) : 0.f;
+            Dp = __fmul_rn(Dp, io);
+            zref = Dp;
+        }
         if (WRITE_IMAGES && inside) {
             if (out.p[0]) out.p[0][pix] = C0;
             if (out.p[1]) out.p[1][pix] = C1;
@@ -180,6 +188,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
                 d = C2 - tb; my_loss += fabsf(d); g2 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
                 d = Dp - td; my_loss += lambda_d * fabsf(d);
                 g3 = d > 0.f ? lambda_d * inv : (d < 0.f ? -lambda_d * inv : 0.f);
+                if (NDEPTH) g3 *= __frcp_rn(O);  // O > 0.95 here
             }
             my_loss *= inv;
         }
@@ -219,7 +228,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
                     hit[k] = has && (boff + j) < last && (rho2 <= cfg.cutoff2) && (r[k].z > cfg.z_near) && (r[k].a >= cfg.alpha_min);
                     opac[k] = s3.x;
                     inv1ma[k] = fast_rcp(1.f - r[k].a);
-                    gv[k] = g0 * s3.y + g1 * s3.z + g2 * s3.w + g3 * r[k].z;
+                    gv[k] = g0 * s3.y + g1 * s3.z + g2 * s3.w + g3 * (NDEPTH ? r[k].z - zref : r[k].z);
                     anyh = anyh || hit[k];
                 }
                 if (!__any_sync(0xffffffffu, anyh)) continue;
@@ -534,19 +543,22 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
     const uint32_t tile_cap = (uint32_t)c->tile_cap;
     SgsCounters* snap = after_preprocess ? c->counters_snap + c->snap_slot : nullptr;
     unsigned int* hflag = c->host_flag_want ? c->host_flag_dev : nullptr;  // (sgs_track_iter_host)
-    const int n_help = (c->split_state && tiles >= 4 * SGS_TRACK_HELPERS) ? SGS_TRACK_HELPERS : 0;
+    // D_n = D / O: the walk back carries an opacity upstream that the owner -> helper hand-over does not; no helpers then
+    const bool ndepth = (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) != 0;
+    const int n_help = (!ndepth && c->split_state && tiles >= 4 * SGS_TRACK_HELPERS) ? SGS_TRACK_HELPERS : 0;
     c->track_launch_id += 1;
     c->host_flag_armed = hflag != nullptr;
-    if (any)
-        k_track<true><<<tiles + n_help, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W,
-                                                  cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb, tdepth,
-                                                  lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost,
-                                                  c->cursor, snap, hflag, c->host_flag_val, c->split_state, c->split_flag, c->track_launch_id, n_help);
-    else
-        k_track<false><<<tiles + n_help, SGS_BLOCK, 0, s>>>(c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W,
-                                                   cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, out, trgb, tdepth,
-                                                   lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost,
-                                                   c->cursor, snap, hflag, c->host_flag_val, c->split_state, c->split_flag, c->track_launch_id, n_help);
+#define SGS_TRK_ARGS c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W, cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, \
+                     cam.cy, c->cfgd, out, trgb, tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost, c->cursor,   \
+                     snap, hflag, c->host_flag_val, c->split_state, c->split_flag, c->track_launch_id, n_help
+    if (ndepth) {
+        if (any) k_track<true, true><<<tiles + n_help, SGS_BLOCK, 0, s>>>(SGS_TRK_ARGS);
+        else k_track<false, true><<<tiles + n_help, SGS_BLOCK, 0, s>>>(SGS_TRK_ARGS);
+    } else {
+        if (any) k_track<true, false><<<tiles + n_help, SGS_BLOCK, 0, s>>>(SGS_TRK_ARGS);
+        else k_track<false, false><<<tiles + n_help, SGS_BLOCK, 0, s>>>(SGS_TRK_ARGS);
+    }
+#undef SGS_TRK_ARGS
     {   // next iteration's tile order from this launch's measured tile costs, beside the next K-pre-B
         cudaStream_t os = c->aux_stream ? c->aux_stream : s;
         if (os != s && (cudaEventRecord(c->order_fork, s) != cudaSuccess || cudaStreamWaitEvent(os, c->order_fork, 0) != cudaSuccess))

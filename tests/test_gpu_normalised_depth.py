@@ -1,6 +1,6 @@
 """GPU parity of SGS_FLAG_NORMALISED_DEPTH (depth image D_n = D / O) against the oracle's
 normalise_depth / normalised_depth_upstream (pinned by P16): images, full and pose-only backward, the tracking
-iteration (sgs_track_iter takes the unfused sequence under this flag) and the degenerate cases."""
+iteration (k_track<NDEPTH>, and its equality with render + sgs_backward_tracking) and the degenerate cases."""
 import numpy as np
 import pytest
 import torch
@@ -101,7 +101,8 @@ def test_c2_tracking_iteration_at_full_size(ren):
     ren.backward_tracking(trgb, tdep, 0.5, -1.0, p6b, lb)
     torch.cuda.synchronize()
     assert np.array_equal(planes(im2), gimg)
-    np.testing.assert_allclose(p6b.cpu().numpy(), p6.cpu().numpy(), rtol=1e-5, atol=1e-7 * float(p6.abs().max()))
+    np.testing.assert_allclose(p6b.cpu().numpy(), p6.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(p6.abs().max()))
+    np.testing.assert_allclose(lb.cpu().numpy(), loss.cpu().numpy(), rtol=1e-5)
 
 
 def test_degenerate_cases(ren):
@@ -133,3 +134,38 @@ def test_degenerate_cases(ren):
         assert np.isfinite(a).all()
         assert np.abs(a - og[k]).max() <= 1e-3 * np.abs(og[k]).max() + 1e-6, (k, a, og[k])
     assert np.abs(p6.cpu().numpy() - og["pose"]).max() <= 1e-3 * np.abs(og["pose"]).max()
+
+
+def test_track_iter_long_lists_and_reuse():
+    """k_track<NDEPTH> == render + sgs_backward_tracking on C1 and on tile lists of ~900 entries (several 256-entry batches)
+    and ~6000 entries (pre-sorted path), with and without the kept survivor list."""
+    cases = []
+    sc, cams, _ = scenegen.make_config("C1")
+    cases.append((sc, cams[0]))
+    g = scenegen.SplitMix(11)
+    for n in (900, 6000):
+        mean = np.stack([g.uniform(n, -0.05, 0.05), g.uniform(n, -0.05, 0.05), g.uniform(n, 1.0, 3.0)], 1).astype(np.float32)
+        cases.append((Scene(mean, np.full((n, 2), 0.01, np.float32), np.tile(np.float32([1, 0.1, 0, 0]), (n, 1)),
+                            np.full(n, 0.03 if n > 2000 else 0.2, np.float32),
+                            np.stack([g.uniform(n) for _ in range(3)], 1).astype(np.float32)),
+                      Camera(64, 48, 60.0, 60.0, 32.0, 24.0)))
+    for reuse in (False, True):
+        for sc, cam in cases:
+            r = sgs.Renderer(normalised_depth=True, track_reuse=reuse)
+            t, sf = to_device(sc)
+            c = camera(cam)
+            im, im2 = alloc_images(cam), alloc_images(cam)
+            r.render(sf, c, **im)
+            tgt_rgb = (im["rgb"] * 0.9 + 0.01).contiguous()
+            tgt_dep = (im["depth"] * 1.02).contiguous()
+            p6a, la = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+            r.backward_tracking(tgt_rgb, tgt_dep, 0.5, 1.0, p6a, la)
+            for _ in range(2):   # second call: from the kept list under reuse
+                p6b, lb = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+                r.track_iter(sf, c, tgt_rgb, tgt_dep, 0.5, 1.0, p6b, lb, **im2)
+                torch.cuda.synchronize()
+                assert np.array_equal(planes(im), planes(im2))
+                assert float(la.abs().item()) > 0 and np.abs(p6a.cpu().numpy()).max() > 0
+                np.testing.assert_allclose(lb.cpu().numpy(), la.cpu().numpy(), rtol=1e-5)
+                np.testing.assert_allclose(p6b.cpu().numpy(), p6a.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(p6a.abs().max()))
+            r.close()
