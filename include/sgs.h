@@ -72,8 +72,7 @@ enum {
                                    backward (sgs_backward, the tracking backward) then takes the depth upstream as
                                    dL/dD_n and carries it to dL/dD = g/O and dL/dO -= g D_n/O inside the compositing
                                    backward's prologue.  Losses computed by this library (Eq. 15-19, Eq. 23-26) see D_n.
-                                   sgs_track_iter's one-kernel iteration runs without helper blocks under this flag
-                                   (their hand-over carries no opacity upstream). */
+                                   sgs_track_iter keeps its one-kernel iteration under this flag. */
 };
 
 /* Truncation conventions of Eq. 8 (R3-R7).  sgs_default_config fills the defaults shown. */

@@ -207,7 +207,7 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
               cudaMallocHost(&c->counters_host, sizeof(SgsCounters)) == cudaSuccess &&
               cudaHostAlloc(&c->pinned_small, 8 * sizeof(float), cudaHostAllocMapped) == cudaSuccess &&
               cudaHostAlloc(&c->host_flag, sizeof(unsigned int), cudaHostAllocMapped) == cudaSuccess &&
-              cudaMalloc(&c->split_state, sizeof(float) * 6 * SGS_BLOCK * SGS_TRACK_HELPERS) == cudaSuccess &&
+              cudaMalloc(&c->split_state, sizeof(float) * 8 * SGS_BLOCK * SGS_TRACK_HELPERS) == cudaSuccess &&
               cudaMalloc(&c->split_flag, sizeof(unsigned int) * SGS_TRACK_HELPERS) == cudaSuccess &&
               cudaMemset(c->split_flag, 0, sizeof(unsigned int) * SGS_TRACK_HELPERS) == cudaSuccess &&
               cudaHostGetDevicePointer(&c->pinned_small_dev, c->pinned_small, 0) == cudaSuccess &&

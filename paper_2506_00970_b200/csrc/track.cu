@@ -160,7 +160,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     // ---- Eq. 15-19 in registers (same arithmetic as loss.cu): loss term and upstream gradients of rgb, depth ----
     const float rx = ((float)px + 0.5f - cx) / fx, ry = ((float)py + 0.5f - cy) / fy;  // pixel ray (rx, ry, 1)
     float g0 = 0.f, g1 = 0.f, g2 = 0.f, g3 = 0.f, my_loss = 0.f;
-    // SGS_FLAG_NORMALISED_DEPTH (launched without helpers): the depth image and the loss take D_n = D / O; its upstream g
+    // SGS_FLAG_NORMALISED_DEPTH: the depth image and the loss take D_n = D / O; its upstream g
     // becomes dL/dD = g / O (kept in g3) and dL/dO = -g3 D_n, which the walk back carries as g3 (z - zref), zref = D_n
     float zref = 0.f;
     auto finish_forward = [&]() {
@@ -282,7 +282,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     const bool split = (helper || has_helper) && !presorted && n > TRK_SPLIT_MIN && n <= (uint32_t)TRK_CAP;
     const uint32_t msp = split ? (((n + 1u) / 2u + 31u) & ~31u) : n;  // block 0: [0, msp) on the way back, block 1: [msp, n)
     // per-pixel state the owner hands to its helper: 6 x 256 floats in global memory, published by a flag = this launch's id
-    float* st = split_state + (size_t)slot * (6 * SGS_BLOCK);
+    float* st = split_state + (size_t)slot * (8 * SGS_BLOCK);  // g0..g3, T, last, zref (NDEPTH), one spare
     if (crank == 1) {
         if (split) {
             for (uint32_t e = tid; e < (uint32_t)TRK_CAP; e += SGS_BLOCK) {
@@ -310,6 +310,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
             g0 = __ldcg(st + tid); g1 = __ldcg(st + SGS_BLOCK + tid); g2 = __ldcg(st + 2 * SGS_BLOCK + tid);
             g3 = __ldcg(st + 3 * SGS_BLOCK + tid); T_after = __ldcg(st + 4 * SGS_BLOCK + tid);
             last = __float_as_uint(__ldcg(st + 5 * SGS_BLOCK + tid));
+            if (NDEPTH) zref = __ldcg(st + 6 * SGS_BLOCK + tid);
             const uint32_t wmax = warp_max_last();
             backward_walk(msp, (int)min(n - msp, wmax > msp ? wmax - msp : 0u));
         }
@@ -344,18 +345,22 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         } else {
             forward_walk(0u, msp);
             const float Tm = T, C0m = C0, C1m = C1, C2m = C2, Dpm = Dp;  // the pixel's state between the two parts
+            const float Om = O;
             forward_walk(0u, n, msp);
+            const float Draw = Dp;  // (finish_forward<NDEPTH> turns Dp into D / O)
             finish_forward();
             // hand (g, T_final, last) of this pixel to the helper
             st[tid] = g0; st[SGS_BLOCK + tid] = g1; st[2 * SGS_BLOCK + tid] = g2; st[3 * SGS_BLOCK + tid] = g3;
             st[4 * SGS_BLOCK + tid] = T; st[5 * SGS_BLOCK + tid] = __uint_as_float(last);
+            if (NDEPTH) st[6 * SGS_BLOCK + tid] = zref;
             __threadfence();
             __syncthreads();
             if (tid == 0) *reinterpret_cast<volatile unsigned int*>(split_flag + slot) = launch_id;
             // the way back over [0, msp): transmittance behind entry msp - 1 and the suffix sum of everything behind it,
             // sum_{j >= msp} w_j (g . v_j) = g . (V_final - V_msp) with V the running accumulators of Eq. 8
             T_after = Tm;
-            suffix = g0 * (C0 - C0m) + g1 * (C1 - C1m) + g2 * (C2 - C2m) + g3 * (Dp - Dpm);
+            suffix = g0 * (C0 - C0m) + g1 * (C1 - C1m) + g2 * (C2 - C2m) +
+                     g3 * (NDEPTH ? (Draw - Dpm) - zref * (O - Om) : Draw - Dpm);
             backward_walk(0u, (int)min(msp, warp_max_last()));
         }
     } else {
@@ -543,9 +548,8 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
     const uint32_t tile_cap = (uint32_t)c->tile_cap;
     SgsCounters* snap = after_preprocess ? c->counters_snap + c->snap_slot : nullptr;
     unsigned int* hflag = c->host_flag_want ? c->host_flag_dev : nullptr;  // (sgs_track_iter_host)
-    // D_n = D / O: the walk back carries an opacity upstream that the owner -> helper hand-over does not; no helpers then
     const bool ndepth = (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) != 0;
-    const int n_help = (!ndepth && c->split_state && tiles >= 4 * SGS_TRACK_HELPERS) ? SGS_TRACK_HELPERS : 0;
+    const int n_help = (c->split_state && tiles >= 4 * SGS_TRACK_HELPERS) ? SGS_TRACK_HELPERS : 0;
     c->track_launch_id += 1;
     c->host_flag_armed = hflag != nullptr;
 #define SGS_TRK_ARGS c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W, cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, \
