@@ -169,3 +169,61 @@ def test_track_iter_long_lists_and_reuse():
                 np.testing.assert_allclose(lb.cpu().numpy(), la.cpu().numpy(), rtol=1e-5)
                 np.testing.assert_allclose(p6b.cpu().numpy(), p6a.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(p6a.abs().max()))
             r.close()
+
+
+def test_flag_through_async_prepare_and_host_calls(ren):
+    """The same D_n images and gradients through SGS_FLAG_ASYNC, sgs_prepare + sgs_render, sgs_render_contrib and the
+    HOST-buffer calls (sgs_render_host, sgs_backward_host, sgs_track_iter_host) as through the plain device calls."""
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    up = scenegen.upstream_normal(6, cam.height, cam.width)
+    t, sf = to_device(sc)
+    c = camera(cam)
+
+    def full(r, prep=False, contrib=False):
+        im, g, p6 = alloc_images(cam), alloc_grads(sc.n), torch.zeros(6, device="cuda")
+        if prep:
+            r.prepare(sf, c)
+        if contrib:
+            r.render_contrib(sf, c, torch.zeros(sc.n, device="cuda"), **im)
+        else:
+            r.render(sf, c, **im)
+        r.backward(**split_upstream(up), grads=g, d_pose6=p6)
+        torch.cuda.synchronize()
+        return planes(im), {k: v.cpu().numpy() for k, v in g.items()}, p6.cpu().numpy()
+
+    ref = full(ren)
+    a = sgs.Renderer(async_mode=True, normalised_depth=True)
+    for kw in (dict(), dict(prep=True), dict(contrib=True)):
+        for _ in range(2):
+            img, g, p6 = full(a, **kw)
+        assert np.array_equal(img, ref[0]), kw
+        for k in g:
+            np.testing.assert_allclose(g[k], ref[1][k], rtol=2e-4, atol=1e-5 * np.abs(ref[1][k]).max())
+        np.testing.assert_allclose(p6, ref[2], rtol=1e-4, atol=1e-5 * np.abs(ref[2]).max())
+    pin = lambda x, dt=torch.float32: torch.from_numpy(np.ascontiguousarray(x)).to(dt).pin_memory()
+    a.upload_surfels(pin(sc.mean), pin(sc.scale), pin(sc.quat), pin(sc.opacity), pin(sc.rgb))
+    H, W = cam.height, cam.width
+    h = dict(rgb=torch.zeros(3, H, W).pin_memory(), depth=torch.zeros(1, H, W).pin_memory(),
+             normal=torch.zeros(3, H, W).pin_memory(), alpha=torch.zeros(1, H, W).pin_memory())
+    a.render_host(c, **h)
+    himg = torch.cat([h["rgb"], h["depth"], h["normal"], h["alpha"]], 0).numpy().astype(np.float64)
+    assert np.array_equal(himg, ref[0])
+    u = torch.from_numpy(up)
+    hg = {k: torch.zeros(v.shape).pin_memory() for k, v in ref[1].items()}
+    hp = torch.zeros(6).pin_memory()
+    a.backward_host(d_rgb=u[0:3].contiguous(), d_depth=u[3:4].contiguous(), d_normal=u[4:7].contiguous(),
+                    d_alpha=u[7:8].contiguous(), grads=hg, d_pose6=hp)
+    for k in hg:
+        np.testing.assert_allclose(hg[k].numpy(), ref[1][k], rtol=2e-4, atol=1e-4 * np.abs(ref[1][k]).max())
+    np.testing.assert_allclose(hp.numpy(), ref[2], rtol=1e-4, atol=1e-5 * np.abs(ref[2]).max())
+    # resident tracking iteration == the device-buffer iteration on the same target
+    trgb, tdep = (h["rgb"] * 0.9).contiguous(), (h["depth"] * 1.01).contiguous()
+    a.upload_target(c, trgb.pin_memory(), tdep.pin_memory())
+    loss_h, p6_h = a.track_iter_host(c, 0.5, 1.0)
+    p6d, ld = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+    ren.track_iter(sf, c, trgb.cuda(), tdep.cuda(), 0.5, 1.0, p6d, ld)
+    torch.cuda.synchronize()
+    assert abs(loss_h - float(ld.item())) <= 1e-5 * abs(float(ld.item())) and abs(loss_h) > 0
+    np.testing.assert_allclose(p6_h, p6d.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(p6d.abs().max()))
+    a.close()
