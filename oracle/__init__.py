@@ -134,6 +134,19 @@ def contribution(sc, camv, cfgv, brute=False):
     return contrib
 
 
+def median_depth(sc, camv, cfgv, brute=False):
+    """Median depth image (DESIGN R9m): the intersection depth of the composited splat at which the pixel's transmittance
+    first falls to <= 1/2; 0 where T_final > 1/2.  Returns (median (H,W) f64, fragile (H,W) u8: a composited splat left T
+    within 1e-4 of 1/2)."""
+    mean, scale, quat, opac, rgb, act = _scene_arrays(sc)
+    W, H = int(camv[0]), int(camv[1])
+    img = np.zeros((8, H, W)); med = np.zeros((H, W)); mf = np.zeros((H, W), np.uint8)
+    lib().orc_render_ex2(ctypes.c_int64(sc.n), _p(mean, C_F32), _p(scale, C_F32), _p(quat, C_F32), _p(opac, C_F32),
+                         _p(rgb, C_F32), _p(act, C_U8), _p(camv, C_F64), _p(cfgv, C_F64), ctypes.c_int(int(brute)),
+                         _p(img, C_F64), None, None, None, None, None, None, _p(med, C_F64), _p(mf, C_U8))
+    return med, mf
+
+
 def covisibility(contrib_a, contrib_b, active=None, threshold=0.5):
     """Eq. 22 (L216-221): |G_A n G_B| / |G_A u G_B| with G_V = {k in M_A : C_k^V > 0.5}.  Returns
     (score, n_intersection, n_union); the score of two empty sets is 0."""

@@ -379,11 +379,30 @@ static inline void atomic_add_fwd(double* p, double v) {
 
 /* contrib (nullable, n doubles, zero-initialised by the caller): the contribution of splat k to the view,
  * C_k^V = sum over pixels of its blending coefficient w_k(p) = a_k T_k (Eq. 20-21). */
+void orc_render_ex2(int64_t n, const float* mean, const float* scale, const float* quat, const float* opacity, const float* rgb,
+                    const uint8_t* active, const double* camv, const double* cfgv, int brute, double* img, double* T_final,
+                    int32_t* n_comp, uint8_t* fragile, int64_t* counters, int32_t* qtb_pix, double* contrib, double* median,
+                    uint8_t* median_fragile);
+
 void orc_render_ex(int64_t n, const float* mean, const float* scale, const float* quat,
                    const float* opacity, const float* rgb, const uint8_t* active,
                    const double* camv, const double* cfgv, int brute,
                    double* img, double* T_final, int32_t* n_comp, uint8_t* fragile, int64_t* counters,
                    int32_t* qtb_pix /* nullable: per-pixel Q_tb */, double* contrib) {
+    orc_render_ex2(n, mean, scale, quat, opacity, rgb, active, camv, cfgv, brute, img, T_final, n_comp, fragile, counters, qtb_pix,
+                   contrib, NULL, NULL);
+}
+
+/* + median depth (DESIGN R9m; a variant of the depth image of L118-120): along the pixel's ray
+ * the blending weights w_i of Eq. 8 and the remaining transmittance T_final form a distribution over the
+ * intersection depths z_i (and "nothing hit"); its median is the z_i of the composited splat at which the
+ * transmittance first falls to T_{i+1} = prod_{j<=i}(1 - a_j) <= 1/2.  0 where T_final > 1/2.  median_fragile: some
+ * composited splat left T within 1e-4 of 1/2 (the GPU's fp32 may pick the neighbouring splat there). */
+void orc_render_ex2(int64_t n, const float* mean, const float* scale, const float* quat,
+                    const float* opacity, const float* rgb, const uint8_t* active,
+                    const double* camv, const double* cfgv, int brute,
+                    double* img, double* T_final, int32_t* n_comp, uint8_t* fragile, int64_t* counters,
+                    int32_t* qtb_pix, double* contrib, double* median, uint8_t* median_fragile) {
     Ctx c; ctx_init(&c, n, mean, scale, quat, opacity, rgb, active, camv, cfgv, brute);
     const int W = c.cam.W, H = c.cam.H; const int64_t HW = (int64_t)W * H;
     int64_t Qt = 0, Qc = 0, Qcover = 0, nfrag = 0, Qtb = 0;
@@ -394,7 +413,8 @@ void orc_render_ex(int64_t n, const float* mean, const float* scale, const float
             const double x = i + 0.5, y = j + 0.5; /* pixel centres at half integers (R17) */
             const uint32_t* lst; const int64_t m = cand_count(&c, i, j, &lst);
             double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, T = 1.0;
-            int frag = 0, stopped = 0, nc = 0;
+            int frag = 0, stopped = 0, nc = 0, medfrag = 0;
+            double med = 0.0;
             int64_t qt_pix = 0, qt_last = 0;
             for (int64_t e = 0; e < m; ++e) {
                 const uint32_t raw = lst ? lst[e] : (uint32_t)e;
@@ -420,6 +440,8 @@ void orc_render_ex(int64_t n, const float* mean, const float* scale, const float
                 acc[4] += w * p->tnc[0]; acc[5] += w * p->tnc[1]; acc[6] += w * p->tnc[2];
                 acc[7] += w;
                 if (contrib) atomic_add_fwd(contrib + k, w); /* Eq. 21 */
+                if (T > 0.5 && T * (1.0 - r.a) <= 0.5) med = r.z; /* the one splat that takes T across 1/2 */
+                if (fabs(T * (1.0 - r.a) - 0.5) < 1e-4) medfrag = 1;
                 T *= (1.0 - r.a);
                 ++nc; ++Qc;
                 qt_last = qt_pix;
@@ -430,6 +452,8 @@ void orc_render_ex(int64_t n, const float* mean, const float* scale, const float
             if (n_comp) n_comp[pix] = nc;
             if (qtb_pix) qtb_pix[pix] = (int32_t)qt_last;
             if (fragile) fragile[pix] = (uint8_t)frag;
+            if (median) median[pix] = med;
+            if (median_fragile) median_fragile[pix] = (uint8_t)medfrag;
             nfrag += (frag & 5) != 0;
             Qt += qt_pix; Qtb += qt_last;
         }

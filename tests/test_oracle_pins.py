@@ -676,3 +676,60 @@ def test_p16_upstream_map_is_the_jacobian_transpose_of_the_division():
     assert got[3, 0, 0] == 0.0 and got[7, 0, 0] == up[7, 0, 0]               # O = 0: only the opacity upstream survives
     for ch in (0, 1, 2, 4, 5, 6):
         assert (got[ch] == up[ch]).all()
+
+
+# ---------------------------------------------------------------- P17: median depth (DESIGN R9m)
+def test_p17_median_depth_hand_stacks():
+    """Fronto-parallel splats on the optical axis, principal pixel (G = 1, a_i = o_i): T runs 1 -> 0.7 -> 0.35 for
+    o = (0.3, 0.5, 0.9), so the median is the SECOND splat's depth; o = (0.6, ..) crosses at the first; o = (0.3, 0.2)
+    never reaches 1/2 (T_final = 0.56) and gives 0.  Listed out of depth order on purpose."""
+    cam = Camera(9, 9, 20.0, 20.0, 4.5, 4.5)
+    camv, cfg = oracle.make_cam(cam), oracle.make_cfg()
+    mk = lambda z, o: one_surfel((0, 0, z), (0.3, 0.3), (1, 0, 0, 0), o)
+    med, _ = oracle.median_depth(cat(mk(3.0, 0.9), mk(1.0, 0.3), mk(2.0, 0.5)), camv, cfg)
+    assert med[4, 4] == 2.0
+    med, _ = oracle.median_depth(cat(mk(2.0, 0.5), mk(1.0, 0.6)), camv, cfg)
+    assert med[4, 4] == 1.0
+    med, _ = oracle.median_depth(cat(mk(2.0, 0.2), mk(1.0, 0.3)), camv, cfg)
+    assert med[4, 4] == 0.0
+
+
+def test_p17_median_depth_against_numpy_on_closed_form_footprints():
+    """Six fronto-parallel splats at distinct depths: per pixel, the closed-form alphas (P1) in depth order, a
+    cumulative product, and the first index with T <= 1/2 -- numpy against the oracle at every pixel that is not within
+    1e-4 of the threshold; brute force and skipping traversal agree; a tilted plane's median is the ray-plane depth."""
+    specs = [((0.10, -0.05, 1.5), 0.25, 0.20, 0.45), ((-0.20, 0.10, 2.0), 0.40, 0.30, 0.60), ((0.0, 0.0, 2.5), 0.50, 0.50, 0.35),
+             ((0.15, 0.12, 1.2), 0.12, 0.15, 0.30), ((-0.1, -0.1, 3.0), 0.9, 0.9, 0.95), ((0.3, -0.2, 1.8), 0.2, 0.25, 0.80)]
+    sc = cat(*[one_surfel(mu, (su, sv), (1, 0, 0, 0), o) for mu, su, sv, o in specs])
+    camv, cfg = oracle.make_cam(CAM), oracle.make_cfg()
+    med, mf = oracle.median_depth(sc, camv, cfg)
+    order = np.argsort([s[0][2] for s in specs])
+    T = np.ones((CAM.height, CAM.width)); want = np.zeros_like(T); near = np.zeros(T.shape, bool)
+    for k in order:
+        mu, su, sv, o = specs[k]
+        a = _footprint_alpha(mu, float(np.float32(su)), float(np.float32(sv)), float(np.float32(o)))
+        Tn = T * (1 - a)
+        cross = (a > 0) & (T > 0.5) & (Tn <= 0.5)
+        want[cross] = float(np.float32(mu[2]))
+        near |= (a > 0) & (np.abs(Tn - 0.5) < 2e-4)
+        T = Tn
+    ok = ~near
+    assert (mf.astype(bool) & ok).sum() == 0 and ok.mean() > 0.99
+    assert (want[ok] > 0).sum() > 500 and len(np.unique(want[ok])) >= 4
+    np.testing.assert_allclose(med[ok], want[ok], rtol=0, atol=1e-12)
+    assert np.array_equal(med, oracle.median_depth(sc, camv, cfg, brute=True)[0])
+    # one opaque tilted splat: the median is that splat's intersection depth = the ray-plane depth (P2's closed form)
+    rot = Rotation.from_euler("xyz", [25, -35, 10], degrees=True)
+    qx, qy, qz, qw = rot.as_quat()
+    s1 = one_surfel((0.1, -0.05, 1.8), (0.3, 0.2), (qw, qx, qy, qz), 0.9)
+    med1, _ = oracle.median_depth(s1, camv, cfg)
+    r1 = oracle.render(s1, camv, cfg)
+    q32 = s1.quat[0].astype(np.float64)
+    nrm = Rotation.from_quat([q32[1], q32[2], q32[3], q32[0]]).as_matrix()[:, 2]
+    X, Y = pix_grid(CAM)
+    d = np.stack([(X - CAM.cx) / CAM.fx, (Y - CAM.cy) / CAM.fy, np.ones_like(X)], axis=-1)
+    z = (nrm @ s1.mean[0].astype(np.float64)) / (d @ nrm)
+    m = r1["img"][7] >= 0.5 + 1e-3
+    assert m.sum() > 50
+    np.testing.assert_allclose(med1[m], z[m], rtol=1e-12)
+    assert (med1[r1["img"][7] < 0.5 - 1e-3] == 0).all()
