@@ -171,6 +171,15 @@ SGS_API int sgs_prepare(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_came
 SGS_API int sgs_render_contrib(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_camera* cam, const sgs_images* out,
                                float* contrib, void* cuda_stream);
 
+/* sgs_render that additionally returns the MEDIAN depth image (reading R9m; a variant of the depth
+ * image of L118-120): along a pixel's ray the blending weights w_i = a_i T_i of Eq. 8 and the remaining transmittance
+ * form a distribution over the intersection depths z_i; median[p] is the z_i of the composited splat at which the
+ * transmittance first falls to T_{i+1} <= 1/2, and 0 where the pixel stays below half opacity.  Forward only: the image is
+ * piecewise constant in the opacities and carries no gradient; sgs_backward after this call is that of sgs_render.
+ *   median: DEVICE, H x W floats, overwritten.  Other arguments, status codes and stream order as sgs_render. */
+SGS_API int sgs_render_median(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_camera* cam, const sgs_images* out,
+                              float* median, void* cuda_stream);
+
 /* Covisibility score of two views (Eq. 22): |G_A n G_B| / |G_A u G_B| with
  * G_V = {k : active[k] != 0 and C_k^V > threshold} (paper: threshold 0.5).
  *   contrib_a, contrib_b: DEVICE, n floats (outputs of sgs_render_contrib);  active: DEVICE n bytes or NULL

@@ -54,7 +54,7 @@ class sgs_stats(C.Structure):
 
 
 EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_prepare", "sgs_backward", "sgs_wait_grads", "sgs_tracking_loss",
-           "sgs_backward_tracking", "sgs_track_iter", "sgs_track_new_frame", "sgs_render_contrib", "sgs_covisibility", "sgs_mapping_loss", "sgs_ssim_loss", "sgs_map_correction", "sgs_measure_fp32_peak", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
+           "sgs_backward_tracking", "sgs_track_iter", "sgs_track_new_frame", "sgs_render_contrib", "sgs_render_median", "sgs_covisibility", "sgs_mapping_loss", "sgs_ssim_loss", "sgs_map_correction", "sgs_measure_fp32_peak", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
            "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string"]
 
 _lib = None
@@ -214,6 +214,12 @@ class Renderer:
         """sgs_prepare: preprocess + tile binning only; the next render() of the same (surfels, cam) objects on this
         Renderer skips its binning and orders itself behind this call (the streams may differ)."""
         _check(self.lib.sgs_prepare(self._ctx, C.byref(surfels), C.byref(cam), _stream_ptr(stream)), "sgs_prepare")
+
+    def render_median(self, surfels, cam, median, rgb=None, depth=None, normal=None, alpha=None, stream=None):
+        """sgs_render_median: render + median depth image (R9m) into `median` (H x W floats, device)."""
+        out = _images(rgb, depth, normal, alpha)
+        _check(self.lib.sgs_render_median(self._ctx, C.byref(surfels), C.byref(cam), C.byref(out), _ptr(median),
+                                          _stream_ptr(stream)), "sgs_render_median")
 
     def render_contrib(self, surfels, cam, contrib, rgb=None, depth=None, normal=None, alpha=None, stream=None):
         """sgs_render_contrib: render + per-splat contribution C_k^V (Eq. 20-21) into `contrib` (n floats, device)."""

@@ -230,6 +230,15 @@ int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const s
     return SGS_OK;
 }
 
+int sgs_render_median(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* out, float* median,
+                      void* stream) {
+    if (!c || !sf || !median) return SGS_INVALID_ARGUMENT;
+    c->median_out = median;
+    const int r = sgs_render(c, sf, cam, out, stream);
+    c->median_out = nullptr;
+    return r;
+}
+
 int sgs_render_contrib(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* out, float* contrib,
                        void* stream) {
     if (!c || !sf || !contrib) return SGS_INVALID_ARGUMENT;

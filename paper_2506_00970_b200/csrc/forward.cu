@@ -13,12 +13,12 @@ namespace {
 
 struct Planes { float* p[8]; };
 
-template <bool CONTRIB, bool NDEPTH>
+template <bool CONTRIB, bool NDEPTH, bool MEDIAN>
 __global__ void __launch_bounds__(SGS_BLOCK, 4)  // 64 registers, four blocks per SM: the D_n variant would take 72 and lose one (measured: with a bound of 1 block the default variant takes 89 registers and C4's forward goes from 246 to 289 us)
 k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
           int tiles_x, SgsCfgDev cfg, Planes out, float* __restrict__ T_final, uint32_t* __restrict__ n_last,
           const uint32_t* __restrict__ cursor, unsigned long long* bucket, uint32_t tile_cap,
-          float* __restrict__ contrib, float2* __restrict__ dn_state) {
+          float* __restrict__ contrib, float2* __restrict__ dn_state, float* __restrict__ median_out) {
     // staged batch, structure of float4 arrays (one base register, immediate offsets, broadcast reads)
     __shared__ float4 sh[5][SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
@@ -73,6 +73,7 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
     }
 
     float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dp = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f, O = 0.f;
+    float med = 0.f;    // MEDIAN (R9m): depth of the splat that takes T across 1/2
     uint32_t last = 0;  // entries [0, last) of the tile list contain every composited pair of this pixel
     bool done = !inside;
 
@@ -133,6 +134,7 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
                     const unsigned ws = __reduce_add_sync(0xffffffffu, (unsigned)__float2uint_rn(w * 16777216.f));
                     if (lane == 0 && ws != 0u) atomicAdd(contrib + __float_as_uint(s4.w), (float)ws * (1.f / 16777216.f));
                 }
+                if (MEDIAN) med = (pass && T > 0.5f && Tn <= 0.5f) ? z : med;
                 T = pass ? Tn : T;
                 last = pass ? base - start + j + 1 : last;
             }
@@ -153,6 +155,7 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
         if (out.p[5]) out.p[5][pix] = N1;
         if (out.p[6]) out.p[6][pix] = N2;
         if (out.p[7]) out.p[7][pix] = O;
+        if (MEDIAN) median_out[pix] = med;
         T_final[pix] = T;
         n_last[pix] = last;
     }
@@ -169,14 +172,17 @@ cudaError_t sgs_launch_forward(sgs_ctx* c, float* const planes[8], cudaStream_t 
 #define SGS_FWD_ARGS c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, c->camd.W, \
                      c->camd.H, c->camd.tiles_x, c->cfgd, out, c->T_final, c->n_last, c->fused_sort ? c->cursor : nullptr,     \
                      reinterpret_cast<unsigned long long*>(c->bucket), (uint32_t)c->tile_cap, c->contrib_out, \
-                     (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) ? c->dn_state : nullptr
+                     (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) ? c->dn_state : nullptr, c->median_out
     const bool nd = (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) != 0;
-    if (c->contrib_out) {
-        if (nd) k_forward<true, true><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
-        else k_forward<true, false><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+    if (c->median_out) {  // (sgs_render_median; never together with the contribution output)
+        if (nd) k_forward<false, true, true><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+        else k_forward<false, false, true><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+    } else if (c->contrib_out) {
+        if (nd) k_forward<true, true, false><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+        else k_forward<true, false, false><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
     } else {
-        if (nd) k_forward<false, true><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
-        else k_forward<false, false><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+        if (nd) k_forward<false, true, false><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+        else k_forward<false, false, false><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
     }
 #undef SGS_FWD_ARGS
     return cudaGetLastError();

@@ -107,6 +107,7 @@ struct sgs_ctx {
     float* ssim_maps; int64_t ssim_cap;  // 9 derivative planes of sgs_ssim_loss
     float* pose_inc; int inc_cap;    // per-keyframe increments of sgs_map_correction (16 floats each)
     unsigned int* covis_cnt;         // 4 counters of k_covisibility (cudaMalloc, lazily)
+    float* median_out;               // sgs_render_median: median depth plane of the current forward, else nullptr
     float* contrib_out;              // sgs_render_contrib: per-splat contribution output of the current forward, or NULL
     int64_t cursor_cap;              // tiles the cursor / tile_order arrays hold
     int64_t tile_cap, bucket_cap;    // entries per tile; allocated keys
