@@ -60,11 +60,18 @@ enum {
 };
 
 enum {
-    SGS_FLAG_ASYNC = 1,         /* never synchronise the host in sgs_render (CUDA-graph capturable) */
+    SGS_FLAG_ASYNC = 1,         /* never synchronise the host in sgs_render; an overflow is reported by a later call */
     SGS_FLAG_RADIX_BINNING = 2, /* bin with the global LSD radix sort of the 64-bit keys instead of the
                                    default per-tile buckets + in-tile sort; same list, kept for A/B checks */
     SGS_FLAG_TRACK_REUSE = 4,   /* sgs_track_iter: the map is frozen between sgs_track_new_frame calls, see there */
     SGS_FLAG_LAZY_GRADS = 8,    /* sgs_backward: d_surfels / d_pose6 are complete only behind sgs_wait_grads, see there */
+    SGS_FLAG_GRAPH = 32,        /* SGS_FLAG_ASYNC for stream capture: sgs_render, sgs_render_contrib / _median, sgs_backward,
+                                   sgs_backward_tracking, sgs_track_iter and the loss calls enqueue kernels and copies on the
+                                   caller's stream ONLY (the context has no stream of its own, queries and waits for no
+                                   event), so the sequence can be recorded into a CUDA graph once an eager run has brought the
+                                   workspace to size (a call that had to grow it would allocate: do not capture the first).
+                                   Nothing reports a bucket overflow by itself in this mode: sgs_get_stats (which
+                                   synchronises the device) does.  sgs_prepare is SGS_INVALID_ARGUMENT. */
     SGS_FLAG_NORMALISED_DEPTH = 16 /* SURVEY 8(f) NEXT-3 (variant of R9; Eq. 8 L116-120 renders D = sum w z and
                                    O = sum w): the depth image is the expected depth D_n = D / O (0 where O = 0), i.e.
                                    the blend weights renormalised to sum to one, so a partly transparent surface keeps

@@ -221,7 +221,8 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
               cudaEventCreateWithFlags(&c->order_fork, cudaEventDisableTiming) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->order_done, cudaEventDisableTiming) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->join_ev, cudaEventDisableTiming) == cudaSuccess &&
-              cudaStreamCreateWithPriority(&c->aux_stream, cudaStreamNonBlocking, prio_hi) == cudaSuccess;
+              ((cfg->flags & SGS_FLAG_GRAPH) != 0 ||  // capture mode: everything stays on the caller's stream
+               cudaStreamCreateWithPriority(&c->aux_stream, cudaStreamNonBlocking, prio_hi) == cudaSuccess);
     if (!ok) { cudaGetLastError(); sgs_destroy(c); return SGS_CUDA_ERROR; }
     c->pose6_dev = c->loss_dev + 1;
     cudaMemset(c->counters, 0, sizeof(SgsCounters));

@@ -4,12 +4,15 @@
 #include "sgs_internal.h"
 
 static inline bool radix_mode(const sgs_ctx* c) { return (c->cfg.flags & SGS_FLAG_RADIX_BINNING) != 0; }
+// SGS_FLAG_GRAPH: no event is queried, waited for or shared with another stream and the ctx has no stream of its own, so a
+// stream capture sees kernels and copies only; the counters still reach pinned memory, nobody polls them
+static inline bool graph_mode(const sgs_ctx* c) { return (c->cfg.flags & SGS_FLAG_GRAPH) != 0; }
 
 static int64_t grown_tile_cap(int64_t max_tile) { return max_tile + max_tile / 2 + 64; }
 
 // async mode: examine the counters of the previous render (already copied to pinned memory)
 static int check_pending(sgs_ctx* c, cudaStream_t s) {
-    if (!c->pending_check) return SGS_OK;
+    if (!c->pending_check || graph_mode(c)) return SGS_OK;
     if (c->pending_lazy) {
         // sgs_track_iter copies the counters after its fused kernel: waiting here would serialise host and device,
         // so an overflow of iteration i is reported by the first call that finds the copy complete
@@ -71,7 +74,7 @@ static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, bool want_
         }
         c->last_entries = (int64_t)c->counters_host->n_entries;
         c->last_surv = (int64_t)c->counters_host->n_surv;
-    } else if (!defer) {
+    } else if (!defer && !graph_mode(c)) {
         cudaEventRecord(c->counters_ready, cs);
         c->copy_in_flight = cs != s;
         c->pending_check = true;
@@ -115,7 +118,7 @@ static int bin_radix(sgs_ctx* c, const sgs_surfels* sf, bool async, cudaStream_t
             if (cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
         }
         c->launch_entries = E;  // exact grids
-    } else {
+    } else if (!graph_mode(c)) {
         cudaEventRecord(c->counters_ready, s);
         c->pending_check = true;
         c->pending_lazy = false;
@@ -145,7 +148,7 @@ static int bin_view(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, bo
     const int64_t pixels = (int64_t)cam->width * cam->height;
     if ((r = sgs_ensure_surfels(c, sf->n, s)) != SGS_OK) return r;
     if ((r = sgs_ensure_image(c, tiles, pixels, s)) != SGS_OK) return r;
-    const bool async = (c->cfg.flags & SGS_FLAG_ASYNC) != 0;
+    const bool async = (c->cfg.flags & (SGS_FLAG_ASYNC | SGS_FLAG_GRAPH)) != 0;
     c->last_surfels = *sf;
     c->last_cam = *cam;
     return radix_mode(c) ? bin_radix(c, sf, async, s) : bin_buckets(c, sf, async, want_order, s);
@@ -191,7 +194,7 @@ static bool same_view(const sgs_ctx* c, const sgs_surfels* sf, const sgs_camera*
 }
 
 int sgs_prepare(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, void* stream) {
-    if (!c) return SGS_INVALID_ARGUMENT;
+    if (!c || graph_mode(c)) return SGS_INVALID_ARGUMENT;  // (two streams and an event between them: not for a capture)
     cudaStream_t s = (cudaStream_t)stream;
     c->prepared = false;
     // the binning buffers are still read by the ctx's last render / backward, possibly on another stream
@@ -226,7 +229,7 @@ int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const s
     if (sgs_launch_forward(c, planes, s) != cudaSuccess) return SGS_CUDA_ERROR;
     c->have_forward = true;
     c->have_binning = true;
-    c->work_recorded = cudaEventRecord(c->work_ev, s) == cudaSuccess;
+    c->work_recorded = !graph_mode(c) && cudaEventRecord(c->work_ev, s) == cudaSuccess;
     return SGS_OK;
 }
 
@@ -305,6 +308,7 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
             return SGS_CUDA_ERROR;
         if (cudaMemcpyAsync(c->counters_host, c->counters_snap + c->snap_slot, sizeof(SgsCounters), cudaMemcpyDeviceToHost, cs) != cudaSuccess)
             return SGS_CUDA_ERROR;
+        if (graph_mode(c)) { c->have_binning = true; return SGS_OK; }  // (one slot, one stream: nothing to order, nobody polls)
         const cudaEvent_t t = c->counters_ready_prev; c->counters_ready_prev = c->counters_ready; c->counters_ready = t;
         c->prev_copy_on_aux = c->snap_copy_on_aux;
         cudaEventRecord(c->counters_ready, cs);
@@ -343,7 +347,7 @@ int sgs_backward(sgs_ctx* c, const sgs_images* upstream, const sgs_surfel_grads*
     }
     c->grads_on_aux = false;
     if (sgs_launch_backward(c, up, dg, d_pose6, s) != cudaSuccess) return SGS_CUDA_ERROR;
-    c->work_recorded = cudaEventRecord(c->work_ev, c->grads_on_aux ? c->aux_stream : s) == cudaSuccess;
+    c->work_recorded = !graph_mode(c) && cudaEventRecord(c->work_ev, c->grads_on_aux ? c->aux_stream : s) == cudaSuccess;
     return SGS_OK;
 }
 
@@ -455,7 +459,8 @@ int sgs_get_binning(sgs_ctx* c, int64_t* n_entries, const uint64_t** keys, const
 
 int sgs_get_stats(sgs_ctx* c, sgs_stats* out) {
     if (!c || !out) return SGS_INVALID_ARGUMENT;
-    if (c->pending_check && cudaEventSynchronize(c->counters_ready) != cudaSuccess) return SGS_CUDA_ERROR;
+    if (graph_mode(c)) { if (cudaDeviceSynchronize() != cudaSuccess) return SGS_CUDA_ERROR; }
+    else if (c->pending_check && cudaEventSynchronize(c->counters_ready) != cudaSuccess) return SGS_CUDA_ERROR;
     out->n_visible = c->counters_host->n_visible;
     out->n_entries = (int64_t)c->counters_host->n_entries;
     out->capacity = radix_mode(c) ? c->e_cap : c->tile_cap;

@@ -1,0 +1,70 @@
+"""SGS_FLAG_GRAPH makes the calls capturable: sgs_render + sgs_backward (full, with the pose) and sgs_track_iter recorded
+into a CUDA graph once the workspace has its size, replayed, give the results of the eager calls -- also after the
+inputs (map colours, target) were changed in place between replays."""
+import numpy as np
+import pytest
+import torch
+
+import scenegen
+
+pytestmark = pytest.mark.gpu
+
+sgs = pytest.importorskip("paper_2506_00970_b200")
+from gpu_common import to_device, camera, alloc_images, planes, alloc_grads, split_upstream  # noqa: E402
+
+
+def test_render_backward_and_track_iter_in_a_cuda_graph():
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    up = split_upstream(scenegen.upstream_normal(4, cam.height, cam.width))
+    t, sf = to_device(sc)
+    c = camera(cam)
+    r = sgs.Renderer(graph=True)
+    im, g, p6 = alloc_images(cam), alloc_grads(sc.n), torch.zeros(6, device="cuda")
+    p6t, lt = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+    tgt_rgb, tgt_dep = torch.rand(3, cam.height, cam.width, device="cuda"), torch.rand(1, cam.height, cam.width, device="cuda") + 1.0
+
+    def step():
+        r.render(sf, c, **im)
+        r.backward(**up, grads=g, d_pose6=p6)
+        r.track_iter(sf, c, tgt_rgb, tgt_dep, 0.5, 1.0, p6t, lt)
+
+    def snapshot():
+        torch.cuda.synchronize()
+        return (planes(im), {k: v.cpu().numpy() for k, v in g.items()}, p6.cpu().numpy(), p6t.cpu().numpy(), lt.cpu().numpy())
+
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        for _ in range(3):      # workspace reaches its size; nothing is allocated during capture
+            step()
+    torch.cuda.current_stream().wait_stream(s)
+    eager = snapshot()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=s):
+        step()
+    for round_ in range(2):
+        for v in list(im.values()) + list(g.values()) + [p6, p6t, lt]:
+            v.fill_(-3.0)
+        graph.replay()
+        got = snapshot()
+        assert np.array_equal(got[0], eager[0])
+        for k in got[1]:
+            np.testing.assert_allclose(got[1][k], eager[1][k], rtol=2e-4, atol=1e-5 * np.abs(eager[1][k]).max())
+        np.testing.assert_allclose(got[2], eager[2], rtol=1e-4, atol=1e-5 * np.abs(eager[2]).max())
+        np.testing.assert_allclose(got[3], eager[3], rtol=1e-4, atol=1e-6 * np.abs(eager[3]).max())
+        np.testing.assert_allclose(got[4], eager[4], rtol=1e-5)
+        if round_ == 0:         # new inputs in the same buffers: the replay must follow them
+            t["rgb"].mul_(0.5)
+            tgt_rgb.mul_(0.7)
+            with torch.cuda.stream(s):
+                step()
+            torch.cuda.current_stream().wait_stream(s)
+            eager2 = snapshot()
+            assert not np.array_equal(eager2[0], eager[0])
+            eager = eager2
+    st = r.stats()
+    assert st["overflow"] == 0 and st["n_entries"] > 0
+    with pytest.raises(sgs.SgsError):
+        r.prepare(sf, c)
+    r.close()
