@@ -123,8 +123,9 @@ def aggregate_replicas(ms_local, pixels, renders_per_rank, world, dist=None, dev
 class Workload:
     """Device-resident inputs + the step function for one config."""
 
-    def __init__(self, name, iters_override=None, contrib=False, prefetch=True, reuse=True, normalised_depth=False):
+    def __init__(self, name, iters_override=None, contrib=False, prefetch=True, reuse=True, normalised_depth=False, graph=False):
         self.contrib = contrib
+        self.graph, self.cg, self.eager_steps = graph, None, 0
         nd = self.normalised_depth = normalised_depth
         import torch
         import scenegen
@@ -138,7 +139,7 @@ class Workload:
         self.t = dict(mean=d(sc.mean), scale=d(sc.scale), quat=d(sc.quat), opacity=d(sc.opacity), rgb=d(sc.rgb),
                       active=d(sc.active, torch.uint8))
         self.sf = sgs.Renderer.surfels(*(self.t[k] for k in ("mean", "scale", "quat", "opacity", "rgb", "active")))
-        self.ren = sgs.Renderer(async_mode=True, track_reuse=self.tracking and reuse, normalised_depth=nd)
+        self.ren = sgs.Renderer(async_mode=not graph, graph=graph, track_reuse=self.tracking and reuse, normalised_depth=nd)
         # mapping window: a second context + a side stream, so that sgs_prepare (binning) of view v+1 runs under the
         # compositing kernels of view v (include/sgs.h); tracking iterations depend on one another and use one context
         two = prefetch and not self.tracking and len(self.cams) > 1
@@ -213,10 +214,21 @@ class Workload:
                          grads=self.grads_of[id(ren)], d_pose6=self.p6_of[id(ren)])
 
     def step(self):
-        if self.tracking:
-            self.ren.track_new_frame()   # a step is the tracking of one frame: the survivor list is built once per step
-            for _ in range(self.iters):
-                self.one(0)
+        if self.tracking and self.graph and self.cg is not None:
+            self.cg.replay()             # --graph: the whole frame (list build + iterations) is one CUDA graph launch
+        elif self.tracking:
+            def frame():
+                self.ren.track_new_frame()   # a step is the tracking of one frame: the survivor list is built once per step
+                for _ in range(self.iters):
+                    self.one(0)
+            if self.graph and self.eager_steps >= 2:   # workspace at size after two eager frames: record the third
+                self.cg = self.torch.cuda.CUDAGraph()
+                with self.torch.cuda.graph(self.cg):
+                    frame()
+                self.cg.replay()
+            else:
+                frame()
+                self.eager_steps += 1
         elif len(self.rens) == 1:
             for v in range(len(self.cams)):
                 self.one(v)
@@ -343,6 +355,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-reuse", action="store_true", help="tracking configs: run the pre-cull over the whole map every iteration")
     ap.add_argument("--no-prefetch", action="store_true", help="mapping configs: one context, binning of each view in line")
+    ap.add_argument("--graph", action="store_true", help="tracking configs: SGS_FLAG_GRAPH, each step (frame) replayed as one CUDA graph")
     ap.add_argument("--normalised-depth", action="store_true", help="SGS_FLAG_NORMALISED_DEPTH: depth image D/O (tracking takes the unfused sequence)")
     ap.add_argument("--contrib", action="store_true", help="mapping configs: render with sgs_render_contrib (C_k output on)")
     args = ap.parse_args()
@@ -363,10 +376,13 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    wl = Workload(args.config, args.iters, args.contrib, not args.no_prefetch, not args.no_reuse, args.normalised_depth)
+    wl = Workload(args.config, args.iters, args.contrib, not args.no_prefetch, not args.no_reuse, args.normalised_depth, args.graph)
     K, W = args.steps, max(args.warmup, 3)
+    per_step = []
     for _ in range(W):
+        l0 = sum(r.stats()["kernel_launches"] for r in wl.rens)
         wl.step()
+        per_step.append(sum(r.stats()["kernel_launches"] for r in wl.rens) - l0)
     torch.cuda.synchronize()
     launches0 = sum(r.stats()["kernel_launches"] for r in wl.rens)
 
@@ -386,6 +402,8 @@ def main():
     time.sleep(0.3)
     ms = timed_pass()
     launches = sum(r.stats()["kernel_launches"] for r in wl.rens) - launches0   # of the timed region only
+    if args.graph and wl.cg is not None:   # replays do not pass the library's launch counter: the recorded step's count x K
+        launches = per_step[2] * K
     # the timed region can be shorter than nvidia-smi's start-up: keep the same load running (untimed) until the sampler
     # has seen it a few times, so that `clocks` is always a reading under this workload
     t_wait = time.time()
@@ -398,6 +416,7 @@ def main():
     renders = wl.renders_per_step * K * world
 
     # second pass with per-stage CUDA events (roofline), not part of `value`
+    wl.graph = False   # (--graph: the stage events live in the eager calls)
     for r in wl.rens:
         r.set_profiling(True)
         r.get_profile(reset=True)
@@ -484,6 +503,8 @@ def main():
                                      if len(wl.rens) > 1 else "in line (sgs_render / sgs_track_iter)")),
                 clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roof, stages=stages, cpu_baseline=cpu,
                 stage_us={k: round(1e3 * v[0] / v[1], 2) for k, v in prof.items() if v[1]})
+    if args.graph:
+        line["config"]["launch"] = "one CUDA graph per step (SGS_FLAG_GRAPH); not the default workload"
     if args.normalised_depth:
         line["config"]["depth"] = "normalised D/O (SGS_FLAG_NORMALISED_DEPTH); not the default workload"
     print(json.dumps(line))
