@@ -59,7 +59,8 @@ static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, bool want_
     // async mode: the 32-byte copy runs on the ctx's own stream so that it is not a link of the caller's chain
     // (K-pre-B -> copy -> compositing); the next preprocess on this ctx waits for it before it clears the counters
     cudaStream_t cs = (async && c->aux_stream) ? c->aux_stream : s;
-    if (!defer) {
+    c->stats_src = c->counters;
+    if (!defer && !graph_mode(c)) {  // (capture mode: nobody polls; sgs_get_stats fetches them itself)
         if (cs != s && (cudaEventRecord(c->fork_ev, s) != cudaSuccess || cudaStreamWaitEvent(cs, c->fork_ev, 0) != cudaSuccess))
             return SGS_CUDA_ERROR;
         if ((r = copy_counters(c, cs)) != SGS_OK) return r;
@@ -105,7 +106,8 @@ static int bin_radix(sgs_ctx* c, const sgs_surfels* sf, bool async, cudaStream_t
         if (hint < c->launch_entries) c->launch_entries = hint;
     }
     if (sgs_launch_preprocess(c, sf, s) != cudaSuccess) return SGS_CUDA_ERROR;
-    if ((r = copy_counters(c, s)) != SGS_OK) return r;
+    c->stats_src = c->counters;
+    if (!graph_mode(c) && (r = copy_counters(c, s)) != SGS_OK) return r;
     if (!async) {
         if (cudaStreamSynchronize(s) != cudaSuccess) return SGS_CUDA_ERROR;
         const int64_t E = (int64_t)c->counters_host->n_entries;
@@ -283,6 +285,9 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
             c->surv_valid = false;  // another map, or the pose has left the list's margin: build it again, centred here
         c->use_surv_cache = true;
     }
+    // capture mode with a kept list: the longest-first tile order is renewed by the first iteration of a frame only (it sits on
+    // the iteration's chain there: no side stream); the order is a scheduling hint, results do not depend on it
+    c->order_skip = graph_mode(c) && (c->cfg.flags & SGS_FLAG_TRACK_REUSE) && c->surv_valid;
     c->defer_counters = true;  // (bin_buckets clears it when it cannot honour it)
     int r = bin_view(c, sf, cam, false, s);
     c->use_surv_cache = false;
@@ -303,12 +308,13 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
         // ... copied on the ctx's own stream: a copy between K-track and the next iteration's K-pre-B is a link of the
         // iteration's dependency chain (measured on C2: 82.3 -> 72.2 us per iteration).  Two snapshot slots alternate, and
         // an iteration waits for the copy of the slot it is about to overwrite, which is one iteration old.
+        c->stats_src = c->counters_snap + c->snap_slot;
+        if (graph_mode(c)) { c->have_binning = true; return SGS_OK; }  // (one slot, one stream; no copy on the iteration's chain)
         cudaStream_t cs = c->aux_stream ? c->aux_stream : s;
         if (cs != s && (cudaEventRecord(c->fork_ev, s) != cudaSuccess || cudaStreamWaitEvent(cs, c->fork_ev, 0) != cudaSuccess))
             return SGS_CUDA_ERROR;
         if (cudaMemcpyAsync(c->counters_host, c->counters_snap + c->snap_slot, sizeof(SgsCounters), cudaMemcpyDeviceToHost, cs) != cudaSuccess)
             return SGS_CUDA_ERROR;
-        if (graph_mode(c)) { c->have_binning = true; return SGS_OK; }  // (one slot, one stream: nothing to order, nobody polls)
         const cudaEvent_t t = c->counters_ready_prev; c->counters_ready_prev = c->counters_ready; c->counters_ready = t;
         c->prev_copy_on_aux = c->snap_copy_on_aux;
         cudaEventRecord(c->counters_ready, cs);
@@ -459,7 +465,10 @@ int sgs_get_binning(sgs_ctx* c, int64_t* n_entries, const uint64_t** keys, const
 
 int sgs_get_stats(sgs_ctx* c, sgs_stats* out) {
     if (!c || !out) return SGS_INVALID_ARGUMENT;
-    if (graph_mode(c)) { if (cudaDeviceSynchronize() != cudaSuccess) return SGS_CUDA_ERROR; }
+    if (graph_mode(c)) {
+        if (cudaDeviceSynchronize() != cudaSuccess) return SGS_CUDA_ERROR;
+        if (c->stats_src && cudaMemcpy(c->counters_host, c->stats_src, sizeof(SgsCounters), cudaMemcpyDeviceToHost) != cudaSuccess) return SGS_CUDA_ERROR;
+    }
     else if (c->pending_check && cudaEventSynchronize(c->counters_ready) != cudaSuccess) return SGS_CUDA_ERROR;
     out->n_visible = c->counters_host->n_visible;
     out->n_entries = (int64_t)c->counters_host->n_entries;

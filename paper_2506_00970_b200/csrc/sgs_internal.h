@@ -169,6 +169,8 @@ struct sgs_ctx {
     // K-track helpers (track.cu): per helper 6 x 256 floats of per-pixel state and a flag word, the launch counter they compare with
     float* split_state; unsigned int* split_flag; unsigned int track_launch_id;
     cudaEvent_t order_fork, order_done; bool order_pending;  // k_track_order on aux_stream
+    bool order_skip;                 // SGS_FLAG_GRAPH + SGS_FLAG_TRACK_REUSE: the tile order is renewed once per frame only
+    const SgsCounters* stats_src;    // SGS_FLAG_GRAPH: where the last binning's counters sit on the device (sgs_get_stats copies them)
     int64_t host_img_cap, host_grads_cap;
     int64_t partial_cap;             // floats in pose_partial
     int64_t launches;                // kernels launched by this ctx

@@ -563,7 +563,7 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
         else k_track<false, false><<<tiles + n_help, SGS_BLOCK, 0, s>>>(SGS_TRK_ARGS);
     }
 #undef SGS_TRK_ARGS
-    {   // next iteration's tile order from this launch's measured tile costs, beside the next K-pre-B
+    if (!c->order_skip) {   // next iteration's tile order from this launch's measured tile costs, beside the next K-pre-B
         cudaStream_t os = c->aux_stream ? c->aux_stream : s;
         if (os != s && (cudaEventRecord(c->order_fork, s) != cudaSuccess || cudaStreamWaitEvent(os, c->order_fork, 0) != cudaSuccess))
             return cudaErrorUnknown;
