@@ -142,7 +142,7 @@ class Workload:
         self.ren = sgs.Renderer(async_mode=not graph, graph=graph, track_reuse=self.tracking and reuse, normalised_depth=nd)
         # mapping window: a second context + a side stream, so that sgs_prepare (binning) of view v+1 runs under the
         # compositing kernels of view v (include/sgs.h); tracking iterations depend on one another and use one context
-        two = prefetch and not self.tracking and len(self.cams) > 1
+        two = prefetch and not self.tracking and len(self.cams) > 1 and not graph   # (capture mode: one context, one stream)
         if two:  # + SGS_FLAG_LAZY_GRADS: a view's per-surfel kernel runs under the next view's forward; joined at the step's end
             self.ren.close()
             self.ren = sgs.Renderer(async_mode=True, lazy_grads=True, normalised_depth=nd)
@@ -214,10 +214,14 @@ class Workload:
                          grads=self.grads_of[id(ren)], d_pose6=self.p6_of[id(ren)])
 
     def step(self):
-        if self.tracking and self.graph and self.cg is not None:
-            self.cg.replay()             # --graph: the whole frame (list build + iterations) is one CUDA graph launch
-        elif self.tracking:
+        if self.graph and self.cg is not None:
+            self.cg.replay()             # --graph: the whole step (frame / window of views) is one CUDA graph launch
+        elif self.tracking or self.graph:
             def frame():
+                if not self.tracking:
+                    for v in range(len(self.cams)):
+                        self.one(v)
+                    return
                 self.ren.track_new_frame()   # a step is the tracking of one frame: the survivor list is built once per step
                 for _ in range(self.iters):
                     self.one(0)
@@ -355,7 +359,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-reuse", action="store_true", help="tracking configs: run the pre-cull over the whole map every iteration")
     ap.add_argument("--no-prefetch", action="store_true", help="mapping configs: one context, binning of each view in line")
-    ap.add_argument("--graph", action="store_true", help="tracking configs: SGS_FLAG_GRAPH, each step (frame) replayed as one CUDA graph")
+    ap.add_argument("--graph", action="store_true", help="SGS_FLAG_GRAPH: each step (a tracking frame, or a mapping window on one context) replayed as one CUDA graph")
     ap.add_argument("--normalised-depth", action="store_true", help="SGS_FLAG_NORMALISED_DEPTH: depth image D/O (tracking takes the unfused sequence)")
     ap.add_argument("--contrib", action="store_true", help="mapping configs: render with sgs_render_contrib (C_k output on)")
     args = ap.parse_args()
