@@ -68,3 +68,45 @@ def test_render_backward_and_track_iter_in_a_cuda_graph():
     with pytest.raises(sgs.SgsError):
         r.prepare(sf, c)
     r.close()
+
+
+def test_mapping_iteration_in_a_cuda_graph():
+    """render -> Eq. 23-26 mapping loss -> SSIM term -> full backward, recorded once and replayed, equals the eager calls."""
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    t, sf = to_device(sc)
+    c = camera(cam)
+    r = sgs.Renderer(graph=True)
+    im, upi, g, p6 = alloc_images(cam), alloc_images(cam), alloc_grads(sc.n), torch.zeros(6, device="cuda")
+    loss = torch.zeros(1, device="cuda")
+    trgb = torch.rand(3, cam.height, cam.width, device="cuda")
+    tdep = torch.rand(1, cam.height, cam.width, device="cuda") + 1.5
+
+    def step():
+        loss.zero_()
+        r.render(sf, c, **im)
+        r.mapping_loss(c, im, trgb, tdep, 0.875, 0.5, 0.02, -1.0, upi, loss)
+        r.ssim_loss(im["rgb"], trgb, 0.125, upi["rgb"], loss)
+        r.backward(d_rgb=upi["rgb"], d_depth=upi["depth"], d_normal=upi["normal"], d_alpha=upi["alpha"], grads=g, d_pose6=p6)
+
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        for _ in range(3):
+            step()
+    torch.cuda.current_stream().wait_stream(s)
+    torch.cuda.synchronize()
+    eager = ({k: v.cpu().numpy() for k, v in g.items()}, p6.cpu().numpy(), float(loss.item()), planes(upi))
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=s):
+        step()
+    for v in list(g.values()) + list(upi.values()) + [p6, loss]:
+        v.fill_(-3.0)
+    graph.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(planes(upi), eager[3]) and eager[2] > 0
+    assert abs(float(loss.item()) - eager[2]) <= 1e-5 * eager[2]
+    for k in g:
+        np.testing.assert_allclose(g[k].cpu().numpy(), eager[0][k], rtol=2e-4, atol=1e-5 * np.abs(eager[0][k]).max())
+    np.testing.assert_allclose(p6.cpu().numpy(), eager[1], rtol=1e-4, atol=1e-5 * np.abs(eager[1]).max())
+    r.close()
