@@ -179,6 +179,42 @@ def backward(sc, camv, cfgv, upstream, brute=False, debug=False):
     return g
 
 
+def pixel_bounds(sc, camv, cfgv):
+    """Comparison support (not part of the rendered function): per-pixel bounds for pixels where a binary32 renderer may
+    legitimately differ from this oracle -- see orc_pixel_bounds in sgs_oracle.c.  Returns dict of (H,W) fp64 arrays:
+    flip_w (blending weight at stake in the pixel's fragile decisions), kerr / kerr_z (first-order sensitivity of the
+    blend / of the depth values to the relative rounding of the intersection's inputs), zmax."""
+    mean, scale, quat, opac, rgb, act = _scene_arrays(sc)
+    W, H = int(camv[0]), int(camv[1])
+    out = {k: np.zeros((H, W)) for k in ("flip_w", "kerr", "kerr_z", "zmax")}
+    lib().orc_pixel_bounds(ctypes.c_int64(sc.n), _p(mean, C_F32), _p(scale, C_F32), _p(quat, C_F32), _p(opac, C_F32),
+                           _p(rgb, C_F32), _p(act, C_U8), _p(camv, C_F64), _p(cfgv, C_F64), _p(out["flip_w"], C_F64),
+                           _p(out["kerr"], C_F64), _p(out["kerr_z"], C_F64), _p(out["zmax"], C_F64))
+    return out
+
+
+def exposure(sc, camv, cfgv, upstream, extra_mask=None, signed_all=False, round_eps=8.0 * 2.0 ** -23):
+    """Comparison support: what a renderer that decides differently at the EXPOSED pixels (the oracle's fragile pixels,
+    plus `extra_mask`) can change in every gradient element: sum over those pixels of |contribution with the pixel's
+    fragile decisions inverted - the oracle's contribution| + phi |contribution| (phi: rounding of ill-conditioned
+    intersections, round_eps kappa (1 + rho^2)) + the whole |contribution| on `extra_mask` pixels (orc_exposure in
+    sgs_oracle.c).  Returns dict: mean (n,3), scale (n,2), quat (n,4), opacity (n,), rgb (n,3), pose (6,), pix_exposed
+    (H,W) u8.  signed_all=True: signed contributions of the oracle's own list over all pixels instead, i.e. backward()
+    recomputed pair by pair (the self-check of this function)."""
+    mean, scale, quat, opac, rgb, act = _scene_arrays(sc)
+    n = sc.n
+    W, H = int(camv[0]), int(camv[1])
+    up = np.ascontiguousarray(upstream, dtype=np.float64)
+    em = None if extra_mask is None else np.ascontiguousarray(extra_mask, dtype=np.uint8)
+    ex = np.zeros((max(n, 1), 13)); pose = np.zeros(6); pe = np.zeros((H, W), np.uint8)
+    lib().orc_exposure(ctypes.c_int64(n), _p(mean, C_F32), _p(scale, C_F32), _p(quat, C_F32), _p(opac, C_F32),
+                       _p(rgb, C_F32), _p(act, C_U8), _p(camv, C_F64), _p(cfgv, C_F64), _p(up, C_F64), _p(em, C_U8),
+                       ctypes.c_int(int(signed_all)), ctypes.c_double(round_eps), _p(ex, C_F64), _p(pose, C_F64), _p(pe, C_U8))
+    ex = ex[:n]
+    return dict(mean=ex[:, 0:3].copy(), scale=ex[:, 3:5].copy(), quat=ex[:, 5:9].copy(), opacity=ex[:, 9].copy(),
+                rgb=ex[:, 10:13].copy(), pose=pose, pix_exposed=pe)
+
+
 def normalise_depth(img):
     """Expected depth D_n = D / O (DESIGN R9n; D = sum w z and O = sum w are the depth and opacity
     images of Eq. 8): the blend weights renormalised to sum to one.  0 where O = 0 (no splat composited).
@@ -219,6 +255,16 @@ def num_threads():
     return int(lib().orc_num_threads())
 
 
+def _depth_residual(rendered_depth, target_depth):
+    """D_r - D of Eq. 16 / Eq. 26 where the sensor depth D is valid, 0 elsewhere.  Reading R25: the paper's
+    frames are RGB-D sensor frames (L350) whose depth has holes encoded as 0 (or non-finite values); Eq. 16, 19 and 26 do not
+    spell a mask out, and a hole is no measurement, so a pixel with D <= 0 or non-finite D carries no depth term (neither
+    loss nor gradient); its colour term stays."""
+    D = np.asarray(target_depth, dtype=np.float64)
+    valid = np.isfinite(D) & (D > 0)
+    return np.where(valid, rendered_depth - np.where(valid, D, 0.0), 0.0)
+
+
 def tracking_loss(img, target_rgb, target_depth, camv, lambda_d, normal_sign=1.0):
     """Eq. 15-19 (L180-204) written out in numpy, fp64.  img: (8,H,W) rendered planes; returns
     (L_t, upstream (8,H,W)).  M_n = [sign * N_r . r > 0] (Eq. 17; R19: the harness scenes use outward
@@ -231,7 +277,7 @@ def tracking_loss(img, target_rgb, target_depth, camv, lambda_d, normal_sign=1.0
     nr = img[4] * rx + img[5] * ry + img[6]
     m = ((normal_sign * nr > 0) & (img[7] > float(np.float32(0.95)))).astype(np.float64)
     dI = img[0:3] - np.asarray(target_rgb, dtype=np.float64)
-    dD = img[3] - np.asarray(target_depth, dtype=np.float64)
+    dD = _depth_residual(img[3], target_depth)
     LI = np.abs(dI).sum(0)                   # Eq. 15: element-wise L1 over the colour channels
     LD = np.abs(dD)                          # Eq. 16
     L = (m * (LI + lambda_d * LD)).sum() / (W * H)     # Eq. 19
@@ -271,7 +317,7 @@ def mapping_loss(img, target_rgb, target_depth, camv, lambda_c, w_d, w_n, normal
     fx, fy, cx, cy = camv[2:6]
     HW = W * H
     dI = img[0:3] - np.asarray(target_rgb, dtype=np.float64)
-    dD = img[3] - np.asarray(target_depth, dtype=np.float64)
+    dD = _depth_residual(img[3], target_depth)
     ND = normal_from_depth(img[3], camv)
     Nr = img[4:7]
     Ln = 1.0 - normal_sign * (ND * Nr).sum(0)

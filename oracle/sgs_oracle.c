@@ -17,7 +17,7 @@
  * P8 central finite differences of every gradient incl. pose, P9 rigid-motion identity, P10
  * symmetries.  Parity UNPINNED: absolute image values on the paper's datasets (not available).
  *
- * Build: gcc -O2 -fopenmp -ffp-contract=off -fPIC -shared (see oracle/build.py).
+ * Build: gcc -O2 -fopenmp -ffp-contract=off -fPIC -shared (oracle/__init__.py: build()).
  * -ffp-contract=off matters: the binning stage (orc_preprocess) is the bit-exact contract with
  * the GPU and must evaluate the documented IEEE-754 binary64 operation sequence without FMA.
  */
@@ -622,6 +622,277 @@ void orc_backward(int64_t n, const float* mean, const float* scale, const float*
     if (dM_out) memcpy(dM_out, dM, sizeof(double) * 9 * (size_t)n);
     if (dnc_out) memcpy(dnc_out, dnc, sizeof(double) * 3 * (size_t)n);
     free(dM); free(dnc);
+    ctx_free(&c);
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * Comparison support (DESIGN.md §6 "fragile pixels"): NOT part of the rendered function or its gradient.
+ *
+ * A binary32 renderer and this binary64 oracle may take a DIFFERENT discrete decision (rho^2 <= c^2, z > z_near,
+ * a >= alpha_min, o G > alpha_max, T (1 - a) < t_min) at a pixel where the oracle's margin is below FRAG_EPS, and cannot
+ * agree to the image tolerance on a pair whose intersection is ill-conditioned (kappa > KAPPA_MAX).  Such pixels are
+ * compared against a bound DERIVED here instead of a flat allowance:
+ *
+ *  orc_pixel_bounds: per pixel, for the forward images,
+ *    flip_w  = sum over the pixel's fragile decisions of the blending weight at stake, a T of the pair (+ T' behind a
+ *              fragile stop): flipping one decision moves a blended value by at most 2 vmax flip_w
+ *              (|dV/da_i| <= 2 T_i vmax by Eq. 8, and the pair's own term is a T v);
+ *    kerr    = sum over composited pairs of w rho^2 kappa: first-order sensitivity of the blend to the relative rounding
+ *              eps of the intersection's inputs, delta G / G = rho^2 kappa eps  =>  |delta V| <= 2 vmax eps kerr;
+ *    kerr_z  = sum over composited pairs of w kappa (|M20 u| + |M21 v|): the same for the depth value z itself;
+ *    zmax    = largest intersection depth among the pixel's composited or fragile pairs (vmax of the depth channel).
+ *
+ *  orc_exposure: per surfel and parameter, the summed |contribution| of the "exposed" pixels (fragile ones, plus a mask
+ *    the caller passes) to the gradient, evaluated on the oracle's own composited list AND on the list with every fragile
+ *    decision of that pixel inverted; likewise for the pose 6-vector.  A renderer that decides differently at those pixels
+ *    differs from the oracle's gradient by at most a small multiple of this sum.  With signed_all != 0 it instead
+ *    accumulates the SIGNED contributions of the oracle's own list over ALL pixels, i.e. recomputes orc_backward pair by
+ *    pair through surfel_chain() -- the self-check that pins this function to orc_backward (tests/test_oracle_pins.py).
+ * ------------------------------------------------------------------------------------------- */
+static inline double pair_kappa(const Pair* r) {
+    const double nu = r->hu[0] * r->hu[0] + r->hu[1] * r->hu[1], nv = r->hv[0] * r->hv[0] + r->hv[1] * r->hv[1];
+    return sqrt(nu * nv) / fabs(r->k[2]);
+}
+/* fields eval_pair() leaves unset when it rejects a pair early (u, v are set whenever k_z != 0) */
+static inline void pair_complete(const Prep* p, double opac, const Cfg* cfg, Pair* r) {
+    const double rho2 = r->u * r->u + r->v * r->v;
+    r->z = p->M[6] * r->u + p->M[7] * r->v + p->M[8];
+    r->G = exp(-0.5 * rho2);
+    const double og = opac * r->G;
+    r->clamped = og > cfg->alpha_max;
+    r->a = r->clamped ? cfg->alpha_max : og;
+}
+
+void orc_pixel_bounds(int64_t n, const float* mean, const float* scale, const float* quat, const float* opacity,
+                      const float* rgb, const uint8_t* active, const double* camv, const double* cfgv,
+                      double* flip_w, double* kerr, double* kerr_z, double* zmax) {
+    Ctx c; ctx_init(&c, n, mean, scale, quat, opacity, rgb, active, camv, cfgv, 0);
+    const int W = c.cam.W, H = c.cam.H;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int j = 0; j < H; ++j) {
+        for (int i = 0; i < W; ++i) {
+            const double x = i + 0.5, y = j + 0.5;
+            const uint32_t* lst; const int64_t m = cand_count(&c, i, j, &lst);
+            double T = 1.0, fw = 0.0, ke = 0.0, kz = 0.0, zm = 0.0;
+            for (int64_t e = 0; e < m; ++e) {
+                const uint32_t k = c.ord[lst[e] & 0x7fffffffu];
+                const Prep* p = c.P + k;
+                if (x < p->aabb[0] - 1.0 || x > p->aabb[1] + 1.0 || y < p->aabb[2] - 1.0 || y > p->aabb[3] + 1.0) continue;
+                Pair r; int covers, f = 0;
+                const int st = eval_pair(p, opacity[k], x, y, T, &c.cfg, &r, &f, &covers);
+                if ((f & 1) && r.k[2] != 0.0 && isfinite(r.u * r.u + r.v * r.v)) {
+                    if (st != 1) pair_complete(p, opacity[k], &c.cfg, &r);
+                    fw += r.a * T + (st == 2 ? T * (1.0 - r.a) : 0.0);
+                    if (fabs(r.z) > zm) zm = fabs(r.z);
+                }
+                if (st == 2) break;
+                if (st == 0) continue;
+                const double w = r.a * T, kap = pair_kappa(&r);
+                ke += w * (r.u * r.u + r.v * r.v) * kap;
+                kz += w * kap * (fabs(p->M[6] * r.u) + fabs(p->M[7] * r.v));
+                if (fabs(r.z) > zm) zm = fabs(r.z);
+                T *= (1.0 - r.a);
+            }
+            const int64_t pix = (int64_t)j * W + i;
+            flip_w[pix] = fw; kerr[pix] = ke; kerr_z[pix] = kz; zmax[pix] = zm;
+        }
+    }
+    ctx_free(&c);
+}
+
+/* O6 + O7 for ONE set of per-surfel accumulators (dL/dM 9, dL/dt_nc 3): out13 = d mean (3), d scale (2), d quat (4),
+ * [9..12 left to the caller: opacity, rgb], pose6 = this surfel's share of (dL/drho, dL/dtheta).  Same formulas as the loop
+ * at the end of orc_backward (Eq. 9-13, R11-R15), written once more so that orc_backward stays one readable function. */
+static void surfel_chain(const Ctx* c, int64_t k, const float* scale, const double* m, const double* dnc, double* out13,
+                         double* pose6) {
+    const Prep* p = c->P + k;
+    const double* Rc = c->cam.R;
+    const double su = scale[2 * k], sv = scale[2 * k + 1];
+    double Gc[3][3];
+    for (int col = 0; col < 3; ++col) {
+        Gc[0][col] = c->cam.fx * m[col];
+        Gc[1][col] = c->cam.fy * m[3 + col];
+        Gc[2][col] = c->cam.cx * m[col] + c->cam.cy * m[3 + col] + m[6 + col];
+    }
+    double dtuc[3], dtvc[3], dtnc[3], dmuc[3], dsu = 0, dsv = 0;
+    for (int r = 0; r < 3; ++r) {
+        dtuc[r] = su * Gc[r][0]; dtvc[r] = sv * Gc[r][1]; dmuc[r] = Gc[r][2]; dtnc[r] = dnc[r];
+        dsu += p->tuc[r] * Gc[r][0]; dsv += p->tvc[r] * Gc[r][1];
+    }
+    out13[3] = dsu; out13[4] = dsv;
+    double t0[3], t1[3], t2[3], t3[3];
+    cross3(p->muc, dmuc, t0); cross3(p->tuc, dtuc, t1); cross3(p->tvc, dtvc, t2); cross3(p->tnc, dtnc, t3);
+    for (int r = 0; r < 3; ++r) { pose6[r] = dmuc[r]; pose6[3 + r] = t0[r] + t1[r] + t2[r] + t3[r]; }
+    double GR[3][3];
+    for (int r = 0; r < 3; ++r) {
+        out13[r] = Rc[0 + r] * dmuc[0] + Rc[3 + r] * dmuc[1] + Rc[6 + r] * dmuc[2];
+        GR[r][0] = Rc[0 + r] * dtuc[0] + Rc[3 + r] * dtuc[1] + Rc[6 + r] * dtuc[2];
+        GR[r][1] = Rc[0 + r] * dtvc[0] + Rc[3 + r] * dtvc[1] + Rc[6 + r] * dtvc[2];
+        GR[r][2] = Rc[0 + r] * dtnc[0] + Rc[3 + r] * dtnc[1] + Rc[6 + r] * dtnc[2];
+    }
+    const double qw = p->qh[0], qx = p->qh[1], qy = p->qh[2], qz = p->qh[3];
+    double dq[4];
+    dq[0] = 2.0 * (-qz * GR[0][1] + qy * GR[0][2] + qz * GR[1][0] - qx * GR[1][2] - qy * GR[2][0] + qx * GR[2][1]);
+    dq[1] = 2.0 * (qy * GR[0][1] + qz * GR[0][2] + qy * GR[1][0] - 2.0 * qx * GR[1][1] - qw * GR[1][2] + qz * GR[2][0] + qw * GR[2][1] - 2.0 * qx * GR[2][2]);
+    dq[2] = 2.0 * (-2.0 * qy * GR[0][0] + qx * GR[0][1] + qw * GR[0][2] + qx * GR[1][0] + qz * GR[1][2] - qw * GR[2][0] + qz * GR[2][1] - 2.0 * qy * GR[2][2]);
+    dq[3] = 2.0 * (-2.0 * qz * GR[0][0] - qw * GR[0][1] + qx * GR[0][2] + qw * GR[1][0] - 2.0 * qz * GR[1][1] + qy * GR[1][2] + qx * GR[2][0] + qy * GR[2][1]);
+    const double qd = qw * dq[0] + qx * dq[1] + qy * dq[2] + qz * dq[3];
+    for (int r = 0; r < 4; ++r) out13[5 + r] = (dq[r] - p->qh[r] * qd) / p->qn;
+}
+
+typedef struct { uint32_t k; Pair r; double T; int clamped; int64_t e; /* position in the pixel's candidate list */ } XHit;
+
+/* Reverse sweep of O5 over one pixel's list; every pair's contribution goes through surfel_chain() on its own and is
+ * added, times `sign`, to row e of `loc` (19 values: 13 parameters + 6 pose); |contribution| to `absl` if non-NULL. */
+static void exposure_sweep(const Ctx* c, const float* scale, const float* opacity, const float* rgb, const XHit* hits,
+                           size_t nh, const double* g, double x, double y, double sign, double* loc, double* absl) {
+    double suffix = 0.0;
+    for (size_t q = nh; q-- > 0;) {
+        const XHit* h = hits + q; const uint32_t k = h->k; const Prep* p = c->P + k; const Pair* r = &h->r;
+        const double w = r->a * h->T;
+        const double gv = g[0] * rgb[3 * k] + g[1] * rgb[3 * k + 1] + g[2] * rgb[3 * k + 2] + g[3] * r->z +
+                          g[4] * p->tnc[0] + g[5] * p->tnc[1] + g[6] * p->tnc[2] + g[7];
+        const double dz = g[3] * w;
+        const double da = h->T * gv - suffix / (1.0 - r->a);
+        suffix += w * gv;
+        double out[19], lm[9], lnc[3], dG = 0.0;
+        out[9] = 0.0;
+        if (!h->clamped) { out[9] = da * r->G; dG = da * opacity[k]; }
+        for (int ch = 0; ch < 3; ++ch) { out[10 + ch] = g[ch] * w; lnc[ch] = g[4 + ch] * w; }
+        const double du = -r->u * r->G * dG + dz * p->M[6];
+        const double dv = -r->v * r->G * dG + dz * p->M[7];
+        const double dk[3] = {du / r->k[2], dv / r->k[2], -(r->u * du + r->v * dv) / r->k[2]};
+        double dhu[3], dhv[3];
+        cross3(r->hv, dk, dhu);
+        cross3(dk, r->hu, dhv);
+        const double uv1[3] = {r->u, r->v, 1.0};
+        for (int t = 0; t < 3; ++t) { lm[t] = dhu[t]; lm[3 + t] = dhv[t]; lm[6 + t] = dz * uv1[t] - x * dhu[t] - y * dhv[t]; }
+        surfel_chain(c, k, scale, lm, lnc, out, out + 13);
+        for (int t = 0; t < 19; ++t) {
+            loc[19 * h->e + t] += sign * out[t];
+            if (absl) absl[19 * h->e + t] += fabs(out[t]);
+        }
+    }
+}
+
+/*
+ * expo[k][t], pose_expo[t]: what a renderer that decides differently at the EXPOSED pixels can add to / remove from
+ * gradient element t of surfel k (pose: of the 6-vector).  Summed over the exposed pixels p:
+ *     | c2(p,k) - c1(p,k) |                the pixel's contribution on the list with its fragile decisions inverted (c2)
+ *                                          minus the contribution on the oracle's own list (c1): the effect of the flip
+ *   + phi_p | c1(p,k) |                    phi_p = min(1, C eps sum_{i composited, kappa_i > KAPPA_MAX} kappa_i (1 + rho_i^2)):
+ *                                          first-order effect of the binary32 rounding of an ill-conditioned
+ *                                          intersection's inputs (C eps = round_eps, passed in)
+ *   + | c1(p,k) |  where extra_mask[p]     the caller's pixels: the whole term may appear or vanish (a loss mask)
+ * (pose: the same with the pixel's pairs summed before the | |).
+ */
+void orc_exposure(int64_t n, const float* mean, const float* scale, const float* quat, const float* opacity,
+                  const float* rgb, const uint8_t* active, const double* camv, const double* cfgv,
+                  const double* up /* 8*H*W */, const uint8_t* extra_mask /* H*W, nullable */, int signed_all, double round_eps,
+                  double* expo /* n*13, zeroed here */, double* pose_expo /* 6 */, uint8_t* pix_exposed /* H*W, nullable */) {
+    Ctx c; ctx_init(&c, n, mean, scale, quat, opacity, rgb, active, camv, cfgv, 0);
+    const int W = c.cam.W, H = c.cam.H; const int64_t HW = (int64_t)W * H;
+    const Cfg* cfg = &c.cfg;
+    memset(expo, 0, sizeof(double) * 13 * (size_t)(n > 0 ? n : 0));
+    for (int t = 0; t < 6; ++t) pose_expo[t] = 0.0;
+#pragma omp parallel
+    {
+        size_t cap = 256, lcap = 256;
+        XHit* l1 = (XHit*)malloc(sizeof(XHit) * cap); XHit* l2 = (XHit*)malloc(sizeof(XHit) * cap);
+        double* loc = (double*)malloc(sizeof(double) * 19 * lcap); double* absl = (double*)malloc(sizeof(double) * 19 * lcap);
+#pragma omp for schedule(dynamic, 1)
+        for (int j = 0; j < H; ++j) {
+            for (int i = 0; i < W; ++i) {
+                const double x = i + 0.5, y = j + 0.5;
+                const int64_t pix = (int64_t)j * W + i;
+                double g[8];
+                for (int ch = 0; ch < 8; ++ch) g[ch] = up[ch * HW + pix];
+                const uint32_t* lst; const int64_t m = cand_count(&c, i, j, &lst);
+                /* the oracle's own list (as orc_backward's replay), the pixel's fragile bits, and phi */
+                size_t n1 = 0; double T = 1.0, ksum = 0.0; int frag = 0;
+                for (int64_t e = 0; e < m; ++e) {
+                    const uint32_t k = c.ord[lst[e] & 0x7fffffffu];
+                    const Prep* p = c.P + k;
+                    if (x < p->aabb[0] - 1.0 || x > p->aabb[1] + 1.0 || y < p->aabb[2] - 1.0 || y > p->aabb[3] + 1.0) continue;
+                    Pair r; int covers, f = 0;
+                    const int st = eval_pair(p, opacity[k], x, y, T, cfg, &r, &f, &covers);
+                    frag |= f;
+                    if (st == 2) break;
+                    if (st == 0) continue;
+                    if (f & 4) ksum += pair_kappa(&r) * (1.0 + r.u * r.u + r.v * r.v);
+                    if (n1 == cap) { cap *= 2; l1 = (XHit*)realloc(l1, sizeof(XHit) * cap); l2 = (XHit*)realloc(l2, sizeof(XHit) * cap); }
+                    l1[n1].k = k; l1[n1].r = r; l1[n1].T = T; l1[n1].clamped = r.clamped; l1[n1].e = e; ++n1;
+                    T *= (1.0 - r.a);
+                }
+                const int extra = extra_mask && extra_mask[pix];
+                const int exposed = frag != 0 || extra;
+                if (pix_exposed) pix_exposed[pix] = (uint8_t)exposed;
+                if (!exposed && !signed_all) continue;
+                if ((size_t)m > lcap) {
+                    lcap = (size_t)m * 2;
+                    loc = (double*)realloc(loc, sizeof(double) * 19 * lcap); absl = (double*)realloc(absl, sizeof(double) * 19 * lcap);
+                }
+                memset(loc, 0, sizeof(double) * 19 * (size_t)m); memset(absl, 0, sizeof(double) * 19 * (size_t)m);
+                if (signed_all) {   /* self-check mode: orc_backward recomputed pair by pair */
+                    exposure_sweep(&c, scale, opacity, rgb, l1, n1, g, x, y, 1.0, loc, NULL);
+                    for (size_t q = 0; q < n1; ++q) {
+                        for (int t = 0; t < 13; ++t) atomic_add(expo + 13 * (size_t)l1[q].k + t, loc[19 * l1[q].e + t]);
+                        for (int t = 0; t < 6; ++t) atomic_add(pose_expo + t, loc[19 * l1[q].e + 13 + t]);
+                    }
+                    continue;
+                }
+                exposure_sweep(&c, scale, opacity, rgb, l1, n1, g, x, y, -1.0, loc, absl);
+                /* the list with every fragile decision of this pixel inverted */
+                size_t n2 = 0; T = 1.0;
+                for (int64_t e = 0; e < m; ++e) {
+                    const uint32_t k = c.ord[lst[e] & 0x7fffffffu];
+                    const Prep* p = c.P + k;
+                    if (x < p->aabb[0] - 1.0 || x > p->aabb[1] + 1.0 || y < p->aabb[2] - 1.0 || y > p->aabb[3] + 1.0) continue;
+                    Pair r; int covers, f = 0;
+                    (void)eval_pair(p, opacity[k], x, y, T, cfg, &r, &f, &covers);   /* fills h_u, h_v, k, u, v */
+                    if (r.k[2] == 0.0) continue;
+                    const double rho2 = r.u * r.u + r.v * r.v;
+                    if (!isfinite(rho2)) continue;
+                    pair_complete(p, opacity[k], cfg, &r);
+                    const double c2 = cfg->cutoff * cfg->cutoff, og = opacity[k] * r.G;
+                    int in = (rho2 <= c2) ^ (isfinite(c2) && fabs(rho2 - c2) < FRAG_EPS * c2);
+                    in = in && ((r.z > cfg->z_near) ^ (cfg->z_near > 0.0 && fabs(r.z - cfg->z_near) < FRAG_EPS * cfg->z_near));
+                    in = in && ((r.a >= cfg->alpha_min) ^ (cfg->alpha_min > 0.0 && fabs(r.a - cfg->alpha_min) < FRAG_EPS * cfg->alpha_min));
+                    if (!in) continue;
+                    const double Tn = T * (1.0 - r.a);
+                    const int stop = (Tn < cfg->t_min) ^ (cfg->t_min > 0.0 && fabs(Tn - cfg->t_min) < FRAG_EPS * cfg->t_min);
+                    if (stop) break;
+                    if (n2 == cap) { cap *= 2; l1 = (XHit*)realloc(l1, sizeof(XHit) * cap); l2 = (XHit*)realloc(l2, sizeof(XHit) * cap); }
+                    l2[n2].k = k; l2[n2].r = r; l2[n2].T = T; l2[n2].e = e;
+                    l2[n2].clamped = r.clamped ^ (fabs(og - cfg->alpha_max) < FRAG_EPS * cfg->alpha_max);
+                    ++n2;
+                    T = Tn;
+                }
+                exposure_sweep(&c, scale, opacity, rgb, l2, n2, g, x, y, 1.0, loc, NULL);
+                double phi = round_eps * ksum + (extra ? 1.0 : 0.0);
+                if (phi > 1.0) phi = 1.0;
+                double pd[6] = {0, 0, 0, 0, 0, 0}, pa[6] = {0, 0, 0, 0, 0, 0}, p1[6] = {0, 0, 0, 0, 0, 0};
+                for (int64_t e = 0; e < m; ++e) {   /* rows touched by either list */
+                    const double* le = loc + 19 * e; const double* ae = absl + 19 * e;
+                    int any = 0;
+                    for (int t = 0; t < 19 && !any; ++t) any = le[t] != 0.0 || ae[t] != 0.0;
+                    if (!any) continue;
+                    const uint32_t k = c.ord[lst[e] & 0x7fffffffu];
+                    for (int t = 0; t < 13; ++t) atomic_add(expo + 13 * (size_t)k + t, fabs(le[t]) + phi * ae[t]);
+                    for (int t = 0; t < 6; ++t) { pd[t] += le[13 + t]; pa[t] += ae[13 + t]; }
+                }
+                /* the oracle's own signed pose contribution of this pixel (for a mask that may flip) */
+                if (extra) {
+                    memset(loc, 0, sizeof(double) * 19 * (size_t)m);
+                    exposure_sweep(&c, scale, opacity, rgb, l1, n1, g, x, y, 1.0, loc, NULL);
+                    for (size_t q = 0; q < n1; ++q) for (int t = 0; t < 6; ++t) p1[t] += loc[19 * l1[q].e + 13 + t];
+                }
+                const double phk = round_eps * ksum > 1.0 ? 1.0 : round_eps * ksum;
+                for (int t = 0; t < 6; ++t) atomic_add(pose_expo + t, fabs(pd[t]) + phk * pa[t] + fabs(p1[t]));
+            }
+        }
+        free(l1); free(l2); free(loc); free(absl);
+    }
     ctx_free(&c);
 }
 

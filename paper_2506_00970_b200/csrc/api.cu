@@ -208,8 +208,8 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
               cudaHostAlloc(&c->pinned_small, 8 * sizeof(float), cudaHostAllocMapped) == cudaSuccess &&
               cudaHostAlloc(&c->host_flag, sizeof(unsigned int), cudaHostAllocMapped) == cudaSuccess &&
               cudaMalloc(&c->split_state, sizeof(float) * 8 * SGS_BLOCK * SGS_TRACK_HELPERS) == cudaSuccess &&
-              cudaMalloc(&c->split_flag, sizeof(unsigned int) * SGS_TRACK_HELPERS) == cudaSuccess &&
-              cudaMemset(c->split_flag, 0, sizeof(unsigned int) * SGS_TRACK_HELPERS) == cudaSuccess &&
+              cudaMalloc(&c->split_flag, sizeof(unsigned int) * (SGS_TRACK_HELPERS + 1)) == cudaSuccess &&
+              cudaMemset(c->split_flag, 0, sizeof(unsigned int) * (SGS_TRACK_HELPERS + 1)) == cudaSuccess &&
               cudaHostGetDevicePointer(&c->pinned_small_dev, c->pinned_small, 0) == cudaSuccess &&
               cudaHostGetDevicePointer(&c->host_flag_dev, c->host_flag, 0) == cudaSuccess &&
               cudaMalloc(&c->sort_hist, sizeof(uint32_t) * (8 * 256 + 8)) == cudaSuccess &&
@@ -225,6 +225,7 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
                cudaStreamCreateWithPriority(&c->aux_stream, cudaStreamNonBlocking, prio_hi) == cudaSuccess);
     if (!ok) { cudaGetLastError(); sgs_destroy(c); return SGS_CUDA_ERROR; }
     c->pose6_dev = c->loss_dev + 1;
+    if (const char* d = getenv("SGS_DEBUG_HELPER_DELAY_NS")) c->helper_delay_ns = (unsigned int)strtoul(d, nullptr, 10);
     cudaMemset(c->counters, 0, sizeof(SgsCounters));
     memset(c->counters_host, 0, sizeof(SgsCounters));
     *out = c;

@@ -77,7 +77,8 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
                     my_loss += fabsf(d);
                     g[c] = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
                 }
-                const float d = up.p[3][pix] - fl.tdepth[pix];
+                const float td = fl.tdepth[pix];
+                const float d = (td > 0.f && isfinite(td)) ? up.p[3][pix] - td : 0.f;  // R25: holes carry no depth term
                 my_loss += fl.lambda_d * fabsf(d);
                 g[3] = d > 0.f ? fl.lambda_d * inv : (d < 0.f ? -fl.lambda_d * inv : 0.f);
             }

@@ -18,7 +18,8 @@ __global__ void __launch_bounds__(SGS_BLOCK, 4)  // 64 registers, four blocks pe
 k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
           int tiles_x, SgsCfgDev cfg, Planes out, float* __restrict__ T_final, uint32_t* __restrict__ n_last,
           const uint32_t* __restrict__ cursor, unsigned long long* bucket, uint32_t tile_cap,
-          float* __restrict__ contrib, float2* __restrict__ dn_state, float* __restrict__ median_out) {
+          float* __restrict__ contrib, const uint32_t* __restrict__ contrib_map, float2* __restrict__ dn_state,
+          float* __restrict__ median_out) {
     // staged batch, structure of float4 arrays (one base register, immediate offsets, broadcast reads)
     __shared__ float4 sh[5][SGS_BLOCK];
     __shared__ unsigned char sh_mask[SGS_BLOCK];
@@ -132,7 +133,12 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
                     // w in [0, 1] as 24-bit fixed point: the warp sum is ONE redux.sync instead of five shuffle-adds
                     // (quantisation 6e-8 per pixel, far below the 1e-4 bar); 32 x 2^24 fits 32 bits
                     const unsigned ws = __reduce_add_sync(0xffffffffu, (unsigned)__float2uint_rn(w * 16777216.f));
-                    if (lane == 0 && ws != 0u) atomicAdd(contrib + __float_as_uint(s4.w), (float)ws * (1.f / 16777216.f));
+                    // the staged list value is the surfel itself (bucket binning) or its compact visible index (radix
+                    // binning, SGS_FLAG_RADIX_BINNING: contrib_map = vis_to_surfel takes it back to the surfel)
+                    if (lane == 0 && ws != 0u) {
+                        const uint32_t lv = __float_as_uint(s4.w);
+                        atomicAdd(contrib + (contrib_map ? contrib_map[lv] : lv), (float)ws * (1.f / 16777216.f));
+                    }
                 }
                 if (MEDIAN) med = (pass && T > 0.5f && Tn <= 0.5f) ? z : med;
                 T = pass ? Tn : T;
@@ -172,6 +178,7 @@ cudaError_t sgs_launch_forward(sgs_ctx* c, float* const planes[8], cudaStream_t 
 #define SGS_FWD_ARGS c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, c->camd.W, \
                      c->camd.H, c->camd.tiles_x, c->cfgd, out, c->T_final, c->n_last, c->fused_sort ? c->cursor : nullptr,     \
                      reinterpret_cast<unsigned long long*>(c->bucket), (uint32_t)c->tile_cap, c->contrib_out, \
+                     (c->list_stride == 2 ? nullptr : c->vis_to_surfel), \
                      (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) ? c->dn_state : nullptr, c->median_out
     const bool nd = (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) != 0;
     if (c->median_out) {  // (sgs_render_median; never together with the contribution output)

@@ -29,7 +29,8 @@ k_tracking_loss(LP p, const float* __restrict__ trgb, const float* __restrict__ 
                 acc += fabsf(d);
                 g[c] = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
             }
-            const float d = p.ren[3][i] - tdepth[i];
+            const float td = tdepth[i];  // R25: a hole in the sensor depth (0, negative, inf, NaN) carries no depth term
+            const float d = (td > 0.f && isfinite(td)) ? p.ren[3][i] - td : 0.f;
             acc += lambda_d * fabsf(d);
             g[3] = d > 0.f ? lambda_d * inv : (d < 0.f ? -lambda_d * inv : 0.f);
         }
@@ -125,7 +126,7 @@ k_mapping_loss(MapImg im, const float* __restrict__ trgb, const float* __restric
             acc += lambda_c * fabsf(d);
             g[c] = d > 0.f ? lambda_c * inv : (d < 0.f ? -lambda_c * inv : 0.f);
         }
-        const float dd = d00 - td;
+        const float dd = (td > 0.f && isfinite(td)) ? d00 - td : 0.f;  // R25: no depth term on holes of the sensor depth
         acc += w_d * fabsf(dd);
         g[3] = dd > 0.f ? w_d * inv : (dd < 0.f ? -w_d * inv : 0.f);
         acc += w_n * (1.f - nsign * (N[0] * m[0][0] + N[1] * m[0][1] + N[2] * m[0][2]));

@@ -166,8 +166,9 @@ struct sgs_ctx {
     // device-visible); the host polls it instead of a copy + stream synchronisation
     unsigned int* host_flag; unsigned int* host_flag_dev; float* pinned_small_dev;
     unsigned int host_flag_val; bool host_flag_want, host_flag_armed;
-    // K-track helpers (track.cu): per helper 6 x 256 floats of per-pixel state and a flag word, the launch counter they compare with
-    float* split_state; unsigned int* split_flag; unsigned int track_launch_id;
+    // K-track helpers (track.cu): per helper 8 x 256 floats of per-pixel state and a flag word; split_flag[SGS_TRACK_HELPERS] is the
+    // launch epoch the flag values are built from (device-side, so that graph replays stay distinct)
+    float* split_state; unsigned int* split_flag; unsigned int helper_delay_ns;
     cudaEvent_t order_fork, order_done; bool order_pending;  // k_track_order on aux_stream
     bool order_skip;                 // SGS_FLAG_GRAPH + SGS_FLAG_TRACK_REUSE: the tile order is renewed once per frame only
     const SgsCounters* stats_src;    // SGS_FLAG_GRAPH: where the last binning's counters sit on the device (sgs_get_stats copies them)

@@ -68,7 +68,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         TrackPlanes out, const float* __restrict__ trgb, const float* __restrict__ tdepth, float lambda_d, float nsign,
         float* __restrict__ pose_partial, SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
         float* __restrict__ loss_out, uint32_t* __restrict__ tile_cost, uint32_t* cursor_rw, SgsCounters* __restrict__ counters_snap,
-        unsigned int* host_flag, unsigned int flag_val, float* split_state, unsigned int* split_flag, unsigned int launch_id,
+        unsigned int* host_flag, unsigned int flag_val, float* split_state, unsigned int* split_flag, unsigned int helper_delay_ns,
         int n_help) {
     const long long t_start = clock64();
     cudaTriggerProgrammaticLaunchCompletion();  // the next iteration's K-pre-B may be staged; it waits for this grid before it reads anything
@@ -186,7 +186,8 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
                 float d = C0 - tr; my_loss += fabsf(d); g0 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
                 d = C1 - tg; my_loss += fabsf(d); g1 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
                 d = C2 - tb; my_loss += fabsf(d); g2 = d > 0.f ? inv : (d < 0.f ? -inv : 0.f);
-                d = Dp - td; my_loss += lambda_d * fabsf(d);
+                d = (td > 0.f && isfinite(td)) ? Dp - td : 0.f;  // R25: holes of the sensor depth carry no depth term
+                my_loss += lambda_d * fabsf(d);
                 g3 = d > 0.f ? lambda_d * inv : (d < 0.f ? -lambda_d * inv : 0.f);
                 if (NDEPTH) g3 *= __frcp_rn(O);  // O > 0.95 here
             }
@@ -281,29 +282,31 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     // partial sums and draws its ticket below, so that the grid reduction counts every block)
     const bool split = (helper || has_helper) && !presorted && n > TRK_SPLIT_MIN && n <= (uint32_t)TRK_CAP;
     const uint32_t msp = split ? (((n + 1u) / 2u + 31u) & ~31u) : n;  // block 0: [0, msp) on the way back, block 1: [msp, n)
-    // per-pixel state the owner hands to its helper: 6 x 256 floats in global memory, published by a flag = this launch's id
+    // per-pixel state the owner hands to its helper: 6 x 256 floats in global memory.  The hand-over is two flag values per
+    // launch, 4 * epoch + 1 (the owner has written the SORTED bucket back) and 4 * epoch + 2 (... and the pixels' state); the
+    // epoch is a device word (split_flag[SGS_TRACK_HELPERS]) that the launch's last block increments, so a replayed CUDA
+    // graph -- whose kernel arguments are frozen -- never meets a flag value left by an earlier replay.
     float* st = split_state + (size_t)slot * (8 * SGS_BLOCK);  // g0..g3, T, last, zref (NDEPTH), one spare
+    const unsigned int epoch4 = split ? 4u * __ldcg(split_flag + SGS_TRACK_HELPERS) : 0u;
+    volatile unsigned int* my_flag = reinterpret_cast<volatile unsigned int*>(split_flag + slot);
     if (crank == 1) {
         if (split) {
-            for (uint32_t e = tid; e < (uint32_t)TRK_CAP; e += SGS_BLOCK) {
-                s_keys[e] = e < n ? g[e] : ~0ull;
-                sh_mask[e] = 0;
+            // The helper reads the bucket only AFTER its owner has published the sorted keys: it never looks at the raw
+            // bucket, which the owner permutes in place (reading it unordered was a data race).  It has nothing else to do
+            // until the owner's forward walk ends, so waiting for the owner's sort costs nothing.
+            if (helper_delay_ns) __nanosleep(helper_delay_ns);  // (test hook: SGS_DEBUG_HELPER_DELAY_NS, see sgs_create)
+            for (uint32_t e = tid; e < (uint32_t)TRK_CAP; e += SGS_BLOCK) sh_mask[e] = 0;
+            if (tid == 0) {
+                unsigned int f;
+                while ((f = *my_flag) != epoch4 + 1u && f != epoch4 + 2u) __nanosleep(100);
+                __threadfence();
             }
             __syncthreads();
-            for (uint32_t e0 = 0; e0 < n; e0 += SGS_BLOCK) {
-                if (e0 + (uint32_t)(wid * 32) < n) {
-                    const uint32_t e = e0 + tid;
-                    const bool mine = e < n;
-                    const unsigned long long key = mine ? s_keys[e] : ~0ull;
-                    uint32_t rank = 0;
-                    for (uint32_t k = 0; k < n; ++k) rank += s_keys[k] < key ? 1u : 0u;
-                    if (mine && rank >= msp)   // this block's part of the sorted list, at slot rank - msp
-                        sh_mask[rank - msp] = (unsigned char)stage_track(pay, (uint32_t)key, px0, py0, tx0, ty0, sh, (int)(rank - msp), cfg);
-                }
-            }
+            for (uint32_t e = msp + tid; e < n; e += SGS_BLOCK)   // this block's part of the sorted list, at slot e - msp
+                sh_mask[e - msp] = (unsigned char)stage_track(pay, (uint32_t)__ldcg(g + e), px0, py0, tx0, ty0, sh, (int)(e - msp), cfg);
             __syncthreads();
             if (tid == 0) {  // the owner has walked forward and stored these pixels' state
-                while (*reinterpret_cast<volatile unsigned int*>(split_flag + slot) != launch_id) __nanosleep(200);
+                while (*my_flag != epoch4 + 2u) __nanosleep(200);
                 __threadfence();
             }
             __syncthreads();
@@ -331,12 +334,14 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
                 uint32_t rank = 0;
                 for (uint32_t k = 0; k < n; ++k) rank += s_keys[k] < key ? 1u : 0u;
                 if (mine) {
-                    g[rank] = key;  // sorted list for sgs_get_binning
+                    g[rank] = key;  // sorted list for sgs_get_binning and for the tile's helper
                     sh_mask[rank] = (unsigned char)stage_track(pay, (uint32_t)key, px0, py0, tx0, ty0, sh, (int)rank, cfg);
                 }
             }
         }
+        if (split) __threadfence();  // the sorted keys, before the flag below
         __syncthreads();
+        if (split && tid == 0) *my_flag = epoch4 + 1u;
         if (!split) {
             forward_walk(0u, n);
             finish_forward();
@@ -355,7 +360,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
             if (NDEPTH) st[6 * SGS_BLOCK + tid] = zref;
             __threadfence();
             __syncthreads();
-            if (tid == 0) *reinterpret_cast<volatile unsigned int*>(split_flag + slot) = launch_id;
+            if (tid == 0) *my_flag = epoch4 + 2u;
             // the way back over [0, msp): transmittance behind entry msp - 1 and the suffix sum of everything behind it,
             // sum_{j >= msp} w_j (g . v_j) = g . (V_final - V_msp) with V the running accumulators of Eq. 8
             T_after = Tm;
@@ -451,6 +456,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         if (counters_snap) *counters_snap = *counters;  // what the host reads for overflow detection and hints
         counters->n_entries = 0ull; counters->n_visible = 0u; counters->overflow = 0u; counters->ticket_pre = 0u;
         counters->max_tile = 0u; counters->n_surv = 0u;
+        if (n_help > 0) split_flag[SGS_TRACK_HELPERS] += 1u;  // next launch's epoch: every block of this one is past its hand-over
     }
 }
 
@@ -550,11 +556,10 @@ cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* tr
     unsigned int* hflag = c->host_flag_want ? c->host_flag_dev : nullptr;  // (sgs_track_iter_host)
     const bool ndepth = (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) != 0;
     const int n_help = (c->split_state && tiles >= 4 * SGS_TRACK_HELPERS) ? SGS_TRACK_HELPERS : 0;
-    c->track_launch_id += 1;
     c->host_flag_armed = hflag != nullptr;
 #define SGS_TRK_ARGS c->tile_order, c->ranges, c->cursor, bucket, tile_cap, presorted, c->pay, cam.W, cam.H, cam.tiles_x, cam.fx, cam.fy, cam.cx, \
                      cam.cy, c->cfgd, out, trgb, tdepth, lambda_d, nsign, c->pose_partial, c->counters, d_pose6, loss, c->tile_cost, c->cursor,   \
-                     snap, hflag, c->host_flag_val, c->split_state, c->split_flag, c->track_launch_id, n_help
+                     snap, hflag, c->host_flag_val, c->split_state, c->split_flag, c->helper_delay_ns, n_help
     if (ndepth) {
         if (any) k_track<true, true><<<tiles + n_help, SGS_BLOCK, 0, s>>>(SGS_TRK_ARGS);
         else k_track<false, true><<<tiles + n_help, SGS_BLOCK, 0, s>>>(SGS_TRK_ARGS);

@@ -2,6 +2,8 @@
 (SGS_FLAG_ASYNC renderer, same scenes, same views): binning bit-exact, whole images, the Eq. 15-19 loss,
 and the backward the config asks for (pose-only for the tracking-shaped C2/C5, full + pose for the
 mapping-shaped C3/C4) against the oracle on WHOLE images -- the fp64 oracle finishes a view in seconds.
+Every pixel and every gradient element is bounded (gpu_common: the strict bars, plus oracle-derived allowances on
+fragile pixels only); the benchmarked tracking path is held to north_star's 1e-3 plus an oracle-computed flip slack.
 Every oracle input comes from scenegen/ or from the oracle itself (target frame, upstream gradients);
 nothing the CUDA path produced is fed to it."""
 import numpy as np
@@ -14,7 +16,8 @@ import scenegen
 pytestmark = pytest.mark.gpu
 
 sgs = pytest.importorskip("paper_2506_00970_b200")
-from gpu_common import (to_device, camera, alloc_images, planes, alloc_grads, image_check, grad_check)  # noqa: E402
+from gpu_common import (to_device, camera, alloc_images, planes, alloc_grads, image_check, assert_image_check,  # noqa: E402
+                        assert_grads, assert_pose, tracking_reference, tracking_flips, tracking_slack, GROUPS, C_EXPO)
 
 LAMBDA_D, NSIGN = 0.5, -1.0
 
@@ -61,53 +64,65 @@ def check_config(name, views, full):
             im, upi = alloc_images(cam), alloc_images(cam)
             render_settled(ren, sf, c, im)
             # ---- binning: bit-exact
-            assert_binning(ren.get_binning(sc.n, tiles), oracle.binning(sc, camv, cfg))
-            # ---- images
+            ob = oracle.binning(sc, camv, cfg)
+            assert_binning(ren.get_binning(sc.n, tiles), ob)
+            # ---- images: every pixel (fragile ones within the oracle-derived allowance)
             o = oracle.render(sc, camv, cfg)
             gimg = planes(im)
-            chk = image_check(gimg, o["img"], o["fragile"])
-            assert chk["n_bad"] == 0 and chk["fragile_ok"] and chk["fragile_frac"] < 0.05, (name, v, chk)
-            # ---- Eq. 15-19 against a target frame rendered BY THE ORACLE at the perturbed pose
+            assert_image_check(image_check(gimg, o["img"], o["fragile"], oracle.pixel_bounds(sc, camv, cfg)), (name, v))
+            # ---- Eq. 15-19 against a target frame rendered BY THE ORACLE at the perturbed pose (as binary32: the frame
+            # both sides see)
             T_tgt = scenegen.perturb_pose(cam.T_cw, tau0(info.get("tau0_seed", 2000 + v)))
-            tgt = oracle.render(sc, oracle.make_cam(cam, T_tgt), cfg, counters=False)["img"]
-            L_ref, up_ref = oracle.tracking_loss(o["img"], tgt[0:3], tgt[3], camv, LAMBDA_D, NSIGN)
+            tgt = oracle.render(sc, oracle.make_cam(cam, T_tgt), cfg, counters=False)["img"].astype(np.float32).astype(np.float64)
+            tr = tracking_reference(sc, camv, cfg, o, tgt, LAMBDA_D, NSIGN, oracle)
+            L_ref, up_ref = tr["L"], tr["up"]
             assert (up_ref != 0).mean() > 0.02
             trgb = torch.from_numpy(tgt[0:3].astype(np.float32)).cuda()
             tdep = torch.from_numpy(tgt[3:4].astype(np.float32)).cuda()
             loss = torch.zeros(1, device="cuda")
             ren.tracking_loss(c, im, trgb, tdep, LAMBDA_D, NSIGN, upi, loss)
-            assert abs(float(loss.item()) - L_ref) <= 2e-4 * abs(L_ref), (float(loss.item()), L_ref)
-            # the loss's gradient is +-1/|Omega| per pixel: it may differ from the oracle's only where a mask or a
-            # sign sits on a rounding edge
-            assert (np.sign(planes(upi)) != np.sign(up_ref)).any(axis=0).mean() < 2e-3
+            # the loss's gradient is +-1/|Omega| per pixel: it may differ from the oracle's only where a mask or a sign
+            # sits inside the image bar (asserted), and those pixels bound what the fused paths may differ by
+            D = tracking_flips(tr, planes(upi))
+            assert D.any(0).mean() < 2e-4, D.sum(axis=(1, 2))
+            pose_slack, loss_slack = tracking_slack(sc, camv, cfg, tr, D, oracle)
+            assert abs(float(loss.item()) - L_ref) <= tr["loss_tol"] + loss_slack, (float(loss.item()), L_ref)
             # ---- backward on the ORACLE's upstream gradients (same array to both sides)
             u = torch.from_numpy(up_ref.astype(np.float32)).cuda()
             up32 = u.cpu().numpy().astype(np.float64)
-            og = oracle.backward(sc, camv, cfg, up32)
+            og, ex = oracle.backward(sc, camv, cfg, up32), oracle.exposure(sc, camv, cfg, up32)
             kw = dict(d_rgb=u[0:3].contiguous(), d_depth=u[3:4].contiguous(), d_normal=u[4:7].contiguous(),
                       d_alpha=u[7:8].contiguous())
             p6 = torch.full((6,), 3.0, device="cuda")
             if full:
-                g = alloc_grads(sc.n)
-                ren.backward(**kw, grads=g, d_pose6=p6)
-                torch.cuda.synchronize()
-                for k in ("mean", "scale", "quat", "opacity", "rgb"):
-                    gk = g[k].cpu().numpy()
-                    ck = grad_check(gk, og[k])
-                    assert ck["frac_bad"] <= 2e-3, (name, v, k, ck)
-                    assert (gk[oracle.binning(sc, camv, cfg)["culled"].astype(bool)] == 0).all()
+                # the mapping-shaped configs: EVERY element of every surfel gradient, under the mapping loss of Eq. 24-26
+                # (dense upstream on all channels), then under the tracking loss's masked upstream
+                _, upm = oracle.mapping_loss(o["img"], tgt[0:3], tgt[3], camv, 0.875, 0.5, 0.02, NSIGN)
+                for upx in (upm, up32):
+                    ux = torch.from_numpy(upx.astype(np.float32)).cuda()
+                    ux64 = ux.cpu().numpy().astype(np.float64)
+                    ogx, exx = oracle.backward(sc, camv, cfg, ux64), oracle.exposure(sc, camv, cfg, ux64)
+                    g = alloc_grads(sc.n)
+                    ren.backward(d_rgb=ux[0:3].contiguous(), d_depth=ux[3:4].contiguous(), d_normal=ux[4:7].contiguous(),
+                                 d_alpha=ux[7:8].contiguous(), grads=g, d_pose6=p6)
+                    torch.cuda.synchronize()
+                    gn = {k: g[k].cpu().numpy() for k in GROUPS}
+                    assert_grads(gn, ogx, exx, (name, v))
+                    for k in GROUPS:
+                        assert (gn[k][ob["culled"].astype(bool)] == 0).all()
+                    assert_pose(p6.cpu().numpy(), ogx["pose"], exx["pose"], (name, v))
             else:
                 ren.backward(**kw, d_pose6=p6)
-            pose = p6.cpu().numpy().astype(np.float64)
-            assert np.abs(pose - og["pose"]).max() <= 1e-3 * np.abs(og["pose"]).max(), (name, v, pose, og["pose"])
+                assert_pose(p6.cpu().numpy(), og["pose"], ex["pose"], (name, v))
             if not full:
-                # the launch bench.py times: Eq. 15-19 evaluated inside the pose-only backward on the GPU's own
-                # images (its per-pixel signs/masks may sit on the other side of a rounding edge at a few pixels)
+                # the launch bench.py times: Eq. 15-19 evaluated inside the pose-only backward on the GPU's own images:
+                # north_star's 1e-3 plus what the masks / signs that came out differently (D) can change
+                allow = tr["ex"]["pose"] + pose_slack / C_EXPO
                 p6f, lossf = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
                 ren.backward_tracking(trgb, tdep, LAMBDA_D, NSIGN, p6f, lossf)
-                assert abs(float(lossf.item()) - L_ref) <= 2e-4 * abs(L_ref)
+                assert abs(float(lossf.item()) - L_ref) <= tr["loss_tol"] + loss_slack
                 posef = p6f.cpu().numpy().astype(np.float64)
-                assert np.abs(posef - og["pose"]).max() <= 2e-3 * np.abs(og["pose"]).max(), (name, v, posef, og["pose"])
+                assert_pose(posef, tr["og"]["pose"], allow, (name, v, "backward_tracking"))
                 # ... and the single-launch iteration (sgs_track_iter: sort + render + loss + backward in one kernel)
                 im2 = alloc_images(cam)
                 p6t, losst = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
@@ -115,11 +130,11 @@ def check_config(name, views, full):
                     ren.track_iter(sf, c, trgb, tdep, LAMBDA_D, NSIGN, p6t, losst, **im2)
                     ren.stats()
                 assert np.array_equal(planes(im2), gimg)                      # same images, bit for bit
-                assert_binning(ren.get_binning(sc.n, tiles), oracle.binning(sc, camv, cfg))
+                assert_binning(ren.get_binning(sc.n, tiles), ob)
                 assert abs(float(losst.item()) - float(lossf.item())) <= 1e-6 * abs(L_ref)
                 poset = p6t.cpu().numpy().astype(np.float64)
                 assert np.abs(poset - posef).max() <= 1e-5 * np.abs(posef).max(), (poset, posef)
-                assert np.abs(poset - og["pose"]).max() <= 2e-3 * np.abs(og["pose"]).max(), (name, v, poset, og["pose"])
+                assert_pose(poset, tr["og"]["pose"], allow, (name, v, "track_iter"))
                 ren.track_iter(sf, c, trgb, tdep, LAMBDA_D, NSIGN, p6t, losst)   # no image outputs
                 np.testing.assert_allclose(p6t.cpu().numpy(), poset, rtol=1e-5, atol=1e-7 * np.abs(poset).max())
     finally:

@@ -1,8 +1,9 @@
 """GPU parity of the per-splat contribution C_k^V (Eq. 20-21) and the covisibility score (Eq. 22):
 sgs_render_contrib / sgs_covisibility against oracle.contribution / oracle.covisibility.
-C_k is a sum of blending coefficients, compared at 1e-4 relative with an absolute floor of 1e-3 "pixels" (a
-threshold flip of one fragile pixel moves one coefficient by at most o exp(-4.5) = 0.011); the covisibility counts
-are integer work and must match exactly on identical inputs."""
+C_k is a sum of blending coefficients: EVERY splat is compared at 1e-4 relative with an absolute floor of 1e-3 "pixels"
+(the 24-bit fixed-point warp sum quantises each pixel's coefficient to 6e-8) plus the oracle-derived exposure of the
+fragile pixels the splat touches (C_k is the colour gradient of sum_p I_r(p), so oracle.exposure of that upstream bounds
+what a flipped decision can move); the covisibility counts are integer work and must match exactly on identical inputs."""
 import numpy as np
 import pytest
 import torch
@@ -13,7 +14,7 @@ import scenegen
 pytestmark = pytest.mark.gpu
 
 sgs = pytest.importorskip("paper_2506_00970_b200")
-from gpu_common import to_device, camera, alloc_images, planes  # noqa: E402
+from gpu_common import to_device, camera, alloc_images, planes, C_EXPO  # noqa: E402
 
 
 def gpu_contrib(ren, sf, n, cam, T_cw=None):
@@ -31,26 +32,33 @@ def gpu_contrib(ren, sf, n, cam, T_cw=None):
     return contrib, im
 
 
-def check_contrib(C_gpu, C_ref):
+def contrib_exposure(sc, camv, cfg, cam):
+    up = np.zeros((8, cam.height, cam.width)); up[0] = 1.0       # d/d rgb_k[0] of sum_p I_r(p) = sum_p w_k(p) = C_k
+    return oracle.exposure(sc, camv, cfg, up)["rgb"][:, 0]
+
+
+def check_contrib(C_gpu, C_ref, expo):
     err = np.abs(C_gpu - C_ref)
-    bound = 1e-4 * np.abs(C_ref) + 1e-3
-    bad = err > bound
-    assert bad.mean() <= 2e-3, (bad.sum(), err.max())
-    assert err.max() <= 0.05, err.max()
-    assert ((C_ref == 0) <= (C_gpu < 1e-3)).all()
+    bound = 1e-4 * np.abs(C_ref) + 1e-3 + C_EXPO * expo
+    assert (err <= bound).all(), (int((err > bound).sum()), float((err / bound).max()))
+    assert C_EXPO * expo.sum() <= 0.01 * C_ref.sum()             # the allowance is a small part of what is compared
+    assert ((C_ref == 0) <= (C_gpu <= C_EXPO * expo + 1e-3)).all()
 
 
-@pytest.mark.parametrize("name,view", [("C1", 0), ("C2", 0), ("C3", 3), ("C5", 0)])
-def test_contribution_matches_oracle(name, view):
+@pytest.mark.parametrize("name,view,radix", [("C1", 0, False), ("C2", 0, False), ("C3", 3, False), ("C5", 0, False),
+                                             ("C1", 0, True), ("C2", 0, True)])
+def test_contribution_matches_oracle(name, view, radix):
+    """radix: under SGS_FLAG_RADIX_BINNING the tile lists hold compact visible indices; the contribution must still land
+    on the splat itself (it used to land on the list value)."""
     sc, cams, _ = scenegen.make_config(name)
     cam = cams[view]
     camv, cfg = oracle.make_cam(cam), oracle.make_cfg()
-    ren = sgs.Renderer(async_mode=(name != "C1"))
+    ren = sgs.Renderer(async_mode=(name != "C1"), radix_binning=radix)
     t, sf = to_device(sc)
     contrib, im = gpu_contrib(ren, sf, sc.n, cam)
     C_gpu = contrib.cpu().numpy().astype(np.float64)
     C_ref = oracle.contribution(sc, camv, cfg)
-    check_contrib(C_gpu, C_ref)
+    check_contrib(C_gpu, C_ref, contrib_exposure(sc, camv, cfg, cam))
     culled = oracle.binning(sc, camv, cfg)["culled"].astype(bool)
     assert (C_gpu[culled] == 0).all()                                    # exactly zero for inactive / culled
     # sum_k C_k = sum_p O(p) on the GPU's own outputs (Eq. 21 vs Eq. 8)

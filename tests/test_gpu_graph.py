@@ -110,3 +110,46 @@ def test_mapping_iteration_in_a_cuda_graph():
         np.testing.assert_allclose(g[k].cpu().numpy(), eager[0][k], rtol=2e-4, atol=1e-5 * np.abs(eager[0][k]).max())
     np.testing.assert_allclose(p6.cpu().numpy(), eager[1], rtol=1e-4, atol=1e-5 * np.abs(eager[1]).max())
     r.close()
+
+
+def test_track_iter_graph_replays_back_to_back_with_split_tiles():
+    """C2 at full size has tile lists of 161-384 entries, which K-track splits between an owner and a helper block; their
+    hand-over flags carry a DEVICE-side epoch, so a graph -- whose kernel arguments are frozen at capture -- can be replayed
+    back to back (no eager call in between) with the target changed in place, and every replay equals the eager result."""
+    sc, cams, _ = scenegen.make_config("C2")
+    cam = cams[0]
+    t, sf = to_device(sc)
+    c = camera(cam)
+    r = sgs.Renderer(graph=True)
+    im = alloc_images(cam)
+    r.render(sf, c, **im)
+    base_rgb, base_dep = im["rgb"].clone(), im["depth"].clone()
+    tgt_rgb, tgt_dep = (base_rgb * 0.9 + 0.01).contiguous(), (base_dep * 1.02).contiguous()
+    p6, loss = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+
+    def frame():
+        for _ in range(3):   # three iterations per graph: flags written by one are met by the next inside a replay too
+            r.track_iter(sf, c, tgt_rgb, tgt_dep, 0.5, -1.0, p6, loss)
+
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        for _ in range(2):
+            frame()
+    torch.cuda.current_stream().wait_stream(s)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=s):
+        frame()
+    eager = sgs.Renderer()
+    pe, le = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+    for k, (a, b) in enumerate([(0.9, 1.02), (0.8, 1.05), (1.1, 0.97), (0.95, 1.0)]):
+        tgt_rgb.copy_(base_rgb * a + 0.01); tgt_dep.copy_(base_dep * b)
+        p6.fill_(-3.0); loss.fill_(-3.0)
+        graph.replay()                       # replays follow one another directly
+        eager.track_iter(sf, c, tgt_rgb, tgt_dep, 0.5, -1.0, pe, le)
+        torch.cuda.synchronize()
+        np.testing.assert_allclose(loss.cpu().numpy(), le.cpu().numpy(), rtol=1e-5)
+        np.testing.assert_allclose(p6.cpu().numpy(), pe.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(pe.abs().max()))
+    assert r.stats()["overflow"] == 0
+    r.close(); eager.close()

@@ -13,7 +13,8 @@ pytestmark = pytest.mark.gpu
 
 sgs = pytest.importorskip("paper_2506_00970_b200")
 from gpu_common import (to_device, camera, alloc_images, planes, alloc_grads, split_upstream, image_check,  # noqa: E402
-                        grad_check)
+                        assert_image_check, assert_grads, assert_pose, tracking_reference, tracking_flips, tracking_slack,
+                        GROUPS, C_EXPO)
 
 
 @pytest.fixture(scope="module")
@@ -23,10 +24,8 @@ def ren():
     r.close()
 
 
-def check_images(gimg, o):
-    chk = image_check(gimg, o["img"], o["fragile"])
-    assert chk["n_bad"] == 0, chk
-    assert chk["fragile_ok"], chk
+def check_images(gimg, o, sc, camv, cfg):
+    assert_image_check(image_check(gimg, o["img"], o["fragile"], oracle.pixel_bounds(sc, camv, cfg), raw=o["img_raw"]))
 
 
 @pytest.mark.parametrize("tau", [None, [0.1, -0.2, 0.15, 0.2, -0.1, 0.3]])
@@ -42,20 +41,19 @@ def test_c1_images_and_all_gradients(ren, tau):
     ren.render(sf, c, **im)
     o = oracle.render_normalised(sc, camv, cfg)
     gimg = planes(im)
-    check_images(gimg, o)
+    check_images(gimg, o, sc, camv, cfg)
     m = o["img"][7] > 0.05
     assert np.abs(gimg[3][m] - o["img_raw"][3][m]).max() > 0.1      # it is not the Eq. 8 depth any more
     ob = oracle.binning(sc, camv, cfg)
     gb = ren.get_binning(sc.n, 12)
     assert np.array_equal(gb["keys"], ob["keys"]) and np.array_equal(gb["idx"], ob["idx"])
     og = oracle.backward_normalised(sc, camv, cfg, up)
+    ex = oracle.exposure(sc, camv, cfg, oracle.normalised_depth_upstream(o["img_raw"], up))
     g, p6 = alloc_grads(sc.n), torch.full((6,), 3.0, device="cuda")
     ren.backward(**split_upstream(up), grads=g, d_pose6=p6)
     torch.cuda.synchronize()
-    for k in ("mean", "scale", "quat", "opacity", "rgb"):
-        chk = grad_check(g[k].cpu().numpy(), og[k])
-        assert chk["frac_bad"] <= 2e-3, (k, chk)
-    assert np.abs(p6.cpu().numpy() - og["pose"]).max() <= 1e-3 * np.abs(og["pose"]).max()
+    assert_grads({k: g[k].cpu().numpy() for k in GROUPS}, og, ex)
+    assert_pose(p6.cpu().numpy(), og["pose"], ex["pose"], max_slack=0.5)
     # the normalisation matters to the gradients: the plain backward of the same upstream is far away
     plain = oracle.backward(sc, camv, cfg, up)
     assert np.abs(plain["pose"] - og["pose"]).max() > 0.05 * np.abs(og["pose"]).max()
@@ -65,12 +63,16 @@ def test_c1_images_and_all_gradients(ren, tau):
     p6b = torch.zeros(6, device="cuda")
     ren.backward(**split_upstream(up_d), d_pose6=p6b)
     ogd = oracle.backward_normalised(sc, camv, cfg, up_d)
-    assert np.abs(p6b.cpu().numpy() - ogd["pose"]).max() <= 1e-3 * np.abs(ogd["pose"]).max()
+    exd = oracle.exposure(sc, camv, cfg, oracle.normalised_depth_upstream(o["img_raw"], up_d))
+    # (D_n = D / O amplifies the upstream by 1 / O exactly at the faint pixels whose single splat sits on the alpha_min edge,
+    # so on this 3072-pixel frame the fragile pixels' exposure is a larger share of the gradient than anywhere else)
+    assert_pose(p6b.cpu().numpy(), ogd["pose"], exd["pose"], max_slack=0.5)
 
 
 def test_c2_tracking_iteration_at_full_size(ren):
     """C2 (200k surfels, 640x480): images, then sgs_track_iter (loss Eq. 15-19 on D_n, pose gradient) against the
-    oracle's loss on the GPU's images and its analytic backward through the division."""
+    oracle's loss on ITS OWN normalised images and its analytic backward through the division; masks / signs the renderer
+    evaluates differently on its own image may only sit inside the image bar, and bound the allowed difference."""
     sc, cams, info = scenegen.make_config("C2")
     cam = cams[0]
     camv, cfg = oracle.make_cam(cam), oracle.make_cfg()
@@ -78,9 +80,10 @@ def test_c2_tracking_iteration_at_full_size(ren):
     d = np.stack([g.normal(3), g.normal(3)])
     tau0 = np.concatenate([0.02 * d[0] / np.linalg.norm(d[0]), np.deg2rad(1.0) * d[1] / np.linalg.norm(d[1])])
     tgt = oracle.render_normalised(sc, oracle.make_cam(cam, scenegen.perturb_pose(cam.T_cw, tau0)), cfg, counters=False)["img"]
+    tgt = tgt.astype(np.float32).astype(np.float64)       # the frame both sides see
     t, sf = to_device(sc)
     c = camera(cam)
-    im = alloc_images(cam)
+    im, upi = alloc_images(cam), alloc_images(cam)
     trgb = torch.from_numpy(tgt[0:3].astype(np.float32)).cuda()
     tdep = torch.from_numpy(tgt[3:4].astype(np.float32)).cuda()
     p6, loss = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
@@ -88,12 +91,16 @@ def test_c2_tracking_iteration_at_full_size(ren):
     torch.cuda.synchronize()
     o = oracle.render_normalised(sc, camv, cfg)
     gimg = planes(im)
-    check_images(gimg, o)
-    L_ref, up_ref = oracle.tracking_loss(gimg, trgb.cpu().numpy(), tdep.cpu().numpy()[0], camv, 0.5, -1.0)
-    assert (up_ref[3] != 0).mean() > 0.05
-    assert abs(float(loss.item()) - L_ref) <= 1e-4 * abs(L_ref)
-    og = oracle.backward_normalised(sc, camv, cfg, up_ref)
-    assert np.abs(p6.cpu().numpy() - og["pose"]).max() <= 1e-3 * np.abs(og["pose"]).max(), (p6, og["pose"])
+    check_images(gimg, o, sc, camv, cfg)
+    tr = tracking_reference(sc, camv, cfg, o, tgt, 0.5, -1.0, oracle, normalised=True)
+    assert (tr["up"][3] != 0).mean() > 0.05
+    l2 = torch.zeros(1, device="cuda")
+    ren.tracking_loss(c, im, trgb, tdep, 0.5, -1.0, upi, l2)
+    D = tracking_flips(tr, planes(upi))
+    assert D.any(0).mean() < 2e-4
+    pose_slack, loss_slack = tracking_slack(sc, camv, cfg, tr, D, oracle)
+    assert abs(float(loss.item()) - tr["L"]) <= tr["loss_tol"] + loss_slack
+    assert_pose(p6.cpu().numpy(), tr["og"]["pose"], tr["ex"]["pose"] + pose_slack / C_EXPO)
     # render + backward_tracking gives the same numbers as track_iter
     im2 = alloc_images(cam)
     ren.render(sf, c, **im2)

@@ -1,6 +1,9 @@
 """GPU parity: the CUDA path (through the C ABI binding) against the CPU oracle, element by element,
 on the same seeded inputs.  Bars (BASELINE.json north_star): binning bit-exact; images
-1e-4 rel / 1e-5 abs outside the oracle's fragile mask; gradients 1e-3 rel (+1e-3 RMS(group) floor)."""
+1e-4 rel / 1e-5 abs on every non-fragile pixel, fragile pixels within the oracle-derived allowance
+(oracle.pixel_bounds); EVERY gradient element within 1e-3 rel (+1e-3 RMS(group) floor) plus the oracle-derived
+exposure of the fragile pixels (oracle.exposure), which is zero for most elements and asserted small in total.
+Nothing the CUDA path produced is ever an input of the oracle."""
 import numpy as np
 import pytest
 import torch
@@ -13,7 +16,7 @@ pytestmark = pytest.mark.gpu
 
 sgs = pytest.importorskip("paper_2506_00970_b200")
 from gpu_common import (to_device, camera, alloc_images, planes, alloc_grads, split_upstream, image_check,  # noqa: E402
-                        grad_check)
+                        assert_image_check, assert_grads, assert_pose, tracking_reference, tracking_flips, tracking_slack, C_EXPO)
 
 
 @pytest.fixture(scope="module")
@@ -50,21 +53,8 @@ def assert_binning(gb, ob):
     assert np.array_equal(gb["ranges"], ob["ranges"])
 
 
-def assert_images(gpu_img, o):
-    chk = image_check(gpu_img, o["img"], o["fragile"])
-    assert chk["n_bad"] == 0, chk
-    assert chk["fragile_ok"], chk
-    assert chk["fragile_frac"] < 0.05, chk
-
-
-def assert_grads(g, og, max_bad=2e-3):
-    for k in ("mean", "scale", "quat", "opacity", "rgb"):
-        chk = grad_check(g[k], og[k])
-        assert chk["frac_bad"] <= max_bad, (k, chk)
-
-
-def assert_pose(p, op, rtol=1e-3):
-    assert np.abs(p - op).max() <= rtol * np.abs(op).max(), (p, op)
+def assert_images(gpu_img, o, sc, camv, cfg, ctx=None):
+    assert_image_check(image_check(gpu_img, o["img"], o["fragile"], oracle.pixel_bounds(sc, camv, cfg)), ctx)
 
 
 POSES = [None, [0.1, -0.2, 0.15, 0.2, -0.1, 0.3]]
@@ -81,26 +71,29 @@ def test_c1_full(ren, tau):
     out = run_gpu(ren, sc, cam, up, T_cw=T)
     assert_binning(out["bin"], oracle.binning(sc, camv, cfg))
     o = oracle.render(sc, camv, cfg)
-    assert_images(out["img"], o)
-    og = oracle.backward(sc, camv, cfg, up)
-    assert_grads(out["grads"], og)
-    assert_pose(out["pose"], og["pose"])
+    assert_images(out["img"], o, sc, camv, cfg)
+    og, ex = oracle.backward(sc, camv, cfg, up), oracle.exposure(sc, camv, cfg, up)
+    assert_grads(out["grads"], og, ex)
+    assert_pose(out["pose"], og["pose"], ex["pose"])
     # pose-only mode (per-pixel Eq. 11-13) against the same oracle
     out2 = run_gpu(ren, sc, cam, up, full=False, T_cw=T)
-    assert_pose(out2["pose"], og["pose"])
+    assert_pose(out2["pose"], og["pose"], ex["pose"])
 
 
 def test_c2_tracking_shape(ren):
-    """Config 2 (200k surfels, 640x480): binning, images, tracking loss (Eq. 15-19), pose-only backward."""
+    """Config 2 (200k surfels, 640x480): binning, images, tracking loss (Eq. 15-19), pose-only backward -- each stage on
+    the ORACLE's inputs: the loss kernel is run on the oracle's image (rounded to binary32), the backward on the oracle's
+    upstream gradients; the fused paths, which evaluate the loss on the renderer's own image, may differ from the oracle only
+    through masks / signs that sit inside the image bar (tracking_flips asserts that), by at most tracking_slack."""
     sc, cams, info = scenegen.make_config("C2")
     cam = cams[0]
     camv, cfg = oracle.make_cam(cam), oracle.make_cfg()
-    # target frame: the oracle's own render at the perturbed pose Exp(tau0) T
+    # target frame: the oracle's own render at the perturbed pose Exp(tau0) T, as binary32 (what the C ABI carries)
     g = scenegen.SplitMix(info["tau0_seed"])
     d = np.stack([g.normal(3), g.normal(3)])
     tau0 = np.concatenate([0.02 * d[0] / np.linalg.norm(d[0]), np.deg2rad(1.0) * d[1] / np.linalg.norm(d[1])])
     T_tgt = scenegen.perturb_pose(cam.T_cw, tau0)
-    tgt = oracle.render(sc, oracle.make_cam(cam, T_tgt), cfg, counters=False)["img"]
+    tgt = oracle.render(sc, oracle.make_cam(cam, T_tgt), cfg, counters=False)["img"].astype(np.float32).astype(np.float64)
     t, sf = to_device(sc)
     c = camera(cam)
     im, upi = alloc_images(cam), alloc_images(cam)
@@ -109,28 +102,43 @@ def test_c2_tracking_shape(ren):
     assert_binning(ren.get_binning(sc.n, tiles), oracle.binning(sc, camv, cfg))
     o = oracle.render(sc, camv, cfg)
     gimg = planes(im)
-    assert_images(gimg, o)
-    # loss kernel on the GPU's own images vs the numpy definition on the same images
+    assert_images(gimg, o, sc, camv, cfg)
+    tr = tracking_reference(sc, camv, cfg, o, tgt, 0.5, -1.0, oracle)
+    L_ref, up_ref, og = tr["L"], tr["up"], tr["og"]
+    assert (up_ref != 0).mean() > 0.05
     trgb = torch.from_numpy(tgt[0:3].astype(np.float32)).cuda()
     tdep = torch.from_numpy(tgt[3:4].astype(np.float32)).cuda()
+    # loss kernel on the ORACLE's image as binary32: same masks and signs except where the rounding of the image itself
+    # crosses a threshold (candidates only), same loss
+    o32 = o["img"].astype(np.float32)
+    oim = dict(rgb=torch.from_numpy(o32[0:3]).cuda(), depth=torch.from_numpy(o32[3:4]).cuda(),
+               normal=torch.from_numpy(o32[4:7]).cuda(), alpha=torch.from_numpy(o32[7:8]).cuda())
     loss = torch.zeros(1, device="cuda")
-    ren.tracking_loss(c, im, trgb, tdep, 0.5, -1.0, upi, loss)
-    L_ref, up_ref = oracle.tracking_loss(gimg, trgb.cpu().numpy(), tdep.cpu().numpy()[0], camv, 0.5, -1.0)
-    assert abs(float(loss.item()) - L_ref) <= 1e-4 * abs(L_ref)
-    up_gpu = planes(upi)
-    assert np.abs(up_gpu - up_ref).max() <= 1e-6 * np.abs(up_ref).max()
-    assert (up_ref != 0).mean() > 0.05
-    # pose-only backward on those upstream gradients vs the oracle's analytic backward
+    ren.tracking_loss(c, oim, trgb, tdep, 0.5, -1.0, upi, loss)
+    D0 = tracking_flips(tr, planes(upi))
+    assert D0.sum() <= 1e-4 * D0[0].size and abs(float(loss.item()) - L_ref) <= 1e-5 * abs(L_ref) + tracking_slack(sc, camv, cfg, tr, D0, oracle)[1]
+    same = ~D0.any(0)
+    assert np.abs(planes(upi) - up_ref)[:, same].max() <= 1e-6 * np.abs(up_ref).max()
+    # pose-only backward on the oracle's upstream gradients vs the oracle's analytic backward
+    u = torch.from_numpy(up_ref.astype(np.float32)).cuda()
+    og32 = oracle.backward(sc, camv, cfg, u.cpu().numpy().astype(np.float64))
     p6 = torch.zeros(6, device="cuda")
-    ren.backward(d_rgb=upi["rgb"], d_depth=upi["depth"], d_normal=upi["normal"], d_alpha=upi["alpha"], d_pose6=p6)
-    og = oracle.backward(sc, camv, cfg, up_gpu)
-    assert_pose(p6.cpu().numpy().astype(np.float64), og["pose"])
+    ren.backward(d_rgb=u[0:3].contiguous(), d_depth=u[3:4].contiguous(), d_normal=u[4:7].contiguous(),
+                 d_alpha=u[7:8].contiguous(), d_pose6=p6)
+    assert_pose(p6.cpu().numpy(), og32["pose"], tr["ex"]["pose"])
+    # the renderer's own loss on its own image: which masks / signs came out differently, and what that may change
+    ren.tracking_loss(c, im, trgb, tdep, 0.5, -1.0, upi, loss.zero_())
+    D = tracking_flips(tr, planes(upi))
+    pose_slack, loss_slack = tracking_slack(sc, camv, cfg, tr, D, oracle)
+    assert abs(float(loss.item()) - L_ref) <= tr["loss_tol"] + loss_slack
     # fused loss + backward (sgs_backward_tracking) == loss kernel followed by backward, and == the oracle
     p6f, lossf = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
     ren.backward_tracking(trgb, tdep, 0.5, -1.0, p6f, lossf)
-    assert abs(float(lossf.item()) - L_ref) <= 1e-4 * abs(L_ref)
-    assert_pose(p6f.cpu().numpy().astype(np.float64), og["pose"])
-    np.testing.assert_allclose(p6f.cpu().numpy(), p6.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(p6.abs().max()))
+    assert abs(float(lossf.item()) - L_ref) <= tr["loss_tol"] + loss_slack
+    assert_pose(p6f.cpu().numpy(), og["pose"], tr["ex"]["pose"] + pose_slack / C_EXPO)
+    p6u = torch.zeros(6, device="cuda")
+    ren.backward(d_rgb=upi["rgb"], d_depth=upi["depth"], d_normal=upi["normal"], d_alpha=upi["alpha"], d_pose6=p6u)
+    np.testing.assert_allclose(p6f.cpu().numpy(), p6u.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(p6u.abs().max()))
 
 
 def test_backward_is_repeatable_and_overwrites(ren):
@@ -194,10 +202,10 @@ def test_edge_cases(ren):
     ob = oracle.binning(sc, camv, cfg)
     assert_binning(out["bin"], ob)
     assert ob["culled"][5] and ob["culled"][6]
-    assert_images(out["img"], oracle.render(sc, camv, cfg))
-    og = oracle.backward(sc, camv, cfg, up)
-    assert_grads(out["grads"], og, max_bad=5e-3)
-    assert_pose(out["pose"], og["pose"])
+    assert_images(out["img"], oracle.render(sc, camv, cfg), sc, camv, cfg)
+    og, ex = oracle.backward(sc, camv, cfg, up), oracle.exposure(sc, camv, cfg, up)
+    assert_grads(out["grads"], og, ex)
+    assert_pose(out["pose"], og["pose"], ex["pose"])
 
 
 def test_invalid_arguments(ren):
@@ -250,10 +258,12 @@ def test_async_mode_and_host_path():
     sync.close(); a.close()
 
 
-def test_radix_binning_path_gives_the_same_list():
+@pytest.mark.parametrize("name,n_override", [("C2", 60000), ("C3", None)])
+def test_radix_binning_path_gives_the_same_list(name, n_override):
     """SGS_FLAG_RADIX_BINNING (global LSD radix sort of the 64-bit tile|depth keys) and the default
-    per-tile buckets + in-tile sort produce the identical sorted list, images and gradients."""
-    sc, cams, _ = scenegen.make_config("C2", n_override=60000)
+    per-tile buckets + in-tile sort produce the identical sorted list, images and gradients -- on a small map and on C3
+    view 0 at full size (3225 tiles = 12 tile bits, E = 0.74 M: multi-tile look-back chains in every pass)."""
+    sc, cams, _ = scenegen.make_config(name, n_override=n_override) if n_override else scenegen.make_config(name)
     cam = cams[0]
     up = scenegen.upstream_normal(8, cam.height, cam.width)
     a, b = sgs.Renderer(), sgs.Renderer(radix_binning=True)
@@ -265,6 +275,43 @@ def test_radix_binning_path_gives_the_same_list():
     for k in ra["grads"]:
         np.testing.assert_allclose(ra["grads"][k], rb["grads"][k], rtol=1e-3, atol=1e-4 * np.abs(ra["grads"][k]).max())
     a.close(); b.close()
+
+
+def test_track_helpers_wait_for_their_owner(monkeypatch):
+    """K-track's helper blocks (second half of the walk back of the 32 longest tile lists) read the tile's bucket only
+    after the owner block has published the SORTED keys, and the hand-over flags are built from a device-side epoch.  With
+    every helper delayed by 0.2 ms (SGS_DEBUG_HELPER_DELAY_NS: the owners are long past their sort, mid-way through their
+    walks) and over several back-to-back iterations the pose gradient, loss, images and binning equal those of an
+    undelayed context -- a helper that ranked a half-permuted bucket, or met a stale flag, would not."""
+    sc, cams, info = scenegen.make_config("C2")
+    cam = cams[0]
+    camv, cfg = oracle.make_cam(cam), oracle.make_cfg()
+    ob = oracle.binning(sc, camv, cfg)
+    lens = ob["ranges"][:, 1].astype(np.int64) - ob["ranges"][:, 0]
+    assert (lens > 160).sum() >= 4 and lens.max() <= 384          # tiles that split between owner and helper exist
+    t, sf = to_device(sc)
+    c = camera(cam)
+    tiles = ((cam.width + 15) // 16) * ((cam.height + 15) // 16)
+    ref = sgs.Renderer()
+    im0 = alloc_images(cam)
+    ref.render(sf, c, **im0)
+    tgt_rgb, tgt_dep = (im0["rgb"] * 0.9 + 0.01).contiguous(), (im0["depth"] * 1.02).contiguous()
+    pr, lr = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+    for _ in range(3):
+        ref.track_iter(sf, c, tgt_rgb, tgt_dep, 0.5, -1.0, pr, lr)
+    monkeypatch.setenv("SGS_DEBUG_HELPER_DELAY_NS", "200000")
+    slow = sgs.Renderer()
+    monkeypatch.delenv("SGS_DEBUG_HELPER_DELAY_NS")
+    for it in range(4):
+        im = alloc_images(cam)
+        p6, loss = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+        slow.track_iter(sf, c, tgt_rgb, tgt_dep, 0.5, -1.0, p6, loss, **im)
+        torch.cuda.synchronize()
+        assert np.array_equal(planes(im), planes(im0))
+        np.testing.assert_allclose(loss.cpu().numpy(), lr.cpu().numpy(), rtol=1e-5)
+        np.testing.assert_allclose(p6.cpu().numpy(), pr.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(pr.abs().max()))
+    assert_binning(slow.get_binning(sc.n, tiles), ob)
+    ref.close(); slow.close()
 
 
 def test_tile_bucket_overflow_grows(ren):
@@ -281,7 +328,7 @@ def test_tile_bucket_overflow_grows(ren):
     ob = oracle.binning(sc, camv, cfg)
     assert (ob["ranges"][:, 1] - ob["ranges"][:, 0]).max() > 2048
     assert_binning(out["bin"], ob)
-    assert_images(out["img"], oracle.render(sc, camv, cfg))
+    assert_images(out["img"], oracle.render(sc, camv, cfg), sc, camv, cfg)
     a = sgs.Renderer(async_mode=True)
     t, sf = to_device(sc)
     im = alloc_images(cam)
@@ -368,7 +415,7 @@ def test_random_poses_binning_and_images(ren):
         ob = oracle.binning(sc, camv, cfg)
         assert ob["E"] > 1000
         assert_binning(ren.get_binning(sc.n, tiles), ob)
-        assert_images(planes(im), oracle.render(sc, camv, cfg))
+        assert_images(planes(im), oracle.render(sc, camv, cfg), sc, camv, cfg, k)
 
 
 @pytest.mark.parametrize("reuse", [False, True])
@@ -425,13 +472,15 @@ def test_stress_scene_masks_stay_conservative(ren):
         out = run_gpu(ren, sc, cam, up, T_cw=T)
         assert_binning(out["bin"], oracle.binning(sc, camv, cfg))
         o = oracle.render(sc, camv, cfg)
-        chk = image_check(out["img"], o["img"], o["fragile"])
-        assert chk["n_bad"] == 0 and chk["fragile_ok"] and chk["fragile_frac"] < 0.12, chk
-        og = oracle.backward(sc, camv, cfg, up)
-        assert_grads(out["grads"], og, max_bad=5e-3)
-        assert_pose(out["pose"], og["pose"], rtol=2e-3)
+        chk = image_check(out["img"], o["img"], o["fragile"], oracle.pixel_bounds(sc, camv, cfg))
+        # (this scene is BUILT of edge-on splats and slivers: 5-6 % of its pixels hold a pair with kappa > 32, so the
+        # fragile fraction is the scene's, not the renderer's; the bound on those pixels is still the derived one)
+        assert chk["n_bad"] == 0 and chk["n_bad_fragile"] == 0 and chk["fragile_frac"] < 0.08, chk
+        og, ex = oracle.backward(sc, camv, cfg, up), oracle.exposure(sc, camv, cfg, up)
+        assert_grads(out["grads"], og, ex)
+        assert_pose(out["pose"], og["pose"], ex["pose"])
         out2 = run_gpu(ren, sc, cam, up, full=False, T_cw=T)
-        assert_pose(out2["pose"], og["pose"], rtol=2e-3)
+        assert_pose(out2["pose"], og["pose"], ex["pose"])
     r2 = sgs.Renderer()
     t, sf = to_device(sc)
     c = camera(cam)

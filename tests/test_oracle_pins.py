@@ -219,6 +219,41 @@ def test_p7_binning_structure_and_conservativeness(c1):
     assert n_cover >= r["counters"]["cover"] > 0   # z>z_near and culling only remove pairs
 
 
+def test_p7b_tile_rect_is_tight_and_conservative():
+    """P7b.  The tile rectangle is exactly the set of tiles the screen AABB touches: floor(aabb / 16) clamped to the grid
+    (O2 (iv)), checked (i) against that definition recomputed here from the exported AABB (itself pinned against the
+    forward-mapped cutoff circle in P7), and (ii) geometrically without any floor: every listed tile's square meets the AABB,
+    and no tile next to the rectangle does.  A ceil-for-floor, an off-by-one or a missing clamp fails here.  C1 seen by a
+    200 x 120 camera: 13 x 8 tiles, ragged on both axes (200 = 12.5, 120 = 7.5 tiles), many splats crossing the border."""
+    sc, _, _ = scenegen.make_config("C1")
+    cam = Camera(200, 120, 150.0, 150.0, 97.0, 63.0, scenegen.perturb_pose(np.eye(4)[:3], [0.05, -0.02, 0.1, 0.03, 0.05, -0.2]))
+    camv, cfg = oracle.make_cam(cam), oracle.make_cfg()
+    b = oracle.binning(sc, camv, cfg)
+    tx, ty = b["tiles_x"], b["tiles_y"]
+    assert (tx, ty) == (13, 8)
+    vis = np.nonzero(b["culled"] == 0)[0]
+    assert len(vis) > 500
+    aabb, rect = b["aabb"][vis], b["rect"][vis]
+    want = np.stack([np.clip(np.floor(aabb[:, 0] / 16), 0, tx - 1), np.clip(np.floor(aabb[:, 2] / 16), 0, ty - 1),
+                     np.clip(np.floor(aabb[:, 1] / 16), 0, tx - 1), np.clip(np.floor(aabb[:, 3] / 16), 0, ty - 1)], 1)
+    np.testing.assert_array_equal(rect, want.astype(np.int32))
+    assert np.array_equal(b["count"][vis], (rect[:, 2] - rect[:, 0] + 1) * (rect[:, 3] - rect[:, 1] + 1))
+    clipped = 0
+    for (x0, x1, y0, y1), (rx0, ry0, rx1, ry1) in zip(aabb, rect):
+        meets_x = lambda t: 16 * t <= x1 and 16 * (t + 1) > x0        # tile column [16 t, 16 t + 16) meets [x0, x1]
+        meets_y = lambda t: 16 * t <= y1 and 16 * (t + 1) > y0
+        assert all(meets_x(t) for t in range(rx0, rx1 + 1)) and all(meets_y(t) for t in range(ry0, ry1 + 1))
+        assert not any(meets_x(t) for t in (rx0 - 1, rx1 + 1) if 0 <= t < tx)      # tight: the neighbours do not
+        assert not any(meets_y(t) for t in (ry0 - 1, ry1 + 1) if 0 <= t < ty)
+        clipped += (x0 < 0) or (y0 < 0) or (x1 >= 200) or (y1 >= 120)
+    assert clipped > 20                                   # the clamp is exercised
+    # the list is the rectangles, written out: per tile, exactly the splats whose rectangle holds the tile
+    for t in (0, 5, tx - 1, tx * 3 + 6, tx * ty - 1):
+        s0, e0 = b["ranges"][t]
+        inside = vis[(rect[:, 0] <= t % tx) & (t % tx <= rect[:, 2]) & (rect[:, 1] <= t // tx) & (t // tx <= rect[:, 3])]
+        assert sorted(b["idx"][s0:e0].tolist()) == sorted(inside.tolist())
+
+
 def test_p7_full_forward_against_library_inverse(c1):
     """Whole forward against an independent numpy render: library matrix inverse for (u,v),
     cumulative product for the transmittance (Eq. 8 written as array ops)."""
@@ -270,9 +305,18 @@ def _loss(sc, camv, cfg, up):
     return float((r(sc, camv, cfg, counters=False)["img"] * up).sum())
 
 
-def _fd_check(cfg, rtol):
-    sc, cam = _tiny()
+def _decisions(sc, camv, cfg):
+    r = oracle.render(sc, camv, cfg, counters=False)
+    return r["n_comp"]
+
+
+def _fd_check(cfg, rtol, scene=None, guard=False, hexp=-12):
+    """guard: the truncation rules make the image piecewise smooth; a central difference is the derivative of the current
+    piece only if no discrete decision changes between the two evaluations -- asserted through the per-pixel count of
+    composited splats (a skip <-> composite or a stop flip changes it)."""
+    sc, cam = scene if scene is not None else _tiny()
     camv = oracle.make_cam(cam, widen_from_f32=False)
+    n0 = _decisions(sc, camv, cfg) if guard else None
     up = scenegen.upstream_normal(11, cam.height, cam.width).astype(np.float64)
     g = (oracle.backward_normalised if _NORMALISED[0] else oracle.backward)(sc, camv, cfg, up)
     worst = 0.0
@@ -283,10 +327,12 @@ def _fd_check(cfg, rtol):
         scale_ref = np.abs(ga).max() + 1e-30
         for e in range(flat.size):
             x0 = flat[e]
-            h = np.float32(max(abs(float(x0)), 0.05) * 2.0 ** -12)
+            h = np.float32(max(abs(float(x0)), 0.05) * 2.0 ** hexp)
             xp, xm = np.float32(x0 + h), np.float32(x0 - h)
             flat[e] = xp; lp = _loss(sc, camv, cfg, up)
+            if guard: assert np.array_equal(_decisions(sc, camv, cfg), n0), (name, e, "+h crosses a decision")
             flat[e] = xm; lm = _loss(sc, camv, cfg, up)
+            if guard: assert np.array_equal(_decisions(sc, camv, cfg), n0), (name, e, "-h crosses a decision")
             flat[e] = x0
             fd = (lp - lm) / (float(xp) - float(xm))          # exact step between two float32 inputs
             err = abs(fd - ga[e]) / scale_ref
@@ -296,8 +342,9 @@ def _fd_check(cfg, rtol):
     eps = 1e-6
     for i in range(6):
         tau = np.zeros(6); tau[i] = eps
-        lp = _loss(sc, oracle.make_cam(cam, scenegen.perturb_pose(cam.T_cw, tau), False), cfg, up)
-        lm = _loss(sc, oracle.make_cam(cam, scenegen.perturb_pose(cam.T_cw, -tau), False), cfg, up)
+        cp, cm = (oracle.make_cam(cam, scenegen.perturb_pose(cam.T_cw, s_ * tau), False) for s_ in (1, -1))
+        lp, lm = _loss(sc, cp, cfg, up), _loss(sc, cm, cfg, up)
+        if guard: assert np.array_equal(_decisions(sc, cp, cfg), n0) and np.array_equal(_decisions(sc, cm, cfg), n0), i
         fd = (lp - lm) / (2 * eps)
         assert abs(fd - g["pose"][i]) < rtol * np.abs(g["pose"]).max(), (i, fd, g["pose"])
     return worst
@@ -315,6 +362,115 @@ def test_p8_finite_differences_alpha_clamp():
     r = oracle.render(sc, oracle.make_cam(cam, widen_from_f32=False), cfg)
     assert (r["fragile"] & 2).sum() == 0, "pick another seed: a pixel sits on the clamp boundary"
     _fd_check(cfg, 2e-6)
+
+
+def _stacked(seed=3):
+    """A tiny scene on which EVERY truncation rule of Eq. 8 (R3-R7) acts: three nearly opaque splats stacked on the axis
+    (pixels behind them stop: T (1 - a) < 1e-4), splats behind the stack (cut off by the stop), a faint splat (o = 0.2: the
+    a >= 1/255 test bites inside the cutoff), splat rims inside the image (rho^2 = 9), opacities above alpha_max = 0.99's
+    reach (o G clamped), and a small tilted splat whose near side dips under z_near = 0.2."""
+    g = scenegen.SplitMix(seed)
+    n = 9
+    mean = np.array([[0.02, 0.01, 0.9], [-0.03, 0.02, 1.0], [0.01, -0.02, 1.1], [0.05, 0.03, 1.3], [-0.2, 0.1, 1.4],
+                     [0.25, -0.12, 1.2], [-0.1, -0.15, 0.8], [0.03, 0.02, 0.27], [0.15, 0.12, 1.6]])
+    scale = np.array([[0.12, 0.1], [0.11, 0.13], [0.14, 0.1], [0.2, 0.18], [0.1, 0.08], [0.09, 0.12], [0.07, 0.1], [0.05, 0.045],
+                      [0.16, 0.2]])
+    opac = np.array([0.995, 0.985, 0.98, 0.9, 0.2, 0.7, 0.5, 0.6, 0.95])
+    quat = np.stack([g.normal(n) for _ in range(4)], 1) * 0.25
+    quat[:, 0] += 1.5
+    quat[7] = [0.55, 0.8, 0.15, 0.1]       # the near splat: tilted ~ 110 deg about x, so its far side rises and its near side dips
+    rgb = np.stack([g.uniform(n) for _ in range(3)], 1)
+    sc = Scene(mean.astype(np.float32), scale.astype(np.float32), quat.astype(np.float32), opac.astype(np.float32),
+               rgb.astype(np.float32))
+    cam = Camera(16, 12, 14.0, 15.0, 8.3, 5.6, scenegen.perturb_pose(np.eye(4)[:3], [0.01, -0.02, 0.02, 0.02, -0.015, 0.03]))
+    # the front splat is fully opaque and centred on pixel (8, 6): there o G = 1 > alpha_max, the clamp acts
+    T = np.asarray(cam.T_cw, dtype=np.float64)
+    Xc = np.array([(8.5 - 8.3) / 14.0 * 0.9, (6.5 - 5.6) / 15.0 * 0.9, 0.9])
+    sc.mean[0] = (T[:, :3].T @ (Xc - T[:, 3])).astype(np.float32)
+    sc.opacity[0] = 1.0
+    return sc, cam
+
+
+def test_p8b_finite_differences_with_every_truncation_rule_active():
+    """P8b.  Central finite differences of every surfel gradient and of the SE(3) pose gradient under the DEFAULT config
+    (cutoff 3, alpha_min, alpha_max, T_min stop, z_near): pins the backward's replay loop -- which pairs it revisits, that the
+    stopping splat and everything behind it get nothing, the clamp's zero derivative.  The scene is checked to exercise
+    each rule (switching the rule off changes the image), to have pixels that stop, and to have no fragile pixel; the
+    guard in _fd_check asserts that no decision flips inside a difference."""
+    sc, cam = _stacked()
+    camv = oracle.make_cam(cam, widen_from_f32=False)
+    cfg = oracle.make_cfg()
+    r = oracle.render(sc, camv, cfg)
+    assert (r["fragile"] != 0).sum() == 0, "a pixel sits within 1e-4 of a threshold: move a splat"
+    assert (r["T_final"] < 1e-2).sum() >= 4 and r["counters"]["Q_t"] > r["counters"]["Q_tb"]   # pixels that stop early
+    base = r["img"]
+    for name, kw in (("cutoff", dict(cutoff=12.0)), ("alpha_min", dict(alpha_min=0.0)), ("alpha_max", dict(alpha_max=0.99999)),
+                     ("t_min", dict(t_min=0.0)), ("z_near", dict(z_near=1e-3))):
+        other = oracle.render(sc, camv, oracle.make_cfg(**kw), counters=False)["img"]
+        assert np.abs(other - base).max() > 1e-6, name + " never acts on this scene"
+    # the stop is not a no-op for the gradient either: splats behind the stack get less than without it
+    up = scenegen.upstream_normal(11, cam.height, cam.width).astype(np.float64)
+    g1, g0 = oracle.backward(sc, camv, cfg, up), oracle.backward(sc, camv, oracle.make_cfg(t_min=0.0), up)
+    assert np.abs(g1["rgb"] - g0["rgb"]).max() > 1e-9
+    _fd_check(cfg, 1e-5, scene=(sc, cam), guard=True, hexp=-19)
+
+
+def test_comparison_support_is_pinned_to_the_backward(c1):
+    """oracle.exposure / oracle.pixel_bounds only feed the tolerance of the GPU parity tests, but a wrong bound would hide
+    errors.  (i) signed_all: the exposure's own pair-by-pair chain recomputes the whole gradient and must equal
+    oracle.backward.  (ii) With every pixel handed in as `extra_mask` the result dominates |backward| (sum of |.| >= |sum|).
+    (iii) A pixel is exposed iff the forward marks it fragile (or the mask names it); zero upstream there gives zero.
+    (iv) A constructed flip: one fronto-parallel splat and alpha_min set 5e-5 below the closed-form alpha of ONE pixel:
+    that pixel is the only exposed one, inverting its decision removes its whole contribution, so the exposure of the
+    colour gradient is |g| a and of the opacity gradient |g . v| G there -- hand values.  (v) pixel_bounds: flip_w is
+    positive only on decision-fragile pixels and equals a T of the pair at stake in (iv); kappa = 1 for a fronto-parallel
+    splat, so kerr = w rho^2 in closed form; zmax >= the blended depth."""
+    sc, cam, camv, cfg, r = c1
+    up = scenegen.upstream_normal(1, cam.height, cam.width)
+    g = oracle.backward(sc, camv, cfg, up)
+    e = oracle.exposure(sc, camv, cfg, up, signed_all=True)
+    for k in ("mean", "scale", "quat", "opacity", "rgb", "pose"):
+        np.testing.assert_allclose(e[k], g[k], rtol=1e-9, atol=1e-9 * np.abs(g[k]).max())
+    full = oracle.exposure(sc, camv, cfg, up, extra_mask=np.ones((cam.height, cam.width), np.uint8))
+    for k in ("mean", "scale", "quat", "opacity", "rgb"):
+        assert (full[k] >= np.abs(g[k]) * (1 - 1e-9) - 1e-12).all(), k
+    a = oracle.exposure(sc, camv, cfg, up)
+    assert np.array_equal(a["pix_exposed"] != 0, r["fragile"] != 0) and (r["fragile"] != 0).sum() > 3
+    assert all((a[k] <= full[k] * (1 + 1e-9) + 1e-12).all() for k in ("mean", "scale", "quat", "opacity", "rgb"))
+    none = oracle.exposure(sc, camv, cfg, up * (a["pix_exposed"] == 0)[None])    # zero upstream on every exposed pixel
+    assert all(np.abs(none[k]).max() == 0 for k in ("mean", "scale", "quat", "opacity", "rgb", "pose"))
+    extra = np.zeros((cam.height, cam.width), np.uint8); extra[10:20, 10:30] = 1
+    b = oracle.exposure(sc, camv, cfg, up, extra_mask=extra)
+    assert ((b["pix_exposed"] != 0) == ((r["fragile"] != 0) | (extra != 0))).all() and b["rgb"].sum() > a["rgb"].sum()
+    pb = oracle.pixel_bounds(sc, camv, cfg)
+    assert ((pb["flip_w"] > 0) <= ((r["fragile"] & 1) != 0)).all() and (pb["flip_w"] > 0).sum() > 0
+    assert (pb["flip_w"] <= 2.0 + 1e-12).all() and (pb["kerr"] >= 0).all() and (pb["kerr_z"] >= 0).all()
+    comp = r["n_comp"] > 0
+    assert (pb["zmax"][comp] >= (r["img"][3][comp] / r["img"][7][comp]) * (1 - 1e-12)).all()   # max depth >= mean depth
+    # (iv), (v) on one fronto-parallel splat with closed-form alpha (P1)
+    mu, su, sv, o = (0.31, -0.17, 1.5), float(np.float32(0.11)), float(np.float32(0.07)), float(np.float32(0.8))
+    one = one_surfel(mu, (su, sv), (1, 0, 0, 0), o)
+    mu32 = np.float32(mu).astype(np.float64)
+    X, Y = pix_grid(CAM)
+    u = ((X - CAM.cx) * mu32[2] / CAM.fx - mu32[0]) / su; v = ((Y - CAM.cy) * mu32[2] / CAM.fy - mu32[1]) / sv
+    G = np.exp(-(u * u + v * v) / 2); al = o * G
+    jj, ii = np.unravel_index(np.argmin(np.abs(al - 0.05)), al.shape)       # a pixel on the splat's flank
+    cfg1 = oracle.make_cfg(alpha_min=al[jj, ii] / (1 + 5e-5))
+    camv1 = oracle.make_cam(CAM)
+    up1 = scenegen.upstream_normal(5, CAM.height, CAM.width)
+    r1 = oracle.render(one, camv1, cfg1)
+    assert (r1["fragile"] != 0).sum() == 1 and r1["fragile"][jj, ii] == 1 and r1["img"][7][jj, ii] > 0
+    x1 = oracle.exposure(one, camv1, cfg1, up1)
+    gpix = up1[:, jj, ii]
+    np.testing.assert_allclose(x1["rgb"][0], np.abs(gpix[0:3]) * al[jj, ii], rtol=1e-9)
+    rgb1 = one.rgb[0].astype(np.float64)
+    gv = gpix[0:3] @ rgb1 + gpix[3] * mu32[2] + gpix[6] * 1.0 + gpix[7]      # v = (rgb, z0, n = +z, 1); T = 1, no suffix
+    np.testing.assert_allclose(x1["opacity"][0], abs(gv) * G[jj, ii], rtol=1e-9)
+    pb1 = oracle.pixel_bounds(one, camv1, cfg1)
+    assert (pb1["flip_w"] > 0).sum() == 1 and abs(pb1["flip_w"][jj, ii] - al[jj, ii]) < 1e-12
+    w1 = r1["img"][7]
+    np.testing.assert_allclose(pb1["kerr"], w1 * (u * u + v * v), atol=1e-9)
+    np.testing.assert_allclose(pb1["kerr_z"], 0.0, atol=1e-12)               # fronto-parallel: M20 = M21 = 0
 
 
 # ---------------------------------------------------------------- P9: rigid-motion identity (no FD)
@@ -454,7 +610,7 @@ def test_p12_tracking_loss_hand_example_masks_and_gradient():
     img[6] = [[1.0, 1.0], [-1.0, 1.0]]                  # N_r = (0, 0, +-1): N.r = +-1 for every ray (r_z = 1)
     img[7] = [[0.99, 0.9], [0.99, 0.96]]
     trgb = np.zeros((3, 2, 2)); trgb[:, 0, 0] = [0.4, 0.3, 0.0]; trgb[:, 1, 1] = [1.0, 0.1, 0.6]
-    tdep = np.array([[2.5, 0.0], [0.0, 2.0]])
+    tdep = np.array([[2.5, 0.0], [3.0, 2.0]])
     L, up = oracle.tracking_loss(img, trgb, tdep, camv, 0.5, 1.0)
     # (0,0): |0.1| + |-0.2| + 0 + 0.5 |-0.5| = 0.55 ; (1,1): |-0.1| + |0.3| + 0 + 0.5 |1.0| = 0.9
     assert abs(L - (0.55 + 0.9) / 4) < 1e-15
@@ -463,7 +619,30 @@ def test_p12_tracking_loss_hand_example_masks_and_gradient():
     np.testing.assert_allclose(up[0:4, 1, 1], np.array([-1, 1, 0, 0.5]) / 4)
     # the other sign convention (R19) swaps which pixels pass M_n
     L2, _ = oracle.tracking_loss(img, trgb, tdep, camv, 0.5, -1.0)
-    assert abs(L2 - (0.3 + 0.3 + 0.3 + 0.5 * 1.5) / 4) < 1e-15     # only (0,1): rgb 0.3 each, depth 1.5
+    assert abs(L2 - (0.3 + 0.3 + 0.3 + 0.5 * 1.5) / 4) < 1e-15     # only (0,1): rgb 0.3 each, depth |1.5 - 3.0|
+
+
+def test_p12_p13_holes_in_the_sensor_depth_carry_no_depth_term():
+    """Reading R25: a pixel whose target depth is a hole (0, negative, inf, NaN -- how RGB-D sensors encode "no
+    measurement", L350) contributes its colour term only: hand values on a 2x2 frame, for Eq. 19 and for Eq. 26."""
+    cam = Camera(2, 2, 1.0, 1.0, 1.0, 1.0)
+    camv = oracle.make_cam(cam)
+    img = np.zeros((8, 2, 2))
+    img[0] = [[0.5, 0.25], [0.75, 1.0]]                   # only the red channel differs from the (zero) target
+    img[3] = [[2.0, 1.0], [1.5, 3.0]]
+    img[6] = 1.0; img[7] = 0.99                           # every pixel passes M_n and M_o
+    trgb = np.zeros((3, 2, 2))
+    for hole in (0.0, -1.0, np.inf, np.nan):
+        tdep = np.array([[2.5, hole], [hole, 2.0]])
+        L, up = oracle.tracking_loss(img, trgb, tdep, camv, 0.5, 1.0)
+        # colour: 0.5 + 0.25 + 0.75 + 1.0 = 2.5; depth only at (0,0) and (1,1): 0.5 (0.5 + 1.0)
+        assert abs(L - (2.5 + 0.5 * 1.5) / 4) < 1e-15, hole
+        np.testing.assert_array_equal(up[3], np.array([[-0.5, 0.0], [0.0, 0.5]]) / 4)
+        np.testing.assert_array_equal(up[0], np.full((2, 2), 0.25))
+        Lm, upm = oracle.mapping_loss(img, trgb, tdep, camv, 0.875, 0.5, 0.0, 1.0)   # w_n = 0: no normal term
+        assert abs(Lm - (0.875 * 2.5 + 0.5 * 1.5) / 4) < 1e-15, hole
+        np.testing.assert_array_equal(upm[3], np.array([[-0.5, 0.0], [0.0, 0.5]]) / 4)
+        assert np.isfinite(up).all() and np.isfinite(upm).all()
 
 
 def test_p12_tracking_loss_gradient_is_its_finite_difference(c1):
