@@ -26,7 +26,7 @@
  *     not flipped, not normalised), alpha = sum w (R9, R10).
  *   - Pose gradient: d_pose6 = (dL/drho, dL/dtheta) for the left perturbation
  *     T <- Exp(tau) o T_cw, tau = (rho, theta), translation first (Eq. 12-13, R15).
- *   - Gradients are OVERWRITTEN, and are exactly zero for inactive or culled surfels.
+ *   - Gradients are OVERWRITTEN, and are exactly zero for inactive or culled surfels (sgs_backward_accumulate adds).
  */
 #ifndef SGS_H
 #define SGS_H
@@ -148,6 +148,8 @@ enum { SGS_STAGE_PREPROCESS = 0, SGS_STAGE_SORT = 1, SGS_STAGE_FORWARD = 2, SGS_
        SGS_STAGE_BACKWARD = 4, SGS_STAGE_TRACK = 5 /* sgs_track_iter's fused kernel */, SGS_STAGE_COUNT = 6 };
 
 SGS_API int sgs_default_config(sgs_config* cfg);
+/* (Test hook: if the environment variable SGS_DEBUG_HELPER_DELAY_NS is set when the ctx is created, the helper blocks of
+ * sgs_track_iter's kernel sleep that many nanoseconds before they start -- results must not depend on it.) */
 SGS_API int sgs_create(sgs_ctx** out, const sgs_config* cfg);
 SGS_API int sgs_destroy(sgs_ctx* ctx);
 
@@ -204,6 +206,19 @@ SGS_API int sgs_covisibility(sgs_ctx* ctx, const float* contrib_a, const float* 
  * SGS_WORKSPACE_OVERFLOW (async mode: that render had overflowed; render again), SGS_OUT_OF_MEMORY, SGS_CUDA_ERROR. */
 SGS_API int sgs_backward(sgs_ctx* ctx, const sgs_images* upstream, const sgs_surfel_grads* d_surfels, float* d_pose6,
                  void* cuda_stream);
+
+/* sgs_backward that ADDS this view's surfel gradients to d_surfels instead of overwriting them: the paper's mapping
+ * iteration samples N_a + N_i keyframes and takes ONE optimiser step on their summed loss (L248-252, Tab. I), so
+ * the gradients of a window of views are a sum.  Nothing is zero-filled (sgs_backward's five N-sized memsets and its write of
+ * all N x 13 values go away; only the splats a view sees are touched): the caller zeroes d_surfels once per window
+ * (sgs_zero_grads, or its own memset).  d_pose6 is still OVERWRITTEN: every view has its own pose.  d_surfels must not be
+ * NULL.  Calls of one window must be ordered (same stream, or one ctx under SGS_FLAG_LAZY_GRADS); two contexts working on
+ * one window need an accumulator each.  Other arguments, state and errors as sgs_backward. */
+SGS_API int sgs_backward_accumulate(sgs_ctx* ctx, const sgs_images* upstream, const sgs_surfel_grads* d_surfels,
+                                    float* d_pose6, void* cuda_stream);
+
+/* Zero-fills the non-NULL arrays of d_surfels (n surfels) on the stream: the start of an accumulation window. */
+SGS_API int sgs_zero_grads(sgs_ctx* ctx, const sgs_surfel_grads* d_surfels, int64_t n, void* cuda_stream);
 
 /* SGS_FLAG_LAZY_GRADS.  The last kernel of a full sgs_backward (per-surfel chain rule Eq. 9-10, pose reduction Eq. 13,
  * latency-bound) then stays on a stream of the ctx and `cuda_stream` does not wait for it, so that the next view's
@@ -296,6 +311,22 @@ SGS_API int sgs_upload_target(sgs_ctx* ctx, const sgs_camera* cam, const float* 
                       const float* host_depth /*HxW*/, void* cuda_stream);
 SGS_API int sgs_track_iter_host(sgs_ctx* ctx, const sgs_camera* cam, float lambda_d, float normal_sign,
                         float* host_loss, float* host_d_pose6, void* cuda_stream);
+
+/* Mapping window on the resident map through HOST buffers (L234-252: per sampled keyframe render, Eq. 24-26 loss, full
+ * backward; one optimiser step per window).  sgs_map_view_host uploads the keyframe (HOST rgb 3xHxW, depth HxW; pinned memory
+ * keeps the copy asynchronous), renders the resident map, evaluates L = Eq. 24-26 (sgs_mapping_loss(lambda_c, w_d, w_n) +
+ * sgs_ssim_loss(ssim_weight); ssim_weight 0 skips the SSIM term) and ADDS the view's surfel gradients to the ctx's window
+ * accumulator on the device.  Nothing waits: *host_loss (1 float, nullable) and host_pose6 (6 floats, nullable; this view's
+ * dL/dtau) are written by sgs_sync_host.  At most 64 views between two sgs_sync_host calls (SGS_INVALID_ARGUMENT beyond).
+ * sgs_fetch_grads_host ends the window: the accumulated gradients are copied to host_d_surfels (HOST, n x {3,2,4,1,3} floats,
+ * NULL arrays skipped) on a stream of the ctx behind the window's last kernel, the accumulator is re-zeroed behind the copy,
+ * and the next window fills a second accumulator meanwhile; the host arrays are complete after sgs_sync_host, which waits
+ * for `cuda_stream` and for the ctx's copies and delivers the pending per-view results. */
+SGS_API int sgs_map_view_host(sgs_ctx* ctx, const sgs_camera* cam, const float* host_target_rgb, const float* host_target_depth,
+                              float lambda_c, float w_d, float w_n, float ssim_weight, float normal_sign, float* host_loss,
+                              float* host_pose6, void* cuda_stream);
+SGS_API int sgs_fetch_grads_host(sgs_ctx* ctx, const sgs_surfel_grads* host_d_surfels, void* cuda_stream);
+SGS_API int sgs_sync_host(sgs_ctx* ctx, void* cuda_stream);
 
 /* SSIM term of the colour loss (Eq. 24; reading R24): per channel the structural similarity index of [87],
  * 11 x 11 Gaussian window (sigma 1.5), zero padding, C1 = 0.01^2, C2 = 0.03^2;

@@ -56,7 +56,8 @@ class sgs_stats(C.Structure):
 
 EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_prepare", "sgs_backward", "sgs_wait_grads", "sgs_tracking_loss",
            "sgs_backward_tracking", "sgs_track_iter", "sgs_track_new_frame", "sgs_render_contrib", "sgs_render_median", "sgs_covisibility", "sgs_mapping_loss", "sgs_ssim_loss", "sgs_map_correction", "sgs_measure_fp32_peak", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
-           "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string"]
+           "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string",
+           "sgs_backward_accumulate", "sgs_zero_grads", "sgs_map_view_host", "sgs_fetch_grads_host", "sgs_sync_host"]
 
 _lib = None
 _LIVE = weakref.WeakSet()
@@ -234,17 +235,52 @@ class Renderer:
                                          _ptr(active, torch.uint8), C.c_float(threshold), _ptr(result3),
                                          _stream_ptr(stream)), "sgs_covisibility")
 
-    def backward(self, d_rgb=None, d_depth=None, d_normal=None, d_alpha=None, grads=None, d_pose6=None, stream=None):
+    @staticmethod
+    def _grads(grads, device_type="cuda"):
+        g = sgs_surfel_grads()
+        p = lambda t: _ptr(t, torch.float32, device_type)
+        g.mean, g.scale, g.quat = p(grads.get("mean")), p(grads.get("scale")), p(grads.get("quat"))
+        g.opacity, g.rgb = p(grads.get("opacity")), p(grads.get("rgb"))
+        return g
+
+    def backward(self, d_rgb=None, d_depth=None, d_normal=None, d_alpha=None, grads=None, d_pose6=None, stream=None,
+                 accumulate=False):
         """sgs_backward.  grads: dict of preallocated device tensors mean/scale/quat/opacity/rgb, or None
-        (pose-only).  d_pose6: device tensor of 6 floats or None."""
+        (pose-only).  d_pose6: device tensor of 6 floats or None.  accumulate=True: sgs_backward_accumulate (the surfel
+        gradients are ADDED to `grads`, which the caller zeroes once per window: zero_grads)."""
         up = _images(d_rgb, d_depth, d_normal, d_alpha)
-        g = None
-        if grads is not None:
-            g = sgs_surfel_grads()
-            g.mean, g.scale, g.quat = _ptr(grads.get("mean")), _ptr(grads.get("scale")), _ptr(grads.get("quat"))
-            g.opacity, g.rgb = _ptr(grads.get("opacity")), _ptr(grads.get("rgb"))
-        _check(self.lib.sgs_backward(self._ctx, C.byref(up), C.byref(g) if g is not None else None, _ptr(d_pose6),
-                                     _stream_ptr(stream)), "sgs_backward")
+        g = self._grads(grads) if grads is not None else None
+        fn, name = (self.lib.sgs_backward_accumulate, "sgs_backward_accumulate") if accumulate else (self.lib.sgs_backward, "sgs_backward")
+        _check(fn(self._ctx, C.byref(up), C.byref(g) if g is not None else None, _ptr(d_pose6), _stream_ptr(stream)), name)
+
+    def zero_grads(self, grads, stream=None):
+        """sgs_zero_grads: the start of an accumulation window."""
+        n = next(v for v in grads.values() if v is not None).shape[0]
+        g = self._grads(grads)
+        _check(self.lib.sgs_zero_grads(self._ctx, C.byref(g), C.c_int64(n), _stream_ptr(stream)), "sgs_zero_grads")
+
+    def map_view_host(self, cam, target_rgb, target_depth, lambda_c, w_d, w_n, ssim_weight, normal_sign, loss=None, pose6=None,
+                      stream=None):
+        """sgs_map_view_host: one view of a mapping window on the resident map, HOST (ideally pinned) target frame in;
+        loss (1 float) / pose6 (6 floats): HOST tensors filled by sync_host()."""
+        self._win_keep = getattr(self, "_win_keep", [])
+        self._win_keep.append((target_rgb, target_depth, loss, pose6))      # alive until sync_host
+        _check(self.lib.sgs_map_view_host(self._ctx, C.byref(cam), _ptr(target_rgb, torch.float32, "cpu"),
+                                          _ptr(target_depth, torch.float32, "cpu"), C.c_float(lambda_c), C.c_float(w_d),
+                                          C.c_float(w_n), C.c_float(ssim_weight), C.c_float(normal_sign),
+                                          _ptr(loss, torch.float32, "cpu"), _ptr(pose6, torch.float32, "cpu"),
+                                          _stream_ptr(stream)), "sgs_map_view_host")
+
+    def fetch_grads_host(self, grads, stream=None):
+        """sgs_fetch_grads_host: ends the window; `grads` (HOST tensors) are complete after sync_host()."""
+        self._win_keep = getattr(self, "_win_keep", [])
+        self._win_keep.append(grads)
+        g = self._grads(grads, "cpu")
+        _check(self.lib.sgs_fetch_grads_host(self._ctx, C.byref(g), _stream_ptr(stream)), "sgs_fetch_grads_host")
+
+    def sync_host(self, stream=None):
+        _check(self.lib.sgs_sync_host(self._ctx, _stream_ptr(stream)), "sgs_sync_host")
+        self._win_keep = []
 
     def tracking_loss(self, cam, ren, target_rgb, target_depth, lambda_d, normal_sign, up, loss, stream=None):
         """sgs_tracking_loss.  ren/up: dicts with rgb, depth, normal, alpha device tensors."""

@@ -160,4 +160,104 @@ int sgs_track_iter_host(sgs_ctx* c, const sgs_camera* cam, float lambda_d, float
     return SGS_OK;
 }
 
+
+// ---- mapping window on the resident map (an iteration optimises over N_a + N_i views) ----
+static int window_setup(sgs_ctx* c, int64_t n, cudaStream_t s) {
+    if (!c->copy_stream) {
+        if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->win_filled, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->win_drained[0], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->win_drained[1], cudaEventDisableTiming) != cudaSuccess ||
+            cudaMallocHost(&c->win_results, sizeof(float) * 8 * SGS_WIN_RING) != cudaSuccess)
+            return SGS_CUDA_ERROR;
+    }
+    for (int k = 0; k < 2; ++k) {
+        if (c->win_cap[k] >= n * 13 + 16) continue;
+        if (c->win_draining[k]) { cudaEventSynchronize(c->win_drained[k]); c->win_draining[k] = false; }
+        if (!grow(c, c->win_grads[k], c->win_cap[k], n * 13 + 16, s)) return SGS_OUT_OF_MEMORY;
+        if (cudaMemsetAsync(c->win_grads[k], 0, sizeof(float) * (size_t)(n * 13 + 16), s) != cudaSuccess) return SGS_CUDA_ERROR;
+    }
+    return SGS_OK;
+}
+
+static void window_grads(sgs_ctx* c, int slot, int64_t n, sgs_surfel_grads* dg) {
+    float* b = c->win_grads[slot];
+    dg->mean = b; dg->scale = b + 3 * n; dg->quat = b + 5 * n; dg->opacity = b + 9 * n; dg->rgb = b + 10 * n;
+}
+
+int sgs_map_view_host(sgs_ctx* c, const sgs_camera* cam, const float* h_rgb, const float* h_depth, float lambda_c, float w_d,
+                      float w_n, float ssim_weight, float normal_sign, float* h_loss, float* h_pose6, void* stream) {
+    if (!c || !sgs_cam_valid(cam) || !h_rgb || !h_depth) return SGS_INVALID_ARGUMENT;
+    if (!c->resident.mean && c->resident.n != 0) return SGS_NO_FORWARD_STATE;
+    if (c->win_n_pending >= SGS_WIN_RING) return SGS_INVALID_ARGUMENT;  // call sgs_sync_host first
+    cudaStream_t s = (cudaStream_t)stream;
+    const int64_t px = (int64_t)cam->width * cam->height, n = c->resident.n;
+    int r = ensure_host_images(c, px, s);
+    if (r != SGS_OK) return r;
+    if ((r = window_setup(c, n, s)) != SGS_OK) return r;
+    if ((r = sgs_upload_target(c, cam, h_rgb, h_depth, stream)) != SGS_OK) return r;
+    const int slot = c->win_slot;
+    if (c->win_draining[slot]) {  // the copy-out (and re-zeroing) of this accumulator, two windows ago, must be complete
+        if (cudaStreamWaitEvent(s, c->win_drained[slot], 0) != cudaSuccess) return SGS_CUDA_ERROR;
+        c->win_draining[slot] = false;
+    }
+    sgs_images ren, up, tgt = {c->target_rgb, c->target_depth, nullptr, nullptr};
+    dev_images(c->host_img_dev, px, &ren);
+    dev_images(c->host_up_dev, px, &up);
+    if ((r = sgs_render(c, &c->resident, cam, &ren, stream)) != SGS_OK) return r;
+    float* res = c->win_results + 8 * c->win_n_pending;  // (pinned; this view's loss and pose gradient land here)
+    if (cudaMemsetAsync(c->loss_dev, 0, sizeof(float), s) != cudaSuccess) return SGS_CUDA_ERROR;
+    if ((r = sgs_mapping_loss(c, cam, &ren, &tgt, lambda_c, w_d, w_n, normal_sign, &up, c->loss_dev, stream)) != SGS_OK) return r;
+    if (ssim_weight != 0.f &&
+        (r = sgs_ssim_loss(c, cam->width, cam->height, ren.rgb, tgt.rgb, ssim_weight, up.rgb, c->loss_dev, stream)) != SGS_OK)
+        return r;
+    sgs_surfel_grads dg;
+    window_grads(c, slot, n, &dg);
+    if ((r = sgs_backward_accumulate(c, &up, &dg, c->pose6_dev, stream)) != SGS_OK) return r;
+    if ((r = sgs_wait_grads(c, stream)) != SGS_OK) return r;
+    c->win_dirty = true;
+    if (cudaMemcpyAsync(res, c->loss_dev, sizeof(float) * 7, cudaMemcpyDeviceToHost, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    c->win_pending[c->win_n_pending].loss = h_loss;
+    c->win_pending[c->win_n_pending].pose6 = h_pose6;
+    c->win_n_pending += 1;
+    return SGS_OK;
+}
+
+int sgs_fetch_grads_host(sgs_ctx* c, const sgs_surfel_grads* hg, void* stream) {
+    if (!c || !hg) return SGS_INVALID_ARGUMENT;
+    if (!c->copy_stream || !c->win_grads[c->win_slot]) return SGS_NO_FORWARD_STATE;
+    cudaStream_t s = (cudaStream_t)stream, cs = c->copy_stream;
+    const int64_t n = c->resident.n;
+    const int slot = c->win_slot;
+    sgs_surfel_grads dg;
+    window_grads(c, slot, n, &dg);
+    bool ok = cudaEventRecord(c->win_filled, s) == cudaSuccess && cudaStreamWaitEvent(cs, c->win_filled, 0) == cudaSuccess;
+    if (hg->mean) ok = ok && cudaMemcpyAsync(hg->mean, dg.mean, sizeof(float) * 3 * n, cudaMemcpyDeviceToHost, cs) == cudaSuccess;
+    if (hg->scale) ok = ok && cudaMemcpyAsync(hg->scale, dg.scale, sizeof(float) * 2 * n, cudaMemcpyDeviceToHost, cs) == cudaSuccess;
+    if (hg->quat) ok = ok && cudaMemcpyAsync(hg->quat, dg.quat, sizeof(float) * 4 * n, cudaMemcpyDeviceToHost, cs) == cudaSuccess;
+    if (hg->opacity) ok = ok && cudaMemcpyAsync(hg->opacity, dg.opacity, sizeof(float) * n, cudaMemcpyDeviceToHost, cs) == cudaSuccess;
+    if (hg->rgb) ok = ok && cudaMemcpyAsync(hg->rgb, dg.rgb, sizeof(float) * 3 * n, cudaMemcpyDeviceToHost, cs) == cudaSuccess;
+    ok = ok && cudaMemsetAsync(c->win_grads[slot], 0, sizeof(float) * (size_t)(n * 13), cs) == cudaSuccess &&
+         cudaEventRecord(c->win_drained[slot], cs) == cudaSuccess;
+    if (!ok) return SGS_CUDA_ERROR;
+    c->win_draining[slot] = true;
+    c->win_slot ^= 1;
+    c->win_dirty = false;
+    return SGS_OK;
+}
+
+int sgs_sync_host(sgs_ctx* c, void* stream) {
+    if (!c) return SGS_INVALID_ARGUMENT;
+    if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return SGS_CUDA_ERROR;
+    if (c->copy_stream && cudaStreamSynchronize(c->copy_stream) != cudaSuccess) return SGS_CUDA_ERROR;
+    c->win_draining[0] = c->win_draining[1] = false;
+    for (int k = 0; k < c->win_n_pending; ++k) {
+        const float* res = c->win_results + 8 * k;
+        if (c->win_pending[k].loss) *c->win_pending[k].loss = res[0];
+        if (c->win_pending[k].pose6) memcpy(c->win_pending[k].pose6, res + 1, sizeof(float) * 6);
+    }
+    c->win_n_pending = 0;
+    return SGS_OK;
+}
+
 }  // extern "C"

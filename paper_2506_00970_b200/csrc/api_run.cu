@@ -333,7 +333,8 @@ int sgs_track_new_frame(sgs_ctx* c) {
     return SGS_OK;
 }
 
-int sgs_backward(sgs_ctx* c, const sgs_images* upstream, const sgs_surfel_grads* dg, float* d_pose6, void* stream) {
+static int backward_impl(sgs_ctx* c, const sgs_images* upstream, const sgs_surfel_grads* dg, float* d_pose6, bool accumulate,
+                         void* stream) {
     if (!c) return SGS_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     int r = check_pending(c, s);
@@ -352,9 +353,31 @@ int sgs_backward(sgs_ctx* c, const sgs_images* upstream, const sgs_surfel_grads*
         if (upstream->alpha) up[7] = upstream->alpha;
     }
     c->grads_on_aux = false;
-    if (sgs_launch_backward(c, up, dg, d_pose6, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    if (sgs_launch_backward(c, up, dg, d_pose6, accumulate, s) != cudaSuccess) return SGS_CUDA_ERROR;
     c->work_recorded = !graph_mode(c) && cudaEventRecord(c->work_ev, c->grads_on_aux ? c->aux_stream : s) == cudaSuccess;
     return SGS_OK;
+}
+
+int sgs_backward(sgs_ctx* c, const sgs_images* upstream, const sgs_surfel_grads* dg, float* d_pose6, void* stream) {
+    return backward_impl(c, upstream, dg, d_pose6, false, stream);
+}
+
+int sgs_backward_accumulate(sgs_ctx* c, const sgs_images* upstream, const sgs_surfel_grads* dg, float* d_pose6, void* stream) {
+    if (!dg) return SGS_INVALID_ARGUMENT;
+    return backward_impl(c, upstream, dg, d_pose6, true, stream);
+}
+
+int sgs_zero_grads(sgs_ctx* c, const sgs_surfel_grads* dg, int64_t n, void* stream) {
+    if (!c || !dg || n < 0) return SGS_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t m = (size_t)n;
+    bool ok = true;
+    if (dg->mean) ok = ok && cudaMemsetAsync(dg->mean, 0, sizeof(float) * 3 * m, s) == cudaSuccess;
+    if (dg->scale) ok = ok && cudaMemsetAsync(dg->scale, 0, sizeof(float) * 2 * m, s) == cudaSuccess;
+    if (dg->quat) ok = ok && cudaMemsetAsync(dg->quat, 0, sizeof(float) * 4 * m, s) == cudaSuccess;
+    if (dg->opacity) ok = ok && cudaMemsetAsync(dg->opacity, 0, sizeof(float) * m, s) == cudaSuccess;
+    if (dg->rgb) ok = ok && cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * m, s) == cudaSuccess;
+    return ok ? SGS_OK : SGS_CUDA_ERROR;
 }
 
 int sgs_wait_grads(sgs_ctx* c, void* stream) {

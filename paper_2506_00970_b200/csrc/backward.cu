@@ -275,7 +275,7 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
                   float* __restrict__ acc, const float* __restrict__ mean, const float* __restrict__ scale,
                   const float* __restrict__ quat, SgsCamDev cam, sgs_surfel_grads out,
                   float* __restrict__ pose_partial, SgsCounters* __restrict__ counters_rw,
-                  float* __restrict__ d_pose6, int survivors) {
+                  float* __restrict__ d_pose6, int survivors, int accumulate) {
     __shared__ float s_red[8][6];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     // compacted mode: v < N_v, surfel = vis_to_surfel[v]; bucket mode (no compaction): v = surfel index
@@ -323,12 +323,15 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
         float dtu[3], dtv[3];
 #pragma unroll
         for (int r = 0; r < 3; ++r) { dtu[r] = su * dau[r]; dtv[r] = sv * dav[r]; }
+        // sgs_backward_accumulate: this view's gradient is ADDED to what the window has so far (one thread per surfel and
+        // kernel, kernels of a window in stream order: plain read-modify-write)
+        auto put = [accumulate](float* p, float v) { *p = accumulate ? *p + v : v; };
         if (out.scale) {
-            out.scale[2 * i] = tuc[0] * dau[0] + tuc[1] * dau[1] + tuc[2] * dau[2];
-            out.scale[2 * i + 1] = tvc[0] * dav[0] + tvc[1] * dav[1] + tvc[2] * dav[2];
+            put(out.scale + 2 * i, tuc[0] * dau[0] + tuc[1] * dau[1] + tuc[2] * dau[2]);
+            put(out.scale + 2 * i + 1, tvc[0] * dav[0] + tvc[1] * dav[1] + tvc[2] * dav[2]);
         }
-        if (out.opacity) out.opacity[i] = a[15];
-        if (out.rgb) { out.rgb[3 * i] = a[12]; out.rgb[3 * i + 1] = a[13]; out.rgb[3 * i + 2] = a[14]; }
+        if (out.opacity) put(out.opacity + i, a[15]);
+        if (out.rgb) { put(out.rgb + 3 * i, a[12]); put(out.rgb + 3 * i + 1, a[13]); put(out.rgb + 3 * i + 2, a[14]); }
         // pose share: rho += dmu; theta += mu_c x dmu + t_uc x dtu + t_vc x dtv + t_nc x dtn   (Eq. 13)
         p6[0] += dmu[0]; p6[1] += dmu[1]; p6[2] += dmu[2];
         p6[3] += (muc[1] * dmu[2] - muc[2] * dmu[1]) + (tuc[1] * dtu[2] - tuc[2] * dtu[1]) +
@@ -342,7 +345,7 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
 #pragma unroll
         for (int r = 0; r < 3; ++r) {
             const float c0 = cam.Rf[r], c1 = cam.Rf[3 + r], c2 = cam.Rf[6 + r];
-            if (out.mean) out.mean[3 * i + r] = c0 * dmu[0] + c1 * dmu[1] + c2 * dmu[2];
+            if (out.mean) put(out.mean + 3 * i + r, c0 * dmu[0] + c1 * dmu[1] + c2 * dmu[2]);
             G[r][0] = c0 * dtu[0] + c1 * dtu[1] + c2 * dtu[2];
             G[r][1] = c0 * dtv[0] + c1 * dtv[1] + c2 * dtv[2];
             G[r][2] = c0 * dtn[0] + c1 * dtn[1] + c2 * dtn[2];
@@ -357,10 +360,10 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
             dq[3] = 2.f * (-2.f * qz * G[0][0] - qw * G[0][1] + qx * G[0][2] + qw * G[1][0] - 2.f * qz * G[1][1] +
                            qy * G[1][2] + qx * G[2][0] + qy * G[2][1]);
             const float qd = qw * dq[0] + qx * dq[1] + qy * dq[2] + qz * dq[3];
-            out.quat[4 * i] = (dq[0] - qw * qd) * qi;
-            out.quat[4 * i + 1] = (dq[1] - qx * qd) * qi;
-            out.quat[4 * i + 2] = (dq[2] - qy * qd) * qi;
-            out.quat[4 * i + 3] = (dq[3] - qz * qd) * qi;
+            put(out.quat + 4 * i, (dq[0] - qw * qd) * qi);
+            put(out.quat + 4 * i + 1, (dq[1] - qx * qd) * qi);
+            put(out.quat + 4 * i + 2, (dq[2] - qy * qd) * qi);
+            put(out.quat + 4 * i + 3, (dq[3] - qz * qd) * qi);
         }
     }
     }
@@ -383,7 +386,7 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
 }  // namespace
 
 cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_surfel_grads* dg, float* d_pose6,
-                                cudaStream_t s) {
+                                bool accumulate, cudaStream_t s) {
     SgsStage st(c, SGS_STAGE_BACKWARD, s);
     const int tiles = c->camd.tiles_x * c->camd.tiles_y;
     CPlanes u;
@@ -406,18 +409,21 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     // exact zeros for every surfel the per-surfel kernel does not visit (inactive, culled): 52 B per surfel of plain
     // HBM writes that nothing before k_surfel_backward depends on -- forked onto the ctx's own stream so that they run
     // beside the issue-bound k_backward, joined in front of k_surfel_backward
+    // (sgs_backward_accumulate: nothing is zeroed -- surfels this view does not see keep what the window has so far)
     cudaStream_t ms = c->aux_stream ? c->aux_stream : s;
-    if (ms != s) {
+    const bool fill = !accumulate;
+    if (ms != s && fill) {
         if ((e = cudaEventRecord(c->fork_ev, s)) != cudaSuccess) return e;
         if ((e = cudaStreamWaitEvent(ms, c->fork_ev, 0)) != cudaSuccess) return e;
     }
+    if (fill)
     if (dg->mean && e == cudaSuccess) e = cudaMemsetAsync(dg->mean, 0, sizeof(float) * 3 * (size_t)n, ms);
-    if (dg->scale && e == cudaSuccess) e = cudaMemsetAsync(dg->scale, 0, sizeof(float) * 2 * (size_t)n, ms);
-    if (dg->quat && e == cudaSuccess) e = cudaMemsetAsync(dg->quat, 0, sizeof(float) * 4 * (size_t)n, ms);
-    if (dg->opacity && e == cudaSuccess) e = cudaMemsetAsync(dg->opacity, 0, sizeof(float) * (size_t)n, ms);
-    if (dg->rgb && e == cudaSuccess) e = cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * (size_t)n, ms);
+    if (fill && dg->scale && e == cudaSuccess) e = cudaMemsetAsync(dg->scale, 0, sizeof(float) * 2 * (size_t)n, ms);
+    if (fill && dg->quat && e == cudaSuccess) e = cudaMemsetAsync(dg->quat, 0, sizeof(float) * 4 * (size_t)n, ms);
+    if (fill && dg->opacity && e == cudaSuccess) e = cudaMemsetAsync(dg->opacity, 0, sizeof(float) * (size_t)n, ms);
+    if (fill && dg->rgb && e == cudaSuccess) e = cudaMemsetAsync(dg->rgb, 0, sizeof(float) * 3 * (size_t)n, ms);
     if (e != cudaSuccess) return e;
-    if (ms != s && (e = cudaEventRecord(c->join_ev, ms)) != cudaSuccess) return e;
+    if (ms != s && fill && (e = cudaEventRecord(c->join_ev, ms)) != cudaSuccess) return e;
     c->launches += 1;
     if (dn) k_backward<false, false, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                   cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
@@ -433,7 +439,7 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     if (lazy) {
         if ((e = cudaEventRecord(c->fork_ev, s)) != cudaSuccess) return e;       // k_backward enqueued
         if ((e = cudaStreamWaitEvent(ms, c->fork_ev, 0)) != cudaSuccess) return e;
-    } else if (ms != s && (e = cudaStreamWaitEvent(s, c->join_ev, 0)) != cudaSuccess) return e;
+    } else if (ms != s && fill && (e = cudaStreamWaitEvent(s, c->join_ev, 0)) != cudaSuccess) return e;
     // one thread per listed surfel; the list length is only known on the device: grid-stride from a hinted grid
     const bool bucket_mode = c->list_stride == 2;
     int64_t want = n;
@@ -446,7 +452,7 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     c->grads_on_aux = lazy;
     k_surfel_backward<<<blocks, 256, 0, ks>>>(c->counters, c->vis_to_surfel, c->culled, c->acc, c->last_surfels.mean,
                                              c->last_surfels.scale, c->last_surfels.quat, cam, *dg, c->pose_partial,
-                                             c->counters, d_pose6, bucket_mode ? 1 : 0);
+                                             c->counters, d_pose6, bucket_mode ? 1 : 0, accumulate ? 1 : 0);
     return cudaGetLastError();
 }
 

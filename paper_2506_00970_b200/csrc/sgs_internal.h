@@ -54,6 +54,7 @@ struct SgsCamDev {
 // SGS_FLAG_TRACK_REUSE: a survivor list stays valid for poses within this translation / rotation of the pose it was built for
 constexpr float SGS_REUSE_MARGIN_T = 0.03f, SGS_REUSE_MARGIN_R = 0.02f;
 
+constexpr int SGS_WIN_RING = 64;       // views whose (loss, pose gradient) may be in flight between two sgs_sync_host calls
 constexpr int SGS_TRACK_HELPERS = 32;  // K-track: extra blocks that walk back the second half of the longest tile lists
 
 struct SurvInputs { float4 *p0, *p1, *p2; float* p3; };  // (mean, opacity), quat, (scale, r, g), b
@@ -173,6 +174,12 @@ struct sgs_ctx {
     bool order_skip;                 // SGS_FLAG_GRAPH + SGS_FLAG_TRACK_REUSE: the tile order is renewed once per frame only
     const SgsCounters* stats_src;    // SGS_FLAG_GRAPH: where the last binning's counters sit on the device (sgs_get_stats copies them)
     int64_t host_img_cap, host_grads_cap;
+    // mapping window on the resident map (sgs_map_view_host / sgs_fetch_grads_host): two device accumulators of n x 13 floats
+    // (one fills while the other drains to the host on copy_stream), and a pinned ring of per-view results
+    float* win_grads[2]; int64_t win_cap[2]; int win_slot; bool win_dirty;
+    cudaStream_t copy_stream; cudaEvent_t win_filled, win_drained[2]; bool win_draining[2];
+    float* win_results;              // pinned, SGS_WIN_RING x 8 floats: loss, pose6
+    struct { float* loss; float* pose6; } win_pending[64]; int win_n_pending;
     int64_t partial_cap;             // floats in pose_partial
     int64_t launches;                // kernels launched by this ctx
     int prof_on; int prof_n, prof_cap; cudaEvent_t* prof_ev; int* prof_stage;  // event pairs: ev[2i], ev[2i+1]
@@ -193,7 +200,7 @@ cudaError_t sgs_launch_preprocess(sgs_ctx* c, const sgs_surfels* sf, cudaStream_
 cudaError_t sgs_launch_sort_and_ranges(sgs_ctx* c, cudaStream_t s);
 cudaError_t sgs_launch_forward(sgs_ctx* c, float* const planes[8], cudaStream_t s);
 cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_surfel_grads* dg, float* d_pose6,
-                                cudaStream_t s);
+                                bool accumulate, cudaStream_t s);
 cudaError_t sgs_launch_tracking_loss(sgs_ctx* c, const sgs_camera* cam, const float* const ren[8], const float* trgb,
                                      const float* tdepth, float lambda_d, float nsign, float* const up[8], float* loss,
                                      cudaStream_t s);

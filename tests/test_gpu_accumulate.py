@@ -1,0 +1,128 @@
+"""Gradient accumulation over a mapping window (one optimiser step on the summed loss of N_a + N_i
+views): sgs_backward_accumulate against the SUM of the oracle's per-view gradients, element by element (each view
+contributes its own strict bar and its own fragile-pixel exposure to the bound), and the HOST-buffer window calls
+(sgs_map_view_host / sgs_fetch_grads_host / sgs_sync_host) against the device-buffer sequence they wrap."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import scenegen
+
+pytestmark = pytest.mark.gpu
+
+sgs = pytest.importorskip("paper_2506_00970_b200")
+from gpu_common import (to_device, camera, alloc_images, alloc_grads, split_upstream, assert_pose, GROUPS, C_EXPO)  # noqa: E402
+
+
+def window_against_oracle(sc, cam_views, ups, async_mode=False):
+    """cam_views: [(Camera, T_cw or None)], ups: upstream (8,H,W) per view."""
+    cfg = oracle.make_cfg()
+    ren = sgs.Renderer(async_mode=async_mode)
+    t, sf = to_device(sc)
+    g = alloc_grads(sc.n)                     # poisoned with 7.0: zero_grads must clear it
+    ren.zero_grads(g)
+    ref = {k: 0.0 for k in GROUPS}
+    bound = {k: 0.0 for k in GROUPS}
+    seen = np.zeros(sc.n, bool)
+    for (cam, T), up in zip(cam_views, ups):
+        camv, c = oracle.make_cam(cam, T), camera(cam, T)
+        im = alloc_images(cam)
+        for _ in range(3 if async_mode else 1):
+            try:
+                ren.render(sf, c, **im); ren.stats(); ren.render(sf, c, **im)
+                break
+            except sgs.SgsError as e:
+                if e.status != sgs.SGS_WORKSPACE_OVERFLOW:
+                    raise
+        u = torch.from_numpy(up.astype(np.float32)).cuda()
+        up32 = u.cpu().numpy().astype(np.float64)
+        p6 = torch.full((6,), 5.0, device="cuda")
+        ren.backward(**split_upstream(up32), grads=g, d_pose6=p6, accumulate=True)
+        og, ex = oracle.backward(sc, camv, cfg, up32), oracle.exposure(sc, camv, cfg, up32)
+        assert_pose(p6.cpu().numpy(), og["pose"], ex["pose"])      # the pose gradient is per view: overwritten, not summed
+        for k in GROUPS:
+            ref[k] = ref[k] + og[k]
+            bound[k] = bound[k] + 1e-3 * np.abs(og[k]) + 1e-3 * np.sqrt(np.mean(og[k] ** 2)) + C_EXPO * ex[k]
+        seen |= oracle.binning(sc, camv, cfg)["culled"] == 0
+    torch.cuda.synchronize()
+    for k in GROUPS:
+        got = g[k].cpu().numpy().astype(np.float64)
+        err = np.abs(got - ref[k])
+        assert (err <= bound[k]).all(), (k, int((err > bound[k]).sum()), float((err / bound[k]).max()))
+        assert (got[~seen] == 0).all()         # splats no view of the window saw keep the window's zero
+    ren.close()
+
+
+def test_three_view_window_on_c1():
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    taus = [None, [0.05, 0.02, -0.04, 0.1, -0.05, 0.2], [-0.1, 0.05, 0.02, -0.2, 0.1, 0.05]]
+    views = [(cam, None if tau is None else scenegen.perturb_pose(cam.T_cw, tau)) for tau in taus]
+    ups = [scenegen.upstream_normal(20 + i, cam.height, cam.width) for i in range(3)]
+    window_against_oracle(sc, views, ups)
+
+
+def test_two_view_window_on_c3_at_full_size():
+    """C3 views 0 and 7 (500 k surfels, 1200 x 680) under the mapping loss of Eq. 24-26 (dense upstream)."""
+    sc, cams, _ = scenegen.make_config("C3")
+    cfg = oracle.make_cfg()
+    views, ups = [], []
+    for v in (0, 7):
+        cam = cams[v]
+        camv = oracle.make_cam(cam)
+        img = oracle.render(sc, camv, cfg, counters=False)["img"]
+        T_tgt = scenegen.perturb_pose(cam.T_cw, np.array([0.02, 0.0, -0.01, 0.0, 0.01, 0.005]))
+        tgt = oracle.render(sc, oracle.make_cam(cam, T_tgt), cfg, counters=False)["img"]
+        _, up = oracle.mapping_loss(img, tgt[0:3], tgt[3], camv, 0.875, 0.5, 0.02, -1.0)
+        views.append((cam, None)); ups.append(up)
+    window_against_oracle(sc, views, ups, async_mode=True)
+
+
+def test_host_window_calls_equal_the_device_sequence():
+    """sgs_map_view_host x 3 + sgs_fetch_grads_host, twice in a row (both accumulators of the double buffer, the re-zeroing
+    behind the copy-out), against render + mapping_loss + ssim_loss + backward_accumulate on device buffers."""
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    H, W = cam.height, cam.width
+    t, sf = to_device(sc)
+    taus = [None, [0.05, 0.02, -0.04, 0.1, -0.05, 0.2], [-0.1, 0.05, 0.02, -0.2, 0.1, 0.05]]
+    cs = [camera(cam, None if tau is None else scenegen.perturb_pose(cam.T_cw, tau)) for tau in taus]
+    g0 = scenegen.SplitMix(77)
+    tgts = [(torch.from_numpy(g0.uniform(3 * H * W).reshape(3, H, W).astype(np.float32)),
+             torch.from_numpy((1.5 + g0.uniform(H * W)).reshape(1, H, W).astype(np.float32))) for _ in range(6)]
+    dev = sgs.Renderer()
+    host = sgs.Renderer()
+    pin = lambda x, dt=torch.float32: torch.from_numpy(np.ascontiguousarray(x)).to(dt).pin_memory()
+    host.upload_surfels(pin(sc.mean), pin(sc.scale), pin(sc.quat), pin(sc.opacity), pin(sc.rgb))
+    hg = [{k: torch.full(v.shape, 9.0).pin_memory() for k, v in alloc_grads(sc.n).items()} for _ in range(2)]
+    hl = [torch.zeros(1).pin_memory() for _ in range(6)]
+    hp = [torch.zeros(6).pin_memory() for _ in range(6)]
+    want = []
+    for w in range(2):
+        g = alloc_grads(sc.n)
+        dev.zero_grads(g)
+        for v in range(3):
+            trgb, tdep = tgts[3 * w + v]
+            im, up = alloc_images(cam), alloc_images(cam)
+            loss, p6 = torch.zeros(1, device="cuda"), torch.zeros(6, device="cuda")
+            dev.render(sf, cs[v], **im)
+            dev.mapping_loss(cs[v], im, trgb.cuda(), tdep.cuda(), 0.875, 0.5, 0.02, -1.0, up, loss)
+            dev.ssim_loss(im["rgb"], trgb.cuda(), 0.125, up["rgb"], loss)
+            dev.backward(d_rgb=up["rgb"], d_depth=up["depth"], d_normal=up["normal"], d_alpha=up["alpha"], grads=g, d_pose6=p6,
+                         accumulate=True)
+            want.append((float(loss.item()), p6.cpu().numpy()))
+            host.map_view_host(cs[v], trgb.pin_memory(), tdep.pin_memory(), 0.875, 0.5, 0.02, 0.125, -1.0, hl[3 * w + v], hp[3 * w + v])
+        host.fetch_grads_host(hg[w])            # no wait: the second window is enqueued behind it
+        want.append({k: x.cpu().numpy() for k, x in g.items()})
+    host.sync_host()
+    for w in range(2):
+        ref = want[4 * w + 3]
+        for k in ref:
+            assert np.abs(ref[k]).max() > 0
+            np.testing.assert_allclose(hg[w][k].numpy(), ref[k], rtol=2e-4, atol=1e-5 * np.abs(ref[k]).max())
+        for v in range(3):
+            L, p = want[4 * w + v]
+            assert abs(float(hl[3 * w + v].item()) - L) <= 1e-5 * abs(L) and L > 0
+            np.testing.assert_allclose(hp[3 * w + v].numpy(), p, rtol=1e-4, atol=1e-5 * np.abs(p).max())
+    dev.close(); host.close()
