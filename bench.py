@@ -1,15 +1,19 @@
 #!/usr/bin/env python
 """bench.py -- forward+backward throughput of the B200 surfel renderer on BASELINE.json's configs.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input:
   C2 / C5 (tracking-shaped): one frame = `iters` iterations of render -> Eq. 15-19 loss -> pose-only backward
-  C1 / C3 / C4 (mapping-shaped): one window = every view rendered and back-propagated (full backward + pose)
-`value` is megapixels/s (W*H*renders / device time), inputs resident in HBM; `e2e` is the same metric
-through the HOST-buffer C-ABI calls with the copies inside the timed region.  The roofline object is
-for the dominant stage, timed in a second pass of the same K steps with CUDA events around every
-stage (sgs_set_profiling), so the headline value is not perturbed by the extra event records.
+  C1 / C3 / C4 (mapping-shaped): every view rendered and back-propagated (Eq. 24-26 loss, full backward + pose), the
+      surfel gradients summed over windows of N_a + N_i = 5 views (Tab. I) by sgs_backward_accumulate
+Without --config ALL FIVE configs of BASELINE.json run one after the other; the line's headline (`value`, `roofline`,
+`e2e`, `cpu_baseline`, `config.workload`) is C4, the largest single-GPU configuration, and `per_config` carries the same
+figures for C1..C5.  `value` is megapixels/s (W*H*renders / device time), inputs resident in HBM; `e2e` is the same
+metric through the HOST-buffer C-ABI calls with the copies inside the timed region.  The roofline object is for the
+dominant stage, timed in a second pass of the same K steps with CUDA events around every stage (sgs_set_profiling), so
+the headline value is not perturbed by the extra event records; its `traffic` is read from profiles/r02_traffic.json,
+which `bench.py --ingest-ncu` writes from an `ncu --set full` capture of that kernel.
 Rank 0 prints ONE JSON line.  --impl reference times the CPU oracle (oracle/) on the host cores."""
 import argparse
 import json
@@ -29,10 +33,39 @@ UNIT = "MP/s"
 # Algorithmic flops per (pixel, entry) pair, counted from the oracle's formulas with FMA = 2
 # (DESIGN.md §7): tested pair 26; composited pair +26 forward, +102 full backward, +94 pose-only backward.
 F_TEST, F_COMP_FWD, F_COMP_BWD_FULL, F_COMP_BWD_POSE = 26, 26, 102, 94
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
-# captures (profiles/r01_*.md; ncu flushes L2 before every replay, so these are cold-cache figures)
-NCU_TRAFFIC = {("C2", "track"): 8.49e6, ("C2", "backward"): 30.6e6, ("C2", "forward"): 14.0e6,
-               ("C4", "backward"): 70.2e6, ("C3", "backward"): 68.3e6, ("C4", "forward"): 31.5e6, ("C5", "track"): 31.3e6}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of each config's kernels: profiles/r02_traffic.json, written by
+# `bench.py --ingest-ncu` from `ncu --set full` captures (ncu flushes L2 before every replay: cold-cache figures)
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
+WINDOW = 5            # views per mapping window: N_a + N_i (Tab. I)
+KERNEL_OF_STAGE = {"forward": "k_forward", "backward": "k_backward", "track": "k_track", "preprocess": "k_pre_project",
+                   "sort": "k_tile_order"}
+
+
+def load_traffic(config, stage):
+    try:
+        return json.load(open(TRAFFIC_JSON)).get(config, {}).get(stage, {}).get("dram_bytes_per_launch")
+    except (OSError, ValueError):
+        return None
+
+
+def ingest_ncu(csv_path, config):
+    """`ncu -i X.ncu-rep --page raw --csv` of a capture of one bench step -> profiles/r02_traffic.json[config][stage] =
+    mean dram__bytes_read.sum + dram__bytes_write.sum per launch of that stage's kernel (all captured launches)."""
+    import csv
+    rows = list(csv.reader(open(csv_path)))
+    hdr = next(i for i, r in enumerate(rows) if "Kernel Name" in r)
+    names, units = rows[hdr], rows[hdr + 1]
+    kn, rd, wr = names.index("Kernel Name"), names.index("dram__bytes_read.sum"), names.index("dram__bytes_write.sum")
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    out = json.load(open(TRAFFIC_JSON)) if os.path.exists(TRAFFIC_JSON) else {}
+    cfg = out.setdefault(config, {})
+    for stage, kern in KERNEL_OF_STAGE.items():
+        vals = [float(r[rd].replace(",", "")) * scale[units[rd]] + float(r[wr].replace(",", "")) * scale[units[wr]]
+                for r in rows[hdr + 2:] if len(r) > wr and kern in r[kn]]
+        if vals:
+            cfg[stage] = dict(kernel=kern, launches=len(vals), dram_bytes_per_launch=sum(vals) / len(vals), source=os.path.basename(csv_path))
+    json.dump(out, open(TRAFFIC_JSON, "w"), indent=1, sort_keys=True)
+    return cfg
 
 
 def load_peaks():
@@ -209,9 +242,15 @@ class Workload:
         ren.mapping_loss(cam, self.im, trgb, tdep, 0.875, 0.5, 0.02, -1.0, self.up, self.loss)
         ren.ssim_loss(self.im["rgb"], trgb, 0.125, self.up["rgb"], self.loss)   # + (1 - lambda_c) L_SSIM: Eq. 24 complete
         u = self.up
-        if True:
-            ren.backward(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"],
-                         grads=self.grads_of[id(ren)], d_pose6=self.p6_of[id(ren)])
+        ren.backward(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"],
+                     grads=self.grads_of[id(ren)], d_pose6=self.p6_of[id(ren)], accumulate=True)
+
+    def begin_window(self):
+        """Start of a mapping window: the consumer of the last window's gradients (the optimiser step) is past, every
+        context's accumulator is zeroed."""
+        for r in self.rens:
+            r.wait_grads()
+            r.zero_grads(self.grads_of[id(r)])
 
     def step(self):
         if self.graph and self.cg is not None:
@@ -220,6 +259,8 @@ class Workload:
             def frame():
                 if not self.tracking:
                     for v in range(len(self.cams)):
+                        if v % WINDOW == 0:
+                            self.begin_window()
                         self.one(v)
                     return
                 self.ren.track_new_frame()   # a step is the tracking of one frame: the survivor list is built once per step
@@ -235,6 +276,8 @@ class Workload:
                 self.eager_steps += 1
         elif len(self.rens) == 1:
             for v in range(len(self.cams)):
+                if v % WINDOW == 0:
+                    self.begin_window()
                 self.one(v)
         else:
             main = self.torch.cuda.current_stream()
@@ -242,6 +285,8 @@ class Workload:
             nv = len(self.cams)
             self.rens[0].prepare(self.sf, self.ccams[0], stream=self.side)
             for v in range(nv):
+                if v % WINDOW == 0:
+                    self.begin_window()   # (each context sums the views it renders; the optimiser adds the two accumulators)
                 if v + 1 < nv:
                     self.rens[(v + 1) % 2].prepare(self.sf, self.ccams[v + 1], stream=self.side)
                 self.one(v, self.rens[v % 2])   # its render finds the binning prepared and orders itself behind it
@@ -261,15 +306,15 @@ class Workload:
                       active=pin(sc.active, torch.uint8))
         self.h_targets = [(a.cpu().pin_memory(), b.cpu().pin_memory()) for a, b in self.targets]
         if not self.tracking:
-            self.h_up = {k: v.cpu().pin_memory() for k, v in self.up.items()}
-            self.h_grads = {k: torch.zeros(v.shape).pin_memory() for k, v in self.grads.items()}
-            self.h_p6 = torch.zeros(6).pin_memory()
-            self.h_im = {k: v.cpu().pin_memory() for k, v in self.im.items()}
+            self.h_grads = [{k: torch.zeros(v.shape).pin_memory() for k, v in self.grads.items()} for _ in range(2)]
+            self.h_p6 = [torch.zeros(6).pin_memory() for _ in self.cams]
+            self.h_loss = [torch.zeros(1).pin_memory() for _ in self.cams]
 
     def step_e2e(self):
         """Tracking: upload map + target frame, then `iters` x sgs_track_iter_host (loss + 6-vector read back
-        every iteration).  Mapping: upload map; per view render_host (images to host) + backward_host
-        (upstream from host, all gradients back to host)."""
+        every iteration).  Mapping: upload map; per view sgs_map_view_host (keyframe from the host; render, Eq. 24-26,
+        full backward summed into the window on the device; loss + 6-vector back); per window of 5 views
+        sgs_fetch_grads_host (all N x 13 gradients back to the host); sgs_sync_host at the end of the step."""
         r, h = self.ren, self.h
         r.upload_surfels(h["mean"], h["scale"], h["quat"], h["opacity"], h["rgb"], h["active"])
         if self.tracking:
@@ -277,12 +322,13 @@ class Workload:
             for _ in range(self.iters):
                 loss, p6 = r.track_iter_host(self.ccams[0], 0.5, -1.0)
             return loss
-        for v in range(len(self.cams)):
-            r.render_host(self.ccams[v], **self.h_im)
-            u = self.h_up
-            r.backward_host(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"],
-                            grads=self.h_grads, d_pose6=self.h_p6)
-        return float(self.h_p6[0])
+        nv = len(self.cams)
+        for v in range(nv):
+            r.map_view_host(self.ccams[v], *self.h_targets[v], 0.875, 0.5, 0.02, 0.125, -1.0, self.h_loss[v], self.h_p6[v])
+            if (v + 1) % WINDOW == 0 or v + 1 == nv:
+                r.fetch_grads_host(self.h_grads[(v // WINDOW) % 2])
+        r.sync_host()
+        return float(self.h_loss[0][0])
 
     def e2e_bytes(self):
         n, px = self.sc.n, self.H * self.W
@@ -290,97 +336,96 @@ class Workload:
         if self.tracking:
             return h2d + px * 16 + self.iters * 48, self.iters * 28
         k = len(self.cams)
-        return h2d + k * (px * 32 + 48), k * (px * 32 + n * 52 + 24)
+        windows = (k + WINDOW - 1) // WINDOW
+        return h2d + k * (px * 16 + 48), windows * n * 52 + k * 28
 
 
-def cpu_baseline(name, max_views=1):
-    """The oracle as it stands, on the host cores: forward + analytic backward of `max_views` view(s)."""
+def cpu_baseline(sc, cams, name, samples=3):
+    """The oracle as it stands, on the host cores: fp64 forward + analytic backward (to surfels and pose) of one view,
+    `samples` views of the config (0, 1, 2, ... cyclically), the MEDIAN reported."""
     import oracle
-    import scenegen
-    sc, cams, info = scenegen.make_config(name)
     cfg = oracle.make_cfg()
+    secs = []
+    for k in range(samples):
+        cam = cams[k % len(cams)]
+        camv = oracle.make_cam(cam)
+        up = np.ones((8, cam.height, cam.width)) / (cam.height * cam.width)
+        t0 = time.time()
+        oracle.render(sc, camv, cfg, counters=False)
+        oracle.backward(sc, camv, cfg, up)
+        secs.append(time.time() - t0)
+    dt = float(np.median(secs))
     cam = cams[0]
-    camv = oracle.make_cam(cam)
-    up = scenegen.upstream_normal(7, cam.height, cam.width)
-    t0 = time.time()
-    r = oracle.render(sc, camv, cfg, counters=False)
-    oracle.backward(sc, camv, cfg, up)
-    dt = time.time() - t0
+    n_act = int(sc.n if sc.active is None else sc.active.sum())
     return dict(value=cam.width * cam.height / dt / 1e6, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
-                sample=f"1 iteration (fp64 forward + analytic backward to surfels and pose) of {name} view 0, {dt:.2f} s",
-                seconds=dt), (sc, cams, info)
+                surfels_per_s=n_act / dt,
+                sample=f"median of {samples} samples, each 1 view of {name} (fp64 forward + analytic backward to surfels and pose): "
+                       + ", ".join(f"{t:.2f}" for t in secs) + " s", seconds=dt)
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle timed on the host cores; each step is ONE forward+backward of
-    view 0 of the config (a bounded sample of the workload)."""
+    """--impl reference: the CPU oracle timed on the host cores on OUR arm's config (default C4).  A step renders and
+    back-propagates `m` views of the config, walking through its views cyclically from step to step; m is the largest
+    number of views (at most the config's own views per step) that keeps the whole --steps/--warmup run within a few
+    minutes, decided from one timed view -- a bounded sample of the workload, stated in config.workload."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     import oracle
     import scenegen
-    sc, cams, info = scenegen.make_config(args.config)
-    cfg, cam = oracle.make_cfg(), cams[0]
-    camv = oracle.make_cam(cam)
-    up = scenegen.upstream_normal(7, cam.height, cam.width)
+    name = args.config or "C4"
+    sc, cams, info = scenegen.make_config(name)
+    cfg = oracle.make_cfg()
+    tracking = info["mode"] == "pose"
+    per_step = info["iters"] if tracking else len(cams)
+    ups = {}
 
-    def step():
+    def view(k):
+        cam = cams[k % len(cams)]
+        if (cam.height, cam.width) not in ups:
+            ups[(cam.height, cam.width)] = np.ones((8, cam.height, cam.width)) / (cam.height * cam.width)
+        camv = oracle.make_cam(cam)
         oracle.render(sc, camv, cfg, counters=False)
-        oracle.backward(sc, camv, cfg, up)
+        oracle.backward(sc, camv, cfg, ups[(cam.height, cam.width)])
 
+    t0 = time.time()
+    view(0)
+    t_view = time.time() - t0
+    budget = 150.0 / max(1, args.steps + args.warmup)
+    m = int(max(1, min(per_step, budget // max(t_view, 1e-6))))
+    k = 0
     for _ in range(args.warmup):
-        step()
+        for _ in range(m):
+            view(k); k += 1
     t0 = time.time()
     for _ in range(args.steps):
-        step()
+        for _ in range(m):
+            view(k); k += 1
     dt = time.time() - t0
-    mp = cam.width * cam.height * args.steps / dt / 1e6
+    cam = cams[0]
+    mp = cam.width * cam.height * m * args.steps / dt / 1e6
     n_act = int(sc.n if sc.active is None else sc.active.sum())
+    sample = (f"every step: {m} of the config's {per_step} renders per step (fp64 forward + analytic backward to surfels and "
+              f"pose each), views taken cyclically")
     line = dict(metric=METRIC, value=mp, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
                 ms_per_step=1e3 * dt / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
-                data="synthetic", impl="reference", surfels_per_s=n_act * args.steps / dt,
-                config=dict(workload=f"{args.config}: 1 forward+backward of view 0 per step (bounded sample)",
-                            surfels=sc.n, width=cam.width, height=cam.height),
-                cpu_baseline=dict(value=mp, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
-                                  sample="every step: one fp64 forward + analytic backward of view 0"),
+                data="synthetic", impl="reference", surfels_per_s=n_act * m * args.steps / dt,
+                config=dict(workload=f"{name}: {sample} (bounded sample of the same workload)",
+                            surfels=sc.n, active=n_act, width=cam.width, height=cam.height, renders_per_step=m,
+                            renders_per_step_of_the_workload=per_step),
+                cpu_baseline=dict(value=mp, unit=UNIT, cores=oracle.num_threads(), kind="oracle", sample=sample),
                 e2e=dict(value=mp, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
     print(json.dumps(line))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--iters", type=int, default=None, help="override iterations per tracking step")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-reuse", action="store_true", help="tracking configs: run the pre-cull over the whole map every iteration")
-    ap.add_argument("--no-prefetch", action="store_true", help="mapping configs: one context, binning of each view in line")
-    ap.add_argument("--graph", action="store_true", help="SGS_FLAG_GRAPH: each step (a tracking frame, or a mapping window on one context) replayed as one CUDA graph")
-    ap.add_argument("--normalised-depth", action="store_true", help="SGS_FLAG_NORMALISED_DEPTH: depth image D/O (tracking takes the unfused sequence)")
-    ap.add_argument("--contrib", action="store_true", help="mapping configs: render with sgs_render_contrib (C_k output on)")
-    args = ap.parse_args()
-    if args.impl == "reference":
-        return run_reference(args)
-
-    import torch
-    import torch.distributed as dist
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
+def run_config(name, args, torch, dist, world, rank, local, peaks):
+    """One config: timed pass (value), profiled pass (stages / roofline), end-to-end pass, oracle baseline + counters."""
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    wl = Workload(args.config, args.iters, args.contrib, not args.no_prefetch, not args.no_reuse, args.normalised_depth, args.graph)
+    wl = Workload(name, args.iters, args.contrib, not args.no_prefetch, not args.no_reuse, args.normalised_depth, args.graph)
     K, W = args.steps, max(args.warmup, 3)
     per_step = []
     for _ in range(W):
@@ -448,70 +493,128 @@ def main():
             dist.all_reduce(te, op=dist.ReduceOp.MAX)
         h2d, d2h = wl.e2e_bytes()
         e2e = dict(value=px * renders / float(te.item()) / 1e6, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
-                   timing="wall clock around K steps incl. pinned-host copies and per-iteration readback")
-    if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+                   timing="wall clock around K steps incl. pinned-host copies and the read-back of every result")
+    out = dict(value=value, unit=UNIT, ms_per_step=ms_max / K, surfels_per_s=wl.n_active * renders / (ms_max * 1e-3),
+               e2e=e2e, gpu_launches=int(launches), clocks=clocks,
+               stage_us={k: round(1e3 * v[0] / v[1], 2) for k, v in prof.items() if v[1]},
+               config=dict(workload=f"{name} ({'tracking' if wl.tracking else 'mapping'}-shaped): "
+                           f"{wl.renders_per_step} x (render + {'Eq.15-19' if wl.tracking else 'Eq.24-26'} loss + "
+                           f"{'pose-only' if wl.tracking else 'full+pose'} backward) per step",
+                           surfels=wl.sc.n, active=wl.n_active, width=wl.W, height=wl.H, renders_per_step=wl.renders_per_step,
+                           l2="flushed between steps by a 256 MiB write; iterations inside a step reuse the map as tracking does",
+                           replicas=world,
+                           survivor_list=("built once per step (frame) with a 3 cm / 0.02 rad pose margin, SGS_FLAG_TRACK_REUSE"
+                                          if (wl.tracking and not args.no_reuse) else "every render"),
+                           binning=("sgs_prepare of view v+1 on a second context and a side stream, under view v's compositing"
+                                    if len(wl.rens) > 1 else "in line (sgs_render / sgs_track_iter)")))
+    if not wl.tracking:
+        out["config"]["gradients"] = f"summed over windows of {WINDOW} views (sgs_backward_accumulate), zeroed per window"
+    if args.graph:
+        out["config"]["launch"] = "one CUDA graph per step (SGS_FLAG_GRAPH); not the default workload"
+    if args.normalised_depth:
+        out["config"]["depth"] = "normalised D/O (SGS_FLAG_NORMALISED_DEPTH); not the default workload"
+    sc, cams, tracking, n_active = wl.sc, wl.cams, wl.tracking, wl.n_active
+    for r in wl.rens:
+        r.close()
+    del wl
+    torch.cuda.empty_cache()
+    if rank != 0 or args.no_cpu_baseline:
+        out.update(roofline=None, stages={}, cpu_baseline=None)
+        return out
+    import oracle
+    out["cpu_baseline"] = cpu_baseline(sc, cams, name)
+    # algorithmic work per render from the oracle's counters (view 0 stands for every view)
+    camv, cfg = oracle.make_cam(cams[0]), oracle.make_cfg()
+    cnt = oracle.render(sc, camv, cfg)["counters"]
+    E = oracle.preprocess(sc, camv, cfg)["E"]
+    fcb = F_COMP_BWD_POSE if tracking else F_COMP_BWD_FULL
+    work = dict(preprocess=("hbm", (sc.n if sc.active is not None else 0) + n_active * 56 + cnt["n_vis"] * 76 + E * 12),
+                sort=("hbm", E * 24 + E * 8),
+                forward=("alu", F_TEST * cnt["Q_t"] + F_COMP_FWD * cnt["Q_c"]),
+                loss=("hbm", px * (12 + 8) * 4 + (0 if tracking else px * 3 * 4 * 12)),
+                backward=("alu", F_TEST * cnt["Q_tb"] + fcb * cnt["Q_c"]),
+                # sgs_track_iter's single kernel: forward + pose-only backward of the same view
+                track=("alu", F_TEST * (cnt["Q_t"] + cnt["Q_tb"]) + (F_COMP_FWD + F_COMP_BWD_POSE) * cnt["Q_c"]))
+    stages = {}
+    tot_ms = sum(v[0] for v in prof.values()) or 1.0
+    for st, (ms_s, calls) in prof.items():
+        if calls == 0:
+            continue
+        kind, units = work[st]
+        per = ms_s / calls * 1e-3
+        if kind == "hbm":
+            ach, peak, unit = units / per / 1e9, peaks["hbm_gbs"], "GB/s"
+        else:
+            ach, peak, unit = units / per / 1e12, fp32_peak_tflops(peaks), "TFLOP/s"
+        stages[st] = dict(bound=kind, achieved=ach, peak=peak, unit=unit, frac=ach / peak, ms_per_launch=per * 1e3,
+                          share=ms_s / tot_ms, algorithmic_units=units)
+    dom = max(stages, key=lambda k: stages[k]["share"])
+    roof = dict(stages[dom])
+    nominal = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    roof.update(kernel=dom, traffic=load_traffic(name, dom),
+                peak_source=peaks["source"] + (" HBM copy" if roof["bound"] == "hbm" else
+                            ("; alu peak = measured FMA loop (sgs_measure_fp32_peak), nominal 148 SM x 128 lanes x 2 x max SM clock = %.1f" % nominal
+                             if peaks.get("fp32_tflops_measured") else "; alu peak = 148 SM x 128 lanes x 2 x max SM clock")),
+                counters=dict(cnt, E=E))
+    out.update(roofline=roof, stages=stages)
+    return out
 
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default=None, choices=["C1", "C2", "C3", "C4", "C5"],
+                    help="one config only (default: all five, headline C4)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--iters", type=int, default=None, help="override iterations per tracking step")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-reuse", action="store_true", help="tracking configs: run the pre-cull over the whole map every iteration")
+    ap.add_argument("--no-prefetch", action="store_true", help="mapping configs: one context, binning of each view in line")
+    ap.add_argument("--graph", action="store_true", help="SGS_FLAG_GRAPH: each step (a tracking frame, or a mapping window on one context) replayed as one CUDA graph")
+    ap.add_argument("--normalised-depth", action="store_true", help="SGS_FLAG_NORMALISED_DEPTH: depth image D/O (tracking takes the unfused sequence)")
+    ap.add_argument("--contrib", action="store_true", help="mapping configs: render with sgs_render_contrib (C_k output on)")
+    ap.add_argument("--ingest-ncu", default=None, metavar="RAW_CSV",
+                    help="no benchmark: read `ncu -i X.ncu-rep --page raw --csv` of a capture of --config and update profiles/r02_traffic.json")
+    args = ap.parse_args()
+    if args.ingest_ncu:
+        print(json.dumps(ingest_ncu(args.ingest_ncu, args.config or "C4"), indent=1))
+        return
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import paper_2506_00970_b200 as sgs
     peaks = load_peaks()
     try:
-        peaks["fp32_tflops_measured"] = wl.sgs.measure_fp32_peak()
+        peaks["fp32_tflops_measured"] = sgs.measure_fp32_peak()
     except Exception:
         peaks["fp32_tflops_measured"] = None
-    cpu, roof, stages = None, None, {}
-    if not args.no_cpu_baseline:
-        cpu, (sc, cams, info) = cpu_baseline(args.config)
-        # algorithmic work per render from the oracle's counters (view 0 stands for every view)
-        import oracle
-        camv, cfg = oracle.make_cam(cams[0]), oracle.make_cfg()
-        cnt = oracle.render(sc, camv, cfg)["counters"]
-        E = oracle.preprocess(sc, camv, cfg)["E"]
-        n_act = wl.n_active
-        fcb = F_COMP_BWD_POSE if wl.tracking else F_COMP_BWD_FULL
-        work = dict(preprocess=("hbm", (sc.n if sc.active is not None else 0) + n_act * 56 + cnt["n_vis"] * 76 + E * 12),
-                    sort=("hbm", E * 24 + E * 8),
-                    forward=("alu", F_TEST * cnt["Q_t"] + F_COMP_FWD * cnt["Q_c"]),
-                    loss=("hbm", px * (12 + 8) * 4 + (0 if wl.tracking else px * 3 * 4 * 12)),
-                    backward=("alu", F_TEST * cnt["Q_tb"] + fcb * cnt["Q_c"]),
-                    # sgs_track_iter's single kernel: forward + pose-only backward of the same view
-                    track=("alu", F_TEST * (cnt["Q_t"] + cnt["Q_tb"]) + (F_COMP_FWD + F_COMP_BWD_POSE) * cnt["Q_c"]))
-        tot_ms = sum(v[0] for v in prof.values()) or 1.0
-        for st, (ms_s, calls) in prof.items():
-            if calls == 0:
-                continue
-            kind, units = work[st]
-            per = ms_s / calls * 1e-3
-            if kind == "hbm":
-                ach, peak, unit = units / per / 1e9, peaks["hbm_gbs"], "GB/s"
-            else:
-                ach, peak, unit = units / per / 1e12, fp32_peak_tflops(peaks), "TFLOP/s"
-            stages[st] = dict(bound=kind, achieved=ach, peak=peak, unit=unit, frac=ach / peak, ms_per_launch=per * 1e3,
-                              share=ms_s / tot_ms, algorithmic_units=units)
-        dom = max(stages, key=lambda k: stages[k]["share"])
-        roof = dict(stages[dom])
-        roof.update(kernel=dom, traffic=NCU_TRAFFIC.get((args.config, dom)), peak_source=peaks["source"] + (" HBM copy" if roof["bound"] == "hbm" else
-                    ("; alu peak = measured FMA loop (sgs_measure_fp32_peak), nominal 148 SM x 128 lanes x 2 x max SM clock = %.1f" % (148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12) if peaks.get("fp32_tflops_measured") else "; alu peak = 148 SM x 128 lanes x 2 x max SM clock")), counters=dict(cnt, E=E))
-    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=ms_max / K,
-                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
-                surfels_per_s=wl.n_active * renders / (ms_max * 1e-3),
-                config=dict(workload=f"{args.config} ({'tracking' if wl.tracking else 'mapping'}-shaped): "
-                            f"{wl.renders_per_step} x (render + {'Eq.15-19' if wl.tracking else 'Eq.24-26'} loss + "
-                            f"{'pose-only' if wl.tracking else 'full+pose'} backward) per step",
-                            surfels=wl.sc.n, active=wl.n_active, width=wl.W, height=wl.H, renders_per_step=wl.renders_per_step,
-                            l2="flushed between steps by a 256 MiB write; iterations inside a step reuse the map as tracking does",
-                            replicas=world,
-                            survivor_list=("built once per step (frame) with a 3 cm / 0.02 rad pose margin, SGS_FLAG_TRACK_REUSE"
-                                           if (wl.tracking and not args.no_reuse) else "every render"),
-                            binning=("sgs_prepare of view v+1 on a second context and a side stream, under view v's compositing"
-                                     if len(wl.rens) > 1 else "in line (sgs_render / sgs_track_iter)")),
-                clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roof, stages=stages, cpu_baseline=cpu,
-                stage_us={k: round(1e3 * v[0] / v[1], 2) for k, v in prof.items() if v[1]})
-    if args.graph:
-        line["config"]["launch"] = "one CUDA graph per step (SGS_FLAG_GRAPH); not the default workload"
-    if args.normalised_depth:
-        line["config"]["depth"] = "normalised D/O (SGS_FLAG_NORMALISED_DEPTH); not the default workload"
-    print(json.dumps(line))
+    names = [args.config] if args.config else ["C1", "C2", "C3", "C4", "C5"]
+    head = args.config or "C4"
+    res = {n: run_config(n, args, torch, dist, world, rank, local, peaks) for n in names}
+    if rank == 0:
+        h = res[head]
+        line = dict(metric=METRIC, value=h["value"], unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+                    ms_per_step=h["ms_per_step"], higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+                    data="synthetic", surfels_per_s=h["surfels_per_s"], config=h["config"], clocks=h["clocks"], e2e=h["e2e"],
+                    gpu_launches=sum(r["gpu_launches"] for r in res.values()), roofline=h["roofline"], stages=h["stages"],
+                    cpu_baseline=h["cpu_baseline"], stage_us=h["stage_us"])
+        if len(names) > 1:
+            line["config"] = dict(h["config"], headline="C4, the largest single-GPU configuration of BASELINE.json; per_config has all five")
+            line["per_config"] = {n: {k: r[k] for k in ("value", "surfels_per_s", "ms_per_step", "roofline", "e2e", "cpu_baseline",
+                                                         "gpu_launches", "stage_us", "clocks")} | {"workload": r["config"]["workload"]}
+                                  for n, r in res.items()}
+        print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 

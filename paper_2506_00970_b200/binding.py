@@ -79,9 +79,8 @@ def load_library():
         lib = C.CDLL(_LIB_PATH)
         for name in EXPORTS:
             getattr(lib, name)  # AttributeError if a declared symbol is not exported
-        lib.sgs_status_string.restype = C.c_char_p
-        for name in EXPORTS[:-1]:
-            getattr(lib, name).restype = C.c_int
+        for name in EXPORTS:
+            getattr(lib, name).restype = C.c_char_p if name == "sgs_status_string" else C.c_int
         _lib = lib
     return _lib
 

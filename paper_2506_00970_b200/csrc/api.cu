@@ -5,6 +5,20 @@
 #include <string.h>
 #include "sgs_internal.h"
 
+// A few words from device memory to MAPPED pinned host memory, written by a kernel.  Used instead of a device-to-host
+// cudaMemcpyAsync for results the host polls or a stream's next kernel sits behind: a copy command queues on the copy
+// engine BEHIND whatever bulk transfer is in flight (measured: with sgs_fetch_grads_host's 104 MB copy-out running, the 28-byte
+// result copy of the next view -- and with it that view's kernels -- waited for it: 18.7 ms per C4 step instead of 12.9).
+__global__ void k_publish_words(unsigned int* __restrict__ dst, const unsigned int* __restrict__ src, int n) {
+    const int i = threadIdx.x;
+    if (i < n) dst[i] = src[i];
+    __threadfence_system();
+}
+cudaError_t sgs_launch_publish(void* dst_mapped, const void* src, int words, cudaStream_t s) {
+    k_publish_words<<<1, 32 * ((words + 31) / 32), 0, s>>>((unsigned int*)dst_mapped, (const unsigned int*)src, words);
+    return cudaGetLastError();
+}
+
 void* sgs_ws_alloc(sgs_ctx* c, size_t bytes, cudaStream_t s) {
     if (bytes == 0) bytes = 16;
     void* p = nullptr;
@@ -204,7 +218,8 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
     bool ok = cudaMalloc(&c->counters, sizeof(SgsCounters)) == cudaSuccess &&
               cudaMalloc(&c->counters_snap, 2 * sizeof(SgsCounters)) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->counters_ready_prev, cudaEventDisableTiming) == cudaSuccess &&
-              cudaMallocHost(&c->counters_host, sizeof(SgsCounters)) == cudaSuccess &&
+              cudaHostAlloc(&c->counters_host, sizeof(SgsCounters), cudaHostAllocMapped) == cudaSuccess &&
+              cudaHostGetDevicePointer(&c->counters_host_dev, c->counters_host, 0) == cudaSuccess &&
               cudaHostAlloc(&c->pinned_small, 8 * sizeof(float), cudaHostAllocMapped) == cudaSuccess &&
               cudaHostAlloc(&c->host_flag, sizeof(unsigned int), cudaHostAllocMapped) == cudaSuccess &&
               cudaMalloc(&c->split_state, sizeof(float) * 8 * SGS_BLOCK * SGS_TRACK_HELPERS) == cudaSuccess &&
@@ -239,7 +254,7 @@ int sgs_destroy(sgs_ctx* c) {
     void* ptrs[] = {c->scan_state, c->vis_to_surfel, c->culled, c->pay.store, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
                     c->sort_state, c->ranges, c->T_final, c->n_last, c->dn_state, c->img_scratch, c->pose_partial, c->resident_store,
                     c->resident_active, c->target_rgb, c->host_img_dev, c->host_up_dev, c->host_grads_dev,
-                    c->win_grads[0], c->win_grads[1], c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->pose_inc, c->ssim_maps, c->surv_cnt, c->surv_in, c->export_keys, c->export_ranges};
+                    c->win_grads[0], c->win_grads[1], c->win_tgt[0], c->win_tgt[1], c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->pose_inc, c->ssim_maps, c->surv_cnt, c->surv_in, c->export_keys, c->export_ranges};
     for (void* p : ptrs) sgs_ws_free(c, p, s);
     if (c->counters) cudaFree(c->counters);
     if (c->counters_snap) cudaFree(c->counters_snap);
@@ -261,6 +276,11 @@ int sgs_destroy(sgs_ctx* c) {
     if (c->join_ev) cudaEventDestroy(c->join_ev);
     if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->in_stream) cudaStreamDestroy(c->in_stream);
+    for (int k = 0; k < 2; ++k) {
+        if (c->win_tgt_ready[k]) cudaEventDestroy(c->win_tgt_ready[k]);
+        if (c->win_tgt_free[k]) cudaEventDestroy(c->win_tgt_free[k]);
+    }
     if (c->win_filled) cudaEventDestroy(c->win_filled);
     if (c->win_drained[0]) cudaEventDestroy(c->win_drained[0]);
     if (c->win_drained[1]) cudaEventDestroy(c->win_drained[1]);

@@ -168,7 +168,13 @@ static int window_setup(sgs_ctx* c, int64_t n, cudaStream_t s) {
             cudaEventCreateWithFlags(&c->win_filled, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&c->win_drained[0], cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&c->win_drained[1], cudaEventDisableTiming) != cudaSuccess ||
-            cudaMallocHost(&c->win_results, sizeof(float) * 8 * SGS_WIN_RING) != cudaSuccess)
+            cudaHostAlloc(&c->win_results, sizeof(float) * 8 * SGS_WIN_RING, cudaHostAllocMapped) != cudaSuccess ||
+            cudaHostGetDevicePointer(&c->win_results_dev, c->win_results, 0) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&c->in_stream, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->win_tgt_ready[0], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->win_tgt_ready[1], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->win_tgt_free[0], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->win_tgt_free[1], cudaEventDisableTiming) != cudaSuccess)
             return SGS_CUDA_ERROR;
     }
     for (int k = 0; k < 2; ++k) {
@@ -195,17 +201,31 @@ int sgs_map_view_host(sgs_ctx* c, const sgs_camera* cam, const float* h_rgb, con
     int r = ensure_host_images(c, px, s);
     if (r != SGS_OK) return r;
     if ((r = window_setup(c, n, s)) != SGS_OK) return r;
-    if ((r = sgs_upload_target(c, cam, h_rgb, h_depth, stream)) != SGS_OK) return r;
+    // keyframe: host -> one of two device buffers on the ctx's upload stream (runs under the previous view's kernels; the
+    // buffer's previous user, two views ago, has recorded win_tgt_free behind its last reader)
+    const int ts = c->win_tgt_slot;
+    c->win_tgt_slot ^= 1;
+    if (c->win_tgt_cap[ts] < px * 4) {
+        if (c->win_tgt_used[ts]) { cudaEventSynchronize(c->win_tgt_free[ts]); c->win_tgt_used[ts] = false; }
+        if (!grow(c, c->win_tgt[ts], c->win_tgt_cap[ts], px * 4, s)) return SGS_OUT_OF_MEMORY;
+    }
+    if (c->win_tgt_used[ts] && cudaStreamWaitEvent(c->in_stream, c->win_tgt_free[ts], 0) != cudaSuccess) return SGS_CUDA_ERROR;
+    float* t_rgb = c->win_tgt[ts]; float* t_depth = t_rgb + 3 * px;
+    if (cudaMemcpyAsync(t_rgb, h_rgb, sizeof(float) * 3 * px, cudaMemcpyHostToDevice, c->in_stream) != cudaSuccess ||
+        cudaMemcpyAsync(t_depth, h_depth, sizeof(float) * px, cudaMemcpyHostToDevice, c->in_stream) != cudaSuccess ||
+        cudaEventRecord(c->win_tgt_ready[ts], c->in_stream) != cudaSuccess)
+        return SGS_CUDA_ERROR;
     const int slot = c->win_slot;
     if (c->win_draining[slot]) {  // the copy-out (and re-zeroing) of this accumulator, two windows ago, must be complete
         if (cudaStreamWaitEvent(s, c->win_drained[slot], 0) != cudaSuccess) return SGS_CUDA_ERROR;
         c->win_draining[slot] = false;
     }
-    sgs_images ren, up, tgt = {c->target_rgb, c->target_depth, nullptr, nullptr};
+    sgs_images ren, up, tgt = {t_rgb, t_depth, nullptr, nullptr};
     dev_images(c->host_img_dev, px, &ren);
     dev_images(c->host_up_dev, px, &up);
     if ((r = sgs_render(c, &c->resident, cam, &ren, stream)) != SGS_OK) return r;
-    float* res = c->win_results + 8 * c->win_n_pending;  // (pinned; this view's loss and pose gradient land here)
+    if (cudaStreamWaitEvent(s, c->win_tgt_ready[ts], 0) != cudaSuccess) return SGS_CUDA_ERROR;
+    float* res = c->win_results_dev + 8 * c->win_n_pending;  // (mapped host memory; this view's loss and pose gradient land here)
     if (cudaMemsetAsync(c->loss_dev, 0, sizeof(float), s) != cudaSuccess) return SGS_CUDA_ERROR;
     if ((r = sgs_mapping_loss(c, cam, &ren, &tgt, lambda_c, w_d, w_n, normal_sign, &up, c->loss_dev, stream)) != SGS_OK) return r;
     if (ssim_weight != 0.f &&
@@ -213,10 +233,13 @@ int sgs_map_view_host(sgs_ctx* c, const sgs_camera* cam, const float* h_rgb, con
         return r;
     sgs_surfel_grads dg;
     window_grads(c, slot, n, &dg);
+    if (cudaEventRecord(c->win_tgt_free[ts], s) != cudaSuccess) return SGS_CUDA_ERROR;   // (the losses were its last readers)
+    c->win_tgt_used[ts] = true;
     if ((r = sgs_backward_accumulate(c, &up, &dg, c->pose6_dev, stream)) != SGS_OK) return r;
     if ((r = sgs_wait_grads(c, stream)) != SGS_OK) return r;
     c->win_dirty = true;
-    if (cudaMemcpyAsync(res, c->loss_dev, sizeof(float) * 7, cudaMemcpyDeviceToHost, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    if (sgs_launch_publish(res, c->loss_dev, 7, s) != cudaSuccess) return SGS_CUDA_ERROR;
+    c->launches += 1;
     c->win_pending[c->win_n_pending].loss = h_loss;
     c->win_pending[c->win_n_pending].pose6 = h_pose6;
     c->win_n_pending += 1;
@@ -250,6 +273,8 @@ int sgs_sync_host(sgs_ctx* c, void* stream) {
     if (!c) return SGS_INVALID_ARGUMENT;
     if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return SGS_CUDA_ERROR;
     if (c->copy_stream && cudaStreamSynchronize(c->copy_stream) != cudaSuccess) return SGS_CUDA_ERROR;
+    if (c->in_stream && cudaStreamSynchronize(c->in_stream) != cudaSuccess) return SGS_CUDA_ERROR;
+    c->win_tgt_used[0] = c->win_tgt_used[1] = false;
     c->win_draining[0] = c->win_draining[1] = false;
     for (int k = 0; k < c->win_n_pending; ++k) {
         const float* res = c->win_results + 8 * k;

@@ -40,8 +40,9 @@ static int check_pending(sgs_ctx* c, cudaStream_t s) {
 }
 
 static int copy_counters(sgs_ctx* c, cudaStream_t s) {
-    return cudaMemcpyAsync(c->counters_host, c->counters, sizeof(SgsCounters), cudaMemcpyDeviceToHost, s) == cudaSuccess
-               ? SGS_OK : SGS_CUDA_ERROR;
+    static_assert(sizeof(SgsCounters) % 4 == 0, "");
+    c->launches += 1;   // (a one-warp kernel to mapped host memory, not a copy command: see k_publish_words)
+    return sgs_launch_publish(c->counters_host_dev, c->counters, (int)(sizeof(SgsCounters) / 4), s) == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
 }
 
 // binning through per-tile buckets + in-tile sort (default)

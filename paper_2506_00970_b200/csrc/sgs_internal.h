@@ -126,7 +126,8 @@ struct sgs_ctx {
     float* img_saved[8];             // planes the backward needs when the caller did not ask for them
     float* img_scratch;              // 8 planes, pix_cap each
     SgsCounters* counters;           // device
-    SgsCounters* counters_host;      // pinned
+    SgsCounters* counters_host;      // pinned + mapped
+    SgsCounters* counters_host_dev;  // its device address
     cudaEvent_t counters_ready;
     cudaStream_t aux_stream;           // sgs_backward: the gradient memsets run beside k_backward (fork / join by events)
     cudaEvent_t fork_ev, join_ev;
@@ -178,7 +179,10 @@ struct sgs_ctx {
     // (one fills while the other drains to the host on copy_stream), and a pinned ring of per-view results
     float* win_grads[2]; int64_t win_cap[2]; int win_slot; bool win_dirty;
     cudaStream_t copy_stream; cudaEvent_t win_filled, win_drained[2]; bool win_draining[2];
-    float* win_results;              // pinned, SGS_WIN_RING x 8 floats: loss, pose6
+    float* win_results; float* win_results_dev;   // pinned + mapped, SGS_WIN_RING x 8 floats: loss, pose6
+    // keyframe uploads of sgs_map_view_host run on their own stream into one of two buffers, under the previous view's kernels
+    cudaStream_t in_stream; float* win_tgt[2]; int64_t win_tgt_cap[2]; int win_tgt_slot;
+    cudaEvent_t win_tgt_ready[2], win_tgt_free[2]; bool win_tgt_used[2];
     struct { float* loss; float* pose6; } win_pending[64]; int win_n_pending;
     int64_t partial_cap;             // floats in pose_partial
     int64_t launches;                // kernels launched by this ctx
@@ -226,6 +230,8 @@ cudaError_t sgs_launch_covisibility(sgs_ctx* c, const float* ca, const float* cb
 cudaError_t sgs_launch_export_bucket(sgs_ctx* c, int64_t n_entries, cudaStream_t s);
 int sgs_ensure_buckets(sgs_ctx* c, int tiles, int64_t tile_cap, cudaStream_t s);
 int sgs_ensure_export(sgs_ctx* c, int tiles, int64_t entries, cudaStream_t s);
+
+cudaError_t sgs_launch_publish(void* dst_mapped, const void* src, int words, cudaStream_t s);  // <= 1024 words
 
 // ---- workspace helpers (api.cu) ----
 void* sgs_ws_alloc(sgs_ctx* c, size_t bytes, cudaStream_t s);

@@ -556,8 +556,8 @@ def test_track_reuse_keeps_the_binning_exact():
     """SGS_FLAG_TRACK_REUSE: along a pose trajectory (steps inside the survivor list's 3 cm / 0.02 rad margin, a step
     that leaves it, another map, a new frame) every iteration's binning is bit-identical to the oracle's and images,
     loss and pose gradient equal those of a context without the flag; the list is rebuilt exactly when it has to be
-    (kernel launch counts: 5 launches when K-pre-A and the gather of the listed splats run, 3 otherwise: K-pre-B, K-track and
-    the one-block tile-order kernel)."""
+    (kernel launch counts: 6 launches when K-pre-A and the gather of the listed splats run, 4 otherwise: K-pre-B, the one-warp
+    kernel that publishes the counters to the host, K-track and the one-block tile-order kernel)."""
     sc, _, _ = scenegen.make_config("C2", n_override=30000)
     sc2 = Scene(sc.mean + np.float32(0.01), sc.scale, sc.quat, sc.opacity, sc.rgb, sc.active)
     cfg = oracle.make_cfg()
@@ -574,14 +574,14 @@ def test_track_reuse_keeps_the_binning_exact():
     ra.track_iter(sf, camera(base), tgt_rgb, tgt_dep, 0.5, -1.0, p0, l0_)   # first call: workspace + tile order set up
     ra.track_new_frame()
     # (tau relative to T0, which map, new frame first?, expected number of kernel launches of the iteration)
-    steps = [([0, 0, 0, 0, 0, 0], 0, False, 5),
-             ([0.01, -0.005, 0.008, 0.004, -0.006, 0.005], 0, False, 3),        # inside the margin: list reused
-             ([-0.015, 0.01, 0.005, -0.008, 0.004, -0.007], 0, False, 3),
-             ([0.05, 0.0, 0.02, 0.0, 0.03, 0.0], 0, False, 5),                   # outside: rebuilt around this pose
-             ([0.055, 0.004, 0.018, 0.003, 0.033, -0.004], 0, False, 3),        # inside the NEW list's margin
-             ([0.055, 0.004, 0.018, 0.003, 0.033, -0.004], 1, False, 5),        # another map
-             ([0.055, 0.004, 0.018, 0.003, 0.033, -0.004], 1, False, 3),
-             ([0.055, 0.004, 0.018, 0.003, 0.033, -0.004], 1, True, 5)]         # new frame
+    steps = [([0, 0, 0, 0, 0, 0], 0, False, 6),
+             ([0.01, -0.005, 0.008, 0.004, -0.006, 0.005], 0, False, 4),        # inside the margin: list reused
+             ([-0.015, 0.01, 0.005, -0.008, 0.004, -0.007], 0, False, 4),
+             ([0.05, 0.0, 0.02, 0.0, 0.03, 0.0], 0, False, 6),                   # outside: rebuilt around this pose
+             ([0.055, 0.004, 0.018, 0.003, 0.033, -0.004], 0, False, 4),        # inside the NEW list's margin
+             ([0.055, 0.004, 0.018, 0.003, 0.033, -0.004], 1, False, 6),        # another map
+             ([0.055, 0.004, 0.018, 0.003, 0.033, -0.004], 1, False, 4),
+             ([0.055, 0.004, 0.018, 0.003, 0.033, -0.004], 1, True, 6)]         # new frame
     for tau, which, new_frame, want_launches in steps:
         T = scenegen.perturb_pose(T0, tau)
         cam = Camera(base.width, base.height, base.fx, base.fy, base.cx, base.cy, T)
