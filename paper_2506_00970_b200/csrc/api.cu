@@ -11,8 +11,7 @@
 // result copy of the next view -- and with it that view's kernels -- waited for it: 18.7 ms per C4 step instead of 12.9).
 __global__ void k_publish_words(unsigned int* __restrict__ dst, const unsigned int* __restrict__ src, int n) {
     const int i = threadIdx.x;
-    if (i < n) dst[i] = src[i];
-    __threadfence_system();
+    if (i < n) dst[i] = src[i];   // (visible to the host once the kernel has completed: every reader waits for that)
 }
 cudaError_t sgs_launch_publish(void* dst_mapped, const void* src, int words, cudaStream_t s) {
     k_publish_words<<<1, 32 * ((words + 31) / 32), 0, s>>>((unsigned int*)dst_mapped, (const unsigned int*)src, words);
@@ -51,7 +50,7 @@ int sgs_ensure_surfels(sgs_ctx* c, int64_t n, cudaStream_t s) {
     cudaStreamSynchronize(s);
     const size_t m = (size_t)(n + n / 8 + 1024);
     const size_t blocks = (m + SGS_PRE_BLOCK - 1) / SGS_PRE_BLOCK + 1;
-    bool ok = ws_realloc(c, c->scan_state, blocks, s) && ws_realloc(c, c->vis_to_surfel, m, s) &&
+    bool ok = ws_realloc(c, c->scan_state, blocks, s) && ws_realloc(c, c->vis_to_surfel, m, s) && ws_realloc(c, c->vis_list, m, s) &&
               ws_realloc(c, c->culled, m, s) && ws_realloc(c, c->pay.store, m * 8, s) &&
               ws_realloc(c, c->acc, m * SGS_ACC_STRIDE, s, true);  // invariant: acc is all-zero between backward calls
     if (!ok) return SGS_OUT_OF_MEMORY;
@@ -251,7 +250,7 @@ int sgs_destroy(sgs_ctx* c) {
     if (!c) return SGS_OK;
     cudaDeviceSynchronize();
     cudaStream_t s = 0;
-    void* ptrs[] = {c->scan_state, c->vis_to_surfel, c->culled, c->pay.store, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
+    void* ptrs[] = {c->scan_state, c->vis_to_surfel, c->vis_list, c->culled, c->pay.store, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
                     c->sort_state, c->ranges, c->T_final, c->n_last, c->dn_state, c->img_scratch, c->pose_partial, c->resident_store,
                     c->resident_active, c->target_rgb, c->host_img_dev, c->host_up_dev, c->host_grads_dev,
                     c->win_grads[0], c->win_grads[1], c->win_tgt[0], c->win_tgt[1], c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->pose_inc, c->ssim_maps, c->surv_cnt, c->surv_in, c->export_keys, c->export_ranges};

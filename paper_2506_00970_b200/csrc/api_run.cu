@@ -25,6 +25,7 @@ static int check_pending(sgs_ctx* c, cudaStream_t s) {
     const int64_t E = (int64_t)c->counters_host->n_entries;
     c->last_entries = E;
     c->last_surv = (int64_t)c->counters_host->n_surv;
+    c->last_vis = (int64_t)c->counters_host->n_visible;
     if (radix_mode(c)) {
         if (c->counters_host->overflow) {
             c->have_forward = c->have_binning = c->prepared = false;
@@ -76,6 +77,7 @@ static int bin_buckets(sgs_ctx* c, const sgs_surfels* sf, bool async, bool want_
         }
         c->last_entries = (int64_t)c->counters_host->n_entries;
         c->last_surv = (int64_t)c->counters_host->n_surv;
+        c->last_vis = (int64_t)c->counters_host->n_visible;
     } else if (!defer && !graph_mode(c)) {
         cudaEventRecord(c->counters_ready, cs);
         c->copy_in_flight = cs != s;

@@ -22,6 +22,9 @@ namespace {
 struct CPlanes { const float* p[8]; };
 
 constexpr int BWD_K = 2;  // entries per trip of the reverse walk
+#ifndef SGS_BWD_MIN_BLOCKS
+#define SGS_BWD_MIN_BLOCKS 4
+#endif
 
 struct StagedBwd {
     float4 s0, s1, s2, s3, s4;  // as StagedFwd
@@ -35,7 +38,7 @@ struct StagedBwd {
 struct FusedLoss { const float* trgb; const float* tdepth; float lambda_d, nsign; float* loss; };
 
 template <bool POSE_ONLY, bool FUSED, bool NDEPTH>
-__global__ void __launch_bounds__(SGS_BLOCK)
+__global__ void __launch_bounds__(SGS_BLOCK, SGS_BWD_MIN_BLOCKS)
 k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
            int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg, CPlanes up,
            const float* __restrict__ T_final, const uint32_t* __restrict__ n_last, float* __restrict__ acc,
@@ -282,14 +285,13 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
     // grid-stride over the surfels: a bounded grid keeps the per-block ticket of the pose reduction off the
     // critical path (one same-address atomic per block)
     float p6[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    // list: the compacted visible surfels (radix binning: acc is indexed by the list position) or K-pre-A's survivor
-    // list (bucket binning: a superset of the visible surfels; acc is indexed by the surfel itself).  Everything
-    // else -- inactive, pre-culled -- keeps the zeros the launcher's memsets wrote.
-    const unsigned int n_loop = survivors ? counters->n_surv : counters->n_visible;
+    // list: the visible surfels, compact (radix binning: vis_to_surfel, acc indexed by the list position; bucket binning:
+    // K-pre-B's vis_list, acc indexed by the surfel itself: `survivors` != 0).  Everything else -- inactive, culled --
+    // keeps the zeros the launcher's memsets wrote.
+    const unsigned int n_loop = counters->n_visible;
     for (unsigned int v = blockIdx.x * blockDim.x + tid; v < n_loop; v += gridDim.x * blockDim.x) {
     const uint32_t i = vis_to_surfel[v];
-    const bool live = survivors ? (culled[i] == 0) : true;
-    if (live) {
+    {
         float a[16];
         float4* ap = reinterpret_cast<float4*>(acc + (size_t)(survivors ? i : v) * SGS_ACC_STRIDE);
 #pragma unroll
@@ -443,14 +445,14 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     // one thread per listed surfel; the list length is only known on the device: grid-stride from a hinted grid
     const bool bucket_mode = c->list_stride == 2;
     int64_t want = n;
-    if (bucket_mode && c->last_surv > 0 && c->last_surv + c->last_surv / 4 < want) want = c->last_surv + c->last_surv / 4;
+    if (c->last_vis > 0 && c->last_vis + c->last_vis / 4 < want) want = c->last_vis + c->last_vis / 4;
     int blocks = (int)((want + 255) / 256);
     if (blocks > 148 * 8) blocks = 148 * 8;
     if (n == 0) return d_pose6 ? cudaMemsetAsync(d_pose6, 0, sizeof(float) * 6, ks) : cudaSuccess;
     if (blocks < 1) blocks = 1;
     c->launches += 1;
     c->grads_on_aux = lazy;
-    k_surfel_backward<<<blocks, 256, 0, ks>>>(c->counters, c->vis_to_surfel, c->culled, c->acc, c->last_surfels.mean,
+    k_surfel_backward<<<blocks, 256, 0, ks>>>(c->counters, bucket_mode ? c->vis_list : c->vis_to_surfel, c->culled, c->acc, c->last_surfels.mean,
                                              c->last_surfels.scale, c->last_surfels.quat, cam, *dg, c->pose_partial,
                                              c->counters, d_pose6, bucket_mode ? 1 : 0, accumulate ? 1 : 0);
     return cudaGetLastError();

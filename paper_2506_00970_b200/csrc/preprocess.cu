@@ -331,7 +331,8 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
               SgsPayload pay, uint8_t* __restrict__ culled, SgsCounters* __restrict__ counters,
               const uint32_t* surv_list, const unsigned int* n_surv_in,  // written by the PREVIOUS grid: no __restrict__,
               // or the compiler may hoist their loads above the conditional grid-dependency wait (it did: stale counts)
-              uint32_t* __restrict__ cursor, uint64_t* __restrict__ bucket, uint32_t tile_cap, SurvInputs cin, int early) {
+              uint32_t* __restrict__ cursor, uint64_t* __restrict__ bucket, uint32_t tile_cap, SurvInputs cin, int early,
+              uint32_t* __restrict__ vis_list) {
     __shared__ unsigned int s_off[SGS_PREB_BLOCK + 1];
     __shared__ unsigned long long s_key[SGS_PREB_BLOCK];
     __shared__ unsigned int s_rect[SGS_PREB_BLOCK];   // tile index of the rectangle's first tile
@@ -373,11 +374,16 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
         unsigned int wcnt = cnt;
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) wcnt += __shfl_xor_sync(0xffffffffu, wcnt, off);
+        unsigned int vbase = 0;
         if (lane == 0 && vis_mask) {
-            atomicAdd(&counters->n_visible, (unsigned int)__popc(vis_mask));
+            vbase = atomicAdd(&counters->n_visible, (unsigned int)__popc(vis_mask));
             atomicAdd(&counters->n_entries, (unsigned long long)wcnt);
         }
+        vbase = __shfl_sync(0xffffffffu, vbase, 0);
         if (o.vis) {
+            // the visible surfels, compact (arrival order): what the per-surfel backward walks -- K-pre-A's survivor list
+            // is several times longer (C4: every splat the frustum test cannot exclude) and costs it a sector per entry
+            vis_list[vbase + __popc(vis_mask & ((1u << lane) - 1u))] = (uint32_t)i;
             if (!cin.p0) { in_o = opacity[i]; in_c[0] = rgb[3 * i]; in_c[1] = rgb[3 * i + 1]; in_c[2] = rgb[3 * i + 2]; }
             pay.g0[i] = make_float4(o.P, o.Q, o.R, o.S);
             pay.g1[i] = make_float4(o.D, o.E, o.F, in_o);
@@ -536,7 +542,7 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     const cudaError_t le = cudaLaunchKernelEx(&cfg, k_pre_project, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd,
                                               c->cfgd, c->pay, c->culled, c->counters, (const uint32_t*)c->vis_to_surfel,
                                               (const unsigned int*)n_surv, c->cursor, c->bucket, (uint32_t)c->tile_cap, cin,
-                                              (cached && prezeroed && cin.p0) ? 1 : 0);
+                                              (cached && prezeroed && cin.p0) ? 1 : 0, c->vis_list);
     if (le != cudaSuccess) return le;
     return cudaGetLastError();
 }

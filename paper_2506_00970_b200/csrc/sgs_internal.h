@@ -87,7 +87,9 @@ struct sgs_ctx {
     int64_t bytes;
     // per-surfel
     unsigned long long* scan_state;  // chained-scan status words, one per K-pre block
-    uint32_t* vis_to_surfel;         // n_cap
+    uint32_t* vis_to_surfel;         // n_cap: radix binning: compact visible index -> surfel; bucket binning: K-pre-A's survivor list
+    uint32_t* vis_list;              // n_cap, bucket binning: the surfels that passed K-pre-B's exact culling (arrival order)
+    int64_t last_vis;                // N_v of the last checked render (grid hint of the per-surfel backward), 0 = unknown
     uint8_t* culled;                 // n_cap
     SgsPayload pay;                  // n_cap each
     float* acc;                      // n_cap x 16 backward accumulators
