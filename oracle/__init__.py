@@ -49,16 +49,18 @@ def _p(a, t):
     return None if a is None else a.ctypes.data_as(t)
 
 
-def make_cfg(tile=16, cutoff=3.0, alpha_min=1.0 / 255.0, alpha_max=0.99, t_min=1e-4, z_near=0.2):
+def make_cfg(tile=16, cutoff=3.0, alpha_min=1.0 / 255.0, alpha_max=0.99, t_min=1e-4, z_near=0.2, tight=False):
     """Truncation constants (readings R3-R7).  Values pass through float32 first because the C-ABI
-    config struct holds floats: both sides then use the identical real numbers."""
+    config struct holds floats: both sides then use the identical real numbers.  tight: the binning variant of
+    readings R26 + R27 (opacity-aware cutoff, tile-exact culling) -- the rendered function is the
+    same, the tile lists are shorter."""
     f = lambda v: float(np.float32(v))
-    return np.array([tile, f(cutoff), f(alpha_min), f(alpha_max), f(t_min), f(z_near)], dtype=np.float64)
+    return np.array([tile, f(cutoff), f(alpha_min), f(alpha_max), f(t_min), f(z_near), 1.0 if tight else 0.0, 0.0], dtype=np.float64)
 
 
 def smooth_cfg(tile=16):
     """Plain Eq. 8: no cutoff, no alpha bounds, no stop, no near plane (used for finite differences)."""
-    return np.array([tile, np.inf, 0.0, 1.0, 0.0, 0.0], dtype=np.float64)
+    return np.array([tile, np.inf, 0.0, 1.0, 0.0, 0.0, 0.0, 0.0], dtype=np.float64)
 
 
 def make_cam(cam, T_cw=None, widen_from_f32=True):
@@ -78,12 +80,19 @@ def _scene_arrays(sc):
     return f(sc.mean), f(sc.scale), f(sc.quat), f(sc.opacity), f(sc.rgb), act
 
 
+def two_ln_upper(r):
+    """The upper bound of 2 ln r the tight binning uses for the opacity-aware cutoff (reading R26)."""
+    f = lib().orc_two_ln_upper
+    f.restype = ctypes.c_double
+    return float(f(ctypes.c_double(r)))
+
+
 def preprocess(sc, camv, cfgv):
-    mean, scale, quat, _, _, act = _scene_arrays(sc)
+    mean, scale, quat, opac, _, act = _scene_arrays(sc)
     n = mean.shape[0]
     out = dict(culled=np.zeros(n, np.uint8), depth_bits=np.zeros(n, np.uint32), rect=np.zeros((n, 4), np.int32),
                count=np.zeros(n, np.uint32), M=np.zeros((n, 9)), aabb=np.zeros((n, 4)))
-    E = lib().orc_preprocess(ctypes.c_int64(n), _p(mean, C_F32), _p(scale, C_F32), _p(quat, C_F32), _p(act, C_U8),
+    E = lib().orc_preprocess(ctypes.c_int64(n), _p(mean, C_F32), _p(scale, C_F32), _p(quat, C_F32), _p(opac, C_F32), _p(act, C_U8),
                              _p(camv, C_F64), _p(cfgv, C_F64), _p(out["culled"], C_U8), _p(out["depth_bits"], C_U32),
                              _p(out["rect"], C_I32), _p(out["count"], C_U32), _p(out["M"], C_F64), _p(out["aabb"], C_F64))
     out["E"] = int(E)
@@ -99,8 +108,9 @@ def binning(sc, camv, cfgv):
     keys = np.zeros(max(E, 1), np.uint64)
     idx = np.zeros(max(E, 1), np.uint32)
     ranges = np.zeros((tx * ty, 2), np.uint32)
-    lib().orc_bin(ctypes.c_int64(sc.n), _p(pre["culled"], C_U8), _p(pre["depth_bits"], C_U32), _p(pre["rect"], C_I32),
-                  ctypes.c_int(tx), ctypes.c_int(ty), ctypes.c_int64(E), _p(keys, C_U64), _p(idx, C_U32), _p(ranges, C_U32))
+    mean, scale, quat, opac, _, act = _scene_arrays(sc)
+    lib().orc_bin(ctypes.c_int64(sc.n), _p(mean, C_F32), _p(scale, C_F32), _p(quat, C_F32), _p(opac, C_F32), _p(act, C_U8),
+                  _p(camv, C_F64), _p(cfgv, C_F64), ctypes.c_int64(E), _p(keys, C_U64), _p(idx, C_U32), _p(ranges, C_U32))
     pre.update(keys=keys[:E], idx=idx[:E], ranges=ranges, tiles_x=tx, tiles_y=ty)
     return pre
 

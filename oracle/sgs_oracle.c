@@ -38,6 +38,7 @@ typedef struct {
 typedef struct {
     int tile;
     double cutoff, alpha_min, alpha_max, t_min, z_near;
+    int tight; /* binning variant of readings R26 + R27: opacity-aware cutoff and tile-exact culling */
 } Cfg;
 
 /* Per-surfel derived quantities (all fp64). */
@@ -51,6 +52,10 @@ typedef struct {
     double Rw[9];        /* R(qh), columns t_u, t_v, t_n (world) */
     double tuc[3], tvc[3], tnc[3], muc[3];
     double M[9];         /* rows M0, M1, M2 of K [s_u t_uc, s_v t_vc, mu_c] */
+    /* tight binning only: c2k = the splat's own cutoff^2 (R26); the footprint rho^2 <= c2k as the screen conic
+     * q(x', y') = A x'^2 + 2 B x' y' + C y'^2 + 2 D x' + 2 E y' + F <= 0 in coordinates relative to (q_cx, q_cy) (R27) */
+    double c2k, q_cx, q_cy, qA, qB, qC, qD, qE, qF;
+    int q_ok;            /* the conic is a well-conditioned ellipse: the per-tile test applies (else every tile of the rect is listed) */
 } Prep;
 
 static void load_cam(const double* c, Cam* cam) {
@@ -64,7 +69,27 @@ static void load_cam(const double* c, Cam* cam) {
 static void load_cfg(const double* c, Cfg* cfg) {
     cfg->tile = (int)c[0]; cfg->cutoff = c[1]; cfg->alpha_min = c[2];
     cfg->alpha_max = c[3]; cfg->t_min = c[4]; cfg->z_near = c[5];
+    cfg->tight = c[6] != 0.0;
 }
+
+/* R26: an UPPER bound of 2 ln r (r >= 1) from +, -, x, / alone, so that the CUDA preprocess can evaluate the identical
+ * binary64 sequence (no transcendental in the binning path):  r = m 2^e with m in [1, 2) by exact halvings;
+ * ln m = 2 atanh(t), t = (m - 1) / (m + 1) <= 1/3, by 13 terms of the odd series in Horner form (truncation < 2e-13);
+ * the result is inflated by 1e-9 relative + 1e-9 absolute, far above the series' and the roundings' error.  An upper bound
+ * keeps the variant conservative: a pair with o G >= alpha_min always has rho^2 <= 2 ln(o / alpha_min) <= two_ln_upper(). */
+static double two_ln_upper(double r) {
+    double m = r, e = 0.0;
+    while (m >= 2.0) { m = m * 0.5; e = e + 1.0; }
+    const double t = (m - 1.0) / (m + 1.0), t2 = t * t;
+    double p = 1.0 / 25.0;
+    p = p * t2 + 1.0 / 23.0; p = p * t2 + 1.0 / 21.0; p = p * t2 + 1.0 / 19.0; p = p * t2 + 1.0 / 17.0;
+    p = p * t2 + 1.0 / 15.0; p = p * t2 + 1.0 / 13.0; p = p * t2 + 1.0 / 11.0; p = p * t2 + 1.0 / 9.0;
+    p = p * t2 + 1.0 / 7.0; p = p * t2 + 1.0 / 5.0; p = p * t2 + 1.0 / 3.0; p = p * t2 + 1.0;
+    const double ln_m = 2.0 * (t * p);
+    const double ln_r = e * 0.69314718055994540 + ln_m;   /* (0.6931471805599454 > ln 2 = 0.693147180559945309...) */
+    return (2.0 * ln_r) * (1.0 + 1e-9) + 1e-9;
+}
+double orc_two_ln_upper(double r) { return two_ln_upper(r); }
 
 static uint32_t f32_bits(float f) { uint32_t u; memcpy(&u, &f, 4); return u; }
 
@@ -84,7 +109,7 @@ static uint32_t f32_bits(float f) { uint32_t u; memcpy(&u, &f, 4); return u; }
  */
 static inline double dot3r(const double* r, const double* v) { return (r[0] * v[0] + r[1] * v[1]) + r[2] * v[2]; }
 
-static void prep_surfel(const float* mean, const float* scale, const float* quat, int is_active,
+static void prep_surfel(const float* mean, const float* scale, const float* quat, float opacity, int is_active,
                         const Cam* cam, const Cfg* cfg, Prep* p) {
     memset(p, 0, sizeof(*p));
     p->culled = 1;
@@ -126,7 +151,16 @@ static void prep_surfel(const float* mean, const float* scale, const float* quat
         p->culled = 0;
         return;
     }
-    const double c2 = cfg->cutoff * cfg->cutoff;
+    double c2 = cfg->cutoff * cfg->cutoff;
+    if (cfg->tight && cfg->alpha_min > 0.0) {
+        /* R26: the splat's own support.  a = min(alpha_max, o G) >= alpha_min  <=>  o exp(-rho^2 / 2) >= alpha_min  <=>
+         * rho^2 <= 2 ln(o / alpha_min); a splat with o < alpha_min contributes nowhere and is culled. */
+        const double r = (double)opacity / cfg->alpha_min;
+        if (!(r >= 1.0)) return;
+        const double c2o = two_ln_upper(r);
+        if (c2o < c2) c2 = c2o;
+    }
+    p->c2k = c2;
     const double den = c2 * (M[6] * M[6] + M[7] * M[7]) - M[8] * M[8];
     if (!(den < 0.0)) return;
     const double ctrx = (c2 * (M[0] * M[6] + M[1] * M[7]) - M[2] * M[8]) / den;
@@ -147,24 +181,77 @@ static void prep_surfel(const float* mean, const float* scale, const float* quat
     const int tx0 = (int)fx0, tx1 = (int)fx1, ty0 = (int)fy0, ty1 = (int)fy1;
     p->rect[0] = tx0; p->rect[1] = ty0; p->rect[2] = tx1; p->rect[3] = ty1;
     p->culled = 0;
+    if (cfg->tight) {
+        /* R27: the footprint as a conic.  k = (M0 - x M2) x (M1 - y M2) = C0 + x Cx + y Cy with C0 = M0 x M1, Cx = M1 x M2,
+         * Cy = M2 x M0, so k_x = a.p, k_y = b.p, k_z = c.p for p = (x, y, 1) and rho^2 <= c2k  <=>
+         * (a.p)^2 + (b.p)^2 - c2k (c.p)^2 <= 0.  Coordinates are taken relative to the AABB's centre (ctr_x, ctr_y). */
+        const double C0[3] = {M[1] * M[5] - M[2] * M[4], M[2] * M[3] - M[0] * M[5], M[0] * M[4] - M[1] * M[3]};
+        const double Cx[3] = {M[4] * M[8] - M[5] * M[7], M[5] * M[6] - M[3] * M[8], M[3] * M[7] - M[4] * M[6]};
+        const double Cy[3] = {M[7] * M[2] - M[8] * M[1], M[8] * M[0] - M[6] * M[2], M[6] * M[1] - M[7] * M[0]};
+        const double a1 = Cx[0], a2 = Cy[0], a3 = (Cx[0] * ctrx + Cy[0] * ctry) + C0[0];
+        const double b1 = Cx[1], b2 = Cy[1], b3 = (Cx[1] * ctrx + Cy[1] * ctry) + C0[1];
+        const double c1 = Cx[2], c2_ = Cy[2], c3 = (Cx[2] * ctrx + Cy[2] * ctry) + C0[2];
+        p->q_cx = ctrx; p->q_cy = ctry;
+        p->qA = (a1 * a1 + b1 * b1) - c2 * (c1 * c1);
+        p->qB = (a1 * a2 + b1 * b2) - c2 * (c1 * c2_);
+        p->qC = (a2 * a2 + b2 * b2) - c2 * (c2_ * c2_);
+        p->qD = (a1 * a3 + b1 * b3) - c2 * (c1 * c3);
+        p->qE = (a2 * a3 + b2 * b3) - c2 * (c2_ * c3);
+        p->qF = (a3 * a3 + b3 * b3) - c2 * (c3 * c3);
+        const double det = p->qA * p->qC - p->qB * p->qB;
+        p->q_ok = p->qA > 0.0 && p->qC > 0.0 && det > 1e-12 * (p->qA * p->qC);
+    }
 }
 
-static Prep* prep_all(int64_t n, const float* mean, const float* scale, const float* quat,
+/* R27: is tile (tx, ty) of the surfel's rectangle LISTED?  Always in the default binning.  Tight binning: iff the
+ * ellipse q <= 0 meets the rectangle spanned by the tile's pixel centres (clipped to the image).  q is convex, so its
+ * minimum over the rectangle is attained at the ellipse centre clamped into the rectangle or on one of the four edges
+ * (each a 1-D convex quadratic, minimised and clamped); listed iff that minimum is <= tol, tol = 1e-9 of the largest
+ * magnitude q's terms reach on the rectangle (conservative against the binary64 rounding of the coefficients). */
+static inline double conic_q(const Prep* p, double x, double y) {
+    return ((((p->qA * x) * x + (2.0 * p->qB) * (x * y)) + (p->qC * y) * y) + ((2.0 * p->qD) * x + (2.0 * p->qE) * y)) + p->qF;
+}
+static inline double clampd(double v, double lo, double hi) { return v < lo ? lo : (v > hi ? hi : v); }
+static int tile_listed(const Prep* p, int tx, int ty, const Cam* cam, const Cfg* cfg) {
+    if (!cfg->tight || !p->q_ok) return 1;
+    const double ts = (double)cfg->tile;
+    double x1 = ts * tx + (ts - 0.5), y1 = ts * ty + (ts - 0.5);
+    if (x1 > cam->W - 0.5) x1 = cam->W - 0.5;
+    if (y1 > cam->H - 0.5) y1 = cam->H - 0.5;
+    const double x0 = (ts * tx + 0.5) - p->q_cx, y0 = (ts * ty + 0.5) - p->q_cy;
+    x1 = x1 - p->q_cx; y1 = y1 - p->q_cy;
+    const double det = p->qA * p->qC - p->qB * p->qB;
+    const double xc = (p->qB * p->qE - p->qC * p->qD) / det, yc = (p->qB * p->qD - p->qA * p->qE) / det;
+    double qm = conic_q(p, clampd(xc, x0, x1), clampd(yc, y0, y1));
+    double v;
+    v = conic_q(p, x0, clampd(-(p->qB * x0 + p->qE) / p->qC, y0, y1)); if (v < qm) qm = v;
+    v = conic_q(p, x1, clampd(-(p->qB * x1 + p->qE) / p->qC, y0, y1)); if (v < qm) qm = v;
+    v = conic_q(p, clampd(-(p->qB * y0 + p->qD) / p->qA, x0, x1), y0); if (v < qm) qm = v;
+    v = conic_q(p, clampd(-(p->qB * y1 + p->qD) / p->qA, x0, x1), y1); if (v < qm) qm = v;
+    double R = fabs(x0);
+    if (fabs(x1) > R) R = fabs(x1);
+    if (fabs(y0) > R) R = fabs(y0);
+    if (fabs(y1) > R) R = fabs(y1);
+    const double tol = 1e-9 * ((fabs(p->qF) + (2.0 * (fabs(p->qD) + fabs(p->qE))) * R) + ((p->qA + p->qC) + 2.0 * fabs(p->qB)) * (R * R));
+    return qm <= tol;
+}
+
+static Prep* prep_all(int64_t n, const float* mean, const float* scale, const float* quat, const float* opacity,
                       const uint8_t* active, const Cam* cam, const Cfg* cfg) {
     Prep* P = (Prep*)malloc(sizeof(Prep) * (size_t)(n > 0 ? n : 1));
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < n; ++i)
-        prep_surfel(mean + 3 * i, scale + 2 * i, quat + 4 * i, active ? active[i] != 0 : 1, cam, cfg, P + i);
+        prep_surfel(mean + 3 * i, scale + 2 * i, quat + 4 * i, opacity ? opacity[i] : 1.f, active ? active[i] != 0 : 1, cam, cfg, P + i);
     return P;
 }
 
 /* ---- public: stage O2, per-surfel part.  Returns E = sum of tile counts. ---- */
-int64_t orc_preprocess(int64_t n, const float* mean, const float* scale, const float* quat,
+int64_t orc_preprocess(int64_t n, const float* mean, const float* scale, const float* quat, const float* opacity,
                        const uint8_t* active, const double* camv, const double* cfgv,
                        uint8_t* culled, uint32_t* depth_bits, int32_t* rect, uint32_t* count,
                        double* M_out, double* aabb_out) {
     Cam cam; Cfg cfg; load_cam(camv, &cam); load_cfg(cfgv, &cfg);
-    Prep* P = prep_all(n, mean, scale, quat, active, &cam, &cfg);
+    Prep* P = prep_all(n, mean, scale, quat, opacity, active, &cam, &cfg);
     int64_t E = 0;
     for (int64_t i = 0; i < n; ++i) {
         const Prep* p = P + i;
@@ -172,7 +259,9 @@ int64_t orc_preprocess(int64_t n, const float* mean, const float* scale, const f
         depth_bits[i] = p->culled ? 0u : p->depth_bits;
         uint32_t c = 0;
         for (int j = 0; j < 4; ++j) rect[4 * i + j] = p->culled ? 0 : p->rect[j];
-        if (!p->culled) c = (uint32_t)((p->rect[2] - p->rect[0] + 1) * (p->rect[3] - p->rect[1] + 1));
+        if (!p->culled)
+            for (int ty = p->rect[1]; ty <= p->rect[3]; ++ty)
+                for (int tx = p->rect[0]; tx <= p->rect[2]; ++tx) c += (uint32_t)tile_listed(p, tx, ty, &cam, &cfg);
         count[i] = c;
         E += c;
         if (M_out) memcpy(M_out + 9 * i, p->M, sizeof(double) * 9);
@@ -192,19 +281,26 @@ static int cmp_entry(const void* a, const void* b) {
 
 /* ---- public: stage O2, list part.  key = tile_id << 32 | depth bits (R2); entries emitted
  * surfel-major, tiles row-major; stable sort => ties ordered by surfel index; ranges[t] = [start,end). */
-void orc_bin(int64_t n, const uint8_t* culled, const uint32_t* depth_bits, const int32_t* rect,
-             int tiles_x, int tiles_y, int64_t E, uint64_t* keys, uint32_t* idx, uint32_t* ranges) {
+void orc_bin(int64_t n, const float* mean, const float* scale, const float* quat, const float* opacity,
+             const uint8_t* active, const double* camv, const double* cfgv, int64_t E, uint64_t* keys, uint32_t* idx,
+             uint32_t* ranges) {
+    Cam cam; Cfg cfg; load_cam(camv, &cam); load_cfg(cfgv, &cfg);
+    Prep* P = prep_all(n, mean, scale, quat, opacity, active, &cam, &cfg);
+    const int tiles_x = (cam.W + cfg.tile - 1) / cfg.tile, tiles_y = (cam.H + cfg.tile - 1) / cfg.tile;
     Entry* e = (Entry*)malloc(sizeof(Entry) * (size_t)(E > 0 ? E : 1));
     int64_t m = 0;
     for (int64_t i = 0; i < n; ++i) {
-        if (culled[i]) continue;
-        for (int ty = rect[4 * i + 1]; ty <= rect[4 * i + 3]; ++ty)
-            for (int tx = rect[4 * i + 0]; tx <= rect[4 * i + 2]; ++tx) {
-                e[m].key = ((uint64_t)(uint32_t)(ty * tiles_x + tx) << 32) | depth_bits[i];
+        const Prep* p = P + i;
+        if (p->culled) continue;
+        for (int ty = p->rect[1]; ty <= p->rect[3]; ++ty)
+            for (int tx = p->rect[0]; tx <= p->rect[2]; ++tx) {
+                if (!tile_listed(p, tx, ty, &cam, &cfg)) continue;
+                e[m].key = ((uint64_t)(uint32_t)(ty * tiles_x + tx) << 32) | p->depth_bits;
                 e[m].idx = (uint32_t)i;
                 ++m;
             }
     }
+    free(P);
     qsort(e, (size_t)m, sizeof(Entry), cmp_entry);
     const int tiles = tiles_x * tiles_y;
     for (int t = 0; t < tiles; ++t) { ranges[2 * t] = 0; ranges[2 * t + 1] = 0; }
@@ -245,7 +341,7 @@ static uint32_t* global_order(int64_t n, const Prep* P, int64_t* n_vis) {
  * Q_t, the pairs a tile-list traversal tests).  B equals the tile size so the flag is meaningful.
  */
 typedef struct { int bx, by, B; int64_t* start; uint32_t* list; } Buckets;
-static void build_buckets(const Prep* P, const uint32_t* ord, int64_t n_vis, const Cam* cam, int B, Buckets* bk) {
+static void build_buckets(const Prep* P, const uint32_t* ord, int64_t n_vis, const Cam* cam, const Cfg* cfg, int B, Buckets* bk) {
     bk->B = B; bk->bx = (cam->W + B - 1) / B; bk->by = (cam->H + B - 1) / B;
     const int nb = bk->bx * bk->by;
     bk->start = (int64_t*)calloc((size_t)nb + 1, sizeof(int64_t));
@@ -271,7 +367,8 @@ static void build_buckets(const Prep* P, const uint32_t* ord, int64_t n_vis, con
                 for (int bx = (int)x0; bx <= (int)x1; ++bx) {
                     const int b = by * bk->bx + bx;
                     if (pass == 0) { bk->start[b]++; continue; }
-                    const int inside = bx >= p->rect[0] && bx <= p->rect[2] && by >= p->rect[1] && by <= p->rect[3];
+                    const int inside = bx >= p->rect[0] && bx <= p->rect[2] && by >= p->rect[1] && by <= p->rect[3] &&
+                                       tile_listed(p, bx, by, cam, cfg);
                     bk->list[fill[b]++] = (uint32_t)j | (inside ? 0x80000000u : 0u); /* j = rank in ord */
                 }
         }
@@ -352,9 +449,9 @@ static void ctx_init(Ctx* c, int64_t n, const float* mean, const float* scale, c
                      const double* camv, const double* cfgv, int brute) {
     load_cam(camv, &c->cam); load_cfg(cfgv, &c->cfg);
     c->n = n; c->opacity = opacity; c->rgb = rgb; c->brute = brute;
-    c->P = prep_all(n, mean, scale, quat, active, &c->cam, &c->cfg);
+    c->P = prep_all(n, mean, scale, quat, opacity, active, &c->cam, &c->cfg);
     c->ord = global_order(n, c->P, &c->n_vis);
-    build_buckets(c->P, c->ord, c->n_vis, &c->cam, c->cfg.tile, &c->bk);
+    build_buckets(c->P, c->ord, c->n_vis, &c->cam, &c->cfg, c->cfg.tile, &c->bk);
 }
 static void ctx_free(Ctx* c) { free(c->P); free(c->ord); free_buckets(&c->bk); }
 

@@ -912,3 +912,98 @@ def test_p17_median_depth_against_numpy_on_closed_form_footprints():
     assert m.sum() > 50
     np.testing.assert_allclose(med1[m], z[m], rtol=1e-12)
     assert (med1[r1["img"][7] < 0.5 - 1e-3] == 0).all()
+
+
+# ---------------------------------------------------------------- P18: tight binning (readings R26, R27)
+def test_p18_two_ln_upper_is_a_tight_upper_bound():
+    """R26's logarithm from +, -, x, / alone: never below 2 ln r (conservative), never more than 3e-9 (rel + abs) above."""
+    rs = np.concatenate([[1.0, 1.0 + 2.0 ** -40, 2.0, 4.0, 255.0, 255.0 * 0.1, 1e6], np.exp(np.linspace(0, 14, 400)),
+                         255.0 * np.linspace(1 / 255, 1, 200), 2.0 ** np.arange(0, 20) * (1 - 2.0 ** -52)])
+    rs = rs[rs >= 1.0]
+    got = np.array([oracle.two_ln_upper(float(r)) for r in rs])
+    ref = 2.0 * np.log(rs)
+    assert (got >= ref).all()
+    assert (got <= ref * (1 + 3e-9) + 3e-9).all()
+
+
+def _tight_pair(sc, cam, T=None):
+    camv = oracle.make_cam(cam, T)
+    return camv, oracle.make_cfg(), oracle.make_cfg(tight=True)
+
+
+def test_p18_tight_binning_leaves_the_rendered_function_unchanged(c1):
+    """The variant only shortens the tile lists: images, transmittance, composited counts are bit-identical to the default
+    binning in fp64 (brute force and skipping mode) and the gradients agree to the order of the fp64 sums."""
+    sc, cam, camv, cfg, r = c1
+    _, _, cfgt = _tight_pair(sc, cam)
+    for brute in (False, True):
+        rt = oracle.render(sc, camv, cfgt, brute=brute)
+        assert np.array_equal(rt["img"], r["img"]) and np.array_equal(rt["T_final"], r["T_final"])
+        assert np.array_equal(rt["n_comp"], r["n_comp"])
+    assert oracle.render(sc, camv, cfgt)["counters"]["Q_t"] < 0.9 * r["counters"]["Q_t"]      # ... but fewer pairs are tested
+    up = scenegen.upstream_normal(1, cam.height, cam.width)
+    g, gt = oracle.backward(sc, camv, cfg, up), oracle.backward(sc, camv, cfgt, up)
+    for k in ("mean", "scale", "quat", "opacity", "rgb", "pose"):
+        np.testing.assert_allclose(gt[k], g[k], rtol=1e-10, atol=1e-9)
+
+
+def test_p18_tight_lists_are_conservative_and_shorter(c1):
+    """Every pair that can be composited -- rho^2 <= min(c^2, 2 ln(o / alpha_min)) with (u, v) from a LIBRARY matrix inverse
+    and numpy's log -- lies in its pixel's tile list; the list is a subset of the default one; counts add up."""
+    sc, cam, camv, cfg, r = c1
+    cam2 = Camera(200, 120, 150.0, 150.0, 97.0, 63.0, scenegen.perturb_pose(np.eye(4)[:3], [0.05, -0.02, 0.1, 0.03, 0.05, -0.2]))
+    for cm in (cam, cam2):
+        cv, cfg0, cfgt = _tight_pair(sc, cm)
+        b0, bt = oracle.binning(sc, cv, cfg0), oracle.binning(sc, cv, cfgt)
+        assert bt["E"] == int(bt["count"].sum()) == len(bt["keys"]) and bt["E"] < 0.9 * b0["E"]
+        assert (np.diff(bt["keys"].astype(np.uint64)) >= 0).all()
+        assert set(zip(bt["keys"].tolist(), bt["idx"].tolist())) <= set(zip(b0["keys"].tolist(), b0["idx"].tolist()))
+        assert ((bt["culled"] == 0) <= (b0["culled"] == 0)).all()
+        X, Y = pix_grid(cm)
+        tid = (np.arange(cm.height)[:, None] // 16) * bt["tiles_x"] + (np.arange(cm.width)[None, :] // 16)
+        members = [set(bt["idx"][s:e].tolist()) for s, e in bt["ranges"]]
+        amin = cfg0[2]
+        n_pairs = 0
+        for k in np.nonzero(b0["culled"] == 0)[0]:
+            u, v = _numpy_uv(b0["M"][k].reshape(3, 3), X, Y)
+            c2k = min(9.0, 2.0 * np.log(float(sc.opacity[k]) / amin))
+            cover = (u * u + v * v <= c2k)
+            n_pairs += int(cover.sum())
+            for t in np.unique(tid[cover]):
+                assert k in members[t], (k, t)
+        assert n_pairs > 2000
+
+
+def test_p18_lone_splat_lists_exactly_the_tiles_its_support_reaches():
+    """A large faint splat (o = 0.1: support rho^2 <= 2 ln(25.5) = 6.48 < 9), tilted: the tight list is the set of tiles
+    whose pixel-centre rectangle the support ellipse reaches, found here by dense sampling of rho^2 (0.1 px grid, library
+    inverse) -- a tile the sampling finds must be listed; a listed tile the sampling misses must be a corner graze."""
+    rot = Rotation.from_euler("xyz", [40, -30, 20], degrees=True)
+    qx, qy, qz, qw = rot.as_quat()
+    cam = Camera(160, 112, 140.0, 140.0, 80.0, 56.0)
+    sc = one_surfel((0.05, -0.02, 1.6), (0.22, 0.12), (qw, qx, qy, qz), 0.1)
+    camv, cfg0, cfgt = _tight_pair(sc, cam)
+    b0, bt = oracle.binning(sc, camv, cfg0), oracle.binning(sc, camv, cfgt)
+    assert bt["E"] < b0["E"] and bt["E"] > 8
+    listed = set((bt["keys"] >> np.uint64(32)).astype(int).tolist())
+    M = b0["M"][0].reshape(3, 3)
+    c2k = oracle.two_ln_upper(float(np.float32(0.1)) / cfg0[2])
+    assert abs(c2k - 2 * np.log(25.5)) < 1e-6
+    hit, near = set(), set()
+    for ty in range(bt["tiles_y"]):
+        for tx in range(bt["tiles_x"]):
+            xs = np.linspace(16 * tx + 0.5, min(16 * tx + 15.5, cam.width - 0.5), 151)
+            ys = np.linspace(16 * ty + 0.5, min(16 * ty + 15.5, cam.height - 0.5), 151)
+            Xs, Ys = np.meshgrid(xs, ys)
+            u, v = _numpy_uv(M, Xs, Ys)
+            m = (u * u + v * v).min()
+            if m <= c2k:
+                hit.add(ty * bt["tiles_x"] + tx)
+            if m <= c2k * 1.02:
+                near.add(ty * bt["tiles_x"] + tx)
+    assert hit <= listed <= near, (sorted(listed - hit), sorted(hit - listed))
+    assert len(hit) >= 10
+    # o < alpha_min: the splat has no support at all and is culled
+    faint = one_surfel((0.05, -0.02, 1.6), (0.22, 0.12), (qw, qx, qy, qz), 0.003)
+    assert oracle.binning(faint, camv, cfgt)["culled"][0] == 1 and oracle.binning(faint, camv, cfg0)["culled"][0] == 0
+    assert oracle.render(faint, camv, cfg0)["img"].max() == 0.0
