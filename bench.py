@@ -156,7 +156,8 @@ def aggregate_replicas(ms_local, pixels, renders_per_rank, world, dist=None, dev
 class Workload:
     """Device-resident inputs + the step function for one config."""
 
-    def __init__(self, name, iters_override=None, contrib=False, prefetch=True, reuse=True, normalised_depth=False, graph=False):
+    def __init__(self, name, iters_override=None, contrib=False, prefetch=True, reuse=True, normalised_depth=False, graph=False,
+                 tight=False):
         self.contrib = contrib
         self.graph, self.cg, self.eager_steps = graph, None, 0
         nd = self.normalised_depth = normalised_depth
@@ -172,14 +173,15 @@ class Workload:
         self.t = dict(mean=d(sc.mean), scale=d(sc.scale), quat=d(sc.quat), opacity=d(sc.opacity), rgb=d(sc.rgb),
                       active=d(sc.active, torch.uint8))
         self.sf = sgs.Renderer.surfels(*(self.t[k] for k in ("mean", "scale", "quat", "opacity", "rgb", "active")))
-        self.ren = sgs.Renderer(async_mode=not graph, graph=graph, track_reuse=self.tracking and reuse, normalised_depth=nd)
+        self.ren = sgs.Renderer(async_mode=not graph, graph=graph, track_reuse=self.tracking and reuse, normalised_depth=nd,
+                                tight_binning=tight)
         # mapping window: a second context + a side stream, so that sgs_prepare (binning) of view v+1 runs under the
         # compositing kernels of view v (include/sgs.h); tracking iterations depend on one another and use one context
         two = prefetch and not self.tracking and len(self.cams) > 1 and not graph   # (capture mode: one context, one stream)
         if two:  # + SGS_FLAG_LAZY_GRADS: a view's per-surfel kernel runs under the next view's forward; joined at the step's end
             self.ren.close()
-            self.ren = sgs.Renderer(async_mode=True, lazy_grads=True, normalised_depth=nd)
-        self.rens = [self.ren] + ([sgs.Renderer(async_mode=True, lazy_grads=True, normalised_depth=nd)] if two else [])
+            self.ren = sgs.Renderer(async_mode=True, lazy_grads=True, normalised_depth=nd, tight_binning=tight)
+        self.rens = [self.ren] + ([sgs.Renderer(async_mode=True, lazy_grads=True, normalised_depth=nd, tight_binning=tight)] if two else [])
         self.side = torch.cuda.Stream(priority=-1) if len(self.rens) > 1 else None
         cam0 = self.cams[0]
         self.H, self.W = cam0.height, cam0.width
@@ -425,7 +427,8 @@ def run_config(name, args, torch, dist, world, rank, local, peaks):
             dist.barrier()
         torch.cuda.synchronize()
 
-    wl = Workload(name, args.iters, args.contrib, not args.no_prefetch, not args.no_reuse, args.normalised_depth, args.graph)
+    wl = Workload(name, args.iters, args.contrib, not args.no_prefetch, not args.no_reuse, args.normalised_depth, args.graph,
+                  args.tight)
     K, W = args.steps, max(args.warmup, 3)
     per_step = []
     for _ in range(W):
@@ -511,6 +514,8 @@ def run_config(name, args, torch, dist, world, rank, local, peaks):
         out["config"]["gradients"] = f"summed over windows of {WINDOW} views (sgs_backward_accumulate), zeroed per window"
     if args.graph:
         out["config"]["launch"] = "one CUDA graph per step (SGS_FLAG_GRAPH); not the default workload"
+    if args.tight:
+        out["config"]["binning_variant"] = "SGS_FLAG_TIGHT_BINNING (readings R26, R27); not the default workload"
     if args.normalised_depth:
         out["config"]["depth"] = "normalised D/O (SGS_FLAG_NORMALISED_DEPTH); not the default workload"
     sc, cams, tracking, n_active = wl.sc, wl.cams, wl.tracking, wl.n_active
@@ -524,7 +529,7 @@ def run_config(name, args, torch, dist, world, rank, local, peaks):
     import oracle
     out["cpu_baseline"] = cpu_baseline(sc, cams, name)
     # algorithmic work per render from the oracle's counters (view 0 stands for every view)
-    camv, cfg = oracle.make_cam(cams[0]), oracle.make_cfg()
+    camv, cfg = oracle.make_cam(cams[0]), oracle.make_cfg(tight=args.tight)
     cnt = oracle.render(sc, camv, cfg)["counters"]
     E = oracle.preprocess(sc, camv, cfg)["E"]
     fcb = F_COMP_BWD_POSE if tracking else F_COMP_BWD_FULL
@@ -575,6 +580,7 @@ def main():
     ap.add_argument("--no-prefetch", action="store_true", help="mapping configs: one context, binning of each view in line")
     ap.add_argument("--graph", action="store_true", help="SGS_FLAG_GRAPH: each step (a tracking frame, or a mapping window on one context) replayed as one CUDA graph")
     ap.add_argument("--normalised-depth", action="store_true", help="SGS_FLAG_NORMALISED_DEPTH: depth image D/O (tracking takes the unfused sequence)")
+    ap.add_argument("--tight", action="store_true", help="SGS_FLAG_TIGHT_BINNING: opacity-aware cutoff + tile-exact culling (shorter tile lists, same images)")
     ap.add_argument("--contrib", action="store_true", help="mapping configs: render with sgs_render_contrib (C_k output on)")
     ap.add_argument("--ingest-ncu", default=None, metavar="RAW_CSV",
                     help="no benchmark: read `ncu -i X.ncu-rep --page raw --csv` of a capture of --config and update profiles/r02_traffic.json")

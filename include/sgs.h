@@ -72,6 +72,14 @@ enum {
                                    workspace to size (a call that had to grow it would allocate: do not capture the first).
                                    Nothing reports a bucket overflow by itself in this mode: sgs_get_stats (which
                                    synchronises the device) does.  sgs_prepare is SGS_INVALID_ARGUMENT. */
+    SGS_FLAG_TIGHT_BINNING = 64, /* SURVEY 8(f) NEXT-3, readings R26 + R27 (Eq. 8 L114-116 with the truncation rules R3/R4):
+                                   the tile lists hold only what can contribute.  (i) Opacity-aware cutoff: a pair contributes only if
+                                   o exp(-rho^2/2) >= alpha_min, so splat k's support is rho^2 <= c_k^2 = min(cutoff^2, 2 ln(o_k /
+                                   alpha_min)); its screen AABB and tile rectangle are those of that ellipse, and o_k < alpha_min is
+                                   culled.  (ii) Tile-exact culling: a tile of the rectangle is listed only if the support ellipse
+                                   reaches the rectangle of the tile's pixel centres.  Images and gradients are those of the default
+                                   binning (same rendered function); sgs_get_binning returns the shorter lists, bit-identical to the
+                                   oracle's tight mode.  Not together with SGS_FLAG_RADIX_BINNING (sgs_create: SGS_INVALID_ARGUMENT). */
     SGS_FLAG_NORMALISED_DEPTH = 16 /* SURVEY 8(f) NEXT-3 (variant of R9; Eq. 8 L116-120 renders D = sum w z and
                                    O = sum w): the depth image is the expected depth D_n = D / O (0 where O = 0), i.e.
                                    the blend weights renormalised to sum to one, so a partly transparent surface keeps

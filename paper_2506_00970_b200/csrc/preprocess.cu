@@ -28,6 +28,52 @@ __device__ __forceinline__ unsigned long long warp_incl_scan(unsigned long long 
     return v;
 }
 
+// R26 (oracle: two_ln_upper): an upper bound of 2 ln r, r >= 1, from +, -, x, / alone in the oracle's operation order
+__device__ __forceinline__ double two_ln_upper(double r) {
+    double m = r, e = 0.0;
+    while (m >= 2.0) { m = m * 0.5; e = e + 1.0; }
+    const double t = (m - 1.0) / (m + 1.0), t2 = t * t;
+    double p = 1.0 / 25.0;
+    p = p * t2 + 1.0 / 23.0; p = p * t2 + 1.0 / 21.0; p = p * t2 + 1.0 / 19.0; p = p * t2 + 1.0 / 17.0;
+    p = p * t2 + 1.0 / 15.0; p = p * t2 + 1.0 / 13.0; p = p * t2 + 1.0 / 11.0; p = p * t2 + 1.0 / 9.0;
+    p = p * t2 + 1.0 / 7.0; p = p * t2 + 1.0 / 5.0; p = p * t2 + 1.0 / 3.0; p = p * t2 + 1.0;
+    const double ln_m = 2.0 * (t * p);
+    const double ln_r = e * 0.69314718055994540 + ln_m;
+    return (2.0 * ln_r) * (1.0 + 1e-9) + 1e-9;
+}
+
+// R27: the support ellipse as a screen conic relative to (cx, cy); ok = well-conditioned ellipse (else: list every tile)
+struct Conic { double cx, cy, A, B, C, D, E, F; int ok; };
+
+__device__ __forceinline__ double conic_q(const Conic& k, double x, double y) {
+    return ((((k.A * x) * x + (2.0 * k.B) * (x * y)) + (k.C * y) * y) + ((2.0 * k.D) * x + (2.0 * k.E) * y)) + k.F;
+}
+__device__ __forceinline__ double clampd(double v, double lo, double hi) { return v < lo ? lo : (v > hi ? hi : v); }
+// the oracle's tile_listed(), same binary64 sequence
+__device__ __forceinline__ bool tile_listed(const Conic& k, int tx, int ty, int W, int H) {
+    if (!k.ok) return true;
+    const double ts = (double)SGS_TILE;
+    double x1 = ts * tx + (ts - 0.5), y1 = ts * ty + (ts - 0.5);
+    if (x1 > W - 0.5) x1 = W - 0.5;
+    if (y1 > H - 0.5) y1 = H - 0.5;
+    const double x0 = (ts * tx + 0.5) - k.cx, y0 = (ts * ty + 0.5) - k.cy;
+    x1 = x1 - k.cx; y1 = y1 - k.cy;
+    const double det = k.A * k.C - k.B * k.B;
+    const double xc = (k.B * k.E - k.C * k.D) / det, yc = (k.B * k.D - k.A * k.E) / det;
+    double qm = conic_q(k, clampd(xc, x0, x1), clampd(yc, y0, y1));
+    double v;
+    v = conic_q(k, x0, clampd(-(k.B * x0 + k.E) / k.C, y0, y1)); if (v < qm) qm = v;
+    v = conic_q(k, x1, clampd(-(k.B * x1 + k.E) / k.C, y0, y1)); if (v < qm) qm = v;
+    v = conic_q(k, clampd(-(k.B * y0 + k.D) / k.A, x0, x1), y0); if (v < qm) qm = v;
+    v = conic_q(k, clampd(-(k.B * y1 + k.D) / k.A, x0, x1), y1); if (v < qm) qm = v;
+    double R = fabs(x0);
+    if (fabs(x1) > R) R = fabs(x1);
+    if (fabs(y0) > R) R = fabs(y0);
+    if (fabs(y1) > R) R = fabs(y1);
+    const double tol = 1e-9 * ((fabs(k.F) + (2.0 * (fabs(k.D) + fabs(k.E))) * R) + ((k.A + k.C) + 2.0 * fabs(k.B)) * (R * R));
+    return qm <= tol;
+}
+
 struct PreOut {
     bool vis;
     uint32_t depth_bits;
@@ -42,7 +88,7 @@ struct PreOut {
 
 __device__ __forceinline__ void preprocess_one(const float* __restrict__ mean, const float* __restrict__ scale,
                                                const float* __restrict__ quat, const SgsCamDev& cam,
-                                               const SgsCfgDev& cfg, PreOut& o) {
+                                               const SgsCfgDev& cfg, PreOut& o, const float opacity = 1.f, Conic* conic = nullptr) {
     o.vis = false;
     const double w = quat[0], x = quat[1], y = quat[2], z = quat[3];
     const double qn = sqrt(((w * w + x * x) + y * y) + z * z);
@@ -75,7 +121,13 @@ __device__ __forceinline__ void preprocess_one(const float* __restrict__ mean, c
     }
     o.depth_bits = __float_as_uint((float)muc[2]);
     if (!(muc[2] > cfg.z_near_d)) return;
-    const double c2 = cfg.cutoff2_d;
+    double c2 = cfg.cutoff2_d;
+    if (conic != nullptr && cfg.alpha_min_d > 0.0) {   // SGS_FLAG_TIGHT_BINNING, R26: the splat's own support
+        const double r = (double)opacity / cfg.alpha_min_d;
+        if (!(r >= 1.0)) return;
+        const double c2o = two_ln_upper(r);
+        if (c2o < c2) c2 = c2o;
+    }
     const double den = c2 * (M[6] * M[6] + M[7] * M[7]) - M[8] * M[8];
     if (!(den < 0.0)) return;
     const double ctrx = (c2 * (M[0] * M[6] + M[1] * M[7]) - M[2] * M[8]) / den;
@@ -93,6 +145,23 @@ __device__ __forceinline__ void preprocess_one(const float* __restrict__ mean, c
     if (fy1 > (double)(cam.tiles_y - 1)) fy1 = (double)(cam.tiles_y - 1);
     o.tx0 = (int)fx0; o.tx1 = (int)fx1; o.ty0 = (int)fy0; o.ty1 = (int)fy1;
     o.vis = true;
+    if (conic != nullptr) {   // R27: the footprint as a conic (the oracle's sequence, prep_surfel)
+        const double C0[3] = {M[1] * M[5] - M[2] * M[4], M[2] * M[3] - M[0] * M[5], M[0] * M[4] - M[1] * M[3]};
+        const double Cx[3] = {M[4] * M[8] - M[5] * M[7], M[5] * M[6] - M[3] * M[8], M[3] * M[7] - M[4] * M[6]};
+        const double Cy[3] = {M[7] * M[2] - M[8] * M[1], M[8] * M[0] - M[6] * M[2], M[6] * M[1] - M[7] * M[0]};
+        const double a1 = Cx[0], a2 = Cy[0], a3 = (Cx[0] * ctrx + Cy[0] * ctry) + C0[0];
+        const double b1 = Cx[1], b2 = Cy[1], b3 = (Cx[1] * ctrx + Cy[1] * ctry) + C0[1];
+        const double c1 = Cx[2], c2_ = Cy[2], c3 = (Cx[2] * ctrx + Cy[2] * ctry) + C0[2];
+        conic->cx = ctrx; conic->cy = ctry;
+        conic->A = (a1 * a1 + b1 * b1) - c2 * (c1 * c1);
+        conic->B = (a1 * a2 + b1 * b2) - c2 * (c1 * c2_);
+        conic->C = (a2 * a2 + b2 * b2) - c2 * (c2_ * c2_);
+        conic->D = (a1 * a3 + b1 * b3) - c2 * (c1 * c3);
+        conic->E = (a2 * a3 + b2 * b3) - c2 * (c2_ * c3);
+        conic->F = (a3 * a3 + b3 * b3) - c2 * (c3 * c3);
+        const double det = conic->A * conic->C - conic->B * conic->B;
+        conic->ok = (conic->A > 0.0 && conic->C > 0.0 && det > 1e-12 * (conic->A * conic->C)) ? 1 : 0;
+    }
     o.bb[0] = __double2float_rd(xmin); o.bb[1] = __double2float_ru(xmax);
     o.bb[2] = __double2float_rd(ymin); o.bb[3] = __double2float_ru(ymax);
     // ---- payload (no decision depends on it; rounded to fp32 at the end) ----
@@ -325,6 +394,7 @@ k_surv_gather(const uint32_t* __restrict__ surv_list, const unsigned int* __rest
 
 constexpr int SGS_PREB_BLOCK = 128, SGS_PREB_LOG2 = 7, PREB_EMIT = 4;  // K-pre-B block: small, so that few survivors still spread over the SMs
 
+template <bool TIGHT>
 __global__ void __launch_bounds__(SGS_PREB_BLOCK)
 k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, const float* __restrict__ quat,
               const float* __restrict__ opacity, const float* __restrict__ rgb, SgsCamDev cam, SgsCfgDev cfg,
@@ -338,6 +408,7 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
     __shared__ unsigned int s_rect[SGS_PREB_BLOCK];   // tile index of the rectangle's first tile
     __shared__ unsigned int s_w[SGS_PREB_BLOCK];      // rectangle width in tiles
     __shared__ unsigned int s_wsum[SGS_PREB_BLOCK / 32];
+    __shared__ Conic s_conic[TIGHT ? SGS_PREB_BLOCK : 1];   // SGS_FLAG_TIGHT_BINNING: each survivor's support conic (R27)
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     // early (list and inputs kept from an earlier iteration, this grid staged programmatically behind K-track): nothing
     // the first round reads is written by the previous kernel, so its loads and the projection run before the wait and
@@ -362,8 +433,12 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
                 in_m[0] = mean[3 * i]; in_m[1] = mean[3 * i + 1]; in_m[2] = mean[3 * i + 2];
                 in_s[0] = scale[2 * i]; in_s[1] = scale[2 * i + 1];
                 in_q[0] = quat[4 * i]; in_q[1] = quat[4 * i + 1]; in_q[2] = quat[4 * i + 2]; in_q[3] = quat[4 * i + 3];
+                if (TIGHT) in_o = opacity[i];
             }
-            preprocess_one(in_m, in_s, in_q, cam, cfg, o);
+            Conic kq;
+            kq.ok = 0;
+            preprocess_one(in_m, in_s, in_q, cam, cfg, o, in_o, TIGHT ? &kq : nullptr);
+            if (TIGHT) s_conic[tid] = kq;
         }
         if (must_wait) { cudaGridDependencySynchronize(); must_wait = false; }
         if (n_surv_in != &counters->n_surv && r0 == 0 && tid == 0) counters->n_surv = n_surv;  // for the host's grid hint
@@ -377,14 +452,14 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
         unsigned int vbase = 0;
         if (lane == 0 && vis_mask) {
             vbase = atomicAdd(&counters->n_visible, (unsigned int)__popc(vis_mask));
-            atomicAdd(&counters->n_entries, (unsigned long long)wcnt);
+            if (!TIGHT) atomicAdd(&counters->n_entries, (unsigned long long)wcnt);   // (TIGHT: counted at emission, below)
         }
         vbase = __shfl_sync(0xffffffffu, vbase, 0);
         if (o.vis) {
             // the visible surfels, compact (arrival order): what the per-surfel backward walks -- K-pre-A's survivor list
             // is several times longer (C4: every splat the frustum test cannot exclude) and costs it a sector per entry
             vis_list[vbase + __popc(vis_mask & ((1u << lane) - 1u))] = (uint32_t)i;
-            if (!cin.p0) { in_o = opacity[i]; in_c[0] = rgb[3 * i]; in_c[1] = rgb[3 * i + 1]; in_c[2] = rgb[3 * i + 2]; }
+            if (!cin.p0) { if (!TIGHT) in_o = opacity[i]; in_c[0] = rgb[3 * i]; in_c[1] = rgb[3 * i + 1]; in_c[2] = rgb[3 * i + 2]; }
             pay.g0[i] = make_float4(o.P, o.Q, o.R, o.S);
             pay.g1[i] = make_float4(o.D, o.E, o.F, in_o);
             pay.g2[i] = make_double2(o.xc, o.yc);
@@ -419,6 +494,7 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
         s_off[tid] = wbase + incl - cnt;  // exclusive
         if (tid == 0) s_off[SGS_PREB_BLOCK] = total;
         __syncthreads();
+        unsigned int n_listed = 0;
         for (unsigned int e0 = tid; e0 < total; e0 += PREB_EMIT * SGS_PREB_BLOCK) {
             // PREB_EMIT entries per trip so that their cursor atomics are all in flight before the first dependent store
             uint32_t t[PREB_EMIT];
@@ -438,6 +514,10 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
                 const unsigned int local = e - s_off[lo], w = s_w[lo];
                 t[k] = s_rect[lo] + (local / w) * (unsigned int)cam.tiles_x + (local % w);
                 key[k] = s_key[lo];
+                if (TIGHT && ok[k]) {   // R27: only tiles the support ellipse reaches are listed
+                    ok[k] = tile_listed(s_conic[lo], (int)(t[k] % (unsigned int)cam.tiles_x), (int)(t[k] / (unsigned int)cam.tiles_x), cam.W, cam.H);
+                    n_listed += ok[k] ? 1u : 0u;
+                }
             }
             uint32_t pos[PREB_EMIT];
 #pragma unroll
@@ -449,6 +529,11 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
                     if (pos[k] < tile_cap) bucket[(size_t)t[k] * tile_cap + pos[k]] = key[k];
                     else atomicMax(&counters->max_tile, pos[k] + 1u);
                 }
+        }
+        if (TIGHT) {
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) n_listed += __shfl_xor_sync(0xffffffffu, n_listed, off);
+            if (lane == 0 && n_listed) atomicAdd(&counters->n_entries, (unsigned long long)n_listed);
         }
         __syncthreads();  // the round's shared arrays are free again
     }
@@ -539,7 +624,7 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     cfg.attrs = attr;
     // programmatic dependent launch behind K-pre-A, or (list reused, previous launch on the stream = K-track) behind K-track
     cfg.numAttrs = ((run_a && !cin.p0) || (cached && prezeroed)) ? 1 : 0;
-    const cudaError_t le = cudaLaunchKernelEx(&cfg, k_pre_project, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd,
+    const cudaError_t le = cudaLaunchKernelEx(&cfg, c->cfgd.tight ? k_pre_project<true> : k_pre_project<false>, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd,
                                               c->cfgd, c->pay, c->culled, c->counters, (const uint32_t*)c->vis_to_surfel,
                                               (const unsigned int*)n_surv, c->cursor, c->bucket, (uint32_t)c->tile_cap, cin,
                                               (cached && prezeroed && cin.p0) ? 1 : 0, c->vis_list);

@@ -63,6 +63,7 @@ struct SgsCfgDev {
     float cutoff2, alpha_min, alpha_max, t_min, z_near;
     float cutoff;   // sqrt(cutoff2)
     double cutoff2_d, z_near_d;
+    double alpha_min_d; int tight;   // SGS_FLAG_TIGHT_BINNING (R26, R27)
 };
 
 // Device-side counters of one render (also copied to pinned host memory).

@@ -51,10 +51,11 @@ def assert_binning(gb, ob):
     assert np.array_equal(gb["ranges"], ob["ranges"])
 
 
-def check_config(name, views, full):
+def check_config(name, views, full, tight=False):
+    """tight: SGS_FLAG_TIGHT_BINNING against the oracle's tight mode (readings R26, R27): the same checks, shorter lists."""
     sc, cams, info = scenegen.make_config(name)
-    cfg = oracle.make_cfg()
-    ren = sgs.Renderer(async_mode=True)
+    cfg = oracle.make_cfg(tight=tight)
+    ren = sgs.Renderer(async_mode=True, tight_binning=tight)
     t, sf = to_device(sc)
     try:
         for v in views:
@@ -66,6 +67,8 @@ def check_config(name, views, full):
             # ---- binning: bit-exact
             ob = oracle.binning(sc, camv, cfg)
             assert_binning(ren.get_binning(sc.n, tiles), ob)
+            if tight:
+                assert ob["E"] < 0.95 * oracle.binning(sc, camv, oracle.make_cfg())["E"]
             # ---- images: every pixel (fragile ones within the oracle-derived allowance)
             o = oracle.render(sc, camv, cfg)
             gimg = planes(im)
@@ -155,3 +158,10 @@ def test_c4_full_size():
 
 def test_c5_full_size():
     check_config("C5", [0], full=False)
+
+
+@pytest.mark.parametrize("name,views,full", [("C2", [0], False), ("C3", [0], True), ("C4", [6], True), ("C5", [0], False)])
+def test_tight_binning_full_size(name, views, full):
+    """SGS_FLAG_TIGHT_BINNING (opacity-aware cutoff + tile-exact culling) on every full-size config: the shorter lists are
+    bit-identical to the oracle's tight mode; images, losses and gradients meet the same bars as with the default binning."""
+    check_config(name, views, full, tight=True)

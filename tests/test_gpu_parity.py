@@ -80,6 +80,36 @@ def test_c1_full(ren, tau):
     assert_pose(out2["pose"], og["pose"], ex["pose"])
 
 
+@pytest.mark.parametrize("tau", POSES)
+def test_c1_tight_binning(tau):
+    """SGS_FLAG_TIGHT_BINNING on C1 (opacities 0.1 .. 0.99, so the opacity-aware cutoff bites): the list is the oracle's tight
+    list bit for bit and a strict subset of the default one; images are BIT-IDENTICAL to the default binning's on the GPU too
+    (the dropped entries composite nothing); gradients and pose against the oracle."""
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    T = None if tau is None else scenegen.perturb_pose(cam.T_cw, tau)
+    camv, cfgt = oracle.make_cam(cam, T), oracle.make_cfg(tight=True)
+    up = scenegen.upstream_normal(1, cam.height, cam.width)
+    rt, rd = sgs.Renderer(tight_binning=True), sgs.Renderer()
+    out, ref = run_gpu(rt, sc, cam, up, T_cw=T), run_gpu(rd, sc, cam, up, T_cw=T)
+    ob = oracle.binning(sc, camv, cfgt)
+    assert_binning(out["bin"], ob)
+    assert out["bin"]["E"] < 0.9 * ref["bin"]["E"]
+    assert np.array_equal(out["img"], ref["img"])
+    o = oracle.render(sc, camv, cfgt)
+    assert_images(out["img"], o, sc, camv, cfgt)
+    og, ex = oracle.backward(sc, camv, cfgt, up), oracle.exposure(sc, camv, cfgt, up)
+    assert_grads(out["grads"], og, ex)
+    assert_pose(out["pose"], og["pose"], ex["pose"])
+    # a splat below alpha_min is culled by the tight binning and composites nothing under the default one
+    faint = Scene(sc.mean[:50], sc.scale[:50], sc.quat[:50], np.full(50, 0.003, np.float32), sc.rgb[:50])
+    a, b = run_gpu(rt, faint, cam), run_gpu(rd, faint, cam)
+    assert a["bin"]["E"] == 0 and a["bin"]["culled"].all() and b["bin"]["E"] > 0 and (a["img"] == 0).all() and (b["img"] == 0).all()
+    with pytest.raises(sgs.SgsError):
+        sgs.Renderer(tight_binning=True, radix_binning=True)
+    rt.close(); rd.close()
+
+
 def test_c2_tracking_shape(ren):
     """Config 2 (200k surfels, 640x480): binning, images, tracking loss (Eq. 15-19), pose-only backward -- each stage on
     the ORACLE's inputs: the loss kernel is run on the oracle's image (rounded to binary32), the backward on the oracle's
