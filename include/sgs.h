@@ -281,6 +281,19 @@ SGS_API int sgs_track_iter(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_c
                            float lambda_d, float normal_sign, const sgs_images* out, float* d_pose6, float* loss,
                            void* cuda_stream);
 
+/* sgs_track_iter with the pose in DEVICE memory (L204: the pose is iterated "until convergence or reaching the maximum number
+ * of iterations"): d_T_cw (DEVICE, 12 floats, row-major 3x4 [R | t]) is read by the preprocess kernels when they run, so the
+ * caller's own pose-update kernel -- d_pose6 in, d_T_cw out -- can sit between the iterations of one stream or of one captured
+ * CUDA graph (SGS_FLAG_GRAPH) with no host round trip.  cam carries the image size and intrinsics; its T_cw is ignored.
+ * With SGS_FLAG_TRACK_REUSE the kept survivor list is built around the device pose of the iteration that builds it (the first
+ * after sgs_track_new_frame); the host cannot see later poses, so the check against the list's margin is made on the device.
+ * INVALID RESULTS ARE NaN: an iteration whose pose has left the margin (call sgs_track_new_frame and repeat), or -- in every
+ * mode of sgs_track_iter -- one whose tile buckets overflowed, writes NaN to *loss and d_pose6 instead of numbers computed
+ * from incomplete lists.  Not with SGS_FLAG_RADIX_BINNING (SGS_INVALID_ARGUMENT).  Otherwise as sgs_track_iter. */
+SGS_API int sgs_track_iter_dev(sgs_ctx* ctx, const sgs_surfels* surfels, const sgs_camera* cam, const float* d_T_cw,
+                               const sgs_images* target, float lambda_d, float normal_sign, const sgs_images* out,
+                               float* d_pose6, float* loss, void* cuda_stream);
+
 /* SGS_FLAG_TRACK_REUSE.  Tracking optimises the pose of ONE frame over many iterations against a frozen map (L204).
  * With the flag set, the caller promises that between two sgs_track_new_frame calls the arrays behind a bytewise-equal
  * sgs_surfels struct (means, scales, active flags) do not change.  sgs_track_iter then keeps the survivor list of its

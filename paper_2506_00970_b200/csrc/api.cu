@@ -230,6 +230,7 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
               cudaHostGetDevicePointer(&c->pinned_small_dev, c->pinned_small, 0) == cudaSuccess &&
               cudaHostGetDevicePointer(&c->host_flag_dev, c->host_flag, 0) == cudaSuccess &&
               cudaMalloc(&c->sort_hist, sizeof(uint32_t) * (8 * 256 + 8)) == cudaSuccess &&
+              cudaMalloc(&c->surv_pose_dev, sizeof(float) * 12) == cudaSuccess &&
               cudaMalloc(&c->loss_dev, sizeof(float) * 8) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->counters_ready, cudaEventDisableTiming) == cudaSuccess &&
               cudaEventCreateWithFlags(&c->prepared_ev, cudaEventDisableTiming) == cudaSuccess &&
@@ -267,6 +268,7 @@ int sgs_destroy(sgs_ctx* c) {
     if (c->split_state) cudaFree(c->split_state);
     if (c->split_flag) cudaFree(c->split_flag);
     if (c->sort_hist) cudaFree(c->sort_hist);
+    if (c->surv_pose_dev) cudaFree(c->surv_pose_dev);
     if (c->loss_dev) cudaFree(c->loss_dev);
     if (c->covis_cnt) cudaFree(c->covis_cnt);
     if (c->counters_ready) cudaEventDestroy(c->counters_ready);

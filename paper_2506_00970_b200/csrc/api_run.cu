@@ -284,7 +284,8 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
             if (!(c->surv_in = sgs_ws_alloc(c, 52 * (size_t)sf->n + 64, s))) return SGS_OUT_OF_MEMORY;
             c->surv_in_cap = sf->n;
         }
-        if (c->surv_valid && !(memcmp(&c->surv_sf, sf, sizeof(*sf)) == 0 && pose_within_margin(&c->surv_cam, cam)))
+        // (device-resident pose: the host cannot check the margin; K-pre-B does and the iteration turns NaN, see sgs_track_iter_dev)
+        if (c->surv_valid && !(memcmp(&c->surv_sf, sf, sizeof(*sf)) == 0 && (c->pose_dev != nullptr || pose_within_margin(&c->surv_cam, cam))))
             c->surv_valid = false;  // another map, or the pose has left the list's margin: build it again, centred here
         c->use_surv_cache = true;
     }
@@ -328,6 +329,15 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
     }
     c->have_binning = true;
     return SGS_OK;
+}
+
+int sgs_track_iter_dev(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const float* d_T_cw, const sgs_images* target,
+                       float lambda_d, float normal_sign, const sgs_images* out, float* d_pose6, float* loss, void* stream) {
+    if (!c || !d_T_cw || radix_mode(c)) return SGS_INVALID_ARGUMENT;
+    c->pose_dev = d_T_cw;
+    const int r = sgs_track_iter(c, sf, cam, target, lambda_d, normal_sign, out, d_pose6, loss, stream);
+    c->pose_dev = nullptr;
+    return r;
 }
 
 int sgs_track_new_frame(sgs_ctx* c) {

@@ -323,13 +323,56 @@ k_preprocess(int64_t n, const float* __restrict__ mean, const float* __restrict_
 //            the block in shared memory and appends them to a global list with ONE atomic per block.
 //   K-pre-B  dense: one thread per survivor runs the binary64 sequence, writes the payload, and the
 //            block's tile entries are spread over its threads (one (surfel, tile) pair each).
-template <int SGS_PREA_ITEMS>
+// sgs_track_iter_dev: the pose T_cw (row-major 3x4) lives in DEVICE memory -- a tracker's own update kernel writes it between
+// the iterations of one stream or CUDA graph -- and replaces the pose fields of the camera struct the host filled.
+__device__ __forceinline__ void load_pose(SgsCamDev& cam, const float* __restrict__ T) {
+    float ta = 1.f;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) { const float v = __ldg(T + 4 * i + j); cam.R[3 * i + j] = (double)v; cam.Rf[3 * i + j] = v; }
+        const float t = __ldg(T + 4 * i + 3);
+        cam.t[i] = (double)t; cam.tf[i] = t; ta += fabsf(t);
+    }
+    cam.pc_tabs = ta;
+}
+
+// is `cur` = Exp(tau) o `ref` with |rho|, |theta| inside 80 % of the survivor list's margins?  (api_run.cu: pose_within_margin)
+__device__ __forceinline__ bool pose_inside_margin(const float* __restrict__ ref, const float* __restrict__ cur) {
+    double Rd[9];
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {
+            double v = 0.0;
+            for (int k = 0; k < 3; ++k) v += (double)cur[4 * i + k] * (double)ref[4 * j + k];
+            Rd[3 * i + j] = v;
+        }
+    double cosang = 0.5 * (Rd[0] + Rd[4] + Rd[8] - 1.0);
+    if (!(cosang <= 1.0)) cosang = 1.0;
+    if (!(cosang >= -1.0)) return false;
+    double d2 = 0.0;
+    for (int i = 0; i < 3; ++i) {
+        const double v = (double)cur[4 * i + 3] - (Rd[3 * i] * ref[3] + Rd[3 * i + 1] * ref[7] + Rd[3 * i + 2] * ref[11]);
+        d2 += v * v;
+    }
+    const double mt = 0.8 * SGS_REUSE_MARGIN_T, mr = 0.8 * SGS_REUSE_MARGIN_R;
+    return d2 <= mt * mt && cosang >= 1.0 - 0.5 * mr * mr;   // (cos mr >= 1 - mr^2 / 2: slightly stricter, no transcendental)
+}
+
+template <int SGS_PREA_ITEMS, bool DEVPOSE>
 __global__ void __launch_bounds__(SGS_PRE_BLOCK)
 k_pre_select(int64_t n, const float* __restrict__ mean, const float* __restrict__ scale,
-             const uint8_t* __restrict__ active, SgsCamDev cam, SgsCfgDev cfg, uint8_t* __restrict__ culled,
-             unsigned int* __restrict__ n_surv, uint32_t* __restrict__ surv_list) {
+             const uint8_t* __restrict__ active, SgsCamDev cam_in, SgsCfgDev cfg, uint8_t* __restrict__ culled,
+             unsigned int* __restrict__ n_surv, uint32_t* __restrict__ surv_list, const float* __restrict__ pose_dev,
+             float* __restrict__ surv_pose) {
     constexpr int SGS_PREA_SPAN = SGS_PREA_ITEMS * SGS_PRE_BLOCK;
     cudaTriggerProgrammaticLaunchCompletion();  // K-pre-B may be staged now; it waits for this grid before reading
+    SgsCamDev camL;
+    if (DEVPOSE) {
+        camL = cam_in;
+        load_pose(camL, pose_dev);
+        if (surv_pose != nullptr && blockIdx.x == 0 && threadIdx.x < 12) surv_pose[threadIdx.x] = __ldg(pose_dev + threadIdx.x);
+    }
+    const SgsCamDev& cam = DEVPOSE ? camL : cam_in;
     __shared__ unsigned short s_list[SGS_PREA_SPAN];
     __shared__ unsigned int s_n, s_base;
     const int tid = threadIdx.x, lane = tid & 31;
@@ -394,15 +437,18 @@ k_surv_gather(const uint32_t* __restrict__ surv_list, const unsigned int* __rest
 
 constexpr int SGS_PREB_BLOCK = 128, SGS_PREB_LOG2 = 7, PREB_EMIT = 4;  // K-pre-B block: small, so that few survivors still spread over the SMs
 
-template <bool TIGHT>
+template <bool TIGHT, bool DEVPOSE>
 __global__ void __launch_bounds__(SGS_PREB_BLOCK)
 k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, const float* __restrict__ quat,
-              const float* __restrict__ opacity, const float* __restrict__ rgb, SgsCamDev cam, SgsCfgDev cfg,
+              const float* __restrict__ opacity, const float* __restrict__ rgb, SgsCamDev cam_in, SgsCfgDev cfg,
               SgsPayload pay, uint8_t* __restrict__ culled, SgsCounters* __restrict__ counters,
               const uint32_t* surv_list, const unsigned int* n_surv_in,  // written by the PREVIOUS grid: no __restrict__,
               // or the compiler may hoist their loads above the conditional grid-dependency wait (it did: stale counts)
               uint32_t* __restrict__ cursor, uint64_t* __restrict__ bucket, uint32_t tile_cap, SurvInputs cin, int early,
-              uint32_t* __restrict__ vis_list) {
+              uint32_t* __restrict__ vis_list, const float* __restrict__ pose_dev, const float* surv_pose) {
+    SgsCamDev camL;
+    if (DEVPOSE) { camL = cam_in; load_pose(camL, pose_dev); }
+    const SgsCamDev& cam = DEVPOSE ? camL : cam_in;
     __shared__ unsigned int s_off[SGS_PREB_BLOCK + 1];
     __shared__ unsigned long long s_key[SGS_PREB_BLOCK];
     __shared__ unsigned int s_rect[SGS_PREB_BLOCK];   // tile index of the rectangle's first tile
@@ -442,6 +488,9 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
         }
         if (must_wait) { cudaGridDependencySynchronize(); must_wait = false; }
         if (n_surv_in != &counters->n_surv && r0 == 0 && tid == 0) counters->n_surv = n_surv;  // for the host's grid hint
+        // a kept survivor list covers poses near the one it was built around; the host cannot see a device-resident pose,
+        // so the check is made here and K-track turns the iteration's results into NaN when it fails
+        if (DEVPOSE && surv_pose != nullptr && r0 == 0 && tid == 0 && !pose_inside_margin(surv_pose, pose_dev)) counters->stale = 1u;
         if (have) culled[i] = o.vis ? 0 : 1;
         const unsigned int cnt = o.vis ? (unsigned int)((o.tx1 - o.tx0 + 1) * (o.ty1 - o.ty0 + 1)) : 0u;
         // totals: one atomic per warp
@@ -585,13 +634,14 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
         cam_a.pm_t = SGS_REUSE_MARGIN_T; cam_a.pm_r = SGS_REUSE_MARGIN_R;
         c->surv_valid = true; c->surv_sf = *sf; c->surv_cam = c->last_cam;
     }
+    const float* pd = c->pose_dev;
+    float* sp_w = (pd && c->use_surv_cache) ? c->surv_pose_dev : nullptr;          // K-pre-A records the pose the list is built around
+    const float* sp_r = (pd && cached) ? c->surv_pose_dev : nullptr;                // K-pre-B checks a kept list against it
     if (run_a) {
-        if (wide)
-            k_pre_select<4><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, cam_a, c->cfgd, c->culled,
-                                                               n_surv, c->vis_to_surfel);
-        else
-            k_pre_select<1><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(n, sf->mean, sf->scale, sf->active, cam_a, c->cfgd, c->culled,
-                                                               n_surv, c->vis_to_surfel);
+#define SGS_PREA_ARGS n, sf->mean, sf->scale, sf->active, cam_a, c->cfgd, c->culled, n_surv, c->vis_to_surfel, pd, sp_w
+        if (wide) { if (pd) k_pre_select<4, true><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(SGS_PREA_ARGS); else k_pre_select<4, false><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(SGS_PREA_ARGS); }
+        else { if (pd) k_pre_select<1, true><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(SGS_PREA_ARGS); else k_pre_select<1, false><<<blocks_a, SGS_PRE_BLOCK, 0, s>>>(SGS_PREA_ARGS); }
+#undef SGS_PREA_ARGS
     }
     SurvInputs cin = {nullptr, nullptr, nullptr, nullptr};
     if (c->use_surv_cache && c->surv_in) {
@@ -624,10 +674,12 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     cfg.attrs = attr;
     // programmatic dependent launch behind K-pre-A, or (list reused, previous launch on the stream = K-track) behind K-track
     cfg.numAttrs = ((run_a && !cin.p0) || (cached && prezeroed)) ? 1 : 0;
-    const cudaError_t le = cudaLaunchKernelEx(&cfg, c->cfgd.tight ? k_pre_project<true> : k_pre_project<false>, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd,
+    auto kern = c->cfgd.tight ? (pd ? k_pre_project<true, true> : k_pre_project<true, false>)
+                              : (pd ? k_pre_project<false, true> : k_pre_project<false, false>);
+    const cudaError_t le = cudaLaunchKernelEx(&cfg, kern, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd,
                                               c->cfgd, c->pay, c->culled, c->counters, (const uint32_t*)c->vis_to_surfel,
                                               (const unsigned int*)n_surv, c->cursor, c->bucket, (uint32_t)c->tile_cap, cin,
-                                              (cached && prezeroed && cin.p0) ? 1 : 0, c->vis_list);
+                                              (cached && prezeroed && cin.p0) ? 1 : 0, c->vis_list, pd, sp_r);
     if (le != cudaSuccess) return le;
     return cudaGetLastError();
 }

@@ -15,7 +15,7 @@ __device__ __forceinline__ float warp_sum(float v) {
 // Returns (to every thread of the block) whether this block was the last one.
 __device__ __forceinline__ bool finish_pose(const float* __restrict__ partial, unsigned int n_blocks,
                                             SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
-                                            float* __restrict__ loss_out = nullptr) {
+                                            float* __restrict__ loss_out = nullptr, bool invalid = false) {
     __shared__ bool s_is_last;
     __shared__ double s_sum[8][7];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -45,6 +45,7 @@ __device__ __forceinline__ bool finish_pose(const float* __restrict__ partial, u
     if (tid < 7) {
         double v = 0;
         for (int w2 = 0; w2 < (int)(blockDim.x >> 5); ++w2) v += s_sum[w2][tid];
+        if (invalid) v = (double)__int_as_float(0x7fc00000);  // the caller's lists were incomplete: NaN, not a plausible number
         if (tid < 6) d_pose6[tid] = (float)v;
         else if (loss_out) *loss_out = (float)v;
     }

@@ -75,6 +75,8 @@ struct SgsCounters {
     unsigned int ticket_bwd;        // last-block-done ticket for the pose reduction
     unsigned int max_tile;          // bucket mode: largest per-tile entry count seen (> tile_cap => overflow)
     unsigned int n_surv;            // bucket mode: surfels that passed the cheap tests of K-pre-A (the list K-pre-B walks)
+    unsigned int stale;             // sgs_track_iter_dev + SGS_FLAG_TRACK_REUSE: the device pose has left the kept survivor list's margin
+    unsigned int pad_;
 };
 
 struct sgs_ctx {
@@ -141,6 +143,8 @@ struct sgs_ctx {
     bool surv_valid, use_surv_cache;   // list valid for (surv_sf, poses near surv_cam) / this preprocess launch uses it
     sgs_surfels surv_sf;
     sgs_camera surv_cam;
+    float* surv_pose_dev;              // 12 floats: the DEVICE pose the kept list was built around (sgs_track_iter_dev)
+    const float* pose_dev;             // non-NULL inside sgs_track_iter_dev: the preprocess kernels read T_cw from here
     int narrow_prepare;                // > 0 inside sgs_prepare: K-pre-B blocks per SM
     bool grads_on_aux;                 // SGS_FLAG_LAZY_GRADS: the last sgs_backward left its final kernel on aux_stream
     bool copy_in_flight;               // counters_ready was recorded on aux_stream and nothing on the caller's stream waited for it yet

@@ -441,7 +441,12 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         pose_partial[(size_t)blockIdx.x * 8 + tid] = s;
     }
     if (tid == 0 && crank == 0) tile_cost[tile] = (uint32_t)((clock64() - t_start) >> 8);  // feedback for the next iteration's order
-    if (!finish_pose(pose_partial, gridDim.x, counters, d_pose6, loss_out)) return;
+    // A tile bucket that overflowed (entries dropped) or a kept survivor list the device-resident pose has left (splats
+    // possibly missing) must not pass for a result: the iteration's loss and pose gradient are NaN.  Under SGS_FLAG_GRAPH and
+    // with SGS_FLAG_ASYNC nothing else tells the caller in time (the host sees the counters one call later, or never).
+    const bool invalid = *reinterpret_cast<volatile unsigned int*>(&counters->max_tile) > tile_cap ||
+                         *reinterpret_cast<volatile unsigned int*>(&counters->stale) != 0u;
+    if (!finish_pose(pose_partial, gridDim.x, counters, d_pose6, loss_out, invalid)) return;
     if (host_flag) {  // sgs_track_iter_host: d_pose6 / loss_out are pinned HOST memory; publish them before the housekeeping below
         if (tid < 7) __threadfence_system();
         __syncthreads();
@@ -455,7 +460,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     if (tid == 0) {
         if (counters_snap) *counters_snap = *counters;  // what the host reads for overflow detection and hints
         counters->n_entries = 0ull; counters->n_visible = 0u; counters->overflow = 0u; counters->ticket_pre = 0u;
-        counters->max_tile = 0u; counters->n_surv = 0u;
+        counters->max_tile = 0u; counters->n_surv = 0u; counters->stale = 0u;
         if (n_help > 0) split_flag[SGS_TRACK_HELPERS] += 1u;  // next launch's epoch: every block of this one is past its hand-over
     }
 }

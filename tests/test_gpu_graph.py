@@ -153,3 +153,100 @@ def test_track_iter_graph_replays_back_to_back_with_split_tiles():
         np.testing.assert_allclose(p6.cpu().numpy(), pe.cpu().numpy(), rtol=1e-4, atol=1e-6 * float(pe.abs().max()))
     assert r.stats()["overflow"] == 0
     r.close(); eager.close()
+
+
+def test_track_iter_dev_pose_changes_inside_one_graph():
+    """sgs_track_iter_dev reads T_cw from device memory when the kernels run: a frame of 10 iterations at 10 DIFFERENT poses
+    (a device-to-device copy stands for the tracker's pose update between iterations), captured as ONE graph with a kept
+    survivor list, equals 10 eager host-pose calls -- and follows new poses written into the same device tensor before a
+    replay.  A pose that leaves the kept list's margin turns that iteration's loss and gradient into NaN (the host cannot
+    see it; the device check does), and so does a tile-bucket overflow."""
+    from scenegen import Camera, Scene
+    sc, cams, _ = scenegen.make_config("C2", n_override=60000)
+    cam = cams[0]
+    t, sf = to_device(sc)
+    c = camera(cam)
+    g = scenegen.SplitMix(123)
+
+    def pose_set(scale):
+        Ts = []
+        for k in range(10):
+            tau = np.concatenate([scale * 0.012 * g.normal(3) / 3, scale * 0.007 * g.normal(3) / 3])
+            Ts.append(scenegen.perturb_pose(cam.T_cw, tau).astype(np.float32))
+        return Ts
+
+    ref = sgs.Renderer()
+    im = alloc_images(cam)
+    ref.render(sf, c, **im)
+    tgt_rgb, tgt_dep = (im["rgb"] * 0.9 + 0.01).contiguous(), (im["depth"] * 1.02).contiguous()
+
+    def eager(Ts):
+        out = []
+        pe, le = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+        for T in Ts:
+            ref.track_iter(sf, camera(cam, T), tgt_rgb, tgt_dep, 0.5, -1.0, pe, le)
+            out.append((pe.cpu().numpy().copy(), float(le.item())))
+        return out
+
+    r = sgs.Renderer(graph=True, track_reuse=True)
+    T_all = torch.zeros(10, 12, device="cuda")
+    T_cur = torch.zeros(12, device="cuda")
+    p6_all, loss_all = torch.zeros(10, 6, device="cuda"), torch.zeros(10, device="cuda")
+
+    def frame():
+        r.track_new_frame()
+        for k in range(10):
+            T_cur.copy_(T_all[k])                 # "the tracker's update kernel"
+            r.track_iter_dev(sf, c, T_cur, tgt_rgb, tgt_dep, 0.5, -1.0, p6_all[k], loss_all[k:k + 1])
+
+    Ts = pose_set(1.0)
+    T_all.copy_(torch.from_numpy(np.stack([T.reshape(12) for T in Ts])))
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        for _ in range(2):
+            frame()
+    torch.cuda.current_stream().wait_stream(s)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=s):
+        frame()
+    for round_ in range(2):
+        want = eager(Ts)
+        p6_all.fill_(-3.0); loss_all.fill_(-3.0)
+        graph.replay()
+        torch.cuda.synchronize()
+        for k in range(10):
+            assert abs(float(loss_all[k]) - want[k][1]) <= 1e-5 * abs(want[k][1])
+            np.testing.assert_allclose(p6_all[k].cpu().numpy(), want[k][0], rtol=1e-4, atol=1e-6 * np.abs(want[k][0]).max())
+        assert len({round(w[1], 9) for w in want}) == 10          # the ten iterations really differ
+        Ts = pose_set(0.7)                                        # new poses, same device tensor
+        T_all.copy_(torch.from_numpy(np.stack([T.reshape(12) for T in Ts])))
+    # iterations 6.. leave the margin of the list built at iteration 0: NaN, not numbers from an incomplete list
+    far = scenegen.perturb_pose(cam.T_cw, [0.2, 0.0, 0.1, 0.0, 0.05, 0.0]).astype(np.float32).reshape(12)
+    T_all[6:] = torch.from_numpy(far).cuda()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.isfinite(loss_all[:6]).all() and torch.isfinite(p6_all[:6]).all()
+    assert torch.isnan(loss_all[6:]).all() and torch.isnan(p6_all[6:]).all()
+    r.close(); ref.close()
+    # a tile-bucket overflow in async mode: that iteration's results are NaN at once; the NEXT call reports it
+    n = 6000
+    mean = np.stack([g.uniform(n, -0.02, 0.02), g.uniform(n, -0.02, 0.02), g.uniform(n, 1.0, 3.0)], 1).astype(np.float32)
+    dense = Scene(mean, np.full((n, 2), 0.01, np.float32), np.tile(np.float32([1, 0, 0, 0]), (n, 1)),
+                  np.full(n, 0.05, np.float32), np.full((n, 3), 0.5, np.float32))
+    small = Camera(64, 48, 60.0, 60.0, 32.0, 24.0)
+    td, sfd = to_device(dense)
+    a = sgs.Renderer(async_mode=True)
+    pa, la = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+    trgb, tdep = torch.full((3, 48, 64), 0.3, device="cuda"), torch.full((1, 48, 64), 1.5, device="cuda")
+    a.track_iter(sfd, camera(small), trgb, tdep, 0.5, 1.0, pa, la)
+    torch.cuda.synchronize()
+    assert torch.isnan(la).all() and torch.isnan(pa).all()
+    with pytest.raises(sgs.SgsError) as e:
+        a.stats(); a.track_iter(sfd, camera(small), trgb, tdep, 0.5, 1.0, pa, la)
+    assert e.value.status == sgs.SGS_WORKSPACE_OVERFLOW
+    a.track_iter(sfd, camera(small), trgb, tdep, 0.5, 1.0, pa, la)
+    torch.cuda.synchronize()
+    assert torch.isfinite(la).all() and torch.isfinite(pa).all()
+    a.close()
