@@ -157,7 +157,7 @@ class Workload:
     """Device-resident inputs + the step function for one config."""
 
     def __init__(self, name, iters_override=None, contrib=False, prefetch=True, reuse=True, normalised_depth=False, graph=False,
-                 tight=False):
+                 tight=False, radix=False):
         self.contrib = contrib
         self.graph, self.cg, self.eager_steps = graph, None, 0
         nd = self.normalised_depth = normalised_depth
@@ -173,11 +173,11 @@ class Workload:
         self.t = dict(mean=d(sc.mean), scale=d(sc.scale), quat=d(sc.quat), opacity=d(sc.opacity), rgb=d(sc.rgb),
                       active=d(sc.active, torch.uint8))
         self.sf = sgs.Renderer.surfels(*(self.t[k] for k in ("mean", "scale", "quat", "opacity", "rgb", "active")))
-        self.ren = sgs.Renderer(async_mode=not graph, graph=graph, track_reuse=self.tracking and reuse, normalised_depth=nd,
-                                tight_binning=tight)
+        self.ren = sgs.Renderer(async_mode=not graph, graph=graph, track_reuse=self.tracking and reuse and not radix,
+                                normalised_depth=nd, tight_binning=tight, radix_binning=radix)
         # mapping window: a second context + a side stream, so that sgs_prepare (binning) of view v+1 runs under the
         # compositing kernels of view v (include/sgs.h); tracking iterations depend on one another and use one context
-        two = prefetch and not self.tracking and len(self.cams) > 1 and not graph   # (capture mode: one context, one stream)
+        two = prefetch and not self.tracking and len(self.cams) > 1 and not graph and not radix   # (capture mode: one context, one stream)
         if two:  # + SGS_FLAG_LAZY_GRADS: a view's per-surfel kernel runs under the next view's forward; joined at the step's end
             self.ren.close()
             self.ren = sgs.Renderer(async_mode=True, lazy_grads=True, normalised_depth=nd, tight_binning=tight)
@@ -428,7 +428,7 @@ def run_config(name, args, torch, dist, world, rank, local, peaks):
         torch.cuda.synchronize()
 
     wl = Workload(name, args.iters, args.contrib, not args.no_prefetch, not args.no_reuse, args.normalised_depth, args.graph,
-                  args.tight)
+                  args.tight, args.radix)
     K, W = args.steps, max(args.warmup, 3)
     per_step = []
     for _ in range(W):
@@ -514,6 +514,8 @@ def run_config(name, args, torch, dist, world, rank, local, peaks):
         out["config"]["gradients"] = f"summed over windows of {WINDOW} views (sgs_backward_accumulate), zeroed per window"
     if args.graph:
         out["config"]["launch"] = "one CUDA graph per step (SGS_FLAG_GRAPH); not the default workload"
+    if args.radix:
+        out["config"]["binning"] = "SGS_FLAG_RADIX_BINNING: global onesweep radix sort of (tile << 32 | depth) keys, in line; not the default workload"
     if args.tight:
         out["config"]["binning_variant"] = "SGS_FLAG_TIGHT_BINNING (readings R26, R27); not the default workload"
     if args.normalised_depth:
@@ -581,6 +583,7 @@ def main():
     ap.add_argument("--graph", action="store_true", help="SGS_FLAG_GRAPH: each step (a tracking frame, or a mapping window on one context) replayed as one CUDA graph")
     ap.add_argument("--normalised-depth", action="store_true", help="SGS_FLAG_NORMALISED_DEPTH: depth image D/O (tracking takes the unfused sequence)")
     ap.add_argument("--tight", action="store_true", help="SGS_FLAG_TIGHT_BINNING: opacity-aware cutoff + tile-exact culling (shorter tile lists, same images)")
+    ap.add_argument("--radix", action="store_true", help="SGS_FLAG_RADIX_BINNING: the global LSD radix sort of the 64-bit keys instead of the per-tile buckets (A/B; one context, in line)")
     ap.add_argument("--contrib", action="store_true", help="mapping configs: render with sgs_render_contrib (C_k output on)")
     ap.add_argument("--ingest-ncu", default=None, metavar="RAW_CSV",
                     help="no benchmark: read `ncu -i X.ncu-rep --page raw --csv` of a capture of --config and update profiles/r02_traffic.json")

@@ -360,6 +360,11 @@ SGS_API int sgs_ssim_loss(sgs_ctx* ctx, int width, int height, const float* rend
 
 /* Map correction after pose-graph optimisation (Eq. 31-32), in place: Delta T_f = T_f^o T_f^{-1} and
  * mu_k <- Delta T_f mu_k, R_k <- Delta R_f R_k with f = frame_id[k], the splat's closest observed keyframe.
+ * CONVENTION (reading R29): Eq. 31-32 as printed keep a splat fixed in its keyframe's camera frame -- the purpose of the
+ * correction, L302-306 -- exactly when the poses are CAMERA-TO-WORLD (as a pose graph stores them): then
+ * (T_f^o)^{-1} mu' = T_f^{-1} mu.  T_orig / T_opt are therefore camera-to-world [R | t]; a caller holding the world-to-camera
+ * poses of sgs_camera.T_cw passes their inverses ([R^T | -R^T t]).  tests/test_gpu_map_correction.py renders a map from
+ * the optimised keyframe after the correction and finds the image of the original map from the original keyframe.
  *   mean (n x 3), quat (n x 4, (w,x,y,z), 16-byte aligned), frame_id (n x int32; ids outside [0, n_frames) leave the
  *   splat untouched), T_orig / T_opt (n_frames x 12, row-major 3x4 [R|t] of T_f and T_f^o): all DEVICE. */
 SGS_API int sgs_map_correction(sgs_ctx* ctx, int64_t n, float* mean, float* quat, const int32_t* frame_id, int n_frames,

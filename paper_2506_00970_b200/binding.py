@@ -308,6 +308,8 @@ class Renderer:
                                       C.c_float(weight), _ptr(upstream_rgb), _ptr(loss), _stream_ptr(stream)), "sgs_ssim_loss")
 
     def map_correction(self, mean, quat, frame_id, T_orig, T_opt, stream=None):
+        """sgs_map_correction (Eq. 31-32), in place.  T_orig / T_opt: (n_frames, 12) CAMERA-TO-WORLD keyframe poses [R | t]
+        (reading R29; pass the inverses of world-to-camera poses)."""
         """sgs_map_correction (Eq. 31-32), in place on mean / quat."""
         _check(self.lib.sgs_map_correction(self._ctx, C.c_int64(mean.shape[0]), _ptr(mean), _ptr(quat),
                                            _ptr(frame_id, torch.int32), C.c_int(T_orig.shape[0]), _ptr(T_orig), _ptr(T_opt),

@@ -9,8 +9,9 @@
 //     f = [ r x (a_v g_u - a_u g_v) + (a_u x a_v) g_z ] / (r . (a_u x a_v))
 //     dL/dmu_c = sum f,  dL/d(s_u t_uc) = sum u f,  dL/d(s_v t_vc) = sum v f
 // which IS the matrix dL/dH_c of Eq. 9 (= W^T dL/dT) accumulated directly.
-//   full mode     : 16 values per (warp, surfel) are reduced with a transposed butterfly (16 shuffles
-//                   instead of 80) and land as ONE 64-byte red.global.add per warp.
+//   full mode     : 16 values per (warp, surfel) are summed over the warp through a shared-memory scratch (16 transposed
+//                   STS per lane, 4 LDS.128 + packed adds over half a row, one shuffle joins the halves) and land as ONE
+//                   64-byte red.global.add per warp into acc[surfel][16]; k_surfel_backward finishes per surfel.
 //   pose-only mode: Eq. 11-13 applied per pixel: dL/drho = sum f, dL/dtheta = r x sum z f + N x g_N;
 //                   no per-surfel traffic at all -- registers -> block -> grid reduction to 6 values.
 #include "pair.cuh"

@@ -67,3 +67,45 @@ def test_map_correction_bandwidth():
     print(f"map_correction: {us:.1f} us for {n} splats = {gbs:.0f} GB/s algorithmic")
     assert torch.isfinite(m_d).all() and gbs > 500.0
     ren.close()
+
+
+def test_correction_keeps_splats_fixed_in_their_keyframe_camera():
+    """Reading R29 (convention of T_orig / T_opt): with CAMERA-TO-WORLD poses, Eq. 31-32 keep every splat where it was in its
+    keyframe's camera frame, so the map rendered from the OPTIMISED keyframe after the correction is the image of the
+    original map from the original keyframe (what the correction is for, L302-306).  Passing the world-to-camera poses of
+    sgs_camera instead deforms the map: the image changes -- the test tells the two conventions apart."""
+    import sys, os
+    sys.path.insert(0, os.path.dirname(__file__))
+    from gpu_common import to_device, camera, alloc_images, planes
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    T_cw = scenegen.perturb_pose(cam.T_cw, [0.05, -0.02, 0.03, 0.02, 0.04, -0.03]).astype(np.float64)
+    T_cw_o = scenegen.perturb_pose(T_cw, [0.12, 0.05, -0.08, 0.15, -0.1, 0.2]).astype(np.float64)
+
+    def inv(T):
+        R, t = T[:, :3], T[:, 3]
+        return np.concatenate([R.T, (-R.T @ t)[:, None]], 1)
+
+    ren = sgs.Renderer()
+    t, sf = to_device(sc)
+    im0 = alloc_images(cam)
+    ren.render(sf, camera(cam, T_cw), **im0)
+    ref = planes(im0)
+    assert oracle is not None and np.abs(ref[7]).max() > 0.5
+    fid = torch.zeros(sc.n, dtype=torch.int32, device="cuda")
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    for conv, same in ((inv, True), (lambda T: T, False)):
+        t2, sf2 = to_device(sc)
+        ren.map_correction(t2["mean"], t2["quat"], fid, d(conv(T_cw).reshape(1, 12)), d(conv(T_cw_o).reshape(1, 12)))
+        im1 = alloc_images(cam)
+        ren.render(sf2, camera(cam, T_cw_o), **im1)
+        err = np.abs(planes(im1) - ref).max()
+        assert (err < 2e-3) == same, (same, err)
+    # ... and the oracle agrees on what the corrected map looks like from the optimised keyframe
+    mu2, R2 = oracle.map_correction(sc.mean, sc.quat, np.zeros(sc.n, np.int64), inv(T_cw)[None], inv(T_cw_o)[None])
+    q2 = Rotation.from_matrix(R2).as_quat()[:, [3, 0, 1, 2]]
+    sc2 = scenegen.Scene(mu2.astype(np.float32), sc.scale, q2.astype(np.float32), sc.opacity, sc.rgb)
+    o = oracle.render(sc2, oracle.make_cam(cam, T_cw_o), oracle.make_cfg(), counters=False)["img"]
+    good = np.abs(o - ref) < 2e-3
+    assert good.mean() > 0.995          # (positions and quaternions went through binary32: a few threshold pixels may flip)
+    ren.close()
