@@ -49,18 +49,20 @@ def _p(a, t):
     return None if a is None else a.ctypes.data_as(t)
 
 
-def make_cfg(tile=16, cutoff=3.0, alpha_min=1.0 / 255.0, alpha_max=0.99, t_min=1e-4, z_near=0.2, tight=False):
+def make_cfg(tile=16, cutoff=3.0, alpha_min=1.0 / 255.0, alpha_max=0.99, t_min=1e-4, z_near=0.2, tight=False, lowpass=False):
     """Truncation constants (readings R3-R7).  Values pass through float32 first because the C-ABI
     config struct holds floats: both sides then use the identical real numbers.  tight: the binning variant of
     readings R26 + R27 (opacity-aware cutoff, tile-exact culling) -- the rendered function is the
-    same, the tile lists are shorter."""
+    same, the tile lists are shorter.  lowpass: the compositing variant of reading R28 (screen-space low-pass filter:
+    rho^2 = min(u^2 + v^2, 2 |x - x_c|^2), centre depth where the screen term wins)."""
     f = lambda v: float(np.float32(v))
-    return np.array([tile, f(cutoff), f(alpha_min), f(alpha_max), f(t_min), f(z_near), 1.0 if tight else 0.0, 0.0], dtype=np.float64)
+    return np.array([tile, f(cutoff), f(alpha_min), f(alpha_max), f(t_min), f(z_near), 1.0 if tight else 0.0,
+                     1.0 if lowpass else 0.0], dtype=np.float64)
 
 
-def smooth_cfg(tile=16):
+def smooth_cfg(tile=16, lowpass=False):
     """Plain Eq. 8: no cutoff, no alpha bounds, no stop, no near plane (used for finite differences)."""
-    return np.array([tile, np.inf, 0.0, 1.0, 0.0, 0.0, 0.0, 0.0], dtype=np.float64)
+    return np.array([tile, np.inf, 0.0, 1.0, 0.0, 0.0, 0.0, 1.0 if lowpass else 0.0], dtype=np.float64)
 
 
 def make_cam(cam, T_cw=None, widen_from_f32=True):

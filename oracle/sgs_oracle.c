@@ -39,6 +39,7 @@ typedef struct {
     int tile;
     double cutoff, alpha_min, alpha_max, t_min, z_near;
     int tight; /* binning variant of readings R26 + R27: opacity-aware cutoff and tile-exact culling */
+    int lowpass; /* compositing variant of reading R28: screen-space low-pass filter */
 } Cfg;
 
 /* Per-surfel derived quantities (all fp64). */
@@ -70,6 +71,7 @@ static void load_cfg(const double* c, Cfg* cfg) {
     cfg->tile = (int)c[0]; cfg->cutoff = c[1]; cfg->alpha_min = c[2];
     cfg->alpha_max = c[3]; cfg->t_min = c[4]; cfg->z_near = c[5];
     cfg->tight = c[6] != 0.0;
+    cfg->lowpass = c[7] != 0.0;
 }
 
 /* R26: an UPPER bound of 2 ln r (r >= 1) from +, -, x, / alone, so that the CUDA preprocess can evaluate the identical
@@ -167,7 +169,19 @@ static void prep_surfel(const float* mean, const float* scale, const float* quat
     const double ctry = (c2 * (M[3] * M[6] + M[4] * M[7]) - M[5] * M[8]) / den;
     const double hx = sqrt(ctrx * ctrx - (c2 * (M[0] * M[0] + M[1] * M[1]) - M[2] * M[2]) / den);
     const double hy = sqrt(ctry * ctry - (c2 * (M[3] * M[3] + M[4] * M[4]) - M[5] * M[5]) / den);
-    const double xmin = ctrx - hx, xmax = ctrx + hx, ymin = ctry - hy, ymax = ctry + hy;
+    double xmin = ctrx - hx, xmax = ctrx + hx, ymin = ctry - hy, ymax = ctry + hy;
+    if (cfg->lowpass) {
+        /* R28: the screen-space Gaussian of the filter reaches rho_2d^2 = 2 |x - x_c|^2 <= c^2, a disc of radius c / sqrt 2
+         * around the projected centre; the footprint is the union.  A splat so close to edge-on that its own ellipse is not
+         * representable (non-finite half axes) is kept through the disc. */
+        const double xc = M[2] / M[8], yc = M[5] / M[8], rf = cfg->cutoff * 0.70710678118654757;
+        if (!(isfinite(xmin) && isfinite(xmax))) { xmin = xc; xmax = xc; }
+        if (!(isfinite(ymin) && isfinite(ymax))) { ymin = yc; ymax = yc; }
+        if (xc - rf < xmin) xmin = xc - rf;
+        if (xc + rf > xmax) xmax = xc + rf;
+        if (yc - rf < ymin) ymin = yc - rf;
+        if (yc + rf > ymax) ymax = yc + rf;
+    }
     p->aabb[0] = xmin; p->aabb[1] = xmax; p->aabb[2] = ymin; p->aabb[3] = ymax;
     if (!(isfinite(xmin) && isfinite(xmax) && isfinite(ymin) && isfinite(ymax))) return;
     if (!(xmax > 0.0 && xmin < (double)cam->W && ymax > 0.0 && ymin < (double)cam->H)) return;
@@ -390,6 +404,8 @@ static void free_buckets(Buckets* bk) { free(bk->start); free(bk->list); }
 typedef struct {
     double hu[3], hv[3], k[3], u, v, z, G, a;
     int clamped;
+    int use2d;      /* R28: the screen-space term of the low-pass filter gave rho^2 (and the depth is the centre's) */
+    double dx, dy;  /* R28: pixel minus projected centre */
 } Pair;
 
 #define FRAG_EPS 1e-4
@@ -402,15 +418,34 @@ static inline int eval_pair(const Prep* p, double opac, double x, double y, doub
     r->k[1] = r->hu[2] * r->hv[0] - r->hu[0] * r->hv[2];
     r->k[2] = r->hu[0] * r->hv[1] - r->hu[1] * r->hv[0];
     *covers = 0;
-    if (r->k[2] == 0.0) return 0;
-    r->u = r->k[0] / r->k[2];
-    r->v = r->k[1] / r->k[2];
-    const double rho2 = r->u * r->u + r->v * r->v;
-    if (!isfinite(rho2)) return 0;
+    r->use2d = 0;
+    double rho2;
+    if (cfg->lowpass) {
+        /* R28: rho^2 = min(u^2 + v^2, 2 |x - x_c|^2), x_c = (M02, M12) / M22 the projected centre; the screen term also
+         * stands in where the intersection is undefined.  Where it wins the pair's depth is the centre depth M22. */
+        r->dx = x - M[2] / M[8]; r->dy = y - M[5] / M[8];
+        const double rho2_2d = 2.0 * (r->dx * r->dx + r->dy * r->dy);
+        double rho2_3d = INFINITY;
+        r->u = 0.0; r->v = 0.0;
+        if (r->k[2] != 0.0) {
+            r->u = r->k[0] / r->k[2]; r->v = r->k[1] / r->k[2];
+            rho2_3d = r->u * r->u + r->v * r->v;
+            if (!isfinite(rho2_3d)) rho2_3d = INFINITY;
+        }
+        if (isfinite(rho2_3d) && fabs(rho2_3d - rho2_2d) < FRAG_EPS * rho2_2d) *frag |= 1;   /* which term wins decides depth and gradient */
+        r->use2d = !(rho2_3d <= rho2_2d);
+        rho2 = r->use2d ? rho2_2d : rho2_3d;
+    } else {
+        if (r->k[2] == 0.0) return 0;
+        r->u = r->k[0] / r->k[2];
+        r->v = r->k[1] / r->k[2];
+        rho2 = r->u * r->u + r->v * r->v;
+        if (!isfinite(rho2)) return 0;
+    }
     const double c2 = cfg->cutoff * cfg->cutoff;
     if (isfinite(c2) && fabs(rho2 - c2) < FRAG_EPS * c2) *frag |= 1;
     if (rho2 > c2) return 0;
-    r->z = M[6] * r->u + M[7] * r->v + M[8];
+    r->z = r->use2d ? M[8] : M[6] * r->u + M[7] * r->v + M[8];
     if (cfg->z_near > 0.0 && fabs(r->z - cfg->z_near) < FRAG_EPS * cfg->z_near) *frag |= 1;
     if (!(r->z > cfg->z_near)) return 0;
     *covers = 1;
@@ -428,7 +463,7 @@ static inline int eval_pair(const Prep* p, double opac, double x, double y, doub
      * splat against the ray.  Beyond KAPPA_MAX the fp32 rounding of the INPUTS already moves (u,v)
      * by more than the image tolerance allows (delta G / G ~ rho^2 kappa 2e-7), so no binary32
      * renderer can be held to 1e-4 there: flag bit 2 (value 4) of the fragile mask. */
-    {
+    if (!r->use2d) {
         const double nu = r->hu[0] * r->hu[0] + r->hu[1] * r->hu[1], nv = r->hv[0] * r->hv[0] + r->hv[1] * r->hv[1];
         if (sqrt(nu * nv) > KAPPA_MAX * fabs(r->k[2])) *frag |= 4;
     }
@@ -656,6 +691,15 @@ void orc_backward(int64_t n, const float* mean, const float* scale, const float*
                     suffix += w * gv;
                     double dG = 0.0;
                     if (!r->clamped) { atomic_add(d_opacity + k, da * r->G); dG = da * opacity[k]; }
+                    if (r->use2d) {
+                        /* R28, screen term: G = exp(-|x - x_c|^2), z = M22;  x_c = M02 / M22, y_c = M12 / M22:
+                         * dG/dx_c = 2 dx G, dG/dy_c = 2 dy G;  dx_c/dM02 = 1 / M22, dx_c/dM22 = -x_c / M22 (same for y) */
+                        const double gxc = 2.0 * r->dx * r->G * dG, gyc = 2.0 * r->dy * r->G * dG, m22 = p->M[8];
+                        atomic_add(dM + 9 * k + 2, gxc / m22);
+                        atomic_add(dM + 9 * k + 5, gyc / m22);
+                        atomic_add(dM + 9 * k + 8, dz - (gxc * (p->M[2] / m22) + gyc * (p->M[5] / m22)) / m22);
+                        continue;
+                    }
                     const double du = -r->u * r->G * dG + dz * p->M[6];
                     const double dv = -r->v * r->G * dG + dz * p->M[7];
                     const double dk[3] = {du / r->k[2], dv / r->k[2], -(r->u * du + r->v * dv) / r->k[2]};
@@ -751,9 +795,18 @@ static inline double pair_kappa(const Pair* r) {
     return sqrt(nu * nv) / fabs(r->k[2]);
 }
 /* fields eval_pair() leaves unset when it rejects a pair early (u, v are set whenever k_z != 0) */
+/* the pair's rho^2 (R28: of the term r->use2d names) */
+static inline double pair_rho2(const Cfg* cfg, const Pair* r) {
+    return (cfg->lowpass && r->use2d) ? 2.0 * (r->dx * r->dx + r->dy * r->dy) : r->u * r->u + r->v * r->v;
+}
+/* does eval_pair() define the pair's geometry at all? (default: the intersection must exist; R28: the screen term always does) */
+static inline int pair_defined(const Cfg* cfg, const Pair* r) {
+    if (cfg->lowpass) return 1;
+    return r->k[2] != 0.0 && isfinite(r->u * r->u + r->v * r->v);
+}
 static inline void pair_complete(const Prep* p, double opac, const Cfg* cfg, Pair* r) {
-    const double rho2 = r->u * r->u + r->v * r->v;
-    r->z = p->M[6] * r->u + p->M[7] * r->v + p->M[8];
+    const double rho2 = pair_rho2(cfg, r);
+    r->z = (cfg->lowpass && r->use2d) ? p->M[8] : p->M[6] * r->u + p->M[7] * r->v + p->M[8];
     r->G = exp(-0.5 * rho2);
     const double og = opac * r->G;
     r->clamped = og > cfg->alpha_max;
@@ -777,14 +830,14 @@ void orc_pixel_bounds(int64_t n, const float* mean, const float* scale, const fl
                 if (x < p->aabb[0] - 1.0 || x > p->aabb[1] + 1.0 || y < p->aabb[2] - 1.0 || y > p->aabb[3] + 1.0) continue;
                 Pair r; int covers, f = 0;
                 const int st = eval_pair(p, opacity[k], x, y, T, &c.cfg, &r, &f, &covers);
-                if ((f & 1) && r.k[2] != 0.0 && isfinite(r.u * r.u + r.v * r.v)) {
+                if ((f & 1) && pair_defined(&c.cfg, &r)) {
                     if (st != 1) pair_complete(p, opacity[k], &c.cfg, &r);
                     fw += r.a * T + (st == 2 ? T * (1.0 - r.a) : 0.0);
                     if (fabs(r.z) > zm) zm = fabs(r.z);
                 }
                 if (st == 2) break;
                 if (st == 0) continue;
-                const double w = r.a * T, kap = pair_kappa(&r);
+                const double w = r.a * T, kap = r.use2d ? 0.0 : pair_kappa(&r);   /* (R28 screen term: no intersection, no kappa) */
                 ke += w * (r.u * r.u + r.v * r.v) * kap;
                 kz += w * kap * (fabs(p->M[6] * r.u) + fabs(p->M[7] * r.v));
                 if (fabs(r.z) > zm) zm = fabs(r.z);
@@ -856,6 +909,12 @@ static void exposure_sweep(const Ctx* c, const float* scale, const float* opacit
         out[9] = 0.0;
         if (!h->clamped) { out[9] = da * r->G; dG = da * opacity[k]; }
         for (int ch = 0; ch < 3; ++ch) { out[10 + ch] = g[ch] * w; lnc[ch] = g[4 + ch] * w; }
+        if (r->use2d) {   /* R28, screen term (as in orc_backward) */
+            const double gxc = 2.0 * r->dx * r->G * dG, gyc = 2.0 * r->dy * r->G * dG, m22 = p->M[8];
+            for (int t = 0; t < 9; ++t) lm[t] = 0.0;
+            lm[2] = gxc / m22; lm[5] = gyc / m22;
+            lm[8] = dz - (gxc * (p->M[2] / m22) + gyc * (p->M[5] / m22)) / m22;
+        } else {
         const double du = -r->u * r->G * dG + dz * p->M[6];
         const double dv = -r->v * r->G * dG + dz * p->M[7];
         const double dk[3] = {du / r->k[2], dv / r->k[2], -(r->u * du + r->v * dv) / r->k[2]};
@@ -864,6 +923,7 @@ static void exposure_sweep(const Ctx* c, const float* scale, const float* opacit
         cross3(dk, r->hu, dhv);
         const double uv1[3] = {r->u, r->v, 1.0};
         for (int t = 0; t < 3; ++t) { lm[t] = dhu[t]; lm[3 + t] = dhv[t]; lm[6 + t] = dz * uv1[t] - x * dhu[t] - y * dhv[t]; }
+        }
         surfel_chain(c, k, scale, lm, lnc, out, out + 13);
         for (int t = 0; t < 19; ++t) {
             loc[19 * h->e + t] += sign * out[t];
@@ -947,9 +1007,12 @@ void orc_exposure(int64_t n, const float* mean, const float* scale, const float*
                     if (x < p->aabb[0] - 1.0 || x > p->aabb[1] + 1.0 || y < p->aabb[2] - 1.0 || y > p->aabb[3] + 1.0) continue;
                     Pair r; int covers, f = 0;
                     (void)eval_pair(p, opacity[k], x, y, T, cfg, &r, &f, &covers);   /* fills h_u, h_v, k, u, v */
-                    if (r.k[2] == 0.0) continue;
-                    const double rho2 = r.u * r.u + r.v * r.v;
-                    if (!isfinite(rho2)) continue;
+                    if (!pair_defined(cfg, &r)) continue;
+                    if (cfg->lowpass && r.k[2] != 0.0) {   /* R28: which term wins is a decision too */
+                        const double r3 = r.u * r.u + r.v * r.v, r2 = 2.0 * (r.dx * r.dx + r.dy * r.dy);
+                        if (isfinite(r3) && fabs(r3 - r2) < FRAG_EPS * r2) r.use2d = !r.use2d;
+                    }
+                    const double rho2 = pair_rho2(cfg, &r);
                     pair_complete(p, opacity[k], cfg, &r);
                     const double c2 = cfg->cutoff * cfg->cutoff, og = opacity[k] * r.G;
                     int in = (rho2 <= c2) ^ (isfinite(c2) && fabs(rho2 - c2) < FRAG_EPS * c2);

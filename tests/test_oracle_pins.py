@@ -1007,3 +1007,93 @@ def test_p18_lone_splat_lists_exactly_the_tiles_its_support_reaches():
     faint = one_surfel((0.05, -0.02, 1.6), (0.22, 0.12), (qw, qx, qy, qz), 0.003)
     assert oracle.binning(faint, camv, cfgt)["culled"][0] == 1 and oracle.binning(faint, camv, cfg0)["culled"][0] == 0
     assert oracle.render(faint, camv, cfg0)["img"].max() == 0.0
+
+
+# ---------------------------------------------------------------- P19: screen-space low-pass filter (reading R28)
+def test_p19_lowpass_closed_forms():
+    """R28: rho^2 = min(u^2 + v^2, 2 |x - x_c|^2).  (i) A splat far smaller than a pixel, centred between pixel centres,
+    renders nothing without the filter and the closed form o exp(-|x - x_c|^2) (depth plane: that times the centre depth)
+    with it.  (ii) A splat several pixels wide is untouched: its own Gaussian is the larger one everywhere (sigma_px^2 > 1/2),
+    images bit-identical.  (iii) An edge-on splat (its plane contains the viewing ray) is invisible without the filter and
+    a blob at its centre depth with it."""
+    cfg0, cfgf = oracle.make_cfg(), oracle.make_cfg(lowpass=True)
+    camv = oracle.make_cam(CAM)
+    X, Y = pix_grid(CAM)
+    z0 = 2.0
+    xc, yc = 30.3, 20.8                                  # projected centre, between pixel centres
+    mu = ((xc - CAM.cx) / CAM.fx * z0, (yc - CAM.cy) / CAM.fy * z0, z0)
+    tiny = one_surfel(mu, (1e-4, 1e-4), (1, 0, 0, 0), 0.9)
+    assert oracle.render(tiny, camv, cfg0)["img"].max() == 0.0
+    r = oracle.render(tiny, camv, cfgf)
+    mu32 = np.float32(mu).astype(np.float64)
+    xc32, yc32 = CAM.fx * mu32[0] / mu32[2] + CAM.cx, CAM.fy * mu32[1] / mu32[2] + CAM.cy
+    d2 = (X - xc32) ** 2 + (Y - yc32) ** 2
+    a = float(np.float32(0.9)) * np.exp(-d2)
+    a[(2 * d2 > 9.0) | (a < float(np.float32(1 / 255)))] = 0.0
+    assert (a > 0).sum() >= 9
+    np.testing.assert_allclose(r["img"][7], a, atol=1e-12)
+    np.testing.assert_allclose(r["img"][3], a * mu32[2], atol=1e-12)
+    b = oracle.binning(tiny, camv, cfgf)
+    np.testing.assert_allclose(b["aabb"][0], [xc32 - 3 / np.sqrt(2), xc32 + 3 / np.sqrt(2), yc32 - 3 / np.sqrt(2), yc32 + 3 / np.sqrt(2)], atol=1e-9)
+    big = one_surfel((0.31, -0.17, 1.5), (0.11, 0.07), (1, 0, 0, 0), 0.8)       # sigma_px = 60 * 0.07 / 1.5 = 2.8 px
+    assert np.array_equal(oracle.render(big, camv, cfg0)["img"], oracle.render(big, camv, cfgf)["img"])
+    # edge-on: the splat's plane contains the ray through its centre (normal t_n = x axis, centre on the optical axis)
+    rot = Rotation.from_euler("y", 90, degrees=True)
+    qx, qy, qz, qw = rot.as_quat()
+    edge = one_surfel((0.0, 0.0, 1.5), (0.1, 0.1), (qw, qx, qy, qz), 0.9)
+    r0, rf = oracle.render(edge, camv, cfg0), oracle.render(edge, camv, cfgf)
+    col = int(CAM.cx)                                                              # the pixel columns next to the axis
+    assert r0["img"][7][:, col - 3:col + 3].max() < 0.9 * rf["img"][7][:, col - 3:col + 3].max()
+    m = rf["img"][7] > 0.2
+    assert m.sum() >= 4
+    np.testing.assert_allclose(rf["img"][3][m] / rf["img"][7][m], 1.5, rtol=0.05)   # depth ~ the centre's (exactly where the screen term wins)
+
+
+def _filter_scene():
+    """_tiny's six splats plus a sub-pixel one, a one-pixel one and a nearly edge-on one: pairs of both kinds exist."""
+    sc, cam = _tiny()
+    extra_mu = np.float32([[0.05, 0.03, 1.0], [-0.1, -0.05, 1.2], [0.12, -0.08, 0.9]])
+    extra_s = np.float32([[2e-3, 2e-3], [0.03, 0.04], [0.15, 0.12]])
+    rot = Rotation.from_euler("xyz", [5, 86, 10], degrees=True).as_quat()
+    extra_q = np.float32([[1, 0.1, 0.05, 0.02], [0.9, -0.2, 0.1, 0.3], [rot[3], rot[0], rot[1], rot[2]]])
+    cat2 = lambda a, b: np.concatenate([a, b])
+    sc2 = Scene(cat2(sc.mean, extra_mu), cat2(sc.scale, extra_s), cat2(sc.quat, extra_q), cat2(sc.opacity, np.float32([0.8, 0.7, 0.9])),
+                cat2(sc.rgb, np.float32([[0.9, 0.1, 0.2], [0.2, 0.8, 0.3], [0.3, 0.3, 0.9]])))
+    return sc2, cam
+
+
+def test_p19_lowpass_gradients_are_finite_differences():
+    """Every surfel gradient and the SE(3) pose gradient with the filter on: plain Eq. 8 + filter, and the default
+    truncation rules + filter.  The min() of R28 is a kink like the other decisions: no pixel may sit on it (fragile
+    mask empty) and the guard of _fd_check watches the composited counts."""
+    sc, cam = _filter_scene()
+    camv = oracle.make_cam(cam, widen_from_f32=False)
+    for cfg, guard in ((oracle.smooth_cfg(lowpass=True), False), (oracle.make_cfg(lowpass=True), True)):
+        r = oracle.render(sc, camv, cfg)
+        plain = oracle.render(sc, camv, oracle.smooth_cfg() if not guard else oracle.make_cfg())
+        assert (r["fragile"] & 1).sum() == 0, "a pixel sits on a decision: move a splat"
+        assert np.abs(r["img"] - plain["img"]).max() > 1e-3          # the screen term does win somewhere
+        _fd_check(cfg, 1e-5, scene=(sc, cam), guard=guard, hexp=-19)
+
+
+def test_p19_lowpass_lists_are_conservative(c1):
+    """Every pair with min(rho_3d^2, rho_2d^2) <= c^2 (library inverse; 2 |x - x_c|^2 from M) is in its pixel's tile list."""
+    sc, cam, camv, cfg, r = c1
+    small = Scene(sc.mean, (sc.scale * np.float32(0.05)), sc.quat, sc.opacity, sc.rgb)    # 0.5 - 2.5 mm: mostly sub-pixel
+    cfgf = oracle.make_cfg(lowpass=True)
+    b = oracle.binning(small, camv, cfgf)
+    X, Y = pix_grid(cam)
+    tid = (np.arange(cam.height)[:, None] // 16) * b["tiles_x"] + (np.arange(cam.width)[None, :] // 16)
+    members = [set(b["idx"][s:e].tolist()) for s, e in b["ranges"]]
+    n2d = 0
+    for k in np.nonzero(b["culled"] == 0)[0]:
+        M = b["M"][k].reshape(3, 3)
+        u, v = _numpy_uv(M, X, Y)
+        r2 = 2 * ((X - M[0, 2] / M[2, 2]) ** 2 + (Y - M[1, 2] / M[2, 2]) ** 2)
+        cover = np.minimum(u * u + v * v, r2) <= 9.0
+        n2d += int((cover & (r2 < u * u + v * v)).sum())
+        for t in np.unique(tid[cover]):
+            assert k in members[t]
+    assert n2d > 1000
+    rf, r0 = oracle.render(small, camv, cfgf), oracle.render(small, camv, oracle.make_cfg())
+    assert rf["img"][7].sum() > 3 * r0["img"][7].sum()                # the filter is what makes these splats visible
