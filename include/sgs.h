@@ -80,6 +80,15 @@ enum {
                                    reaches the rectangle of the tile's pixel centres.  Images and gradients are those of the default
                                    binning (same rendered function); sgs_get_binning returns the shorter lists, bit-identical to the
                                    oracle's tight mode.  Not together with SGS_FLAG_RADIX_BINNING (sgs_create: SGS_INVALID_ARGUMENT). */
+    SGS_FLAG_LOWPASS = 128,     /* SURVEY 8(f) NEXT-3, reading R28 (the paper states no filter, R8; this is the published 2DGS remedy for
+                                   sub-pixel and edge-on splats, restated): the Gaussian weight of a pair is the larger of the splat's
+                                   own and a screen-space Gaussian of sigma = sqrt(2)/2 px around the projected centre x_c,
+                                   rho^2 = min(u^2 + v^2, 2 |x - x_c|^2); where the screen term wins the pair's depth is the centre
+                                   depth, and its gradient reaches the splat through x_c.  The footprint is the cutoff ellipse united
+                                   with the disc of radius cutoff / sqrt 2 around x_c.  Supported by sgs_render, sgs_prepare,
+                                   sgs_backward(_accumulate), sgs_backward_tracking and the loss calls; sgs_track_iter takes the
+                                   unfused sequence; sgs_render_contrib / sgs_render_median return SGS_INVALID_ARGUMENT; not together
+                                   with SGS_FLAG_TIGHT_BINNING or SGS_FLAG_NORMALISED_DEPTH (sgs_create: SGS_INVALID_ARGUMENT). */
     SGS_FLAG_NORMALISED_DEPTH = 16 /* SURVEY 8(f) NEXT-3 (variant of R9; Eq. 8 L116-120 renders D = sum w z and
                                    O = sum w): the depth image is the expected depth D_n = D / O (0 where O = 0), i.e.
                                    the blend weights renormalised to sum to one, so a partly transparent surface keeps

@@ -20,6 +20,7 @@ SGS_FLAG_LAZY_GRADS = 8
 SGS_FLAG_NORMALISED_DEPTH = 16
 SGS_FLAG_GRAPH = 32
 SGS_FLAG_TIGHT_BINNING = 64
+SGS_FLAG_LOWPASS = 128
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
 FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p, C.c_void_p)
@@ -139,7 +140,7 @@ class Renderer:
     """One sgs_ctx.  Method names follow the C calls (sgs_render -> render, ...)."""
 
     def __init__(self, tile=16, cutoff=3.0, alpha_min=1.0 / 255.0, alpha_max=0.99, t_min=1e-4, z_near=0.2,
-                 async_mode=False, radix_binning=False, track_reuse=False, lazy_grads=False, normalised_depth=False, graph=False, tight_binning=False, device="cuda:0", torch_allocator=True):
+                 async_mode=False, radix_binning=False, track_reuse=False, lazy_grads=False, normalised_depth=False, graph=False, tight_binning=False, lowpass=False, device="cuda:0", torch_allocator=True):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2506_00970_b200 needs a CUDA device; there is no CPU fallback")
         self.lib = load_library()
@@ -153,7 +154,7 @@ class Renderer:
         cfg.flags = ((SGS_FLAG_ASYNC if async_mode else 0) | (SGS_FLAG_RADIX_BINNING if radix_binning else 0) |
                      (SGS_FLAG_TRACK_REUSE if track_reuse else 0) | (SGS_FLAG_LAZY_GRADS if lazy_grads else 0) |
                      (SGS_FLAG_NORMALISED_DEPTH if normalised_depth else 0) | (SGS_FLAG_GRAPH if graph else 0) |
-                     (SGS_FLAG_TIGHT_BINNING if tight_binning else 0))
+                     (SGS_FLAG_TIGHT_BINNING if tight_binning else 0) | (SGS_FLAG_LOWPASS if lowpass else 0))
         if torch_allocator:
             dev_index = self.device.index or 0
 

@@ -201,7 +201,8 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
     if (cfg->tile != SGS_TILE || !(cfg->cutoff > 0.f) || !isfinite(cfg->cutoff) || !(cfg->alpha_min >= 0.f) ||
         !(cfg->alpha_max > 0.f) || !(cfg->alpha_max < 1.f) || !(cfg->t_min >= 0.f) || !(cfg->z_near > 0.f) ||
         ((cfg->alloc == nullptr) != (cfg->free == nullptr)) ||
-        ((cfg->flags & SGS_FLAG_TIGHT_BINNING) && (cfg->flags & SGS_FLAG_RADIX_BINNING)))
+        ((cfg->flags & SGS_FLAG_TIGHT_BINNING) && (cfg->flags & SGS_FLAG_RADIX_BINNING)) ||
+        ((cfg->flags & SGS_FLAG_LOWPASS) && (cfg->flags & (SGS_FLAG_TIGHT_BINNING | SGS_FLAG_NORMALISED_DEPTH))))
         return SGS_INVALID_ARGUMENT;
     sgs_ctx* c = new (std::nothrow) sgs_ctx;
     if (!c) return SGS_OUT_OF_MEMORY;
@@ -215,6 +216,7 @@ int sgs_create(sgs_ctx** out, const sgs_config* cfg) {
     c->cfgd.z_near_d = (double)cfg->z_near;
     c->cfgd.alpha_min_d = (double)cfg->alpha_min;
     c->cfgd.tight = (cfg->flags & SGS_FLAG_TIGHT_BINNING) ? 1 : 0;
+    c->cfgd.lowpass = (cfg->flags & SGS_FLAG_LOWPASS) ? 1 : 0;
     int prio_lo = 0, prio_hi = 0;  // the ctx's own stream carries short latency-bound work: let it in first
     cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
     bool ok = cudaMalloc(&c->counters, sizeof(SgsCounters)) == cudaSuccess &&

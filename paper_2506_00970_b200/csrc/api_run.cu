@@ -240,7 +240,7 @@ int sgs_render(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const s
 
 int sgs_render_median(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* out, float* median,
                       void* stream) {
-    if (!c || !sf || !median) return SGS_INVALID_ARGUMENT;
+    if (!c || !sf || !median || c->cfgd.lowpass) return SGS_INVALID_ARGUMENT;
     c->median_out = median;
     const int r = sgs_render(c, sf, cam, out, stream);
     c->median_out = nullptr;
@@ -249,7 +249,7 @@ int sgs_render_median(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, 
 
 int sgs_render_contrib(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const sgs_images* out, float* contrib,
                        void* stream) {
-    if (!c || !sf || !contrib) return SGS_INVALID_ARGUMENT;
+    if (!c || !sf || !contrib || c->cfgd.lowpass) return SGS_INVALID_ARGUMENT;
     if (sf->n > 0 && cudaMemsetAsync(contrib, 0, sizeof(float) * (size_t)sf->n, (cudaStream_t)stream) != cudaSuccess)
         return SGS_CUDA_ERROR;
     c->contrib_out = contrib;
@@ -269,7 +269,7 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
                    float normal_sign, const sgs_images* out, float* d_pose6, float* loss, void* stream) {
     if (!c || !target || !target->rgb || !target->depth || !d_pose6) return SGS_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
-    if (radix_mode(c)) {  // A/B binning path: the unfused sequence
+    if (radix_mode(c) || c->cfgd.lowpass) {  // A/B binning path, SGS_FLAG_LOWPASS: the unfused sequence
         int r = sgs_render(c, sf, cam, out, stream);
         if (r != SGS_OK) return r;
         r = sgs_backward_tracking(c, target, lambda_d, normal_sign, d_pose6, loss, stream);
@@ -333,7 +333,7 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
 
 int sgs_track_iter_dev(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, const float* d_T_cw, const sgs_images* target,
                        float lambda_d, float normal_sign, const sgs_images* out, float* d_pose6, float* loss, void* stream) {
-    if (!c || !d_T_cw || radix_mode(c)) return SGS_INVALID_ARGUMENT;
+    if (!c || !d_T_cw || radix_mode(c) || c->cfgd.lowpass) return SGS_INVALID_ARGUMENT;
     c->pose_dev = d_T_cw;
     const int r = sgs_track_iter(c, sf, cam, target, lambda_d, normal_sign, out, d_pose6, loss, stream);
     c->pose_dev = nullptr;

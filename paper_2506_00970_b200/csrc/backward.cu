@@ -38,7 +38,7 @@ struct StagedBwd {
 // upstream images through HBM; the loss itself rides in slot 6 of the pose partials.
 struct FusedLoss { const float* trgb; const float* tdepth; float lambda_d, nsign; float* loss; };
 
-template <bool POSE_ONLY, bool FUSED, bool NDEPTH>
+template <bool POSE_ONLY, bool FUSED, bool NDEPTH, bool LOWPASS = false>
 __global__ void __launch_bounds__(SGS_BLOCK, SGS_BWD_MIN_BLOCKS)
 k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
            int tiles_x, float fx, float fy, float cx, float cy, SgsCfgDev cfg, CPlanes up,
@@ -107,6 +107,7 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
     }
     float suffix = 0.f;
     float F0 = 0.f, F1 = 0.f, F2 = 0.f, Z0 = 0.f, Z1 = 0.f, Z2 = 0.f, Nn0 = 0.f, Nn1 = 0.f, Nn2 = 0.f;
+    float E0 = 0.f, E1 = 0.f, E2 = 0.f;  // R28, pose-only: sum of Z_c (d x f) over screen-term pairs, d = (ddx / fx, ddy / fy, 0)
 
     // block-wide maximum of `last` decides how many batches exist
     uint32_t wmax = last;
@@ -131,16 +132,21 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
             pmask = warp_patch_mask(pay.g7[v], (float)(tx * SGS_TILE), (float)(ty * SGS_TILE));
             const double2 g2 = pay.g2[v];
             StagedBwd st;
-            stage_entry(g0, g1, g2, g3, px0, py0, st.s0, st.s1, st.s2);
+            float xy0[2];
+            stage_entry(g0, g1, g2, g3, px0, py0, st.s0, st.s1, st.s2, xy0);
+
             st.s3 = make_float4(g1.w, g3.w, g4.x, g4.y);
             st.s4 = make_float4(g4.z, g4.w, g5.x, 0.f);  // .w <- m.z below
             const float aux = g5.y, auy = g5.z, auz = g5.w, avx = g6.x, avy = g6.y, avz = g6.z;
             st.s5 = make_float4(aux, auy, auz, avx);
             st.s6 = make_float4(avy, avz, auy * avz - auz * avy, auz * avx - aux * avz);
             st.s4.w = aux * avy - auy * avx;
+            // R28: the record has no spare slot and the kernel's static shared memory is at its 48 KB limit, so under the flag
+            // the pixel-minus-centre offsets of the tile's first pixel take m.x, m.y's place and m = a_u x a_v is rebuilt per pair
+            if (LOWPASS) { st.s6.z = xy0[0]; st.s6.w = xy0[1]; }
             sh_v[tid] = v;
             sh[tid] = st;
-            pmask = refine_patch_mask(pmask, st.s0, st.s1, st.s2, g1.w, cfg.cutoff2, cfg.alpha_min);
+            if (!LOWPASS) pmask = refine_patch_mask(pmask, st.s0, st.s1, st.s2, g1.w, cfg.cutoff2, cfg.alpha_min);
         }
         sh_mask[tid] = (unsigned char)pmask;
         __syncthreads();
@@ -156,7 +162,8 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
             int jj[BWD_K];
             PairResult r[BWD_K];
             float inv1ma[BWD_K], gv[BWD_K], opac[BWD_K], da[BWD_K], w[BWD_K];
-            bool hit[BWD_K];
+            float ddx[BWD_K], ddy[BWD_K], zc[BWD_K];   // R28 only
+            bool hit[BWD_K], use2d[BWD_K];
 #pragma unroll
             for (int k = 0; k < BWD_K; ++k) {
                 const bool has = m != 0u;
@@ -170,8 +177,17 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
                 const float dn = __fmaf_rn(ly, s1.w, __fmaf_rn(lx, s0.w, s2.x));
                 const float inv = fast_rcp(dn);
                 r[k].u = __fmul_rn(un, inv); r[k].v = __fmul_rn(vn, inv);
-                const float rho2 = __fmaf_rn(r[k].v, r[k].v, __fmul_rn(r[k].u, r[k].u));
+                float rho2 = __fmaf_rn(r[k].v, r[k].v, __fmul_rn(r[k].u, r[k].u));
                 r[k].z = __fmaf_rn(s2.z, r[k].v, __fmaf_rn(s2.y, r[k].u, s2.w));
+                use2d[k] = false;
+                if (LOWPASS) {   // R28, the forward's sequence: rho^2 = min(u^2 + v^2, 2 |x - x_c|^2), centre depth where the screen term wins
+                    const float4 xy = sh[j].s6;
+                    ddx[k] = __fadd_rn(lx, xy.z); ddy[k] = __fadd_rn(ly, xy.w); zc[k] = s2.w;
+                    const float r2 = __fmul_rn(2.f, __fmaf_rn(ddy[k], ddy[k], __fmul_rn(ddx[k], ddx[k])));
+                    use2d[k] = !(rho2 <= r2);
+                    rho2 = use2d[k] ? r2 : rho2;
+                    r[k].z = use2d[k] ? s2.w : r[k].z;
+                }
                 r[k].G = fast_ex2(__fmul_rn(rho2, -0.72134752044448170368f));
                 r[k].a = fminf(cfg.alpha_max, __fmul_rn(s3.x, r[k].G));
                 hit[k] = has && (boff + (uint32_t)j) < last && (rho2 <= cfg.cutoff2) && (r[k].z > cfg.z_near) &&
@@ -200,13 +216,29 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
                 const float gu = -r[k].u * r[k].G * dG, gvv = -r[k].v * r[k].G * dG, gz = g[3] * w[k];
                 // f = [ r x (a_v gu - a_u gv) + m gz ] / (r . m)
                 const float q0 = s5.w * gu - s5.x * gvv, q1 = s6.x * gu - s5.y * gvv, q2 = s6.y * gu - s5.z * gvv;
-                const float m0 = s6.z, m1 = s6.w, m2 = s4.w;
+                const float m0 = LOWPASS ? s5.y * s6.y - s5.z * s6.x : s6.z, m1 = LOWPASS ? s5.z * s5.w - s5.x * s6.y : s6.w, m2 = s4.w;
                 const float inv_rm = fast_rcp(rx * m0 + ry * m1 + m2);
                 // a rejected pair may carry inf / NaN: its lanes contribute exact zeros
-                const float f0 = hit[k] ? (ry * q2 - q1 + m0 * gz) * inv_rm : 0.f;
-                const float f1 = hit[k] ? (q0 - rx * q2 + m1 * gz) * inv_rm : 0.f;
-                const float f2 = hit[k] ? (rx * q1 - ry * q0 + m2 * gz) * inv_rm : 0.f;
-                const float uk = hit[k] ? r[k].u : 0.f, vk = hit[k] ? r[k].v : 0.f, zk = hit[k] ? r[k].z : 0.f;
+                float f0 = hit[k] ? (ry * q2 - q1 + m0 * gz) * inv_rm : 0.f;
+                float f1 = hit[k] ? (q0 - rx * q2 + m1 * gz) * inv_rm : 0.f;
+                float f2 = hit[k] ? (rx * q1 - ry * q0 + m2 * gz) * inv_rm : 0.f;
+                float uk = hit[k] ? r[k].u : 0.f, vk = hit[k] ? r[k].v : 0.f;
+                const float zk = hit[k] ? r[k].z : 0.f;
+                if (LOWPASS) {
+                    // R28, screen term: G = exp(-|x - x_c|^2) and z = Z_c depend on the centre only.  dL/dx_c = 2 ddx G dL/dG;
+                    // x_c = fx X / Z + cx  =>  the force on mu_c is (gxc fx, gyc fy, -(gxc (x_c - cx) + gyc (y_c - cy))) / Z + (0, 0, gz),
+                    // with x_c - cx = fx rx - ddx; the tangents get nothing (u f = v f = 0).
+                    const float gxc = 2.f * ddx[k] * r[k].G * dG, gyc = 2.f * ddy[k] * r[k].G * dG, iz = fast_rcp(zc[k]);
+                    const bool s2d = hit[k] && use2d[k];
+                    f0 = s2d ? gxc * fx * iz : f0;
+                    f1 = s2d ? gyc * fy * iz : f1;
+                    f2 = s2d ? gz - (gxc * (fx * rx - ddx[k]) + gyc * (fy * ry - ddy[k])) * iz : f2;
+                    uk = s2d ? 0.f : uk; vk = s2d ? 0.f : vk;
+                    if (POSE_ONLY && s2d) {   // mu_c x f = Z_c (r - d) x f, d = (ddx / fx, ddy / fy, 0): the r part rides in Z0..Z2
+                        const float dxr = zc[k] * ddx[k] / fx, dyr = zc[k] * ddy[k] / fy;
+                        E0 = fmaf(dyr, f2, E0); E1 = fmaf(-dxr, f2, E1); E2 = fmaf(dxr, f1, fmaf(-dyr, f0, E2));
+                    }
+                }
                 if (POSE_ONLY) {
                     F0 += f0; F1 += f1; F2 += f2;
                     Z0 = fmaf(zk, f0, Z0); Z1 = fmaf(zk, f1, Z1); Z2 = fmaf(zk, f2, Z2);
@@ -249,9 +281,9 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
         float p6[7];
         p6[6] = my_loss;
         p6[0] = F0; p6[1] = F1; p6[2] = F2;
-        p6[3] = (ry * Z2 - Z1) + (Nn1 * g[6] - Nn2 * g[5]);
-        p6[4] = (Z0 - rx * Z2) + (Nn2 * g[4] - Nn0 * g[6]);
-        p6[5] = (rx * Z1 - ry * Z0) + (Nn0 * g[5] - Nn1 * g[4]);
+        p6[3] = (ry * Z2 - Z1) + (Nn1 * g[6] - Nn2 * g[5]) - E0;
+        p6[4] = (Z0 - rx * Z2) + (Nn2 * g[4] - Nn0 * g[6]) - E1;
+        p6[5] = (rx * Z1 - ry * Z0) + (Nn0 * g[5] - Nn1 * g[4]) - E2;
 #pragma unroll
         for (int c = 0; c < 7; ++c) {
             const float s = warp_sum(inside ? p6[c] : 0.f);
@@ -399,7 +431,10 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     if (dg == nullptr) {  // pose-only (tracking, L204)
         if (d_pose6 == nullptr) return cudaSuccess;
         c->launches += 1;
-        if (dn) k_backward<true, false, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
+        if (c->cfgd.lowpass) k_backward<true, false, false, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
+                                                     cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
+                                                     c->acc, c->pose_partial, c->counters, d_pose6, FusedLoss{}, dn);
+        else if (dn) k_backward<true, false, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                      cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
                                                      c->acc, c->pose_partial, c->counters, d_pose6, FusedLoss{}, dn);
         else k_backward<true, false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
@@ -428,7 +463,10 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     if (e != cudaSuccess) return e;
     if (ms != s && fill && (e = cudaEventRecord(c->join_ev, ms)) != cudaSuccess) return e;
     c->launches += 1;
-    if (dn) k_backward<false, false, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
+    if (c->cfgd.lowpass) k_backward<false, false, false, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
+                                                  cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
+                                                  c->acc, c->pose_partial, c->counters, nullptr, FusedLoss{}, dn);
+    else if (dn) k_backward<false, false, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
                                                   cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final, c->n_last,
                                                   c->acc, c->pose_partial, c->counters, nullptr, FusedLoss{}, dn);
     else k_backward<false, false, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H, cam.tiles_x,
@@ -470,7 +508,10 @@ cudaError_t sgs_launch_backward_tracking(sgs_ctx* c, const float* trgb, const fl
     const float2* dn = (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) ? c->dn_state : nullptr;
     FusedLoss fl{trgb, tdepth, lambda_d, nsign, loss};
     c->launches += 1;
-    if (dn) k_backward<true, true, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H,
+    if (c->cfgd.lowpass) k_backward<true, true, false, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H,
+                                                       cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final,
+                                                       c->n_last, c->acc, c->pose_partial, c->counters, d_pose6, fl, dn);
+    else if (dn) k_backward<true, true, true><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H,
                                                        cam.tiles_x, cam.fx, cam.fy, cam.cx, cam.cy, c->cfgd, u, c->T_final,
                                                        c->n_last, c->acc, c->pose_partial, c->counters, d_pose6, fl, dn);
     else k_backward<true, true, false><<<tiles, SGS_BLOCK, 0, s>>>(c->render_order_valid ? c->render_order : nullptr, c->ranges, c->list_vals, c->list_stride, c->pay, cam.W, cam.H,

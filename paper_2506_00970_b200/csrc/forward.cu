@@ -13,7 +13,7 @@ namespace {
 
 struct Planes { float* p[8]; };
 
-template <bool CONTRIB, bool NDEPTH, bool MEDIAN>
+template <bool CONTRIB, bool NDEPTH, bool MEDIAN, bool LOWPASS = false>
 __global__ void __launch_bounds__(SGS_BLOCK, 4)  // 64 registers, four blocks per SM: the D_n variant would take 72 and lose one (measured: with a bound of 1 block the default variant takes 89 registers and C4's forward goes from 246 to 289 us)
 k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges, const uint32_t* __restrict__ vals, int vstride, SgsPayload pay, int W, int H,
           int tiles_x, SgsCfgDev cfg, Planes out, float* __restrict__ T_final, uint32_t* __restrict__ n_last,
@@ -21,7 +21,7 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
           float* __restrict__ contrib, const uint32_t* __restrict__ contrib_map, float2* __restrict__ dn_state,
           float* __restrict__ median_out) {
     // staged batch, structure of float4 arrays (one base register, immediate offsets, broadcast reads)
-    __shared__ float4 sh[5][SGS_BLOCK];
+    __shared__ float4 sh[LOWPASS ? 6 : 5][SGS_BLOCK];   // (R28: plane 5 = pixel-minus-centre offsets of the tile's first pixel)
     __shared__ unsigned char sh_mask[SGS_BLOCK];
     const uint32_t sa = smem_addr(&sh[0][0]), sm_a = smem_addr(sh_mask);
     constexpr uint32_t PL = SGS_BLOCK * 16;  // bytes per staged plane
@@ -88,12 +88,14 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
             const float4 g0 = pay.g0[v], g1 = pay.g1[v], g3 = pay.g3[v], g4 = pay.g4[v], g5 = pay.g5[v], g7 = pay.g7[v];
             const double2 g2 = pay.g2[v];
             float4 s0, s1, s2;
-            stage_entry(g0, g1, g2, g3, px0, py0, s0, s1, s2);
+            float xy0[2];
+            stage_entry(g0, g1, g2, g3, px0, py0, s0, s1, s2, xy0);
             sh[0][tid] = s0; sh[1][tid] = s1; sh[2][tid] = s2;
             sh[3][tid] = make_float4(g1.w, g3.w, g4.x, g4.y);
             sh[4][tid] = make_float4(g4.z, g4.w, g5.x, __uint_as_float(v));
-            mask = refine_patch_mask(warp_patch_mask(g7, (float)(tx * SGS_TILE), (float)(ty * SGS_TILE)), s0, s1, s2, g1.w,
-                                     cfg.cutoff2, cfg.alpha_min);
+            mask = warp_patch_mask(g7, (float)(tx * SGS_TILE), (float)(ty * SGS_TILE));
+            if (LOWPASS) sh[LOWPASS ? 5 : 0][tid] = make_float4(xy0[0], xy0[1], 0.f, 0.f);   // (the conic test knows nothing of the disc)
+            else mask = refine_patch_mask(mask, s0, s1, s2, g1.w, cfg.cutoff2, cfg.alpha_min);
         }
         sh_mask[tid] = (unsigned char)mask;
         __syncthreads();
@@ -112,11 +114,19 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
                 const float dn = __fmaf_rn(ly, s1.w, __fmaf_rn(lx, s0.w, s2.x));
                 const float inv = fast_rcp(dn);
                 const float u = __fmul_rn(un, inv), v = __fmul_rn(vn, inv);
-                const float rho2 = __fmaf_rn(v, v, __fmul_rn(u, u));
+                float rho2 = __fmaf_rn(v, v, __fmul_rn(u, u));
+                bool use2d = false;
+                if (LOWPASS) {   // R28: rho^2 = min(u^2 + v^2, 2 |x - x_c|^2); the screen term also where the intersection is undefined
+                    const float4 s5 = lds128(ea + 5 * PL);
+                    const float ddx = __fadd_rn(lx, s5.x), ddy = __fadd_rn(ly, s5.y);
+                    const float r2 = __fmul_rn(2.f, __fmaf_rn(ddy, ddy, __fmul_rn(ddx, ddx)));
+                    use2d = !(rho2 <= r2);
+                    rho2 = use2d ? r2 : rho2;
+                }
                 bool pass = !done && (rho2 <= cfg.cutoff2);
                 if (!__any_sync(0xffffffffu, pass)) continue;
                 const float4 s3 = lds128(ea + 3 * PL), s4 = lds128(ea + 4 * PL);
-                const float z = __fmaf_rn(s2.z, v, __fmaf_rn(s2.y, u, s2.w));
+                const float z = (LOWPASS && use2d) ? s2.w : __fmaf_rn(s2.z, v, __fmaf_rn(s2.y, u, s2.w));
                 const float G = fast_ex2(__fmul_rn(rho2, -0.72134752044448170368f));
                 const float a = fminf(cfg.alpha_max, __fmul_rn(s3.x, G));
                 pass = pass && (z > cfg.z_near) && (a >= cfg.alpha_min);
@@ -181,7 +191,9 @@ cudaError_t sgs_launch_forward(sgs_ctx* c, float* const planes[8], cudaStream_t 
                      (c->list_stride == 2 ? nullptr : c->vis_to_surfel), \
                      (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) ? c->dn_state : nullptr, c->median_out
     const bool nd = (c->cfg.flags & SGS_FLAG_NORMALISED_DEPTH) != 0;
-    if (c->median_out) {  // (sgs_render_median; never together with the contribution output)
+    if (c->cfgd.lowpass) {   // (sgs_render only: the contribution / median outputs are refused under the flag, api_run.cu)
+        k_forward<false, false, false, true><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
+    } else if (c->median_out) {  // (sgs_render_median; never together with the contribution output)
         if (nd) k_forward<false, true, true><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
         else k_forward<false, false, true><<<tiles, SGS_BLOCK, 0, s>>>(SGS_FWD_ARGS);
     } else if (c->contrib_out) {

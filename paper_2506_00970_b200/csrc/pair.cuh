@@ -131,8 +131,10 @@ __device__ __forceinline__ unsigned refine_patch_mask(const unsigned m, const fl
 
 // Builds the staged record of entry `v` for the tile whose first pixel centre is (px0, py0).
 __device__ __forceinline__ void stage_entry(const float4 g0, const float4 g1, const double2 g2, const float4 g3,
-                                            const double px0, const double py0, float4& s0, float4& s1, float4& s2) {
+                                            const double px0, const double py0, float4& s0, float4& s1, float4& s2,
+                                            float* xy0 = nullptr) {
     const float X0 = (float)(px0 - g2.x), Y0 = (float)(py0 - g2.y);  // xt, yt of the tile's first pixel
+    if (xy0) { xy0[0] = X0; xy0[1] = Y0; }   // (SGS_FLAG_LOWPASS: pixel - projected centre = (lx + X0, ly + Y0))
     const float P = g0.x, Q = g0.y, R = g0.z, S = g0.w, D = g1.x, E = g1.y, F = g1.z;
     s0 = make_float4(P, Q, __fmaf_rn(Y0, Q, __fmul_rn(X0, P)), -E);
     s1 = make_float4(R, S, __fmaf_rn(Y0, S, __fmul_rn(X0, R)), -F);

@@ -134,7 +134,16 @@ __device__ __forceinline__ void preprocess_one(const float* __restrict__ mean, c
     const double ctry = (c2 * (M[3] * M[6] + M[4] * M[7]) - M[5] * M[8]) / den;
     const double hx = sqrt(ctrx * ctrx - (c2 * (M[0] * M[0] + M[1] * M[1]) - M[2] * M[2]) / den);
     const double hy = sqrt(ctry * ctry - (c2 * (M[3] * M[3] + M[4] * M[4]) - M[5] * M[5]) / den);
-    const double xmin = ctrx - hx, xmax = ctrx + hx, ymin = ctry - hy, ymax = ctry + hy;
+    double xmin = ctrx - hx, xmax = ctrx + hx, ymin = ctry - hy, ymax = ctry + hy;
+    if (cfg.lowpass) {   // R28: footprint = cutoff ellipse united with the filter's disc (the oracle's sequence, prep_surfel)
+        const double xcf = M[2] / M[8], ycf = M[5] / M[8], rf = (double)cfg.cutoff * 0.70710678118654757;
+        if (!(isfinite(xmin) && isfinite(xmax))) { xmin = xcf; xmax = xcf; }
+        if (!(isfinite(ymin) && isfinite(ymax))) { ymin = ycf; ymax = ycf; }
+        if (xcf - rf < xmin) xmin = xcf - rf;
+        if (xcf + rf > xmax) xmax = xcf + rf;
+        if (ycf - rf < ymin) ymin = ycf - rf;
+        if (ycf + rf > ymax) ymax = ycf + rf;
+    }
     if (!(isfinite(xmin) && isfinite(xmax) && isfinite(ymin) && isfinite(ymax))) return;
     if (!(xmax > 0.0 && xmin < (double)cam.W && ymax > 0.0 && ymin < (double)cam.H)) return;
     const double ts = (double)SGS_TILE;
@@ -202,7 +211,10 @@ __device__ __forceinline__ bool precull_f32(const float* __restrict__ mean, cons
     const float d = 1e-5f * (fabsf(m0) + fabsf(m1) + fabsf(m2) + cam.pc_tabs) + cam.pm_t +
                     cam.pm_r * (fabsf(X) + fabsf(Y) + fabsf(Z));
     if (Z + d < cfg.z_near) return true;
-    const float r = cfg.cutoff * fmaxf(fabsf(scale[0]), fabsf(scale[1])) * 1.00001f + d;
+    float r = cfg.cutoff * fmaxf(fabsf(scale[0]), fabsf(scale[1])) * 1.00001f + d;
+    // SGS_FLAG_LOWPASS (R28): the footprint also holds the disc of cutoff / sqrt 2 pixels around the projected centre, i.e.
+    // that many pixels times Z / f sideways at the centre's depth (every side-plane normal below is at least f long)
+    if (cfg.lowpass) r += cfg.cutoff * 0.70711f * (fmaxf(Z, 0.f) + d) / fminf(cam.fx, cam.fy) * 1.0001f;
     // left: fx X + cx Z < 0 ; right: fx X + (cx - W) Z > 0 ; top / bottom alike.  Normals un-normalised:
     // compare against r * |normal| (|normal| rounded up on the host, cam.pc_n, and r rounded up above).
     if (cam.fx * X + cam.cx * Z < -r * cam.pc_n[0]) return true;

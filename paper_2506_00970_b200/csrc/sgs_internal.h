@@ -64,6 +64,7 @@ struct SgsCfgDev {
     float cutoff;   // sqrt(cutoff2)
     double cutoff2_d, z_near_d;
     double alpha_min_d; int tight;   // SGS_FLAG_TIGHT_BINNING (R26, R27)
+    int lowpass;                     // SGS_FLAG_LOWPASS (R28)
 };
 
 // Device-side counters of one render (also copied to pinned host memory).
