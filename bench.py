@@ -157,7 +157,7 @@ class Workload:
     """Device-resident inputs + the step function for one config."""
 
     def __init__(self, name, iters_override=None, contrib=False, prefetch=True, reuse=True, normalised_depth=False, graph=False,
-                 tight=False, radix=False):
+                 tight=False, radix=False, two_streams=False):
         self.contrib = contrib
         self.graph, self.cg, self.eager_steps = graph, None, 0
         nd = self.normalised_depth = normalised_depth
@@ -183,6 +183,15 @@ class Workload:
             self.ren = sgs.Renderer(async_mode=True, lazy_grads=True, normalised_depth=nd, tight_binning=tight)
         self.rens = [self.ren] + ([sgs.Renderer(async_mode=True, lazy_grads=True, normalised_depth=nd, tight_binning=tight)] if two else [])
         self.side = torch.cuda.Stream(priority=-1) if len(self.rens) > 1 else None
+        # --two-streams: each of the two contexts works through its views on a stream of its own (binning in line, own image
+        # and upstream buffers), so one view's loss and backward run beside the other's binning and forward
+        self.two_streams = two_streams and len(self.rens) > 1
+        if self.two_streams:
+            for r in self.rens:
+                r.close()
+            self.ren = sgs.Renderer(async_mode=True, normalised_depth=nd, tight_binning=tight)
+            self.rens = [self.ren, sgs.Renderer(async_mode=True, normalised_depth=nd, tight_binning=tight)]
+            self.streams = [torch.cuda.Stream(), torch.cuda.Stream()]
         cam0 = self.cams[0]
         self.H, self.W = cam0.height, cam0.width
         z = lambda c: torch.zeros((c, self.H, self.W), device="cuda")
@@ -213,6 +222,11 @@ class Workload:
         for r in self.rens[1:]:   # the second context's workspace settles on the same views
             for c in self.ccams:
                 self._render_retry(c, r)
+        if self.two_streams:
+            zz = lambda c: torch.zeros((c, self.H, self.W), device="cuda")
+            self.bufs = [dict(im=dict(rgb=zz(3), depth=zz(1), normal=zz(3), alpha=zz(1)),
+                              up=dict(rgb=zz(3), depth=zz(1), normal=zz(3), alpha=zz(1)), loss=torch.zeros(1, device="cuda"))
+                         for _ in self.rens]
         self.flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
     def _render_retry(self, cam, ren=None):
@@ -228,11 +242,19 @@ class Workload:
                     raise
         raise RuntimeError("workspace did not settle")
 
-    def one(self, v, ren=None):
+    def one(self, v, ren=None, bufs=None):
         """render -> loss -> backward for view v (everything enqueued, no host sync)."""
         ren = ren or self.ren
         cam = self.ccams[v]
         trgb, tdep = self.targets[v]
+        if bufs is not None:   # --two-streams: this context's own buffers, on the current (its own) stream
+            im, up, loss = bufs["im"], bufs["up"], bufs["loss"]
+            ren.render(self.sf, cam, **im)
+            ren.mapping_loss(cam, im, trgb, tdep, 0.875, 0.5, 0.02, -1.0, up, loss)
+            ren.ssim_loss(im["rgb"], trgb, 0.125, up["rgb"], loss)
+            ren.backward(d_rgb=up["rgb"], d_depth=up["depth"], d_normal=up["normal"], d_alpha=up["alpha"],
+                         grads=self.grads_of[id(ren)], d_pose6=self.p6_of[id(ren)], accumulate=True)
+            return
         if self.tracking:  # one tracking iteration: K-pre + K-track (render, Eq. 15-19 loss, pose-only backward); images written
             ren.track_iter(self.sf, cam, trgb, tdep, 0.5, -1.0, self.p6, self.loss, **self.im)
             return
@@ -281,6 +303,19 @@ class Workload:
                 if v % WINDOW == 0:
                     self.begin_window()
                 self.one(v)
+        elif self.two_streams:
+            torch = self.torch
+            main = torch.cuda.current_stream()
+            nv = len(self.cams)
+            for w0 in range(0, nv, WINDOW):   # a window: both streams start behind the main stream (optimiser step of the last window) ...
+                for k, st in enumerate(self.streams):
+                    st.wait_stream(main)
+                    with torch.cuda.stream(st):
+                        self.rens[k].zero_grads(self.grads_of[id(self.rens[k])])
+                        for v in range(w0 + k, min(w0 + WINDOW, nv), 2):
+                            self.one(v, self.rens[k], self.bufs[k])
+                for st in self.streams:       # ... and the main stream (the consumer of the window's gradients) waits for both
+                    main.wait_stream(st)
         else:
             main = self.torch.cuda.current_stream()
             self.side.wait_stream(main)   # the step's first launch stays behind the timed region's start event
@@ -428,7 +463,7 @@ def run_config(name, args, torch, dist, world, rank, local, peaks):
         torch.cuda.synchronize()
 
     wl = Workload(name, args.iters, args.contrib, not args.no_prefetch, not args.no_reuse, args.normalised_depth, args.graph,
-                  args.tight, args.radix)
+                  args.tight, args.radix, args.two_streams)
     K, W = args.steps, max(args.warmup, 3)
     per_step = []
     for _ in range(W):
@@ -508,7 +543,8 @@ def run_config(name, args, torch, dist, world, rank, local, peaks):
                            replicas=world,
                            survivor_list=("built once per step (frame) with a 3 cm / 0.02 rad pose margin, SGS_FLAG_TRACK_REUSE"
                                           if (wl.tracking and not args.no_reuse) else "every render"),
-                           binning=("sgs_prepare of view v+1 on a second context and a side stream, under view v's compositing"
+                           binning=("two contexts on two streams, views alternating; binning in line on each" if getattr(wl, "two_streams", False) else
+                                    "sgs_prepare of view v+1 on a second context and a side stream, under view v's compositing"
                                     if len(wl.rens) > 1 else "in line (sgs_render / sgs_track_iter)")))
     if not wl.tracking:
         out["config"]["gradients"] = f"summed over windows of {WINDOW} views (sgs_backward_accumulate), zeroed per window"
@@ -583,6 +619,7 @@ def main():
     ap.add_argument("--graph", action="store_true", help="SGS_FLAG_GRAPH: each step (a tracking frame, or a mapping window on one context) replayed as one CUDA graph")
     ap.add_argument("--normalised-depth", action="store_true", help="SGS_FLAG_NORMALISED_DEPTH: depth image D/O (tracking takes the unfused sequence)")
     ap.add_argument("--tight", action="store_true", help="SGS_FLAG_TIGHT_BINNING: opacity-aware cutoff + tile-exact culling (shorter tile lists, same images)")
+    ap.add_argument("--two-streams", action="store_true", help="mapping configs: two contexts on two streams, views alternating (no prefetch pipeline)")
     ap.add_argument("--radix", action="store_true", help="SGS_FLAG_RADIX_BINNING: the global LSD radix sort of the 64-bit keys instead of the per-tile buckets (A/B; one context, in line)")
     ap.add_argument("--contrib", action="store_true", help="mapping configs: render with sgs_render_contrib (C_k output on)")
     ap.add_argument("--ingest-ncu", default=None, metavar="RAW_CSV",
