@@ -603,6 +603,29 @@ def run_config(name, args, torch, dist, world, rank, local, peaks):
     return out
 
 
+def probe_staging(args):
+    """--probe-staging: no benchmark.  Renders view 0 of --config (default C2) and times the staging of its tile lists alone,
+    by LDG gathers (mode 0, what the kernels do) and by one cp.async.bulk per record (mode 1): sgs_probe_staging."""
+    import torch
+    import scenegen
+    import paper_2506_00970_b200 as sgs
+    name = args.config or "C2"
+    sc, cams, info = scenegen.make_config(name)
+    cam = cams[0]
+    d = lambda a, dt=torch.float32: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to("cuda", dt)
+    keep = [d(sc.mean), d(sc.scale), d(sc.quat), d(sc.opacity), d(sc.rgb), d(sc.active, torch.uint8)]   # (the struct borrows them)
+    sf = sgs.Renderer.surfels(*keep)
+    ren = sgs.Renderer()
+    z = lambda c: torch.zeros((c, cam.height, cam.width), device="cuda")
+    ren.render(sf, sgs.make_camera(cam.width, cam.height, cam.fx, cam.fy, cam.cx, cam.cy, cam.T_cw), rgb=z(3), depth=z(1), normal=z(3), alpha=z(1))
+    st = ren.stats()
+    out = dict(config=name, n_entries=st["n_entries"], tiles=((cam.width + 15) // 16) * ((cam.height + 15) // 16))
+    for rep in range(2):
+        for mode, key in ((0, "ldg_gather_us"), (1, "bulk_copy_us")):
+            out[key] = ren.probe_staging(mode, reps=50)
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -622,6 +645,7 @@ def main():
     ap.add_argument("--two-streams", action="store_true", help="mapping configs: two contexts on two streams, views alternating (no prefetch pipeline)")
     ap.add_argument("--radix", action="store_true", help="SGS_FLAG_RADIX_BINNING: the global LSD radix sort of the 64-bit keys instead of the per-tile buckets (A/B; one context, in line)")
     ap.add_argument("--contrib", action="store_true", help="mapping configs: render with sgs_render_contrib (C_k output on)")
+    ap.add_argument("--probe-staging", action="store_true", help="no benchmark: time the staging of --config's tile lists by LDG gathers and by cp.async.bulk (sgs_probe_staging)")
     ap.add_argument("--ingest-ncu", default=None, metavar="RAW_CSV",
                     help="no benchmark: read `ncu -i X.ncu-rep --page raw --csv` of a capture of --config and update profiles/r02_traffic.json")
     args = ap.parse_args()
@@ -630,6 +654,8 @@ def main():
         return
     if args.impl == "reference":
         return run_reference(args)
+    if args.probe_staging:
+        return probe_staging(args)
 
     import torch
     import torch.distributed as dist

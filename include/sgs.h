@@ -384,6 +384,14 @@ SGS_API int sgs_map_correction(sgs_ctx* ctx, int64_t n, float* mean, float* quat
  * kernels' roofline.  tflops: HOST double. */
 SGS_API int sgs_measure_fp32_peak(double* tflops, void* cuda_stream);
 
+/* A measurement, not a step of the path (north_star: "TMA bulk copies where that pays"): runs the staging of the compositing
+ * kernels -- gather of the tile lists' 128-byte payload records, re-basing, seven 16-byte planes into shared memory -- over the
+ * tile lists of the ctx's last sgs_render, `reps` times, with mode 0 = one thread per entry gathering seven 16-byte loads (what
+ * the kernels do) or mode 1 = one cp.async.bulk (TMA) of the 128-byte record per entry into shared memory, completed through
+ * an mbarrier, then the same arithmetic from shared memory.  us_per_launch: HOST double.  Waits.  SGS_NO_FORWARD_STATE
+ * without a preceding sgs_render. */
+SGS_API int sgs_probe_staging(sgs_ctx* ctx, int mode, int reps, double* us_per_launch, void* cuda_stream);
+
 SGS_API const char* sgs_status_string(int status);
 
 #ifdef __cplusplus

@@ -59,7 +59,7 @@ class sgs_stats(C.Structure):
 EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_prepare", "sgs_backward", "sgs_wait_grads", "sgs_tracking_loss",
            "sgs_backward_tracking", "sgs_track_iter", "sgs_track_new_frame", "sgs_render_contrib", "sgs_render_median", "sgs_covisibility", "sgs_mapping_loss", "sgs_ssim_loss", "sgs_map_correction", "sgs_measure_fp32_peak", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
            "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string",
-           "sgs_track_iter_dev", "sgs_backward_accumulate", "sgs_zero_grads", "sgs_map_view_host", "sgs_fetch_grads_host", "sgs_sync_host"]
+           "sgs_track_iter_dev", "sgs_probe_staging", "sgs_backward_accumulate", "sgs_zero_grads", "sgs_map_view_host", "sgs_fetch_grads_host", "sgs_sync_host"]
 
 _lib = None
 _LIVE = weakref.WeakSet()
@@ -339,6 +339,13 @@ class Renderer:
         _check(self.lib.sgs_track_iter_dev(self._ctx, C.byref(surfels), C.byref(cam), _ptr(d_T_cw), C.byref(t), C.c_float(lambda_d),
                                            C.c_float(normal_sign), C.byref(out), _ptr(d_pose6), _ptr(loss), _stream_ptr(stream)),
                "sgs_track_iter_dev")
+
+    def probe_staging(self, mode, reps=20, stream=None):
+        """sgs_probe_staging: microseconds per launch of the staging alone over the last render's tile lists (mode 0: LDG
+        gathers, mode 1: one cp.async.bulk per 128-byte record)."""
+        us = C.c_double(0.0)
+        _check(self.lib.sgs_probe_staging(self._ctx, C.c_int(mode), C.c_int(reps), C.byref(us), _stream_ptr(stream)), "sgs_probe_staging")
+        return float(us.value)
 
     def get_binning(self, n, tiles):
         """sgs_get_binning -> numpy copies: keys (E,) u64, idx (E,) u32, ranges (tiles,2) u32, culled (n,) u8."""
