@@ -37,7 +37,7 @@ F_TEST, F_COMP_FWD, F_COMP_BWD_FULL, F_COMP_BWD_POSE = 26, 26, 102, 94
 # `bench.py --ingest-ncu` from `ncu --set full` captures (ncu flushes L2 before every replay: cold-cache figures)
 TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_traffic.json")
 WINDOW = 5            # views per mapping window: N_a + N_i (Tab. I)
-KERNEL_OF_STAGE = {"forward": "k_forward", "backward": "k_backward", "track": "k_track", "preprocess": "k_pre_project",
+KERNEL_OF_STAGE = {"forward": "k_forward<", "backward": "k_backward<", "track": "k_track<", "preprocess": "k_pre_project<",
                    "sort": "k_tile_order"}
 
 
@@ -63,7 +63,7 @@ def ingest_ncu(csv_path, config):
         vals = [float(r[rd].replace(",", "")) * scale[units[rd]] + float(r[wr].replace(",", "")) * scale[units[wr]]
                 for r in rows[hdr + 2:] if len(r) > wr and kern in r[kn]]
         if vals:
-            cfg[stage] = dict(kernel=kern, launches=len(vals), dram_bytes_per_launch=sum(vals) / len(vals), source=os.path.basename(csv_path))
+            cfg[stage] = dict(kernel=kern.rstrip("<"), launches=len(vals), dram_bytes_per_launch=sum(vals) / len(vals), source=os.path.basename(csv_path))
     json.dump(out, open(TRAFFIC_JSON, "w"), indent=1, sort_keys=True)
     return cfg
 

@@ -308,7 +308,7 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
 __global__ void __launch_bounds__(256)
 k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __restrict__ vis_to_surfel,
                   const uint8_t* __restrict__ culled,
-                  float* __restrict__ acc, const float* __restrict__ mean, const float* __restrict__ scale,
+                  float* __restrict__ acc, SgsPayload pay,
                   const float* __restrict__ quat, SgsCamDev cam, sgs_surfel_grads out,
                   float* __restrict__ pose_partial, SgsCounters* __restrict__ counters_rw,
                   float* __restrict__ d_pose6, int survivors, int accumulate) {
@@ -337,20 +337,20 @@ k_surfel_backward(const SgsCounters* __restrict__ counters, const uint32_t* __re
         const float qn = sqrtf(qw0 * qw0 + qx0 * qx0 + qy0 * qy0 + qz0 * qz0);
         const float qi = 1.f / qn;
         const float qw = qw0 * qi, qx = qx0 * qi, qy = qy0 * qi, qz = qz0 * qi;
-        const float tu[3] = {1.f - 2.f * (qy * qy + qz * qz), 2.f * (qx * qy + qw * qz), 2.f * (qx * qz - qw * qy)};
-        const float tv[3] = {2.f * (qx * qy - qw * qz), 1.f - 2.f * (qx * qx + qz * qz), 2.f * (qy * qz + qw * qx)};
-        const float tn[3] = {2.f * (qx * qz + qw * qy), 2.f * (qy * qz - qw * qx), 1.f - 2.f * (qx * qx + qy * qy)};
-        const float su = scale[2 * i], sv = scale[2 * i + 1];
-        const float m[3] = {mean[3 * i], mean[3 * i + 1], mean[3 * i + 2]};
-        float tuc[3], tvc[3], tnc[3], muc[3];
-#pragma unroll
-        for (int r = 0; r < 3; ++r) {
-            const float r0 = cam.Rf[3 * r], r1 = cam.Rf[3 * r + 1], r2 = cam.Rf[3 * r + 2];
-            tuc[r] = r0 * tu[0] + r1 * tu[1] + r2 * tu[2];
-            tvc[r] = r0 * tv[0] + r1 * tv[1] + r2 * tv[2];
-            tnc[r] = r0 * tn[0] + r1 * tn[1] + r2 * tn[2];
-            muc[r] = r0 * m[0] + r1 * m[1] + r2 * m[2] + cam.tf[r];
-        }
+        // The camera-space frame comes from the splat's payload record (contiguous, still in L2 from the compositing
+        // kernels) instead of the map's mean / scale arrays (two or three more scattered DRAM sectors per splat; this
+        // kernel moves 900 B of DRAM per visible splat at 5 % issue utilisation, profiles/r02_c4.md): a_u = s_u t_uc and
+        // a_v = s_v t_vc give the scales as their lengths, n_c is t_nc, and mu_c = ((x_c - cx) / fx, (y_c - cy) / fy, 1) z_c.
+        const size_t pv = survivors ? (size_t)i : (size_t)v;
+        const float4 g3 = pay.g3[pv], g4 = pay.g4[pv], g5 = pay.g5[pv], g6 = pay.g6[pv];
+        const double2 g2 = pay.g2[pv];
+        const float au[3] = {g5.y, g5.z, g5.w}, av[3] = {g6.x, g6.y, g6.z};
+        const float su = sqrtf(au[0] * au[0] + au[1] * au[1] + au[2] * au[2]), sv = sqrtf(av[0] * av[0] + av[1] * av[1] + av[2] * av[2]);
+        const float isu = 1.f / su, isv = 1.f / sv;
+        const float tuc[3] = {au[0] * isu, au[1] * isu, au[2] * isu}, tvc[3] = {av[0] * isv, av[1] * isv, av[2] * isv};
+        const float tnc[3] = {g4.z, g4.w, g5.x};
+        const float zc = g3.z;
+        const float muc[3] = {(float)((g2.x - (double)cam.cx) / (double)cam.fx) * zc, (float)((g2.y - (double)cam.cy) / (double)cam.fy) * zc, zc};
         const float* dmu = a;        // dL/dmu_c
         const float* dau = a + 3;    // dL/d(s_u t_uc)
         const float* dav = a + 6;    // dL/d(s_v t_vc)
@@ -491,8 +491,8 @@ cudaError_t sgs_launch_backward(sgs_ctx* c, const float* const up[8], const sgs_
     if (blocks < 1) blocks = 1;
     c->launches += 1;
     c->grads_on_aux = lazy;
-    k_surfel_backward<<<blocks, 256, 0, ks>>>(c->counters, bucket_mode ? c->vis_list : c->vis_to_surfel, c->culled, c->acc, c->last_surfels.mean,
-                                             c->last_surfels.scale, c->last_surfels.quat, cam, *dg, c->pose_partial,
+    k_surfel_backward<<<blocks, 256, 0, ks>>>(c->counters, bucket_mode ? c->vis_list : c->vis_to_surfel, c->culled, c->acc, c->pay,
+                                             c->last_surfels.quat, cam, *dg, c->pose_partial,
                                              c->counters, d_pose6, bucket_mode ? 1 : 0, accumulate ? 1 : 0);
     return cudaGetLastError();
 }

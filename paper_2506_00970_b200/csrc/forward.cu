@@ -7,6 +7,7 @@
 // the mask bytes, then find-first-set), reading the staged records as warp-wide broadcasts.  A warp leaves the batch loop when all its pixels are
 // saturated; the block stops fetching batches when every pixel is.
 #include "pair.cuh"
+#include "regsort.cuh"
 #include "sgs_internal.h"
 
 namespace {
@@ -44,15 +45,20 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
         if (tid == 0) { ranges[2 * tile] = start; ranges[2 * tile + 1] = end; }
         unsigned long long* g = bucket + (size_t)start;
         unsigned long long* sk = reinterpret_cast<unsigned long long*>(&sh[0][0]);
-        if (n >= 2 && n <= 256) {
-            const bool mine = (uint32_t)tid < n;
-            const unsigned long long key = mine ? g[tid] : ~0ull;
-            if (mine) sk[tid] = key;
-            __syncthreads();
-            uint32_t rank = 0;
-            for (uint32_t k = 0; k < n; ++k) rank += sk[k] < key ? 1u : 0u;
-            if (mine) g[rank] = key;
-        } else if (n > 256) {
+        if (n >= 2 && n <= 512) {   // keys in registers: shuffles + a few shared-memory exchanges (regsort.cuh)
+            uint32_t npad = 32;
+            while (npad < n) npad <<= 1;
+            if (n <= 256) {
+                unsigned long long key[1] = {(uint32_t)tid < n ? g[tid] : ~0ull};
+                block_sort_keys<1>(key, sk, tid, npad);
+                if ((uint32_t)tid < n) g[tid] = key[0];
+            } else {
+                unsigned long long key[2] = {g[tid], (uint32_t)tid + 256u < n ? g[tid + 256] : ~0ull};
+                block_sort_keys<2>(key, sk, tid, npad);
+                g[tid] = key[0];
+                if ((uint32_t)tid + 256u < n) g[tid + 256] = key[1];
+            }
+        } else if (n > 512) {
             uint32_t npad = 512;
             while (npad < n) npad <<= 1;
             for (uint32_t i = tid; i < npad; i += SGS_BLOCK) sk[i] = i < n ? g[i] : ~0ull;
