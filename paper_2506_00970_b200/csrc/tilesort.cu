@@ -145,10 +145,19 @@ __global__ void k_export_copy(const uint64_t* __restrict__ bucket, const uint32_
                               const uint32_t* __restrict__ xr, uint64_t* __restrict__ keys, uint32_t* __restrict__ idx) {
     const uint32_t t = blockIdx.x;
     const uint32_t s = ranges[2 * t], n = ranges[2 * t + 1] - s, d = xr[2 * t];
+    // Buckets of up to 384 entries are ranked here (keys are unique): K-track leaves the bucket of a tile it splits
+    // between an owner and a helper block unsorted in memory (both rank the raw bucket concurrently, track.cu).  Longer
+    // buckets were sorted in place by whichever kernel walked them.
+    const bool rank_here = n <= 384u;
     for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
         const uint64_t k = bucket[s + i];
-        keys[d + i] = ((uint64_t)t << 32) | (k >> 32);
-        idx[d + i] = (uint32_t)k;
+        uint32_t pos = i;
+        if (rank_here) {
+            pos = 0;
+            for (uint32_t j = 0; j < n; ++j) pos += bucket[s + j] < k ? 1u : 0u;
+        }
+        keys[d + pos] = ((uint64_t)t << 32) | (k >> 32);
+        idx[d + pos] = (uint32_t)k;
     }
 }
 

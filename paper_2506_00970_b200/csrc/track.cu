@@ -282,28 +282,34 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     // partial sums and draws its ticket below, so that the grid reduction counts every block)
     const bool split = (helper || has_helper) && !presorted && n > TRK_SPLIT_MIN && n <= (uint32_t)TRK_CAP;
     const uint32_t msp = split ? (((n + 1u) / 2u + 31u) & ~31u) : n;  // block 0: [0, msp) on the way back, block 1: [msp, n)
-    // per-pixel state the owner hands to its helper: 6 x 256 floats in global memory.  The hand-over is two flag values per
-    // launch, 4 * epoch + 1 (the owner has written the SORTED bucket back) and 4 * epoch + 2 (... and the pixels' state); the
-    // epoch is a device word (split_flag[SGS_TRACK_HELPERS]) that the launch's last block increments, so a replayed CUDA
-    // graph -- whose kernel arguments are frozen -- never meets a flag value left by an earlier replay.
+    // per-pixel state the owner hands to its helper: 6 x 256 floats in global memory, published by the flag value
+    // 4 * epoch + 2; the epoch is a device word (split_flag[SGS_TRACK_HELPERS]) that the launch's last block increments, so
+    // a replayed CUDA graph -- whose kernel arguments are frozen -- never meets a flag value left by an earlier replay.
+    // Owner and helper both rank the tile's RAW bucket by themselves, at the same time: the owner of a split tile therefore
+    // does not write the sorted keys back in place (a helper scheduled late would rank a half-permuted bucket);
+    // sgs_get_binning's export ranks short buckets itself (tilesort.cu, k_export_copy).
     float* st = split_state + (size_t)slot * (8 * SGS_BLOCK);  // g0..g3, T, last, zref (NDEPTH), one spare
     const unsigned int epoch4 = split ? 4u * __ldcg(split_flag + SGS_TRACK_HELPERS) : 0u;
     volatile unsigned int* my_flag = reinterpret_cast<volatile unsigned int*>(split_flag + slot);
     if (crank == 1) {
         if (split) {
-            // The helper reads the bucket only AFTER its owner has published the sorted keys: it never looks at the raw
-            // bucket, which the owner permutes in place (reading it unordered was a data race).  It has nothing else to do
-            // until the owner's forward walk ends, so waiting for the owner's sort costs nothing.
             if (helper_delay_ns) __nanosleep(helper_delay_ns);  // (test hook: SGS_DEBUG_HELPER_DELAY_NS, see sgs_create)
-            for (uint32_t e = tid; e < (uint32_t)TRK_CAP; e += SGS_BLOCK) sh_mask[e] = 0;
-            if (tid == 0) {
-                unsigned int f;
-                while ((f = *my_flag) != epoch4 + 1u && f != epoch4 + 2u) __nanosleep(100);
-                __threadfence();
+            for (uint32_t e = tid; e < (uint32_t)TRK_CAP; e += SGS_BLOCK) {
+                s_keys[e] = e < n ? g[e] : ~0ull;   // the raw bucket: nobody writes it during this launch
+                sh_mask[e] = 0;
             }
             __syncthreads();
-            for (uint32_t e = msp + tid; e < n; e += SGS_BLOCK)   // this block's part of the sorted list, at slot e - msp
-                sh_mask[e - msp] = (unsigned char)stage_track(pay, (uint32_t)__ldcg(g + e), px0, py0, tx0, ty0, sh, (int)(e - msp), cfg);
+            for (uint32_t e0 = 0; e0 < n; e0 += SGS_BLOCK) {
+                if (e0 + (uint32_t)(wid * 32) < n) {
+                    const uint32_t e = e0 + tid;
+                    const bool mine = e < n;
+                    const unsigned long long key = mine ? s_keys[e] : ~0ull;
+                    uint32_t rank = 0;
+                    for (uint32_t k = 0; k < n; ++k) rank += s_keys[k] < key ? 1u : 0u;
+                    if (mine && rank >= msp)   // this block's part of the sorted list, at slot rank - msp
+                        sh_mask[rank - msp] = (unsigned char)stage_track(pay, (uint32_t)key, px0, py0, tx0, ty0, sh, (int)(rank - msp), cfg);
+                }
+            }
             __syncthreads();
             if (tid == 0) {  // the owner has walked forward and stored these pixels' state
                 while (*my_flag != epoch4 + 2u) __nanosleep(200);
@@ -334,14 +340,12 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
                 uint32_t rank = 0;
                 for (uint32_t k = 0; k < n; ++k) rank += s_keys[k] < key ? 1u : 0u;
                 if (mine) {
-                    g[rank] = key;  // sorted list for sgs_get_binning and for the tile's helper
+                    if (!split) g[rank] = key;  // sorted list for sgs_get_binning (a split tile's bucket stays raw: its helper ranks it too)
                     sh_mask[rank] = (unsigned char)stage_track(pay, (uint32_t)key, px0, py0, tx0, ty0, sh, (int)rank, cfg);
                 }
             }
         }
-        if (split) __threadfence();  // the sorted keys, before the flag below
         __syncthreads();
-        if (split && tid == 0) *my_flag = epoch4 + 1u;
         if (!split) {
             forward_walk(0u, n);
             finish_forward();
