@@ -293,7 +293,9 @@ int sgs_track_iter(sgs_ctx* c, const sgs_surfels* sf, const sgs_camera* cam, con
     // the iteration's chain there: no side stream); the order is a scheduling hint, results do not depend on it
     c->order_skip = graph_mode(c) && (c->cfg.flags & SGS_FLAG_TRACK_REUSE) && c->surv_valid;
     c->defer_counters = true;  // (bin_buckets clears it when it cannot honour it)
+    c->track_binning = true;
     int r = bin_view(c, sf, cam, false, s);
+    c->track_binning = false;
     c->use_surv_cache = false;
     const bool deferred = c->defer_counters;
     c->defer_counters = false;

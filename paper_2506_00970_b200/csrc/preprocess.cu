@@ -512,14 +512,17 @@ k_pre_project(const float* __restrict__ mean, const float* __restrict__ scale, c
         for (int off = 16; off > 0; off >>= 1) wcnt += __shfl_xor_sync(0xffffffffu, wcnt, off);
         unsigned int vbase = 0;
         if (lane == 0 && vis_mask) {
-            vbase = atomicAdd(&counters->n_visible, (unsigned int)__popc(vis_mask));
+            if (vis_list != nullptr) vbase = atomicAdd(&counters->n_visible, (unsigned int)__popc(vis_mask));
+            else atomicAdd(&counters->n_visible, (unsigned int)__popc(vis_mask));   // (no return value: a RED, nothing waits)
             if (!TIGHT) atomicAdd(&counters->n_entries, (unsigned long long)wcnt);   // (TIGHT: counted at emission, below)
         }
-        vbase = __shfl_sync(0xffffffffu, vbase, 0);
+        // (vis_list == nullptr inside sgs_track_iter: no per-surfel backward follows, and waiting for the atomic's return value
+        // is a dependent L2 round trip per round of a kernel that sits on the tracking iteration's chain)
+        if (vis_list != nullptr) vbase = __shfl_sync(0xffffffffu, vbase, 0);
         if (o.vis) {
             // the visible surfels, compact (arrival order): what the per-surfel backward walks -- K-pre-A's survivor list
             // is several times longer (C4: every splat the frustum test cannot exclude) and costs it a sector per entry
-            vis_list[vbase + __popc(vis_mask & ((1u << lane) - 1u))] = (uint32_t)i;
+            if (vis_list != nullptr) vis_list[vbase + __popc(vis_mask & ((1u << lane) - 1u))] = (uint32_t)i;
             if (!cin.p0) { if (!TIGHT) in_o = opacity[i]; in_c[0] = rgb[3 * i]; in_c[1] = rgb[3 * i + 1]; in_c[2] = rgb[3 * i + 2]; }
             pay.g0[i] = make_float4(o.P, o.Q, o.R, o.S);
             pay.g1[i] = make_float4(o.D, o.E, o.F, in_o);
@@ -691,7 +694,7 @@ cudaError_t sgs_launch_preprocess_bucket(sgs_ctx* c, const sgs_surfels* sf, cuda
     const cudaError_t le = cudaLaunchKernelEx(&cfg, kern, sf->mean, sf->scale, sf->quat, sf->opacity, sf->rgb, c->camd,
                                               c->cfgd, c->pay, c->culled, c->counters, (const uint32_t*)c->vis_to_surfel,
                                               (const unsigned int*)n_surv, c->cursor, c->bucket, (uint32_t)c->tile_cap, cin,
-                                              (cached && prezeroed && cin.p0) ? 1 : 0, c->vis_list, pd, sp_r);
+                                              (cached && prezeroed && cin.p0) ? 1 : 0, c->track_binning ? nullptr : c->vis_list, pd, sp_r);
     if (le != cudaSuccess) return le;
     return cudaGetLastError();
 }

@@ -15,7 +15,7 @@ __device__ __forceinline__ float warp_sum(float v) {
 // Returns (to every thread of the block) whether this block was the last one.
 __device__ __forceinline__ bool finish_pose(const float* __restrict__ partial, unsigned int n_blocks,
                                             SgsCounters* __restrict__ counters, float* __restrict__ d_pose6,
-                                            float* __restrict__ loss_out = nullptr, bool invalid = false) {
+                                            float* __restrict__ loss_out = nullptr, unsigned int check_tile_cap = 0u) {
     __shared__ bool s_is_last;
     __shared__ double s_sum[8][7];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -28,6 +28,12 @@ __device__ __forceinline__ bool finish_pose(const float* __restrict__ partial, u
     __syncthreads();
     if (!s_is_last) return false;
     __threadfence();
+    // (K-track's validity check, see below: the two counters are fetched here so that their latency hides under the partial sums)
+    unsigned int chk_max = 0u, chk_stale = 0u;
+    if (check_tile_cap != 0u) {
+        chk_max = *reinterpret_cast<volatile unsigned int*>(&counters->max_tile);
+        chk_stale = *reinterpret_cast<volatile unsigned int*>(&counters->stale);
+    }
     double a[7] = {0, 0, 0, 0, 0, 0, 0};
     for (unsigned int b = tid; b < n_blocks; b += blockDim.x) {
         const float4 lo = __ldcg(reinterpret_cast<const float4*>(partial + (size_t)b * 8));
@@ -45,7 +51,10 @@ __device__ __forceinline__ bool finish_pose(const float* __restrict__ partial, u
     if (tid < 7) {
         double v = 0;
         for (int w2 = 0; w2 < (int)(blockDim.x >> 5); ++w2) v += s_sum[w2][tid];
-        if (invalid) v = (double)__int_as_float(0x7fc00000);  // the caller's lists were incomplete: NaN, not a plausible number
+        // check_tile_cap != 0 (K-track): a tile bucket that overflowed (entries dropped) or a kept survivor list the
+        // device-resident pose has left (splats possibly missing) must not pass for a result -- NaN, not a plausible number.
+        // Only this, the last, block looks (the counters are final since the preprocess ended).
+        if (check_tile_cap != 0u && (chk_max > check_tile_cap || chk_stale != 0u)) v = (double)__int_as_float(0x7fc00000);
         if (tid < 6) d_pose6[tid] = (float)v;
         else if (loss_out) *loss_out = (float)v;
     }

@@ -146,6 +146,7 @@ struct sgs_ctx {
     sgs_camera surv_cam;
     float* surv_pose_dev;              // 12 floats: the DEVICE pose the kept list was built around (sgs_track_iter_dev)
     const float* pose_dev;             // non-NULL inside sgs_track_iter_dev: the preprocess kernels read T_cw from here
+    bool track_binning;                // inside sgs_track_iter's fused path: K-pre-B need not build vis_list
     int narrow_prepare;                // > 0 inside sgs_prepare: K-pre-B blocks per SM
     bool grads_on_aux;                 // SGS_FLAG_LAZY_GRADS: the last sgs_backward left its final kernel on aux_stream
     bool copy_in_flight;               // counters_ready was recorded on aux_stream and nothing on the caller's stream waited for it yet

@@ -94,6 +94,8 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     const double px0 = (double)(tx * SGS_TILE) + 0.5, py0 = (double)(ty * SGS_TILE) + 0.5;
     const size_t pix = (size_t)py * W + px, HW = (size_t)W * H;
 
+    // (the hand-over epoch of split tiles, see below: fetched here, with the frame's pixel, so that no later load depends on it)
+    const unsigned int epoch_raw = n_help > 0 ? __ldcg(split_flag + SGS_TRACK_HELPERS) : 0u;
     // the current frame's pixel: issued first, consumed after the forward walk
     float tr = 0.f, tg = 0.f, tb = 0.f, td = 0.f;
     if (inside) { tr = __ldg(trgb + pix); tg = __ldg(trgb + HW + pix); tb = __ldg(trgb + 2 * HW + pix); td = __ldg(tdepth + pix); }
@@ -289,7 +291,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     // does not write the sorted keys back in place (a helper scheduled late would rank a half-permuted bucket);
     // sgs_get_binning's export ranks short buckets itself (tilesort.cu, k_export_copy).
     float* st = split_state + (size_t)slot * (8 * SGS_BLOCK);  // g0..g3, T, last, zref (NDEPTH), one spare
-    const unsigned int epoch4 = split ? 4u * __ldcg(split_flag + SGS_TRACK_HELPERS) : 0u;
+    const unsigned int epoch4 = 4u * epoch_raw;
     volatile unsigned int* my_flag = reinterpret_cast<volatile unsigned int*>(split_flag + slot);
     if (crank == 1) {
         if (split) {
@@ -448,9 +450,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     // A tile bucket that overflowed (entries dropped) or a kept survivor list the device-resident pose has left (splats
     // possibly missing) must not pass for a result: the iteration's loss and pose gradient are NaN.  Under SGS_FLAG_GRAPH and
     // with SGS_FLAG_ASYNC nothing else tells the caller in time (the host sees the counters one call later, or never).
-    const bool invalid = *reinterpret_cast<volatile unsigned int*>(&counters->max_tile) > tile_cap ||
-                         *reinterpret_cast<volatile unsigned int*>(&counters->stale) != 0u;
-    if (!finish_pose(pose_partial, gridDim.x, counters, d_pose6, loss_out, invalid)) return;
+    if (!finish_pose(pose_partial, gridDim.x, counters, d_pose6, loss_out, tile_cap)) return;
     if (host_flag) {  // sgs_track_iter_host: d_pose6 / loss_out are pinned HOST memory; publish them before the housekeeping below
         if (tid < 7) __threadfence_system();
         __syncthreads();
@@ -465,7 +465,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         if (counters_snap) *counters_snap = *counters;  // what the host reads for overflow detection and hints
         counters->n_entries = 0ull; counters->n_visible = 0u; counters->overflow = 0u; counters->ticket_pre = 0u;
         counters->max_tile = 0u; counters->n_surv = 0u; counters->stale = 0u;
-        if (n_help > 0) split_flag[SGS_TRACK_HELPERS] += 1u;  // next launch's epoch: every block of this one is past its hand-over
+        if (n_help > 0) atomicAdd(split_flag + SGS_TRACK_HELPERS, 1u);  // next launch's epoch (every block of this one is past its hand-over); a RED: nothing waits for a load
     }
 }
 
