@@ -249,6 +249,32 @@ def test_invalid_arguments(ren):
     with pytest.raises(sgs.SgsError) as e:
         fresh.backward(d_pose6=torch.zeros(6, device="cuda"))
     assert e.value.status == sgs.SGS_NO_FORWARD_STATE
+    # the other documented refusals: a map of 2^24 or more splats (the tile keys hold 24 index bits), an image beyond 16384
+    # pixels on a side, non-finite pose entries, accumulate without gradient arrays, a window fetch / staging probe without
+    # the state they need
+    import ctypes as C
+    big = sgs.sgs_surfels()
+    C.memmove(C.byref(big), C.byref(sf), C.sizeof(big))
+    big.n = 1 << 24
+    cam_ok = sgs.make_camera(64, 48, 60, 60, 32, 24, np.eye(4)[:3])
+    for bad_sf, bad_cam in ((big, cam_ok), (sf, sgs.make_camera(20000, 48, 60, 60, 32, 24, np.eye(4)[:3])),
+                            (sf, sgs.make_camera(64, 48, 60, 60, 32, 24, np.full((3, 4), np.nan)))):
+        with pytest.raises(sgs.SgsError) as e:
+            fresh.render(bad_sf, bad_cam)
+        assert e.value.status == sgs.SGS_INVALID_ARGUMENT
+    fresh.render(sf, cam_ok)
+    with pytest.raises(sgs.SgsError) as e:
+        fresh.backward(d_pose6=torch.zeros(6, device="cuda"), accumulate=True)          # no gradient arrays to add to
+    assert e.value.status == sgs.SGS_INVALID_ARGUMENT
+    other = sgs.Renderer()
+    for call in (lambda: other.probe_staging(0), lambda: other.fetch_grads_host({"mean": torch.zeros(sc.n, 3).pin_memory()})):
+        with pytest.raises(sgs.SgsError) as e:
+            call()
+        assert e.value.status == sgs.SGS_NO_FORWARD_STATE
+    with pytest.raises(sgs.SgsError) as e:
+        other.probe_staging(2)
+    assert e.value.status == sgs.SGS_INVALID_ARGUMENT
+    other.close()
     fresh.close()
 
 
