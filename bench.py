@@ -159,6 +159,7 @@ class Workload:
     def __init__(self, name, iters_override=None, contrib=False, prefetch=True, reuse=True, normalised_depth=False, graph=False,
                  tight=False, radix=False, two_streams=False):
         self.contrib = contrib
+        self.dense_fetch = False
         self.graph, self.cg, self.eager_steps = graph, None, 0
         nd = self.normalised_depth = normalised_depth
         import torch
@@ -344,6 +345,9 @@ class Workload:
         self.h_targets = [(a.cpu().pin_memory(), b.cpu().pin_memory()) for a, b in self.targets]
         if not self.tracking:
             self.h_grads = [{k: torch.zeros(v.shape).pin_memory() for k, v in self.grads.items()} for _ in range(2)]
+            self.h_ids = [torch.zeros(self.sc.n, dtype=torch.int32).pin_memory() for _ in range(2)]
+            nw = (len(self.cams) + WINDOW - 1) // WINDOW
+            self.h_counts = [torch.zeros(1, dtype=torch.int64).pin_memory() for _ in range(nw)]
             self.h_p6 = [torch.zeros(6).pin_memory() for _ in self.cams]
             self.h_loss = [torch.zeros(1).pin_memory() for _ in self.cams]
 
@@ -351,7 +355,8 @@ class Workload:
         """Tracking: upload map + target frame, then `iters` x sgs_track_iter_host (loss + 6-vector read back
         every iteration).  Mapping: upload map; per view sgs_map_view_host (keyframe from the host; render, Eq. 24-26,
         full backward summed into the window on the device; loss + 6-vector back); per window of 5 views
-        sgs_fetch_grads_host (all N x 13 gradients back to the host); sgs_sync_host at the end of the step."""
+        sgs_fetch_grads_sparse_host (the rows of the surfels the window touched, ids + 13 floats each, written to the host
+        by the device; --dense-fetch: sgs_fetch_grads_host, all N x 13); sgs_sync_host at the end of the step."""
         r, h = self.ren, self.h
         r.upload_surfels(h["mean"], h["scale"], h["quat"], h["opacity"], h["rgb"], h["active"])
         if self.tracking:
@@ -363,7 +368,11 @@ class Workload:
         for v in range(nv):
             r.map_view_host(self.ccams[v], *self.h_targets[v], 0.875, 0.5, 0.02, 0.125, -1.0, self.h_loss[v], self.h_p6[v])
             if (v + 1) % WINDOW == 0 or v + 1 == nv:
-                r.fetch_grads_host(self.h_grads[(v // WINDOW) % 2])
+                w = v // WINDOW
+                if self.dense_fetch:
+                    r.fetch_grads_host(self.h_grads[w % 2])
+                else:
+                    r.fetch_grads_sparse_host(self.h_ids[w % 2], self.h_grads[w % 2], self.h_counts[w])
         r.sync_host()
         return float(self.h_loss[0][0])
 
@@ -374,7 +383,10 @@ class Workload:
             return h2d + px * 16 + self.iters * 48, self.iters * 28
         k = len(self.cams)
         windows = (k + WINDOW - 1) // WINDOW
-        return h2d + k * (px * 16 + 48), windows * n * 52 + k * 28
+        if self.dense_fetch:
+            return h2d + k * (px * 16 + 48), windows * n * 52 + k * 28
+        rows = sum(int(c.item()) for c in self.h_counts)    # counted from the last step's windows
+        return h2d + k * (px * 16 + 48), rows * 56 + windows * 8 + k * 28
 
 
 def cpu_baseline(sc, cams, name, samples=3):
@@ -518,6 +530,7 @@ def run_config(name, args, torch, dist, world, rank, local, peaks):
     # end to end through the HOST-buffer C-ABI calls
     e2e = None
     if not args.no_e2e:
+        wl.dense_fetch = args.dense_fetch
         wl.setup_e2e()
         wl.step_e2e()
         barrier()
@@ -546,6 +559,9 @@ def run_config(name, args, torch, dist, world, rank, local, peaks):
                            binning=("two contexts on two streams, views alternating; binning in line on each" if getattr(wl, "two_streams", False) else
                                     "sgs_prepare of view v+1 on a second context and a side stream, under view v's compositing"
                                     if len(wl.rens) > 1 else "in line (sgs_render / sgs_track_iter)")))
+    if not wl.tracking and e2e is not None:
+        e2e["gradients"] = ("all n x 13 floats per window (sgs_fetch_grads_host)" if args.dense_fetch else
+                            "rows of the surfels each window touched: ids + 13 floats (sgs_fetch_grads_sparse_host)")
     if not wl.tracking:
         out["config"]["gradients"] = f"summed over windows of {WINDOW} views (sgs_backward_accumulate), zeroed per window"
     if args.graph:
@@ -637,6 +653,7 @@ def main():
     ap.add_argument("--iters", type=int, default=None, help="override iterations per tracking step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--dense-fetch", action="store_true", help="e2e leg of the mapping configs: sgs_fetch_grads_host (all N x 13 floats per window) instead of the sparse hand-over")
     ap.add_argument("--no-reuse", action="store_true", help="tracking configs: run the pre-cull over the whole map every iteration")
     ap.add_argument("--no-prefetch", action="store_true", help="mapping configs: one context, binning of each view in line")
     ap.add_argument("--graph", action="store_true", help="SGS_FLAG_GRAPH: each step (a tracking frame, or a mapping window on one context) replayed as one CUDA graph")

@@ -356,6 +356,19 @@ SGS_API int sgs_map_view_host(sgs_ctx* ctx, const sgs_camera* cam, const float* 
                               float lambda_c, float w_d, float w_n, float ssim_weight, float normal_sign, float* host_loss,
                               float* host_pose6, void* cuda_stream);
 SGS_API int sgs_fetch_grads_host(sgs_ctx* ctx, const sgs_surfel_grads* host_d_surfels, void* cuda_stream);
+/* The same hand-over, sparse: a window only touches the surfels its views see (L248-252; in a 2 M-surfel map a view sees
+ * ~7 %), so instead of n dense rows the device delivers the rows that hold anything.  Row k < count of every non-NULL
+ * array of host_rows ({3,2,4,1,3} floats per row) is the accumulated gradient of surfel host_ids[k]; ids ascend; a surfel
+ * is listed iff at least one of its 13 accumulated values is not +-0 (NaN counts), so scattering the rows into zeros gives
+ * exactly what sgs_fetch_grads_host would have delivered, bit for bit.  host_ids and the arrays of host_rows (HOST, room
+ * for `cap` rows; pinned memory keeps the copies asynchronous) are written by copy commands that a LATER call of this
+ * group enqueues, once the device has packed the rows and published their number (sgs_map_view_host if the pack is
+ * complete by then, the next fetch, or sgs_sync_host): they must stay valid until sgs_sync_host, after which they and
+ * *host_count (HOST, nullable: the number of listed surfels) are complete.  If the count exceeds cap, only the first cap
+ * rows are delivered and the rest of the window is lost (cap = n can not overflow).  The accumulator is re-zeroed and the
+ * double buffer swapped as in sgs_fetch_grads_host; at most 64 fetches between two sgs_sync_host calls. */
+SGS_API int sgs_fetch_grads_sparse_host(sgs_ctx* ctx, int32_t* host_ids, const sgs_surfel_grads* host_rows, int64_t cap,
+                                        int64_t* host_count, void* cuda_stream);
 SGS_API int sgs_sync_host(sgs_ctx* ctx, void* cuda_stream);
 
 /* SSIM term of the colour loss (Eq. 24; reading R24): per channel the structural similarity index of [87],

@@ -59,7 +59,7 @@ class sgs_stats(C.Structure):
 EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_prepare", "sgs_backward", "sgs_wait_grads", "sgs_tracking_loss",
            "sgs_backward_tracking", "sgs_track_iter", "sgs_track_new_frame", "sgs_render_contrib", "sgs_render_median", "sgs_covisibility", "sgs_mapping_loss", "sgs_ssim_loss", "sgs_map_correction", "sgs_measure_fp32_peak", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
            "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string",
-           "sgs_track_iter_dev", "sgs_probe_staging", "sgs_backward_accumulate", "sgs_zero_grads", "sgs_map_view_host", "sgs_fetch_grads_host", "sgs_sync_host"]
+           "sgs_track_iter_dev", "sgs_probe_staging", "sgs_backward_accumulate", "sgs_zero_grads", "sgs_map_view_host", "sgs_fetch_grads_host", "sgs_sync_host", "sgs_fetch_grads_sparse_host"]
 
 _lib = None
 _LIVE = weakref.WeakSet()
@@ -279,6 +279,18 @@ class Renderer:
         self._win_keep.append(grads)
         g = self._grads(grads, "cpu")
         _check(self.lib.sgs_fetch_grads_host(self._ctx, C.byref(g), _stream_ptr(stream)), "sgs_fetch_grads_host")
+
+    def fetch_grads_sparse_host(self, ids, rows, count, stream=None):
+        """sgs_fetch_grads_sparse_host: ends the window; rows [0, count) of the PINNED host tensors in `rows` (dict like
+        grads) hold the gradients of surfels ids[0..count) (int32, ascending); count: HOST int64 tensor of one element.
+        All complete after sync_host()."""
+        self._win_keep = getattr(self, "_win_keep", [])
+        self._win_keep.append((ids, rows, count))
+        g = self._grads(rows, "cpu")
+        cap = min([ids.shape[0]] + [v.shape[0] for v in rows.values() if v is not None])
+        _check(self.lib.sgs_fetch_grads_sparse_host(self._ctx, _ptr(ids, torch.int32, "cpu"), C.byref(g), C.c_int64(cap),
+                                                    _ptr(count, torch.int64, "cpu"), _stream_ptr(stream)),
+               "sgs_fetch_grads_sparse_host")
 
     def sync_host(self, stream=None):
         _check(self.lib.sgs_sync_host(self._ctx, _stream_ptr(stream)), "sgs_sync_host")

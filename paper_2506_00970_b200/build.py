@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libsgs.so")
 OBJ = os.path.join(HERE, "build")
-SOURCES = ["api.cu", "api_run.cu", "api_host.cu", "preprocess.cu", "sort.cu", "tilesort.cu", "forward.cu", "backward.cu", "track.cu", "loss.cu", "ssim.cu", "probe.cu"]
+SOURCES = ["api.cu", "api_run.cu", "api_host.cu", "preprocess.cu", "sort.cu", "tilesort.cu", "forward.cu", "backward.cu", "track.cu", "loss.cu", "ssim.cu", "probe.cu", "window.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC,-fvisibility=hidden", "--use-local-env"]
 

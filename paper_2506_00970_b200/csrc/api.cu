@@ -259,7 +259,7 @@ int sgs_destroy(sgs_ctx* c) {
     void* ptrs[] = {c->scan_state, c->vis_to_surfel, c->vis_list, c->culled, c->pay.store, c->acc, c->keys[0], c->keys[1], c->vals[0], c->vals[1], c->idx_export,
                     c->sort_state, c->ranges, c->T_final, c->n_last, c->dn_state, c->img_scratch, c->pose_partial, c->resident_store,
                     c->resident_active, c->target_rgb, c->host_img_dev, c->host_up_dev, c->host_grads_dev,
-                    c->win_grads[0], c->win_grads[1], c->win_tgt[0], c->win_tgt[1], c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->pose_inc, c->ssim_maps, c->surv_cnt, c->surv_in, c->export_keys, c->export_ranges};
+                    c->win_grads[0], c->win_grads[1], c->win_tgt[0], c->win_tgt[1], c->win_scratch, c->win_stage, c->bucket, c->cursor, c->tile_order, c->render_order, c->tile_cost, c->pose_inc, c->ssim_maps, c->surv_cnt, c->surv_in, c->export_keys, c->export_ranges};
     for (void* p : ptrs) sgs_ws_free(c, p, s);
     if (c->counters) cudaFree(c->counters);
     if (c->counters_snap) cudaFree(c->counters_snap);
@@ -291,6 +291,8 @@ int sgs_destroy(sgs_ctx* c) {
     if (c->win_drained[0]) cudaEventDestroy(c->win_drained[0]);
     if (c->win_drained[1]) cudaEventDestroy(c->win_drained[1]);
     if (c->win_results) cudaFreeHost(c->win_results);
+    if (c->win_counts) cudaFreeHost(c->win_counts);
+    if (c->win_packed) cudaEventDestroy(c->win_packed);
     for (int i = 0; i < 2 * c->prof_cap; ++i) cudaEventDestroy(c->prof_ev[i]);
     free(c->prof_ev); free(c->prof_stage);
     delete c;

@@ -24,6 +24,35 @@ static void dev_images(float* base, int64_t pixels, sgs_images* im) {
     im->rgb = base; im->depth = base + 3 * pixels; im->normal = base + 4 * pixels; im->alpha = base + 7 * pixels;
 }
 
+// sgs_fetch_grads_sparse_host, second half: once the pack kernel of the last sparse fetch has run, the row count sits in
+// mapped memory and the copy commands of exactly that many rows can be enqueued (on the ctx's copy stream, behind the pack).
+// wait == false: only if the pack is already complete (called from the window calls that follow the fetch).
+static int flush_sparse(sgs_ctx* c, bool wait) {
+    if (!c->win_sp.pending) return SGS_OK;
+    if (!wait) {
+        const cudaError_t q = cudaEventQuery(c->win_packed);
+        if (q == cudaErrorNotReady) return SGS_OK;
+        if (q != cudaSuccess) return SGS_CUDA_ERROR;
+    } else if (cudaEventSynchronize(c->win_packed) != cudaSuccess) return SGS_CUDA_ERROR;
+    c->win_sp.pending = false;
+    const int64_t n = c->win_sp.n;
+    int64_t rows = (int64_t)c->win_counts[c->win_sp.ring];
+    if (rows > c->win_sp.cap) rows = c->win_sp.cap;
+    if (rows <= 0) return SGS_OK;
+    const float* st = reinterpret_cast<const float*>(c->win_stage);
+    cudaStream_t cs = c->copy_stream;
+    const sgs_surfel_grads& h = c->win_sp.rows;
+    const size_t r4 = sizeof(float) * (size_t)rows;
+    bool ok = true;
+    if (c->win_sp.ids) ok = ok && cudaMemcpyAsync(c->win_sp.ids, st, r4, cudaMemcpyDeviceToHost, cs) == cudaSuccess;
+    if (h.mean) ok = ok && cudaMemcpyAsync(h.mean, st + n, 3 * r4, cudaMemcpyDeviceToHost, cs) == cudaSuccess;
+    if (h.scale) ok = ok && cudaMemcpyAsync(h.scale, st + 4 * n, 2 * r4, cudaMemcpyDeviceToHost, cs) == cudaSuccess;
+    if (h.quat) ok = ok && cudaMemcpyAsync(h.quat, st + 6 * n, 4 * r4, cudaMemcpyDeviceToHost, cs) == cudaSuccess;
+    if (h.opacity) ok = ok && cudaMemcpyAsync(h.opacity, st + 10 * n, r4, cudaMemcpyDeviceToHost, cs) == cudaSuccess;
+    if (h.rgb) ok = ok && cudaMemcpyAsync(h.rgb, st + 11 * n, 3 * r4, cudaMemcpyDeviceToHost, cs) == cudaSuccess;
+    return ok ? SGS_OK : SGS_CUDA_ERROR;
+}
+
 extern "C" {
 
 int sgs_upload_surfels(sgs_ctx* c, const sgs_surfels* h, void* stream) {
@@ -170,6 +199,9 @@ static int window_setup(sgs_ctx* c, int64_t n, cudaStream_t s) {
             cudaEventCreateWithFlags(&c->win_drained[1], cudaEventDisableTiming) != cudaSuccess ||
             cudaHostAlloc(&c->win_results, sizeof(float) * 8 * SGS_WIN_RING, cudaHostAllocMapped) != cudaSuccess ||
             cudaHostGetDevicePointer(&c->win_results_dev, c->win_results, 0) != cudaSuccess ||
+            cudaHostAlloc(&c->win_counts, sizeof(uint32_t) * SGS_WIN_RING, cudaHostAllocMapped) != cudaSuccess ||
+            cudaHostGetDevicePointer(&c->win_counts_dev, c->win_counts, 0) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->win_packed, cudaEventDisableTiming) != cudaSuccess ||
             cudaStreamCreateWithFlags(&c->in_stream, cudaStreamNonBlocking) != cudaSuccess ||
             cudaEventCreateWithFlags(&c->win_tgt_ready[0], cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&c->win_tgt_ready[1], cudaEventDisableTiming) != cudaSuccess ||
@@ -201,6 +233,7 @@ int sgs_map_view_host(sgs_ctx* c, const sgs_camera* cam, const float* h_rgb, con
     int r = ensure_host_images(c, px, s);
     if (r != SGS_OK) return r;
     if ((r = window_setup(c, n, s)) != SGS_OK) return r;
+    if ((r = flush_sparse(c, false)) != SGS_OK) return r;
     // keyframe: host -> one of two device buffers on the ctx's upload stream (runs under the previous view's kernels; the
     // buffer's previous user, two views ago, has recorded win_tgt_free behind its last reader)
     const int ts = c->win_tgt_slot;
@@ -243,12 +276,13 @@ int sgs_map_view_host(sgs_ctx* c, const sgs_camera* cam, const float* h_rgb, con
     c->win_pending[c->win_n_pending].loss = h_loss;
     c->win_pending[c->win_n_pending].pose6 = h_pose6;
     c->win_n_pending += 1;
-    return SGS_OK;
+    return flush_sparse(c, false);
 }
 
 int sgs_fetch_grads_host(sgs_ctx* c, const sgs_surfel_grads* hg, void* stream) {
     if (!c || !hg) return SGS_INVALID_ARGUMENT;
     if (!c->copy_stream || !c->win_grads[c->win_slot]) return SGS_NO_FORWARD_STATE;
+    if (flush_sparse(c, true) != SGS_OK) return SGS_CUDA_ERROR;
     cudaStream_t s = (cudaStream_t)stream, cs = c->copy_stream;
     const int64_t n = c->resident.n;
     const int slot = c->win_slot;
@@ -269,8 +303,37 @@ int sgs_fetch_grads_host(sgs_ctx* c, const sgs_surfel_grads* hg, void* stream) {
     return SGS_OK;
 }
 
+int sgs_fetch_grads_sparse_host(sgs_ctx* c, int32_t* h_ids, const sgs_surfel_grads* hg, int64_t cap, int64_t* h_count,
+                                void* stream) {
+    if (!c || !hg || cap < 0) return SGS_INVALID_ARGUMENT;
+    if (!c->copy_stream || !c->win_grads[c->win_slot]) return SGS_NO_FORWARD_STATE;
+    if (c->win_n_cnt_pending >= SGS_WIN_RING) return SGS_INVALID_ARGUMENT;  // call sgs_sync_host first
+    cudaStream_t s = (cudaStream_t)stream, cs = c->copy_stream;
+    const int64_t n = c->resident.n;
+    const int slot = c->win_slot;
+    int r = flush_sparse(c, true);   // the previous fetch's rows leave the staging buffer first (its pack ran a window ago)
+    if (r != SGS_OK) return r;
+    if (!grow(c, c->win_scratch, c->win_scratch_cap, sgs_window_scratch_words(n), cs) ||
+        !grow(c, c->win_stage, c->win_stage_cap, sgs_window_stage_words(n), cs))
+        return SGS_OUT_OF_MEMORY;
+    const int k = c->win_n_cnt_pending;
+    c->win_counts[k] = 0;
+    bool ok = cudaEventRecord(c->win_filled, s) == cudaSuccess && cudaStreamWaitEvent(cs, c->win_filled, 0) == cudaSuccess &&
+              sgs_launch_window_compact(c, c->win_grads[slot], n, c->win_scratch, c->win_stage, c->win_counts_dev + k, cs) == cudaSuccess &&
+              cudaEventRecord(c->win_packed, cs) == cudaSuccess && cudaEventRecord(c->win_drained[slot], cs) == cudaSuccess;
+    if (!ok) return SGS_CUDA_ERROR;
+    c->win_sp.pending = true; c->win_sp.ring = k; c->win_sp.n = n; c->win_sp.cap = cap; c->win_sp.ids = h_ids; c->win_sp.rows = *hg;
+    c->win_cnt_pending[k] = h_count;
+    c->win_n_cnt_pending = k + 1;
+    c->win_draining[slot] = true;
+    c->win_slot ^= 1;
+    c->win_dirty = false;
+    return SGS_OK;
+}
+
 int sgs_sync_host(sgs_ctx* c, void* stream) {
     if (!c) return SGS_INVALID_ARGUMENT;
+    if (flush_sparse(c, true) != SGS_OK) return SGS_CUDA_ERROR;
     if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return SGS_CUDA_ERROR;
     if (c->copy_stream && cudaStreamSynchronize(c->copy_stream) != cudaSuccess) return SGS_CUDA_ERROR;
     if (c->in_stream && cudaStreamSynchronize(c->in_stream) != cudaSuccess) return SGS_CUDA_ERROR;
@@ -282,6 +345,9 @@ int sgs_sync_host(sgs_ctx* c, void* stream) {
         if (c->win_pending[k].pose6) memcpy(c->win_pending[k].pose6, res + 1, sizeof(float) * 6);
     }
     c->win_n_pending = 0;
+    for (int k = 0; k < c->win_n_cnt_pending; ++k)
+        if (c->win_cnt_pending[k]) *c->win_cnt_pending[k] = (int64_t)c->win_counts[k];
+    c->win_n_cnt_pending = 0;
     return SGS_OK;
 }
 

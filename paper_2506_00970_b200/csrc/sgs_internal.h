@@ -193,6 +193,12 @@ struct sgs_ctx {
     cudaStream_t in_stream; float* win_tgt[2]; int64_t win_tgt_cap[2]; int win_tgt_slot;
     cudaEvent_t win_tgt_ready[2], win_tgt_free[2]; bool win_tgt_used[2];
     struct { float* loss; float* pose6; } win_pending[64]; int win_n_pending;
+    // sgs_fetch_grads_sparse_host (window.cu): compaction scratch, row staging, a mapped ring of row counts; the copy-out of
+    // the last fetch is enqueued by the first window call that finds its pack complete (win_sp: what it has to deliver)
+    uint32_t* win_scratch; int64_t win_scratch_cap; uint32_t* win_stage; int64_t win_stage_cap;
+    uint32_t* win_counts; uint32_t* win_counts_dev; cudaEvent_t win_packed;
+    struct { bool pending; int ring; int64_t n, cap; int32_t* ids; sgs_surfel_grads rows; } win_sp;
+    int64_t* win_cnt_pending[64]; int win_n_cnt_pending;
     int64_t partial_cap;             // floats in pose_partial
     int64_t launches;                // kernels launched by this ctx
     int prof_on; int prof_n, prof_cap; cudaEvent_t* prof_ev; int* prof_stage;  // event pairs: ev[2i], ev[2i+1]
@@ -240,6 +246,10 @@ cudaError_t sgs_launch_export_bucket(sgs_ctx* c, int64_t n_entries, cudaStream_t
 int sgs_ensure_buckets(sgs_ctx* c, int tiles, int64_t tile_cap, cudaStream_t s);
 int sgs_ensure_export(sgs_ctx* c, int tiles, int64_t entries, cudaStream_t s);
 
+int64_t sgs_window_scratch_words(int64_t n);
+int64_t sgs_window_stage_words(int64_t n);
+cudaError_t sgs_launch_window_compact(sgs_ctx* c, float* acc, int64_t n, uint32_t* scratch, uint32_t* stage, uint32_t* count_mapped,
+                                      cudaStream_t s);
 cudaError_t sgs_launch_publish(void* dst_mapped, const void* src, int words, cudaStream_t s);  // <= 1024 words
 
 // ---- workspace helpers (api.cu) ----

@@ -2,6 +2,8 @@
 views): sgs_backward_accumulate against the SUM of the oracle's per-view gradients, element by element (each view
 contributes its own strict bar and its own fragile-pixel exposure to the bound), and the HOST-buffer window calls
 (sgs_map_view_host / sgs_fetch_grads_host / sgs_sync_host) against the device-buffer sequence they wrap."""
+import ctypes
+
 import numpy as np
 import pytest
 import torch
@@ -126,3 +128,67 @@ def test_host_window_calls_equal_the_device_sequence():
             assert abs(float(hl[3 * w + v].item()) - L) <= 1e-5 * abs(L) and L > 0
             np.testing.assert_allclose(hp[3 * w + v].numpy(), p, rtol=1e-4, atol=1e-5 * np.abs(p).max())
     dev.close(); host.close()
+
+
+def test_sparse_window_fetch_delivers_exactly_the_touched_rows():
+    """sgs_fetch_grads_sparse_host against sgs_fetch_grads_host on the same views: two windows in a row (both accumulators,
+    the re-zeroing behind the read), the map padded with surfels behind the camera so that most rows stay zero.  The listed
+    ids ascend, are exactly the rows the dense fetch has non-zero, and carry its values (the two runs differ by the order
+    of the atomic adds inside a view only); the rows past `count` are not written.  The second window's arrays are pageable memory."""
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    H, W = cam.height, cam.width
+    n0, pad = sc.n, 3000                       # ragged against the 1024-surfel blocks and the 32-surfel flag words
+    back = np.linalg.inv(np.vstack([cam.T_cw[:3], [0, 0, 0, 1]]))[:3] @ np.array([0.0, 0.0, -2.0, 1.0])
+    mean = np.vstack([np.tile(back, (pad // 2, 1)), sc.mean, np.tile(back, (pad - pad // 2, 1))])
+    rep = lambda a: np.concatenate([np.repeat(a[:1], pad // 2, 0), a, np.repeat(a[:1], pad - pad // 2, 0)])
+    n = n0 + pad
+    pin = lambda x, dt=torch.float32: torch.from_numpy(np.ascontiguousarray(x)).to(dt).pin_memory()
+    taus = [None, [0.05, 0.02, -0.04, 0.1, -0.05, 0.2], [-0.1, 0.05, 0.02, -0.2, 0.1, 0.05]]
+    cs = [camera(cam, None if tau is None else scenegen.perturb_pose(cam.T_cw, tau)) for tau in taus]
+    g0 = scenegen.SplitMix(78)
+    tgts = [(pin(g0.uniform(3 * H * W).reshape(3, H, W)), pin((1.5 + g0.uniform(H * W)).reshape(1, H, W))) for _ in range(6)]
+    shapes = dict(mean=3, scale=2, quat=4, opacity=1, rgb=3)
+    res = {}
+    for mode in ("dense", "sparse"):
+        ren = sgs.Renderer()
+        ren.upload_surfels(pin(mean), pin(rep(sc.scale)), pin(rep(sc.quat)), pin(rep(sc.opacity)), pin(rep(sc.rgb)))
+        out = []
+        for w in range(2):
+            for v in range(3):
+                ren.map_view_host(cs[v], *tgts[3 * w + v], 0.875, 0.5, 0.02, 0.125, -1.0)
+            if mode == "dense":
+                hg = {k: torch.full((n, d), 9.0).pin_memory() for k, d in shapes.items()}
+                ren.fetch_grads_host(hg)
+                out.append(hg)
+            else:
+                pm = (lambda x: x.pin_memory()) if w == 0 else (lambda x: x)
+                rows = {k: pm(torch.full((n, d), 9.0)) for k, d in shapes.items()}
+                ids, cnt = pm(torch.full((n,), -7, dtype=torch.int32)), torch.full((1,), -1, dtype=torch.int64).pin_memory()
+                ren.fetch_grads_sparse_host(ids, rows, cnt)
+                out.append((ids, rows, cnt))
+        ren.sync_host()
+        res[mode] = out
+        if mode == "sparse":   # a third, empty window: nothing is listed (the accumulator was zeroed behind the reads)
+            ids, cnt = torch.full((n,), -7, dtype=torch.int32).pin_memory(), torch.full((1,), -1, dtype=torch.int64).pin_memory()
+            rows = {k: torch.full((n, d), 9.0).pin_memory() for k, d in shapes.items()}
+            ren.fetch_grads_sparse_host(ids, rows, cnt); ren.fetch_grads_sparse_host(ids, rows, cnt)
+            ren.sync_host()
+            assert int(cnt.item()) == 0 and (ids.numpy() == -7).all() and all((r.numpy() == 9.0).all() for r in rows.values())
+            assert ren.lib.sgs_fetch_grads_sparse_host(ren._ctx, None, None, ctypes.c_int64(-1), None, None) == sgs.SGS_INVALID_ARGUMENT
+        ren.close()
+    for w in range(2):
+        dense = {k: v.numpy() for k, v in res["dense"][w].items()}
+        ids, rows, cnt = res["sparse"][w]
+        k = int(cnt.item())
+        i = ids.numpy()[:k].astype(np.int64)
+        nz = np.zeros(n, bool)
+        for a in dense.values():
+            nz |= (a != 0).any(axis=1)
+        assert 0 < k < n0 + 1 and (np.diff(i) > 0).all() and i.min() >= pad // 2 and i.max() < pad // 2 + n0
+        assert np.array_equal(i, np.nonzero(nz)[0])
+        assert (ids.numpy()[k:] == -7).all()
+        for name, a in dense.items():
+            r = rows[name].numpy()
+            assert (r[k:] == 9.0).all()
+            np.testing.assert_allclose(r[:k], a[i], rtol=2e-4, atol=1e-5 * np.abs(a).max())
