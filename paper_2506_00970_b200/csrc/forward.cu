@@ -8,6 +8,7 @@
 // saturated; the block stops fetching batches when every pixel is.
 #include "pair.cuh"
 #include "regsort.cuh"
+#include "histsort.cuh"
 #include "sgs_internal.h"
 
 namespace {
@@ -23,7 +24,7 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
           float* __restrict__ median_out) {
     // staged batch, structure of float4 arrays (one base register, immediate offsets, broadcast reads)
     __shared__ float4 sh[LOWPASS ? 6 : 5][SGS_BLOCK];   // (R28: plane 5 = pixel-minus-centre offsets of the tile's first pixel)
-    __shared__ unsigned char sh_mask[SGS_BLOCK];
+    __shared__ __align__(16) unsigned char sh_mask[SGS_BLOCK];
     const uint32_t sa = smem_addr(&sh[0][0]), sm_a = smem_addr(sh_mask);
     constexpr uint32_t PL = SGS_BLOCK * 16;  // bytes per staged plane
     const int tile = tile_order ? (int)tile_order[blockIdx.x] : (int)blockIdx.x;  // longest tiles first
@@ -45,7 +46,12 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
         if (tid == 0) { ranges[2 * tile] = start; ranges[2 * tile + 1] = end; }
         unsigned long long* g = bucket + (size_t)start;
         unsigned long long* sk = reinterpret_cast<unsigned long long*>(&sh[0][0]);
-        if (n >= 2 && n <= 512) {   // keys in registers: shuffles + a few shared-memory exchanges (regsort.cuh)
+        // more than 128 keys: counting pass over the depth + rank inside each depth bin (histsort.cuh; linear in n); it declines
+        // buckets whose depths crowd into one bin, which take the networks below like the short ones
+        static_assert(sizeof(sh) >= 2048 * 8 + HS_SCRATCH_WORDS * 4 && SGS_BLOCK >= 32 * 4 && HS_BINS == 4 * SGS_BLOCK, "");
+        const bool sorted = n > 128 && hist_sort_keys(g, n, sk, reinterpret_cast<uint32_t*>(sk + 2048), reinterpret_cast<uint32_t*>(sh_mask), tid);
+        if (sorted) {
+        } else if (n >= 2 && n <= 512) {   // keys in registers: shuffles + a few shared-memory exchanges (regsort.cuh)
             uint32_t npad = 32;
             while (npad < n) npad <<= 1;
             if (n <= 256) {
