@@ -412,6 +412,35 @@ def test_tile_bucket_overflow_grows(ren):
     b.close()
 
 
+@pytest.mark.parametrize("crowded", [False, True])
+def test_fused_sort_of_long_buckets(ren, crowded):
+    """Buckets of 129..2048 keys take the counting sort of histsort.cuh inside k_forward; a bucket whose depths crowd into
+    one bin (here 400 splats at exactly the same depth beside a wide depth range) is declined by it and takes the bitonic
+    networks.  Either way the exported lists equal the oracle's bit for bit and the images meet the image bar."""
+    g = scenegen.SplitMix(11)
+    n = 1500
+    z = g.uniform(n, 1.0, 3.0)
+    if crowded:
+        z[:400] = 2.0
+    x = g.uniform(n, -0.02, 0.02)
+    x[1100:] += 0.35 * z[1100:]               # 400 of them project 21 px to the right: a tile of their own
+    mean = np.stack([x, g.uniform(n, -0.02, 0.02), z], 1).astype(np.float32)
+    sc = Scene(mean, np.full((n, 2), 0.01, np.float32), np.tile(np.float32([1, 0, 0, 0]), (n, 1)),
+               np.full(n, 0.05, np.float32), np.full((n, 3), 0.5, np.float32))
+    cam = Camera(64, 48, 60.0, 60.0, 32.0, 24.0)
+    camv, cfg = oracle.make_cam(cam), oracle.make_cfg()
+    ob = oracle.binning(sc, camv, cfg)
+    ln = ob["ranges"][:, 1] - ob["ranges"][:, 0]
+    assert ln.max() <= 2048 and (ln > 512).any() and ((ln > 128) & (ln <= 512)).any()
+    if crowded:   # the 400 equal depths share a tile: more than HS_MAX_BIN = 96 keys in one depth bin
+        s0, e0 = ob["ranges"][int(np.argmax(ln))]
+        d = ob["keys"][s0:e0] & 0xffffffff
+        assert np.bincount((d - d.min()).astype(np.int64) >> max(0, int(d.max() - d.min()).bit_length() - 10)).max() > 96
+    out = run_gpu(ren, sc, cam)
+    assert_binning(out["bin"], ob)
+    assert_images(out["img"], oracle.render(sc, camv, cfg), sc, camv, cfg)
+
+
 def test_track_iter_matches_unfused_sequence():
     """sgs_track_iter == sgs_render + sgs_backward_tracking on C1 (short lists) and on a tile list longer than one
     256-entry batch and longer than the in-kernel sort bound (bucket regrowth -> pre-sorted path)."""
