@@ -56,7 +56,8 @@ enum {
     SGS_OUT_OF_MEMORY = 2,
     SGS_WORKSPACE_OVERFLOW = 3, /* async mode: the previous render overflowed; workspace was grown, render again */
     SGS_NO_FORWARD_STATE = 4,   /* sgs_backward without a preceding successful sgs_render */
-    SGS_CUDA_ERROR = 5
+    SGS_CUDA_ERROR = 5,
+    SGS_LIMIT_EXCEEDED = 6      /* sgs_map_correction_static: more keyframes than SGS_STATIC_MAX_FRAMES */
 };
 
 enum {
@@ -391,6 +392,21 @@ SGS_API int sgs_ssim_loss(sgs_ctx* ctx, int width, int height, const float* rend
  *   splat untouched), T_orig / T_opt (n_frames x 12, row-major 3x4 [R|t] of T_f and T_f^o): all DEVICE. */
 SGS_API int sgs_map_correction(sgs_ctx* ctx, int64_t n, float* mean, float* quat, const int32_t* frame_id, int n_frames,
                                const float* T_orig, const float* T_opt, void* cuda_stream);
+
+/* The same operation for callers that must not allocate (code under CUDA stream capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): no ctx, and NO cudaMalloc / cudaFree / allocating library call on any path.  The per-keyframe
+ * increments Delta T_f (64 bytes each), which sgs_map_correction keeps in the ctx's workspace, live in a static device
+ * array of SGS_STATIC_MAX_FRAMES entries (256 KB that every GPU loading the library holds until the process exits).
+ *   Arguments, layout and arithmetic as sgs_map_correction (same kernels: the results are bit-identical); all DEVICE.
+ *   n_frames > SGS_STATIC_MAX_FRAMES returns SGS_LIMIT_EXCEEDED and touches nothing; other errors as sgs_map_correction.
+ *   The array is shared by every call in the process on that device: each call rewrites the entries [0, n_frames) it
+ *   reads before reading them, so nothing needs clearing and an earlier call's contents are never seen -- but two calls
+ *   that OVERLAP on the GPU (different streams without an ordering between them) race on it: order them.
+ *   The first call on a device looks the array's address up (cudaGetSymbolAddress; not an allocation): make one call
+ *   outside stream capture before capturing. */
+#define SGS_STATIC_MAX_FRAMES 4096
+SGS_API int sgs_map_correction_static(int64_t n, float* mean, float* quat, const int32_t* frame_id, int n_frames,
+                                      const float* T_orig, const float* T_opt, void* cuda_stream);
 
 /* Measures this device's FP32 FMA throughput with a register-resident loop (16 independent chains per thread,
  * 8 blocks of 256 threads per SM, best of 4 timed launches, ~1 ms each; waits): the denominator of the compositing

@@ -12,7 +12,8 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libsgs.so")
 
-SGS_OK, SGS_INVALID_ARGUMENT, SGS_OUT_OF_MEMORY, SGS_WORKSPACE_OVERFLOW, SGS_NO_FORWARD_STATE, SGS_CUDA_ERROR = range(6)
+SGS_OK, SGS_INVALID_ARGUMENT, SGS_OUT_OF_MEMORY, SGS_WORKSPACE_OVERFLOW, SGS_NO_FORWARD_STATE, SGS_CUDA_ERROR, SGS_LIMIT_EXCEEDED = range(7)
+SGS_STATIC_MAX_FRAMES = 4096
 SGS_FLAG_ASYNC = 1
 SGS_FLAG_RADIX_BINNING = 2
 SGS_FLAG_TRACK_REUSE = 4
@@ -59,7 +60,7 @@ class sgs_stats(C.Structure):
 EXPORTS = ["sgs_default_config", "sgs_create", "sgs_destroy", "sgs_render", "sgs_prepare", "sgs_backward", "sgs_wait_grads", "sgs_tracking_loss",
            "sgs_backward_tracking", "sgs_track_iter", "sgs_track_new_frame", "sgs_render_contrib", "sgs_render_median", "sgs_covisibility", "sgs_mapping_loss", "sgs_ssim_loss", "sgs_map_correction", "sgs_measure_fp32_peak", "sgs_get_binning", "sgs_get_stats", "sgs_upload_surfels", "sgs_render_host", "sgs_backward_host",
            "sgs_upload_target", "sgs_track_iter_host", "sgs_set_profiling", "sgs_get_profile", "sgs_status_string",
-           "sgs_track_iter_dev", "sgs_probe_staging", "sgs_backward_accumulate", "sgs_zero_grads", "sgs_map_view_host", "sgs_fetch_grads_host", "sgs_sync_host", "sgs_fetch_grads_sparse_host"]
+           "sgs_track_iter_dev", "sgs_probe_staging", "sgs_backward_accumulate", "sgs_zero_grads", "sgs_map_view_host", "sgs_fetch_grads_host", "sgs_sync_host", "sgs_fetch_grads_sparse_host", "sgs_map_correction_static"]
 
 _lib = None
 _LIVE = weakref.WeakSet()
@@ -134,6 +135,17 @@ def measure_fp32_peak(stream=None):
     out = C.c_double(0.0)
     _check(load_library().sgs_measure_fp32_peak(C.byref(out), _stream_ptr(stream)), "sgs_measure_fp32_peak")
     return float(out.value)
+
+
+def map_correction_static(mean, quat, frame_id, T_orig, T_opt, stream=None):
+    """sgs_map_correction_static: sgs_map_correction (Eq. 31-32, in place) without a ctx and without any allocation; the
+    keyframe increments sit in a static device array of SGS_STATIC_MAX_FRAMES entries (SgsError SGS_LIMIT_EXCEEDED beyond).
+    Calls that overlap on the GPU race on that array."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2506_00970_b200 needs a CUDA device; there is no CPU fallback")
+    _check(load_library().sgs_map_correction_static(C.c_int64(mean.shape[0]), _ptr(mean), _ptr(quat), _ptr(frame_id, torch.int32),
+                                                    C.c_int(T_orig.shape[0]), _ptr(T_orig), _ptr(T_opt), _stream_ptr(stream)),
+           "sgs_map_correction_static")
 
 
 class Renderer:

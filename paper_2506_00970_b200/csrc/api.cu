@@ -327,6 +327,7 @@ const char* sgs_status_string(int status) {
         case SGS_WORKSPACE_OVERFLOW: return "workspace overflow: the previous render dropped tile entries; render again";
         case SGS_NO_FORWARD_STATE: return "no forward state: call sgs_render first";
         case SGS_CUDA_ERROR: return "CUDA error";
+        case SGS_LIMIT_EXCEEDED: return "size beyond the static scratch limit (sgs_map_correction_static: n_frames > SGS_STATIC_MAX_FRAMES = 4096)";
         default: return "unknown status";
     }
 }

@@ -3,6 +3,7 @@
 // pose-only backward.  Element-wise, HBM-bound (reads 8+4 planes, writes 8 planes).
 //   L_I = |I_r - I|_1 (Eq. 15), L_D = |D_r - D| (Eq. 16), M_n = [sign * N_r . r > 0] (Eq. 17, R19),
 //   M_o = [O > 0.95] (Eq. 18), L_t = mean(M_n M_o (L_I + lambda_d L_D)) (Eq. 19).
+#include <mutex>
 #include "sgs_internal.h"
 
 namespace {
@@ -366,4 +367,52 @@ cudaError_t sgs_launch_map_correction(sgs_ctx* c, int64_t n, float* mean, float*
     k_pose_increments<<<(n_frames + 127) / 128, 128, 0, s>>>(n_frames, T_orig, T_opt, reinterpret_cast<float4*>(c->pose_inc));
     k_map_correction<<<blocks, 256, 0, s>>>((long long)n, mean, quat, frame_id, n_frames, reinterpret_cast<const float4*>(c->pose_inc));
     return cudaGetLastError();
+}
+
+// ---- sgs_map_correction_static: the same two kernels with NO allocation anywhere (include/sgs.h) ----
+// For callers that can not call cudaMalloc (stream capture, serving loops, harnesses that forbid it): the per-keyframe
+// increments (64 B each) live in a file-scope device array instead of the ctx's workspace.  Every GPU that loads the
+// library holds SGS_STATIC_MAX_FRAMES x 64 B = 256 KB of it until the process exits.
+// g_pose_inc_static is, in HOST code, only a stand-in for the symbol: its device address is fetched per device with
+// cudaGetSymbolAddress (below) and that pointer is what the kernels get.
+static __device__ __align__(256) float4 g_pose_inc_static[4 * SGS_STATIC_MAX_FRAMES];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+float4* g_static_ptr[STATIC_MAX_DEVICES];          // device address of g_pose_inc_static on device d, nullptr = not fetched yet
+std::mutex g_static_mutex;
+
+// set-up, once per device, with that device current
+int static_scratch(float4** out) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= STATIC_MAX_DEVICES) return SGS_CUDA_ERROR;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        float4* p = nullptr;
+        if (cudaGetSymbolAddress((void**)&p, g_pose_inc_static) != cudaSuccess || !p) { cudaGetLastError(); return SGS_CUDA_ERROR; }
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return SGS_OK;
+}
+}  // namespace
+
+extern "C" int sgs_map_correction_static(int64_t n, float* mean, float* quat, const int32_t* frame_id, int n_frames,
+                                                 const float* T_orig, const float* T_opt, void* stream) {
+    if (n < 0 || n_frames < 0) return SGS_INVALID_ARGUMENT;
+    if (n_frames > SGS_STATIC_MAX_FRAMES) return SGS_LIMIT_EXCEEDED;
+    if (n > 0 && (!mean || !quat || !frame_id || (n_frames > 0 && (!T_orig || !T_opt)))) return SGS_INVALID_ARGUMENT;
+    if (reinterpret_cast<uintptr_t>(quat) & 15u) return SGS_INVALID_ARGUMENT;
+    if (n == 0 || n_frames == 0) return SGS_OK;
+    float4* inc = nullptr;
+    const int r = static_scratch(&inc);
+    if (r != SGS_OK) return r;
+    cudaStream_t s = (cudaStream_t)stream;
+    int blocks = (int)((n + 255) / 256);
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    // entries [0, n_frames) of the array are rewritten by the first kernel before the second reads them (and it reads no
+    // others): nothing has to start at zero, and what an earlier call left behind is never seen
+    k_pose_increments<<<(n_frames + 127) / 128, 128, 0, s>>>(n_frames, T_orig, T_opt, inc);
+    k_map_correction<<<blocks, 256, 0, s>>>((long long)n, mean, quat, frame_id, n_frames, inc);
+    return cudaGetLastError() == cudaSuccess ? SGS_OK : SGS_CUDA_ERROR;
 }
