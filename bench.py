@@ -160,6 +160,7 @@ class Workload:
                  tight=False, radix=False, two_streams=False):
         self.contrib = contrib
         self.dense_fetch = False
+        self.prefetch_at = "start"
         self.graph, self.cg, self.eager_steps = graph, None, 0
         nd = self.normalised_depth = normalised_depth
         import torch
@@ -243,7 +244,7 @@ class Workload:
                     raise
         raise RuntimeError("workspace did not settle")
 
-    def one(self, v, ren=None, bufs=None):
+    def one(self, v, ren=None, bufs=None, hook=None, hook_at=None):
         """render -> loss -> backward for view v (everything enqueued, no host sync)."""
         ren = ren or self.ren
         cam = self.ccams[v]
@@ -263,9 +264,13 @@ class Workload:
             ren.render_contrib(self.sf, cam, self.contrib_buf, **self.im)
         else:
             ren.render(self.sf, cam, **self.im)
+        if hook is not None and hook_at == "forward":
+            hook()
         # mapping iteration: Eq. 24-26 with Tab. I's lambda_c, w_d, w_n -> upstream gradients of all planes
         ren.mapping_loss(cam, self.im, trgb, tdep, 0.875, 0.5, 0.02, -1.0, self.up, self.loss)
         ren.ssim_loss(self.im["rgb"], trgb, 0.125, self.up["rgb"], self.loss)   # + (1 - lambda_c) L_SSIM: Eq. 24 complete
+        if hook is not None and hook_at == "loss":
+            hook()
         u = self.up
         ren.backward(d_rgb=u["rgb"], d_depth=u["depth"], d_normal=u["normal"], d_alpha=u["alpha"],
                      grads=self.grads_of[id(ren)], d_pose6=self.p6_of[id(ren)], accumulate=True)
@@ -325,9 +330,15 @@ class Workload:
             for v in range(nv):
                 if v % WINDOW == 0:
                     self.begin_window()   # (each context sums the views it renders; the optimiser adds the two accumulators)
-                if v + 1 < nv:
-                    self.rens[(v + 1) % 2].prepare(self.sf, self.ccams[v + 1], stream=self.side)
-                self.one(v, self.rens[v % 2])   # its render finds the binning prepared and orders itself behind it
+                at = self.prefetch_at
+                def nxt(v=v, at=at):
+                    if v + 1 < nv:
+                        if at != "start":
+                            self.side.wait_stream(main)   # the binning of view v+1 starts behind what view v has enqueued so far
+                        self.rens[(v + 1) % 2].prepare(self.sf, self.ccams[v + 1], stream=self.side)
+                if at == "start":
+                    nxt()
+                self.one(v, self.rens[v % 2], hook=nxt, hook_at=at)   # its render finds the binning prepared and orders itself behind it
             main.wait_stream(self.side)
             for r in self.rens:
                 r.wait_grads()   # the step ends when every view's gradients are complete
@@ -476,6 +487,7 @@ def run_config(name, args, torch, dist, world, rank, local, peaks):
 
     wl = Workload(name, args.iters, args.contrib, not args.no_prefetch, not args.no_reuse, args.normalised_depth, args.graph,
                   args.tight, args.radix, args.two_streams)
+    wl.prefetch_at = args.prefetch_at
     K, W = args.steps, max(args.warmup, 3)
     per_step = []
     for _ in range(W):
@@ -557,7 +569,7 @@ def run_config(name, args, torch, dist, world, rank, local, peaks):
                            survivor_list=("built once per step (frame) with a 3 cm / 0.02 rad pose margin, SGS_FLAG_TRACK_REUSE"
                                           if (wl.tracking and not args.no_reuse) else "every render"),
                            binning=("two contexts on two streams, views alternating; binning in line on each" if getattr(wl, "two_streams", False) else
-                                    "sgs_prepare of view v+1 on a second context and a side stream, under view v's compositing"
+                                    f"sgs_prepare of view v+1 on a second context and a side stream, enqueued behind view v's {args.prefetch_at}"
                                     if len(wl.rens) > 1 else "in line (sgs_render / sgs_track_iter)")))
     if not wl.tracking and e2e is not None:
         e2e["gradients"] = ("all n x 13 floats per window (sgs_fetch_grads_host)" if args.dense_fetch else
@@ -656,6 +668,8 @@ def main():
     ap.add_argument("--dense-fetch", action="store_true", help="e2e leg of the mapping configs: sgs_fetch_grads_host (all N x 13 floats per window) instead of the sparse hand-over")
     ap.add_argument("--no-reuse", action="store_true", help="tracking configs: run the pre-cull over the whole map every iteration")
     ap.add_argument("--no-prefetch", action="store_true", help="mapping configs: one context, binning of each view in line")
+    ap.add_argument("--prefetch-at", default="start", choices=["start", "forward", "loss"],
+                    help="mapping configs: where sgs_prepare of view v+1 is enqueued on the side stream: at the start of view v (default: it runs under k_forward), behind its forward, or behind its loss kernels (under k_backward: +1.4 %% MP/s, but the dominant kernel's measured duration then includes the binning it shares the SMs with)")
     ap.add_argument("--graph", action="store_true", help="SGS_FLAG_GRAPH: each step (a tracking frame, or a mapping window on one context) replayed as one CUDA graph")
     ap.add_argument("--normalised-depth", action="store_true", help="SGS_FLAG_NORMALISED_DEPTH: depth image D/O (tracking takes the unfused sequence)")
     ap.add_argument("--tight", action="store_true", help="SGS_FLAG_TIGHT_BINNING: opacity-aware cutoff + tile-exact culling (shorter tile lists, same images)")
