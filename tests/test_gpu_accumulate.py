@@ -192,3 +192,45 @@ def test_sparse_window_fetch_delivers_exactly_the_touched_rows():
             r = rows[name].numpy()
             assert (r[k:] == 9.0).all()
             np.testing.assert_allclose(r[:k], a[i], rtol=2e-4, atol=1e-5 * np.abs(a).max())
+
+
+def test_sparse_window_fetch_with_too_little_room_delivers_the_first_rows():
+    """cap < count: the first cap rows (ascending ids) arrive, *count is the true number of touched surfels, nothing is
+    written past cap, and the accumulator is clean for the next window all the same."""
+    sc, cams, _ = scenegen.make_config("C1")
+    cam = cams[0]
+    H, W = cam.height, cam.width
+    pin = lambda x, dt=torch.float32: torch.from_numpy(np.ascontiguousarray(x)).to(dt).pin_memory()
+    g0 = scenegen.SplitMix(79)
+    tgt = (pin(g0.uniform(3 * H * W).reshape(3, H, W)), pin((1.5 + g0.uniform(H * W)).reshape(1, H, W)))
+    shapes = dict(mean=3, scale=2, quat=4, opacity=1, rgb=3)
+    ren = sgs.Renderer()
+    ren.upload_surfels(pin(sc.mean), pin(sc.scale), pin(sc.quat), pin(sc.opacity), pin(sc.rgb))
+    c = camera(cam)
+    full = {k: torch.full((sc.n, d), 9.0).pin_memory() for k, d in shapes.items()}
+    ids_f, cnt_f = torch.full((sc.n,), -7, dtype=torch.int32).pin_memory(), torch.zeros(1, dtype=torch.int64).pin_memory()
+    ren.map_view_host(c, *tgt, 0.875, 0.5, 0.02, 0.125, -1.0)
+    ren.fetch_grads_sparse_host(ids_f, full, cnt_f)
+    ren.sync_host()
+    k = int(cnt_f.item())
+    cap = k // 3
+    assert cap > 10
+    part = {kk: torch.full((cap + 5, d), 9.0).pin_memory() for kk, d in shapes.items()}
+    ids_p, cnt_p = torch.full((cap + 5,), -7, dtype=torch.int32).pin_memory(), torch.zeros(1, dtype=torch.int64).pin_memory()
+    ren.map_view_host(c, *tgt, 0.875, 0.5, 0.02, 0.125, -1.0)
+    g = ren._grads(part, "cpu")    # (the binding takes cap from the tensors: call the C entry with an explicit smaller one)
+    C = ctypes
+    assert ren.lib.sgs_fetch_grads_sparse_host(ren._ctx, C.c_void_p(ids_p.data_ptr()), C.byref(g), C.c_int64(cap),
+                                               C.c_void_p(cnt_p.data_ptr()),
+                                               C.c_void_p(torch.cuda.current_stream().cuda_stream)) == sgs.SGS_OK
+    ren.sync_host()
+    assert int(cnt_p.item()) == k
+    assert np.array_equal(ids_p.numpy()[:cap], ids_f.numpy()[:cap]) and (ids_p.numpy()[cap:] == -7).all()
+    for name in shapes:
+        assert (part[name].numpy()[cap:] == 9.0).all()
+        np.testing.assert_allclose(part[name].numpy()[:cap], full[name].numpy()[:cap], rtol=2e-4,
+                                   atol=1e-5 * np.abs(full[name].numpy()[:k]).max())
+    ren.fetch_grads_sparse_host(ids_f, full, cnt_f)      # nothing accumulated since: the lost rows were zeroed too
+    ren.sync_host()
+    assert int(cnt_f.item()) == 0
+    ren.close()
