@@ -41,23 +41,28 @@ __device__ __forceinline__ unsigned stage_track(const SgsPayload& pay, uint32_t 
     const double2 g2 = pay.g2[v];
     float4 s0, s1, s2;
     stage_entry(g0, g1, g2, g3, px0, py0, s0, s1, s2);
-    sh[0][tid] = s0; sh[1][tid] = s1; sh[2][tid] = s2;
-    sh[3][tid] = make_float4(g1.w, g3.w, g4.x, g4.y);
+    // K-track's own plane layout: operands that meet in one packed (two binary32 lanes) instruction sit in aligned pairs --
+    //   plane 0 (P, R, Q, S), plane 1 (U0, V0, E', F'): (un, vn) = (ly, ly) (Q, S) + ((lx, lx) (P, R) + (U0, V0))
+    //   plane 3 (r, g, b, n.z), plane 4 (n.x, n.y, opacity, m.z): the forward's accumulations take (r, g), (b, n.z), (n.x, n.y)
+    // Per lane the operations and their order are those of pair.cuh / k_forward: the results are bit-identical.
+    sh[0][tid] = make_float4(s0.x, s1.x, s0.y, s1.y); sh[1][tid] = make_float4(s0.z, s1.z, s0.w, s1.w); sh[2][tid] = s2;
+    sh[3][tid] = make_float4(g3.w, g4.x, g4.y, g5.x);
     const float aux = g5.y, auy = g5.z, auz = g5.w, avx = g6.x, avy = g6.y, avz = g6.z;
     sh[5][tid] = make_float4(aux, auy, auz, avx);
     sh[6][tid] = make_float4(avy, avz, auy * avz - auz * avy, auz * avx - aux * avz);
-    sh[4][tid] = make_float4(g4.z, g4.w, g5.x, aux * avy - auy * avx);  // n_c.y, n_c.z (with g4.w), ..., m.z
+    sh[4][tid] = make_float4(g4.z, g4.w, g1.w, aux * avy - auy * avx);
     return refine_patch_mask(warp_patch_mask(g7, tx0, ty0), s0, s1, s2, g1.w, cfg.cutoff2, cfg.alpha_min);
 }
 
 // (u, v) and rho^2 of one pair (pair.cuh's sequence)
 __device__ __forceinline__ float pair_rho2(const float4 s0, const float4 s1, const float4 s2, float lx, float ly, float& u,
                                            float& v) {
-    const float un = __fmaf_rn(ly, s0.y, __fmaf_rn(lx, s0.x, s0.z));
-    const float vn = __fmaf_rn(ly, s1.y, __fmaf_rn(lx, s1.x, s1.z));
-    const float dn = __fmaf_rn(ly, s1.w, __fmaf_rn(lx, s0.w, s2.x));
+    // s0 = (P, R, Q, S), s1 = (U0, V0, E', F') (stage_track): un and vn in two packed FMAs
+    const float2 uvn = __ffma2_rn(make_float2(ly, ly), make_float2(s0.z, s0.w),
+                                  __ffma2_rn(make_float2(lx, lx), make_float2(s0.x, s0.y), make_float2(s1.x, s1.y)));
+    const float dn = __fmaf_rn(ly, s1.w, __fmaf_rn(lx, s1.z, s2.x));
     const float inv = fast_rcp(dn);
-    u = __fmul_rn(un, inv); v = __fmul_rn(vn, inv);
+    u = __fmul_rn(uvn.x, inv); v = __fmul_rn(uvn.y, inv);
     return __fmaf_rn(v, v, __fmul_rn(u, u));
 }
 
@@ -101,7 +106,14 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     if (inside) { tr = __ldg(trgb + pix); tg = __ldg(trgb + HW + pix); tb = __ldg(trgb + 2 * HW + pix); td = __ldg(tdepth + pix); }
 
     // ---- forward walk over the staged batch [boff, boff + nb) (Eq. 8, as k_forward) ----
-    float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f, Dp = 0.f, N0 = 0.f, N1 = 0.f, N2 = 0.f, O = 0.f;
+    float T = 1.f, Dp = 0.f, O = 0.f;
+    float2 C01 = make_float2(0.f, 0.f), C2N2 = make_float2(0.f, 0.f), N01 = make_float2(0.f, 0.f);   // (C0, C1), (C2, N2), (N0, N1)
+#define C0 C01.x
+#define C1 C01.y
+#define C2 C2N2.x
+#define N2 C2N2.y
+#define N0 N01.x
+#define N1 N01.y
     uint32_t last = 0;
     bool done = !inside;
     auto forward_walk = [&](const uint32_t boff, const uint32_t nb, const uint32_t j0 = 0u) {  // slots [j0, nb), j0 % 32 == 0
@@ -126,7 +138,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
                     jl[k] = boff + j + 1u;
                     ea[k] = sa + j * 16u;
                     const float4 s0 = lds128(ea[k]), s1 = lds128(ea[k] + TRK_PL), s2 = lds128(ea[k] + 2 * TRK_PL);
-                    const float opac = lds32(ea[k] + 3 * TRK_PL);
+                    const float opac = lds32(ea[k] + 4 * TRK_PL + 8);
                     float u, v;
                     const float rho2 = pair_rho2(s0, s1, s2, lx, ly, u, v);
                     const float z = __fmaf_rn(s2.z, v, __fmaf_rn(s2.y, u, s2.w));
@@ -150,9 +162,11 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
                     T = pass ? Tn : T;
                     last = pass ? jl[k] : last;
                     const float4 s3 = lds128(ea[k] + 3 * TRK_PL), s4 = lds128(ea[k] + 4 * TRK_PL);
-                    C0 = __fmaf_rn(w, s3.y, C0); C1 = __fmaf_rn(w, s3.z, C1); C2 = __fmaf_rn(w, s3.w, C2);
+                    const float2 w2 = make_float2(w, w);
+                    C01 = __ffma2_rn(w2, make_float2(s3.x, s3.y), C01);
+                    C2N2 = __ffma2_rn(w2, make_float2(s3.z, s3.w), C2N2);
+                    N01 = __ffma2_rn(w2, make_float2(s4.x, s4.y), N01);
                     Dp = __fmaf_rn(w, zz[k], Dp);
-                    N0 = __fmaf_rn(w, s4.x, N0); N1 = __fmaf_rn(w, s4.y, N1); N2 = __fmaf_rn(w, s4.z, N2);
                     O += w;
                 }
             }
@@ -227,11 +241,12 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
                     const float rho2 = pair_rho2(s0, s1, s2, lx, ly, r[k].u, r[k].v);
                     r[k].z = __fmaf_rn(s2.z, r[k].v, __fmaf_rn(s2.y, r[k].u, s2.w));
                     r[k].G = fast_ex2(__fmul_rn(rho2, -0.72134752044448170368f));
-                    r[k].a = fminf(cfg.alpha_max, __fmul_rn(s3.x, r[k].G));
+                    const float op = lds32(ea[k] + 4 * TRK_PL + 8);
+                    r[k].a = fminf(cfg.alpha_max, __fmul_rn(op, r[k].G));
                     hit[k] = has && (boff + j) < last && (rho2 <= cfg.cutoff2) && (r[k].z > cfg.z_near) && (r[k].a >= cfg.alpha_min);
-                    opac[k] = s3.x;
+                    opac[k] = op;
                     inv1ma[k] = fast_rcp(1.f - r[k].a);
-                    gv[k] = g0 * s3.y + g1 * s3.z + g2 * s3.w + g3 * (NDEPTH ? r[k].z - zref : r[k].z);
+                    gv[k] = g0 * s3.x + g1 * s3.y + g2 * s3.z + g3 * (NDEPTH ? r[k].z - zref : r[k].z);
                     anyh = anyh || hit[k];
                 }
                 if (!__any_sync(0xffffffffu, anyh)) continue;
@@ -535,6 +550,12 @@ __global__ void k_iota(uint32_t* __restrict__ p, int n) {
     if (i < n) p[i] = (uint32_t)i;
 }
 
+#undef C0
+#undef C1
+#undef C2
+#undef N0
+#undef N1
+#undef N2
 }  // namespace
 
 cudaError_t sgs_launch_track(sgs_ctx* c, float* const planes[8], const float* trgb, const float* tdepth, float lambda_d,
