@@ -106,7 +106,10 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
     if (inside) { tr = __ldg(trgb + pix); tg = __ldg(trgb + HW + pix); tb = __ldg(trgb + 2 * HW + pix); td = __ldg(tdepth + pix); }
 
     // ---- forward walk over the staged batch [boff, boff + nb) (Eq. 8, as k_forward) ----
-    float T = 1.f, Dp = 0.f, O = 0.f;
+    float T = 1.f;
+    float2 DO = make_float2(0.f, 0.f);   // (Dp, O): O + w * 1 is O + w exactly
+#define Dp DO.x
+#define O DO.y
     float2 C01 = make_float2(0.f, 0.f), C2N2 = make_float2(0.f, 0.f), N01 = make_float2(0.f, 0.f);   // (C0, C1), (C2, N2), (N0, N1)
 #define C0 C01.x
 #define C1 C01.y
@@ -166,8 +169,7 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
                     C01 = __ffma2_rn(w2, make_float2(s3.x, s3.y), C01);
                     C2N2 = __ffma2_rn(w2, make_float2(s3.z, s3.w), C2N2);
                     N01 = __ffma2_rn(w2, make_float2(s4.x, s4.y), N01);
-                    Dp = __fmaf_rn(w, zz[k], Dp);
-                    O += w;
+                    DO = __ffma2_rn(w2, make_float2(zz[k], 1.f), DO);
                 }
             }
         }
@@ -214,7 +216,12 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
 
     // ---- reverse walk over the staged batch (as k_backward<POSE_ONLY>, g_normal = g_alpha = 0) ----
     float T_after = 1.f, suffix = 0.f;
-    float F0 = 0.f, F1 = 0.f, F2 = 0.f, Z0 = 0.f, Z1 = 0.f, Z2 = 0.f;
+    float F2 = 0.f, Z2 = 0.f;
+    float2 F01 = make_float2(0.f, 0.f), Z01 = make_float2(0.f, 0.f);
+#define F0 F01.x
+#define F1 F01.y
+#define Z0 Z01.x
+#define Z1 Z01.y
     auto backward_walk = [&](const uint32_t boff, const int jend) {  // entries [0, jend) of the staged batch, back to front
         for (int c0 = ((jend - 1) >> 5) << 5; c0 >= 0 && jend > 0; c0 -= 32) {
             unsigned m = __ballot_sync(0xffffffffu, (c0 + lane < jend) && ((lds_u8(sm_a + c0 + lane) >> wid) & 1u));
@@ -275,8 +282,8 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
                     const float f1 = hit[k] ? (q0 - rx * q2 + m1 * gz) * inv_rm : 0.f;
                     const float f2 = hit[k] ? (rx * q1 - ry * q0 + m2 * gz) * inv_rm : 0.f;
                     const float zk = hit[k] ? r[k].z : 0.f;  // a rejected pair may carry inf / NaN
-                    F0 += f0; F1 += f1; F2 += f2;
-                    Z0 = fmaf(zk, f0, Z0); Z1 = fmaf(zk, f1, Z1); Z2 = fmaf(zk, f2, Z2);
+                    F01 = __fadd2_rn(F01, make_float2(f0, f1)); F2 += f2;
+                    Z01 = __ffma2_rn(make_float2(zk, zk), make_float2(f0, f1), Z01); Z2 = fmaf(zk, f2, Z2);
                 }
             }
         }
@@ -550,6 +557,12 @@ __global__ void k_iota(uint32_t* __restrict__ p, int n) {
     if (i < n) p[i] = (uint32_t)i;
 }
 
+#undef F0
+#undef F1
+#undef Z0
+#undef Z1
+#undef Dp
+#undef O
 #undef C0
 #undef C1
 #undef C2
