@@ -58,6 +58,7 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
     const int px = tx * SGS_TILE + lxi, py = ty * SGS_TILE + lyi;
     const bool inside = px < W && py < H;
     const float lx = (float)lxi, ly = (float)lyi;
+    const float2 lx2 = make_float2(lx, lx), ly2 = make_float2(ly, ly);
     const double px0 = (double)(tx * SGS_TILE) + 0.5, py0 = (double)(ty * SGS_TILE) + 0.5;
     const uint32_t start = ranges[2 * tile];
 
@@ -133,7 +134,10 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
             const double2 g2 = pay.g2[v];
             StagedBwd st;
             float xy0[2];
-            stage_entry(g0, g1, g2, g3, px0, py0, st.s0, st.s1, st.s2, xy0);
+            float4 t0, t1;
+            stage_entry(g0, g1, g2, g3, px0, py0, t0, t1, st.s2, xy0);
+            // (P, R, Q, S) and (U0, V0, E', F'): the operands of the packed (un, vn) in aligned pairs, as in K-track
+            st.s0 = make_float4(t0.x, t1.x, t0.y, t1.y); st.s1 = make_float4(t0.z, t1.z, t0.w, t1.w);
 
             st.s3 = make_float4(g1.w, g3.w, g4.x, g4.y);
             st.s4 = make_float4(g4.z, g4.w, g5.x, 0.f);  // .w <- m.z below
@@ -146,7 +150,7 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
             if (LOWPASS) { st.s6.z = xy0[0]; st.s6.w = xy0[1]; }
             sh_v[tid] = v;
             sh[tid] = st;
-            if (!LOWPASS) pmask = refine_patch_mask(pmask, st.s0, st.s1, st.s2, g1.w, cfg.cutoff2, cfg.alpha_min);
+            if (!LOWPASS) pmask = refine_patch_mask(pmask, t0, t1, st.s2, g1.w, cfg.cutoff2, cfg.alpha_min);
         }
         sh_mask[tid] = (unsigned char)pmask;
         __syncthreads();
@@ -172,11 +176,10 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
                 const int j = c0 + hb;
                 jj[k] = j;
                 const float4 s0 = sh[j].s0, s1 = sh[j].s1, s2 = sh[j].s2, s3 = sh[j].s3, s4 = sh[j].s4;
-                const float un = __fmaf_rn(ly, s0.y, __fmaf_rn(lx, s0.x, s0.z));
-                const float vn = __fmaf_rn(ly, s1.y, __fmaf_rn(lx, s1.x, s1.z));
-                const float dn = __fmaf_rn(ly, s1.w, __fmaf_rn(lx, s0.w, s2.x));
+                const float2 uvn = __ffma2_rn(ly2, make_float2(s0.z, s0.w), __ffma2_rn(lx2, make_float2(s0.x, s0.y), make_float2(s1.x, s1.y)));
+                const float dn = __fmaf_rn(ly, s1.w, __fmaf_rn(lx, s1.z, s2.x));
                 const float inv = fast_rcp(dn);
-                r[k].u = __fmul_rn(un, inv); r[k].v = __fmul_rn(vn, inv);
+                r[k].u = __fmul_rn(uvn.x, inv); r[k].v = __fmul_rn(uvn.y, inv);
                 float rho2 = __fmaf_rn(r[k].v, r[k].v, __fmul_rn(r[k].u, r[k].u));
                 r[k].z = __fmaf_rn(s2.z, r[k].v, __fmaf_rn(s2.y, r[k].u, s2.w));
                 use2d[k] = false;
@@ -248,8 +251,12 @@ k_backward(const uint32_t* __restrict__ tile_order, const uint32_t* __restrict__
                     x[0] = f0; x[1] = f1; x[2] = f2;
                     x[3] = uk * f0; x[4] = uk * f1; x[5] = uk * f2;
                     x[6] = vk * f0; x[7] = vk * f1; x[8] = vk * f2;
-                    x[9] = w[k] * g[4]; x[10] = w[k] * g[5]; x[11] = w[k] * g[6];
-                    x[12] = w[k] * g[0]; x[13] = w[k] * g[1]; x[14] = w[k] * g[2];
+                    {   // six products w * g as three packed multiplies (g[4], g[5]), (g[6], g[0]), (g[1], g[2])
+                        const float2 w2 = make_float2(w[k], w[k]);
+                        const float2 a45 = __fmul2_rn(w2, make_float2(g[4], g[5])), a60 = __fmul2_rn(w2, make_float2(g[6], g[0])),
+                                     a12 = __fmul2_rn(w2, make_float2(g[1], g[2]));
+                        x[9] = a45.x; x[10] = a45.y; x[11] = a60.x; x[12] = a60.y; x[13] = a12.x; x[14] = a12.y;
+                    }
                     x[15] = (clamped || !hit[k]) ? 0.f : da[k] * r[k].G;
                     // Sum of the 16 values over the warp through shared memory (ncu: the register butterfly -- 16 SHFL,
                     // 30 SEL, 16 FADD -- was 32 % of this kernel's instructions; removing it altogether saved 95 us per
