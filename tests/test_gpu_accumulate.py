@@ -234,3 +234,63 @@ def test_sparse_window_fetch_with_too_little_room_delivers_the_first_rows():
     ren.sync_host()
     assert int(cnt_f.item()) == 0
     ren.close()
+
+
+def test_bench_launch_configuration_on_c4():
+    """The configuration bench.py times on the mapping configs, at C4's full size (2 M surfels, 1200 x 680): two contexts
+    (async, lazy gradients), the binning of the next view prepared on a side stream while the current view composites, each
+    context ADDING its views' gradients to its own accumulator.  Views 0 and 6 under the Eq. 24-26 upstream (the oracle's);
+    every gradient element of each view against the oracle with the strict bar + the exposure of fragile pixels."""
+    from gpu_common import assert_grads
+    sc, cams, _ = scenegen.make_config("C4")
+    cfg = oracle.make_cfg()
+    t, sf = to_device(sc)
+    rens = [sgs.Renderer(async_mode=True, lazy_grads=True) for _ in range(2)]
+    side = torch.cuda.Stream()
+    views = (0, 6)
+    ccams = [camera(cams[v]) for v in views]
+    ups = []
+    for v in views:
+        camv = oracle.make_cam(cams[v])
+        img = oracle.render(sc, camv, cfg, counters=False)["img"]
+        T_tgt = scenegen.perturb_pose(cams[v].T_cw, np.array([0.02, 0.0, -0.01, 0.0, 0.01, 0.005]))
+        tgt = oracle.render(sc, oracle.make_cam(cams[v], T_tgt), cfg, counters=False)["img"]
+        _, up = oracle.mapping_loss(img, tgt[0:3], tgt[3], camv, 0.875, 0.5, 0.02, -1.0)
+        ups.append(torch.from_numpy(up.astype(np.float32)).cuda())
+    for k in range(2):   # workspaces at size: an overflowing first render regrows and is reported once (async mode)
+        im = alloc_images(cams[views[k]])
+        for _ in range(3):
+            try:
+                rens[k].render(sf, ccams[k], **im); rens[k].stats(); rens[k].render(sf, ccams[k], **im)
+                break
+            except sgs.SgsError as e:
+                if e.status != sgs.SGS_WORKSPACE_OVERFLOW:
+                    raise
+    torch.cuda.synchronize()
+    grads = [alloc_grads(sc.n) for _ in range(2)]
+    p6 = [torch.zeros(6, device="cuda") for _ in range(2)]
+    main = torch.cuda.current_stream()
+    side.wait_stream(main)
+    for k in range(2):
+        rens[k].zero_grads(grads[k])
+    rens[0].prepare(sf, ccams[0], stream=side)
+    ims = [alloc_images(cams[v]) for v in views]
+    for k in range(2):
+        if k + 1 < 2:
+            rens[k + 1].prepare(sf, ccams[k + 1], stream=side)      # next view's binning under this view's kernels
+        rens[k].render(sf, ccams[k], **ims[k])                      # finds its binning prepared, orders itself behind it
+        u = ups[k]
+        rens[k].backward(d_rgb=u[0:3].contiguous(), d_depth=u[3:4].contiguous(), d_normal=u[4:7].contiguous(),
+                         d_alpha=u[7:8].contiguous(), grads=grads[k], d_pose6=p6[k], accumulate=True)
+    main.wait_stream(side)
+    for r in rens:
+        r.wait_grads()
+    torch.cuda.synchronize()
+    for k, v in enumerate(views):
+        camv = oracle.make_cam(cams[v])
+        up32 = ups[k].cpu().numpy().astype(np.float64)
+        og, ex = oracle.backward(sc, camv, cfg, up32), oracle.exposure(sc, camv, cfg, up32)
+        assert_grads({kk: x.cpu().numpy() for kk, x in grads[k].items()}, og, ex, ("C4", v))
+        assert_pose(p6[k].cpu().numpy(), og["pose"], ex["pose"], ("C4", v))
+    for r in rens:
+        r.close()
