@@ -165,3 +165,53 @@ def test_tight_binning_full_size(name, views, full):
     """SGS_FLAG_TIGHT_BINNING (opacity-aware cutoff + tile-exact culling) on every full-size config: the shorter lists are
     bit-identical to the oracle's tight mode; images, losses and gradients meet the same bars as with the default binning."""
     check_config(name, views, full, tight=True)
+
+
+@pytest.mark.parametrize("name", ["C2", "C5"])
+def test_tracking_launch_configuration_with_the_kept_survivor_list(name):
+    """What bench.py times on the tracking configs: SGS_FLAG_ASYNC + SGS_FLAG_TRACK_REUSE, the survivor list built once per
+    frame (sgs_track_new_frame) and kept while the pose moves inside its margin.  Three poses of one frame (the keyframe's,
+    then two steps of 8 mm / 0.3 deg): at each, binning bit-exact, images and the pose gradient / loss of sgs_track_iter
+    against the oracle at THAT pose (1e-3 + the oracle-computed flip slack)."""
+    sc, cams, info = scenegen.make_config(name)
+    cfg = oracle.make_cfg()
+    cam = cams[0]
+    ren = sgs.Renderer(async_mode=True, track_reuse=True)
+    t, sf = to_device(sc)
+    tiles = ((cam.width + 15) // 16) * ((cam.height + 15) // 16)
+    T_tgt = scenegen.perturb_pose(cam.T_cw, tau0(info.get("tau0_seed", 2000)))
+    tgt = oracle.render(sc, oracle.make_cam(cam, T_tgt), cfg, counters=False)["img"].astype(np.float32).astype(np.float64)
+    trgb = torch.from_numpy(tgt[0:3].astype(np.float32)).cuda()
+    tdep = torch.from_numpy(tgt[3:4].astype(np.float32)).cuda()
+    step = np.array([0.004, -0.005, 0.004, 0.003, 0.002, -0.003])
+    try:
+        ren.track_new_frame()
+        for it in range(3):
+            T = scenegen.perturb_pose(cam.T_cw, it * step) if it else cam.T_cw
+            camv, c = oracle.make_cam(cam, T), camera(cam, T)
+            im, upi = alloc_images(cam), alloc_images(cam)
+            p6, loss = torch.zeros(6, device="cuda"), torch.zeros(1, device="cuda")
+            for _ in range(4):   # (async mode: an overflow of the first iteration is reported by the next call)
+                try:
+                    ren.track_iter(sf, c, trgb, tdep, LAMBDA_D, NSIGN, p6, loss, **im)
+                    ren.stats()
+                    ren.track_iter(sf, c, trgb, tdep, LAMBDA_D, NSIGN, p6, loss, **im)
+                    break
+                except sgs.SgsError as e:
+                    if e.status != sgs.SGS_WORKSPACE_OVERFLOW:
+                        raise
+            torch.cuda.synchronize()
+            ob = oracle.binning(sc, camv, cfg)
+            assert_binning(ren.get_binning(sc.n, tiles), ob)
+            o = oracle.render(sc, camv, cfg)
+            assert_image_check(image_check(planes(im), o["img"], o["fragile"], oracle.pixel_bounds(sc, camv, cfg)), (name, it))
+            tr = tracking_reference(sc, camv, cfg, o, tgt, LAMBDA_D, NSIGN, oracle)
+            l2 = torch.zeros(1, device="cuda")
+            ren.tracking_loss(c, im, trgb, tdep, LAMBDA_D, NSIGN, upi, l2)     # which masks / signs came out differently
+            D = tracking_flips(tr, planes(upi))
+            assert D.any(0).mean() < 2e-4
+            pose_slack, loss_slack = tracking_slack(sc, camv, cfg, tr, D, oracle)
+            assert abs(float(loss.item()) - tr["L"]) <= tr["loss_tol"] + loss_slack
+            assert_pose(p6.cpu().numpy().astype(np.float64), tr["og"]["pose"], tr["ex"]["pose"] + pose_slack / C_EXPO, (name, it))
+    finally:
+        ren.close()
