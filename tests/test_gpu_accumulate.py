@@ -294,3 +294,43 @@ def test_bench_launch_configuration_on_c4():
         assert_pose(p6[k].cpu().numpy(), og["pose"], ex["pose"], ("C4", v))
     for r in rens:
         r.close()
+
+
+def test_sparse_window_fetch_at_c4_size_equals_the_dense_fetch():
+    """2 M surfels: the compaction's block scan runs over more than 1024 blocks of 1024 surfels (its carry path).  Two views of
+    C4 through sgs_map_view_host on two contexts, one fetched dense, one sparse: same rows (ids = the dense fetch's non-zero
+    rows, ascending), same values up to the order of the atomic adds inside a view."""
+    sc, cams, _ = scenegen.make_config("C4")
+    H, W = cams[0].height, cams[0].width
+    pin = lambda x, dt=torch.float32: torch.from_numpy(np.ascontiguousarray(x)).to(dt).pin_memory()
+    g0 = scenegen.SplitMix(80)
+    tgts = [(pin(g0.uniform(3 * H * W).reshape(3, H, W)), pin((1.5 + g0.uniform(H * W)).reshape(1, H, W))) for _ in range(2)]
+    shapes = dict(mean=3, scale=2, quat=4, opacity=1, rgb=3)
+    host = dict(mean=pin(sc.mean), scale=pin(sc.scale), quat=pin(sc.quat), opacity=pin(sc.opacity), rgb=pin(sc.rgb))
+    out = {}
+    for mode in ("dense", "sparse"):
+        ren = sgs.Renderer()
+        ren.upload_surfels(host["mean"], host["scale"], host["quat"], host["opacity"], host["rgb"])
+        for k, v in enumerate((0, 6)):
+            ren.map_view_host(camera(cams[v]), *tgts[k], 0.875, 0.5, 0.02, 0.125, -1.0)
+        rows = {k: torch.full((sc.n, d), 9.0).pin_memory() for k, d in shapes.items()}
+        if mode == "dense":
+            ren.fetch_grads_host(rows)
+            ren.sync_host()
+            out[mode] = {k: v.numpy() for k, v in rows.items()}
+        else:
+            ids, cnt = torch.full((sc.n,), -7, dtype=torch.int32).pin_memory(), torch.zeros(1, dtype=torch.int64).pin_memory()
+            ren.fetch_grads_sparse_host(ids, rows, cnt)
+            ren.sync_host()
+            out[mode] = (ids.numpy(), {k: v.numpy() for k, v in rows.items()}, int(cnt.item()))
+        ren.close()
+    dense = out["dense"]
+    ids, rows, k = out["sparse"]
+    nz = np.zeros(sc.n, bool)
+    for a in dense.values():
+        nz |= (a != 0).any(axis=1)
+    assert 100_000 < k < sc.n // 2 and k == int(nz.sum())
+    assert np.array_equal(ids[:k].astype(np.int64), np.nonzero(nz)[0]) and (ids[k:] == -7).all()
+    for name, a in dense.items():
+        assert (rows[name][k:] == 9.0).all()
+        np.testing.assert_allclose(rows[name][:k], a[ids[:k]], rtol=2e-4, atol=1e-5 * np.abs(a).max())
