@@ -49,7 +49,7 @@ k_forward(const uint32_t* __restrict__ tile_order, uint32_t* __restrict__ ranges
         // more than 128 keys: counting pass over the depth + rank inside each depth bin (histsort.cuh; linear in n); it declines
         // buckets whose depths crowd into one bin, which take the networks below like the short ones
         static_assert(sizeof(sh) >= 2048 * 8 + HS_SCRATCH_WORDS * 4 && SGS_BLOCK >= 32 * 4 && HS_BINS == 4 * SGS_BLOCK, "");
-        const bool sorted = n > 128 && hist_sort_keys(g, n, sk, reinterpret_cast<uint32_t*>(sk + 2048), reinterpret_cast<uint32_t*>(sh_mask), tid);
+        const bool sorted = n > 128 && hist_sort_keys(g, n, sk, reinterpret_cast<uint32_t*>(sk + 2048), reinterpret_cast<uint32_t*>(sh_mask), tid, g);
         if (sorted) {
         } else if (n >= 2 && n <= 512) {   // keys in registers: shuffles + a few shared-memory exchanges (regsort.cuh)
             uint32_t npad = 32;

@@ -20,9 +20,12 @@ constexpr int HS_SCRATCH_WORDS = HS_BINS;   // histogram, then the bins' end cur
 
 // g: the bucket (n keys, 128 < n <= 2048), sk: shared memory for n keys, sw: HS_SCRATCH_WORDS words and s_misc: 32 words of
 // shared memory.
-// All 256 threads must call; ends with the sorted bucket written to g and a __syncthreads().
-__device__ __forceinline__ bool hist_sort_keys(unsigned long long* g, const uint32_t n, unsigned long long* sk, uint32_t* sw,
-                                               uint32_t* s_misc, const int tid) {
+// All 256 threads must call; ends with the sorted keys written and a __syncthreads().
+// out0 / out1: where the sorted keys go (out1 may be null; either may be g itself: g is read for the last time before the
+// barrier in front of step 4).
+__device__ __forceinline__ bool hist_sort_keys(const unsigned long long* g, const uint32_t n, unsigned long long* sk, uint32_t* sw,
+                                               uint32_t* s_misc, const int tid, unsigned long long* out0,
+                                               unsigned long long* out1 = nullptr) {
     uint32_t* s_cnt = sw;                 // [HS_BINS] histogram, then scatter cursors = end of each bin
     const int lane = tid & 31, wid = tid >> 5;
     // 1. depth range
@@ -80,7 +83,8 @@ __device__ __forceinline__ bool hist_sort_keys(unsigned long long* g, const uint
         const uint32_t lo = b ? s_cnt[b - 1] : 0u, hi = s_cnt[b];   // (a bin's end cursor is the next bin's start)
         uint32_t rank = lo;
         for (uint32_t k = lo; k < hi; ++k) rank += sk[k] < key ? 1u : 0u;
-        g[rank] = key;
+        out0[rank] = key;
+        if (out1) out1[rank] = key;
     }
     __syncthreads();
     return true;

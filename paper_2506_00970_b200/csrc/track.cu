@@ -11,6 +11,7 @@
 // Arithmetic is pair.cuh's (identical decisions to k_forward / k_backward); the tracking loss has no
 // normal / alpha gradient, so those terms of the general backward are dropped at compile time.
 #include "pair.cuh"
+#include "histsort.cuh"
 #include "reduce.cuh"
 #include "sgs_internal.h"
 
@@ -64,6 +65,11 @@ __device__ __forceinline__ float pair_rho2(const float4 s0, const float4 s1, con
     const float inv = fast_rcp(dn);
     u = __fmul_rn(uvn.x, inv); v = __fmul_rn(uvn.y, inv);
     return __fmaf_rn(v, v, __fmul_rn(u, u));
+}
+
+// (out of line: inlined it cost the walks registers)
+__device__ __noinline__ bool hist_sort_call(unsigned long long* g, uint32_t n, unsigned long long* sk, uint32_t* sw, uint32_t* s_misc, int tid) {
+    return hist_sort_keys(g, n, sk, sw, s_misc, tid, g);
 }
 
 template <bool WRITE_IMAGES, bool NDEPTH>
@@ -398,7 +404,14 @@ k_track(uint32_t* tile_order, uint32_t* __restrict__ ranges, const uint32_t* cur
         }
     } else {
         // ===== general path: 256-entry batches front to back, then back to front (restaging what was evicted) =====
-        if (!presorted) {  // n > 256: bitonic network in the staging memory, sorted keys back to the bucket
+        // Lists longer than the staging capacity (C5: a quarter of the tiles, 41 % of the entries): counting pass over the depth +
+        // rank inside a depth bin (histsort.cuh, linear in n; scratch = the staging planes), keys back to the bucket; it declines
+        // buckets whose depths crowd into one bin, which take the bitonic network.  (Lists of up to TRK_CAP keys keep the rank by
+        // counting above: measured, the counting sort there gains nothing on C5 and costs C2 3 %.)
+        static_assert(sizeof(float4) * 7 * TRK_CAP >= 2048 * 8 + HS_SCRATCH_WORDS * 4 && sizeof(s_red) >= 32 * 4, "");
+        unsigned long long* hs_keys = reinterpret_cast<unsigned long long*>(&sh[0][0]);
+        if (!presorted && n <= 2048u && hist_sort_call(g, n, hs_keys, reinterpret_cast<uint32_t*>(hs_keys + 2048), reinterpret_cast<uint32_t*>(&s_red[0][0]), tid)) {
+        } else if (!presorted) {  // bitonic network in the staging memory, sorted keys back to the bucket
             unsigned long long* sk = reinterpret_cast<unsigned long long*>(&sh[0][0]);
             uint32_t npad = 512;
             while (npad < n) npad <<= 1;
