@@ -448,8 +448,13 @@ def test_track_iter_matches_unfused_sequence():
     sc, cams, _ = scenegen.make_config("C1")
     cases.append((sc, cams[0]))
     g = scenegen.SplitMix(11)
-    for n in (900, 6000):   # ~n entries on the central tiles: multi-batch; > 2048 -> tilesort pre-pass
-        mean = np.stack([g.uniform(n, -0.05, 0.05), g.uniform(n, -0.05, 0.05), g.uniform(n, 1.0, 3.0)], 1).astype(np.float32)
+    # ~n entries on the central tiles: multi-batch (ordered inside k_track by the counting sort of histsort.cuh; the second 900
+    # has 400 splats at one depth, which that sort declines: the bitonic network); > 2048 -> tilesort pre-pass
+    for n, crowded in ((900, False), (900, True), (6000, False)):
+        z = g.uniform(n, 1.0, 3.0)
+        if crowded:
+            z[:400] = 2.0
+        mean = np.stack([g.uniform(n, -0.05, 0.05), g.uniform(n, -0.05, 0.05), z], 1).astype(np.float32)
         cases.append((Scene(mean, np.full((n, 2), 0.01, np.float32), np.tile(np.float32([1, 0.1, 0, 0]), (n, 1)),
                             np.full(n, 0.03 if n > 2000 else 0.2, np.float32),
                             np.stack([g.uniform(n) for _ in range(3)], 1).astype(np.float32)),
